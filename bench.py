@@ -1,0 +1,347 @@
+#!/usr/bin/env python
+"""bench.py -- effective FP64 TFLOPS of H_eff*Psi (BASELINE.json metric) on N B200 GPUs.
+
+A "step" is one Davidson iteration on the named workload: su2_davidson_step = one full
+H_eff*Psi (fused GEMM-pair kernel + deterministic segmented reduction, SURVEY.md 8(a) a4+a5)
+followed by the Rayleigh-Ritz / residual / orthogonalisation vector algebra (a6).  The plan
+(a1-a3) is built once per bond before the timed region, as in the paper ("execution ... follows
+only after such initialization procedure is completed"); its wall time is reported.
+
+value = CC flops of all ranks / max-over-ranks device time, CC = sum over task-positions of
+min(2mkn+2mnp, 2knp+2mkp) (the paper's definition of TFLOPS).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg4] [--impl reference]
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+sys.path.insert(0, os.path.join(ROOT, "tests"))
+
+METRIC = "effective FP64 TFLOPS of H_eff*Psi (CC / time)"
+UNIT = "TFLOP/s"
+# nominal FP64 / BF16 dense ratio of a B200 (45 TF FP64 per the guide's "B200's 45" vs 2250 TF BF16):
+# roofline.peak = MEASURED bf16 peak x this ratio, as the task statement prescribes for a
+# contraction in a dtype without a measured peak of its own.
+FP64_OVER_BF16_NOMINAL = 45.0 / 2250.0
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return d, "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region."""
+
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, power = [], [], set(), []
+        for ln in self.lines:
+            p = [x.strip() for x in ln.split(",")]
+            if len(p) < 9:
+                continue
+            try:
+                sm.append(float(p[1])); mx.append(float(p[2])); power.append(float(p[3]))
+            except ValueError:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), p[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------ CPU oracle arm
+def oracle_sample_problem(cfg_name, npos_sample):
+    """Bounded sample of the workload for the CPU oracle: the two heaviest row classes of the
+    config (A1 P~1 and B1 Q1, with their Hermitian conjugates) restricted to the first
+    `npos_sample` positions, all sector combinations, full block sizes."""
+    from gen import workloads as W
+    from gen.problem import Problem
+    c = W.CONFIGS[cfg_name]
+    full = W.synthetic_problem(c["L"], c["N"], c["twoS"], c["D"], xi=c["xi"], seed=0, fill=False)
+    keep = [t for t in full.term if t.name.split("^")[0] in ("A1P1", "B1Q1")]
+    fam_l, fam_r, terms = [], [], []
+    import copy
+    for t in keep:
+        t = copy.copy(t)
+        for side, fams, secs, new in (("l", full.fam_l, full.sec_l, fam_l), ("r", full.fam_r, full.sec_r, fam_r)):
+            idx = t.fam_l if side == "l" else t.fam_r
+            f = fams[idx]
+            nf = W.make_family(secs, f.dN, f.twoK, min(npos_sample, f.npos), 0, 900 + idx, f.name)
+            new.append(nf)
+            if side == "l":
+                t.fam_l = len(new) - 1
+            else:
+                t.fam_r = len(new) - 1
+        t.alpha = None if t.alpha is None else t.alpha[:min(npos_sample, len(t.alpha))]
+        terms.append(t)
+    return Problem(n_tot=full.n_tot, twoS_tot=full.twoS_tot, sec_l=full.sec_l, sec_r=full.sec_r, fam_l=fam_l,
+                   fam_r=fam_r, site=full.site, term=terms, meta=dict(full.meta))
+
+
+def time_oracle(cfg_name, steps, warmup, budget_s=20.0):
+    """Times oracle.heff_dense.heff_apply, as it stands, on the bounded sample."""
+    import numpy as np
+    from gen.workloads import random_psi
+    from helpers import oracle_flat
+    from paper_2309_16724_b200 import Plan
+    npos = {"cfg4": 1, "cfg3": 4, "cfg2": 16}.get(cfg_name, 16)
+    prob = oracle_sample_problem(cfg_name, npos)
+    plan = Plan(prob, host_only=True)
+    x = random_psi(plan.psi_len, seed=0)
+    times = []
+    for i in range(warmup + steps):
+        t0 = time.perf_counter()
+        oracle_flat(prob, plan, x)
+        dt = time.perf_counter() - t0
+        if i >= warmup:
+            times.append(dt)
+        if sum(times) > budget_s and len(times) >= 1 and i >= warmup:
+            break
+    try:
+        from threadpoolctl import threadpool_info
+        cores = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+    except Exception:
+        cores = os.cpu_count()
+    ms = 1e3 * sum(times) / len(times)
+    cc = plan.info["cc_flops"]
+    sample = ("rows A1P1,B1Q1 (+h.c.) of %s restricted to %d position(s), all sector combinations, full block sizes; "
+              "CC of the sample %.3e flop" % (cfg_name, npos, cc))
+    return {"value": cc / (ms * 1e-3) / 1e12, "unit": UNIT, "cores": int(cores), "kind": "oracle", "sample": sample,
+            "ms_per_apply": ms, "steps_timed": len(times)}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2309_16724_b200.build import build
+    build()
+    cb = time_oracle(args.config, args.steps, args.warmup)
+    line = {"metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": cb["steps_timed"],
+            "warmup": args.warmup, "ms_per_step": cb["ms_per_apply"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "reference",
+            "config": {"workload": args.config + " (oracle on a bounded sample)", "sample": cb["sample"]},
+            "cpu_baseline": {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------ GPU arm
+def build_operator(cfg_name, device):
+    """Operator families resident in HBM.  cfg1-3: numpy counter-based generator, uploaded;
+    cfg4 (92 GB): generated on the device (seeded torch generator), DESIGN.md "Input recipe"."""
+    import torch
+    from gen import workloads as W
+    from paper_2309_16724_b200.runtime import HeffOperator
+    if cfg_name != "cfg4":
+        prob = W.config_problem(cfg_name, seed=0, fill=True)
+        return prob, HeffOperator(prob, device=device)
+    prob = W.config_problem(cfg_name, seed=0, fill=False)
+    gen = torch.Generator(device=device)
+
+    def fill(side, idx, tensor):
+        fam = (prob.fam_l if side == "l" else prob.fam_r)[idx]
+        secs = prob.sec_l if side == "l" else prob.sec_r
+        gen.manual_seed(1000 * (1 if side == "l" else 2) + idx)
+        off = 0
+        for qo, qi in zip(fam.q_out, fam.q_in):
+            n = fam.npos * secs[qo].dim * secs[qi].dim
+            blk = tensor[off:off + n]
+            blk.normal_(0.0, 1.0 / (secs[qi].dim ** 0.5), generator=gen)
+            if fam.name in ("H_l", "H_r") and qo == qi:
+                v = blk.view(fam.npos, secs[qo].dim, secs[qi].dim)
+                v.copy_(0.5 * (v + v.transpose(1, 2)))
+            off += n
+    return prob, HeffOperator(prob, device=device, device_fill=fill)
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    from gen.workloads import random_psi
+    from paper_2309_16724_b200.binding import kernel_launch_count, probe_fp64_peak
+    from paper_2309_16724_b200.build import build
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl")
+    assert torch.cuda.is_available(), "bench.py needs a GPU (no CPU fallback)"
+    device = "cuda:%d" % local
+    torch.cuda.set_device(device)
+    if rank == 0:
+        build()
+    if world > 1:
+        dist.barrier()
+    stream = torch.cuda.current_stream().cuda_stream
+
+    t0 = time.perf_counter()
+    prob, op = build_operator(args.config, device)
+    setup_s = time.perf_counter() - t0
+    info = op.info
+    cc = info["cc_flops"]
+    psi0 = torch.from_numpy(random_psi(op.psi_len, seed=0)).to(device)
+    solver = op.davidson(psi0, max_subspace=max(4, min(20, args.steps + args.warmup + 2)))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # --- warm-up
+    hist = []
+    for _ in range(args.warmup):
+        hist.append(solver.step())
+    # --- timed region: K Davidson steps, device time, max over ranks
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    l0 = kernel_launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(args.steps):
+        hist.append(solver.step())
+    ev1.record()
+    barrier()
+    launches = kernel_launch_count() - l0
+    ms_total = ev0.elapsed_time(ev1)
+    # --- the dominant kernel alone: su2_heff_apply (fused GEMM pair + reduction), CUDA events
+    x, y = psi0.clone(), op.new_vector()
+    ka0, ka1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    napply = max(1, min(args.steps, 5))
+    op.apply(x, y)
+    torch.cuda.synchronize()
+    ka0.record()
+    for _ in range(napply):
+        op.apply(x, y)
+    ka1.record()
+    torch.cuda.synchronize()
+    apply_ms = ka0.elapsed_time(ka1) / napply
+    clocks = sampler.stop() if rank == 0 else None
+    # --- end to end through the C ABI with HOST buffers (pinned): H2D psi, apply, D2H F, every step
+    xh = psi0.cpu().pin_memory()
+    fh = torch.empty_like(xh).pin_memory()
+    op.apply_host(xh, fh)
+    barrier()
+    t1 = time.perf_counter()
+    ne2e = max(1, min(args.steps, 5))
+    for _ in range(ne2e):
+        op.apply_host(xh, fh)
+    torch.cuda.synchronize()
+    e2e_ms = 1e3 * (time.perf_counter() - t1) / ne2e
+
+    t = torch.tensor([ms_total, apply_ms, e2e_ms], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total, apply_ms, e2e_ms = (float(v) for v in t.cpu())
+    if rank != 0:
+        solver.close()
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    ms_step = ms_total / args.steps
+    peaks, peak_src = measured_peaks()
+    dfma = probe_fp64_peak(0, 20000, 4, stream)
+    dmma = probe_fp64_peak(1, 4000, 4, stream)
+    peak = peaks["bf16_tflops"] * FP64_OVER_BF16_NOMINAL
+    achieved = cc / (apply_ms * 1e-3) / 1e12
+    line = {
+        "metric": METRIC, "value": world * cc / (ms_step * 1e-3) / 1e12, "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "%s: L=%d N=%d S=0 D_SU2=%d middle bond (BASELINE.json configs)" % (
+                       args.config, prob.meta["L"], prob.meta["N"], prob.meta["D"]),
+                   "step": "one su2_davidson_step = H_eff*Psi + Rayleigh-Ritz/residual/orthogonalisation",
+                   "parallelism": "replicas" if world > 1 else "single GPU",
+                   "l2": "inputs exceed L2 (operators %.2f GB resident, streamed every apply)" % (
+                       op.operator_bytes_resident / 1e9),
+                   "psi_len": int(info["psi_len"]), "tasks": int(info["ntasks"]),
+                   "task_positions": int(info["ntask_positions"]), "cc_flops_per_apply": cc,
+                   "executed_flops_per_apply": info["executed_flops"], "work_items": int(info["nwork_items"]),
+                   "segments": int(info["nsegments"]), "plan_seconds": info["plan_seconds"], "setup_seconds": setup_s},
+        "clocks": clocks,
+        "e2e": {"value": world * cc / (e2e_ms * 1e-3) / 1e12, "unit": UNIT, "h2d_bytes_per_step": 8 * op.psi_len,
+                "d2h_bytes_per_step": 8 * op.psi_len, "ms_per_step": e2e_ms,
+                "call": "su2_heff_apply_host (pinned host Psi in, host F out)"},
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "alu", "kernel": "heff_fused_kernel (+reduce_kernel) via su2_heff_apply",
+                     "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                     "peak_source": "%s bf16_tflops x nominal FP64/BF16 ratio 45/2250" % peak_src,
+                     "instruction_path": "FP64 FMA (DFMA)",
+                     "apply_ms": apply_ms, "peak_dfma_loop_measured": dfma, "peak_dmma_loop_measured": dmma,
+                     "frac_of_dfma_measured": achieved / dfma,
+                     "hbm_achieved_gbs": info["operator_bytes"] / (apply_ms * 1e-3) / 1e9, "hbm_peak_gbs": peaks["hbm_gbs"]},
+        "davidson": {"theta": [h[0] for h in hist], "resnorm": [h[1] for h in hist]},
+    }
+    if not args.no_cpu_baseline:
+        line["cpu_baseline"] = {k: v for k, v in time_oracle(args.config, 1, 0, budget_s=15.0).items()
+                                if k in ("value", "unit", "cores", "kind", "sample")}
+    print(json.dumps(line))
+    solver.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="cfg3")
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

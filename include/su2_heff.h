@@ -1,0 +1,188 @@
+/*
+ * su2_heff.h -- C ABI of the B200-native SU(2) spin-adapted two-site DMRG hot path:
+ * the superblock product  F = H_eff * Psi  inside a Davidson eigensolver
+ * (arXiv:2309.16724; all citations are PAPER.md:<line> of the paper text).
+ *
+ * What the library computes.  The paper's Eq. (2)/(3),
+ *
+ *     F{p^F} := F{p^F} + alpha_i A_i{p^A} B_i{p^B} C_i{p^C} D_i{p^D} E{p^E},
+ *
+ * for models whose two site Hilbert spaces decompose into one-dimensional sectors
+ * reduces per (operator-table row, sector combination, position) to
+ *
+ *     F_s (m x p)  +=  coef * alpha_pos * A_pos (m x k) * E_s' (k x n) * D_pos^T (n x p),
+ *
+ * where coef (the paper's "sector-value-table" entry) is the product of the site
+ * operators' reduced elements, the fermion sign and the SU(2) factor C~ of Eq. (5)/(9)
+ * for block x site, site x block and the superblock (the paper's
+ * W^(l), W^(r), W^(h) look-ups), all precomputed at plan time.
+ *
+ * Conventions: subsystems l (left block), B (site), C (site), r (right block) in
+ * Jordan-Wigner order; coupling tree ((l,B)J1,(C,r)J2)S_tot; Wigner-Eckart convention
+ * <S M|T^k_q|S' M'> = <k q; S' M'|S M> <S||T||S'>; all spins are passed DOUBLED (twoS = 2S).
+ * A Psi sector is s = (il, sB, twoJ1, sC, ir, twoJ2); its data is one dense row-major
+ * dim_l(il) x dim_r(ir) FP64 block; Psi and F are flat vectors of these blocks in the order
+ * returned by su2_plan_psi_layout.
+ *
+ * Ownership: the caller owns every device buffer and the CUDA stream.  Host arrays handed to
+ * su2_plan_create are copied and may be freed afterwards; operator-family `data` pointers are
+ * DEVICE pointers that must stay valid and unchanged while the plan is used.  The library
+ * allocates only the plan's own task tables on the device (freed by su2_plan_destroy).
+ * Errors: every entry point returns 0 on success and a negative su2_status otherwise; no
+ * exceptions, no aborts, no partial state.  Results are bit-reproducible for a fixed plan.
+ */
+#ifndef SU2_HEFF_H
+#define SU2_HEFF_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef int32_t su2_status;
+enum {
+  SU2_OK = 0,
+  SU2_ERR_INVALID_ARGUMENT = -1,   /* null pointer, negative size, bad index                     */
+  SU2_ERR_INVALID_SECTOR = -2,     /* block references a sector that does not exist / wrong dN  */
+  SU2_ERR_INVALID_RANK = -3,       /* ranks of a row cannot be coupled (triangle rule), k1 != k2 */
+  SU2_ERR_NOT_FINITE = -4,         /* non-finite alpha or site element                           */
+  SU2_ERR_CUDA = -5,               /* a CUDA runtime call failed (see su2_last_cuda_error)       */
+  SU2_ERR_NO_DEVICE_PLAN = -6,     /* plan was created with SU2_PLAN_HOST_ONLY                   */
+  SU2_ERR_WORKSPACE = -7           /* workspace pointer null although workspace_bytes > 0        */
+};
+const char* su2_status_string(su2_status st);
+const char* su2_last_cuda_error(void);
+/* Number of kernels this library has launched since it was loaded (all entry points). */
+int64_t su2_kernel_launch_count(void);
+
+typedef struct su2_plan su2_plan;             /* opaque */
+typedef struct su2_davidson su2_davidson;     /* opaque */
+
+/* Block sector (N, S) with multiplicity dim = number of multiplets kept. */
+typedef struct { int32_t N, twoS, dim; } su2_sector;
+
+/* One operator *family* on a block: all position-dependent operators of one type
+ * ("dense matrices of the same operator type have a third index ... labeling
+ * their positions ... contiguous segments in memory").  Reduced (Wigner-Eckart) blocks. */
+typedef struct {
+  int32_t dN;                /* particle-number change                                          */
+  int32_t twoK;              /* doubled spin rank k                                             */
+  int32_t npos;              /* number of positions                                             */
+  int32_t nblk;              /* number of non-zero sector blocks                                */
+  const int32_t* q_out;      /* HOST [nblk]: row (bra) sector index of block b                  */
+  const int32_t* q_in;       /* HOST [nblk]: column (ket) sector index of block b               */
+  const int64_t* blk_off;    /* HOST [nblk]: element offset of block b inside `data`            */
+  const double* data;        /* DEVICE: block b = [npos][dim(q_out)][dim(q_in)] row-major       */
+} su2_opfamily;
+
+/* Site operator: reduced elements r[out][in] over the site multiplets 0=(N=0,S=0),
+ * 1=(1,1/2), 2=(2,0) (the site basis shrinks from four to three). */
+typedef struct { double r[3][3]; int32_t dN, twoK; } su2_siteop;
+
+/* Operator-table row: the rank-0 operator
+ *   X = sum_pos alpha[pos] * [[O_l x O_B]^{k1} x [O_C x O_r]^{k2}]^0,  k1 == k2.
+ * The row has npos positions; a family with npos positions is indexed by pos, a family with a
+ * single position (or the identity, index -1) is the same for all positions.
+ * adj_l/adj_r = 1: use the adjoint tensor T~_q = (-1)^(k+q) (T_-q)^dagger of the family (its
+ * stored blocks are read transposed) -- Hermitian-conjugate rows need no second copy. */
+typedef struct {
+  int32_t fam_l, fam_r;      /* family index on l / r, -1 = identity                            */
+  int32_t op_B, op_C;        /* site operator indices                                           */
+  int32_t twoK_L, twoK_R;    /* doubled ranks k1, k2                                            */
+  int32_t adj_l, adj_r;
+  int32_t npos;              /* positions of this row                                           */
+  const double* alpha;       /* HOST [npos] or NULL (all 1.0)                                   */
+} su2_term;
+
+typedef struct {
+  int32_t n_tot, twoS_tot;   /* target particle number and doubled total spin                   */
+  int32_t nsec_l, nsec_r;
+  const su2_sector *sec_l, *sec_r;
+  int32_t nfam_l, nfam_r;
+  const su2_opfamily *fam_l, *fam_r;
+  int32_t nsite;
+  const su2_siteop* site;
+  int32_t nterm;
+  const su2_term* term;
+} su2_problem;
+
+enum {
+  SU2_PLAN_DEFAULT = 0,
+  SU2_PLAN_HOST_ONLY = 1,    /* no device tables: planner tests on CPU                          */
+  SU2_PLAN_FORCE_SPLIT = 2   /* tiny segments: exercises the segmented reduction on small inputs */
+};
+
+typedef struct {
+  int64_t psi_len;           /* number of doubles in Psi / F                                    */
+  int64_t ntasks;            /* sector tasks (paper: rows of all sector-task-tables)            */
+  int64_t ntask_positions;   /* tasks counted once per position (paper's "number of tasks")     */
+  double cc_flops;           /* CC = sum over task-positions of min(2mkn+2mnp, 2knp+2mkp)       */
+  double executed_flops;     /* flops the kernels execute per apply (tile padding, recompute)   */
+  double operator_bytes;     /* 8(mk+np) summed over task-positions (algorithmic HBM traffic)   */
+  int64_t workspace_bytes;   /* device workspace su2_heff_apply needs                           */
+  int32_t npsi_sec;          /* number of Psi sectors                                           */
+  int32_t nsegments;         /* work segments (deterministic segmented reduction)               */
+  int64_t nwork_items;       /* CTA-level work items per apply                                  */
+  double plan_seconds;       /* host time spent in su2_plan_create                              */
+} su2_plan_info_t;
+
+/* Build the plan: enumerate the sector tasks (Eq. (3)), compute the coefficient of each
+ * (sector-value-table), sort them by output sector, cut the lists into
+ * load-balanced segments and upload the tables on `cuda_stream` (synchronises). */
+su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int32_t flags, void* cuda_stream);
+su2_status su2_plan_destroy(su2_plan* plan);
+su2_status su2_plan_info(const su2_plan* plan, su2_plan_info_t* info);
+/* labels: HOST [npsi_sec][6] = (il, sB, twoJ1, sC, ir, twoJ2); offsets: HOST [npsi_sec+1]. */
+su2_status su2_plan_psi_layout(const su2_plan* plan, int32_t* labels, int64_t* offsets);
+
+/* Host copy of the task table, for tests of the planner (HOST arrays of length ntasks):
+ * out_sec/in_sec: Psi sector indices; fam/blk/adj per side (fam -1 = identity); term: the row
+ * the task came from; coef: the precomputed scalar (without alpha). */
+su2_status su2_plan_export_tasks(const su2_plan* plan, int32_t* out_sec, int32_t* in_sec,
+                                 int32_t* fam_l, int32_t* blk_l, int32_t* adj_l,
+                                 int32_t* fam_r, int32_t* blk_r, int32_t* adj_r,
+                                 int32_t* term, double* coef);
+
+/* out_dev = H_eff * psi_dev (overwrites; out must not alias psi).  Asynchronous on the stream.
+ * workspace_dev: DEVICE, >= workspace_bytes, 256-byte aligned. */
+su2_status su2_heff_apply(const su2_plan* plan, const double* psi_dev, double* out_dev,
+                          void* workspace_dev, void* cuda_stream);
+/* Same through HOST buffers: copies psi to the device, applies, copies the result back and
+ * synchronises (the end-to-end entry point; device staging buffers inside workspace_dev, which
+ * must hold workspace_bytes + 2*8*psi_len bytes). */
+su2_status su2_heff_apply_host(const su2_plan* plan, const double* psi_host, double* out_host,
+                               void* workspace_dev, void* cuda_stream);
+/* diag_dev = diagonal of H_eff in the reduced basis (for the Davidson preconditioner). */
+su2_status su2_heff_diag(const su2_plan* plan, double* diag_dev, void* cuda_stream);
+
+/* Davidson eigensolver for the lowest eigenpair (reading G8 in DESIGN.md):
+ * diagonal preconditioner, modified Gram-Schmidt applied twice, subspace <= max_subspace
+ * (restart from the Ritz vector when full).  All vectors live in dav_workspace_dev
+ * (DEVICE, su2_davidson_workspace_bytes bytes, caller-owned). */
+int64_t su2_davidson_workspace_bytes(const su2_plan* plan, int32_t max_subspace);
+su2_status su2_davidson_create(su2_davidson** out, const su2_plan* plan, int32_t max_subspace,
+                               const double* x0_dev, void* dav_workspace_dev, void* cuda_stream);
+/* One iteration: w = H_eff v (su2_heff_apply), Rayleigh-Ritz, residual, new direction.
+ * theta: current Ritz value; resnorm: |H x - theta x|.  Synchronises for the two scalars. */
+su2_status su2_davidson_step(const su2_plan* plan, su2_davidson* dav, void* workspace_dev,
+                             void* cuda_stream, double* theta, double* resnorm);
+su2_status su2_davidson_ritz_vector(const su2_davidson* dav, double* x_dev, void* cuda_stream);
+su2_status su2_davidson_destroy(su2_davidson* dav);
+
+/* Strided-batched FP64 GEMM-pair microbenchmark entry (BASELINE.json configs[4]):
+ * C_b (m x p) += alpha * A_b (m x k) * X_b (k x n) * B_b^T (n x p) for b < batch, all DEVICE,
+ * row-major, dense strides (A_b = A + b*m*k, ...).  Uses the same fused kernel as the apply. */
+su2_status su2_gemm_pair_batched(int32_t m, int32_t k, int32_t n, int32_t p, int64_t batch, double alpha,
+                                 const double* A, const double* X, const double* B, double* C,
+                                 void* cuda_stream);
+
+/* Measurement aid, not on the hot path: register-resident FP64 throughput of the current device
+ * in TFLOP/s (best of 3 timed launches, CUDA events on cuda_stream; synchronises).
+ * kind 0: DFMA loop (FP64 vector pipe); kind 1: mma.sync.m8n8k4.f64 loop (SASS DMMA.8x8x4). */
+su2_status su2_probe_fp64_peak(int32_t kind, int32_t iters, int32_t ctas_per_sm, double* tflops, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SU2_HEFF_H */

@@ -1,0 +1,262 @@
+"""Thin Python binding of the C ABI in include/su2_heff.h (argument marshalling only: every
+step of the hot path runs inside libsu2heff.so).  PyTorch is used by the callers for device
+memory and streams; this module itself only needs ctypes + numpy."""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libsu2heff.so")
+
+
+class Su2Error(RuntimeError):
+    pass
+
+
+class su2_sector(C.Structure):
+    _fields_ = [("N", C.c_int32), ("twoS", C.c_int32), ("dim", C.c_int32)]
+
+
+class su2_opfamily(C.Structure):
+    _fields_ = [("dN", C.c_int32), ("twoK", C.c_int32), ("npos", C.c_int32), ("nblk", C.c_int32),
+                ("q_out", C.POINTER(C.c_int32)), ("q_in", C.POINTER(C.c_int32)),
+                ("blk_off", C.POINTER(C.c_int64)), ("data", C.c_void_p)]
+
+
+class su2_siteop(C.Structure):
+    _fields_ = [("r", (C.c_double * 3) * 3), ("dN", C.c_int32), ("twoK", C.c_int32)]
+
+
+class su2_term(C.Structure):
+    _fields_ = [("fam_l", C.c_int32), ("fam_r", C.c_int32), ("op_B", C.c_int32), ("op_C", C.c_int32),
+                ("twoK_L", C.c_int32), ("twoK_R", C.c_int32), ("adj_l", C.c_int32), ("adj_r", C.c_int32),
+                ("npos", C.c_int32), ("alpha", C.POINTER(C.c_double))]
+
+
+class su2_problem(C.Structure):
+    _fields_ = [("n_tot", C.c_int32), ("twoS_tot", C.c_int32), ("nsec_l", C.c_int32), ("nsec_r", C.c_int32),
+                ("sec_l", C.POINTER(su2_sector)), ("sec_r", C.POINTER(su2_sector)),
+                ("nfam_l", C.c_int32), ("nfam_r", C.c_int32),
+                ("fam_l", C.POINTER(su2_opfamily)), ("fam_r", C.POINTER(su2_opfamily)),
+                ("nsite", C.c_int32), ("site", C.POINTER(su2_siteop)),
+                ("nterm", C.c_int32), ("term", C.POINTER(su2_term))]
+
+
+class su2_plan_info_t(C.Structure):
+    _fields_ = [("psi_len", C.c_int64), ("ntasks", C.c_int64), ("ntask_positions", C.c_int64),
+                ("cc_flops", C.c_double), ("executed_flops", C.c_double), ("operator_bytes", C.c_double),
+                ("workspace_bytes", C.c_int64), ("npsi_sec", C.c_int32), ("nsegments", C.c_int32),
+                ("nwork_items", C.c_int64), ("plan_seconds", C.c_double)]
+
+
+EXPORTS = ["su2_status_string", "su2_last_cuda_error", "su2_kernel_launch_count", "su2_plan_create", "su2_plan_destroy", "su2_plan_info",
+           "su2_plan_psi_layout", "su2_plan_export_tasks", "su2_heff_apply", "su2_heff_apply_host", "su2_heff_diag",
+           "su2_davidson_workspace_bytes", "su2_davidson_create", "su2_davidson_step", "su2_davidson_ritz_vector",
+           "su2_davidson_destroy", "su2_gemm_pair_batched", "su2_probe_fp64_peak"]
+
+SU2_PLAN_HOST_ONLY = 1
+_lib = None
+
+
+def load():
+    """Load libsu2heff.so.  Fails loudly if the extension has not been built: there is no
+    fallback path."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise Su2Error("CUDA extension %s is missing: run __graft_entry__.build() "
+                       "(python -m paper_2309_16724_b200.build)" % LIB_PATH)
+    lib = C.CDLL(LIB_PATH)
+    for name in EXPORTS:
+        getattr(lib, name).restype = C.c_int32
+    lib.su2_status_string.restype = C.c_char_p
+    lib.su2_status_string.argtypes = [C.c_int32]
+    lib.su2_last_cuda_error.restype = C.c_char_p
+    lib.su2_kernel_launch_count.restype = C.c_int64
+    lib.su2_plan_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(su2_problem), C.c_int32, C.c_void_p]
+    lib.su2_plan_destroy.argtypes = [C.c_void_p]
+    lib.su2_plan_info.argtypes = [C.c_void_p, C.POINTER(su2_plan_info_t)]
+    lib.su2_plan_psi_layout.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.su2_plan_export_tasks.argtypes = [C.c_void_p] + [C.c_void_p] * 10
+    lib.su2_heff_apply.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.su2_heff_apply_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.su2_heff_diag.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.su2_davidson_workspace_bytes.restype = C.c_int64
+    lib.su2_davidson_workspace_bytes.argtypes = [C.c_void_p, C.c_int32]
+    lib.su2_davidson_create.argtypes = [C.POINTER(C.c_void_p), C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.su2_davidson_step.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                      C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.su2_davidson_ritz_vector.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.su2_davidson_destroy.argtypes = [C.c_void_p]
+    lib.su2_gemm_pair_batched.argtypes = [C.c_int32] * 4 + [C.c_int64, C.c_double] + [C.c_void_p] * 5
+    lib.su2_probe_fp64_peak.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_double), C.c_void_p]
+    _lib = lib
+    return lib
+
+
+def check(st):
+    if st != 0:
+        lib = load()
+        msg = lib.su2_status_string(st).decode()
+        if st == -5:
+            msg += " (" + lib.su2_last_cuda_error().decode() + ")"
+        raise Su2Error("su2 status %d: %s" % (st, msg))
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def family_block_offsets(fam, secs):
+    """Element offset of each block inside the family's buffer: blocks in order, each
+    [npos][dim(q_out)][dim(q_in)] row-major."""
+    offs, cur = [], 0
+    for qo, qi in zip(fam.q_out, fam.q_in):
+        offs.append(cur)
+        if 0 <= qo < len(secs) and 0 <= qi < len(secs):      # bad indices are rejected by su2_plan_create
+            cur += fam.npos * secs[qo].dim * secs[qi].dim
+    return offs
+
+
+def family_elems(fam, secs):
+    return sum(fam.npos * secs[qo].dim * secs[qi].dim for qo, qi in zip(fam.q_out, fam.q_in))
+
+
+class Plan:
+    """su2_plan wrapper.  `problem` is a gen.problem.Problem-like object (plain data);
+    `family_ptrs` maps ("l"|"r", family index) -> DEVICE base pointer (int) of the family's
+    blocks laid out block after block, each [npos][m][k] (see family_block_offsets); None
+    for a host-only plan (planner tests without a GPU)."""
+
+    def __init__(self, problem, family_ptrs=None, stream=0, host_only=False, force_split=False):
+        lib = load()
+        self._keep = []
+        self.problem = problem
+
+        def sectors(secs):
+            arr = (su2_sector * len(secs))(*[su2_sector(s.N, s.twoS, s.dim) for s in secs])
+            self._keep.append(arr)
+            return arr
+
+        def families(fams, secs, side):
+            arr = (su2_opfamily * max(len(fams), 1))()
+            for i, f in enumerate(fams):
+                qo, qi = _i32(f.q_out), _i32(f.q_in)
+                off = np.asarray(family_block_offsets(f, secs), dtype=np.int64)
+                self._keep += [qo, qi, off]
+                ptr = None if family_ptrs is None else family_ptrs[(side, i)]
+                arr[i] = su2_opfamily(f.dN, f.twoK, f.npos, len(f.q_out),
+                                      qo.ctypes.data_as(C.POINTER(C.c_int32)), qi.ctypes.data_as(C.POINTER(C.c_int32)),
+                                      off.ctypes.data_as(C.POINTER(C.c_int64)), ptr)
+            self._keep.append(arr)
+            return arr
+
+        sl, sr = sectors(problem.sec_l), sectors(problem.sec_r)
+        fl = families(problem.fam_l, problem.sec_l, "l")
+        fr = families(problem.fam_r, problem.sec_r, "r")
+        site = (su2_siteop * len(problem.site))()
+        for i, o in enumerate(problem.site):
+            for a in range(3):
+                for b in range(3):
+                    site[i].r[a][b] = float(o.r[a][b])
+            site[i].dN, site[i].twoK = o.dN, o.twoK
+        terms = (su2_term * max(len(problem.term), 1))()
+        for i, t in enumerate(problem.term):
+            npos = problem.npos_of(t)
+            if t.alpha is None:
+                ap = C.POINTER(C.c_double)()
+            else:
+                a = np.ascontiguousarray(t.alpha, dtype=np.float64)
+                assert a.shape == (npos,), (t.name, a.shape, npos)
+                self._keep.append(a)
+                ap = a.ctypes.data_as(C.POINTER(C.c_double))
+            terms[i] = su2_term(t.fam_l, t.fam_r, t.op_B, t.op_C, t.twoK_L, t.twoK_R, t.adj_l, t.adj_r, npos, ap)
+        self._keep += [site, terms]
+        prob = su2_problem(problem.n_tot, problem.twoS_tot, len(problem.sec_l), len(problem.sec_r), sl, sr,
+                           len(problem.fam_l), len(problem.fam_r), fl, fr, len(problem.site), site,
+                           len(problem.term), terms)
+        self.handle = C.c_void_p()
+        check(lib.su2_plan_create(C.byref(self.handle), C.byref(prob), (SU2_PLAN_HOST_ONLY if host_only else 0) | (2 if force_split else 0),
+                                  C.c_void_p(stream)))
+        info = su2_plan_info_t()
+        check(lib.su2_plan_info(self.handle, C.byref(info)))
+        self.info = {k: getattr(info, k) for k, _ in su2_plan_info_t._fields_}
+        n = self.info["npsi_sec"]
+        labels = np.zeros((n, 6), dtype=np.int32)
+        offsets = np.zeros(n + 1, dtype=np.int64)
+        check(lib.su2_plan_psi_layout(self.handle, labels.ctypes.data, offsets.ctypes.data))
+        self.labels = [tuple(int(x) for x in row) for row in labels]
+        self.offsets = offsets
+        self.psi_len = int(self.info["psi_len"])
+        self.workspace_bytes = int(self.info["workspace_bytes"])
+
+    def export_tasks(self):
+        n = int(self.info["ntasks"])
+        names = ["out_sec", "in_sec", "fam_l", "blk_l", "adj_l", "fam_r", "blk_r", "adj_r", "term"]
+        arrs = {k: np.zeros(n, dtype=np.int32) for k in names}
+        coef = np.zeros(n, dtype=np.float64)
+        check(load().su2_plan_export_tasks(self.handle, *[arrs[k].ctypes.data for k in names], coef.ctypes.data))
+        arrs["coef"] = coef
+        return arrs
+
+    # --- device entry points (pointers are plain ints) ---
+    def heff_apply(self, psi_ptr, out_ptr, workspace_ptr, stream=0):
+        check(load().su2_heff_apply(self.handle, psi_ptr, out_ptr, workspace_ptr, stream))
+
+    def heff_apply_host(self, psi_host_ptr, out_host_ptr, workspace_ptr, stream=0):
+        check(load().su2_heff_apply_host(self.handle, psi_host_ptr, out_host_ptr, workspace_ptr, stream))
+
+    def heff_diag(self, diag_ptr, stream=0):
+        check(load().su2_heff_diag(self.handle, diag_ptr, stream))
+
+    def close(self):
+        if getattr(self, "handle", None):
+            load().su2_plan_destroy(self.handle)
+            self.handle = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Davidson:
+    def __init__(self, plan, max_subspace, x0_ptr, ws_ptr, stream=0):
+        self.plan = plan
+        self.handle = C.c_void_p()
+        check(load().su2_davidson_create(C.byref(self.handle), plan.handle, max_subspace, x0_ptr, ws_ptr, stream))
+
+    @staticmethod
+    def workspace_bytes(plan, max_subspace):
+        return int(load().su2_davidson_workspace_bytes(plan.handle, max_subspace))
+
+    def step(self, workspace_ptr, stream=0):
+        th, rn = C.c_double(), C.c_double()
+        check(load().su2_davidson_step(self.plan.handle, self.handle, workspace_ptr, stream, C.byref(th), C.byref(rn)))
+        return th.value, rn.value
+
+    def ritz_vector(self, x_ptr, stream=0):
+        check(load().su2_davidson_ritz_vector(self.handle, x_ptr, stream))
+
+    def close(self):
+        if getattr(self, "handle", None):
+            load().su2_davidson_destroy(self.handle)
+            self.handle = C.c_void_p()
+
+
+def gemm_pair_batched(m, k, n, p, batch, alpha, a_ptr, x_ptr, b_ptr, c_ptr, stream=0):
+    check(load().su2_gemm_pair_batched(m, k, n, p, batch, alpha, a_ptr, x_ptr, b_ptr, c_ptr, stream))
+
+
+def probe_fp64_peak(kind, iters=20000, ctas_per_sm=4, stream=0):
+    """Measured register-resident FP64 TFLOP/s: kind 0 = DFMA loop, 1 = DMMA.8x8x4 loop."""
+    v = C.c_double()
+    check(load().su2_probe_fp64_peak(kind, iters, ctas_per_sm, C.byref(v), stream))
+    return v.value
+
+
+def kernel_launch_count():
+    return int(load().su2_kernel_launch_count())

@@ -1,0 +1,383 @@
+// sm_100a kernels of the hot path:
+//   heff_fused_kernel : F_tile += coef * sum_pos alpha_pos A_pos E D_pos^T with T = A_pos E held in
+//                       shared memory (the paper's two SBGEMM steps, fused; the sum
+//                       over positions is the K loop of the second product = the stripe trick).
+//   reduce_kernel     : fixed-order sum of the partial tiles of split sectors (no atomics).
+//   diag kernels      : diagonal of H_eff for the Davidson preconditioner.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <string>
+
+#include "su2_internal.h"
+#include "tile_config.h"
+
+namespace su2 {
+
+static thread_local std::string g_cuda_error;
+static long long g_launches = 0;
+void count_launch(int n) { g_launches += n; }
+void set_cuda_error(const char* what, int code) {
+  g_cuda_error = std::string(what) + ": " + cudaGetErrorString((cudaError_t)code);
+}
+#define SU2_CUDA(call)                              \
+  do {                                              \
+    cudaError_t _e = (call);                        \
+    if (_e != cudaSuccess) {                        \
+      set_cuda_error(#call, (int)_e);               \
+      return SU2_ERR_CUDA;                          \
+    }                                               \
+  } while (0)
+
+// ---------------------------------------------------------------------------------------
+// v1 fused GEMM-pair kernel: FP64 FMA, 64x64 output tile, 256 threads, T chunk in smem.
+// ---------------------------------------------------------------------------------------
+constexpr int NTHREADS = 256;
+constexpr int NC = 32;    // columns of T (n-chunk) per pass
+constexpr int KC = 16;    // k-chunk of the first product
+
+struct TileSmem {
+  double As[TILE_M][KC + 1];      // A[row0+i][k0+kk]
+  double Es[KC][NC + 1];          // E[k0+kk][n0+j]
+  double Ts[TILE_M][NC + 1];      // coef*alpha * (A E)[i][j]
+  double Ds[TILE_P][NC + 1];      // D[col0+c][n0+j]
+};
+
+// acc (64x64 tile at (row0,col0), thread (ty,tx) owns rows ty+16i, cols tx+16c)
+//   += coef * sum_{pos0<=pos<pos1} alpha_pos * A_pos[row0:,:] E D_pos[col0:,:]^T
+__device__ __forceinline__ void accumulate_task(const DevTask& t, const double* __restrict__ E, int pos0, int pos1,
+                                                int row0, int col0, TileSmem& sm, double (&acc)[4][4]) {
+  const int tid = threadIdx.x;
+  const int ty = tid / 16, tx = tid % 16;    // second product: rows ty+16*i, cols tx+16*j
+  const int gy = tid / 8, gx = tid % 8;      // first product : rows gy+32*i (i<2), cols gx+8*j (j<4)
+  const bool ta = t.flags & TASK_TRANS_A, td = t.flags & TASK_TRANS_D;
+  for (int pos = pos0; pos < pos1; ++pos) {
+    const double* __restrict__ A = t.A + (int64_t)pos * t.strideA;
+    const double* __restrict__ D = t.D + (int64_t)pos * t.strideD;
+    const double scale = t.coef * (t.alpha ? t.alpha[pos] : 1.0);
+    for (int n0 = 0; n0 < t.n; n0 += NC) {
+      // ---- first product: T[64 x NC] = A[row0:row0+64, :] * E[:, n0:n0+NC]
+      double tacc[2][4];
+#pragma unroll
+      for (int i = 0; i < 2; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) tacc[i][j] = 0.0;
+      for (int k0 = 0; k0 < t.k; k0 += KC) {
+        for (int e = tid; e < TILE_M * KC; e += NTHREADS) {
+          int i, kk;
+          if (!ta) { i = e / KC; kk = e % KC; } else { kk = e / TILE_M; i = e % TILE_M; }
+          const int r = row0 + i, c = k0 + kk;
+          double v = 0.0;
+          if (r < t.m && c < t.k) v = ta ? A[(int64_t)c * t.m + r] : A[(int64_t)r * t.k + c];
+          sm.As[i][kk] = v;
+        }
+        for (int e = tid; e < KC * NC; e += NTHREADS) {
+          const int kk = e / NC, j = e % NC;
+          const int r = k0 + kk, c = n0 + j;
+          sm.Es[kk][j] = (r < t.k && c < t.n) ? E[(int64_t)r * t.n + c] : 0.0;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int kk = 0; kk < KC; ++kk) {
+          double a[2], b[4];
+#pragma unroll
+          for (int i = 0; i < 2; ++i) a[i] = sm.As[gy + 32 * i][kk];
+#pragma unroll
+          for (int j = 0; j < 4; ++j) b[j] = sm.Es[kk][gx + 8 * j];
+#pragma unroll
+          for (int i = 0; i < 2; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) tacc[i][j] = fma(a[i], b[j], tacc[i][j]);
+        }
+        __syncthreads();
+      }
+#pragma unroll
+      for (int i = 0; i < 2; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) sm.Ts[gy + 32 * i][gx + 8 * j] = scale * tacc[i][j];
+      // ---- D tile: Ds[c][j] = D[col0+c][n0+j]
+      for (int e = tid; e < TILE_P * NC; e += NTHREADS) {
+        int c, j;
+        if (!td) { c = e / NC; j = e % NC; } else { j = e / TILE_P; c = e % TILE_P; }
+        const int r = col0 + c, q = n0 + j;
+        double v = 0.0;
+        if (r < t.p && q < t.n) v = td ? D[(int64_t)q * t.p + r] : D[(int64_t)r * t.n + q];
+        sm.Ds[c][j] = v;
+      }
+      __syncthreads();
+      // ---- second product: F_tile += T * Ds^T  (K = NC columns of this position's stripe)
+#pragma unroll 8
+      for (int j = 0; j < NC; ++j) {
+        double a[4], b[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) a[i] = sm.Ts[ty + 16 * i][j];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) b[c] = sm.Ds[tx + 16 * c][j];
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int c = 0; c < 4; ++c) acc[i][c] = fma(a[i], b[c], acc[i][c]);
+      }
+      __syncthreads();
+    }
+  }
+}
+
+__global__ void __launch_bounds__(NTHREADS)
+heff_fused_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __restrict__ units,
+                  const DevTask* __restrict__ tasks, const double* __restrict__ psi, double* __restrict__ out,
+                  double* __restrict__ partial, int* __restrict__ counter) {
+  __shared__ TileSmem sm;
+  __shared__ int s_w;
+  const int tid = threadIdx.x;
+  const int ty = tid / 16, tx = tid % 16;
+  for (;;) {
+    if (tid == 0) s_w = atomicAdd(counter, 1);
+    __syncthreads();
+    const int w = s_w;
+    __syncthreads();
+    if (w >= nwork) break;
+    const DevWork wk = work[w];
+    double acc[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+      for (int j = 0; j < 4; ++j) acc[i][j] = 0.0;
+    for (int u = wk.unit0; u < wk.unit1; ++u) {
+      const DevUnit un = units[u];
+      const DevTask t = tasks[un.task];
+      accumulate_task(t, psi + t.e_off, un.pos0, un.pos1, wk.row0, wk.col0, sm, acc);
+    }
+    double* __restrict__ dst = (wk.to_partial ? partial : out) + wk.dst_off;
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const int r = wk.row0 + ty + 16 * i, q = wk.col0 + tx + 16 * c;
+        if (r < wk.m && q < wk.p) dst[(int64_t)r * wk.p + q] = acc[i][c];
+      }
+  }
+}
+
+// BASELINE.json configs[4]: C_b += alpha A_b X_b B_b^T; blockIdx.x = tile, blockIdx.y/z = batch index.
+__global__ void __launch_bounds__(NTHREADS)
+gemm_pair_kernel(int m, int k, int n, int p, int64_t batch, double alpha, const double* __restrict__ A,
+                 const double* __restrict__ X, const double* __restrict__ B, double* __restrict__ C) {
+  __shared__ TileSmem sm;
+  const int tiles_p = (p + TILE_P - 1) / TILE_P;
+  const int row0 = (blockIdx.x / tiles_p) * TILE_M, col0 = (blockIdx.x % tiles_p) * TILE_P;
+  const int ty = threadIdx.x / 16, tx = threadIdx.x % 16;
+  for (int64_t b = blockIdx.y; b < batch; b += gridDim.y) {
+    DevTask t;
+    t.A = A + b * (int64_t)m * k; t.D = B + b * (int64_t)p * n; t.alpha = nullptr; t.coef = alpha; t.e_off = 0;
+    t.m = m; t.k = k; t.n = n; t.p = p; t.strideA = 0; t.strideD = 0; t.npos = 1; t.flags = 0;
+    double acc[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+      for (int j = 0; j < 4; ++j) acc[i][j] = 0.0;
+    accumulate_task(t, X + b * (int64_t)k * n, 0, 1, row0, col0, sm, acc);
+    double* __restrict__ dst = C + b * (int64_t)m * p;
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const int r = row0 + ty + 16 * i, q = col0 + tx + 16 * c;
+        if (r < m && q < p) dst[(int64_t)r * p + q] += acc[i][c];
+      }
+  }
+}
+
+// Second pass of the segmented reduction: fixed index order, one thread per element.
+__global__ void __launch_bounds__(256)
+reduce_kernel(const DevReduce* __restrict__ red, const double* __restrict__ partial, double* __restrict__ out) {
+  const DevReduce r = red[blockIdx.y];
+  if (r.nseg == 1) return;                    // written directly by the fused kernel
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < r.size; i += (int64_t)gridDim.x * blockDim.x) {
+    double s = 0.0;
+    for (int g = 0; g < r.nseg; ++g) s += partial[r.part_off + (int64_t)g * r.size + i];
+    out[r.f_off + i] = s;
+  }
+}
+
+// diag(H_eff)[s][a,b] = sum_{tasks s<-s} coef sum_pos alpha_pos A_pos[a,a] D_pos[b,b]
+__global__ void __launch_bounds__(256)
+diag_kernel(const DevDiagTask* __restrict__ dt, const int32_t* __restrict__ begin, const PsiSector* __restrict__ psi_sec,
+            double* __restrict__ diag) {
+  const int s = blockIdx.y;
+  const int m = psi_sec[s].m, p = psi_sec[s].p;
+  const int64_t off = psi_sec[s].off;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < (int64_t)m * p; e += (int64_t)gridDim.x * blockDim.x) {
+    const int a = (int)(e / p), b = (int)(e % p);
+    double acc = 0.0;
+    for (int i = begin[s]; i < begin[s + 1]; ++i) {
+      const DevDiagTask t = dt[i];
+      double v = 0.0;
+      for (int pos = 0; pos < t.npos; ++pos) {
+        const double al = t.alpha ? t.alpha[pos] : 1.0;
+        v += al * t.A[(int64_t)pos * t.strideA + (int64_t)a * m + a] * t.D[(int64_t)pos * t.strideD + (int64_t)b * p + b];
+      }
+      acc += t.coef * v;
+    }
+    diag[off + e] = acc;
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------
+static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, const std::vector<double>& ident_host,
+                       const std::vector<int64_t>& alpha_off_of_task, const std::vector<int64_t>& identA,
+                       const std::vector<int64_t>& identD, void* stream_v) {
+  cudaStream_t stream = (cudaStream_t)stream_v;
+  int dev = 0;
+  SU2_CUDA(cudaGetDevice(&dev));
+  SU2_CUDA(cudaDeviceGetAttribute(&plan->num_sms, cudaDevAttrMultiProcessorCount, dev));
+  const size_t b_tasks = align256(plan->h_tasks.size() * sizeof(DevTask));
+  const size_t b_units = align256(plan->h_units.size() * sizeof(DevUnit));
+  const size_t b_work = align256(plan->h_work.size() * sizeof(DevWork));
+  const size_t b_red = align256(plan->h_reduce.size() * sizeof(DevReduce));
+  const size_t b_diag = align256(plan->h_diag.size() * sizeof(DevDiagTask));
+  const size_t b_dbeg = align256(plan->h_diag_begin.size() * sizeof(int32_t));
+  const size_t b_psi = align256(plan->psi.size() * sizeof(PsiSector));
+  const size_t b_alpha = align256(alpha_host.size() * sizeof(double));
+  const size_t b_ident = align256(ident_host.size() * sizeof(double));
+  const size_t total = b_tasks + b_units + b_work + b_red + b_diag + b_dbeg + b_psi + b_alpha + b_ident + 256;
+  SU2_CUDA(cudaMalloc(&plan->d_blob, total));
+  char* base = (char*)plan->d_blob;
+  size_t off = 0;
+  auto carve = [&](size_t bytes) { char* p = base + off; off += bytes; return p; };
+  plan->d_tasks = (DevTask*)carve(b_tasks);
+  plan->d_units = (DevUnit*)carve(b_units);
+  plan->d_work = (DevWork*)carve(b_work);
+  plan->d_reduce = (DevReduce*)carve(b_red);
+  plan->d_diag = (DevDiagTask*)carve(b_diag);
+  plan->d_diag_begin = (int32_t*)carve(b_dbeg);
+  char* d_psi = carve(b_psi);
+  plan->d_alpha = (double*)carve(b_alpha);
+  plan->d_identity = (double*)carve(b_ident);
+  plan->d_counter = (int32_t*)carve(256);
+  // patch device pointers into the host images
+  for (size_t i = 0; i < plan->h_tasks.size(); ++i) {
+    DevTask& t = plan->h_tasks[i];
+    if (alpha_off_of_task[i] >= 0) t.alpha = plan->d_alpha + alpha_off_of_task[i];
+    if (identA[i] >= 0) t.A = plan->d_identity + identA[i];
+    if (identD[i] >= 0) t.D = plan->d_identity + identD[i];
+    if (!t.A || !t.D) return SU2_ERR_INVALID_ARGUMENT;   // family without device data
+  }
+  for (auto& d : plan->h_diag) {
+    const DevTask& t = plan->h_tasks[d.pad];
+    d.A = t.A; d.D = t.D; d.alpha = t.alpha;
+  }
+  auto up = [&](void* dst, const void* src, size_t bytes) -> cudaError_t {
+    if (bytes == 0) return cudaSuccess;
+    return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, stream);
+  };
+  SU2_CUDA(up(plan->d_tasks, plan->h_tasks.data(), plan->h_tasks.size() * sizeof(DevTask)));
+  SU2_CUDA(up(plan->d_units, plan->h_units.data(), plan->h_units.size() * sizeof(DevUnit)));
+  SU2_CUDA(up(plan->d_work, plan->h_work.data(), plan->h_work.size() * sizeof(DevWork)));
+  SU2_CUDA(up(plan->d_reduce, plan->h_reduce.data(), plan->h_reduce.size() * sizeof(DevReduce)));
+  SU2_CUDA(up(plan->d_diag, plan->h_diag.data(), plan->h_diag.size() * sizeof(DevDiagTask)));
+  SU2_CUDA(up(plan->d_diag_begin, plan->h_diag_begin.data(), plan->h_diag_begin.size() * sizeof(int32_t)));
+  SU2_CUDA(up(d_psi, plan->psi.data(), plan->psi.size() * sizeof(PsiSector)));
+  SU2_CUDA(up(plan->d_alpha, alpha_host.data(), alpha_host.size() * sizeof(double)));
+  SU2_CUDA(up(plan->d_identity, ident_host.data(), ident_host.size() * sizeof(double)));
+  SU2_CUDA(cudaStreamSynchronize(stream));
+  plan->d_psi_sec = d_psi;
+  return SU2_OK;
+}
+
+void free_plan_device(su2_plan* plan) {
+  if (plan && plan->d_blob) {
+    cudaFree(plan->d_blob);
+    plan->d_blob = nullptr;
+  }
+}
+
+su2_status launch_apply(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream_v) {
+  cudaStream_t stream = (cudaStream_t)stream_v;
+  SU2_CUDA(cudaMemsetAsync(plan->d_counter, 0, sizeof(int32_t), stream));
+  const int nwork = (int)plan->h_work.size();
+  if (nwork > 0) {
+    int ctas_per_sm = 0;
+    SU2_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, heff_fused_kernel, NTHREADS, 0));
+    const int grid = std::min(nwork, plan->num_sms * std::max(ctas_per_sm, 1));
+    heff_fused_kernel<<<grid, NTHREADS, 0, stream>>>(plan->d_work, nwork, plan->d_units, plan->d_tasks, psi, out, partial,
+                                                     plan->d_counter);
+    SU2_CUDA(cudaGetLastError());
+    count_launch();
+  }
+  const int nsec = (int)plan->h_reduce.size();
+  if (nsec > 0) {
+    dim3 grid(32, nsec);
+    reduce_kernel<<<grid, 256, 0, stream>>>(plan->d_reduce, partial, out);
+    SU2_CUDA(cudaGetLastError());
+    count_launch();
+  }
+  return SU2_OK;
+}
+
+su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double alpha, const double* A, const double* X,
+                            const double* B, double* C, void* stream_v) {
+  if (batch == 0) return SU2_OK;
+  const int tiles = ((m + TILE_M - 1) / TILE_M) * ((p + TILE_P - 1) / TILE_P);
+  dim3 grid(tiles, (unsigned)std::min<int64_t>(batch, 65535));
+  gemm_pair_kernel<<<grid, NTHREADS, 0, (cudaStream_t)stream_v>>>(m, k, n, p, batch, alpha, A, X, B, C);
+  SU2_CUDA(cudaGetLastError());
+  count_launch();
+  return SU2_OK;
+}
+
+su2_status launch_diag(const su2_plan* plan, double* diag, void* stream_v) {
+  cudaStream_t stream = (cudaStream_t)stream_v;
+  const int nsec = (int)plan->psi.size();
+  if (nsec == 0) return SU2_OK;
+  dim3 grid(64, nsec);
+  diag_kernel<<<grid, 256, 0, stream>>>(plan->d_diag, plan->d_diag_begin, (const PsiSector*)plan->d_psi_sec, diag);
+  SU2_CUDA(cudaGetLastError());
+  count_launch();
+  return SU2_OK;
+}
+
+}  // namespace su2
+
+using namespace su2;
+
+extern "C" const char* su2_last_cuda_error(void) { return g_cuda_error.c_str(); }
+extern "C" int64_t su2_kernel_launch_count(void) { return (int64_t)g_launches; }
+
+extern "C" su2_status su2_heff_apply(const su2_plan* plan, const double* psi_dev, double* out_dev, void* workspace_dev,
+                                     void* cuda_stream) {
+  if (!plan || !psi_dev || !out_dev || psi_dev == out_dev) return SU2_ERR_INVALID_ARGUMENT;
+  if (plan->host_only) return SU2_ERR_NO_DEVICE_PLAN;
+  if (plan->partial_elems > 0 && !workspace_dev) return SU2_ERR_WORKSPACE;
+  return launch_apply(plan, psi_dev, out_dev, (double*)workspace_dev, cuda_stream);
+}
+
+extern "C" su2_status su2_heff_apply_host(const su2_plan* plan, const double* psi_host, double* out_host,
+                                          void* workspace_dev, void* cuda_stream) {
+  if (!plan || !psi_host || !out_host) return SU2_ERR_INVALID_ARGUMENT;
+  if (plan->host_only) return SU2_ERR_NO_DEVICE_PLAN;
+  if (!workspace_dev) return SU2_ERR_WORKSPACE;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  char* ws = (char*)workspace_dev;
+  const size_t wsb = (size_t)plan->info.workspace_bytes;
+  double* d_psi = (double*)(ws + ((wsb + 255) & ~(size_t)255));
+  double* d_out = d_psi + plan->psi_len;
+  SU2_CUDA(cudaMemcpyAsync(d_psi, psi_host, plan->psi_len * sizeof(double), cudaMemcpyHostToDevice, stream));
+  su2_status st = launch_apply(plan, d_psi, d_out, (double*)workspace_dev, cuda_stream);
+  if (st != SU2_OK) return st;
+  SU2_CUDA(cudaMemcpyAsync(out_host, d_out, plan->psi_len * sizeof(double), cudaMemcpyDeviceToHost, stream));
+  SU2_CUDA(cudaStreamSynchronize(stream));
+  return SU2_OK;
+}
+
+extern "C" su2_status su2_heff_diag(const su2_plan* plan, double* diag_dev, void* cuda_stream) {
+  if (!plan || !diag_dev) return SU2_ERR_INVALID_ARGUMENT;
+  if (plan->host_only) return SU2_ERR_NO_DEVICE_PLAN;
+  return launch_diag(plan, diag_dev, cuda_stream);
+}

@@ -1,0 +1,509 @@
+// Host planner: the paper's sector-task-table and sector-value-table
+// built once per bond, then sorted by output sector and cut into load-balanced segments.
+// This replaces the paper's Contract Book / hash scheduling by a plan-time sort.
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+#include <cstring>
+#include <map>
+#include <tuple>
+
+#include "su2_internal.h"
+#include "tile_config.h"
+
+namespace su2 {
+
+// ---------------------------------------------------------------------------------------
+// Wigner symbols (Appendix A, Eqs. (10)-(15)); doubled arguments.
+// ---------------------------------------------------------------------------------------
+static const long double* factorial_table() {
+  static long double tab[171];
+  static bool init = false;
+  if (!init) {
+    tab[0] = 1.0L;
+    for (int i = 1; i <= 170; ++i) tab[i] = tab[i - 1] * i;
+    init = true;
+  }
+  return tab;
+}
+static inline long double fact2(int two_x) { return factorial_table()[two_x / 2]; }  // (two_x/2)!
+static inline bool triad(int a, int b, int c) { return ((a + b + c) % 2 == 0) && std::abs(a - b) <= c && c <= a + b; }
+// g~(a,b,c)^2 of Eq. (15)
+static inline long double gsq(int a, int b, int c) {
+  return fact2(a + b - c) * fact2(a - b + c) * fact2(-a + b + c) / fact2(a + b + c + 2);
+}
+
+// Eq. (13)-(14).
+double wigner6j(int a, int b, int c, int d, int e, int f) {
+  if (!(triad(a, b, c) && triad(c, d, e) && triad(a, e, f) && triad(b, d, f))) return 0.0;
+  const int n2 = a + b + c, n3 = c + d + e, n4 = a + e + f, n5 = b + d + f;
+  const int n6 = a + b + d + e, n7 = a + c + d + f, n8 = b + c + e + f;
+  const int nmin = std::max(std::max(n2, n3), std::max(n4, n5));
+  const int nmax = std::min(n6, std::min(n7, n8));
+  long double s = 0.0L;
+  for (int n = nmin; n <= nmax; n += 2) {
+    long double term = fact2(n + 2) / (fact2(n - n2) * fact2(n - n3) * fact2(n - n4) * fact2(n - n5) *
+                                       fact2(n6 - n) * fact2(n7 - n) * fact2(n8 - n));
+    s += ((n / 2) % 2) ? -term : term;
+  }
+  return (double)(s * sqrtl(gsq(a, b, c) * gsq(c, d, e) * gsq(a, e, f) * gsq(b, d, f)));
+}
+
+// Eq. (10)-(12), PAPER.md:351-367 (x_min with absolute values: DESIGN.md reading G2).
+double wigner9j(int j1, int j2, int j, int k1, int k2, int k, int j1p, int j2p, int jp) {
+  if (!(triad(j1, j2, j) && triad(k1, k2, k) && triad(j1p, j2p, jp) && triad(j1, k1, j1p) && triad(j2, k2, j2p) &&
+        triad(j, k, jp)))
+    return 0.0;
+  const int xmin = std::max(std::abs(j1 - jp), std::max(std::abs(j2 - k), std::abs(k1 - j2p)));
+  const int xmax = std::min(j1 + jp, std::min(j2 + k, k1 + j2p));
+  double s = 0.0;
+  for (int x = xmin; x <= xmax; x += 2) {
+    const double sign = (x % 2) ? -1.0 : 1.0;  // (-1)^(2x)
+    s += sign * (x + 1) * wigner6j(j1, j2, j, k, jp, x) * wigner6j(k1, k2, k, j2, x, j2p) *
+         wigner6j(j1p, j2p, jp, x, j1, k1);
+  }
+  return s;
+}
+
+// SU(2) factor of Eq. (5)/(9) in the Wigner-Eckart convention of su2_heff.h:
+// <(j1 j2)j||[T^k1 x U^k2]^k||(j1' j2')j'> = c_hat * <j1||T||j1'> <j2||U||j2'>.
+double c_hat(int j1, int j2, int j, int k1, int k2, int k, int j1p, int j2p, int jp) {
+  const double w = wigner9j(j1, j2, j, k1, k2, k, j1p, j2p, jp);
+  if (w == 0.0) return 0.0;
+  return std::sqrt((double)(j1 + 1) * (j2 + 1) * (jp + 1) * (k + 1)) * w;
+}
+
+static const int SITE_N[3] = {0, 1, 2};
+static const int SITE_2S[3] = {0, 1, 0};
+
+}  // namespace su2
+
+using namespace su2;
+
+static su2_status validate(const su2_problem* p) {
+  if (!p || p->nsec_l <= 0 || p->nsec_r <= 0 || !p->sec_l || !p->sec_r || p->nsite <= 0 || !p->site || p->nterm < 0)
+    return SU2_ERR_INVALID_ARGUMENT;
+  if (p->nterm > 0 && !p->term) return SU2_ERR_INVALID_ARGUMENT;
+  if ((p->nfam_l > 0 && !p->fam_l) || (p->nfam_r > 0 && !p->fam_r) || p->nfam_l < 0 || p->nfam_r < 0)
+    return SU2_ERR_INVALID_ARGUMENT;
+  for (int side = 0; side < 2; ++side) {
+    const int ns = side ? p->nsec_r : p->nsec_l;
+    const su2_sector* sec = side ? p->sec_r : p->sec_l;
+    for (int i = 0; i < ns; ++i)
+      if (sec[i].dim <= 0 || sec[i].twoS < 0 || sec[i].N < 0) return SU2_ERR_INVALID_SECTOR;
+    const int nf = side ? p->nfam_r : p->nfam_l;
+    const su2_opfamily* fam = side ? p->fam_r : p->fam_l;
+    for (int f = 0; f < nf; ++f) {
+      if (fam[f].npos <= 0 || fam[f].nblk < 0 || fam[f].twoK < 0) return SU2_ERR_INVALID_ARGUMENT;
+      if (fam[f].nblk > 0 && (!fam[f].q_out || !fam[f].q_in || !fam[f].blk_off)) return SU2_ERR_INVALID_ARGUMENT;
+      for (int b = 0; b < fam[f].nblk; ++b) {
+        const int qo = fam[f].q_out[b], qi = fam[f].q_in[b];
+        if (qo < 0 || qo >= ns || qi < 0 || qi >= ns) return SU2_ERR_INVALID_SECTOR;
+        if (sec[qo].N != sec[qi].N + fam[f].dN) return SU2_ERR_INVALID_SECTOR;
+        if (!triad(sec[qi].twoS, fam[f].twoK, sec[qo].twoS)) return SU2_ERR_INVALID_RANK;
+        if (fam[f].blk_off[b] < 0) return SU2_ERR_INVALID_ARGUMENT;
+      }
+    }
+  }
+  for (int s = 0; s < p->nsite; ++s) {
+    for (int o = 0; o < 3; ++o)
+      for (int i = 0; i < 3; ++i) {
+        const double v = p->site[s].r[o][i];
+        if (!std::isfinite(v)) return SU2_ERR_NOT_FINITE;
+        if (v != 0.0 && (SITE_N[o] != SITE_N[i] + p->site[s].dN)) return SU2_ERR_INVALID_SECTOR;
+        if (v != 0.0 && !triad(SITE_2S[i], p->site[s].twoK, SITE_2S[o])) return SU2_ERR_INVALID_RANK;
+      }
+  }
+  for (int t = 0; t < p->nterm; ++t) {
+    const su2_term& tm = p->term[t];
+    if (tm.fam_l < -1 || tm.fam_l >= p->nfam_l || tm.fam_r < -1 || tm.fam_r >= p->nfam_r) return SU2_ERR_INVALID_ARGUMENT;
+    if (tm.op_B < 0 || tm.op_B >= p->nsite || tm.op_C < 0 || tm.op_C >= p->nsite) return SU2_ERR_INVALID_ARGUMENT;
+    if (tm.npos <= 0) return SU2_ERR_INVALID_ARGUMENT;
+    const int kl = tm.fam_l >= 0 ? p->fam_l[tm.fam_l].twoK : 0;
+    const int kr = tm.fam_r >= 0 ? p->fam_r[tm.fam_r].twoK : 0;
+    const int npl = tm.fam_l >= 0 ? p->fam_l[tm.fam_l].npos : 1;
+    const int npr = tm.fam_r >= 0 ? p->fam_r[tm.fam_r].npos : 1;
+    if ((npl != 1 && npl != tm.npos) || (npr != 1 && npr != tm.npos)) return SU2_ERR_INVALID_ARGUMENT;
+    if (tm.twoK_L != tm.twoK_R) return SU2_ERR_INVALID_RANK;  // K = 0: the Hamiltonian is a spin-zero object
+    if (!triad(kl, p->site[tm.op_B].twoK, tm.twoK_L) || !triad(p->site[tm.op_C].twoK, kr, tm.twoK_R))
+      return SU2_ERR_INVALID_RANK;
+    if (tm.alpha)
+      for (int i = 0; i < tm.npos; ++i)
+        if (!std::isfinite(tm.alpha[i])) return SU2_ERR_NOT_FINITE;
+  }
+  return SU2_OK;
+}
+
+extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int32_t flags, void* cuda_stream) {
+  if (!out) return SU2_ERR_INVALID_ARGUMENT;
+  *out = nullptr;
+  su2_status st = validate(p);
+  if (st != SU2_OK) return st;
+  const auto t_start = std::chrono::steady_clock::now();
+
+  su2_plan* plan = new su2_plan();
+  plan->host_only = (flags & SU2_PLAN_HOST_ONLY) != 0;
+  plan->n_tot = p->n_tot;
+  plan->twoS_tot = p->twoS_tot;
+  plan->sec_l.assign(p->sec_l, p->sec_l + p->nsec_l);
+  plan->sec_r.assign(p->sec_r, p->sec_r + p->nsec_r);
+  const auto& sl = plan->sec_l;
+  const auto& sr = plan->sec_r;
+
+  // ---- Psi sectors s = (il, sB, J1, sC, ir, J2) -----------------------------------------
+  std::map<std::tuple<int, int, int, int>, std::vector<int>> by_quad;  // (il,sB,sC,ir) -> sector ids
+  for (int il = 0; il < (int)sl.size(); ++il)
+    for (int sB = 0; sB < 3; ++sB)
+      for (int sC = 0; sC < 3; ++sC)
+        for (int ir = 0; ir < (int)sr.size(); ++ir) {
+          if (sl[il].N + SITE_N[sB] + SITE_N[sC] + sr[ir].N != p->n_tot) continue;
+          for (int j1 = std::abs(sl[il].twoS - SITE_2S[sB]); j1 <= sl[il].twoS + SITE_2S[sB]; j1 += 2)
+            for (int j2 = std::abs(sr[ir].twoS - SITE_2S[sC]); j2 <= sr[ir].twoS + SITE_2S[sC]; j2 += 2) {
+              if (!triad(j1, j2, p->twoS_tot)) continue;
+              PsiSector s{il, sB, j1, sC, ir, j2, plan->psi_len, sl[il].dim, sr[ir].dim};
+              by_quad[std::make_tuple(il, sB, sC, ir)].push_back((int)plan->psi.size());
+              plan->psi.push_back(s);
+              plan->psi_len += (int64_t)s.m * s.p;
+            }
+        }
+
+  // ---- task enumeration + coefficients (sector-task-table, sector-value-table) -----------
+  std::vector<double> alpha_host;                 // concatenated alpha arrays
+  std::vector<int64_t> alpha_off_of_term(p->nterm, -1);
+  for (int t = 0; t < p->nterm; ++t)
+    if (p->term[t].alpha) {
+      alpha_off_of_term[t] = (int64_t)alpha_host.size();
+      alpha_host.insert(alpha_host.end(), p->term[t].alpha, p->term[t].alpha + p->term[t].npos);
+    }
+  std::map<std::tuple<int, int, int, int, int, int, int, int, int>, double> chat_memo;
+  auto chat = [&](int a, int b, int c, int d, int e, int f, int g, int h, int i) {
+    auto key = std::make_tuple(a, b, c, d, e, f, g, h, i);
+    auto it = chat_memo.find(key);
+    if (it != chat_memo.end()) return it->second;
+    const double v = c_hat(a, b, c, d, e, f, g, h, i);
+    chat_memo[key] = v;
+    return v;
+  };
+
+  struct Trans { int q_in, q_out, blk; double phase; };   // applied operator: ket sector -> bra sector
+  auto transitions = [&](const su2_opfamily* fam, int adj, const std::vector<su2_sector>& sec) {
+    std::vector<Trans> tr;
+    if (!fam) {
+      for (int i = 0; i < (int)sec.size(); ++i) tr.push_back({i, i, -1, 1.0});
+      return tr;
+    }
+    for (int b = 0; b < fam->nblk; ++b) {
+      const int qo = fam->q_out[b], qi = fam->q_in[b];
+      if (!adj) {
+        tr.push_back({qi, qo, b, 1.0});
+      } else {
+        // adjoint tensor: <j'||T~||j> = (-1)^(j-j'+k) sqrt((2j+1)/(2j'+1)) <j||T||j'>^T, T: j' -> j stored
+        const int j = sec[qo].twoS, jp = sec[qi].twoS;
+        const int e = (j - jp + fam->twoK) / 2;
+        const double ph = ((e % 2) ? -1.0 : 1.0) * std::sqrt((double)(j + 1) / (double)(jp + 1));
+        tr.push_back({qo, qi, b, ph});
+      }
+    }
+    return tr;
+  };
+
+  for (int t = 0; t < p->nterm; ++t) {
+    const su2_term& tm = p->term[t];
+    const su2_opfamily* fl = tm.fam_l >= 0 ? &p->fam_l[tm.fam_l] : nullptr;
+    const su2_opfamily* fr = tm.fam_r >= 0 ? &p->fam_r[tm.fam_r] : nullptr;
+    const su2_siteop& oB = p->site[tm.op_B];
+    const su2_siteop& oC = p->site[tm.op_C];
+    const int kl = fl ? fl->twoK : 0, kr = fr ? fr->twoK : 0, kB = oB.twoK, kC = oC.twoK;
+    const int k1 = tm.twoK_L, k2 = tm.twoK_R;
+    const int pB = oB.dN & 1, pC = oC.dN & 1, pr = fr ? (fr->dN & 1) : 0;
+    const auto ltr = transitions(fl, tm.adj_l, sl);
+    const auto rtr = transitions(fr, tm.adj_r, sr);
+    for (const Trans& lt : ltr)
+      for (int sBi = 0; sBi < 3; ++sBi) {
+        const int sBo = sBi + oB.dN;
+        if (sBo < 0 || sBo > 2 || oB.r[sBo][sBi] == 0.0) continue;
+        for (int sCi = 0; sCi < 3; ++sCi) {
+          const int sCo = sCi + oC.dN;
+          if (sCo < 0 || sCo > 2 || oC.r[sCo][sCi] == 0.0) continue;
+          for (const Trans& rt : rtr) {
+            auto in_it = by_quad.find(std::make_tuple(lt.q_in, sBi, sCi, rt.q_in));
+            if (in_it == by_quad.end()) continue;
+            auto out_it = by_quad.find(std::make_tuple(lt.q_out, sBo, sCo, rt.q_out));
+            if (out_it == by_quad.end()) continue;
+            // fermion sign with the KET particle numbers (operators ordered O_l O_B O_C O_r)
+            const int nl = sl[lt.q_in].N, nB = SITE_N[sBi], nC = SITE_N[sCi];
+            const int sexp = pB * nl + pC * (nl + nB) + pr * (nl + nB + nC);
+            const double base = ((sexp % 2) ? -1.0 : 1.0) * oB.r[sBo][sBi] * oC.r[sCo][sCi] * lt.phase * rt.phase;
+            const int Sl = sl[lt.q_out].twoS, Slp = sl[lt.q_in].twoS;
+            const int Sr = sr[rt.q_out].twoS, Srp = sr[rt.q_in].twoS;
+            for (int si : in_it->second)
+              for (int so : out_it->second) {
+                const PsiSector& a = plan->psi[so];
+                const PsiSector& b = plan->psi[si];
+                const double cl = chat(Sl, SITE_2S[sBo], a.twoJ1, kl, kB, k1, Slp, SITE_2S[sBi], b.twoJ1);
+                if (cl == 0.0) continue;
+                const double cr = chat(SITE_2S[sCo], Sr, a.twoJ2, kC, kr, k2, SITE_2S[sCi], Srp, b.twoJ2);
+                if (cr == 0.0) continue;
+                const double ct = chat(a.twoJ1, a.twoJ2, p->twoS_tot, k1, k2, 0, b.twoJ1, b.twoJ2, p->twoS_tot);
+                const double coef = base * cl * cr * ct;
+                if (coef == 0.0 || std::fabs(coef) < 1e-300) continue;
+                HostTask ht;
+                ht.out_sec = so; ht.in_sec = si;
+                ht.fam_l = tm.fam_l; ht.blk_l = lt.blk; ht.adj_l = fl ? tm.adj_l : 0;
+                ht.fam_r = tm.fam_r; ht.blk_r = rt.blk; ht.adj_r = fr ? tm.adj_r : 0;
+                ht.term = t; ht.coef = coef;
+                ht.m = a.m; ht.k = b.m; ht.n = b.p; ht.p = a.p; ht.npos = tm.npos;
+                plan->tasks.push_back(ht);
+              }
+          }
+        }
+      }
+  }
+  // plan order: by output sector, then input sector (E reuse), then row
+  std::stable_sort(plan->tasks.begin(), plan->tasks.end(), [](const HostTask& x, const HostTask& y) {
+    return std::tie(x.out_sec, x.in_sec, x.term, x.blk_l, x.blk_r) < std::tie(y.out_sec, y.in_sec, y.term, y.blk_l, y.blk_r);
+  });
+
+  // ---- device task images ---------------------------------------------------------------
+  const int64_t ntask = (int64_t)plan->tasks.size();
+  plan->h_tasks.resize(ntask);
+  std::vector<int64_t> alpha_off_of_task(ntask, -1), identA(ntask, -1), identD(ntask, -1);
+  // identity blocks: one (dim x dim) identity per distinct dim, concatenated
+  std::map<int, int64_t> ident_off;
+  std::vector<double> ident_host;
+  auto ident_for = [&](int dim) {
+    auto it = ident_off.find(dim);
+    if (it != ident_off.end()) return it->second;
+    const int64_t off = (int64_t)ident_host.size();
+    ident_host.resize(off + (int64_t)dim * dim, 0.0);
+    for (int i = 0; i < dim; ++i) ident_host[off + (int64_t)i * dim + i] = 1.0;
+    ident_off[dim] = off;
+    return off;
+  };
+  double cc = 0.0, opbytes = 0.0;
+  int64_t ntp = 0;
+  for (int64_t i = 0; i < ntask; ++i) {
+    const HostTask& ht = plan->tasks[i];
+    DevTask& d = plan->h_tasks[i];
+    std::memset(&d, 0, sizeof(d));
+    d.coef = ht.coef;
+    d.e_off = plan->psi[ht.in_sec].off;
+    d.m = ht.m; d.k = ht.k; d.n = ht.n; d.p = ht.p; d.npos = ht.npos;
+    d.flags = (ht.adj_l ? TASK_TRANS_A : 0u) | (ht.adj_r ? TASK_TRANS_D : 0u);
+    if (ht.fam_l >= 0) {
+      const su2_opfamily& f = p->fam_l[ht.fam_l];
+      d.A = f.data ? f.data + f.blk_off[ht.blk_l] : nullptr;
+      d.strideA = f.npos > 1 ? ht.m * ht.k : 0;
+    } else {
+      identA[i] = ident_for(ht.m);
+      d.strideA = 0;
+    }
+    if (ht.fam_r >= 0) {
+      const su2_opfamily& f = p->fam_r[ht.fam_r];
+      d.D = f.data ? f.data + f.blk_off[ht.blk_r] : nullptr;
+      d.strideD = f.npos > 1 ? ht.p * ht.n : 0;
+    } else {
+      identD[i] = ident_for(ht.p);
+      d.strideD = 0;
+    }
+    alpha_off_of_task[i] = alpha_off_of_term[ht.term];
+    const double m = ht.m, k = ht.k, n = ht.n, pp = ht.p;
+    cc += ht.npos * std::min(2 * m * k * n + 2 * m * n * pp, 2 * k * n * pp + 2 * m * k * pp);
+    opbytes += ht.npos * 8.0 * (m * k + n * pp);
+    ntp += ht.npos;
+  }
+
+  // ---- segments: deterministic segmented reduction (no atomics) ---------------------------
+  // Per output sector the task list is cut into nseg segments of equal work; each (segment, tile)
+  // is one CTA work item.  nseg == 1 writes F directly, otherwise partial copies are summed in
+  // index order by the reduce pass.
+  const int nsec = (int)plan->psi.size();
+  std::vector<int64_t> first_task(nsec + 1, 0);
+  for (const HostTask& ht : plan->tasks) first_task[ht.out_sec + 1]++;
+  for (int s = 0; s < nsec; ++s) first_task[s + 1] += first_task[s];
+  auto pos_cost = [&](const HostTask& ht) {  // flops of one position for ONE output tile (recompute of T per tile)
+    const double tm = std::min<double>(TILE_M, ht.m), tp = std::min<double>(TILE_P, ht.p);
+    return 2.0 * tm * ht.k * ht.n + 2.0 * tm * ht.n * tp;
+  };
+  double total_item_work = 0.0, executed = 0.0;
+  std::vector<double> sec_work(nsec, 0.0);
+  for (int s = 0; s < nsec; ++s) {
+    const int tiles = ((plan->psi[s].m + TILE_M - 1) / TILE_M) * ((plan->psi[s].p + TILE_P - 1) / TILE_P);
+    for (int64_t i = first_task[s]; i < first_task[s + 1]; ++i) sec_work[s] += pos_cost(plan->tasks[i]) * plan->tasks[i].npos;
+    total_item_work += sec_work[s] * tiles;
+  }
+  executed = total_item_work;
+  const double target = (flags & SU2_PLAN_FORCE_SPLIT) ? 2.0e4 : std::max(total_item_work / (148.0 * 24.0), 4.0e6);
+  plan->partial_elems = 0;
+  std::vector<double> work_cost;   // for LPT ordering
+  for (int s = 0; s < nsec; ++s) {
+    const PsiSector& ps = plan->psi[s];
+    const int64_t sz = (int64_t)ps.m * ps.p;
+    const int64_t t0 = first_task[s], t1 = first_task[s + 1];
+    DevReduce red{};
+    red.f_off = ps.off; red.size = sz; red.part_off = 0; red.nseg = 0;
+    if (t1 == t0) {
+      plan->h_reduce.push_back(red);
+      continue;
+    }
+    int nseg = (int)std::min<double>(64.0, std::max(1.0, std::ceil(sec_work[s] / target)));
+    std::vector<std::pair<int32_t, int32_t>> seg_units;   // unit ranges per segment
+    {
+      double acc = 0.0;
+      int seg = 0;
+      int32_t ustart = (int32_t)plan->h_units.size();
+      for (int64_t i = t0; i < t1; ++i) {
+        const HostTask& ht = plan->tasks[i];
+        const double c = pos_cost(ht);
+        int pos = 0;
+        while (pos < ht.npos) {
+          int take = ht.npos - pos;
+          if (seg < nseg - 1) {
+            const double room = sec_work[s] * (seg + 1) / nseg - acc;
+            const int fit = (int)std::floor(room / c + 1e-9);
+            if (fit <= 0) {   // this segment is full: close it
+              seg_units.push_back({ustart, (int32_t)plan->h_units.size()});
+              ustart = (int32_t)plan->h_units.size();
+              ++seg;
+              continue;
+            }
+            take = std::min(take, fit);
+          }
+          plan->h_units.push_back(DevUnit{(int32_t)i, pos, pos + take, 0});
+          pos += take;
+          acc += c * take;
+        }
+      }
+      seg_units.push_back({ustart, (int32_t)plan->h_units.size()});
+    }
+    // drop empty segments
+    std::vector<std::pair<int32_t, int32_t>> segs;
+    for (auto& su : seg_units)
+      if (su.second > su.first) segs.push_back(su);
+    nseg = (int)segs.size();
+    red.nseg = nseg > 1 ? nseg : 1;
+    if (nseg > 1) {
+      red.part_off = plan->partial_elems;
+      plan->partial_elems += (int64_t)nseg * sz;
+    }
+    plan->h_reduce.push_back(red);
+    for (int g = 0; g < nseg; ++g) {
+      double w = 0.0;
+      for (int32_t u = segs[g].first; u < segs[g].second; ++u)
+        w += pos_cost(plan->tasks[plan->h_units[u].task]) * (plan->h_units[u].pos1 - plan->h_units[u].pos0);
+      for (int r0 = 0; r0 < ps.m; r0 += TILE_M)
+        for (int c0 = 0; c0 < ps.p; c0 += TILE_P) {
+          DevWork wk{};
+          wk.unit0 = segs[g].first; wk.unit1 = segs[g].second;
+          wk.row0 = r0; wk.col0 = c0; wk.m = ps.m; wk.p = ps.p;
+          wk.to_partial = nseg > 1 ? 1 : 0;
+          wk.dst_off = nseg > 1 ? red.part_off + (int64_t)g * sz : ps.off;
+          plan->h_work.push_back(wk);
+          work_cost.push_back(w);
+        }
+    }
+    plan->info.nsegments += nseg;
+  }
+  // longest-processing-time-first order for the persistent CTAs' queue
+  {
+    std::vector<int64_t> order(plan->h_work.size());
+    for (size_t i = 0; i < order.size(); ++i) order[i] = (int64_t)i;
+    std::stable_sort(order.begin(), order.end(), [&](int64_t a, int64_t b) { return work_cost[a] > work_cost[b]; });
+    std::vector<DevWork> sorted(order.size());
+    for (size_t i = 0; i < order.size(); ++i) sorted[i] = plan->h_work[order[i]];
+    plan->h_work.swap(sorted);
+  }
+
+  // ---- diagonal tasks (s == s') for the preconditioner -----------------------------------
+  plan->h_diag_begin.assign(nsec + 1, 0);
+  for (int s = 0; s < nsec; ++s) {
+    plan->h_diag_begin[s] = (int32_t)plan->h_diag.size();
+    for (int64_t i = first_task[s]; i < first_task[s + 1]; ++i) {
+      const HostTask& ht = plan->tasks[i];
+      if (ht.in_sec != ht.out_sec) continue;
+      DevDiagTask d{};
+      d.A = plan->h_tasks[i].A; d.D = plan->h_tasks[i].D; d.alpha = nullptr;
+      d.coef = ht.coef; d.f_off = plan->psi[s].off; d.m = ht.m; d.p = ht.p;
+      d.strideA = plan->h_tasks[i].strideA; d.strideD = plan->h_tasks[i].strideD; d.npos = ht.npos;
+      d.pad = (int32_t)i;   // index of the full task: upload_plan copies its patched pointers
+      plan->h_diag.push_back(d);
+    }
+  }
+  plan->h_diag_begin[nsec] = (int32_t)plan->h_diag.size();
+
+  plan->info.psi_len = plan->psi_len;
+  plan->info.ntasks = ntask;
+  plan->info.ntask_positions = ntp;
+  plan->info.cc_flops = cc;
+  plan->info.executed_flops = executed;
+  plan->info.operator_bytes = opbytes;
+  plan->info.workspace_bytes = plan->partial_elems * 8 + 256;
+  plan->info.npsi_sec = nsec;
+  plan->info.nwork_items = (int64_t)plan->h_work.size();
+
+  if (!plan->host_only) {
+    st = upload_plan(plan, alpha_host, ident_host, alpha_off_of_task, identA, identD, cuda_stream);
+    if (st != SU2_OK) {
+      free_plan_device(plan);
+      delete plan;
+      return st;
+    }
+  }
+  plan->info.plan_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_start).count();
+  *out = plan;
+  return SU2_OK;
+}
+
+extern "C" su2_status su2_plan_destroy(su2_plan* plan) {
+  if (!plan) return SU2_ERR_INVALID_ARGUMENT;
+  free_plan_device(plan);
+  delete plan;
+  return SU2_OK;
+}
+
+extern "C" su2_status su2_plan_info(const su2_plan* plan, su2_plan_info_t* info) {
+  if (!plan || !info) return SU2_ERR_INVALID_ARGUMENT;
+  *info = plan->info;
+  return SU2_OK;
+}
+
+extern "C" su2_status su2_plan_psi_layout(const su2_plan* plan, int32_t* labels, int64_t* offsets) {
+  if (!plan || !labels || !offsets) return SU2_ERR_INVALID_ARGUMENT;
+  for (size_t i = 0; i < plan->psi.size(); ++i) {
+    const PsiSector& s = plan->psi[i];
+    int32_t* l = labels + 6 * i;
+    l[0] = s.il; l[1] = s.sB; l[2] = s.twoJ1; l[3] = s.sC; l[4] = s.ir; l[5] = s.twoJ2;
+    offsets[i] = s.off;
+  }
+  offsets[plan->psi.size()] = plan->psi_len;
+  return SU2_OK;
+}
+
+extern "C" su2_status su2_plan_export_tasks(const su2_plan* plan, int32_t* out_sec, int32_t* in_sec, int32_t* fam_l,
+                                            int32_t* blk_l, int32_t* adj_l, int32_t* fam_r, int32_t* blk_r,
+                                            int32_t* adj_r, int32_t* term, double* coef) {
+  if (!plan || !out_sec || !in_sec || !fam_l || !blk_l || !adj_l || !fam_r || !blk_r || !adj_r || !term || !coef)
+    return SU2_ERR_INVALID_ARGUMENT;
+  for (size_t i = 0; i < plan->tasks.size(); ++i) {
+    const HostTask& t = plan->tasks[i];
+    out_sec[i] = t.out_sec; in_sec[i] = t.in_sec;
+    fam_l[i] = t.fam_l; blk_l[i] = t.blk_l; adj_l[i] = t.adj_l;
+    fam_r[i] = t.fam_r; blk_r[i] = t.blk_r; adj_r[i] = t.adj_r;
+    term[i] = t.term; coef[i] = t.coef;
+  }
+  return SU2_OK;
+}
+
+extern "C" const char* su2_status_string(su2_status st) {
+  switch (st) {
+    case SU2_OK: return "ok";
+    case SU2_ERR_INVALID_ARGUMENT: return "invalid argument";
+    case SU2_ERR_INVALID_SECTOR: return "invalid sector reference or particle-number selection rule violated";
+    case SU2_ERR_INVALID_RANK: return "operator ranks cannot be coupled (triangle rule / k1 != k2)";
+    case SU2_ERR_NOT_FINITE: return "non-finite alpha or site element";
+    case SU2_ERR_CUDA: return "CUDA runtime error";
+    case SU2_ERR_NO_DEVICE_PLAN: return "plan has no device tables (SU2_PLAN_HOST_ONLY)";
+    case SU2_ERR_WORKSPACE: return "workspace missing";
+    default: return "unknown status";
+  }
+}

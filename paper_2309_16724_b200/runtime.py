@@ -1,0 +1,103 @@
+"""PyTorch-side plumbing around the C ABI: device memory for operator families, Psi and the
+workspace, and the CUDA stream.  No arithmetic of the hot path happens here: apply(), diag()
+and the Davidson steps run inside libsu2heff.so; a missing extension or GPU raises."""
+import numpy as np
+import torch
+
+from .binding import Davidson, Plan, Su2Error, family_elems
+
+
+def _require_cuda():
+    if not torch.cuda.is_available():
+        raise Su2Error("no CUDA device: the product path has no CPU fallback")
+
+
+class HeffOperator:
+    """H_eff of one superblock problem, resident on one GPU.
+
+    problem: gen.problem.Problem-like plain data.  Family data is taken from
+    problem.fam_*[i].data (list of numpy blocks [npos, m, k]) or, when `device_fill` is given,
+    generated directly on the device by device_fill(side, index, tensor) (143 GB-class
+    workloads cannot be staged through host memory)."""
+
+    def __init__(self, problem, device="cuda:0", device_fill=None, force_split=False):
+        _require_cuda()
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.problem = problem
+        self.family_tensors = {}
+        ptrs = {}
+        for side, fams, secs in (("l", problem.fam_l, problem.sec_l), ("r", problem.fam_r, problem.sec_r)):
+            for i, f in enumerate(fams):
+                n = family_elems(f, secs)
+                if device_fill is not None:
+                    t = torch.empty(max(n, 1), dtype=torch.float64, device=self.device)
+                    device_fill(side, i, t)
+                else:
+                    host = np.concatenate([np.ascontiguousarray(b, dtype=np.float64).ravel() for b in f.data]) \
+                        if len(f.data) else np.zeros(1)
+                    assert host.size == max(n, 1) or n == host.size
+                    t = torch.from_numpy(host).to(self.device)
+                self.family_tensors[(side, i)] = t
+                ptrs[(side, i)] = t.data_ptr()
+        self.stream = torch.cuda.current_stream(self.device)
+        self.plan = Plan(problem, family_ptrs=ptrs, stream=self.stream.cuda_stream, force_split=force_split)
+        self.psi_len = self.plan.psi_len
+        # workspace: partial tiles + staging for the host entry point
+        self.workspace = torch.empty(self.plan.workspace_bytes + 512 + 16 * self.psi_len, dtype=torch.uint8,
+                                     device=self.device)
+        self.operator_bytes_resident = sum(t.numel() * 8 for t in self.family_tensors.values())
+
+    @property
+    def info(self):
+        return self.plan.info
+
+    def new_vector(self):
+        return torch.empty(self.psi_len, dtype=torch.float64, device=self.device)
+
+    def apply(self, psi, out=None):
+        """out = H_eff psi (device tensors, float64, contiguous)."""
+        assert psi.dtype == torch.float64 and psi.is_cuda and psi.is_contiguous() and psi.numel() == self.psi_len
+        if out is None:
+            out = self.new_vector()
+        self.plan.heff_apply(psi.data_ptr(), out.data_ptr(), self.workspace.data_ptr(),
+                             torch.cuda.current_stream(self.device).cuda_stream)
+        return out
+
+    def apply_host(self, psi_host, out_host):
+        """End-to-end entry: pinned host tensors in and out (copies inside the C call)."""
+        assert psi_host.dtype == torch.float64 and not psi_host.is_cuda and psi_host.numel() == self.psi_len
+        self.plan.heff_apply_host(psi_host.data_ptr(), out_host.data_ptr(), self.workspace.data_ptr(),
+                                  torch.cuda.current_stream(self.device).cuda_stream)
+        return out_host
+
+    def diag(self):
+        d = self.new_vector()
+        self.plan.heff_diag(d.data_ptr(), torch.cuda.current_stream(self.device).cuda_stream)
+        return d
+
+    def davidson(self, x0, max_subspace=20):
+        return DavidsonSolver(self, x0, max_subspace)
+
+
+class DavidsonSolver:
+    def __init__(self, op, x0, max_subspace=20):
+        self.op = op
+        nbytes = Davidson.workspace_bytes(op.plan, max_subspace)
+        self.ws = torch.empty(nbytes, dtype=torch.uint8, device=op.device)
+        self.stream = torch.cuda.current_stream(op.device).cuda_stream
+        self.dav = Davidson(op.plan, max_subspace, x0.data_ptr(), self.ws.data_ptr(), self.stream)
+        self.history = []
+
+    def step(self):
+        theta, res = self.dav.step(self.op.workspace.data_ptr(), self.stream)
+        self.history.append((theta, res))
+        return theta, res
+
+    def ritz_vector(self):
+        x = self.op.new_vector()
+        self.dav.ritz_vector(x.data_ptr(), self.stream)
+        return x
+
+    def close(self):
+        self.dav.close()

@@ -1,0 +1,168 @@
+"""GPU parity tests (run on the B200 box): the CUDA path through the C ABI against the oracle,
+element by element, on seeded inputs.  Tolerance (north_star): max |F_gpu - F_oracle| / max |F_oracle|
+<= 1e-10 in FP64."""
+import numpy as np
+import pytest
+
+from gen.workloads import config_problem, integrals, random_psi, synthetic_problem
+from helpers import oracle_flat
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-10
+
+
+def _torch():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+def _operator(prob, **kw):
+    from paper_2309_16724_b200.runtime import HeffOperator
+    return HeffOperator(prob, **kw)
+
+
+def _cfg1(use_adjoints=True):
+    from oracle.abinitio_table import build_problem
+    t, v = integrals(6, seed=0, xi=2.0)
+    return build_problem(t, v, 2, 6, 0, use_adjoints=use_adjoints)
+
+
+def _rel(a, b):
+    return np.abs(a - b).max() / np.abs(b).max()
+
+
+@pytest.mark.parametrize("force_split", [False, True])
+def test_cfg1_exact_hamiltonian_parity(force_split):
+    torch = _torch()
+    prob = _cfg1()
+    op = _operator(prob, force_split=force_split)
+    assert op.psi_len == 175 and len(op.plan.labels) == 53
+    x = random_psi(op.psi_len, seed=0)
+    f_gpu = op.apply(torch.from_numpy(x).cuda()).cpu().numpy()
+    f_ref = oracle_flat(prob, op.plan, x)
+    assert _rel(f_gpu, f_ref) <= TOL
+
+
+@pytest.mark.parametrize("name,force_split", [("mini", False), ("mini", True), ("midi", False), ("midi", True)])
+def test_synthetic_parity_full_oracle(name, force_split):
+    """Random-operator workloads with ragged block sizes (1..17), adjoint rows, alpha per position."""
+    torch = _torch()
+    prob = config_problem(name)
+    op = _operator(prob, force_split=force_split)
+    if force_split:
+        assert op.info["nsegments"] > op.info["npsi_sec"]
+    x = random_psi(op.psi_len, seed=1)
+    f_gpu = op.apply(torch.from_numpy(x).cuda()).cpu().numpy()
+    f_ref = oracle_flat(prob, op.plan, x)
+    assert _rel(f_gpu, f_ref) <= TOL
+
+
+def test_several_tiles_and_ragged_tail():
+    """Blocks larger than one 64x64 tile with ragged tails (L=10, D=300: dims up to ~90)."""
+    torch = _torch()
+    prob = synthetic_problem(10, 10, 0, 300, seed=3)
+    dims = [s.dim for s in prob.sec_l]
+    assert max(dims) > 64 and any(d % 8 for d in dims)
+    op = _operator(prob)
+    x = random_psi(op.psi_len, seed=2)
+    f_gpu = op.apply(torch.from_numpy(x).cuda()).cpu().numpy()
+    f_ref = oracle_flat(prob, op.plan, x)
+    assert _rel(f_gpu, f_ref) <= TOL
+
+
+def test_bitwise_reproducible_and_host_entry():
+    torch = _torch()
+    prob = config_problem("midi")
+    op = _operator(prob, force_split=True)
+    x = torch.from_numpy(random_psi(op.psi_len, seed=4)).cuda()
+    f1 = op.apply(x).clone()
+    f2 = op.apply(x).clone()
+    assert torch.equal(f1, f2)
+    xh = x.cpu().pin_memory()
+    fh = torch.empty_like(xh).pin_memory()
+    op.apply_host(xh, fh)
+    assert torch.equal(fh, f1.cpu())
+
+
+def test_empty_operator_table_gives_zero():
+    torch = _torch()
+    prob = config_problem("mini")
+    prob.term = []
+    op = _operator(prob)
+    x = torch.from_numpy(random_psi(op.psi_len, seed=5)).cuda()
+    out = torch.full_like(x, 7.0)
+    op.apply(x, out)
+    assert float(out.abs().max()) == 0.0
+
+
+def test_diag_matches_oracle_matrix_cfg1():
+    from oracle.heff_dense import heff_matrix, psi_sectors
+    torch = _torch()
+    prob = _cfg1()
+    op = _operator(prob)
+    h = heff_matrix(prob)
+    labels = psi_sectors(prob)
+    offs = np.concatenate([[0], np.cumsum([prob.sec_l[s[0]].dim * prob.sec_r[s[4]].dim for s in labels])])
+    ref = np.zeros(op.psi_len)
+    for i, lab in enumerate(op.plan.labels):
+        j = labels.index(lab)
+        ref[op.plan.offsets[i]:op.plan.offsets[i + 1]] = np.diag(h)[offs[j]:offs[j + 1]]
+    d = op.diag().cpu().numpy()
+    assert np.abs(d - ref).max() <= 1e-12 * np.abs(ref).max()
+
+
+def test_davidson_converges_to_fci_energy_cfg1():
+    """End to end: su2_davidson_step on the exact cfg1 Hamiltonian reaches the lowest (N=6,S=0)
+    eigenvalue of the Jordan-Wigner Hamiltonian (oracle/fock.py)."""
+    from oracle.fock import FockSpace
+    from test_oracle_fock import sector_spectrum
+    torch = _torch()
+    t, v = integrals(6, seed=0, xi=2.0)
+    fs = FockSpace(6)
+    e0 = sector_spectrum(fs, fs.hamiltonian(t, v), 6, 0)[0]
+    op = _operator(_cfg1())
+    x0 = torch.from_numpy(random_psi(op.psi_len, seed=0)).cuda()
+    solver = op.davidson(x0, max_subspace=12)
+    theta = res = None
+    for it in range(60):
+        theta, res = solver.step()
+        if res < 1e-9:
+            break
+    assert res < 1e-9, (it, theta, res)
+    assert abs(theta - e0) < 1e-10
+    xr = solver.ritz_vector()
+    hx = op.apply(xr)
+    assert abs(float(torch.dot(xr, hx)) - e0) < 1e-10
+    assert abs(float(torch.dot(xr, xr)) - 1.0) < 1e-12
+    assert len(solver.history) > 12          # went through at least one restart
+    solver.close()
+
+
+def test_gpu_result_is_hermitian_and_linear_midi():
+    torch = _torch()
+    prob = config_problem("midi")
+    op = _operator(prob)
+    x = torch.from_numpy(random_psi(op.psi_len, seed=6)).cuda()
+    y = torch.from_numpy(random_psi(op.psi_len, seed=7)).cuda()
+    hx, hy = op.apply(x).clone(), op.apply(y).clone()
+    a, b = float(torch.dot(y, hx)), float(torch.dot(x, hy))
+    assert abs(a - b) <= 1e-11 * max(abs(a), float(hx.norm()))
+    hz = op.apply(2.0 * x - 0.5 * y)
+    assert float((hz - (2.0 * hx - 0.5 * hy)).abs().max()) <= 1e-12 * float(hx.abs().max())
+
+
+@pytest.mark.parametrize("m,k,n,p,batch", [(8, 8, 8, 8, 1000), (16, 32, 8, 24, 37), (64, 64, 64, 64, 9),
+                                           (70, 33, 45, 129, 5), (128, 128, 128, 128, 3), (1, 1, 1, 1, 4)])
+def test_gemm_pair_batched(m, k, n, p, batch):
+    """BASELINE.json configs[4]: C += alpha A X B^T, checked against numpy in FP64."""
+    torch = _torch()
+    from paper_2309_16724_b200 import gemm_pair_batched
+    rng = np.random.default_rng(m * 1000 + p)
+    A, X = rng.normal(size=(batch, m, k)), rng.normal(size=(batch, k, n))
+    B, C0 = rng.normal(size=(batch, p, n)), rng.normal(size=(batch, m, p))
+    dA, dX, dB, dC = (torch.from_numpy(a).cuda() for a in (A, X, B, C0))
+    gemm_pair_batched(m, k, n, p, batch, 0.5, dA.data_ptr(), dX.data_ptr(), dB.data_ptr(), dC.data_ptr(),
+                      torch.cuda.current_stream().cuda_stream)
+    ref = C0 + 0.5 * np.einsum("bmk,bkn,bpn->bmp", A, X, B)
+    assert _rel(dC.cpu().numpy(), ref) <= 1e-12

@@ -1,0 +1,90 @@
+"""CPU tests of the host logic behind the C ABI: the library loads without a GPU and exports
+every symbol include/su2_heff.h declares; the planner's task table (enumeration, recoupling
+coefficients, fermion signs, adjoint phases), walked on the host with numpy, equals the oracle."""
+import os
+import re
+
+import numpy as np
+import pytest
+
+from gen.workloads import config_problem, integrals, random_psi
+from helpers import host_walk, oracle_flat
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2309_16724_b200.build import build
+    build()
+    from paper_2309_16724_b200 import load
+    return load()
+
+
+def test_library_exports_every_declared_symbol(lib):
+    header = open(os.path.join(ROOT, "include", "su2_heff.h")).read()
+    declared = set(re.findall(r"\b(su2_[a-z0-9_]+)\s*\(", header))
+    assert {"su2_plan_create", "su2_heff_apply", "su2_davidson_step"} <= declared
+    for name in declared:
+        assert hasattr(lib, name), name
+    from paper_2309_16724_b200.binding import EXPORTS
+    assert set(EXPORTS) == declared
+    assert lib.su2_status_string(0) == b"ok"
+
+
+def _cfg1(use_adjoints):
+    from oracle.abinitio_table import build_problem
+    t, v = integrals(6, seed=0, xi=2.0)
+    return build_problem(t, v, 2, 6, 0, use_adjoints=use_adjoints)
+
+
+@pytest.mark.parametrize("which", ["cfg1", "cfg1-adjoint", "mini", "mini-split"])
+def test_task_table_equals_oracle(lib, which):
+    from paper_2309_16724_b200 import Plan
+    prob = _cfg1(which.endswith("adjoint")) if which.startswith("cfg1") else config_problem("mini")
+    plan = Plan(prob, host_only=True, force_split=which.endswith("split"))
+    if which.startswith("cfg1"):
+        assert plan.psi_len == 175 and plan.info["npsi_sec"] == 53
+    x = random_psi(plan.psi_len, seed=0)
+    ref = oracle_flat(prob, plan, x)
+    got = host_walk(prob, plan, x)
+    assert np.abs(got - ref).max() <= 1e-13 * np.abs(ref).max()
+    assert plan.info["cc_flops"] > 0 and plan.info["ntask_positions"] >= plan.info["ntasks"]
+
+
+def test_plan_statistics_of_the_baseline_configs(lib):
+    """Shapes of BASELINE.json configs[1..3] under the windowed sector rule (G12)."""
+    from paper_2309_16724_b200 import Plan
+    expect = {"cfg2": (138, 85126, 6, 46), "cfg3": (138, 1208228, 30, 131), "cfg4": (138, 19728348, 69, 547)}
+    for name, (nsec, nelem, dmin, dmax) in expect.items():
+        prob = config_problem(name, fill=False)
+        dims = [s.dim for s in prob.sec_l]
+        assert (min(dims), max(dims)) == (dmin, dmax)
+        plan = Plan(prob, host_only=True)
+        assert plan.info["npsi_sec"] == nsec and plan.psi_len == nelem
+        assert plan.info["nwork_items"] > 0
+
+
+def test_invalid_inputs_are_rejected(lib):
+    from paper_2309_16724_b200 import Plan, Su2Error
+    prob = config_problem("mini")
+    prob.term[8].twoK_R = prob.term[8].twoK_L + 2           # k1 != k2
+    with pytest.raises(Su2Error):
+        Plan(prob, host_only=True)
+    prob = config_problem("mini")
+    prob.fam_l[2].q_out[0] = 99                             # sector out of range
+    with pytest.raises(Su2Error):
+        Plan(prob, host_only=True)
+    prob = config_problem("mini")
+    a = np.array(prob.term[10].alpha)
+    a[0] = np.nan
+    prob.term[10].alpha = a
+    with pytest.raises(Su2Error):
+        Plan(prob, host_only=True)
+
+
+def test_device_entry_points_fail_loudly_without_device_plan(lib):
+    from paper_2309_16724_b200 import Plan, Su2Error
+    plan = Plan(config_problem("mini"), host_only=True)
+    with pytest.raises(Su2Error):
+        plan.heff_apply(1, 2, 0)
