@@ -59,9 +59,9 @@ def test_synthetic_parity_full_oracle(name, force_split):
 
 
 def test_several_tiles_and_ragged_tail():
-    """Blocks larger than one 64x64 tile with ragged tails (L=10, D=300: dims up to ~90)."""
+    """Blocks larger than one tile with ragged tails (L=16, D=500: dims 6..109)."""
     torch = _torch()
-    prob = synthetic_problem(10, 10, 0, 300, seed=3)
+    prob = synthetic_problem(16, 16, 0, 500, seed=3)
     dims = [s.dim for s in prob.sec_l]
     assert max(dims) > 64 and any(d % 8 for d in dims)
     op = _operator(prob)
