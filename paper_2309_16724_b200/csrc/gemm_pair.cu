@@ -1,9 +1,150 @@
 // Strided-batched FP64 GEMM-pair microbenchmark entry (BASELINE.json configs[4]):
 //   C_b += alpha * A_b X_b B_b^T, one independent item per batch index.
-// Implemented as a one-sector-per-item plan-less launch of the same fused kernel path.
 #include <cuda_runtime.h>
 
+#include <algorithm>
+
 #include "su2_internal.h"
+
+namespace su2 {
+
+constexpr int TILE_M = 64;
+constexpr int TILE_P = 64;
+constexpr int NTHREADS = 256;
+constexpr int NC = 32;    // columns of T (n-chunk) per pass
+constexpr int KC = 16;    // k-chunk of the first product
+
+struct TileSmem {
+  double As[TILE_M][KC + 1];      // A[row0+i][k0+kk]
+  double Es[KC][NC + 1];          // E[k0+kk][n0+j]
+  double Ts[TILE_M][NC + 1];      // coef*alpha * (A E)[i][j]
+  double Ds[TILE_P][NC + 1];      // D[col0+c][n0+j]
+};
+
+// acc (64x64 tile at (row0,col0), thread (ty,tx) owns rows ty+16i, cols tx+16c)
+//   += coef * sum_{pos0<=pos<pos1} alpha_pos * A_pos[row0:,:] E D_pos[col0:,:]^T
+__device__ __forceinline__ void accumulate_task(const DevTask& t, const double* __restrict__ E, int pos0, int pos1,
+                                                int row0, int col0, TileSmem& sm, double (&acc)[4][4]) {
+  const int tid = threadIdx.x;
+  const int ty = tid / 16, tx = tid % 16;    // second product: rows ty+16*i, cols tx+16*j
+  const int gy = tid / 8, gx = tid % 8;      // first product : rows gy+32*i (i<2), cols gx+8*j (j<4)
+  const bool ta = t.flags & TASK_TRANS_A, td = t.flags & TASK_TRANS_D;
+  for (int pos = pos0; pos < pos1; ++pos) {
+    const double* __restrict__ A = t.A + (int64_t)pos * t.strideA;
+    const double* __restrict__ D = t.D + (int64_t)pos * t.strideD;
+    const double scale = t.coef * (t.alpha ? t.alpha[pos] : 1.0);
+    for (int n0 = 0; n0 < t.n; n0 += NC) {
+      // ---- first product: T[64 x NC] = A[row0:row0+64, :] * E[:, n0:n0+NC]
+      double tacc[2][4];
+#pragma unroll
+      for (int i = 0; i < 2; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) tacc[i][j] = 0.0;
+      for (int k0 = 0; k0 < t.k; k0 += KC) {
+        for (int e = tid; e < TILE_M * KC; e += NTHREADS) {
+          int i, kk;
+          if (!ta) { i = e / KC; kk = e % KC; } else { kk = e / TILE_M; i = e % TILE_M; }
+          const int r = row0 + i, c = k0 + kk;
+          double v = 0.0;
+          if (r < t.m && c < t.k) v = ta ? A[(int64_t)c * t.m + r] : A[(int64_t)r * t.k + c];
+          sm.As[i][kk] = v;
+        }
+        for (int e = tid; e < KC * NC; e += NTHREADS) {
+          const int kk = e / NC, j = e % NC;
+          const int r = k0 + kk, c = n0 + j;
+          sm.Es[kk][j] = (r < t.k && c < t.n) ? E[(int64_t)r * t.n + c] : 0.0;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int kk = 0; kk < KC; ++kk) {
+          double a[2], b[4];
+#pragma unroll
+          for (int i = 0; i < 2; ++i) a[i] = sm.As[gy + 32 * i][kk];
+#pragma unroll
+          for (int j = 0; j < 4; ++j) b[j] = sm.Es[kk][gx + 8 * j];
+#pragma unroll
+          for (int i = 0; i < 2; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) tacc[i][j] = fma(a[i], b[j], tacc[i][j]);
+        }
+        __syncthreads();
+      }
+#pragma unroll
+      for (int i = 0; i < 2; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) sm.Ts[gy + 32 * i][gx + 8 * j] = scale * tacc[i][j];
+      // ---- D tile: Ds[c][j] = D[col0+c][n0+j]
+      for (int e = tid; e < TILE_P * NC; e += NTHREADS) {
+        int c, j;
+        if (!td) { c = e / NC; j = e % NC; } else { j = e / TILE_P; c = e % TILE_P; }
+        const int r = col0 + c, q = n0 + j;
+        double v = 0.0;
+        if (r < t.p && q < t.n) v = td ? D[(int64_t)q * t.p + r] : D[(int64_t)r * t.n + q];
+        sm.Ds[c][j] = v;
+      }
+      __syncthreads();
+      // ---- second product: F_tile += T * Ds^T  (K = NC columns of this position's stripe)
+#pragma unroll 8
+      for (int j = 0; j < NC; ++j) {
+        double a[4], b[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) a[i] = sm.Ts[ty + 16 * i][j];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) b[c] = sm.Ds[tx + 16 * c][j];
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+          for (int c = 0; c < 4; ++c) acc[i][c] = fma(a[i], b[c], acc[i][c]);
+      }
+      __syncthreads();
+    }
+  }
+}
+
+// BASELINE.json configs[4]: C_b += alpha A_b X_b B_b^T; blockIdx.x = tile, blockIdx.y/z = batch index.
+__global__ void __launch_bounds__(NTHREADS)
+gemm_pair_kernel(int m, int k, int n, int p, int64_t batch, double alpha, const double* __restrict__ A,
+                 const double* __restrict__ X, const double* __restrict__ B, double* __restrict__ C) {
+  __shared__ TileSmem sm;
+  const int tiles_p = (p + TILE_P - 1) / TILE_P;
+  const int row0 = (blockIdx.x / tiles_p) * TILE_M, col0 = (blockIdx.x % tiles_p) * TILE_P;
+  const int ty = threadIdx.x / 16, tx = threadIdx.x % 16;
+  for (int64_t b = blockIdx.y; b < batch; b += gridDim.y) {
+    DevTask t;
+    t.A = A + b * (int64_t)m * k; t.D = B + b * (int64_t)p * n; t.alpha = nullptr; t.coef = alpha; t.e_off = 0;
+    t.m = m; t.k = k; t.n = n; t.p = p; t.strideA = 0; t.strideD = 0; t.npos = 1; t.flags = 0;
+    double acc[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+      for (int j = 0; j < 4; ++j) acc[i][j] = 0.0;
+    accumulate_task(t, X + b * (int64_t)k * n, 0, 1, row0, col0, sm, acc);
+    double* __restrict__ dst = C + b * (int64_t)m * p;
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const int r = row0 + ty + 16 * i, q = col0 + tx + 16 * c;
+        if (r < m && q < p) dst[(int64_t)r * p + q] += acc[i][c];
+      }
+  }
+}
+
+
+su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double alpha, const double* A, const double* X,
+                            const double* B, double* C, void* stream_v) {
+  if (batch == 0) return SU2_OK;
+  const int tiles = ((m + TILE_M - 1) / TILE_M) * ((p + TILE_P - 1) / TILE_P);
+  dim3 grid(tiles, (unsigned)std::min<int64_t>(batch, 65535));
+  gemm_pair_kernel<<<grid, NTHREADS, 0, (cudaStream_t)stream_v>>>(m, k, n, p, batch, alpha, A, X, B, C);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { set_cuda_error("gemm_pair_kernel launch", (int)e); return SU2_ERR_CUDA; }
+  count_launch();
+  return SU2_OK;
+}
+
+
+}  // namespace su2
 
 extern "C" su2_status su2_gemm_pair_batched(int32_t m, int32_t k, int32_t n, int32_t p, int64_t batch, double alpha,
                                             const double* A, const double* X, const double* B, double* C,

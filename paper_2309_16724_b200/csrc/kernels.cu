@@ -1,9 +1,7 @@
-// sm_100a kernels of the hot path:
-//   heff_fused_kernel : F_tile += coef * sum_pos alpha_pos A_pos E D_pos^T with T = A_pos E held in
-//                       shared memory (the paper's two SBGEMM steps, fused; the sum
-//                       over positions is the K loop of the second product = the stripe trick).
-//   reduce_kernel     : fixed-order sum of the partial tiles of split sectors (no atomics).
-//   diag kernels      : diagonal of H_eff for the Davidson preconditioner.
+// Host side of su2_heff_apply and the small kernels around the fused GEMM pair (heff_dmma.cu):
+//   reduce_kernel : second pass of the deterministic segmented reduction:
+//                   fixed-order sum of the partial tiles of split sectors (no atomics).
+//   diag_kernel   : diagonal of H_eff for the Davidson preconditioner.
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -12,7 +10,6 @@
 #include <string>
 
 #include "su2_internal.h"
-#include "tile_config.h"
 
 namespace su2 {
 
@@ -30,165 +27,6 @@ void set_cuda_error(const char* what, int code) {
       return SU2_ERR_CUDA;                          \
     }                                               \
   } while (0)
-
-// ---------------------------------------------------------------------------------------
-// v1 fused GEMM-pair kernel: FP64 FMA, 64x64 output tile, 256 threads, T chunk in smem.
-// ---------------------------------------------------------------------------------------
-constexpr int NTHREADS = 256;
-constexpr int NC = 32;    // columns of T (n-chunk) per pass
-constexpr int KC = 16;    // k-chunk of the first product
-
-struct TileSmem {
-  double As[TILE_M][KC + 1];      // A[row0+i][k0+kk]
-  double Es[KC][NC + 1];          // E[k0+kk][n0+j]
-  double Ts[TILE_M][NC + 1];      // coef*alpha * (A E)[i][j]
-  double Ds[TILE_P][NC + 1];      // D[col0+c][n0+j]
-};
-
-// acc (64x64 tile at (row0,col0), thread (ty,tx) owns rows ty+16i, cols tx+16c)
-//   += coef * sum_{pos0<=pos<pos1} alpha_pos * A_pos[row0:,:] E D_pos[col0:,:]^T
-__device__ __forceinline__ void accumulate_task(const DevTask& t, const double* __restrict__ E, int pos0, int pos1,
-                                                int row0, int col0, TileSmem& sm, double (&acc)[4][4]) {
-  const int tid = threadIdx.x;
-  const int ty = tid / 16, tx = tid % 16;    // second product: rows ty+16*i, cols tx+16*j
-  const int gy = tid / 8, gx = tid % 8;      // first product : rows gy+32*i (i<2), cols gx+8*j (j<4)
-  const bool ta = t.flags & TASK_TRANS_A, td = t.flags & TASK_TRANS_D;
-  for (int pos = pos0; pos < pos1; ++pos) {
-    const double* __restrict__ A = t.A + (int64_t)pos * t.strideA;
-    const double* __restrict__ D = t.D + (int64_t)pos * t.strideD;
-    const double scale = t.coef * (t.alpha ? t.alpha[pos] : 1.0);
-    for (int n0 = 0; n0 < t.n; n0 += NC) {
-      // ---- first product: T[64 x NC] = A[row0:row0+64, :] * E[:, n0:n0+NC]
-      double tacc[2][4];
-#pragma unroll
-      for (int i = 0; i < 2; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) tacc[i][j] = 0.0;
-      for (int k0 = 0; k0 < t.k; k0 += KC) {
-        for (int e = tid; e < TILE_M * KC; e += NTHREADS) {
-          int i, kk;
-          if (!ta) { i = e / KC; kk = e % KC; } else { kk = e / TILE_M; i = e % TILE_M; }
-          const int r = row0 + i, c = k0 + kk;
-          double v = 0.0;
-          if (r < t.m && c < t.k) v = ta ? A[(int64_t)c * t.m + r] : A[(int64_t)r * t.k + c];
-          sm.As[i][kk] = v;
-        }
-        for (int e = tid; e < KC * NC; e += NTHREADS) {
-          const int kk = e / NC, j = e % NC;
-          const int r = k0 + kk, c = n0 + j;
-          sm.Es[kk][j] = (r < t.k && c < t.n) ? E[(int64_t)r * t.n + c] : 0.0;
-        }
-        __syncthreads();
-#pragma unroll
-        for (int kk = 0; kk < KC; ++kk) {
-          double a[2], b[4];
-#pragma unroll
-          for (int i = 0; i < 2; ++i) a[i] = sm.As[gy + 32 * i][kk];
-#pragma unroll
-          for (int j = 0; j < 4; ++j) b[j] = sm.Es[kk][gx + 8 * j];
-#pragma unroll
-          for (int i = 0; i < 2; ++i)
-#pragma unroll
-            for (int j = 0; j < 4; ++j) tacc[i][j] = fma(a[i], b[j], tacc[i][j]);
-        }
-        __syncthreads();
-      }
-#pragma unroll
-      for (int i = 0; i < 2; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) sm.Ts[gy + 32 * i][gx + 8 * j] = scale * tacc[i][j];
-      // ---- D tile: Ds[c][j] = D[col0+c][n0+j]
-      for (int e = tid; e < TILE_P * NC; e += NTHREADS) {
-        int c, j;
-        if (!td) { c = e / NC; j = e % NC; } else { j = e / TILE_P; c = e % TILE_P; }
-        const int r = col0 + c, q = n0 + j;
-        double v = 0.0;
-        if (r < t.p && q < t.n) v = td ? D[(int64_t)q * t.p + r] : D[(int64_t)r * t.n + q];
-        sm.Ds[c][j] = v;
-      }
-      __syncthreads();
-      // ---- second product: F_tile += T * Ds^T  (K = NC columns of this position's stripe)
-#pragma unroll 8
-      for (int j = 0; j < NC; ++j) {
-        double a[4], b[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) a[i] = sm.Ts[ty + 16 * i][j];
-#pragma unroll
-        for (int c = 0; c < 4; ++c) b[c] = sm.Ds[tx + 16 * c][j];
-#pragma unroll
-        for (int i = 0; i < 4; ++i)
-#pragma unroll
-          for (int c = 0; c < 4; ++c) acc[i][c] = fma(a[i], b[c], acc[i][c]);
-      }
-      __syncthreads();
-    }
-  }
-}
-
-__global__ void __launch_bounds__(NTHREADS)
-heff_fused_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __restrict__ units,
-                  const DevTask* __restrict__ tasks, const double* __restrict__ psi, double* __restrict__ out,
-                  double* __restrict__ partial, int* __restrict__ counter) {
-  __shared__ TileSmem sm;
-  __shared__ int s_w;
-  const int tid = threadIdx.x;
-  const int ty = tid / 16, tx = tid % 16;
-  for (;;) {
-    if (tid == 0) s_w = atomicAdd(counter, 1);
-    __syncthreads();
-    const int w = s_w;
-    __syncthreads();
-    if (w >= nwork) break;
-    const DevWork wk = work[w];
-    double acc[4][4];
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-      for (int j = 0; j < 4; ++j) acc[i][j] = 0.0;
-    for (int u = wk.unit0; u < wk.unit1; ++u) {
-      const DevUnit un = units[u];
-      const DevTask t = tasks[un.task];
-      accumulate_task(t, psi + t.e_off, un.pos0, un.pos1, wk.row0, wk.col0, sm, acc);
-    }
-    double* __restrict__ dst = (wk.to_partial ? partial : out) + wk.dst_off;
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        const int r = wk.row0 + ty + 16 * i, q = wk.col0 + tx + 16 * c;
-        if (r < wk.m && q < wk.p) dst[(int64_t)r * wk.p + q] = acc[i][c];
-      }
-  }
-}
-
-// BASELINE.json configs[4]: C_b += alpha A_b X_b B_b^T; blockIdx.x = tile, blockIdx.y/z = batch index.
-__global__ void __launch_bounds__(NTHREADS)
-gemm_pair_kernel(int m, int k, int n, int p, int64_t batch, double alpha, const double* __restrict__ A,
-                 const double* __restrict__ X, const double* __restrict__ B, double* __restrict__ C) {
-  __shared__ TileSmem sm;
-  const int tiles_p = (p + TILE_P - 1) / TILE_P;
-  const int row0 = (blockIdx.x / tiles_p) * TILE_M, col0 = (blockIdx.x % tiles_p) * TILE_P;
-  const int ty = threadIdx.x / 16, tx = threadIdx.x % 16;
-  for (int64_t b = blockIdx.y; b < batch; b += gridDim.y) {
-    DevTask t;
-    t.A = A + b * (int64_t)m * k; t.D = B + b * (int64_t)p * n; t.alpha = nullptr; t.coef = alpha; t.e_off = 0;
-    t.m = m; t.k = k; t.n = n; t.p = p; t.strideA = 0; t.strideD = 0; t.npos = 1; t.flags = 0;
-    double acc[4][4];
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-      for (int j = 0; j < 4; ++j) acc[i][j] = 0.0;
-    accumulate_task(t, X + b * (int64_t)k * n, 0, 1, row0, col0, sm, acc);
-    double* __restrict__ dst = C + b * (int64_t)m * p;
-#pragma unroll
-    for (int i = 0; i < 4; ++i)
-#pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        const int r = row0 + ty + 16 * i, q = col0 + tx + 16 * c;
-        if (r < m && q < p) dst[(int64_t)r * p + q] += acc[i][c];
-      }
-  }
-}
 
 // Second pass of the segmented reduction: fixed index order, one thread per element.
 __global__ void __launch_bounds__(256)
@@ -301,16 +139,8 @@ void free_plan_device(su2_plan* plan) {
 su2_status launch_apply(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream_v) {
   cudaStream_t stream = (cudaStream_t)stream_v;
   SU2_CUDA(cudaMemsetAsync(plan->d_counter, 0, sizeof(int32_t), stream));
-  const int nwork = (int)plan->h_work.size();
-  if (nwork > 0) {
-    int ctas_per_sm = 0;
-    SU2_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, heff_fused_kernel, NTHREADS, 0));
-    const int grid = std::min(nwork, plan->num_sms * std::max(ctas_per_sm, 1));
-    heff_fused_kernel<<<grid, NTHREADS, 0, stream>>>(plan->d_work, nwork, plan->d_units, plan->d_tasks, psi, out, partial,
-                                                     plan->d_counter);
-    SU2_CUDA(cudaGetLastError());
-    count_launch();
-  }
+  su2_status st = launch_heff_dmma(plan, psi, out, partial, stream_v);
+  if (st != SU2_OK) return st;
   const int nsec = (int)plan->h_reduce.size();
   if (nsec > 0) {
     dim3 grid(32, nsec);
@@ -318,17 +148,6 @@ su2_status launch_apply(const su2_plan* plan, const double* psi, double* out, do
     SU2_CUDA(cudaGetLastError());
     count_launch();
   }
-  return SU2_OK;
-}
-
-su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double alpha, const double* A, const double* X,
-                            const double* B, double* C, void* stream_v) {
-  if (batch == 0) return SU2_OK;
-  const int tiles = ((m + TILE_M - 1) / TILE_M) * ((p + TILE_P - 1) / TILE_P);
-  dim3 grid(tiles, (unsigned)std::min<int64_t>(batch, 65535));
-  gemm_pair_kernel<<<grid, NTHREADS, 0, (cudaStream_t)stream_v>>>(m, k, n, p, batch, alpha, A, X, B, C);
-  SU2_CUDA(cudaGetLastError());
-  count_launch();
   return SU2_OK;
 }
 

@@ -313,27 +313,43 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
     ntp += ht.npos;
   }
 
-  // ---- segments: deterministic segmented reduction (no atomics) ---------------------------
-  // Per output sector the task list is cut into nseg segments of equal work; each (segment, tile)
-  // is one CTA work item.  nseg == 1 writes F directly, otherwise partial copies are summed in
-  // index order by the reduce pass.
+  // ---- tile class per output sector, segments, work items ---------------------------------
+  // Every output sector gets the tile class (TileCfg<WR>, tile_config.h) with the lowest modelled
+  // cost.  Its task list (plan order) is cut into nseg segments of equal cost; each (segment, tile)
+  // is one CTA work item.  nseg == 1 writes F directly, otherwise the segments write partial
+  // copies that the reduce pass sums in index order: deterministic, no atomics (row a5).
   const int nsec = (int)plan->psi.size();
   std::vector<int64_t> first_task(nsec + 1, 0);
   for (const HostTask& ht : plan->tasks) first_task[ht.out_sec + 1]++;
   for (int s = 0; s < nsec; ++s) first_task[s + 1] += first_task[s];
-  auto pos_cost = [&](const HostTask& ht) {  // flops of one position for ONE output tile (recompute of T per tile)
-    const double tm = std::min<double>(TILE_M, ht.m), tp = std::min<double>(TILE_P, ht.p);
-    return 2.0 * tm * ht.k * ht.n + 2.0 * tm * ht.n * tp;
+  // cost of one position of task ht summed over all tiles of its output sector
+  auto pos_cost_all_tiles = [&](int wr, const HostTask& ht) {
+    const TileShape ts = tile_shape(wr);
+    double c = 0.0;
+    for (int r0 = 0; r0 < ht.m; r0 += ts.tm)
+      for (int c0 = 0; c0 < ht.p; c0 += ts.tp)
+        c += tile_pos_cost(wr, std::min(ts.tm, ht.m - r0), std::min(ts.tp, ht.p - c0), ht.k, ht.n);
+    return c;
   };
-  double total_item_work = 0.0, executed = 0.0;
-  std::vector<double> sec_work(nsec, 0.0);
+  std::vector<int> sec_wr(nsec, 1);
+  std::vector<double> sec_cost(nsec, 0.0);        // summed over tiles
+  double total_cost = 0.0;
   for (int s = 0; s < nsec; ++s) {
-    const int tiles = ((plan->psi[s].m + TILE_M - 1) / TILE_M) * ((plan->psi[s].p + TILE_P - 1) / TILE_P);
-    for (int64_t i = first_task[s]; i < first_task[s + 1]; ++i) sec_work[s] += pos_cost(plan->tasks[i]) * plan->tasks[i].npos;
-    total_item_work += sec_work[s] * tiles;
+    if (first_task[s + 1] == first_task[s]) continue;
+    double best = -1.0;
+    for (int wr : {1, 2, 4}) {
+      double c = 0.0;
+      for (int64_t i = first_task[s]; i < first_task[s + 1]; ++i) c += pos_cost_all_tiles(wr, plan->tasks[i]) * plan->tasks[i].npos;
+      if (best < 0.0 || c < best * 0.97) {   // prefer the smaller tile unless the larger one is clearly cheaper
+        if (best < 0.0 || c < best) { best = c; sec_wr[s] = wr; }
+      }
+    }
+    sec_cost[s] = best;
+    total_cost += best;
   }
-  executed = total_item_work;
-  const double target = (flags & SU2_PLAN_FORCE_SPLIT) ? 2.0e4 : std::max(total_item_work / (148.0 * 24.0), 4.0e6);
+  const double executed = total_cost * NWARPS * 512.0;   // DMMA issue slots x 8 warps x 2*8*8*4 flop
+  // target cost of one work item: ~24 items per SM, but never so small that the pipeline fill dominates
+  const double target = (flags & SU2_PLAN_FORCE_SPLIT) ? 40.0 : std::max(total_cost / (148.0 * 24.0), 2.0e4);
   plan->partial_elems = 0;
   std::vector<double> work_cost;   // for LPT ordering
   for (int s = 0; s < nsec; ++s) {
@@ -346,7 +362,17 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
       plan->h_reduce.push_back(red);
       continue;
     }
-    int nseg = (int)std::min<double>(64.0, std::max(1.0, std::ceil(sec_work[s] / target)));
+    const int wr = sec_wr[s];
+    const TileShape ts = tile_shape(wr);
+    const int ntiles = ((ps.m + ts.tm - 1) / ts.tm) * ((ps.p + ts.tp - 1) / ts.tp);
+    // per-tile cost of a position: the full row tile (the ragged last one is cheaper; LPT evens that out)
+    auto pos_cost = [&](const HostTask& ht) {
+      return tile_pos_cost(wr, std::min(ts.tm, ht.m), std::min(ts.tp, ht.p), ht.k, ht.n);
+    };
+    double tile_work = 0.0;
+    for (int64_t i = t0; i < t1; ++i) tile_work += pos_cost(plan->tasks[i]) * plan->tasks[i].npos;
+    int nseg = (int)std::min<double>(64.0, std::max(1.0, std::ceil(tile_work / target)));
+    (void)ntiles;
     std::vector<std::pair<int32_t, int32_t>> seg_units;   // unit ranges per segment
     {
       double acc = 0.0;
@@ -359,7 +385,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
         while (pos < ht.npos) {
           int take = ht.npos - pos;
           if (seg < nseg - 1) {
-            const double room = sec_work[s] * (seg + 1) / nseg - acc;
+            const double room = tile_work * (seg + 1) / nseg - acc;
             const int fit = (int)std::floor(room / c + 1e-9);
             if (fit <= 0) {   // this segment is full: close it
               seg_units.push_back({ustart, (int32_t)plan->h_units.size()});
@@ -388,16 +414,20 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
     }
     plan->h_reduce.push_back(red);
     for (int g = 0; g < nseg; ++g) {
-      double w = 0.0;
-      for (int32_t u = segs[g].first; u < segs[g].second; ++u)
-        w += pos_cost(plan->tasks[plan->h_units[u].task]) * (plan->h_units[u].pos1 - plan->h_units[u].pos0);
-      for (int r0 = 0; r0 < ps.m; r0 += TILE_M)
-        for (int c0 = 0; c0 < ps.p; c0 += TILE_P) {
+      for (int r0 = 0; r0 < ps.m; r0 += ts.tm)
+        for (int c0 = 0; c0 < ps.p; c0 += ts.tp) {
+          double w = 0.0;
+          for (int32_t u = segs[g].first; u < segs[g].second; ++u) {
+            const HostTask& ht = plan->tasks[plan->h_units[u].task];
+            w += tile_pos_cost(wr, std::min(ts.tm, ps.m - r0), std::min(ts.tp, ps.p - c0), ht.k, ht.n) *
+                 (plan->h_units[u].pos1 - plan->h_units[u].pos0);
+          }
           DevWork wk{};
           wk.unit0 = segs[g].first; wk.unit1 = segs[g].second;
           wk.row0 = r0; wk.col0 = c0; wk.m = ps.m; wk.p = ps.p;
           wk.to_partial = nseg > 1 ? 1 : 0;
           wk.dst_off = nseg > 1 ? red.part_off + (int64_t)g * sz : ps.off;
+          wk.wr = wr;
           plan->h_work.push_back(wk);
           work_cost.push_back(w);
         }

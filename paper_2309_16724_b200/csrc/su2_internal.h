@@ -36,7 +36,7 @@ struct DevWork {
   int32_t row0, col0;     // tile origin inside the (m x p) output block
   int32_t m, p;           // output block dims (p = leading dimension)
   int32_t to_partial;     // 1: dst_off refers to the partial buffer
-  int32_t pad;
+  int32_t wr;             // tile class: warp rows WR of TileCfg<WR> (1, 2 or 4)
 };
 
 // Second pass of the deterministic segmented reduction: F_s = sum_{seg} partial[seg] in index order.
@@ -70,10 +70,6 @@ struct PsiSector {
   int32_t il, sB, twoJ1, sC, ir, twoJ2;
   int64_t off;
   int32_t m, p;
-};
-
-struct Tiling {
-  int32_t tm, tp;     // CTA output tile
 };
 
 }  // namespace su2
@@ -113,6 +109,7 @@ struct su2_plan {
 
 namespace su2 {
 // kernels.cu
+su2_status launch_heff_dmma(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream);   // heff_dmma.cu
 su2_status launch_apply(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream);
 su2_status launch_diag(const su2_plan* plan, double* diag, void* stream);
 su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, const std::vector<double>& ident_host,
