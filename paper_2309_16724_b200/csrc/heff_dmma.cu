@@ -133,21 +133,24 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
-// Tile element (c, j) = src[c*ld + j]  ->  smem [j/4][c][j%4]   (c-major k4 sub-tiles, no padding)
+// Both copies land in the same shared-memory layout, [j/4][j%4][c] with row stride CT+4 doubles
+// (k-major k4 sub-tiles; CT+4 = 4 mod 8 makes the DMMA fragment loads conflict-free), so the math
+// code does not depend on how the operator block is stored.
+// Source stored c-major, element (c, j) = src[c*ld + j]: 8 consecutive lanes read one 64-byte run.
 template <int CT>
 __device__ __forceinline__ void copy_cmajor(double* dst, const double* __restrict__ src, int ld, int cval, int jval) {
   const int cpad = (cval + 7) & ~7;
   const int jpad = jval > 4 ? 8 : 4;
   const int j = threadIdx.x & 7;
   if (j >= jpad) return;
-  double* d = dst + (j >> 2) * (CT * 4) + (j & 3);
+  double* d = dst + (j >> 2) * (4 * (CT + 4)) + (j & 3) * (CT + 4);
   const bool jok = j < jval;
   for (int c = threadIdx.x >> 3; c < cpad; c += NTHREADS / 8) {
     const bool ok = jok && c < cval;
-    cp_async8(d + c * 4, ok ? src + (int64_t)c * ld + j : src, ok);
+    cp_async8(d + c, ok ? src + (int64_t)c * ld + j : src, ok);
   }
 }
-// Tile element (c, j) = src[j*ld + c]  ->  smem [j/4][j%4][c] with row stride CT+4
+// Source stored k-major, element (c, j) = src[j*ld + c]: a warp reads one 256-byte run.
 template <int CT>
 __device__ __forceinline__ void copy_kmajor(double* dst, const double* __restrict__ src, int ld, int cval, int jval) {
   const int cpad = (cval + 7) & ~7;
@@ -167,6 +170,37 @@ __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
   asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
       : "+d"(c[0]), "+d"(c[1])
       : "d"(a), "d"(b));
+}
+
+// One pipeline stage (nsub k4 sub-steps) of a warp-level product: c[ii][j] += A_frag[ii] B_frag[j]
+// for 4 m8-tiles (the first mt active) and NT n8-tiles.  a / b point at this lane's element of the
+// first fragment; A_I / A_SUB / B_SUB are the compile-time strides between m8-tiles / k4 sub-steps
+// (n8-tiles are 8 doubles apart).
+template <int NT, int NACC, int A_I, int A_SUB, int B_SUB>
+__device__ __forceinline__ void mma_stage(double (&c)[4][NACC][2], const double* __restrict__ a,
+                                          const double* __restrict__ b, int nsub, int mt) {
+#pragma unroll
+  for (int sub = 0; sub < 2; ++sub) {
+    if (sub < nsub) {
+      double af[4], bf[NT];
+#pragma unroll
+      for (int ii = 0; ii < 4; ++ii) af[ii] = a[sub * A_SUB + ii * A_I];
+#pragma unroll
+      for (int j = 0; j < NT; ++j) bf[j] = b[sub * B_SUB + j * 8];
+      if (mt == 4) {
+#pragma unroll
+        for (int j = 0; j < NT; ++j)
+#pragma unroll
+          for (int ii = 0; ii < 4; ++ii) dmma(c[ii][j], af[ii], bf[j]);
+      } else {
+#pragma unroll
+        for (int j = 0; j < NT; ++j)
+#pragma unroll
+          for (int ii = 0; ii < 3; ++ii)
+            if (ii < mt) dmma(c[ii][j], af[ii], bf[j]);
+      }
+    }
+  }
 }
 
 template <int WR>
@@ -250,73 +284,55 @@ __device__ void run_item(const DevWork& wk, const DevUnit* __restrict__ units, c
     }
     const double* stage = stages + buf * C::STAGE;
     const int nsub = d.jval > 4 ? 2 : 1;
-    const bool tr = flags & STEP_TRANS;
     if (!(flags & STEP_G2)) {
       // ---- first product: tacc (32 x 8 NT1 per warp) += A_tile E_tile --------------------------
-      const double* As = stage;
-      const double* Es = stage + C::A_SZ;
-      const int a_sub = tr ? 4 * (TM + 4) : TM * 4;
-      const int a_i = tr ? 8 : 32;
-      const int a_off = tr ? t * (TM + 4) + wr * 32 + g : (wr * 32 + g) * 4 + t;
       const int ntiles1 = (d.cval1 + 7) >> 3;
       const int nt1w = (ntiles1 + WC - 1) / WC;
       const int tile0 = wc * nt1w;
       const int nt1 = max(0, min(nt1w, ntiles1 - tile0));
-      const int e_off = t * LDE + tile0 * 8 + g;
+      const double* a = stage + t * (TM + 4) + wr * 32 + g;
+      const double* b = stage + C::A_SZ + t * LDE + tile0 * 8 + g;
       if (flags & STEP_FIRST) {
 #pragma unroll
         for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
           for (int j = 0; j < NT1; ++j) tacc[ii][j][0] = tacc[ii][j][1] = 0.0;
       }
-      if (mt > 0 && nt1 > 0) {
-        for (int sub = 0; sub < nsub; ++sub) {
-          double a[4];
-#pragma unroll
-          for (int ii = 0; ii < 4; ++ii) a[ii] = As[sub * a_sub + a_off + ii * a_i];
-#pragma unroll
-          for (int j = 0; j < NT1; ++j) {
-            if (j < nt1) {
-              const double b = Es[sub * (4 * LDE) + e_off + j * 8];
-#pragma unroll
-              for (int ii = 0; ii < 4; ++ii)
-                if (ii < mt) dmma(tacc[ii][j], a[ii], b);
-            }
-          }
+      if (mt > 0) {
+        switch (nt1) {
+          case 1: mma_stage<1, NT1, 8, 4 * (TM + 4), 4 * LDE>(tacc, a, b, nsub, mt); break;
+          case 2: mma_stage<2, NT1, 8, 4 * (TM + 4), 4 * LDE>(tacc, a, b, nsub, mt); break;
+          case 3: mma_stage<3, NT1, 8, 4 * (TM + 4), 4 * LDE>(tacc, a, b, nsub, mt); break;
+          case 4: mma_stage<4, NT1, 8, 4 * (TM + 4), 4 * LDE>(tacc, a, b, nsub, mt); break;
+          default: break;
         }
       }
       if (flags & STEP_LAST) {
         const double sc = d.scale;
+        double* trow = Ts + (wr * 32 + g) * LDT + tile0 * 8 + 2 * t;
 #pragma unroll
         for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
           for (int j = 0; j < NT1; ++j)
-            if (ii < mt && j < nt1) {
-              double2 v = make_double2(sc * tacc[ii][j][0], sc * tacc[ii][j][1]);
-              *reinterpret_cast<double2*>(Ts + (wr * 32 + ii * 8 + g) * LDT + (tile0 + j) * 8 + 2 * t) = v;
-            }
+            if (ii < mt && j < nt1)
+              *reinterpret_cast<double2*>(trow + ii * 8 * LDT + j * 8) = make_double2(sc * tacc[ii][j][0], sc * tacc[ii][j][1]);
       }
     } else {
       // ---- second product: acc (32 x 8 NT2 per warp) += T_chunk[:, step] D_tile^T ---------------
-      const double* Ds = stage;
-      const int d_sub = tr ? 4 * (TP + 4) : TP * 4;
-      const int d_j = tr ? 8 : 32;
-      const int d_off = tr ? t * (TP + 4) + ctile0 * 8 + g : (ctile0 * 8 + g) * 4 + t;
-      const int t_off = (wr * 32 + g) * LDT + d.s * KS + t;
-      if (mt > 0 && nt2 > 0) {
-        for (int sub = 0; sub < nsub; ++sub) {
-          double a[4];
-#pragma unroll
-          for (int ii = 0; ii < 4; ++ii) a[ii] = Ts[t_off + sub * 4 + ii * 8 * LDT];
-#pragma unroll
-          for (int j = 0; j < NT2; ++j) {
-            if (j < nt2) {
-              const double b = Ds[sub * d_sub + d_off + j * d_j];
-#pragma unroll
-              for (int ii = 0; ii < 4; ++ii)
-                if (ii < mt) dmma(acc[ii][j], a[ii], b);
-            }
-          }
+      const double* a = Ts + (wr * 32 + g) * LDT + d.s * KS + t;
+      const double* b = stage + t * (TP + 4) + ctile0 * 8 + g;
+      if (mt > 0) {
+        switch (nt2) {
+          case 1: mma_stage<1, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, a, b, nsub, mt); break;
+          case 2: mma_stage<2, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, a, b, nsub, mt); break;
+          case 3: mma_stage<3, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, a, b, nsub, mt); break;
+          case 4: mma_stage<4, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, a, b, nsub, mt); break;
+          case 5: mma_stage<5, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, a, b, nsub, mt); break;
+          case 6: mma_stage<6, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, a, b, nsub, mt); break;
+          case 7: mma_stage<7, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, a, b, nsub, mt); break;
+          case 8: mma_stage<8, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, a, b, nsub, mt); break;
+          case 9: mma_stage<9, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, a, b, nsub, mt); break;
+          default: break;
         }
       }
     }
