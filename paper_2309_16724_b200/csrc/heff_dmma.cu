@@ -12,13 +12,19 @@
 // 99.8 % of 148 SM x 64 FMA/clk x 1.965 GHz, against 33.8 TFLOP/s for a DFMA loop
 // (profiles/r01_fp64_peak_probe.txt).
 //
-// Structure: persistent CTAs (one per SM, 8 warps) pull work items (segment x output tile) from an
-// atomic queue in the plan's longest-first order.  Inside an item every (task, position, T-chunk)
-// is a run of pipeline *steps*: first-product steps (A tile + E tile, KS deep) followed by
-// second-product steps (D tile, KS deep).  Steps are described by small descriptors that one
-// thread generates ahead of time into a shared-memory ring, so the control state costs no
-// registers; operand tiles are staged by 8-byte cp.async with zero fill (ragged block sizes and
-// odd leading dimensions need no special cases) NSTAGE-1 steps ahead of the math.
+// Structure: persistent CTAs (one per SM) pull work items (segment x output tile) from an atomic
+// queue in the plan's longest-first order.  Inside an item every (task, position, T-chunk) is a run
+// of pipeline *steps*: first-product steps (A tile + E tile, KS deep) followed by second-product
+// steps (D tile, KS deep).  The CTA is warp-specialised:
+//   * warps 0-3 (one warpgroup, 40 registers after setmaxnreg.dec) are PRODUCERS.  Producer warp w
+//     owns stage buffer w: it walks the item's step sequence with an iterator kept in shared
+//     memory, writes the step descriptor, and stages the operand tiles with 8-byte cp.async + zero
+//     fill (ragged block sizes and odd leading dimensions need no special cases); completion is
+//     signalled on an mbarrier (cp.async.mbarrier.arrive.noinc).
+//   * warps 4-11 (two warpgroups, 232 registers after setmaxnreg.inc) are CONSUMERS: they wait on
+//     the stage's "full" mbarrier, issue only LDS + DMMA, and release the stage on its "empty"
+//     mbarrier.  No CTA-wide barrier exists inside an item; the T hand-over between the two
+//     products uses a named barrier of the 256 consumer threads.
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -45,15 +51,13 @@ struct StepDesc {
   int pad;
 };
 
-struct GenState {       // iterator over the steps of one work item (lives in shared memory)
+struct GenState {       // iterator over the steps of one work item (one per producer warp, in shared memory)
   const double *A, *D, *E, *alpha;
   double coef, scale;
   int m, k, n, p, strideA, strideD, tflags;
   int u, u_end, pos, pos_end, chunk, nchunks, ncw_full, n0, ncw, phase, s, nsteps1, nsteps2, done;
   int row0, col0, rows_valid, cols_valid, nc_max;
 };
-
-constexpr int RING = NSTAGE + 1;
 
 __device__ __forceinline__ void gen_set_chunk(GenState& st) {
   st.n0 = st.chunk * st.ncw_full;
@@ -80,9 +84,23 @@ __device__ __forceinline__ void gen_load_unit(GenState& st, const DevUnit* __res
   gen_set_pos(st);
 }
 
-// Emit the descriptor of the current step and advance the iterator (one thread).
-__device__ void gen_step(GenState& st, StepDesc& d, const DevUnit* __restrict__ units,
-                         const DevTask* __restrict__ tasks, const double* __restrict__ psi) {
+// Move the iterator to the next step.
+__device__ __forceinline__ void gen_advance(GenState& st, const DevUnit* __restrict__ units,
+                                            const DevTask* __restrict__ tasks, const double* __restrict__ psi) {
+  if (st.done) return;
+  ++st.s;
+  if (st.phase == 0) {
+    if (st.s == st.nsteps1) { st.phase = 1; st.s = 0; }
+  } else if (st.s == st.nsteps2) {
+    if (++st.chunk < st.nchunks) gen_set_chunk(st);
+    else if (++st.pos < st.pos_end) gen_set_pos(st);
+    else if (++st.u < st.u_end) gen_load_unit(st, units, tasks, psi);
+    else st.done = 1;
+  }
+}
+
+// Descriptor of the current step.
+__device__ __forceinline__ void gen_fill(const GenState& st, StepDesc& d) {
   if (st.done) {
     d.flags = STEP_END;
     return;
@@ -112,54 +130,73 @@ __device__ void gen_step(GenState& st, StepDesc& d, const DevUnit* __restrict__ 
     d.s = st.s;
     d.flags = STEP_G2 | (tr ? STEP_TRANS : 0);
   }
-  ++st.s;
-  if (st.phase == 0) {
-    if (st.s == st.nsteps1) { st.phase = 1; st.s = 0; }
-  } else if (st.s == st.nsteps2) {
-    if (++st.chunk < st.nchunks) gen_set_chunk(st);
-    else if (++st.pos < st.pos_end) gen_set_pos(st);
-    else if (++st.u < st.u_end) gen_load_unit(st, units, tasks, psi);
-    else st.done = 1;
-  }
 }
 
-// ---- cp.async staging (8-byte elements, zero fill when !valid) ---------------------------
+// ---- PTX helpers -------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, int parity) {
+  unsigned ok;
+  asm volatile(
+      "{\n.reg .pred p;\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+      "selp.u32 %0, 1, 0, p;\n}\n"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, int parity) {
+  while (!mbar_try_wait(bar, parity)) {}
+}
+// arrive on `bar` once all cp.async issued so far by this thread have landed (count pre-charged at init)
+__device__ __forceinline__ void cp_async_mbar_arrive(uint64_t* bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ void cp_async8(double* smem_dst, const double* src, bool valid) {
-  const unsigned dst = (unsigned)__cvta_generic_to_shared(smem_dst);
-  const int sz = valid ? 8 : 0;
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(dst), "l"(src), "r"(sz));
+  const int sz = valid ? 8 : 0;   // src-size 0: destination is zero-filled, nothing is read
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(smem_u32(smem_dst)), "l"(src), "r"(sz) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+__device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, 256;\n" ::: "memory"); }
+__device__ __forceinline__ void cta_bar() { asm volatile("bar.sync 0, 384;\n" ::: "memory"); }
+static_assert(NTHREADS == 384 && NWARPS * 32 == 256, "barrier thread counts are spelled out in the PTX above");
 
-// Both copies land in the same shared-memory layout, [j/4][j%4][c] with row stride CT+4 doubles
+// ---- staging: one producer WARP copies a whole tile ---------------------------------------------
+// Every tile lands in the same shared-memory layout, [j/4][j%4][c] with row stride CT+4 doubles
 // (k-major k4 sub-tiles; CT+4 = 4 mod 8 makes the DMMA fragment loads conflict-free), so the math
 // code does not depend on how the operator block is stored.
 // Source stored c-major, element (c, j) = src[c*ld + j]: 8 consecutive lanes read one 64-byte run.
 template <int CT>
-__device__ __forceinline__ void copy_cmajor(double* dst, const double* __restrict__ src, int ld, int cval, int jval) {
+__device__ __forceinline__ void copy_cmajor(double* dst, const double* __restrict__ src, int ld, int cval, int jval, int lane) {
   const int cpad = (cval + 7) & ~7;
   const int jpad = jval > 4 ? 8 : 4;
-  const int j = threadIdx.x & 7;
+  const int j = lane & 7;
   if (j >= jpad) return;
   double* d = dst + (j >> 2) * (4 * (CT + 4)) + (j & 3) * (CT + 4);
   const bool jok = j < jval;
-  for (int c = threadIdx.x >> 3; c < cpad; c += NTHREADS / 8) {
+  const double* s = src + j;
+#pragma unroll 4
+  for (int c = lane >> 3; c < cpad; c += 4) {
     const bool ok = jok && c < cval;
-    cp_async8(d + c, ok ? src + (int64_t)c * ld + j : src, ok);
+    cp_async8(d + c, ok ? s + (int64_t)c * ld : src, ok);
   }
 }
 // Source stored k-major, element (c, j) = src[j*ld + c]: a warp reads one 256-byte run.
 template <int CT>
-__device__ __forceinline__ void copy_kmajor(double* dst, const double* __restrict__ src, int ld, int cval, int jval) {
+__device__ __forceinline__ void copy_kmajor(double* dst, const double* __restrict__ src, int ld, int cval, int jval, int lane) {
   const int cpad = (cval + 7) & ~7;
   const int jpad = jval > 4 ? 8 : 4;
   for (int j = 0; j < jpad; ++j) {
     double* d = dst + (j >> 2) * (4 * (CT + 4)) + (j & 3) * (CT + 4);
     const double* s = src + (int64_t)j * ld;
     const bool jok = j < jval;
-    for (int c = threadIdx.x; c < cpad; c += NTHREADS) {
+#pragma unroll 4
+    for (int c = lane; c < cpad; c += 32) {
       const bool ok = jok && c < cval;
       cp_async8(d + c, ok ? s + c : src, ok);
     }
@@ -203,32 +240,66 @@ __device__ __forceinline__ void mma_stage(double (&c)[4][NACC][2], const double*
   }
 }
 
+// ---- producer warp w: owns stage buffer w and the item's steps  l  with (base + l) % NSTAGE == w --------
 template <int WR>
-__device__ __forceinline__ void issue_loads(const StepDesc& d, double* stage) {
+__device__ __forceinline__ void producer_item(const DevWork& wk, const DevUnit* __restrict__ units,
+                                              const DevTask* __restrict__ tasks, const double* __restrict__ psi,
+                                              double* smem, GenState& st, StepDesc& desc, uint64_t* full, uint64_t* empty,
+                                              int w, int lane, int first, unsigned& nfill) {
   using C = TileCfg<WR>;
-  const int flags = d.flags;
-  if (flags & STEP_END) return;
-  if (!(flags & STEP_G2)) {
-    if (flags & STEP_TRANS) copy_kmajor<C::TM>(stage, d.src0, d.ld0, d.cval0, d.jval);
-    else copy_cmajor<C::TM>(stage, d.src0, d.ld0, d.cval0, d.jval);
-    copy_kmajor<C::NC>(stage + C::A_SZ, d.src1, d.ld1, d.cval1, d.jval);
-  } else {
-    if (flags & STEP_TRANS) copy_kmajor<C::TP>(stage, d.src0, d.ld0, d.cval0, d.jval);
-    else copy_cmajor<C::TP>(stage, d.src0, d.ld0, d.cval0, d.jval);
+  double* stage = smem + C::TM * C::LDT + w * C::STAGE;
+  if (lane == 0) {
+    st.u = wk.unit0; st.u_end = wk.unit1; st.done = 0;
+    st.row0 = wk.row0; st.col0 = wk.col0;
+    st.rows_valid = min(C::TM, wk.m - wk.row0);
+    st.cols_valid = min(C::TP, wk.p - wk.col0);
+    st.nc_max = C::NC;
+    if (st.u < st.u_end) gen_load_unit(st, units, tasks, psi);
+    else st.done = 1;
+    for (int i = 0; i < first; ++i) gen_advance(st, units, tasks, psi);
+  }
+  __syncwarp();
+#pragma unroll 1
+  for (;;) {
+    mbar_wait(&empty[w], (int)((nfill & 1u) ^ 1u));     // consumers have released the previous fill of this buffer
+    if (lane == 0) {
+      gen_fill(st, desc);
+#pragma unroll 1
+      for (int i = 0; i < NSTAGE; ++i) gen_advance(st, units, tasks, psi);
+    }
+    __syncwarp();
+    const int flags = desc.flags;
+    if (!(flags & STEP_END)) {
+      const double* src0 = desc.src0;
+      const int ld0 = desc.ld0, cval0 = desc.cval0, jval = desc.jval;
+      if (!(flags & STEP_G2)) {
+        if (flags & STEP_TRANS) copy_kmajor<C::TM>(stage, src0, ld0, cval0, jval, lane);
+        else copy_cmajor<C::TM>(stage, src0, ld0, cval0, jval, lane);
+        copy_kmajor<C::NC>(stage + C::A_SZ, desc.src1, desc.ld1, desc.cval1, jval, lane);
+      } else {
+        if (flags & STEP_TRANS) copy_kmajor<C::TP>(stage, src0, ld0, cval0, jval, lane);
+        else copy_cmajor<C::TP>(stage, src0, ld0, cval0, jval, lane);
+      }
+    }
+    cp_async_mbar_arrive(&full[w]);          // 32 deferred arrivals: this lane's copies have landed
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&full[w]);    // +1 (release): the descriptor is visible
+    ++nfill;
+    if (flags & STEP_END) break;
   }
 }
 
-// One work item: TM x TP tile of one output sector, one segment of its (task, position) list.
+// ---- consumer warp cw = (wr, wc): LDS + DMMA only -------------------------------------------------------
 template <int WR>
-__device__ void run_item(const DevWork& wk, const DevUnit* __restrict__ units, const DevTask* __restrict__ tasks,
-                         const double* __restrict__ psi, double* __restrict__ dst, double* smem, GenState& st,
-                         StepDesc* ring) {
+__device__ __forceinline__ void consumer_item(const DevWork& wk, double* __restrict__ dst, double* smem,
+                                              const StepDesc* ring, uint64_t* full, uint64_t* empty, int cw, int lane,
+                                              unsigned& ci) {
   using C = TileCfg<WR>;
   constexpr int WC = C::WC, TM = C::TM, TP = C::TP, NC = C::NC, LDT = C::LDT, LDE = NC + 4;
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
-  const int wr = warp / WC, wc = warp % WC;
+  const int g = lane >> 2, t = lane & 3;
+  const int wr = cw / WC, wc = cw % WC;
   double* Ts = smem;
-  double* stages = smem + TM * LDT;
+  const double* stages = smem + TM * LDT;
 
   const int rows_valid = min(TM, wk.m - wk.row0);
   const int cols_valid = min(TP, wk.p - wk.col0);
@@ -237,20 +308,6 @@ __device__ void run_item(const DevWork& wk, const DevUnit* __restrict__ units, c
   const int ntw2 = (ntiles2 + WC - 1) / WC;
   const int ctile0 = wc * ntw2;
   const int nt2 = max(0, min(ntw2, ntiles2 - ctile0));                     // active n8-tiles (second product)
-
-  if (tid == 0) {
-    st.u = wk.unit0; st.u_end = wk.unit1; st.done = 0;
-    st.row0 = wk.row0; st.col0 = wk.col0; st.rows_valid = rows_valid; st.cols_valid = cols_valid; st.nc_max = NC;
-    if (st.u < st.u_end) gen_load_unit(st, units, tasks, psi);
-    else st.done = 1;
-    for (int i = 0; i < NSTAGE; ++i) gen_step(st, ring[i], units, tasks, psi);
-  }
-  __syncthreads();
-#pragma unroll 1
-  for (int L = 0; L < NSTAGE - 1; ++L) {
-    issue_loads<WR>(ring[L], stages + L * C::STAGE);
-    cp_async_commit();
-  }
 
   double acc[4][NT2][2];
   double tacc[4][NT1][2];
@@ -263,24 +320,19 @@ __device__ void run_item(const DevWork& wk, const DevUnit* __restrict__ units, c
 #pragma unroll
     for (int j = 0; j < NT1; ++j) tacc[i][j][0] = tacc[i][j][1] = 0.0;
 
-  int slot = 0;          // ring slot of step i
-  int buf = 0;           // stage buffer of step i
+  int ends = 0;
 #pragma unroll 1
-  for (int i = 0;; ++i) {
-    cp_async_wait<NSTAGE - 2>();
-    __syncthreads();
-    const StepDesc& d = ring[slot];
+  for (;;) {
+    const int buf = (int)(ci & (NSTAGE - 1));
+    mbar_wait(&full[buf], (int)((ci >> 2) & 1u));
+    ++ci;
+    const StepDesc& d = ring[buf];
     const int flags = d.flags;
-    if (flags & STEP_END) break;
-    {   // stage the operands of step i + NSTAGE - 1 into the buffer that step i - 1 has just released
-      int lslot = slot + NSTAGE - 1; if (lslot >= RING) lslot -= RING;
-      int lbuf = buf + NSTAGE - 1;  if (lbuf >= NSTAGE) lbuf -= NSTAGE;
-      issue_loads<WR>(ring[lslot], stages + lbuf * C::STAGE);
-      cp_async_commit();
-      if (tid == ((i & 7) << 5)) {       // descriptor of step i + NSTAGE, written into the slot of step i - 1
-        int gslot = lslot + 1; if (gslot >= RING) gslot -= RING;
-        gen_step(st, ring[gslot], units, tasks, psi);
-      }
+    if (flags & STEP_END) {
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty[buf]);
+      if (++ends == NSTAGE) break;
+      continue;
     }
     const double* stage = stages + buf * C::STAGE;
     const int nsub = d.jval > 4 ? 2 : 1;
@@ -290,6 +342,7 @@ __device__ void run_item(const DevWork& wk, const DevUnit* __restrict__ units, c
       const int nt1w = (ntiles1 + WC - 1) / WC;
       const int tile0 = wc * nt1w;
       const int nt1 = max(0, min(nt1w, ntiles1 - tile0));
+      const double sc = d.scale;
       const double* a = stage + t * (TM + 4) + wr * 32 + g;
       const double* b = stage + C::A_SZ + t * LDE + tile0 * 8 + g;
       if (flags & STEP_FIRST) {
@@ -303,12 +356,13 @@ __device__ void run_item(const DevWork& wk, const DevUnit* __restrict__ units, c
           case 1: mma_stage<1, NT1, 8, 4 * (TM + 4), 4 * LDE>(tacc, a, b, nsub, mt); break;
           case 2: mma_stage<2, NT1, 8, 4 * (TM + 4), 4 * LDE>(tacc, a, b, nsub, mt); break;
           case 3: mma_stage<3, NT1, 8, 4 * (TM + 4), 4 * LDE>(tacc, a, b, nsub, mt); break;
-          case 4: mma_stage<4, NT1, 8, 4 * (TM + 4), 4 * LDE>(tacc, a, b, nsub, mt); break;
           default: break;
         }
       }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty[buf]);       // stage (and its descriptor) released
       if (flags & STEP_LAST) {
-        const double sc = d.scale;
+        consumer_bar();                              // every warp is done reading the previous T chunk
         double* trow = Ts + (wr * 32 + g) * LDT + tile0 * 8 + 2 * t;
 #pragma unroll
         for (int ii = 0; ii < 4; ++ii)
@@ -316,6 +370,7 @@ __device__ void run_item(const DevWork& wk, const DevUnit* __restrict__ units, c
           for (int j = 0; j < NT1; ++j)
             if (ii < mt && j < nt1)
               *reinterpret_cast<double2*>(trow + ii * 8 * LDT + j * 8) = make_double2(sc * tacc[ii][j][0], sc * tacc[ii][j][1]);
+        consumer_bar();                              // the new T chunk is visible to every warp
       }
     } else {
       // ---- second product: acc (32 x 8 NT2 per warp) += T_chunk[:, step] D_tile^T ---------------
@@ -335,11 +390,10 @@ __device__ void run_item(const DevWork& wk, const DevUnit* __restrict__ units, c
           default: break;
         }
       }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty[buf]);
     }
-    if (++slot == RING) slot = 0;
-    if (++buf == NSTAGE) buf = 0;
   }
-  cp_async_wait<0>();
 
   // ---- epilogue: the tile leaves the registers once per work item -----------------------------
 #pragma unroll
@@ -362,20 +416,53 @@ heff_dmma_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __r
                  const DevTask* __restrict__ tasks, const double* __restrict__ psi, double* __restrict__ out,
                  double* __restrict__ partial, int* __restrict__ counter) {
   extern __shared__ __align__(16) double smem[];
-  __shared__ GenState st;
-  __shared__ StepDesc ring[RING];
-  __shared__ int s_w;
-  for (;;) {
-    __syncthreads();                       // previous item fully retired (smem, ring, s_w)
-    if (threadIdx.x == 0) s_w = atomicAdd(counter, 1);
-    __syncthreads();
-    const int w = s_w;
-    if (w >= nwork) break;
-    const DevWork wk = work[w];
-    double* dst = (wk.to_partial ? partial : out) + wk.dst_off;
-    if (wk.wr == 1) run_item<1>(wk, units, tasks, psi, dst, smem, st, ring);
-    else if (wk.wr == 2) run_item<2>(wk, units, tasks, psi, dst, smem, st, ring);
-    else run_item<4>(wk, units, tasks, psi, dst, smem, st, ring);
+  __shared__ GenState gs[NPRODUCERS];
+  __shared__ StepDesc ring[NSTAGE];
+  __shared__ __align__(8) uint64_t full[NSTAGE];
+  __shared__ __align__(8) uint64_t empty[NSTAGE];
+  __shared__ int s_w, s_base;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  if (tid == 0) {
+    for (int i = 0; i < NSTAGE; ++i) {
+      mbar_init(&full[i], 32 + 1);      // 32 deferred cp.async arrivals + the descriptor writer
+      mbar_init(&empty[i], NWARPS);     // one arrival per consumer warp
+    }
+    s_base = 0;
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  if (warp < NPRODUCERS) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 40;\n");
+    unsigned nfill = 0;                  // fills of this warp's stage buffer so far (mbarrier phase)
+#pragma unroll 1
+    for (;;) {
+      cta_bar();                         // previous item retired; s_base published
+      if (tid == 0) s_w = atomicAdd(counter, 1);
+      cta_bar();
+      const int w = s_w;
+      if (w >= nwork) break;
+      const DevWork wk = work[w];
+      const int first = (warp - s_base) & (NSTAGE - 1);
+      if (wk.wr == 1) producer_item<1>(wk, units, tasks, psi, smem, gs[warp], ring[warp], full, empty, warp, lane, first, nfill);
+      else if (wk.wr == 2) producer_item<2>(wk, units, tasks, psi, smem, gs[warp], ring[warp], full, empty, warp, lane, first, nfill);
+      else producer_item<4>(wk, units, tasks, psi, smem, gs[warp], ring[warp], full, empty, warp, lane, first, nfill);
+    }
+  } else {
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 232;\n");
+    unsigned ci = 0;                     // steps consumed so far: stage buffer = ci % NSTAGE, phase = ci / NSTAGE
+    const int cw = warp - NPRODUCERS;
+#pragma unroll 1
+    for (;;) {
+      cta_bar();
+      cta_bar();
+      const int w = s_w;
+      if (w >= nwork) break;
+      const DevWork wk = work[w];
+      double* dst = (wk.to_partial ? partial : out) + wk.dst_off;
+      if (wk.wr == 1) consumer_item<1>(wk, dst, smem, ring, full, empty, cw, lane, ci);
+      else if (wk.wr == 2) consumer_item<2>(wk, dst, smem, ring, full, empty, cw, lane, ci);
+      else consumer_item<4>(wk, dst, smem, ring, full, empty, cw, lane, ci);
+      if (tid == NPRODUCERS * 32) s_base = (int)(ci & (NSTAGE - 1));
+    }
   }
 }
 

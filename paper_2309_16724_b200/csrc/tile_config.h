@@ -1,7 +1,7 @@
 // Tiling of the fused DMMA GEMM-pair kernel; shared by the planner (choice of tile class per
 // output sector, segmentation, executed-flop count) and the kernels.
 //
-// A CTA (8 warps) owns a TM x TP tile of one output sector F_s and keeps it in registers as
+// A CTA (8 math warps + 4 load warps) owns a TM x TP tile of one output sector F_s and keeps it in registers as
 // m8n8 DMMA accumulators: warp (wr, wc) of a WR x WC warp grid owns rows [32 wr, 32 wr + 32) and
 // up to NT2 n8-tiles of columns.  Per position the first product T = A_pos[rows,:] E is formed in
 // column chunks of at most NC columns (warp tile 32 x 8 NT1), scaled by coef*alpha_pos and parked
@@ -11,22 +11,22 @@
 
 namespace su2 {
 
-constexpr int NTHREADS = 256;   // 8 warps
-constexpr int NWARPS = 8;
+constexpr int NWARPS = 8;              // consumer (math) warps: two warpgroups
+constexpr int NPRODUCERS = 4;          // producer (cp.async) warps: one warpgroup, one stage buffer each
+constexpr int NTHREADS = 32 * (NWARPS + NPRODUCERS);
 constexpr int KS = 8;           // k extent of one pipeline stage (two DMMA k4 steps)
-constexpr int NT1 = 4;          // n8-tiles per warp, first product
+constexpr int NT1 = 3;          // n8-tiles per warp, first product
 constexpr int NT2 = 9;          // n8-tiles per warp, second product
-constexpr int NSTAGE = 4;       // cp.async pipeline depth
+constexpr int NSTAGE = NPRODUCERS;     // pipeline depth
 
 template <int WR>
 struct TileCfg {
   static constexpr int WC = NWARPS / WR;        // warps along the columns
   static constexpr int TM = 32 * WR;            // rows of F per CTA          : 32 / 64 / 128
   static constexpr int TP = 8 * NT2 * WC;       // columns of F per CTA       : 576 / 288 / 144
-  static constexpr int NC = 8 * NT1 * WC;       // max columns of a T chunk   : 256 / 128 / 64
+  static constexpr int NC = 8 * NT1 * WC;       // max columns of a T chunk   : 192 / 96 / 48
   static constexpr int LDT = NC + 4;            // leading dimension of T in shared memory
-  // one pipeline stage (doubles).  A tile: c-major [2][TM][4] or k-major [2][4][TM+4];
-  // E tile: k-major [2][4][NC+4]; D tile: c-major [2][TP][4] or k-major [2][4][TP+4].
+  // one pipeline stage (doubles), every tile k-major [2 sub][4][C+4]: A tile C = TM, E tile C = NC, D tile C = TP.
   static constexpr int A_SZ = 2 * 4 * (TM + 4);
   static constexpr int E_SZ = 2 * 4 * (NC + 4);
   static constexpr int D_SZ = 2 * 4 * (TP + 4);
