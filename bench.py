@@ -99,7 +99,7 @@ def oracle_sample_problem(cfg_name, npos_sample):
     from gen import workloads as W
     from gen.problem import Problem
     c = W.CONFIGS[cfg_name]
-    full = W.synthetic_problem(c["L"], c["N"], c["twoS"], c["D"], xi=c["xi"], seed=0, fill=False)
+    full = W.synthetic_problem(c["L"], c["N"], c["twoS"], c["D"], xi=c["xi"], seed=0, fill=False, pos_cap=c.get("pos_cap"))
     keep = [t for t in full.term if t.name.split("^")[0] in ("A1P1", "B1Q1")]
     fam_l, fam_r, terms = [], [], []
     import copy
@@ -126,7 +126,7 @@ def time_oracle(cfg_name, steps, warmup, budget_s=20.0):
     from gen.workloads import random_psi
     from helpers import oracle_flat
     from paper_2309_16724_b200 import Plan
-    npos = {"cfg4": 1, "cfg3": 4, "cfg2": 16}.get(cfg_name, 16)
+    npos = {"cfg4": 1, "cfg4p": 1, "cfg3": 4, "cfg2": 16}.get(cfg_name, 16)
     prob = oracle_sample_problem(cfg_name, npos)
     plan = Plan(prob, host_only=True)
     x = random_psi(plan.psi_len, seed=0)
@@ -176,7 +176,7 @@ def build_operator(cfg_name, device):
     import torch
     from gen import workloads as W
     from paper_2309_16724_b200.runtime import HeffOperator
-    if cfg_name != "cfg4":
+    if cfg_name not in ("cfg4", "cfg4p"):
         prob = W.config_problem(cfg_name, seed=0, fill=True)
         return prob, HeffOperator(prob, device=device)
     prob = W.config_problem(cfg_name, seed=0, fill=False)

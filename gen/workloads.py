@@ -25,6 +25,9 @@ CONFIGS = {
     # small stand-ins of the same family for fast tests
     "mini": dict(L=8, N=8, twoS=0, D=24, xi=2.0),
     "midi": dict(L=12, N=12, twoS=0, D=64, xi=2.0),
+    # profiling stand-in for cfg4: the same sector tables and block sizes (69-547), but every operator
+    # family keeps only its first 24 positions, so that one apply takes ~1 s and fits an ncu replay
+    "cfg4p": dict(L=76, N=76, twoS=0, D=4096, xi=6.0, pos_cap=24),
 }
 
 TAG_T, TAG_V, TAG_PSI, TAG_ALPHA, TAG_OP = 1, 2, 3, 4, 16
@@ -158,7 +161,7 @@ def make_family(sec, dN, twoK, npos, seed, tag, name, symmetric=False, fill=True
     return fam
 
 
-def synthetic_problem(L, N, twoS, D, xi=2.0, seed=0, fill=True, site_terms=True, hermitian=True):
+def synthetic_problem(L, N, twoS, D, xi=2.0, seed=0, fill=True, site_terms=True, hermitian=True, pos_cap=None):
     """Random-operator problem at the middle bond with the row classes of SURVEY.md 8(c) C3:
     local, 1+3, 2+2 pair (A^S P~^S), 2+2 particle-hole (B^S Q^S), plus a few site-involving
     rows; every non-self-adjoint row is accompanied by its Hermitian conjugate (adjoint
@@ -171,6 +174,8 @@ def synthetic_problem(L, N, twoS, D, xi=2.0, seed=0, fill=True, site_terms=True,
     sid = {o.name: i for i, o in enumerate(site)}
     pairs_le = [(i, j) for i in range(nl) for j in range(i, nl)]
     pairs_lt = [(i, j) for i in range(nl) for j in range(i + 1, nl)]
+    if pos_cap is not None:
+        pairs_le, pairs_lt = pairs_le[:pos_cap], pairs_lt[:pos_cap]
 
     fam_l, fam_r, terms = [], [], []
 
@@ -265,7 +270,7 @@ def synthetic_problem(L, N, twoS, D, xi=2.0, seed=0, fill=True, site_terms=True,
 
 def config_problem(name, seed=0, fill=True):
     c = CONFIGS[name]
-    return synthetic_problem(c["L"], c["N"], c["twoS"], c["D"], xi=c["xi"], seed=seed, fill=fill)
+    return synthetic_problem(c["L"], c["N"], c["twoS"], c["D"], xi=c["xi"], seed=seed, fill=fill, pos_cap=c.get("pos_cap"))
 
 
 def random_psi(psi_len, seed=0):

@@ -158,10 +158,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, int parity) {
 __device__ __forceinline__ void cp_async_mbar_arrive(uint64_t* bar) {
   asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void cp_async8(double* smem_dst, const double* src, bool valid) {
-  const int sz = valid ? 8 : 0;   // src-size 0: destination is zero-filled, nothing is read
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(smem_u32(smem_dst)), "l"(src), "r"(sz) : "memory");
-}
 __device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, 256;\n" ::: "memory"); }
 __device__ __forceinline__ void cta_bar() { asm volatile("bar.sync 0, 384;\n" ::: "memory"); }
 static_assert(NTHREADS == 384 && NWARPS * 32 == 256, "barrier thread counts are spelled out in the PTX above");
@@ -170,20 +166,32 @@ static_assert(NTHREADS == 384 && NWARPS * 32 == 256, "barrier thread counts are 
 // Every tile lands in the same shared-memory layout, [j/4][j%4][c] with row stride CT+4 doubles
 // (k-major k4 sub-tiles; CT+4 = 4 mod 8 makes the DMMA fragment loads conflict-free), so the math
 // code does not depend on how the operator block is stored.
+// The copy loops are written with running addresses (one LDGSTS + two adds per element): a single
+// producer warp has to issue a whole tile, so its instruction count is what bounds the pipeline.
+__device__ __forceinline__ void cp_async8_raw(unsigned dst, const void* src, int sz) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(dst), "l"(src), "r"(sz) : "memory");
+}
 // Source stored c-major, element (c, j) = src[c*ld + j]: 8 consecutive lanes read one 64-byte run.
 template <int CT>
 __device__ __forceinline__ void copy_cmajor(double* dst, const double* __restrict__ src, int ld, int cval, int jval, int lane) {
-  const int cpad = (cval + 7) & ~7;
-  const int jpad = jval > 4 ? 8 : 4;
-  const int j = lane & 7;
-  if (j >= jpad) return;
-  double* d = dst + (j >> 2) * (4 * (CT + 4)) + (j & 3) * (CT + 4);
-  const bool jok = j < jval;
-  const double* s = src + j;
+  const int j = lane & 7, r = lane >> 3;
+  if (j >= (jval > 4 ? 8 : 4)) return;
+  unsigned d = smem_u32(dst + (j >> 2) * (4 * (CT + 4)) + (j & 3) * (CT + 4) + r);
+  const char* s = reinterpret_cast<const char*>(src + (int64_t)r * ld + j);
+  const int64_t sstep = (int64_t)ld * 32;            // four rows further
+  const int szj = j < jval ? 8 : 0;
+  const int ntot = ((cval + 7) & ~7) >> 2;           // iterations up to the padded extent
+  const int nfull = min(ntot, max(0, (cval - r + 3) >> 2));
+  int i = 0;
 #pragma unroll 4
-  for (int c = lane >> 3; c < cpad; c += 4) {
-    const bool ok = jok && c < cval;
-    cp_async8(d + c, ok ? s + (int64_t)c * ld : src, ok);
+  for (; i < nfull; ++i) {
+    cp_async8_raw(d, s, szj);
+    d += 32;
+    s += sstep;
+  }
+  for (; i < ntot; ++i) {                            // rows beyond the block: zero fill
+    cp_async8_raw(d, src, 0);
+    d += 32;
   }
 }
 // Source stored k-major, element (c, j) = src[j*ld + c]: a warp reads one 256-byte run.
@@ -191,15 +199,19 @@ template <int CT>
 __device__ __forceinline__ void copy_kmajor(double* dst, const double* __restrict__ src, int ld, int cval, int jval, int lane) {
   const int cpad = (cval + 7) & ~7;
   const int jpad = jval > 4 ? 8 : 4;
+#pragma unroll 1
   for (int j = 0; j < jpad; ++j) {
-    double* d = dst + (j >> 2) * (4 * (CT + 4)) + (j & 3) * (CT + 4);
-    const double* s = src + (int64_t)j * ld;
-    const bool jok = j < jval;
+    unsigned d = smem_u32(dst + (j >> 2) * (4 * (CT + 4)) + (j & 3) * (CT + 4) + lane);
+    const char* s = reinterpret_cast<const char*>(src + (int64_t)j * ld + lane);
+    const int szj = j < jval ? 8 : 0;
+    int c = lane;
 #pragma unroll 4
-    for (int c = lane; c < cpad; c += 32) {
-      const bool ok = jok && c < cval;
-      cp_async8(d + c, ok ? s + c : src, ok);
+    for (; c < cval; c += 32) {
+      cp_async8_raw(d, s, szj);
+      d += 256;
+      s += 256;
     }
+    if (c < cpad) cp_async8_raw(d, src, 0);          // at most one padded element per lane
   }
 }
 
@@ -241,11 +253,13 @@ __device__ __forceinline__ void mma_stage(double (&c)[4][NACC][2], const double*
 }
 
 // ---- producer warp w: owns stage buffer w and the item's steps  l  with (base + l) % NSTAGE == w --------
+// Descriptors are double-buffered per stage (ring[fill parity][w]): the descriptor of the next fill
+// is generated while the current fill is in flight, off the critical path of the buffer hand-over.
 template <int WR>
 __device__ __forceinline__ void producer_item(const DevWork& wk, const DevUnit* __restrict__ units,
                                               const DevTask* __restrict__ tasks, const double* __restrict__ psi,
-                                              double* smem, GenState& st, StepDesc& desc, uint64_t* full, uint64_t* empty,
-                                              int w, int lane, int first, unsigned& nfill) {
+                                              double* smem, GenState& st, StepDesc (*ring)[NSTAGE], uint64_t* full,
+                                              uint64_t* empty, int w, int lane, int first, unsigned& nfill) {
   using C = TileCfg<WR>;
   double* stage = smem + C::TM * C::LDT + w * C::STAGE;
   if (lane == 0) {
@@ -257,17 +271,15 @@ __device__ __forceinline__ void producer_item(const DevWork& wk, const DevUnit* 
     if (st.u < st.u_end) gen_load_unit(st, units, tasks, psi);
     else st.done = 1;
     for (int i = 0; i < first; ++i) gen_advance(st, units, tasks, psi);
+    gen_fill(st, ring[nfill & 1u][w]);
+#pragma unroll 1
+    for (int i = 0; i < NSTAGE; ++i) gen_advance(st, units, tasks, psi);
   }
-  __syncwarp();
 #pragma unroll 1
   for (;;) {
+    __syncwarp();                                       // descriptor of this fill is visible to the warp
+    const StepDesc& desc = ring[nfill & 1u][w];
     mbar_wait(&empty[w], (int)((nfill & 1u) ^ 1u));     // consumers have released the previous fill of this buffer
-    if (lane == 0) {
-      gen_fill(st, desc);
-#pragma unroll 1
-      for (int i = 0; i < NSTAGE; ++i) gen_advance(st, units, tasks, psi);
-    }
-    __syncwarp();
     const int flags = desc.flags;
     if (!(flags & STEP_END)) {
       const double* src0 = desc.src0;
@@ -286,13 +298,18 @@ __device__ __forceinline__ void producer_item(const DevWork& wk, const DevUnit* 
     if (lane == 0) mbar_arrive(&full[w]);    // +1 (release): the descriptor is visible
     ++nfill;
     if (flags & STEP_END) break;
+    if (lane == 0) {                         // next descriptor, while this fill is in flight
+      gen_fill(st, ring[nfill & 1u][w]);
+#pragma unroll 1
+      for (int i = 0; i < NSTAGE; ++i) gen_advance(st, units, tasks, psi);
+    }
   }
 }
 
 // ---- consumer warp cw = (wr, wc): LDS + DMMA only -------------------------------------------------------
 template <int WR>
 __device__ __forceinline__ void consumer_item(const DevWork& wk, double* __restrict__ dst, double* smem,
-                                              const StepDesc* ring, uint64_t* full, uint64_t* empty, int cw, int lane,
+                                              const StepDesc (*ring)[NSTAGE], uint64_t* full, uint64_t* empty, int cw, int lane,
                                               unsigned& ci) {
   using C = TileCfg<WR>;
   constexpr int WC = C::WC, TM = C::TM, TP = C::TP, NC = C::NC, LDT = C::LDT, LDE = NC + 4;
@@ -324,9 +341,10 @@ __device__ __forceinline__ void consumer_item(const DevWork& wk, double* __restr
 #pragma unroll 1
   for (;;) {
     const int buf = (int)(ci & (NSTAGE - 1));
-    mbar_wait(&full[buf], (int)((ci >> 2) & 1u));
+    const unsigned par = (ci >> 2) & 1u;
+    mbar_wait(&full[buf], (int)par);
     ++ci;
-    const StepDesc& d = ring[buf];
+    const StepDesc& d = ring[par][buf];
     const int flags = d.flags;
     if (flags & STEP_END) {
       __syncwarp();
@@ -417,7 +435,7 @@ heff_dmma_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __r
                  double* __restrict__ partial, int* __restrict__ counter) {
   extern __shared__ __align__(16) double smem[];
   __shared__ GenState gs[NPRODUCERS];
-  __shared__ StepDesc ring[NSTAGE];
+  __shared__ StepDesc ring[2][NSTAGE];
   __shared__ __align__(8) uint64_t full[NSTAGE];
   __shared__ __align__(8) uint64_t empty[NSTAGE];
   __shared__ int s_w, s_base;
@@ -442,9 +460,9 @@ heff_dmma_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __r
       if (w >= nwork) break;
       const DevWork wk = work[w];
       const int first = (warp - s_base) & (NSTAGE - 1);
-      if (wk.wr == 1) producer_item<1>(wk, units, tasks, psi, smem, gs[warp], ring[warp], full, empty, warp, lane, first, nfill);
-      else if (wk.wr == 2) producer_item<2>(wk, units, tasks, psi, smem, gs[warp], ring[warp], full, empty, warp, lane, first, nfill);
-      else producer_item<4>(wk, units, tasks, psi, smem, gs[warp], ring[warp], full, empty, warp, lane, first, nfill);
+      if (wk.wr == 1) producer_item<1>(wk, units, tasks, psi, smem, gs[warp], ring, full, empty, warp, lane, first, nfill);
+      else if (wk.wr == 2) producer_item<2>(wk, units, tasks, psi, smem, gs[warp], ring, full, empty, warp, lane, first, nfill);
+      else producer_item<4>(wk, units, tasks, psi, smem, gs[warp], ring, full, empty, warp, lane, first, nfill);
     }
   } else {
     asm volatile("setmaxnreg.inc.sync.aligned.u32 232;\n");
