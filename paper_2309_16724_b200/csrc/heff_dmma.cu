@@ -38,33 +38,39 @@ namespace {
 
 enum : int { STEP_END = 1, STEP_G2 = 2, STEP_TRANS = 4, STEP_FIRST = 8, STEP_LAST = 16 };
 
-struct StepDesc {
-  const double* src0;   // first product: A tile origin;  second product: D tile origin
-  const double* src1;   // first product: E tile origin
-  double scale;         // coef * alpha_pos, applied when the last first-product step parks T
+enum : int { PH_END = 1, PH_G2 = 2, PH_TRANS = 4 };
+
+// One *phase* = a run of pipeline steps with regular addressing: the first product of one
+// (task, position, T-chunk) -- nsteps stages of an A tile and an E tile, KS deep -- or its second
+// product -- nsteps stages of a D tile.  Step s reads src + s * stride; both producers and consumers
+// derive everything else (valid k extent, first/last flags) from s in registers.
+struct PhaseDesc {
+  const double* src0;   // first product: A tile origin of step 0;  second product: D tile origin
+  const double* src1;   // first product: E tile origin of step 0
+  double scale;         // coef * alpha_pos, applied when the first product parks T
+  int stride0, stride1; // elements between consecutive steps
   int ld0, ld1;         // global leading dimensions
   int cval0;            // valid extent of tile 0 along c (rows of A / columns of F)
   int cval1;            // valid columns of the E tile (= width of the T chunk)
-  int jval;             // valid extent along k (<= KS)
-  int s;                // step index inside its phase
+  int ktot;             // total k extent of the phase (k, or the chunk width)
+  int nsteps;
   int flags;
   int pad;
 };
+constexpr int PHASE_RING = 16;  // producers run at most MAX_STAGE = 8 steps (hence phases) ahead of the consumers and write one more
 
-struct GenState {       // iterator over the steps of one work item (one per producer warp, in shared memory)
+struct GenState {       // iterator over the phases of one work item (shared memory; advanced by one thread)
   const double *A, *D, *E, *alpha;
   double coef, scale;
   int m, k, n, p, strideA, strideD, tflags;
-  int u, u_end, pos, pos_end, chunk, nchunks, ncw_full, n0, ncw, phase, s, nsteps1, nsteps2, done;
+  int u, u_end, pos, pos_end, chunk, nchunks, ncw_full, n0, ncw, phase, done;
   int row0, col0, rows_valid, cols_valid, nc_max;
 };
 
 __device__ __forceinline__ void gen_set_chunk(GenState& st) {
   st.n0 = st.chunk * st.ncw_full;
   st.ncw = min(st.ncw_full, st.n - st.n0);
-  st.nsteps2 = (st.ncw + KS - 1) / KS;
   st.phase = 0;
-  st.s = 0;
 }
 __device__ __forceinline__ void gen_set_pos(GenState& st) {
   st.scale = st.coef * (st.alpha ? st.alpha[st.pos] : 1.0);
@@ -79,56 +85,48 @@ __device__ __forceinline__ void gen_load_unit(GenState& st, const DevUnit* __res
   st.m = t.m; st.k = t.k; st.n = t.n; st.p = t.p;
   st.strideA = t.strideA; st.strideD = t.strideD; st.tflags = (int)t.flags;
   st.pos = un.pos0; st.pos_end = un.pos1;
-  st.nsteps1 = (t.k + KS - 1) / KS;
   chunking(t.n, st.nc_max, st.nchunks, st.ncw_full);
   gen_set_pos(st);
 }
 
-// Move the iterator to the next step.
-__device__ __forceinline__ void gen_advance(GenState& st, const DevUnit* __restrict__ units,
-                                            const DevTask* __restrict__ tasks, const double* __restrict__ psi) {
-  if (st.done) return;
-  ++st.s;
+// Emit the descriptor of the current phase and move to the next one.
+__device__ __forceinline__ void gen_phase(GenState& st, PhaseDesc& d, const DevUnit* __restrict__ units,
+                                          const DevTask* __restrict__ tasks, const double* __restrict__ psi) {
+  if (st.done) {
+    d.flags = PH_END;
+    d.nsteps = 1;
+    return;
+  }
   if (st.phase == 0) {
-    if (st.s == st.nsteps1) { st.phase = 1; st.s = 0; }
-  } else if (st.s == st.nsteps2) {
+    const bool tr = st.tflags & TASK_TRANS_A;
+    d.src0 = st.A + (int64_t)st.pos * st.strideA + (tr ? (int64_t)st.row0 : (int64_t)st.row0 * st.k);
+    d.stride0 = tr ? KS1 * st.m : KS1;
+    d.ld0 = tr ? st.m : st.k;
+    d.src1 = st.E + st.n0;
+    d.stride1 = KS1 * st.n;
+    d.ld1 = st.n;
+    d.cval0 = st.rows_valid;
+    d.cval1 = st.ncw;
+    d.ktot = st.k;
+    d.nsteps = (st.k + KS1 - 1) / KS1;
+    d.scale = st.scale;
+    d.flags = tr ? PH_TRANS : 0;
+    st.phase = 1;
+  } else {
+    const bool tr = st.tflags & TASK_TRANS_D;
+    d.src0 = st.D + (int64_t)st.pos * st.strideD +
+             (tr ? (int64_t)st.n0 * st.p + st.col0 : (int64_t)st.col0 * st.n + st.n0);
+    d.stride0 = tr ? KS2 * st.p : KS2;
+    d.ld0 = tr ? st.p : st.n;
+    d.cval0 = st.cols_valid;
+    d.cval1 = 0;
+    d.ktot = st.ncw;
+    d.nsteps = (st.ncw + KS2 - 1) / KS2;
+    d.flags = PH_G2 | (tr ? PH_TRANS : 0);
     if (++st.chunk < st.nchunks) gen_set_chunk(st);
     else if (++st.pos < st.pos_end) gen_set_pos(st);
     else if (++st.u < st.u_end) gen_load_unit(st, units, tasks, psi);
     else st.done = 1;
-  }
-}
-
-// Descriptor of the current step.
-__device__ __forceinline__ void gen_fill(const GenState& st, StepDesc& d) {
-  if (st.done) {
-    d.flags = STEP_END;
-    return;
-  }
-  if (st.phase == 0) {
-    const int k0 = st.s * KS;
-    const bool tr = st.tflags & TASK_TRANS_A;
-    d.src0 = st.A + (int64_t)st.pos * st.strideA +
-             (tr ? (int64_t)k0 * st.m + st.row0 : (int64_t)st.row0 * st.k + k0);
-    d.ld0 = tr ? st.m : st.k;
-    d.src1 = st.E + (int64_t)k0 * st.n + st.n0;
-    d.ld1 = st.n;
-    d.cval0 = st.rows_valid;
-    d.cval1 = st.ncw;
-    d.jval = min(KS, st.k - k0);
-    d.s = st.s;
-    d.scale = st.scale;
-    d.flags = (tr ? STEP_TRANS : 0) | (st.s == 0 ? STEP_FIRST : 0) | (st.s == st.nsteps1 - 1 ? STEP_LAST : 0);
-  } else {
-    const int j0 = st.n0 + st.s * KS;
-    const bool tr = st.tflags & TASK_TRANS_D;
-    d.src0 = st.D + (int64_t)st.pos * st.strideD +
-             (tr ? (int64_t)j0 * st.p + st.col0 : (int64_t)st.col0 * st.n + j0);
-    d.ld0 = tr ? st.p : st.n;
-    d.cval0 = st.cols_valid;
-    d.jval = min(KS, st.ncw - st.s * KS);
-    d.s = st.s;
-    d.flags = STEP_G2 | (tr ? STEP_TRANS : 0);
   }
 }
 
@@ -162,45 +160,47 @@ __device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, 256;\
 __device__ __forceinline__ void cta_bar() { asm volatile("bar.sync 0, 384;\n" ::: "memory"); }
 static_assert(NTHREADS == 384 && NWARPS * 32 == 256, "barrier thread counts are spelled out in the PTX above");
 
-// ---- staging: one producer WARP copies a whole tile ---------------------------------------------
+__device__ __forceinline__ void producer_bar() { asm volatile("bar.sync 2, 128;\n" ::: "memory"); }
+
+// ---- staging: the four producer warps copy a quarter of every tile each ---------------------------
 // Every tile lands in the same shared-memory layout, [j/4][j%4][c] with row stride CT+4 doubles
 // (k-major k4 sub-tiles; CT+4 = 4 mod 8 makes the DMMA fragment loads conflict-free), so the math
-// code does not depend on how the operator block is stored.
-// The copy loops are written with running addresses (one LDGSTS + two adds per element): a single
-// producer warp has to issue a whole tile, so its instruction count is what bounds the pipeline.
+// code does not depend on how the operator block is stored.  8-byte cp.async with zero fill: ragged
+// block sizes and odd leading dimensions need no special cases.
+// The copy loops are written with running addresses (one LDGSTS + two adds per element).
 __device__ __forceinline__ void cp_async8_raw(unsigned dst, const void* src, int sz) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(dst), "l"(src), "r"(sz) : "memory");
 }
-// Source stored c-major, element (c, j) = src[c*ld + j]: 8 consecutive lanes read one 64-byte run.
+// Source stored c-major, element (c, j) = src[c*ld + j]: 8 consecutive lanes read one 64-byte run, a warp
+// instruction covers 4 rows; producer warp w takes the row groups  c/4 = w (mod 4).
 template <int CT>
-__device__ __forceinline__ void copy_cmajor(double* dst, const double* __restrict__ src, int ld, int cval, int jval, int lane) {
-  const int j = lane & 7, r = lane >> 3;
-  if (j >= (jval > 4 ? 8 : 4)) return;
+__device__ __forceinline__ void copy_cmajor(double* dst, const double* __restrict__ src, int ld, int cval, int jval,
+                                            int w, int lane) {
+  const int j = lane & 7, r = 4 * w + (lane >> 3);
+  if (j >= ((jval + 3) & ~3)) return;
   unsigned d = smem_u32(dst + (j >> 2) * (4 * (CT + 4)) + (j & 3) * (CT + 4) + r);
   const char* s = reinterpret_cast<const char*>(src + (int64_t)r * ld + j);
-  const int64_t sstep = (int64_t)ld * 32;            // four rows further
+  const int64_t sstep = (int64_t)ld * 128;           // sixteen rows further
   const int szj = j < jval ? 8 : 0;
-  const int ntot = ((cval + 7) & ~7) >> 2;           // iterations up to the padded extent
-  const int nfull = min(ntot, max(0, (cval - r + 3) >> 2));
-  int i = 0;
-#pragma unroll 4
-  for (; i < nfull; ++i) {
+  const int cpad = (cval + 7) & ~7;
+  int c = r;
+#pragma unroll 2
+  for (; c < cval; c += 16) {
     cp_async8_raw(d, s, szj);
-    d += 32;
+    d += 128;
     s += sstep;
   }
-  for (; i < ntot; ++i) {                            // rows beyond the block: zero fill
-    cp_async8_raw(d, src, 0);
-    d += 32;
-  }
+  if (c < cpad) cp_async8_raw(d, src, 0);            // rows beyond the block (fewer than 8): zero fill
 }
-// Source stored k-major, element (c, j) = src[j*ld + c]: a warp reads one 256-byte run.
+// Source stored k-major, element (c, j) = src[j*ld + c]: a warp reads one 256-byte run; producer warp w
+// takes the k rows j = w and w + 4.
 template <int CT>
-__device__ __forceinline__ void copy_kmajor(double* dst, const double* __restrict__ src, int ld, int cval, int jval, int lane) {
+__device__ __forceinline__ void copy_kmajor(double* dst, const double* __restrict__ src, int ld, int cval, int jval,
+                                            int w, int lane) {
   const int cpad = (cval + 7) & ~7;
-  const int jpad = jval > 4 ? 8 : 4;
+  const int jpad = (jval + 3) & ~3;
 #pragma unroll 1
-  for (int j = 0; j < jpad; ++j) {
+  for (int j = w; j < jpad; j += 4) {
     unsigned d = smem_u32(dst + (j >> 2) * (4 * (CT + 4)) + (j & 3) * (CT + 4) + lane);
     const char* s = reinterpret_cast<const char*>(src + (int64_t)j * ld + lane);
     const int szj = j < jval ? 8 : 0;
@@ -221,15 +221,15 @@ __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
       : "d"(a), "d"(b));
 }
 
-// One pipeline stage (nsub k4 sub-steps) of a warp-level product: c[ii][j] += A_frag[ii] B_frag[j]
+// One pipeline stage (nsub <= NSUB k4 sub-steps) of a warp-level product: c[ii][j] += A_frag[ii] B_frag[j]
 // for 4 m8-tiles (the first mt active) and NT n8-tiles.  a / b point at this lane's element of the
 // first fragment; A_I / A_SUB / B_SUB are the compile-time strides between m8-tiles / k4 sub-steps
 // (n8-tiles are 8 doubles apart).
-template <int NT, int NACC, int A_I, int A_SUB, int B_SUB>
+template <int NSUB, int NT, int NACC, int A_I, int A_SUB, int B_SUB>
 __device__ __forceinline__ void mma_stage(double (&c)[4][NACC][2], const double* __restrict__ a,
                                           const double* __restrict__ b, int nsub, int mt) {
 #pragma unroll
-  for (int sub = 0; sub < 2; ++sub) {
+  for (int sub = 0; sub < NSUB; ++sub) {
     if (sub < nsub) {
       double af[4], bf[NT];
 #pragma unroll
@@ -252,17 +252,20 @@ __device__ __forceinline__ void mma_stage(double (&c)[4][NACC][2], const double*
   }
 }
 
-// ---- producer warp w: owns stage buffer w and the item's steps  l  with (base + l) % NSTAGE == w --------
-// Descriptors are double-buffered per stage (ring[fill parity][w]): the descriptor of the next fill
-// is generated while the current fill is in flight, off the critical path of the buffer hand-over.
+
+// ---- producer warps: all four walk every step and copy a quarter of its tiles -------------------------
+// Warp 0 / lane 0 also runs the phase iterator, one phase ahead, into the descriptor ring.
 template <int WR>
-__device__ __forceinline__ void producer_item(const DevWork& wk, const DevUnit* __restrict__ units,
+__device__ __forceinline__ void producer_item(const DevWork* __restrict__ wkp, const DevUnit* __restrict__ units,
                                               const DevTask* __restrict__ tasks, const double* __restrict__ psi,
-                                              double* smem, GenState& st, StepDesc (*ring)[NSTAGE], uint64_t* full,
-                                              uint64_t* empty, int w, int lane, int first, unsigned& nfill) {
+                                              double* smem, GenState& st, PhaseDesc* pring, uint64_t* full,
+                                              uint64_t* empty, int w, int lane) {
   using C = TileCfg<WR>;
-  double* stage = smem + C::TM * C::LDT + w * C::STAGE;
-  if (lane == 0) {
+  constexpr int NS = C::NSTAGE;
+  double* stages = smem + C::TM * C::LDT;
+  const bool gen = (w == 0 && lane == 0);
+  if (gen) {
+    const DevWork wk = *wkp;
     st.u = wk.unit0; st.u_end = wk.unit1; st.done = 0;
     st.row0 = wk.row0; st.col0 = wk.col0;
     st.rows_valid = min(C::TM, wk.m - wk.row0);
@@ -270,61 +273,96 @@ __device__ __forceinline__ void producer_item(const DevWork& wk, const DevUnit* 
     st.nc_max = C::NC;
     if (st.u < st.u_end) gen_load_unit(st, units, tasks, psi);
     else st.done = 1;
-    for (int i = 0; i < first; ++i) gen_advance(st, units, tasks, psi);
-    gen_fill(st, ring[nfill & 1u][w]);
-#pragma unroll 1
-    for (int i = 0; i < NSTAGE; ++i) gen_advance(st, units, tasks, psi);
+    gen_phase(st, pring[0], units, tasks, psi);
   }
+  unsigned pq = 0;
+  int b = 0, par = 0;                                  // stage buffer and its fill parity
 #pragma unroll 1
   for (;;) {
-    __syncwarp();                                       // descriptor of this fill is visible to the warp
-    const StepDesc& desc = ring[nfill & 1u][w];
-    mbar_wait(&empty[w], (int)((nfill & 1u) ^ 1u));     // consumers have released the previous fill of this buffer
-    const int flags = desc.flags;
-    if (!(flags & STEP_END)) {
-      const double* src0 = desc.src0;
-      const int ld0 = desc.ld0, cval0 = desc.cval0, jval = desc.jval;
-      if (!(flags & STEP_G2)) {
-        if (flags & STEP_TRANS) copy_kmajor<C::TM>(stage, src0, ld0, cval0, jval, lane);
-        else copy_cmajor<C::TM>(stage, src0, ld0, cval0, jval, lane);
-        copy_kmajor<C::NC>(stage + C::A_SZ, desc.src1, desc.ld1, desc.cval1, jval, lane);
-      } else {
-        if (flags & STEP_TRANS) copy_kmajor<C::TP>(stage, src0, ld0, cval0, jval, lane);
-        else copy_cmajor<C::TP>(stage, src0, ld0, cval0, jval, lane);
-      }
-    }
-    cp_async_mbar_arrive(&full[w]);          // 32 deferred arrivals: this lane's copies have landed
-    __syncwarp();
-    if (lane == 0) mbar_arrive(&full[w]);    // +1 (release): the descriptor is visible
-    ++nfill;
-    if (flags & STEP_END) break;
-    if (lane == 0) {                         // next descriptor, while this fill is in flight
-      gen_fill(st, ring[nfill & 1u][w]);
+    producer_bar();                                     // descriptor pq is visible to the four producer warps
+    // Phase constants are re-read from shared memory every step (volatile: LDS, ~30 cycles) instead of
+    // being held in the 56 producer registers, where they would spill to local memory.
+    const volatile PhaseDesc& d = pring[pq & (PHASE_RING - 1)];
+    const int flags = d.flags, nsteps = d.nsteps;
 #pragma unroll 1
-      for (int i = 0; i < NSTAGE; ++i) gen_advance(st, units, tasks, psi);
+    for (int s = 0; s < nsteps; ++s) {
+      mbar_wait(&empty[b], par ^ 1);                    // consumers have released the previous fill
+      if (!(flags & PH_END)) {
+        double* stage = stages + b * C::STAGE;
+        const double* src0 = d.src0 + (int64_t)s * d.stride0;
+        if (!(flags & PH_G2)) {
+          const int jval = min(KS1, d.ktot - s * KS1);
+          if (flags & PH_TRANS) {
+            copy_kmajor<C::TM>(stage, src0, d.ld0, d.cval0, jval, w, lane);
+          } else {
+            copy_cmajor<C::TM>(stage, src0, d.ld0, d.cval0, jval, w, lane);
+            if (jval > 8) copy_cmajor<C::TM>(stage + 8 * (C::TM + 4), src0 + 8, d.ld0, d.cval0, jval - 8, w, lane);
+          }
+          copy_kmajor<C::NC>(stage + C::A_SZ, d.src1 + (int64_t)s * d.stride1, d.ld1, d.cval1, jval, w, lane);
+        } else {
+          const int jval = min(KS2, d.ktot - s * KS2);
+          if (flags & PH_TRANS) copy_kmajor<C::TP>(stage, src0, d.ld0, d.cval0, jval, w, lane);
+          else copy_cmajor<C::TP>(stage, src0, d.ld0, d.cval0, jval, w, lane);
+        }
+      }
+      cp_async_mbar_arrive(&full[b]);          // 128 deferred arrivals: this lane's copies have landed
+      if (w == 0) {
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&full[b]);  // +1 (release): the phase descriptor is visible
+      }
+      if (++b == NS) { b = 0; par ^= 1; }
+      if (s == 0 && gen && !(flags & PH_END))  // next phase's descriptor, while this step is in flight
+        gen_phase(st, pring[(pq + 1) & (PHASE_RING - 1)], units, tasks, psi);
     }
+    if (flags & PH_END) break;
+    ++pq;
   }
 }
 
-// ---- consumer warp cw = (wr, wc): LDS + DMMA only -------------------------------------------------------
+// ---- consumer warps: LDS + DMMA only ------------------------------------------------------------------
+// All steps of one phase for one warp: wait for the stage, multiply, release the stage.
+// G2 = false: A fragments come from the stage (a_off inside it); G2 = true: from T (a_off + s*KS).
+template <int NS, int STAGE, bool G2, int NT, int NACC, int A_I, int A_SUB, int B_SUB>
+__device__ __forceinline__ void run_phase(double (&c)[4][NACC][2], const double* stages, const double* Ts, int a_off,
+                                          int b_off, int nsteps, int ktot, int mt, int& b, int& par, uint64_t* full,
+                                          uint64_t* empty, int lane) {
+  constexpr int KSX = G2 ? KS2 : KS1;
+#pragma unroll 1
+  for (int s = 0; s < nsteps; ++s) {
+    if (s > 0) mbar_wait(&full[b], par);                        // step 0 was awaited by the caller
+    if (NT > 0 && mt > 0) {
+      const double* stage = stages + b * STAGE;
+      const double* a = G2 ? Ts + a_off + s * KSX : stage + a_off;
+      const int nsub = (min(KSX, ktot - s * KSX) + 3) >> 2;
+      mma_stage<KSX / 4, (NT > 0 ? NT : 1), NACC, A_I, A_SUB, B_SUB>(c, a, stage + b_off, nsub, mt);
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[b]);                      // stage released
+    if (++b == NS) { b = 0; par ^= 1; }
+  }
+}
+
 template <int WR>
-__device__ __forceinline__ void consumer_item(const DevWork& wk, double* __restrict__ dst, double* smem,
-                                              const StepDesc (*ring)[NSTAGE], uint64_t* full, uint64_t* empty, int cw, int lane,
-                                              unsigned& ci) {
+__device__ __forceinline__ void consumer_item(const DevWork* __restrict__ wkp, double* __restrict__ out,
+                                              double* __restrict__ partial, double* smem, const PhaseDesc* pring,
+                                              uint64_t* full, uint64_t* empty, int cw, int lane) {
   using C = TileCfg<WR>;
-  constexpr int WC = C::WC, TM = C::TM, TP = C::TP, NC = C::NC, LDT = C::LDT, LDE = NC + 4;
+  constexpr int WC = C::WC, TM = C::TM, TP = C::TP, NC = C::NC, LDT = C::LDT, LDE = NC + 4, NS = C::NSTAGE, ST = C::STAGE;
   const int g = lane >> 2, t = lane & 3;
   const int wr = cw / WC, wc = cw % WC;
   double* Ts = smem;
   const double* stages = smem + TM * LDT;
 
-  const int rows_valid = min(TM, wk.m - wk.row0);
-  const int cols_valid = min(TP, wk.p - wk.col0);
+  const int rows_valid = min(TM, wkp->m - wkp->row0);
+  const int cols_valid = min(TP, wkp->p - wkp->col0);
   const int mt = max(0, min(4, (rows_valid - wr * 32 + 7) >> 3));          // active m8-tiles of this warp
   const int ntiles2 = (cols_valid + 7) >> 3;
   const int ntw2 = (ntiles2 + WC - 1) / WC;
   const int ctile0 = wc * ntw2;
   const int nt2 = max(0, min(ntw2, ntiles2 - ctile0));                     // active n8-tiles (second product)
+  const int a1_off = t * (TM + 4) + wr * 32 + g;                            // A fragment inside a stage
+  const int t_off = (wr * 32 + g) * LDT + t;                                // A fragment of the second product inside T
+  const int d_off = t * (TP + 4) + ctile0 * 8 + g;                          // D fragment inside a stage
 
   double acc[4][NT2][2];
   double tacc[4][NT1][2];
@@ -332,88 +370,67 @@ __device__ __forceinline__ void consumer_item(const DevWork& wk, double* __restr
   for (int i = 0; i < 4; ++i)
 #pragma unroll
     for (int j = 0; j < NT2; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-#pragma unroll
-  for (int i = 0; i < 4; ++i)
-#pragma unroll
-    for (int j = 0; j < NT1; ++j) tacc[i][j][0] = tacc[i][j][1] = 0.0;
 
-  int ends = 0;
+  unsigned cq = 0;
+  int b = 0, par = 0;                                    // stage buffer and its fill parity
 #pragma unroll 1
   for (;;) {
-    const int buf = (int)(ci & (NSTAGE - 1));
-    const unsigned par = (ci >> 2) & 1u;
-    mbar_wait(&full[buf], (int)par);
-    ++ci;
-    const StepDesc& d = ring[par][buf];
-    const int flags = d.flags;
-    if (flags & STEP_END) {
+    mbar_wait(&full[b], par);                            // first step of the phase: its descriptor is visible too
+    const PhaseDesc& d = pring[cq & (PHASE_RING - 1)];
+    const int flags = d.flags, nsteps = d.nsteps, ktot = d.ktot;
+    if (flags & PH_END) {
       __syncwarp();
-      if (lane == 0) mbar_arrive(&empty[buf]);
-      if (++ends == NSTAGE) break;
-      continue;
+      if (lane == 0) mbar_arrive(&empty[b]);
+      break;
     }
-    const double* stage = stages + buf * C::STAGE;
-    const int nsub = d.jval > 4 ? 2 : 1;
-    if (!(flags & STEP_G2)) {
-      // ---- first product: tacc (32 x 8 NT1 per warp) += A_tile E_tile --------------------------
+    if (!(flags & PH_G2)) {
+      // ---- first product: tacc (32 x 8 NT1 per warp) = A_pos[rows, :] E[:, chunk] ----------------
       const int ntiles1 = (d.cval1 + 7) >> 3;
       const int nt1w = (ntiles1 + WC - 1) / WC;
       const int tile0 = wc * nt1w;
       const int nt1 = max(0, min(nt1w, ntiles1 - tile0));
       const double sc = d.scale;
-      const double* a = stage + t * (TM + 4) + wr * 32 + g;
-      const double* b = stage + C::A_SZ + t * LDE + tile0 * 8 + g;
-      if (flags & STEP_FIRST) {
+      const int e_off = C::A_SZ + t * LDE + tile0 * 8 + g;
 #pragma unroll
-        for (int ii = 0; ii < 4; ++ii)
+      for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
-          for (int j = 0; j < NT1; ++j) tacc[ii][j][0] = tacc[ii][j][1] = 0.0;
+        for (int j = 0; j < NT1; ++j) tacc[ii][j][0] = tacc[ii][j][1] = 0.0;
+      switch (nt1) {
+        case 1: run_phase<NS, ST, false, 1, NT1, 8, 4 * (TM + 4), 4 * LDE>(tacc, stages, Ts, a1_off, e_off, nsteps, ktot, mt, b, par, full, empty, lane); break;
+        case 2: run_phase<NS, ST, false, 2, NT1, 8, 4 * (TM + 4), 4 * LDE>(tacc, stages, Ts, a1_off, e_off, nsteps, ktot, mt, b, par, full, empty, lane); break;
+        case 3: run_phase<NS, ST, false, 3, NT1, 8, 4 * (TM + 4), 4 * LDE>(tacc, stages, Ts, a1_off, e_off, nsteps, ktot, mt, b, par, full, empty, lane); break;
+        default: run_phase<NS, ST, false, 0, NT1, 8, 4 * (TM + 4), 4 * LDE>(tacc, stages, Ts, a1_off, e_off, nsteps, ktot, mt, b, par, full, empty, lane); break;
       }
-      if (mt > 0) {
-        switch (nt1) {
-          case 1: mma_stage<1, NT1, 8, 4 * (TM + 4), 4 * LDE>(tacc, a, b, nsub, mt); break;
-          case 2: mma_stage<2, NT1, 8, 4 * (TM + 4), 4 * LDE>(tacc, a, b, nsub, mt); break;
-          case 3: mma_stage<3, NT1, 8, 4 * (TM + 4), 4 * LDE>(tacc, a, b, nsub, mt); break;
-          default: break;
-        }
-      }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&empty[buf]);       // stage (and its descriptor) released
-      if (flags & STEP_LAST) {
-        consumer_bar();                              // every warp is done reading the previous T chunk
-        double* trow = Ts + (wr * 32 + g) * LDT + tile0 * 8 + 2 * t;
+      consumer_bar();                              // every warp is done reading the previous T chunk
+      double* trow = Ts + (wr * 32 + g) * LDT + tile0 * 8 + 2 * t;
 #pragma unroll
-        for (int ii = 0; ii < 4; ++ii)
+      for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
-          for (int j = 0; j < NT1; ++j)
-            if (ii < mt && j < nt1)
-              *reinterpret_cast<double2*>(trow + ii * 8 * LDT + j * 8) = make_double2(sc * tacc[ii][j][0], sc * tacc[ii][j][1]);
-        consumer_bar();                              // the new T chunk is visible to every warp
-      }
+        for (int j = 0; j < NT1; ++j)
+          if (ii < mt && j < nt1)
+            *reinterpret_cast<double2*>(trow + ii * 8 * LDT + j * 8) = make_double2(sc * tacc[ii][j][0], sc * tacc[ii][j][1]);
+      consumer_bar();                              // the new T chunk is visible to every warp
     } else {
-      // ---- second product: acc (32 x 8 NT2 per warp) += T_chunk[:, step] D_tile^T ---------------
-      const double* a = Ts + (wr * 32 + g) * LDT + d.s * KS + t;
-      const double* b = stage + t * (TP + 4) + ctile0 * 8 + g;
-      if (mt > 0) {
-        switch (nt2) {
-          case 1: mma_stage<1, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, a, b, nsub, mt); break;
-          case 2: mma_stage<2, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, a, b, nsub, mt); break;
-          case 3: mma_stage<3, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, a, b, nsub, mt); break;
-          case 4: mma_stage<4, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, a, b, nsub, mt); break;
-          case 5: mma_stage<5, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, a, b, nsub, mt); break;
-          case 6: mma_stage<6, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, a, b, nsub, mt); break;
-          case 7: mma_stage<7, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, a, b, nsub, mt); break;
-          case 8: mma_stage<8, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, a, b, nsub, mt); break;
-          case 9: mma_stage<9, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, a, b, nsub, mt); break;
-          default: break;
-        }
+      // ---- second product: acc (32 x 8 NT2 per warp) += T_chunk D_pos[cols, chunk]^T --------------
+      switch (nt2) {
+        case 1: run_phase<NS, ST, true, 1, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, stages, Ts, t_off, d_off, nsteps, ktot, mt, b, par, full, empty, lane); break;
+        case 2: run_phase<NS, ST, true, 2, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, stages, Ts, t_off, d_off, nsteps, ktot, mt, b, par, full, empty, lane); break;
+        case 3: run_phase<NS, ST, true, 3, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, stages, Ts, t_off, d_off, nsteps, ktot, mt, b, par, full, empty, lane); break;
+        case 4: run_phase<NS, ST, true, 4, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, stages, Ts, t_off, d_off, nsteps, ktot, mt, b, par, full, empty, lane); break;
+        case 5: run_phase<NS, ST, true, 5, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, stages, Ts, t_off, d_off, nsteps, ktot, mt, b, par, full, empty, lane); break;
+        case 6: run_phase<NS, ST, true, 6, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, stages, Ts, t_off, d_off, nsteps, ktot, mt, b, par, full, empty, lane); break;
+        case 7: run_phase<NS, ST, true, 7, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, stages, Ts, t_off, d_off, nsteps, ktot, mt, b, par, full, empty, lane); break;
+        case 8: run_phase<NS, ST, true, 8, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, stages, Ts, t_off, d_off, nsteps, ktot, mt, b, par, full, empty, lane); break;
+        case 9: run_phase<NS, ST, true, 9, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, stages, Ts, t_off, d_off, nsteps, ktot, mt, b, par, full, empty, lane); break;
+        default: run_phase<NS, ST, true, 0, NT2, 8 * LDT, 4, 4 * (TP + 4)>(acc, stages, Ts, t_off, d_off, nsteps, ktot, mt, b, par, full, empty, lane); break;
       }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&empty[buf]);
     }
+    ++cq;
   }
 
   // ---- epilogue: the tile leaves the registers once per work item -----------------------------
+  const DevWork wk = *wkp;            // re-read here: nothing of it stays live across the item
+  double* dst = (wk.to_partial ? partial : out) + wk.dst_off;
 #pragma unroll
   for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
@@ -434,39 +451,35 @@ heff_dmma_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __r
                  const DevTask* __restrict__ tasks, const double* __restrict__ psi, double* __restrict__ out,
                  double* __restrict__ partial, int* __restrict__ counter) {
   extern __shared__ __align__(16) double smem[];
-  __shared__ GenState gs[NPRODUCERS];
-  __shared__ StepDesc ring[2][NSTAGE];
-  __shared__ __align__(8) uint64_t full[NSTAGE];
-  __shared__ __align__(8) uint64_t empty[NSTAGE];
-  __shared__ int s_w, s_base;
+  __shared__ GenState gs;
+  __shared__ PhaseDesc pring[PHASE_RING];
+  __shared__ __align__(8) uint64_t full[MAX_STAGE];
+  __shared__ __align__(8) uint64_t empty[MAX_STAGE];
+  __shared__ int s_w;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  if (tid == 0) {
-    for (int i = 0; i < NSTAGE; ++i) {
-      mbar_init(&full[i], 32 + 1);      // 32 deferred cp.async arrivals + the descriptor writer
-      mbar_init(&empty[i], NWARPS);     // one arrival per consumer warp
-    }
-    s_base = 0;
-    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
-  }
   if (warp < NPRODUCERS) {
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 40;\n");
-    unsigned nfill = 0;                  // fills of this warp's stage buffer so far (mbarrier phase)
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 56;\n");
 #pragma unroll 1
     for (;;) {
-      cta_bar();                         // previous item retired; s_base published
-      if (tid == 0) s_w = atomicAdd(counter, 1);
+      cta_bar();                         // previous item retired: pipeline drained, barriers idle
+      if (tid == 0) {
+        s_w = atomicAdd(counter, 1);
+        for (int i = 0; i < MAX_STAGE; ++i) {
+          mbar_init(&full[i], NPRODUCERS * 32 + 1);   // deferred cp.async arrivals of every producer lane + the descriptor writer
+          mbar_init(&empty[i], NWARPS);               // one arrival per consumer warp
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+      }
       cta_bar();
       const int w = s_w;
       if (w >= nwork) break;
-      const DevWork wk = work[w];
-      const int first = (warp - s_base) & (NSTAGE - 1);
-      if (wk.wr == 1) producer_item<1>(wk, units, tasks, psi, smem, gs[warp], ring, full, empty, warp, lane, first, nfill);
-      else if (wk.wr == 2) producer_item<2>(wk, units, tasks, psi, smem, gs[warp], ring, full, empty, warp, lane, first, nfill);
-      else producer_item<4>(wk, units, tasks, psi, smem, gs[warp], ring, full, empty, warp, lane, first, nfill);
+      const int wr = work[w].wr;
+      if (wr == 1) producer_item<1>(work + w, units, tasks, psi, smem, gs, pring, full, empty, warp, lane);
+      else if (wr == 2) producer_item<2>(work + w, units, tasks, psi, smem, gs, pring, full, empty, warp, lane);
+      else producer_item<4>(work + w, units, tasks, psi, smem, gs, pring, full, empty, warp, lane);
     }
   } else {
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 232;\n");
-    unsigned ci = 0;                     // steps consumed so far: stage buffer = ci % NSTAGE, phase = ci / NSTAGE
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 224;\n");
     const int cw = warp - NPRODUCERS;
 #pragma unroll 1
     for (;;) {
@@ -474,12 +487,10 @@ heff_dmma_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __r
       cta_bar();
       const int w = s_w;
       if (w >= nwork) break;
-      const DevWork wk = work[w];
-      double* dst = (wk.to_partial ? partial : out) + wk.dst_off;
-      if (wk.wr == 1) consumer_item<1>(wk, dst, smem, ring, full, empty, cw, lane, ci);
-      else if (wk.wr == 2) consumer_item<2>(wk, dst, smem, ring, full, empty, cw, lane, ci);
-      else consumer_item<4>(wk, dst, smem, ring, full, empty, cw, lane, ci);
-      if (tid == NPRODUCERS * 32) s_base = (int)(ci & (NSTAGE - 1));
+      const int wr = work[w].wr;
+      if (wr == 1) consumer_item<1>(work + w, out, partial, smem, pring, full, empty, cw, lane);
+      else if (wr == 2) consumer_item<2>(work + w, out, partial, smem, pring, full, empty, cw, lane);
+      else consumer_item<4>(work + w, out, partial, smem, pring, full, empty, cw, lane);
     }
   }
 }

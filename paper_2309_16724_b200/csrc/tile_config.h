@@ -12,12 +12,13 @@
 namespace su2 {
 
 constexpr int NWARPS = 8;              // consumer (math) warps: two warpgroups
-constexpr int NPRODUCERS = 4;          // producer (cp.async) warps: one warpgroup, one stage buffer each
+constexpr int NPRODUCERS = 4;          // producer (cp.async) warps: one warpgroup; each copies a quarter of every tile
 constexpr int NTHREADS = 32 * (NWARPS + NPRODUCERS);
-constexpr int KS = 8;           // k extent of one pipeline stage (two DMMA k4 steps)
+constexpr int KS1 = 16;         // k extent of one pipeline stage of the first product (four DMMA k4 steps)
+constexpr int KS2 = 8;          // k extent of one pipeline stage of the second product (two DMMA k4 steps)
 constexpr int NT1 = 3;          // n8-tiles per warp, first product
 constexpr int NT2 = 9;          // n8-tiles per warp, second product
-constexpr int NSTAGE = NPRODUCERS;     // pipeline depth
+constexpr int MAX_STAGE = 8;    // upper bound of the pipeline depth (mbarrier arrays)
 
 template <int WR>
 struct TileCfg {
@@ -26,10 +27,12 @@ struct TileCfg {
   static constexpr int TP = 8 * NT2 * WC;       // columns of F per CTA       : 576 / 288 / 144
   static constexpr int NC = 8 * NT1 * WC;       // max columns of a T chunk   : 192 / 96 / 48
   static constexpr int LDT = NC + 4;            // leading dimension of T in shared memory
-  // one pipeline stage (doubles), every tile k-major [2 sub][4][C+4]: A tile C = TM, E tile C = NC, D tile C = TP.
-  static constexpr int A_SZ = 2 * 4 * (TM + 4);
-  static constexpr int E_SZ = 2 * 4 * (NC + 4);
-  static constexpr int D_SZ = 2 * 4 * (TP + 4);
+  static constexpr int NSTAGE = (WR == 1) ? 4 : (WR == 2) ? 8 : 6;   // pipeline depth (what fits beside T in 227 KB)
+  // one pipeline stage (doubles), every tile k-major [k/4][4][C+4]: A tile C = TM, E tile C = NC (KS1 deep),
+  // D tile C = TP (KS2 deep).
+  static constexpr int A_SZ = KS1 * (TM + 4);
+  static constexpr int E_SZ = KS1 * (NC + 4);
+  static constexpr int D_SZ = KS2 * (TP + 4);
   static constexpr int STAGE = (A_SZ + E_SZ > D_SZ) ? (A_SZ + E_SZ) : D_SZ;
   static constexpr int SMEM_DOUBLES = TM * LDT + NSTAGE * STAGE;
 };
@@ -64,7 +67,7 @@ inline double tile_pos_cost(int wr, int rows_valid, int cols_valid, int k, int n
     const int ncw = std::min(ncw_full, n - c * ncw_full);
     const int nt1w = (((ncw + 7) / 8) + ts.wc - 1) / ts.wc;
     cost += (double)mtmax * (nt1w * ((k + 3) / 4) + ntw2 * ((ncw + 3) / 4));
-    cost += 3.0 * ((k + KS - 1) / KS + (ncw + KS - 1) / KS);   // barrier + load issue per stage
+    cost += 4.0 * ((k + KS1 - 1) / KS1 + (ncw + KS2 - 1) / KS2);   // per-stage hand-over
   }
   return cost;
 }
