@@ -13,15 +13,15 @@
 // (profiles/r01_fp64_peak_probe.txt).
 //
 // Structure: persistent CTAs (one per SM) pull work items (segment x output tile) from an atomic
-// queue in the plan's longest-first order.  Inside an item every (task, position, T-chunk) is a run
-// of pipeline *steps*: first-product steps (A tile + E tile, KS deep) followed by second-product
-// steps (D tile, KS deep).  The CTA is warp-specialised:
-//   * warps 0-3 (one warpgroup, 40 registers after setmaxnreg.dec) are PRODUCERS.  Producer warp w
-//     owns stage buffer w: it walks the item's step sequence with an iterator kept in shared
-//     memory, writes the step descriptor, and stages the operand tiles with 8-byte cp.async + zero
-//     fill (ragged block sizes and odd leading dimensions need no special cases); completion is
-//     signalled on an mbarrier (cp.async.mbarrier.arrive.noinc).
-//   * warps 4-11 (two warpgroups, 232 registers after setmaxnreg.inc) are CONSUMERS: they wait on
+// queue in the plan's longest-first order.  Inside an item every (task, position, T-chunk) is a pair
+// of *phases*: the first product (stages of an A tile + an E tile, KS1 deep) and the second product
+// (stages of a D tile, KS2 deep).  The CTA is warp-specialised:
+//   * warps 0-3 (one warpgroup, 56 registers after setmaxnreg.dec) are PRODUCERS.  Every producer warp
+//     walks every stage and copies a quarter of its tiles with 8-byte cp.async + zero fill (ragged
+//     block sizes and odd leading dimensions need no special cases); completion is signalled on the
+//     stage's "full" mbarrier (cp.async.mbarrier.arrive.noinc).  Lane 0 of warp 0 also runs the phase
+//     iterator (state in shared memory) one phase ahead into a ring of phase descriptors.
+//   * warps 4-11 (two warpgroups, 224 registers after setmaxnreg.inc) are CONSUMERS: they wait on
 //     the stage's "full" mbarrier, issue only LDS + DMMA, and release the stage on its "empty"
 //     mbarrier.  No CTA-wide barrier exists inside an item; the T hand-over between the two
 //     products uses a named barrier of the 256 consumer threads.
@@ -36,12 +36,10 @@ namespace su2 {
 
 namespace {
 
-enum : int { STEP_END = 1, STEP_G2 = 2, STEP_TRANS = 4, STEP_FIRST = 8, STEP_LAST = 16 };
-
 enum : int { PH_END = 1, PH_G2 = 2, PH_TRANS = 4 };
 
 // One *phase* = a run of pipeline steps with regular addressing: the first product of one
-// (task, position, T-chunk) -- nsteps stages of an A tile and an E tile, KS deep -- or its second
+// (task, position, T-chunk) -- nsteps stages of an A tile and an E tile, KS1 deep -- or its second
 // product -- nsteps stages of a D tile.  Step s reads src + s * stride; both producers and consumers
 // derive everything else (valid k extent, first/last flags) from s in registers.
 struct PhaseDesc {
@@ -321,7 +319,7 @@ __device__ __forceinline__ void producer_item(const DevWork* __restrict__ wkp, c
 
 // ---- consumer warps: LDS + DMMA only ------------------------------------------------------------------
 // All steps of one phase for one warp: wait for the stage, multiply, release the stage.
-// G2 = false: A fragments come from the stage (a_off inside it); G2 = true: from T (a_off + s*KS).
+// G2 = false: A fragments come from the stage (a_off inside it); G2 = true: from T (a_off + s*KS2).
 template <int NS, int STAGE, bool G2, int NT, int NACC, int A_I, int A_SUB, int B_SUB>
 __device__ __forceinline__ void run_phase(double (&c)[4][NACC][2], const double* stages, const double* Ts, int a_off,
                                           int b_off, int nsteps, int ktot, int mt, int& b, int& par, uint64_t* full,

@@ -130,3 +130,30 @@ def test_rank_mismatched_row_vanishes():
     x = np.random.default_rng(0).normal(size=n)
     f = flatten(prob, heff_apply(prob, unflatten(prob, x), terms=[bad]))
     assert np.abs(f).max() == 0.0
+
+
+def test_sampled_equals_full_oracle():
+    """oracle/heff_sampled.py (step O7: sampled entries for the large configs) against the full
+    M-resolved oracle on workloads where both run: exact cfg1 Hamiltonian and the random 'mini' table."""
+    from gen.workloads import config_problem, integrals, random_psi
+    from oracle.abinitio_table import build_problem
+    from oracle.heff_dense import flatten, heff_apply, psi_sectors, unflatten
+    from oracle.heff_sampled import heff_sample, numpy_block_rows
+    t, v = integrals(6, seed=0, xi=2.0)
+    for prob in (build_problem(t, v, 2, 6, 0, use_adjoints=True), config_problem("mini")):
+        labels = psi_sectors(prob)
+        n = sum(prob.sec_l[s[0]].dim * prob.sec_r[s[4]].dim for s in labels)
+        psi = unflatten(prob, random_psi(n, seed=3), labels)
+        ref = heff_apply(prob, psi)
+        rows = numpy_block_rows(prob)
+        rng = np.random.default_rng(1)
+        checked = 0
+        for lab in labels[::5]:
+            m, p = prob.sec_l[lab[0]].dim, prob.sec_r[lab[4]].dim
+            ra = np.sort(rng.choice(m, size=min(m, 3), replace=False))
+            rb = np.sort(rng.choice(p, size=min(p, 2), replace=False))
+            got = heff_sample(prob, psi, lab, ra, rb, rows)
+            want = ref[lab][np.ix_(ra, rb)]
+            assert np.abs(got - want).max() <= 1e-13 * max(1.0, np.abs(flatten(prob, ref, labels)).max())
+            checked += got.size
+        assert checked > 20
