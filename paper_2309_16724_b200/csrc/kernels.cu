@@ -40,6 +40,19 @@ reduce_kernel(const DevReduce* __restrict__ red, const double* __restrict__ part
   }
 }
 
+// Plan-time position folding (the paper's pre-contraction): dst[e] = sum_pos alpha_pos src[pos][e],
+// positions summed in index order (deterministic).  HBM-bound, runs once per plan.
+__global__ void __launch_bounds__(256)
+fold_kernel(const FoldJob* __restrict__ jobs, const double* __restrict__ alpha, double* __restrict__ fold) {
+  const FoldJob j = jobs[blockIdx.y];
+  const double* __restrict__ al = j.alpha_off >= 0 ? alpha + j.alpha_off : nullptr;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < j.nelem; e += (int64_t)gridDim.x * blockDim.x) {
+    double s = 0.0;
+    for (int pos = 0; pos < j.npos; ++pos) s += (al ? al[pos] : 1.0) * j.src[(int64_t)pos * j.nelem + e];
+    fold[j.dst_off + e] = s;
+  }
+}
+
 // diag(H_eff)[s][a,b] = sum_{tasks s<-s} coef sum_pos alpha_pos A_pos[a,a] D_pos[b,b]
 __global__ void __launch_bounds__(256)
 diag_kernel(const DevDiagTask* __restrict__ dt, const int32_t* __restrict__ begin, const PsiSector* __restrict__ psi_sec,
@@ -70,7 +83,8 @@ static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, const std::vector<double>& ident_host,
                        const std::vector<int64_t>& alpha_off_of_task, const std::vector<int64_t>& identA,
-                       const std::vector<int64_t>& identD, void* stream_v) {
+                       const std::vector<int64_t>& identD, const std::vector<int64_t>& foldA,
+                       const std::vector<int64_t>& foldD, void* stream_v) {
   cudaStream_t stream = (cudaStream_t)stream_v;
   int dev = 0;
   SU2_CUDA(cudaGetDevice(&dev));
@@ -86,6 +100,11 @@ su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, co
   const size_t b_ident = align256(ident_host.size() * sizeof(double));
   const size_t total = b_tasks + b_units + b_work + b_red + b_diag + b_dbeg + b_psi + b_alpha + b_ident + 256;
   SU2_CUDA(cudaMalloc(&plan->d_blob, total));
+  FoldJob* d_jobs = nullptr;
+  if (plan->fold_elems > 0) {
+    SU2_CUDA(cudaMalloc(&plan->d_fold, (size_t)plan->fold_elems * sizeof(double)));
+    SU2_CUDA(cudaMalloc(&d_jobs, plan->h_fold.size() * sizeof(FoldJob)));
+  }
   char* base = (char*)plan->d_blob;
   size_t off = 0;
   auto carve = [&](size_t bytes) { char* p = base + off; off += bytes; return p; };
@@ -105,6 +124,8 @@ su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, co
     if (alpha_off_of_task[i] >= 0) t.alpha = plan->d_alpha + alpha_off_of_task[i];
     if (identA[i] >= 0) t.A = plan->d_identity + identA[i];
     if (identD[i] >= 0) t.D = plan->d_identity + identD[i];
+    if (foldA[i] >= 0) t.A = plan->d_fold + foldA[i];
+    if (foldD[i] >= 0) t.D = plan->d_fold + foldD[i];
     if (!t.A || !t.D) return SU2_ERR_INVALID_ARGUMENT;   // family without device data
   }
   for (auto& d : plan->h_diag) {
@@ -124,7 +145,17 @@ su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, co
   SU2_CUDA(up(d_psi, plan->psi.data(), plan->psi.size() * sizeof(PsiSector)));
   SU2_CUDA(up(plan->d_alpha, alpha_host.data(), alpha_host.size() * sizeof(double)));
   SU2_CUDA(up(plan->d_identity, ident_host.data(), ident_host.size() * sizeof(double)));
+  if (plan->fold_elems > 0) {
+    for (const FoldJob& j : plan->h_fold)
+      if (!j.src) { cudaFree(d_jobs); return SU2_ERR_INVALID_ARGUMENT; }   // family without device data
+    SU2_CUDA(cudaMemcpyAsync(d_jobs, plan->h_fold.data(), plan->h_fold.size() * sizeof(FoldJob), cudaMemcpyHostToDevice, stream));
+    dim3 grid(64, (unsigned)plan->h_fold.size());
+    fold_kernel<<<grid, 256, 0, stream>>>(d_jobs, plan->d_alpha, plan->d_fold);
+    SU2_CUDA(cudaGetLastError());
+    count_launch();
+  }
   SU2_CUDA(cudaStreamSynchronize(stream));
+  if (d_jobs) cudaFree(d_jobs);
   plan->d_psi_sec = d_psi;
   return SU2_OK;
 }
@@ -133,6 +164,10 @@ void free_plan_device(su2_plan* plan) {
   if (plan && plan->d_blob) {
     cudaFree(plan->d_blob);
     plan->d_blob = nullptr;
+  }
+  if (plan && plan->d_fold) {
+    cudaFree(plan->d_fold);
+    plan->d_fold = nullptr;
   }
 }
 

@@ -265,9 +265,45 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
   });
 
   // ---- device task images ---------------------------------------------------------------
+  // ---- position folding (the paper's pre-contraction) -----------------------------
+  // A row whose positions enter through ONE block only (the other factor is the identity or has a
+  // single position) is sum_pos alpha_pos A_pos applied once: that sum does not depend on Psi, so it
+  // is formed at plan time (fold_kernel) and the row's tasks become one-position tasks.
+  std::vector<int> fold_side(p->nterm, -1);          // -1: not folded, 0: l family folded, 1: r family folded
+  std::vector<int64_t> fold_base(p->nterm, -1);      // element offset of the term's folded family in plan->d_fold
+  std::vector<std::vector<int64_t>> fold_blk_off(p->nterm);
+  int64_t fold_elems = 0;
+  for (int t = 0; t < p->nterm; ++t) {
+    const su2_term& tm = p->term[t];
+    const int npl = tm.fam_l >= 0 ? p->fam_l[tm.fam_l].npos : 1;
+    const int npr = tm.fam_r >= 0 ? p->fam_r[tm.fam_r].npos : 1;
+    if (tm.npos <= 1 || (npl > 1) == (npr > 1)) continue;
+    const int side = npl > 1 ? 0 : 1;
+    const su2_opfamily& f = side ? p->fam_r[tm.fam_r] : p->fam_l[tm.fam_l];
+    const auto& sec = side ? sr : sl;
+    fold_side[t] = side;
+    fold_base[t] = fold_elems;
+    fold_blk_off[t].resize(f.nblk);
+    for (int b = 0; b < f.nblk; ++b) {
+      fold_blk_off[t][b] = fold_elems;
+      const int64_t nelem = (int64_t)sec[f.q_out[b]].dim * sec[f.q_in[b]].dim;
+      FoldJob job{};
+      job.src = f.data ? f.data + f.blk_off[b] : nullptr;
+      job.dst_off = fold_elems;
+      job.nelem = nelem;
+      job.npos = f.npos;
+      job.alpha_off = alpha_off_of_term[t];
+      plan->h_fold.push_back(job);
+      fold_elems += nelem;
+    }
+  }
+  plan->fold_elems = fold_elems;
+  for (HostTask& ht : plan->tasks)
+    if (fold_side[ht.term] >= 0) ht.npos = 1;
+
   const int64_t ntask = (int64_t)plan->tasks.size();
   plan->h_tasks.resize(ntask);
-  std::vector<int64_t> alpha_off_of_task(ntask, -1), identA(ntask, -1), identD(ntask, -1);
+  std::vector<int64_t> alpha_off_of_task(ntask, -1), identA(ntask, -1), identD(ntask, -1), foldA(ntask, -1), foldD(ntask, -1);
   // identity blocks: one (dim x dim) identity per distinct dim, concatenated
   std::map<int, int64_t> ident_off;
   std::vector<double> ident_host;
@@ -290,7 +326,11 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
     d.e_off = plan->psi[ht.in_sec].off;
     d.m = ht.m; d.k = ht.k; d.n = ht.n; d.p = ht.p; d.npos = ht.npos;
     d.flags = (ht.adj_l ? TASK_TRANS_A : 0u) | (ht.adj_r ? TASK_TRANS_D : 0u);
-    if (ht.fam_l >= 0) {
+    const int fs = fold_side[ht.term];
+    if (ht.fam_l >= 0 && fs == 0) {
+      foldA[i] = fold_blk_off[ht.term][ht.blk_l];
+      d.strideA = 0;
+    } else if (ht.fam_l >= 0) {
       const su2_opfamily& f = p->fam_l[ht.fam_l];
       d.A = f.data ? f.data + f.blk_off[ht.blk_l] : nullptr;
       d.strideA = f.npos > 1 ? ht.m * ht.k : 0;
@@ -298,7 +338,10 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
       identA[i] = ident_for(ht.m);
       d.strideA = 0;
     }
-    if (ht.fam_r >= 0) {
+    if (ht.fam_r >= 0 && fs == 1) {
+      foldD[i] = fold_blk_off[ht.term][ht.blk_r];
+      d.strideD = 0;
+    } else if (ht.fam_r >= 0) {
       const su2_opfamily& f = p->fam_r[ht.fam_r];
       d.D = f.data ? f.data + f.blk_off[ht.blk_r] : nullptr;
       d.strideD = f.npos > 1 ? ht.p * ht.n : 0;
@@ -306,7 +349,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
       identD[i] = ident_for(ht.p);
       d.strideD = 0;
     }
-    alpha_off_of_task[i] = alpha_off_of_term[ht.term];
+    alpha_off_of_task[i] = fs >= 0 ? -1 : alpha_off_of_term[ht.term];   // folded rows carry alpha inside the block
     const double m = ht.m, k = ht.k, n = ht.n, pp = ht.p;
     cc += ht.npos * std::min(2 * m * k * n + 2 * m * n * pp, 2 * k * n * pp + 2 * m * k * pp);
     opbytes += ht.npos * 8.0 * (m * k + n * pp);
@@ -472,7 +515,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
   plan->info.nwork_items = (int64_t)plan->h_work.size();
 
   if (!plan->host_only) {
-    st = upload_plan(plan, alpha_host, ident_host, alpha_off_of_task, identA, identD, cuda_stream);
+    st = upload_plan(plan, alpha_host, ident_host, alpha_off_of_task, identA, identD, foldA, foldD, cuda_stream);
     if (st != SU2_OK) {
       free_plan_device(plan);
       delete plan;

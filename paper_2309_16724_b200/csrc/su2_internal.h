@@ -46,6 +46,15 @@ struct DevReduce {
   int32_t pad;
 };
 
+// Plan-time position folding: dst[e] = sum_pos alpha[pos] * src[pos * nelem + e].
+struct FoldJob {
+  const double* src;      // block of the family: [npos][nelem]
+  int64_t dst_off;        // element offset inside the plan's folded-operator buffer
+  int64_t nelem;
+  int64_t alpha_off;      // offset into the plan's alpha array, -1: all ones
+  int32_t npos, pad;
+};
+
 // Diagonal tasks (s == s') for su2_heff_diag.
 struct DevDiagTask {
   const double* A;
@@ -90,6 +99,8 @@ struct su2_plan {
   std::vector<su2::DevWork> h_work;
   std::vector<su2::DevReduce> h_reduce;
   std::vector<su2::DevDiagTask> h_diag;
+  std::vector<su2::FoldJob> h_fold;    // plan-time folding jobs
+  int64_t fold_elems = 0;
   std::vector<int32_t> h_diag_begin;   // per psi sector: range into h_diag
   // device tables (owned)
   void* d_blob = nullptr;              // one allocation holding everything below
@@ -101,6 +112,7 @@ struct su2_plan {
   int32_t* d_diag_begin = nullptr;
   double* d_alpha = nullptr;
   double* d_identity = nullptr;
+  double* d_fold = nullptr;            // folded operators (own allocation, freed with the plan)
   int32_t* d_counter = nullptr;
   void* d_psi_sec = nullptr;           // device copy of `psi` (PsiSector[])
   int64_t partial_elems = 0;
@@ -114,7 +126,8 @@ su2_status launch_apply(const su2_plan* plan, const double* psi, double* out, do
 su2_status launch_diag(const su2_plan* plan, double* diag, void* stream);
 su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, const std::vector<double>& ident_host,
                        const std::vector<int64_t>& alpha_off_of_task, const std::vector<int64_t>& identA_off_of_task,
-                       const std::vector<int64_t>& identD_off_of_task, void* stream);
+                       const std::vector<int64_t>& identD_off_of_task, const std::vector<int64_t>& foldA_off_of_task,
+                       const std::vector<int64_t>& foldD_off_of_task, void* stream);
 void free_plan_device(su2_plan* plan);
 su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double alpha, const double* A, const double* X,
                             const double* B, double* C, void* stream);
