@@ -243,6 +243,23 @@ __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
 template <int NSUB, int NT, int NACC, int A_I, int A_SUB, int B_SUB>
 __device__ __forceinline__ void mma_stage(double (&c)[4][NACC][2], const double* __restrict__ a,
                                           const double* __restrict__ b, int nsub, int mt) {
+  if (mt == 4 && nsub == NSUB) {
+    // full stage: one straight-line block, so that the fragment loads of sub-step s+1 can be scheduled
+    // under the DMMAs of sub-step s
+#pragma unroll
+    for (int sub = 0; sub < NSUB; ++sub) {
+      double af[4], bf[NT];
+#pragma unroll
+      for (int ii = 0; ii < 4; ++ii) af[ii] = a[sub * A_SUB + ii * A_I];
+#pragma unroll
+      for (int j = 0; j < NT; ++j) bf[j] = b[sub * B_SUB + j * 8];
+#pragma unroll
+      for (int j = 0; j < NT; ++j)
+#pragma unroll
+        for (int ii = 0; ii < 4; ++ii) dmma(c[ii][j], af[ii], bf[j]);
+    }
+    return;
+  }
 #pragma unroll
   for (int sub = 0; sub < NSUB; ++sub) {
     if (sub < nsub) {
@@ -251,18 +268,11 @@ __device__ __forceinline__ void mma_stage(double (&c)[4][NACC][2], const double*
       for (int ii = 0; ii < 4; ++ii) af[ii] = a[sub * A_SUB + ii * A_I];
 #pragma unroll
       for (int j = 0; j < NT; ++j) bf[j] = b[sub * B_SUB + j * 8];
-      if (mt == 4) {
 #pragma unroll
-        for (int j = 0; j < NT; ++j)
+      for (int j = 0; j < NT; ++j)
 #pragma unroll
-          for (int ii = 0; ii < 4; ++ii) dmma(c[ii][j], af[ii], bf[j]);
-      } else {
-#pragma unroll
-        for (int j = 0; j < NT; ++j)
-#pragma unroll
-          for (int ii = 0; ii < 3; ++ii)
-            if (ii < mt) dmma(c[ii][j], af[ii], bf[j]);
-      }
+        for (int ii = 0; ii < 4; ++ii)
+          if (ii < mt) dmma(c[ii][j], af[ii], bf[j]);
     }
   }
 }

@@ -53,6 +53,33 @@ fold_kernel(const FoldJob* __restrict__ jobs, const double* __restrict__ alpha, 
   }
 }
 
+// Plan-time transposed copy of a right-block operator block, 32x32 tiles through shared memory:
+// dst[pos][j][c] = src[pos][c][j].  blockIdx.x = tile, blockIdx.y = job, blockIdx.z strides positions.
+__global__ void __launch_bounds__(256)
+transpose_kernel(const TransposeJob* __restrict__ jobs, double* __restrict__ trans) {
+  __shared__ double tile[32][33];
+  const TransposeJob j = jobs[blockIdx.y];
+  const int tc = (j.cols + 31) / 32, tr = (j.rows + 31) / 32;
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  for (int pos = blockIdx.z; pos < j.npos; pos += gridDim.z) {
+    const double* __restrict__ src = j.src + (int64_t)pos * j.rows * j.cols;
+    double* __restrict__ dst = trans + j.dst_off + (int64_t)pos * j.rows * j.cols;
+    for (int t = blockIdx.x; t < tr * tc; t += gridDim.x) {
+      const int r0 = (t / tc) * 32, c0 = (t % tc) * 32;
+      for (int i = ty; i < 32; i += 8) {
+        const int r = r0 + i, c = c0 + tx;
+        tile[i][tx] = (r < j.rows && c < j.cols) ? src[(int64_t)r * j.cols + c] : 0.0;
+      }
+      __syncthreads();
+      for (int i = ty; i < 32; i += 8) {
+        const int c = c0 + i, r = r0 + tx;
+        if (c < j.cols && r < j.rows) dst[(int64_t)c * j.rows + r] = tile[tx][i];
+      }
+      __syncthreads();
+    }
+  }
+}
+
 // diag(H_eff)[s][a,b] = sum_{tasks s<-s} coef sum_pos alpha_pos A_pos[a,a] D_pos[b,b]
 __global__ void __launch_bounds__(256)
 diag_kernel(const DevDiagTask* __restrict__ dt, const int32_t* __restrict__ begin, const PsiSector* __restrict__ psi_sec,
@@ -84,7 +111,7 @@ static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, const std::vector<double>& ident_host,
                        const std::vector<int64_t>& alpha_off_of_task, const std::vector<int64_t>& identA,
                        const std::vector<int64_t>& identD, const std::vector<int64_t>& foldA,
-                       const std::vector<int64_t>& foldD, void* stream_v) {
+                       const std::vector<int64_t>& foldD, const std::vector<int64_t>& transD, void* stream_v) {
   cudaStream_t stream = (cudaStream_t)stream_v;
   int dev = 0;
   SU2_CUDA(cudaGetDevice(&dev));
@@ -100,6 +127,17 @@ su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, co
   const size_t b_ident = align256(ident_host.size() * sizeof(double));
   const size_t total = b_tasks + b_units + b_work + b_red + b_diag + b_dbeg + b_psi + b_alpha + b_ident + 256;
   SU2_CUDA(cudaMalloc(&plan->d_blob, total));
+  TransposeJob* d_tjobs = nullptr;
+  if (plan->trans_elems > 0) {
+    bool ok = true;
+    for (const TransposeJob& j : plan->h_trans) ok = ok && j.src != nullptr;
+    // optional: when the copy does not fit, the tasks keep reading the stored layout
+    if (ok && cudaMalloc(&plan->d_trans, (size_t)plan->trans_elems * sizeof(double)) != cudaSuccess) {
+      plan->d_trans = nullptr;
+      (void)cudaGetLastError();
+    }
+    if (plan->d_trans) SU2_CUDA(cudaMalloc(&d_tjobs, plan->h_trans.size() * sizeof(TransposeJob)));
+  }
   FoldJob* d_jobs = nullptr;
   if (plan->fold_elems > 0) {
     SU2_CUDA(cudaMalloc(&plan->d_fold, (size_t)plan->fold_elems * sizeof(double)));
@@ -126,6 +164,10 @@ su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, co
     if (identD[i] >= 0) t.D = plan->d_identity + identD[i];
     if (foldA[i] >= 0) t.A = plan->d_fold + foldA[i];
     if (foldD[i] >= 0) t.D = plan->d_fold + foldD[i];
+    if (transD[i] >= 0 && plan->d_trans) {
+      t.D = plan->d_trans + transD[i];
+      t.flags |= TASK_TRANS_D;
+    }
     if (!t.A || !t.D) return SU2_ERR_INVALID_ARGUMENT;   // family without device data
   }
   for (auto& d : plan->h_diag) {
@@ -154,8 +196,16 @@ su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, co
     SU2_CUDA(cudaGetLastError());
     count_launch();
   }
+  if (plan->d_trans) {
+    SU2_CUDA(cudaMemcpyAsync(d_tjobs, plan->h_trans.data(), plan->h_trans.size() * sizeof(TransposeJob), cudaMemcpyHostToDevice, stream));
+    dim3 grid(64, (unsigned)plan->h_trans.size(), 16);
+    transpose_kernel<<<grid, 256, 0, stream>>>(d_tjobs, plan->d_trans);
+    SU2_CUDA(cudaGetLastError());
+    count_launch();
+  }
   SU2_CUDA(cudaStreamSynchronize(stream));
   if (d_jobs) cudaFree(d_jobs);
+  if (d_tjobs) cudaFree(d_tjobs);
   plan->d_psi_sec = d_psi;
   return SU2_OK;
 }
@@ -168,6 +218,10 @@ void free_plan_device(su2_plan* plan) {
   if (plan && plan->d_fold) {
     cudaFree(plan->d_fold);
     plan->d_fold = nullptr;
+  }
+  if (plan && plan->d_trans) {
+    cudaFree(plan->d_trans);
+    plan->d_trans = nullptr;
   }
 }
 

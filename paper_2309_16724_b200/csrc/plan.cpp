@@ -301,8 +301,38 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
   for (HostTask& ht : plan->tasks)
     if (fold_side[ht.term] >= 0) ht.npos = 1;
 
+  // ---- transposed copies of the right-block families ------------------------------------------
+  // The second product stages D_pos[cols, chunk]: for a row-major block used as stored that is a
+  // gather of 64-byte runs (measured 6.2 TB/s per GPU into shared memory), for a block read transposed it
+  // is one contiguous run per k row (16-byte cp.async, 11-19 TB/s).  Families that are used as stored by
+  // position-batched rows therefore get a transposed copy at plan time (transpose_kernel); if the copy
+  // does not fit in device memory the plan falls back to the stored layout.
+  std::vector<std::vector<int64_t>> trans_blk_off(p->nfam_r);
+  {
+    std::vector<char> need(p->nfam_r, 0);
+    for (const HostTask& ht : plan->tasks)
+      if (ht.fam_r >= 0 && !ht.adj_r && fold_side[ht.term] != 1 && p->fam_r[ht.fam_r].npos > 1) need[ht.fam_r] = 1;
+    int64_t off = 0;
+    for (int f = 0; f < p->nfam_r; ++f) {
+      if (!need[f]) continue;
+      const su2_opfamily& fam = p->fam_r[f];
+      trans_blk_off[f].resize(fam.nblk);
+      for (int b = 0; b < fam.nblk; ++b) {
+        trans_blk_off[f][b] = off;
+        TransposeJob job{};
+        job.src = fam.data ? fam.data + fam.blk_off[b] : nullptr;
+        job.dst_off = off;
+        job.rows = sr[fam.q_out[b]].dim; job.cols = sr[fam.q_in[b]].dim; job.npos = fam.npos;
+        plan->h_trans.push_back(job);
+        off += (int64_t)fam.npos * job.rows * job.cols;
+      }
+    }
+    plan->trans_elems = off;
+  }
+
   const int64_t ntask = (int64_t)plan->tasks.size();
   plan->h_tasks.resize(ntask);
+  std::vector<int64_t> transD(ntask, -1);
   std::vector<int64_t> alpha_off_of_task(ntask, -1), identA(ntask, -1), identD(ntask, -1), foldA(ntask, -1), foldD(ntask, -1);
   // identity blocks: one (dim x dim) identity per distinct dim, concatenated
   std::map<int, int64_t> ident_off;
@@ -345,6 +375,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
       const su2_opfamily& f = p->fam_r[ht.fam_r];
       d.D = f.data ? f.data + f.blk_off[ht.blk_r] : nullptr;
       d.strideD = f.npos > 1 ? ht.p * ht.n : 0;
+      if (!ht.adj_r && !trans_blk_off[ht.fam_r].empty()) transD[i] = trans_blk_off[ht.fam_r][ht.blk_r];
     } else {
       identD[i] = ident_for(ht.p);
       d.strideD = 0;
@@ -515,7 +546,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
   plan->info.nwork_items = (int64_t)plan->h_work.size();
 
   if (!plan->host_only) {
-    st = upload_plan(plan, alpha_host, ident_host, alpha_off_of_task, identA, identD, foldA, foldD, cuda_stream);
+    st = upload_plan(plan, alpha_host, ident_host, alpha_off_of_task, identA, identD, foldA, foldD, transD, cuda_stream);
     if (st != SU2_OK) {
       free_plan_device(plan);
       delete plan;

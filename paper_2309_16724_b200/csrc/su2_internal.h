@@ -55,6 +55,13 @@ struct FoldJob {
   int32_t npos, pad;
 };
 
+// Plan-time transposition of a right-block operator block: dst[pos][j][c] = src[pos][c][j].
+struct TransposeJob {
+  const double* src;      // [npos][rows][cols]
+  int64_t dst_off;        // element offset inside the plan's transposed-operator buffer
+  int32_t rows, cols, npos, pad;
+};
+
 // Diagonal tasks (s == s') for su2_heff_diag.
 struct DevDiagTask {
   const double* A;
@@ -100,6 +107,8 @@ struct su2_plan {
   std::vector<su2::DevReduce> h_reduce;
   std::vector<su2::DevDiagTask> h_diag;
   std::vector<su2::FoldJob> h_fold;    // plan-time folding jobs
+  std::vector<su2::TransposeJob> h_trans;   // plan-time transposition jobs
+  int64_t trans_elems = 0;
   int64_t fold_elems = 0;
   std::vector<int32_t> h_diag_begin;   // per psi sector: range into h_diag
   // device tables (owned)
@@ -113,6 +122,7 @@ struct su2_plan {
   double* d_alpha = nullptr;
   double* d_identity = nullptr;
   double* d_fold = nullptr;            // folded operators (own allocation, freed with the plan)
+  double* d_trans = nullptr;           // transposed copies of right-block families (own allocation; null if it did not fit)
   int32_t* d_counter = nullptr;
   void* d_psi_sec = nullptr;           // device copy of `psi` (PsiSector[])
   int64_t partial_elems = 0;
@@ -127,7 +137,8 @@ su2_status launch_diag(const su2_plan* plan, double* diag, void* stream);
 su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, const std::vector<double>& ident_host,
                        const std::vector<int64_t>& alpha_off_of_task, const std::vector<int64_t>& identA_off_of_task,
                        const std::vector<int64_t>& identD_off_of_task, const std::vector<int64_t>& foldA_off_of_task,
-                       const std::vector<int64_t>& foldD_off_of_task, void* stream);
+                       const std::vector<int64_t>& foldD_off_of_task, const std::vector<int64_t>& transD_off_of_task,
+                       void* stream);
 void free_plan_device(su2_plan* plan);
 su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double alpha, const double* A, const double* X,
                             const double* B, double* C, void* stream);
