@@ -320,14 +320,19 @@ __device__ __forceinline__ void producer_item(const DevWork* __restrict__ wkp, c
           if (flags & PH_TRANS) {
             copy_kmajor<C::TM>(stage, src0, d.ld0, d.cval0, jval, w, lane);
           } else {
-            copy_cmajor<C::TM>(stage, src0, d.ld0, d.cval0, jval, w, lane);
-            if (jval > 8) copy_cmajor<C::TM>(stage + 8 * (C::TM + 4), src0 + 8, d.ld0, d.cval0, jval - 8, w, lane);
+#pragma unroll 1
+            for (int j0 = 0; j0 < jval; j0 += 8)       // copy_cmajor moves 8 k columns per call
+              copy_cmajor<C::TM>(stage + j0 * (C::TM + 4), src0 + j0, d.ld0, d.cval0, jval - j0, w, lane);
           }
           copy_kmajor<C::NC>(stage + C::A_SZ, d.src1 + (int64_t)s * d.stride1, d.ld1, d.cval1, jval, w, lane);
         } else {
           const int jval = min(KS2, d.ktot - s * KS2);
           if (flags & PH_TRANS) copy_kmajor<C::TP>(stage, src0, d.ld0, d.cval0, jval, w, lane);
-          else copy_cmajor<C::TP>(stage, src0, d.ld0, d.cval0, jval, w, lane);
+          else {
+#pragma unroll 1
+            for (int j0 = 0; j0 < jval; j0 += 8)
+              copy_cmajor<C::TP>(stage + j0 * (C::TP + 4), src0 + j0, d.ld0, d.cval0, jval - j0, w, lane);
+          }
         }
       }
       cp_async_mbar_arrive(&full[b]);          // 128 deferred arrivals: this lane's copies have landed
