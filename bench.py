@@ -319,7 +319,8 @@ def run_gpu(args):
                    "psi_len": int(info["psi_len"]), "tasks": int(info["ntasks"]),
                    "task_positions": int(info["ntask_positions"]), "cc_flops_per_apply": cc,
                    "executed_flops_per_apply": info["executed_flops"], "work_items": int(info["nwork_items"]),
-                   "segments": int(info["nsegments"]), "plan_seconds": info["plan_seconds"], "setup_seconds": setup_s},
+                   "segments": int(info["nsegments"]), "plan_seconds": info["plan_seconds"], "setup_seconds": setup_s,
+                   "plan_device_bytes": int(info["plan_device_bytes"])},
         "clocks": clocks,
         "e2e": {"value": whole_job_tflops(cc, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": 8 * op.psi_len,
                 "d2h_bytes_per_step": 8 * op.psi_len, "ms_per_step": e2e_ms,

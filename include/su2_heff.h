@@ -27,7 +27,10 @@
  * Ownership: the caller owns every device buffer and the CUDA stream.  Host arrays handed to
  * su2_plan_create are copied and may be freed afterwards; operator-family `data` pointers are
  * DEVICE pointers that must stay valid and unchanged while the plan is used.  The library
- * allocates only the plan's own task tables on the device (freed by su2_plan_destroy).
+ * allocates on the device only what belongs to the plan (freed by su2_plan_destroy): its task
+ * tables, the position-folded operators of one-sided rows (sum_pos alpha_pos A_pos, formed once per
+ * plan) and, if they fit, transposed copies of the right-block families used by position-batched
+ * rows (su2_plan_info_t.plan_device_bytes; +50 % of the right-block operator bytes).
  * Errors: every entry point returns 0 on success and a negative su2_status otherwise; no
  * exceptions, no aborts, no partial state.  Results are bit-reproducible for a fixed plan.
  */
@@ -116,7 +119,8 @@ enum {
 typedef struct {
   int64_t psi_len;           /* number of doubles in Psi / F                                    */
   int64_t ntasks;            /* sector tasks (paper: rows of all sector-task-tables)            */
-  int64_t ntask_positions;   /* tasks counted once per position (paper's "number of tasks")     */
+  int64_t ntask_positions;   /* tasks counted once per position (paper's "number of tasks"); a row whose
+                                positions enter through one block only is folded to ONE position   */
   double cc_flops;           /* CC = sum over task-positions of min(2mkn+2mnp, 2knp+2mkp)       */
   double executed_flops;     /* flops the kernels execute per apply (tile padding, recompute)   */
   double operator_bytes;     /* 8(mk+np) summed over task-positions (algorithmic HBM traffic)   */
@@ -125,6 +129,7 @@ typedef struct {
   int32_t nsegments;         /* work segments (deterministic segmented reduction)               */
   int64_t nwork_items;       /* CTA-level work items per apply                                  */
   double plan_seconds;       /* host time spent in su2_plan_create                              */
+  int64_t plan_device_bytes; /* device memory owned by the plan (tables, folded and transposed operators) */
 } su2_plan_info_t;
 
 /* Build the plan: enumerate the sector tasks (Eq. (3)), compute the coefficient of each

@@ -127,6 +127,7 @@ su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, co
   const size_t b_ident = align256(ident_host.size() * sizeof(double));
   const size_t total = b_tasks + b_units + b_work + b_red + b_diag + b_dbeg + b_psi + b_alpha + b_ident + 256;
   SU2_CUDA(cudaMalloc(&plan->d_blob, total));
+  plan->info.plan_device_bytes = (int64_t)total;
   TransposeJob* d_tjobs = nullptr;
   if (plan->trans_elems > 0) {
     bool ok = true;
@@ -136,11 +137,15 @@ su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, co
       plan->d_trans = nullptr;
       (void)cudaGetLastError();
     }
-    if (plan->d_trans) SU2_CUDA(cudaMalloc(&d_tjobs, plan->h_trans.size() * sizeof(TransposeJob)));
+    if (plan->d_trans) {
+      SU2_CUDA(cudaMalloc(&d_tjobs, plan->h_trans.size() * sizeof(TransposeJob)));
+      plan->info.plan_device_bytes += plan->trans_elems * (int64_t)sizeof(double);
+    }
   }
   FoldJob* d_jobs = nullptr;
   if (plan->fold_elems > 0) {
     SU2_CUDA(cudaMalloc(&plan->d_fold, (size_t)plan->fold_elems * sizeof(double)));
+    plan->info.plan_device_bytes += plan->fold_elems * (int64_t)sizeof(double);
     SU2_CUDA(cudaMalloc(&d_jobs, plan->h_fold.size() * sizeof(FoldJob)));
   }
   char* base = (char*)plan->d_blob;
