@@ -166,3 +166,49 @@ def test_gemm_pair_batched(m, k, n, p, batch):
                       torch.cuda.current_stream().cuda_stream)
     ref = C0 + 0.5 * np.einsum("bmk,bkn,bpn->bmp", A, X, B)
     assert _rel(dC.cpu().numpy(), ref) <= 1e-12
+
+
+def _wide_problem():
+    """Hand-made table with a right-block sector wider than the widest CTA tile (600 > 576 columns: two column
+    tiles, the first product is recomputed per column tile) and a left sector spanning two 32-row tiles with a
+    ragged tail; both blocks carry position-dependent operators, plus one-sided (folded) and identity rows."""
+    from gen import rng
+    from gen.problem import OpFamily, Problem, Sector, Term
+    from gen.workloads import site_table
+    sec_l = [Sector(0, 0, 37), Sector(1, 1, 9)]
+    sec_r = [Sector(2, 0, 600), Sector(1, 1, 70)]
+    site, _ = site_table()
+    sid = {o.name: i for i, o in enumerate(site)}
+
+    def fam(sec, dN, twoK, npos, tag, name):
+        blocks = [(io, ii) for io, so in enumerate(sec) for ii, si in enumerate(sec)
+                  if so.N == si.N + dN and abs(si.twoS - twoK) <= so.twoS <= si.twoS + twoK and (si.twoS + twoK + so.twoS) % 2 == 0]
+        data = [rng.normal_array(5, 7000 + 16 * tag + b, (npos, sec[io].dim, sec[ii].dim)) / np.sqrt(sec[ii].dim)
+                for b, (io, ii) in enumerate(blocks)]
+        return OpFamily(dN=dN, twoK=twoK, npos=npos, q_out=[b[0] for b in blocks], q_in=[b[1] for b in blocks], data=data, name=name)
+
+    fam_l = [fam(sec_l, 0, 0, 3, 1, "X0(l)"), fam(sec_l, 0, 2, 3, 2, "X1(l)"), fam(sec_l, +1, 1, 3, 3, "c+(l)")]
+    fam_r = [fam(sec_r, 0, 0, 3, 4, "Y0(r)"), fam(sec_r, 0, 2, 3, 5, "Y1(r)"), fam(sec_r, -1, 1, 3, 6, "R~(r)")]
+    a = np.array([0.7, -0.4, 1.1])
+    terms = [Term(0, 0, sid["1"], sid["1"], 0, 0, alpha=a, name="X0Y0"),
+             Term(1, 1, sid["1"], sid["1"], 2, 2, alpha=a[::-1].copy(), name="X1Y1"),
+             Term(2, 2, sid["1"], sid["1"], 1, 1, alpha=None, name="c+R~"),
+             Term(0, 0, sid["1"], sid["1"], 0, 0, alpha=a, adj_l=1, adj_r=1, name="X0Y0^H"),
+             Term(-1, 0, sid["B0"], sid["1"], 0, 0, alpha=a, name="n_B Y0"),        # folded, right block
+             Term(1, -1, sid["1"], sid["B1"], 2, 2, alpha=a, name="X1 s_C"),        # folded, left block
+             Term(-1, -1, sid["B0"], sid["B0"], 0, 0, alpha=np.array([0.3]), name="nn")]
+    return Problem(n_tot=4, twoS_tot=0, sec_l=sec_l, sec_r=sec_r, fam_l=fam_l, fam_r=fam_r, site=site, term=terms,
+                   meta=dict(L=0, N=4, D=0))
+
+
+@pytest.mark.parametrize("force_split", [False, True])
+def test_wide_sector_multiple_column_tiles(force_split):
+    torch = _torch()
+    prob = _wide_problem()
+    op = _operator(prob, force_split=force_split)
+    assert max(s.dim for s in prob.sec_r) > 576
+    x = random_psi(op.psi_len, seed=8)
+    f_gpu = op.apply(torch.from_numpy(x).cuda()).cpu().numpy()
+    f_ref = oracle_flat(prob, op.plan, x)
+    assert np.abs(f_ref).max() > 0
+    assert _rel(f_gpu, f_ref) <= TOL
