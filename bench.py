@@ -212,6 +212,49 @@ def whole_job_tflops(cc_per_rank, world, ms):
     return world * cc_per_rank / (ms * 1e-3) / 1e12
 
 
+def run_cfg5(args):
+    """BASELINE.json configs[4]: strided-batched FP64 GEMM-pair microbenchmark, C_b += alpha A_b X_b B_b^T,
+    square shapes 8..512, batch sized to ~1.5 GB of operands, through su2_gemm_pair_batched."""
+    import torch
+    from paper_2309_16724_b200 import gemm_pair_batched
+    from paper_2309_16724_b200.binding import kernel_launch_count, probe_fp64_peak
+    from paper_2309_16724_b200.build import build
+    assert torch.cuda.is_available(), "bench.py needs a GPU (no CPU fallback)"
+    build()
+    torch.cuda.set_device(0)
+    stream = torch.cuda.current_stream().cuda_stream
+    gen = torch.Generator(device="cuda").manual_seed(0)
+    sweep = []
+    l0 = kernel_launch_count()
+    for b in (8, 16, 32, 64, 128, 256, 512):
+        batch = int(max(1000, min(1000000, 1.5e9 / (4 * b * b * 8))))
+        A, X, B, Cm = (torch.randn(batch, b, b, dtype=torch.float64, device="cuda", generator=gen) for _ in range(4))
+        call = lambda: gemm_pair_batched(b, b, b, b, batch, 0.5, A.data_ptr(), X.data_ptr(), B.data_ptr(), Cm.data_ptr(), stream)
+        for _ in range(max(3, args.warmup)):
+            call()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            call()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.steps
+        flops = 4.0 * b ** 3 * batch
+        sweep.append({"m=k=n=p": b, "batch": batch, "ms": ms, "tflops": flops / ms / 1e9,
+                      "operand_gbs": 8.0 * 5 * b * b * batch / ms / 1e6})
+        del A, X, B, Cm
+    dmma = probe_fp64_peak(1, 4000, 4, stream)
+    best = max(sweep, key=lambda r: r["tflops"])
+    print(json.dumps({"metric": METRIC, "value": best["tflops"], "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+                      "warmup": max(3, args.warmup), "ms_per_step": best["ms"], "higher_is_better": True, "scaling": "weak",
+                      "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": "cfg5: strided-batched GEMM-pair microbenchmark (BASELINE.json configs[4]), square shapes; "
+                                             "value = best shape", "l2": "operands 1.5 GB per shape exceed L2"},
+                      "gpu_launches": kernel_launch_count() - l0, "sweep": sweep,
+                      "roofline": {"bound": "tensor", "achieved": best["tflops"], "peak": dmma, "unit": UNIT,
+                                   "frac": best["tflops"] / dmma, "traffic": None}}))
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
@@ -358,6 +401,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.config == "cfg5":
+        run_cfg5(args)
     else:
         run_gpu(args)
 

@@ -1,16 +1,21 @@
 // Strided-batched FP64 GEMM-pair microbenchmark entry (BASELINE.json configs[4]):
 //   C_b += alpha * A_b X_b B_b^T, one independent item per batch index.
+// Items with at least 64 x 64 outputs run on the fused DMMA kernel of the hot path (heff_dmma.cu): a small
+// kernel writes one task / unit / work-item record per batch item (and output tile) and the persistent
+// kernel consumes them with the accumulate flag.  Smaller items stay on the FP64-FMA tile routine below:
+// the DMMA kernel's per-item pipeline set-up (a few microseconds) would dominate them.
 #include <cuda_runtime.h>
 
 #include <algorithm>
 
 #include "su2_internal.h"
+#include "tile_config.h"
 
 namespace su2 {
 
 constexpr int TILE_M = 64;
 constexpr int TILE_P = 64;
-constexpr int NTHREADS = 256;
+constexpr int GP_THREADS = 256;
 constexpr int NC = 32;    // columns of T (n-chunk) per pass
 constexpr int KC = 16;    // k-chunk of the first product
 
@@ -41,7 +46,7 @@ __device__ __forceinline__ void accumulate_task(const DevTask& t, const double* 
 #pragma unroll
         for (int j = 0; j < 4; ++j) tacc[i][j] = 0.0;
       for (int k0 = 0; k0 < t.k; k0 += KC) {
-        for (int e = tid; e < TILE_M * KC; e += NTHREADS) {
+        for (int e = tid; e < TILE_M * KC; e += GP_THREADS) {
           int i, kk;
           if (!ta) { i = e / KC; kk = e % KC; } else { kk = e / TILE_M; i = e % TILE_M; }
           const int r = row0 + i, c = k0 + kk;
@@ -49,7 +54,7 @@ __device__ __forceinline__ void accumulate_task(const DevTask& t, const double* 
           if (r < t.m && c < t.k) v = ta ? A[(int64_t)c * t.m + r] : A[(int64_t)r * t.k + c];
           sm.As[i][kk] = v;
         }
-        for (int e = tid; e < KC * NC; e += NTHREADS) {
+        for (int e = tid; e < KC * NC; e += GP_THREADS) {
           const int kk = e / NC, j = e % NC;
           const int r = k0 + kk, c = n0 + j;
           sm.Es[kk][j] = (r < t.k && c < t.n) ? E[(int64_t)r * t.n + c] : 0.0;
@@ -74,7 +79,7 @@ __device__ __forceinline__ void accumulate_task(const DevTask& t, const double* 
 #pragma unroll
         for (int j = 0; j < 4; ++j) sm.Ts[gy + 32 * i][gx + 8 * j] = scale * tacc[i][j];
       // ---- D tile: Ds[c][j] = D[col0+c][n0+j]
-      for (int e = tid; e < TILE_P * NC; e += NTHREADS) {
+      for (int e = tid; e < TILE_P * NC; e += GP_THREADS) {
         int c, j;
         if (!td) { c = e / NC; j = e % NC; } else { j = e / TILE_P; c = e % TILE_P; }
         const int r = col0 + c, q = n0 + j;
@@ -102,7 +107,7 @@ __device__ __forceinline__ void accumulate_task(const DevTask& t, const double* 
 }
 
 // BASELINE.json configs[4]: C_b += alpha A_b X_b B_b^T; blockIdx.x = tile, blockIdx.y/z = batch index.
-__global__ void __launch_bounds__(NTHREADS)
+__global__ void __launch_bounds__(GP_THREADS)
 gemm_pair_kernel(int m, int k, int n, int p, int64_t batch, double alpha, const double* __restrict__ A,
                  const double* __restrict__ X, const double* __restrict__ B, double* __restrict__ C) {
   __shared__ TileSmem sm;
@@ -131,18 +136,66 @@ gemm_pair_kernel(int m, int k, int n, int p, int64_t batch, double alpha, const 
 }
 
 
+// one task, one unit and ntile work items per batch index
+__global__ void gemm_pair_tables_kernel(int m, int k, int n, int p, int64_t batch, double alpha, const double* A,
+                                        const double* B, int wr, int tm, int tp, DevTask* tasks, DevUnit* units,
+                                        DevWork* work, int* counter) {
+  const int tr = (m + tm - 1) / tm, tc = (p + tp - 1) / tp;
+  if (blockIdx.x == 0 && threadIdx.x == 0) *counter = 0;
+  for (int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; b < batch; b += (int64_t)gridDim.x * blockDim.x) {
+    DevTask t;
+    t.A = A + b * (int64_t)m * k; t.D = B + b * (int64_t)p * n; t.alpha = nullptr; t.coef = alpha;
+    t.e_off = b * (int64_t)k * n; t.m = m; t.k = k; t.n = n; t.p = p; t.strideA = 0; t.strideD = 0; t.npos = 1; t.flags = 0;
+    tasks[b] = t;
+    units[b] = DevUnit{(int32_t)b, 0, 1, 0};
+    for (int i = 0; i < tr * tc; ++i) {
+      DevWork w;
+      w.dst_off = b * (int64_t)m * p; w.unit0 = (int32_t)b; w.unit1 = (int32_t)b + 1;
+      w.row0 = (i / tc) * tm; w.col0 = (i % tc) * tp; w.m = m; w.p = p; w.to_partial = 2; w.wr = wr;
+      work[b * (int64_t)(tr * tc) + i] = w;
+    }
+  }
+}
+
 su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double alpha, const double* A, const double* X,
                             const double* B, double* C, void* stream_v) {
   if (batch == 0) return SU2_OK;
+  cudaStream_t stream = (cudaStream_t)stream_v;
+  if (m >= 64 && p >= 64 && batch < (int64_t)1 << 24) {
+    // smallest tile class whose width covers p (no recomputation of the first product), like the planner
+    const int wr = p <= 144 ? 4 : (p <= 288 ? 2 : 1);
+    const TileShape ts = tile_shape(wr);
+    const int64_t ntile = (int64_t)((m + ts.tm - 1) / ts.tm) * ((p + ts.tp - 1) / ts.tp);
+    const size_t b_task = ((size_t)batch * sizeof(DevTask) + 255) & ~(size_t)255;
+    const size_t b_unit = ((size_t)batch * sizeof(DevUnit) + 255) & ~(size_t)255;
+    const size_t b_work = ((size_t)(batch * ntile) * sizeof(DevWork) + 255) & ~(size_t)255;
+    char* buf = nullptr;
+    cudaError_t e = cudaMallocAsync((void**)&buf, b_task + b_unit + b_work + 256, stream);
+    if (e != cudaSuccess) { set_cuda_error("cudaMallocAsync(gemm_pair tables)", (int)e); return SU2_ERR_CUDA; }
+    DevTask* tasks = (DevTask*)buf;
+    DevUnit* units = (DevUnit*)(buf + b_task);
+    DevWork* work = (DevWork*)(buf + b_task + b_unit);
+    int* counter = (int*)(buf + b_task + b_unit + b_work);
+    gemm_pair_tables_kernel<<<(unsigned)std::min<int64_t>((batch + 127) / 128, 1024), 128, 0, stream>>>(
+        m, k, n, p, batch, alpha, A, B, wr, ts.tm, ts.tp, tasks, units, work, counter);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) { set_cuda_error("gemm_pair_tables_kernel launch", (int)e); return SU2_ERR_CUDA; }
+    count_launch();
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    su2_status st = launch_heff_dmma_tables(work, (int)(batch * ntile), units, tasks, X, C, nullptr, counter, sms, stream_v);
+    cudaFreeAsync(buf, stream);
+    return st;
+  }
   const int tiles = ((m + TILE_M - 1) / TILE_M) * ((p + TILE_P - 1) / TILE_P);
   dim3 grid(tiles, (unsigned)std::min<int64_t>(batch, 65535));
-  gemm_pair_kernel<<<grid, NTHREADS, 0, (cudaStream_t)stream_v>>>(m, k, n, p, batch, alpha, A, X, B, C);
+  gemm_pair_kernel<<<grid, GP_THREADS, 0, stream>>>(m, k, n, p, batch, alpha, A, X, B, C);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { set_cuda_error("gemm_pair_kernel launch", (int)e); return SU2_ERR_CUDA; }
   count_launch();
   return SU2_OK;
 }
-
 
 }  // namespace su2
 

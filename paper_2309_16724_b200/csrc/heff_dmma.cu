@@ -462,7 +462,8 @@ __device__ __forceinline__ void consumer_item(const DevWork* __restrict__ wkp, d
 
   // ---- epilogue: the tile leaves the registers once per work item -----------------------------
   const DevWork wk = *wkp;            // re-read here: nothing of it stays live across the item
-  double* dst = (wk.to_partial ? partial : out) + wk.dst_off;
+  double* dst = ((wk.to_partial & 1) ? partial : out) + wk.dst_off;
+  const bool accumulate = wk.to_partial & 2;
 #pragma unroll
   for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
@@ -472,8 +473,8 @@ __device__ __forceinline__ void consumer_item(const DevWork* __restrict__ wkp, d
         const int q = wk.col0 + (ctile0 + j) * 8 + 2 * t;
         if (r < wk.m) {
           double* o = dst + (int64_t)r * wk.p + q;
-          if (q < wk.p) o[0] = acc[ii][j][0];
-          if (q + 1 < wk.p) o[1] = acc[ii][j][1];
+          if (q < wk.p) o[0] = accumulate ? o[0] + acc[ii][j][0] : acc[ii][j][0];
+          if (q + 1 < wk.p) o[1] = accumulate ? o[1] + acc[ii][j][1] : acc[ii][j][1];
         }
       }
 }
@@ -529,9 +530,9 @@ heff_dmma_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __r
 
 }  // namespace
 
-su2_status launch_heff_dmma(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream_v) {
+su2_status launch_heff_dmma_tables(const DevWork* work, int nwork, const DevUnit* units, const DevTask* tasks, const double* psi,
+                                   double* out, double* partial, int* counter, int num_sms, void* stream_v) {
   cudaStream_t stream = (cudaStream_t)stream_v;
-  const int nwork = (int)plan->h_work.size();
   if (nwork == 0) return SU2_OK;
   static bool attr_set = false;
   const size_t smem_bytes = (size_t)SMEM_DOUBLES_MAX * sizeof(double);
@@ -540,13 +541,17 @@ su2_status launch_heff_dmma(const su2_plan* plan, const double* psi, double* out
     if (e != cudaSuccess) { set_cuda_error("cudaFuncSetAttribute(heff_dmma_kernel)", (int)e); return SU2_ERR_CUDA; }
     attr_set = true;
   }
-  const int grid = std::min(nwork, plan->num_sms);
-  heff_dmma_kernel<<<grid, NTHREADS, smem_bytes, stream>>>(plan->d_work, nwork, plan->d_units, plan->d_tasks, psi, out,
-                                                           partial, plan->d_counter);
+  const int grid = std::min(nwork, num_sms);
+  heff_dmma_kernel<<<grid, NTHREADS, smem_bytes, stream>>>(work, nwork, units, tasks, psi, out, partial, counter);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { set_cuda_error("heff_dmma_kernel launch", (int)e); return SU2_ERR_CUDA; }
   count_launch();
   return SU2_OK;
+}
+
+su2_status launch_heff_dmma(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream_v) {
+  return launch_heff_dmma_tables(plan->d_work, (int)plan->h_work.size(), plan->d_units, plan->d_tasks, psi, out, partial,
+                                 plan->d_counter, plan->num_sms, stream_v);
 }
 
 }  // namespace su2

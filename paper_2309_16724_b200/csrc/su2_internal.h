@@ -35,7 +35,7 @@ struct DevWork {
   int32_t unit0, unit1;   // units [unit0, unit1)
   int32_t row0, col0;     // tile origin inside the (m x p) output block
   int32_t m, p;           // output block dims (p = leading dimension)
-  int32_t to_partial;     // 1: dst_off refers to the partial buffer
+  int32_t to_partial;     // bit 0: dst_off refers to the partial buffer; bit 1: accumulate into dst (dst += tile)
   int32_t wr;             // tile class: warp rows WR of TileCfg<WR> (1, 2 or 4)
 };
 
@@ -132,6 +132,9 @@ struct su2_plan {
 namespace su2 {
 // kernels.cu
 su2_status launch_heff_dmma(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream);   // heff_dmma.cu
+// the same kernel on caller-built tables (gemm_pair.cu); counter = zeroed device int
+su2_status launch_heff_dmma_tables(const DevWork* work, int nwork, const DevUnit* units, const DevTask* tasks, const double* psi,
+                                   double* out, double* partial, int* counter, int num_sms, void* stream);
 su2_status launch_apply(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream);
 su2_status launch_diag(const su2_plan* plan, double* diag, void* stream);
 su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, const std::vector<double>& ident_host,

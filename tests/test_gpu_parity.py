@@ -153,7 +153,8 @@ def test_gpu_result_is_hermitian_and_linear_midi():
 
 
 @pytest.mark.parametrize("m,k,n,p,batch", [(8, 8, 8, 8, 1000), (16, 32, 8, 24, 37), (64, 64, 64, 64, 9),
-                                           (70, 33, 45, 129, 5), (128, 128, 128, 128, 3), (1, 1, 1, 1, 4)])
+                                           (70, 33, 45, 129, 5), (128, 128, 128, 128, 3), (1, 1, 1, 1, 4),
+                                           (512, 512, 512, 512, 2), (200, 70, 300, 600, 2), (65, 8, 8, 64, 300)])
 def test_gemm_pair_batched(m, k, n, p, batch):
     """BASELINE.json configs[4]: C += alpha A X B^T, checked against numpy in FP64."""
     torch = _torch()
@@ -164,7 +165,7 @@ def test_gemm_pair_batched(m, k, n, p, batch):
     dA, dX, dB, dC = (torch.from_numpy(a).cuda() for a in (A, X, B, C0))
     gemm_pair_batched(m, k, n, p, batch, 0.5, dA.data_ptr(), dX.data_ptr(), dB.data_ptr(), dC.data_ptr(),
                       torch.cuda.current_stream().cuda_stream)
-    ref = C0 + 0.5 * np.einsum("bmk,bkn,bpn->bmp", A, X, B)
+    ref = C0 + 0.5 * np.matmul(np.matmul(A, X), np.swapaxes(B, 1, 2))
     assert _rel(dC.cpu().numpy(), ref) <= 1e-12
 
 
