@@ -17,10 +17,12 @@
 // of *phases*: the first product (stages of an A tile + an E tile, KS1 deep) and the second product
 // (stages of a D tile, KS2 deep).  The CTA is warp-specialised:
 //   * warps 0-3 (one warpgroup, 56 registers after setmaxnreg.dec) are PRODUCERS.  Every producer warp
-//     walks every stage and copies a quarter of its tiles with 8-byte cp.async + zero fill (ragged
-//     block sizes and odd leading dimensions need no special cases); completion is signalled on the
-//     stage's "full" mbarrier (cp.async.mbarrier.arrive.noinc).  Lane 0 of warp 0 also runs the phase
-//     iterator (state in shared memory) one phase ahead into a ring of phase descriptors.
+//     walks every stage and copies a quarter of its tiles with cp.async + zero fill (ragged block sizes
+//     and odd leading dimensions need no special cases): 16-byte copies for sources read along their
+//     contiguous direction (E tiles, blocks read transposed -- which includes the plan's transposed
+//     copies of the right-block families), 8-byte copies for the small row-major A tiles.  Completion is
+//     signalled on the stage's "full" mbarrier (cp.async.mbarrier.arrive.noinc).  Lane 0 of warp 0 also
+//     runs the phase iterator (state in shared memory) one phase ahead into a ring of phase descriptors.
 //   * warps 4-11 (two warpgroups, 224 registers after setmaxnreg.inc) are CONSUMERS: they wait on
 //     the stage's "full" mbarrier, issue only LDS + DMMA, and release the stage on its "empty"
 //     mbarrier.  No CTA-wide barrier exists inside an item; the T hand-over between the two
