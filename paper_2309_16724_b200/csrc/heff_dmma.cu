@@ -213,22 +213,28 @@ __device__ __forceinline__ void copy_kmajor(double* dst, const double* __restric
                                             int w, int lane) {
   const int cpad = (cval + 7) & ~7;
   const int jpad = (jval + 3) & ~3;
+  // The rows w, w+4, ... of this warp start at the same parity (4*ld is even) and their shared-memory rows
+  // are one k4 sub-tile apart: everything but two running addresses is set up once per tile.
+  const double* row = src + (int64_t)w * ld;
+  const int pi = addr_parity(row);
+  const int c0 = pi + 2 * lane;
+  unsigned d0 = smem_u32(dst + w * (CT + 4)) + (unsigned)(c0 + pi) * 8u;      // this lane's first pair
+  const char* s0 = reinterpret_cast<const char*>(row + c0);
+  const int64_t rstep = (int64_t)ld * 32;                                      // four rows further (bytes)
 #pragma unroll 1
   for (int j = w; j < jpad; j += 4) {
-    const double* row = src + (int64_t)j * ld;
-    const int pi = addr_parity(row);
-    const unsigned drow = smem_u32(dst + (j >> 2) * (4 * (CT + 4)) + (j & 3) * (CT + 4));
     const int lim = j < jval ? cval : 0;                       // rows beyond the k extent are zero
-    if (pi && lane == 0) cp_async8_raw(drow + 8, row, lim > 0 ? 8 : 0);
-    int c = pi + 2 * lane;
-    unsigned d = drow + (unsigned)(c + pi) * 8u;
-    const char* s = reinterpret_cast<const char*>(row + c);
+    if (pi && lane == 0) cp_async8_raw(d0 - 8, s0 - 8, lim > 0 ? 8 : 0);      // element 0 -> position 1
+    unsigned d = d0;
+    const char* s = s0;
 #pragma unroll 2
-    for (; c < cpad; c += 64) {
+    for (int c = c0; c < cpad; c += 64) {
       cp_async16_raw(d, s, min(16, max(0, (lim - c) * 8)));
       d += 512;
       s += 512;
     }
+    d0 += 4 * (CT + 4) * 8;
+    s0 += rstep;
   }
 }
 

@@ -14,7 +14,7 @@ namespace su2 {
 constexpr int NWARPS = 8;              // consumer (math) warps: two warpgroups
 constexpr int NPRODUCERS = 4;          // producer (cp.async) warps: one warpgroup; each copies a quarter of every tile
 constexpr int NTHREADS = 32 * (NWARPS + NPRODUCERS);
-constexpr int KS1 = 24;         // k extent of one pipeline stage of the first product (six DMMA k4 steps)
+constexpr int KS1 = 32;         // k extent of one pipeline stage of the first product (eight DMMA k4 steps)
 constexpr int KS2 = 12;         // k extent of one pipeline stage of the second product (three DMMA k4 steps)
 constexpr int NT1 = 3;          // n8-tiles per warp, first product
 constexpr int NT2 = 9;          // n8-tiles per warp, second product
@@ -27,7 +27,7 @@ struct TileCfg {
   static constexpr int TP = 8 * NT2 * WC;       // columns of F per CTA       : 576 / 288 / 144
   static constexpr int NC = 8 * NT1 * WC;       // max columns of a T chunk   : 192 / 96 / 48
   static constexpr int LDT = NC + 4;            // leading dimension of T in shared memory
-  static constexpr int NSTAGE = (WR == 1) ? 3 : (WR == 2) ? 5 : 4;   // pipeline depth (what fits beside T in 227 KB)
+  static constexpr int NSTAGE = (WR == 1) ? 3 : (WR == 2) ? 4 : 3;   // pipeline depth (what fits beside T in 227 KB)
   // one pipeline stage (doubles), every tile k-major [k/4][4][C+4]: A tile C = TM, E tile C = NC (KS1 deep),
   // D tile C = TP (KS2 deep).
   static constexpr int A_SZ = KS1 * (TM + 4);
