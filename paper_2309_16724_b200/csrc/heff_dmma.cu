@@ -173,24 +173,26 @@ __device__ __forceinline__ void cp_async8_raw(unsigned dst, const void* src, int
 }
 // Source stored c-major, element (c, j) = src[c*ld + j]: 8 consecutive lanes read one 64-byte run, a warp
 // instruction covers 4 rows; producer warp w takes the row groups  c/4 = w (mod 4).
-template <int CT>
+template <int CT, int KSX>
 __device__ __forceinline__ void copy_cmajor(double* dst, const double* __restrict__ src, int ld, int cval, int jval,
                                             int w, int lane) {
   const int j = lane & 7, r = 4 * w + (lane >> 3);
-  if (j >= ((jval + 3) & ~3)) return;
+  const int jpad = (jval + 3) & ~3;                  // the consumers read whole k4 sub-tiles
+  const int cpad = (cval + 7) & ~7;
   unsigned d = smem_u32(dst + (j >> 2) * (4 * (CT + 4)) + (j & 3) * (CT + 4) + r);
   const char* s = reinterpret_cast<const char*>(src + (int64_t)r * ld + j);
   const int64_t sstep = (int64_t)ld * 128;           // sixteen rows further
-  const int szj = j < jval ? 8 : 0;
-  const int cpad = (cval + 7) & ~7;
-  int c = r;
-#pragma unroll 2
-  for (; c < cval; c += 16) {
-    cp_async8_raw(d, s, szj);
+#pragma unroll 1
+  for (int c = r; c < cpad; c += 16) {               // rows beyond the block (fewer than 8) are zero-filled
+    const bool rowok = c < cval;
+#pragma unroll
+    for (int g = 0; g < (KSX + 7) / 8; ++g)          // groups of 8 k columns = 2 sub-tiles = 8 (CT+4) doubles apart
+      if (8 * g + j < jpad)
+        cp_async8_raw(d + g * (8 * (CT + 4) * 8), rowok ? s + g * 64 : reinterpret_cast<const char*>(src),
+                      (rowok && 8 * g + j < jval) ? 8 : 0);
     d += 128;
     s += sstep;
   }
-  if (c < cpad) cp_async8_raw(d, src, 0);            // rows beyond the block (fewer than 8): zero fill
 }
 // Source stored k-major, element (c, j) = src[j*ld + c]: runs along c are contiguous, so they move with
 // 16-byte cp.async (half the LSU instructions of the 8-byte path: 19.7 vs 9.3 TB/s measured for this
@@ -328,18 +330,14 @@ __device__ __forceinline__ void producer_item(const DevWork* __restrict__ wkp, c
           if (flags & PH_TRANS) {
             copy_kmajor<C::TM>(stage, src0, d.ld0, d.cval0, jval, w, lane);
           } else {
-#pragma unroll 1
-            for (int j0 = 0; j0 < jval; j0 += 8)       // copy_cmajor moves 8 k columns per call
-              copy_cmajor<C::TM>(stage + j0 * (C::TM + 4), src0 + j0, d.ld0, d.cval0, jval - j0, w, lane);
+            copy_cmajor<C::TM, KS1>(stage, src0, d.ld0, d.cval0, jval, w, lane);
           }
           copy_kmajor<C::NC>(stage + C::A_SZ, d.src1 + (int64_t)s * d.stride1, d.ld1, d.cval1, jval, w, lane);
         } else {
           const int jval = min(KS2, d.ktot - s * KS2);
           if (flags & PH_TRANS) copy_kmajor<C::TP>(stage, src0, d.ld0, d.cval0, jval, w, lane);
           else {
-#pragma unroll 1
-            for (int j0 = 0; j0 < jval; j0 += 8)
-              copy_cmajor<C::TP>(stage + j0 * (C::TP + 4), src0 + j0, d.ld0, d.cval0, jval - j0, w, lane);
+            copy_cmajor<C::TP, KS2>(stage, src0, d.ld0, d.cval0, jval, w, lane);
           }
         }
       }
