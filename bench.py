@@ -36,8 +36,8 @@ FP64_OVER_BF16_NOMINAL = 45.0 / 2250.0
 
 def ncu_traffic(cfg_name):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of heff_dmma_kernel from the committed
-    ncu --set full capture of this workload (profiles/traffic.json), or None."""
-    path = os.path.join(ROOT, "profiles", "traffic.json")
+    ncu --set full capture of this workload (profiles/r01_traffic_per_launch.txt), or None."""
+    path = os.path.join(ROOT, "profiles", "r01_traffic_per_launch.txt")
     if os.path.exists(path):
         with open(path) as f:
             return json.load(f).get(cfg_name)
