@@ -2,11 +2,14 @@
 //   C_b += alpha * A_b X_b B_b^T, one independent item per batch index.
 // Items with at least 64 x 64 outputs run on the fused DMMA kernel of the hot path (heff_dmma.cu): a small
 // kernel writes one task / unit / work-item record per batch item (and output tile) and the persistent
-// kernel consumes them with the accumulate flag.  Smaller items stay on the FP64-FMA tile routine below:
-// the DMMA kernel's per-item pipeline set-up (a few microseconds) would dominate them.
+// kernel consumes them with the accumulate flag.  Items whose operands fit half an SM's shared memory run on
+// the small-block kernel (gemm_pair_small.cu, many items in flight per SM).  What is left (e.g. 8 x 512 x 512 x 8)
+// uses the FP64-FMA tile routine below.
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <cstdio>
+#include <cstdlib>
 
 #include "su2_internal.h"
 #include "tile_config.h"
@@ -187,6 +190,19 @@ su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double al
     su2_status st = launch_heff_dmma_tables(work, (int)(batch * ntile), units, tasks, X, C, nullptr, counter, sms, stream_v);
     cudaFreeAsync(buf, stream);
     return st;
+  }
+  {
+    // small-block regime (HBM-bound): one CTA of 1-4 warps per item, shared memory sized by the item shape.
+    // SU2_GEMM_PAIR_SMALL="wpi,nbuf" overrides the heuristics (tuning aid; "0" disables the kernel).
+    int wpi = 0, nbuf = 0;
+    bool off = false;
+    if (const char* env = std::getenv("SU2_GEMM_PAIR_SMALL")) {
+      if (std::sscanf(env, "%d,%d", &wpi, &nbuf) >= 1 && wpi == 0) off = true;
+    }
+    if (!off) {
+      su2_status st = launch_gemm_pair_small(m, k, n, p, batch, alpha, A, X, B, C, stream_v, wpi, nbuf);
+      if (st != 1) return st;
+    }
   }
   const int tiles = ((m + TILE_M - 1) / TILE_M) * ((p + TILE_P - 1) / TILE_P);
   dim3 grid(tiles, (unsigned)std::min<int64_t>(batch, 65535));

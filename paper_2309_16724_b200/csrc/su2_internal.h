@@ -145,6 +145,9 @@ su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, co
 void free_plan_device(su2_plan* plan);
 su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double alpha, const double* A, const double* X,
                             const double* B, double* C, void* stream);
+// gemm_pair_small.cu: returns SU2_OK after launching, 1 if the item shape does not fit the small-block kernel
+su2_status launch_gemm_pair_small(int m, int k, int n, int p, int64_t batch, double alpha, const double* A, const double* X,
+                                  const double* B, double* C, void* stream, int wpi_force, int nbuf_force);
 void set_cuda_error(const char* what, int code);
 void count_launch(int n = 1);   // kernels launched by this library since load (bench.py's gpu_launches)
 // wigner (plan.cpp)

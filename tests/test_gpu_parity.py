@@ -154,7 +154,14 @@ def test_gpu_result_is_hermitian_and_linear_midi():
 
 @pytest.mark.parametrize("m,k,n,p,batch", [(8, 8, 8, 8, 1000), (16, 32, 8, 24, 37), (64, 64, 64, 64, 9),
                                            (70, 33, 45, 129, 5), (128, 128, 128, 128, 3), (1, 1, 1, 1, 4),
-                                           (512, 512, 512, 512, 2), (200, 70, 300, 600, 2), (65, 8, 8, 64, 300)])
+                                           (512, 512, 512, 512, 2), (200, 70, 300, 600, 2), (65, 8, 8, 64, 300),
+                                           # small-block kernel: square sweep shapes, ragged / odd shapes (8-byte
+                                           # copies), 1, 2 and 4 warps per item, more items than resident CTAs
+                                           (16, 16, 16, 16, 20000), (32, 32, 32, 32, 3000), (7, 5, 9, 3, 501),
+                                           (24, 46, 30, 40, 50), (33, 17, 25, 47, 20), (6, 46, 12, 31, 777),
+                                           (48, 48, 48, 48, 40), (8, 8, 8, 8, 300000), (2, 64, 2, 5, 33),
+                                           # too big for the small-block kernel, too narrow for the DMMA tiles
+                                           (8, 512, 512, 8, 3)])
 def test_gemm_pair_batched(m, k, n, p, batch):
     """BASELINE.json configs[4]: C += alpha A X B^T, checked against numpy in FP64."""
     torch = _torch()
@@ -167,6 +174,28 @@ def test_gemm_pair_batched(m, k, n, p, batch):
                       torch.cuda.current_stream().cuda_stream)
     ref = C0 + 0.5 * np.matmul(np.matmul(A, X), np.swapaxes(B, 1, 2))
     assert _rel(dC.cpu().numpy(), ref) <= 1e-12
+
+
+@pytest.mark.gpu
+def test_gemm_pair_batched_unaligned_and_repeatable():
+    """Operands that start 8 bytes off a 16-byte boundary take the 8-byte copy path of the small-block kernel;
+    two calls on the same inputs give bit-identical results (one CTA owns an item, no atomics)."""
+    torch = _torch()
+    from paper_2309_16724_b200 import gemm_pair_batched
+    m, k, n, p, batch = 12, 20, 16, 10, 4097
+    rng = np.random.default_rng(11)
+    host = [rng.normal(size=(batch, a, b)) for a, b in ((m, k), (k, n), (p, n), (m, p))]
+    ref = host[3] + 0.5 * np.matmul(np.matmul(host[0], host[1]), np.swapaxes(host[2], 1, 2))
+    outs = []
+    for shift in (1, 1, 0):
+        bufs = [torch.zeros(h.size + 1, dtype=torch.float64, device="cuda") for h in host]
+        views = [b[shift:shift + h.size] for b, h in zip(bufs, host)]
+        for v, h in zip(views, host):
+            v.copy_(torch.from_numpy(h.ravel()))
+        gemm_pair_batched(m, k, n, p, batch, 0.5, *(v.data_ptr() for v in views), torch.cuda.current_stream().cuda_stream)
+        outs.append(views[3].cpu().numpy().reshape(batch, m, p))
+    assert _rel(outs[0], ref) <= 1e-12 and _rel(outs[2], ref) <= 1e-12
+    assert np.array_equal(outs[0], outs[1])
 
 
 def _wide_problem():
