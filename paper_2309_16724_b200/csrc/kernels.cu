@@ -232,8 +232,9 @@ void free_plan_device(su2_plan* plan) {
 
 su2_status launch_apply(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream_v) {
   cudaStream_t stream = (cudaStream_t)stream_v;
-  SU2_CUDA(cudaMemsetAsync(plan->d_counter, 0, sizeof(int32_t), stream));
-  su2_status st = launch_heff_dmma(plan, psi, out, partial, stream_v);
+  SU2_CUDA(cudaMemsetAsync(plan->d_counter, 0, 8 * sizeof(int32_t), stream));   // [0]: work queue; small plans: one per size class
+  su2_status st = plan->small_dm8 > 0 ? launch_heff_small(plan, psi, out, partial, stream_v)
+                                      : launch_heff_dmma(plan, psi, out, partial, stream_v);
   if (st != SU2_OK) return st;
   const int nsec = (int)plan->h_reduce.size();
   if (nsec > 0) {

@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <chrono>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <tuple>
@@ -307,8 +308,23 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
   // is one contiguous run per k row (16-byte cp.async, 11-19 TB/s).  Families that are used as stored by
   // position-batched rows therefore get a transposed copy at plan time (transpose_kernel); if the copy
   // does not fit in device memory the plan falls back to the stored layout.
-  std::vector<std::vector<int64_t>> trans_blk_off(p->nfam_r);
+  // ---- small-block plan? (heff_small.cu) -------------------------------------------------------
+  // Every block sector of the bond holds at most SMALL_MAX_DIM multiplets: the whole apply runs on
+  // heff_small_kernel (one CTA per output sector and segment), which reads blocks in either orientation at full
+  // speed, so no transposed copies are made.  SU2_HEFF_SMALL=0 in the environment keeps the large-tile kernel
+  // (A/B measurements only).
   {
+    int maxdim = 0;
+    for (const su2_sector& q : plan->sec_l) maxdim = std::max(maxdim, (int)q.dim);
+    for (const su2_sector& q : plan->sec_r) maxdim = std::max(maxdim, (int)q.dim);
+    const char* env = std::getenv("SU2_HEFF_SMALL");
+    const bool off = env && env[0] == '0';
+    plan->small_dm8 = (maxdim <= SMALL_MAX_DIM && !off) ? std::max(8, (maxdim + 7) & ~7) : 0;
+  }
+  const bool small_plan = plan->small_dm8 > 0;
+
+  std::vector<std::vector<int64_t>> trans_blk_off(p->nfam_r);
+  if (!small_plan) {
     std::vector<char> need(p->nfam_r, 0);
     for (const HostTask& ht : plan->tasks)
       if (ht.fam_r >= 0 && !ht.adj_r && fold_side[ht.term] != 1 && p->fam_r[ht.fam_r].npos > 1) need[ht.fam_r] = 1;
@@ -412,6 +428,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
     if (first_task[s + 1] == first_task[s]) continue;
     double best = -1.0;
     for (int wr : {1, 2, 4}) {
+      if (small_plan && wr != 4) continue;   // cost unit of a small plan: the 128 x 144 class (one tile per sector)
       double c = 0.0;
       for (int64_t i = first_task[s]; i < first_task[s + 1]; ++i) c += pos_cost_all_tiles(wr, plan->tasks[i]) * plan->tasks[i].npos;
       if (best < 0.0 || c < best * 0.97) {   // prefer the smaller tile unless the larger one is clearly cheaper
@@ -421,9 +438,19 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
     sec_cost[s] = best;
     total_cost += best;
   }
-  const double executed = total_cost * NWARPS * 512.0;   // DMMA issue slots x 8 warps x 2*8*8*4 flop
+  double executed = total_cost * NWARPS * 512.0;   // DMMA issue slots x 8 warps x 2*8*8*4 flop
+  if (small_plan) {   // heff_small_kernel: m8n8k4 tiles over (m8, k4, n8) and (m8, n8, p8)
+    executed = 0.0;
+    for (const HostTask& ht : plan->tasks) {
+      const double m8 = (ht.m + 7) & ~7, k4 = (ht.k + 3) & ~3, n8 = (ht.n + 7) & ~7, p8 = (ht.p + 7) & ~7;
+      executed += ht.npos * 2.0 * (m8 * k4 * n8 + m8 * n8 * p8);
+    }
+  }
   // target cost of one work item: ~24 items per SM, but never so small that the pipeline fill dominates
-  const double target = (flags & SU2_PLAN_FORCE_SPLIT) ? 40.0 : std::max(total_cost / (148.0 * 24.0), 2.0e4);
+  // (small plans: a step costs a few hundred cycles and up to 16 CTAs are resident per SM: ~48 items per SM, low floor)
+  const double target = (flags & SU2_PLAN_FORCE_SPLIT) ? 40.0
+                        : small_plan ? std::max(total_cost / (148.0 * 48.0), 3.0e2)
+                                     : std::max(total_cost / (148.0 * 24.0), 2.0e4);
   plan->partial_elems = 0;
   std::vector<double> work_cost;   // for LPT ordering
   for (int s = 0; s < nsec; ++s) {
@@ -501,7 +528,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
           wk.row0 = r0; wk.col0 = c0; wk.m = ps.m; wk.p = ps.p;
           wk.to_partial = nseg > 1 ? 1 : 0;
           wk.dst_off = nseg > 1 ? red.part_off + (int64_t)g * sz : ps.off;
-          wk.wr = wr;
+          wk.wr = small_plan ? 0 : wr;
           plan->h_work.push_back(wk);
           work_cost.push_back(w);
         }
@@ -512,7 +539,25 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
   {
     std::vector<int64_t> order(plan->h_work.size());
     for (size_t i = 0; i < order.size(); ++i) order[i] = (int64_t)i;
-    std::stable_sort(order.begin(), order.end(), [&](int64_t a, int64_t b) { return work_cost[a] > work_cost[b]; });
+    // small plans: first by size class (largest dimension over the item's tasks, rounded up to 8), see heff_small.cu
+    std::vector<int> cls(order.size(), 0);
+    if (small_plan) {
+      for (size_t i = 0; i < order.size(); ++i) {
+        int dmax = 1;
+        for (int32_t u = plan->h_work[i].unit0; u < plan->h_work[i].unit1; ++u) {
+          const HostTask& ht = plan->tasks[plan->h_units[u].task];
+          dmax = std::max({dmax, (int)ht.m, (int)ht.k, (int)ht.n, (int)ht.p});
+        }
+        cls[i] = (dmax + 7) / 8 - 1;
+      }
+      for (int c = 0; c < 7; ++c) plan->small_begin[c] = 0;
+      for (size_t i = 0; i < order.size(); ++i) plan->small_begin[cls[i] + 1]++;
+      for (int c = 0; c < 6; ++c) plan->small_begin[c + 1] += plan->small_begin[c];
+    }
+    std::stable_sort(order.begin(), order.end(), [&](int64_t a, int64_t b) {
+      if (cls[a] != cls[b]) return cls[a] < cls[b];
+      return work_cost[a] > work_cost[b];
+    });
     std::vector<DevWork> sorted(order.size());
     for (size_t i = 0; i < order.size(); ++i) sorted[i] = plan->h_work[order[i]];
     plan->h_work.swap(sorted);

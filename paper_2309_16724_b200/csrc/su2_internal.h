@@ -24,6 +24,10 @@ struct DevTask {
 };
 enum : uint32_t { TASK_TRANS_A = 1u, TASK_TRANS_D = 2u };
 
+// A bond whose block sectors all hold at most this many multiplets runs on heff_small_kernel (heff_small.cu)
+// instead of the 128 x 144 / 64 x 288 / 32 x 576 register tiles of heff_dmma_kernel.
+constexpr int SMALL_MAX_DIM = 48;
+
 // A run of positions of one task inside one segment.
 struct DevUnit {
   int32_t task, pos0, pos1, pad;
@@ -36,7 +40,7 @@ struct DevWork {
   int32_t row0, col0;     // tile origin inside the (m x p) output block
   int32_t m, p;           // output block dims (p = leading dimension)
   int32_t to_partial;     // bit 0: dst_off refers to the partial buffer; bit 1: accumulate into dst (dst += tile)
-  int32_t wr;             // tile class: warp rows WR of TileCfg<WR> (1, 2 or 4)
+  int32_t wr;             // tile class: warp rows WR of TileCfg<WR> (1, 2 or 4); 0 = whole sector (heff_small_kernel)
 };
 
 // Second pass of the deterministic segmented reduction: F_s = sum_{seg} partial[seg] in index order.
@@ -127,6 +131,8 @@ struct su2_plan {
   void* d_psi_sec = nullptr;           // device copy of `psi` (PsiSector[])
   int64_t partial_elems = 0;
   int32_t num_sms = 148;
+  int32_t small_dm8 = 0;               // > 0: small-block plan; largest sector dimension rounded up to 8
+  int32_t small_begin[7] = {0, 0, 0, 0, 0, 0, 0};   // small plans: h_work is sorted by size class (DM8 = 8 (c + 1)); class c = [begin[c], begin[c+1])
 };
 
 namespace su2 {
@@ -135,6 +141,7 @@ su2_status launch_heff_dmma(const su2_plan* plan, const double* psi, double* out
 // the same kernel on caller-built tables (gemm_pair.cu); counter = zeroed device int
 su2_status launch_heff_dmma_tables(const DevWork* work, int nwork, const DevUnit* units, const DevTask* tasks, const double* psi,
                                    double* out, double* partial, int* counter, int num_sms, void* stream);
+su2_status launch_heff_small(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream);   // heff_small.cu
 su2_status launch_apply(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream);
 su2_status launch_diag(const su2_plan* plan, double* diag, void* stream);
 su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, const std::vector<double>& ident_host,
