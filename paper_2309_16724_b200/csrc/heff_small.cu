@@ -72,43 +72,102 @@ __device__ __forceinline__ void hs_copy_any(double* dst, int ld, const double* s
   else hs_copy<1, HS_THREADS>(dst, ld, src, rows, cols, rows_pad, cols_pad, tid);
 }
 
+// K loop of one product for a warp that owns NR x NC m8n8 tiles: straight-line per (NR, NC), no predicated
+// DMMAs (a predicated-off DMMA still takes its slot in the FP64 tensor pipe).  ap / bp: this lane's fragment
+// element of tile row 0 / tile column 0 at k = 0; a_i / b_j: distance to the next owned tile; a_k / b_k: per k4 step.
+template <int NR, int NC, int TRM, int TCM>
+__device__ __forceinline__ void hs_mma_loop(double (&acc)[TRM][TCM][2], const double* ap, int a_i, int a_k,
+                                            const double* bp, int b_j, int b_k, int ksteps) {
+#pragma unroll 2
+  for (int s = 0; s < ksteps; ++s) {
+    double a[NR], b[NC];
+#pragma unroll
+    for (int i = 0; i < NR; ++i) a[i] = ap[i * a_i];
+#pragma unroll
+    for (int j = 0; j < NC; ++j) b[j] = bp[j * b_j];
+#pragma unroll
+    for (int i = 0; i < NR; ++i)
+#pragma unroll
+      for (int j = 0; j < NC; ++j) hs_dmma(acc[i][j], a[i], b[j]);
+    ap += a_k;
+    bp += b_k;
+  }
+}
+
+// nr x nc of the warp's TRM x TCM tile slots exist (prefixes): pick the straight-line instance.
+template <int TRM, int TCM>
+__device__ __forceinline__ void hs_mma(double (&acc)[TRM][TCM][2], int nr, int nc, const double* ap, int a_i, int a_k,
+                                       const double* bp, int b_j, int b_k, int ksteps) {
+#define HS_CASE(R, C)                                                                                              \
+  if (R <= TRM && C <= TCM && nr == R && nc == C)                                                                    \
+    hs_mma_loop<(R <= TRM ? R : 1), (C <= TCM ? C : 1), TRM, TCM>(acc, ap, a_i, a_k, bp, b_j, b_k, ksteps);
+  HS_CASE(1, 1) HS_CASE(1, 2) HS_CASE(2, 1) HS_CASE(2, 2) HS_CASE(3, 1) HS_CASE(3, 2)
+#undef HS_CASE
+  static_assert(TRM <= 3 && TCM <= 2, "add HS_CASE lines");
+}
+
 struct Step { int u, pos; };
 
 }  // namespace
 
 
-// Size class DM8 (largest dimension of any task of the item, rounded up to 8), WARPS warps per CTA.
-// Shared memory: four tiles of DM8 x hs_ld(DM8) doubles: A, D, E, T.
-template <int DM8, int WARPS>
-__global__ void __launch_bounds__(32 * WARPS)
+// Size class DM8 (largest dimension of any task of the item, rounded up to 8); WR x WC warps per CTA, warp
+// (wr, wc) owns the m8n8 tiles (wr + WR i, wc + WC j): the A fragment of a tile row is shared by its TCM column
+// tiles and the B fragment of a tile column by its TRM row tiles (5 fragment loads per 6 DMMAs at 48 x 48).
+// Shared memory: four tiles of DM8 x hs_ld(DM8) doubles: A, D, E, T.  Only E carries true zeros in its pads
+// (rows k..K4, columns n..N8): they annihilate whatever finite numbers earlier steps left in the pads of A and
+// D, and make the pad columns of T exact zeros.
+template <int DM8, int WR, int WC>
+__global__ void __launch_bounds__(32 * WR * WC)
 heff_small_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __restrict__ units,
                   const DevTask* __restrict__ tasks, const double* __restrict__ psi, double* __restrict__ out,
                   double* __restrict__ partial, int* __restrict__ counter) {
-  constexpr int THREADS = 32 * WARPS;
-  constexpr int MAXT = ((DM8 / 8) * (DM8 / 8) + WARPS - 1) / WARPS;   // m8n8 tiles per warp
+  constexpr int WARPS = WR * WC, THREADS = 32 * WARPS;
+  constexpr int TRM = (DM8 / 8 + WR - 1) / WR, TCM = (DM8 / 8 + WC - 1) / WC;   // tiles per warp: rows x columns
   constexpr int LD = ((DM8 + 3) & ~7) + 4, SZ = DM8 * LD;
   extern __shared__ __align__(16) double smem[];
   __shared__ int s_item;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int wr = warp % WR, wc = warp / WR;
   const int fr = lane >> 2, fc = lane & 3;
   double* const As = smem;
   double* const Ds = smem + SZ;
   double* const Es = smem + 2 * SZ;
   double* const Ts = smem + 3 * SZ;
-  for (int e = tid; e < 4 * SZ; e += THREADS) smem[e] = 0.0;   // stale pads must at least be finite
+  for (int e = tid; e < 4 * SZ; e += THREADS) smem[e] = 0.0;   // whatever sits in a pad must be finite
 
+  // dense rows x cols block -> shared rows of stride LD, one warp per row; pads untouched
+  auto copy_rows = [&](double* dst, const double* __restrict__ src, int rows, int cols) {
+    if (!(cols & 1) && !((uintptr_t)src & 15)) {
+      const bool on = 2 * lane < cols;
+      for (int r = warp; r < rows; r += WARPS)
+        if (on) hs_cp16(dst + r * LD + 2 * lane, src + (int64_t)r * cols + 2 * lane, true);
+    } else {
+      const bool on0 = lane < cols, on1 = lane + 32 < cols;
+      for (int r = warp; r < rows; r += WARPS) {
+        if (on0) hs_cp8(dst + r * LD + lane, src + (int64_t)r * cols + lane, true);
+        if (DM8 > 32 && on1) hs_cp8(dst + r * LD + lane + 32, src + (int64_t)r * cols + lane + 32, true);
+      }
+    }
+  };
+  // E: the same with zero fill up to rows_pad x cols_pad
+  auto copy_e = [&](const double* __restrict__ src, int rows, int cols, int rows_pad, int cols_pad) {
+    for (int r = warp; r < rows_pad; r += WARPS)
+      for (int c = lane; c < cols_pad; c += 32) {
+        const bool valid = r < rows && c < cols;
+        hs_cp8(Es + r * LD + c, valid ? src + (int64_t)r * cols + c : src, valid);
+      }
+  };
   auto issue_AE = [&](const DevTask& t, int pos, bool with_e) {
-    const int M8 = (t.m + 7) & ~7, K4 = (t.k + 3) & ~3, N8 = (t.n + 7) & ~7;
     const double* A = t.A + (int64_t)pos * t.strideA;
-    if (t.flags & TASK_TRANS_A) hs_copy_any<THREADS>(As, LD, A, t.k, t.m, K4, M8, tid);
-    else hs_copy_any<THREADS>(As, LD, A, t.m, t.k, M8, K4, tid);
-    if (with_e) hs_copy_any<THREADS>(Es, LD, psi + t.e_off, t.k, t.n, K4, N8, tid);
+    if (t.flags & TASK_TRANS_A) copy_rows(As, A, t.k, t.m);
+    else copy_rows(As, A, t.m, t.k);
+    if (with_e) copy_e(psi + t.e_off, t.k, t.n, (t.k + 3) & ~3, (t.n + 7) & ~7);
   };
   auto issue_D = [&](const DevTask& t, int pos) {
-    const int N8 = (t.n + 7) & ~7, P8 = (t.p + 7) & ~7;
     const double* D = t.D + (int64_t)pos * t.strideD;
-    if (t.flags & TASK_TRANS_D) hs_copy_any<THREADS>(Ds, LD, D, t.n, t.p, N8, P8, tid);
-    else hs_copy_any<THREADS>(Ds, LD, D, t.p, t.n, P8, N8, tid);
+    if (t.flags & TASK_TRANS_D) copy_rows(Ds, D, t.n, t.p);
+    else copy_rows(Ds, D, t.p, t.n);
   };
 
   for (;;) {
@@ -118,10 +177,14 @@ heff_small_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __
     const int item = s_item;
     if (item >= nwork) break;
     const DevWork w = work[item];
-    const int pt = (w.p + 7) >> 3, ntile2 = ((w.m + 7) >> 3) * pt;
-    double acc[MAXT][2];
+    const int M8 = (w.m + 7) & ~7, P8 = (w.p + 7) & ~7;
+    // tile rows / tile columns of F this warp owns (prefixes of its TRM x TCM slots; warp-uniform)
+    const int nr = min(TRM, max(0, (M8 / 8 - wr + WR - 1) / WR)), np = min(TCM, max(0, (P8 / 8 - wc + WC - 1) / WC));
+    double acc[TRM][TCM][2];
 #pragma unroll
-    for (int i = 0; i < MAXT; ++i) acc[i][0] = acc[i][1] = 0.0;
+    for (int i = 0; i < TRM; ++i)
+#pragma unroll
+      for (int j = 0; j < TCM; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
     DevUnit un = units[w.unit0];
     DevTask tc = tasks[un.task];
@@ -151,29 +214,23 @@ heff_small_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __
       const int a_sr = (tc.flags & TASK_TRANS_A) ? 1 : LD, a_sc = (tc.flags & TASK_TRANS_A) ? LD : 1;
       const int d_sr = (tc.flags & TASK_TRANS_D) ? 1 : LD, d_sc = (tc.flags & TASK_TRANS_D) ? LD : 1;
 
-      // ---- first product: T = scale * A E, m8n8 tiles dealt round-robin
+      // ---- first product: T = scale * A E
       {
-        const int nt = N8 >> 3, ntile1 = ((tc.m + 7) >> 3) * nt;
-        double tacc[MAXT][2];
-        int aoff[MAXT], eoff[MAXT];
+        const int nn = min(TCM, max(0, (N8 / 8 - wc + WC - 1) / WC));
+        double tacc[TRM][TCM][2];
 #pragma unroll
-        for (int i = 0; i < MAXT; ++i) {
-          const int tl = warp + WARPS * i, tr = tl / nt, tcn = tl - tr * nt;
-          tacc[i][0] = tacc[i][1] = 0.0;
-          aoff[i] = (8 * tr + fr) * a_sr + fc * a_sc;
-          eoff[i] = fc * LD + 8 * tcn + fr;
-        }
-        for (int k0 = 0; k0 < K4; k0 += 4) {
+        for (int i = 0; i < TRM; ++i)
 #pragma unroll
-          for (int i = 0; i < MAXT; ++i)
-            if (warp + WARPS * i < ntile1) hs_dmma(tacc[i], As[aoff[i] + k0 * a_sc], Es[eoff[i] + k0 * LD]);
-        }
+          for (int j = 0; j < TCM; ++j) tacc[i][j][0] = tacc[i][j][1] = 0.0;
+        hs_mma<TRM, TCM>(tacc, nr, nn, As + (8 * wr + fr) * a_sr + fc * a_sc, 8 * WR * a_sr, 4 * a_sc,
+                         Es + fc * LD + 8 * wc + fr, 8 * WC, 4 * LD, K4 >> 2);
 #pragma unroll
-        for (int i = 0; i < MAXT; ++i) {
-          const int tl = warp + WARPS * i, tr = tl / nt, tcn = tl - tr * nt;
-          if (tl < ntile1)
-            *reinterpret_cast<double2*>(Ts + (8 * tr + fr) * LD + 8 * tcn + 2 * fc) = make_double2(scale * tacc[i][0], scale * tacc[i][1]);
-        }
+        for (int i = 0; i < TRM; ++i)
+#pragma unroll
+          for (int j = 0; j < TCM; ++j)
+            if (i < nr && j < nn)
+              *reinterpret_cast<double2*>(Ts + (8 * (wr + WR * i) + fr) * LD + 8 * (wc + WC * j) + 2 * fc) =
+                  make_double2(scale * tacc[i][j][0], scale * tacc[i][j][1]);
       }
       hs_wait<0>();                        // D of this step
       __syncthreads();                     // T and D visible; A and E free
@@ -183,20 +240,8 @@ heff_small_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __
       }
       hs_commit();
       // ---- second product: F += T D^T, K = n (padded to 8)
-      {
-        int toff[MAXT], doff[MAXT];
-#pragma unroll
-        for (int i = 0; i < MAXT; ++i) {
-          const int tl = warp + WARPS * i, tr = tl / pt, tcn = tl - tr * pt;
-          toff[i] = (8 * tr + fr) * LD + fc;
-          doff[i] = (8 * tcn + fr) * d_sr + fc * d_sc;
-        }
-        for (int k0 = 0; k0 < N8; k0 += 4) {
-#pragma unroll
-          for (int i = 0; i < MAXT; ++i)
-            if (warp + WARPS * i < ntile2) hs_dmma(acc[i], Ts[toff[i] + k0], Ds[doff[i] + k0 * d_sc]);
-        }
-      }
+      hs_mma<TRM, TCM>(acc, nr, np, Ts + (8 * wr + fr) * LD + fc, 8 * WR * LD, 4,
+                       Ds + (8 * wc + fr) * d_sr + fc * d_sc, 8 * WC * d_sr, 4 * d_sc, N8 >> 2);
       hs_wait<0>();                        // A (and E) of the next step
       __syncthreads();                     // ... visible; T and D free
       if (has_next) issue_D(tn, nxt.pos);
@@ -208,31 +253,33 @@ heff_small_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __
     // ---- write the sector: plain store, or += for the accumulate flag
     double* dst = ((w.to_partial & 1) ? partial : out) + w.dst_off;
 #pragma unroll
-    for (int i = 0; i < MAXT; ++i) {
-      const int tl = warp + WARPS * i, tr = tl / pt, tcn = tl - tr * pt;
-      const int r = 8 * tr + fr, c = 8 * tcn + 2 * fc;
-      if (tl < ntile2 && r < w.m) {
-        double* q = dst + (int64_t)r * w.p + c;
-        if (w.to_partial & 2) {
-          if (c < w.p) q[0] += acc[i][0];
-          if (c + 1 < w.p) q[1] += acc[i][1];
-        } else {
-          if (c < w.p) q[0] = acc[i][0];
-          if (c + 1 < w.p) q[1] = acc[i][1];
+    for (int i = 0; i < TRM; ++i)
+#pragma unroll
+      for (int j = 0; j < TCM; ++j) {
+        const int r = 8 * (wr + WR * i) + fr, c = 8 * (wc + WC * j) + 2 * fc;
+        if (i < nr && j < np && r < w.m) {
+          double* q = dst + (int64_t)r * w.p + c;
+          if (w.to_partial & 2) {
+            if (c < w.p) q[0] += acc[i][j][0];
+            if (c + 1 < w.p) q[1] += acc[i][j][1];
+          } else {
+            if (c < w.p) q[0] = acc[i][j][0];
+            if (c + 1 < w.p) q[1] = acc[i][j][1];
+          }
         }
       }
-    }
   }
 }
 
 namespace {
 
-template <int DM8, int WARPS>
+template <int DM8, int WR, int WC>
 su2_status launch_class(const su2_plan* plan, int cls, const double* psi, double* out, double* partial, cudaStream_t stream) {
   const int begin = plan->small_begin[cls], nwork = plan->small_begin[cls + 1] - begin;
   if (nwork <= 0) return SU2_OK;
   const size_t smem = sizeof(double) * 4 * (size_t)DM8 * hs_ld(DM8);
-  auto kern = heff_small_kernel<DM8, WARPS>;
+  constexpr int WARPS = WR * WC;
+  auto kern = heff_small_kernel<DM8, WR, WC>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) { set_cuda_error("cudaFuncSetAttribute(heff_small_kernel)", (int)e); return SU2_ERR_CUDA; }
   int per_sm = 0;
@@ -253,12 +300,12 @@ su2_status launch_class(const su2_plan* plan, int cls, const double* psi, double
 su2_status launch_heff_small(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream_v) {
   cudaStream_t stream = (cudaStream_t)stream_v;
   su2_status st;
-  if ((st = launch_class<48, 8>(plan, 5, psi, out, partial, stream)) != SU2_OK) return st;
-  if ((st = launch_class<40, 8>(plan, 4, psi, out, partial, stream)) != SU2_OK) return st;
-  if ((st = launch_class<32, 4>(plan, 3, psi, out, partial, stream)) != SU2_OK) return st;
-  if ((st = launch_class<24, 4>(plan, 2, psi, out, partial, stream)) != SU2_OK) return st;
-  if ((st = launch_class<16, 4>(plan, 1, psi, out, partial, stream)) != SU2_OK) return st;
-  return launch_class<8, 1>(plan, 0, psi, out, partial, stream);
+  if ((st = launch_class<48, 2, 4>(plan, 5, psi, out, partial, stream)) != SU2_OK) return st;
+  if ((st = launch_class<40, 2, 4>(plan, 4, psi, out, partial, stream)) != SU2_OK) return st;
+  if ((st = launch_class<32, 2, 2>(plan, 3, psi, out, partial, stream)) != SU2_OK) return st;
+  if ((st = launch_class<24, 2, 2>(plan, 2, psi, out, partial, stream)) != SU2_OK) return st;
+  if ((st = launch_class<16, 2, 2>(plan, 1, psi, out, partial, stream)) != SU2_OK) return st;
+  return launch_class<8, 1, 1>(plan, 0, psi, out, partial, stream);
 }
 
 }  // namespace su2

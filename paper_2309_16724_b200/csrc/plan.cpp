@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <chrono>
 #include <cmath>
+#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <map>
@@ -435,6 +436,8 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
         if (best < 0.0 || c < best) { best = c; sec_wr[s] = wr; }
       }
     }
+    if (small_plan)   // + the fixed cost of a step (see step_cost below)
+      for (int64_t i = first_task[s]; i < first_task[s + 1]; ++i) best += 60.0 * plan->tasks[i].npos;
     sec_cost[s] = best;
     total_cost += best;
   }
@@ -467,8 +470,10 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
     const TileShape ts = tile_shape(wr);
     const int ntiles = ((ps.m + ts.tm - 1) / ts.tm) * ((ps.p + ts.tp - 1) / ts.tp);
     // per-tile cost of a position: the full row tile (the ragged last one is cheaper; LPT evens that out)
+    // small plans: a step (one position) costs two CTA barriers and a trip to L2 whatever the block size
+    const double step_cost = small_plan ? 60.0 : 0.0;
     auto pos_cost = [&](const HostTask& ht) {
-      return tile_pos_cost(wr, std::min(ts.tm, ht.m), std::min(ts.tp, ht.p), ht.k, ht.n);
+      return step_cost + tile_pos_cost(wr, std::min(ts.tm, ht.m), std::min(ts.tp, ht.p), ht.k, ht.n);
     };
     double tile_work = 0.0;
     for (int64_t i = t0; i < t1; ++i) tile_work += pos_cost(plan->tasks[i]) * plan->tasks[i].npos;
@@ -520,7 +525,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
           double w = 0.0;
           for (int32_t u = segs[g].first; u < segs[g].second; ++u) {
             const HostTask& ht = plan->tasks[plan->h_units[u].task];
-            w += tile_pos_cost(wr, std::min(ts.tm, ps.m - r0), std::min(ts.tp, ps.p - c0), ht.k, ht.n) *
+            w += (step_cost + tile_pos_cost(wr, std::min(ts.tm, ps.m - r0), std::min(ts.tp, ps.p - c0), ht.k, ht.n)) *
                  (plan->h_units[u].pos1 - plan->h_units[u].pos0);
           }
           DevWork wk{};
@@ -550,9 +555,40 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
         }
         cls[i] = (dmax + 7) / 8 - 1;
       }
+      // a class with too few items to fill the GPU joins the next larger populated class (its kernel handles any
+      // smaller block; one under-filled launch less)
+      {
+        int count[6] = {0, 0, 0, 0, 0, 0};
+        for (size_t i = 0; i < order.size(); ++i) count[cls[i]]++;
+        int remap[6];
+        for (int c = 0; c < 6; ++c) remap[c] = c;
+        for (int c = 0; c < 5; ++c) {
+          if (count[c] == 0 || count[c] >= 4 * 148) continue;
+          int up = c + 1;
+          while (up < 6 && count[up] == 0) ++up;
+          if (up < 6) { count[up] += count[c]; count[c] = 0; remap[c] = up; }
+        }
+        for (int c = 0; c < 6; ++c) while (remap[remap[c]] != remap[c]) remap[c] = remap[remap[c]];
+        for (size_t i = 0; i < order.size(); ++i) cls[i] = remap[cls[i]];
+      }
       for (int c = 0; c < 7; ++c) plan->small_begin[c] = 0;
       for (size_t i = 0; i < order.size(); ++i) plan->small_begin[cls[i] + 1]++;
       for (int c = 0; c < 6; ++c) plan->small_begin[c + 1] += plan->small_begin[c];
+      if (std::getenv("SU2_PLAN_DEBUG")) {
+        int64_t steps[6] = {0}, maxsteps[6] = {0}; double dm[6] = {0};
+        for (size_t i = 0; i < order.size(); ++i) {
+          int64_t st = 0;
+          for (int32_t u = plan->h_work[i].unit0; u < plan->h_work[i].unit1; ++u) {
+            const HostTask& ht = plan->tasks[plan->h_units[u].task];
+            const int np = plan->h_units[u].pos1 - plan->h_units[u].pos0;
+            st += np;
+            dm[cls[i]] += np * (double)(((ht.m + 7) / 8) * ((ht.n + 7) / 8) * ((ht.k + 3) / 4) + ((ht.m + 7) / 8) * ((ht.p + 7) / 8) * ((ht.n + 7) / 8) * 2);
+          }
+          steps[cls[i]] += st; maxsteps[cls[i]] = std::max(maxsteps[cls[i]], st);
+        }
+        for (int c = 0; c < 6; ++c)
+          fprintf(stderr, "class %d: items %d steps %lld maxsteps/item %lld dmma %.0f\n", 8 * (c + 1), plan->small_begin[c + 1] - plan->small_begin[c], (long long)steps[c], (long long)maxsteps[c], dm[c]);
+      }
     }
     std::stable_sort(order.begin(), order.end(), [&](int64_t a, int64_t b) {
       if (cls[a] != cls[b]) return cls[a] < cls[b];
