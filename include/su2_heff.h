@@ -130,6 +130,10 @@ typedef struct {
   int64_t nwork_items;       /* CTA-level work items per apply                                  */
   double plan_seconds;       /* host time spent in su2_plan_create                              */
   int64_t plan_device_bytes; /* device memory owned by the plan (tables, folded and transposed operators) */
+  int32_t small_plan;        /* 1: every block sector holds <= 48 multiplets, su2_heff_apply runs the small-block
+                                kernel (one CTA per output sector and segment); 0: large register tiles.
+                                SU2_HEFF_SMALL=0 in the environment of su2_plan_create forces 0 (A/B measurements) */
+  int32_t reserved;
 } su2_plan_info_t;
 
 /* Build the plan: enumerate the sector tasks (Eq. (3)), compute the coefficient of each

@@ -1,10 +1,10 @@
 // Strided-batched FP64 GEMM-pair microbenchmark entry (BASELINE.json configs[4]):
 //   C_b += alpha * A_b X_b B_b^T, one independent item per batch index.
-// Items with at least 64 x 64 outputs run on the fused DMMA kernel of the hot path (heff_dmma.cu): a small
+// Larger items with at least 64 x 64 outputs run on the fused DMMA kernel of the hot path (heff_dmma.cu): a small
 // kernel writes one task / unit / work-item record per batch item (and output tile) and the persistent
-// kernel consumes them with the accumulate flag.  Items whose operands fit half an SM's shared memory run on
-// the small-block kernel (gemm_pair_small.cu, many items in flight per SM).  What is left (e.g. 8 x 512 x 512 x 8)
-// uses the FP64-FMA tile routine below.
+// kernel consumes them with the accumulate flag.  Items whose operands fit an SM's shared memory are tried first
+// on the small-block kernel (gemm_pair_small.cu, whole items per CTA, many in flight per SM).  What is left
+// (e.g. 8 x 512 x 512 x 8) uses the FP64-FMA tile routine below.
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -164,6 +164,20 @@ su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double al
                             const double* B, double* C, void* stream_v) {
   if (batch == 0) return SU2_OK;
   cudaStream_t stream = (cudaStream_t)stream_v;
+  {
+    // items whose operands fit one SM's shared memory (all dims <= 80 for square shapes): one CTA of 1-16 warps per
+    // item, shared memory sized by the item shape (gemm_pair_small.cu).
+    // SU2_GEMM_PAIR_SMALL="wpi,nbuf" overrides the heuristics (tuning aid; "0" disables the kernel).
+    int wpi = 0, nbuf = 0;
+    bool off = false;
+    if (const char* env = std::getenv("SU2_GEMM_PAIR_SMALL")) {
+      if (std::sscanf(env, "%d,%d", &wpi, &nbuf) >= 1 && wpi == 0) off = true;
+    }
+    if (!off) {
+      su2_status st = launch_gemm_pair_small(m, k, n, p, batch, alpha, A, X, B, C, stream_v, wpi, nbuf);
+      if (st != 1) return st;
+    }
+  }
   if (m >= 64 && p >= 64 && batch < (int64_t)1 << 24) {
     // smallest tile class whose width covers p (no recomputation of the first product), like the planner
     const int wr = p <= 144 ? 4 : (p <= 288 ? 2 : 1);
@@ -190,19 +204,6 @@ su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double al
     su2_status st = launch_heff_dmma_tables(work, (int)(batch * ntile), units, tasks, X, C, nullptr, counter, sms, stream_v);
     cudaFreeAsync(buf, stream);
     return st;
-  }
-  {
-    // small-block regime (HBM-bound): one CTA of 1-4 warps per item, shared memory sized by the item shape.
-    // SU2_GEMM_PAIR_SMALL="wpi,nbuf" overrides the heuristics (tuning aid; "0" disables the kernel).
-    int wpi = 0, nbuf = 0;
-    bool off = false;
-    if (const char* env = std::getenv("SU2_GEMM_PAIR_SMALL")) {
-      if (std::sscanf(env, "%d,%d", &wpi, &nbuf) >= 1 && wpi == 0) off = true;
-    }
-    if (!off) {
-      su2_status st = launch_gemm_pair_small(m, k, n, p, batch, alpha, A, X, B, C, stream_v, wpi, nbuf);
-      if (st != 1) return st;
-    }
   }
   const int tiles = ((m + TILE_M - 1) / TILE_M) * ((p + TILE_P - 1) / TILE_P);
   dim3 grid(tiles, (unsigned)std::min<int64_t>(batch, 65535));

@@ -117,8 +117,8 @@ struct Step { int u, pos; };
 // Shared memory: four tiles of DM8 x hs_ld(DM8) doubles: A, D, E, T.  Only E carries true zeros in its pads
 // (rows k..K4, columns n..N8): they annihilate whatever finite numbers earlier steps left in the pads of A and
 // D, and make the pad columns of T exact zeros.
-template <int DM8, int WR, int WC>
-__global__ void __launch_bounds__(32 * WR * WC)
+template <int DM8, int WR, int WC, int MINB>
+__global__ void __launch_bounds__(32 * WR * WC, MINB)
 heff_small_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __restrict__ units,
                   const DevTask* __restrict__ tasks, const double* __restrict__ psi, double* __restrict__ out,
                   double* __restrict__ partial, int* __restrict__ counter) {
@@ -273,13 +273,13 @@ heff_small_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __
 
 namespace {
 
-template <int DM8, int WR, int WC>
+template <int DM8, int WR, int WC, int MINB>
 su2_status launch_class(const su2_plan* plan, int cls, const double* psi, double* out, double* partial, cudaStream_t stream) {
   const int begin = plan->small_begin[cls], nwork = plan->small_begin[cls + 1] - begin;
   if (nwork <= 0) return SU2_OK;
   const size_t smem = sizeof(double) * 4 * (size_t)DM8 * hs_ld(DM8);
   constexpr int WARPS = WR * WC;
-  auto kern = heff_small_kernel<DM8, WR, WC>;
+  auto kern = heff_small_kernel<DM8, WR, WC, MINB>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) { set_cuda_error("cudaFuncSetAttribute(heff_small_kernel)", (int)e); return SU2_ERR_CUDA; }
   int per_sm = 0;
@@ -300,12 +300,12 @@ su2_status launch_class(const su2_plan* plan, int cls, const double* psi, double
 su2_status launch_heff_small(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream_v) {
   cudaStream_t stream = (cudaStream_t)stream_v;
   su2_status st;
-  if ((st = launch_class<48, 2, 4>(plan, 5, psi, out, partial, stream)) != SU2_OK) return st;
-  if ((st = launch_class<40, 2, 4>(plan, 4, psi, out, partial, stream)) != SU2_OK) return st;
-  if ((st = launch_class<32, 2, 2>(plan, 3, psi, out, partial, stream)) != SU2_OK) return st;
-  if ((st = launch_class<24, 2, 2>(plan, 2, psi, out, partial, stream)) != SU2_OK) return st;
-  if ((st = launch_class<16, 2, 2>(plan, 1, psi, out, partial, stream)) != SU2_OK) return st;
-  return launch_class<8, 1, 1>(plan, 0, psi, out, partial, stream);
+  if ((st = launch_class<48, 2, 4, 2>(plan, 5, psi, out, partial, stream)) != SU2_OK) return st;
+  if ((st = launch_class<40, 2, 4, 3>(plan, 4, psi, out, partial, stream)) != SU2_OK) return st;
+  if ((st = launch_class<32, 2, 2, 6>(plan, 3, psi, out, partial, stream)) != SU2_OK) return st;
+  if ((st = launch_class<24, 2, 2, 8>(plan, 2, psi, out, partial, stream)) != SU2_OK) return st;
+  if ((st = launch_class<16, 2, 2, 8>(plan, 1, psi, out, partial, stream)) != SU2_OK) return st;
+  return launch_class<8, 1, 1, 16>(plan, 0, psi, out, partial, stream);
 }
 
 }  // namespace su2

@@ -574,21 +574,6 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
       for (int c = 0; c < 7; ++c) plan->small_begin[c] = 0;
       for (size_t i = 0; i < order.size(); ++i) plan->small_begin[cls[i] + 1]++;
       for (int c = 0; c < 6; ++c) plan->small_begin[c + 1] += plan->small_begin[c];
-      if (std::getenv("SU2_PLAN_DEBUG")) {
-        int64_t steps[6] = {0}, maxsteps[6] = {0}; double dm[6] = {0};
-        for (size_t i = 0; i < order.size(); ++i) {
-          int64_t st = 0;
-          for (int32_t u = plan->h_work[i].unit0; u < plan->h_work[i].unit1; ++u) {
-            const HostTask& ht = plan->tasks[plan->h_units[u].task];
-            const int np = plan->h_units[u].pos1 - plan->h_units[u].pos0;
-            st += np;
-            dm[cls[i]] += np * (double)(((ht.m + 7) / 8) * ((ht.n + 7) / 8) * ((ht.k + 3) / 4) + ((ht.m + 7) / 8) * ((ht.p + 7) / 8) * ((ht.n + 7) / 8) * 2);
-          }
-          steps[cls[i]] += st; maxsteps[cls[i]] = std::max(maxsteps[cls[i]], st);
-        }
-        for (int c = 0; c < 6; ++c)
-          fprintf(stderr, "class %d: items %d steps %lld maxsteps/item %lld dmma %.0f\n", 8 * (c + 1), plan->small_begin[c + 1] - plan->small_begin[c], (long long)steps[c], (long long)maxsteps[c], dm[c]);
-      }
     }
     std::stable_sort(order.begin(), order.end(), [&](int64_t a, int64_t b) {
       if (cls[a] != cls[b]) return cls[a] < cls[b];
@@ -625,6 +610,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
   plan->info.workspace_bytes = plan->partial_elems * 8 + 256;
   plan->info.npsi_sec = nsec;
   plan->info.nwork_items = (int64_t)plan->h_work.size();
+  plan->info.small_plan = small_plan ? 1 : 0;
 
   if (!plan->host_only) {
     st = upload_plan(plan, alpha_host, ident_host, alpha_off_of_task, identA, identD, foldA, foldD, transD, cuda_stream);

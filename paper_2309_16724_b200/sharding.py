@@ -1,0 +1,97 @@
+"""Position-sharded H_eff*Psi over several GPUs.
+
+The sector tasks are independent and only meet in the accumulation into F ("several million of
+independent operations"); the operator families are > 99 % of the bytes, Psi is small.  So the POSITIONS of
+every operator-table row are cut into `world` contiguous slices: rank r keeps slice r of every position-indexed
+family (and of the row's alpha), applies its share into a private F with the unchanged single-GPU kernels, and
+one all-reduce (sum, FP64) of F per apply completes the product -- the one real exchange step of the path.  Psi is
+replicated; the Psi layout depends on the sector tables only, so it is identical on all ranks.
+
+`shard_problem` is plain data slicing (no arithmetic of the method).  `ShardedHeffOperator.apply` = the local
+`su2_heff_apply` followed by `torch.distributed.all_reduce` (NCCL over NVLink/NVSwitch; gloo in the CPU tests of
+the slicing).  The paper does this accumulation with host threads and lists device-to-device pooling as future
+work.
+"""
+import copy
+
+import numpy as np
+
+
+def position_slice(npos, rank, world):
+    """Contiguous, balanced slice [lo, hi) of `npos` positions owned by `rank`."""
+    return (npos * rank) // world, (npos * (rank + 1)) // world
+
+
+def shard_problem(problem, rank, world):
+    """The part of `problem` rank `rank` of `world` applies.  Summed over ranks the shards give the full operator.
+
+    * a row with P > 1 positions keeps positions position_slice(P, rank, world) (dropped if that is empty); every
+      family it indexes by position is sliced the same way -- a family's slice depends only on its npos, so rows
+      that share a family (a row and its Hermitian conjugate) stay consistent;
+    * a row with a single position (local terms, identity factors) is kept by rank `row index % world` only;
+    * families with one position, sector tables and site operators are replicated.
+    Family `data` blocks are sliced as views ([lo:hi] of the leading axis); blocks of a family without host data
+    (device-generated workloads) are left to the caller's fill function, only `npos` changes."""
+    assert 0 <= rank < world
+    if world == 1:
+        return problem
+    shard = copy.copy(problem)
+
+    def slice_fams(fams):
+        out = []
+        for f in fams:
+            lo, hi = position_slice(f.npos, rank, world)
+            if f.npos <= 1 or hi <= lo:
+                out.append(f)              # replicated (rows that would need an empty slice are dropped below)
+                continue
+            g = copy.copy(f)
+            g.npos = hi - lo
+            g.data = [np.ascontiguousarray(b[lo:hi]) for b in f.data] if f.data is not None else None
+            out.append(g)
+        return out
+
+    shard.fam_l = slice_fams(problem.fam_l)
+    shard.fam_r = slice_fams(problem.fam_r)
+    terms = []
+    for i, t in enumerate(problem.term):
+        npos = problem.npos_of(t)
+        if npos == 1:
+            if i % world == rank:
+                terms.append(t)
+            continue
+        lo, hi = position_slice(npos, rank, world)
+        if hi <= lo:
+            continue
+        u = copy.copy(t)
+        if t.alpha is not None:
+            u.alpha = np.ascontiguousarray(np.asarray(t.alpha)[lo:hi])
+        terms.append(u)
+    shard.term = terms
+    shard.meta = dict(problem.meta, shard=(rank, world))
+    return shard
+
+
+class ShardedHeffOperator:
+    """H_eff of one superblock problem spread over the ranks of a torch.distributed process group, one GPU per
+    rank.  apply(psi) returns the full H_eff psi on every rank."""
+
+    def __init__(self, problem, device, group=None, device_fill=None, force_split=False):
+        import torch.distributed as dist
+        from .runtime import HeffOperator
+        self.group = group
+        live = dist.is_available() and dist.is_initialized()
+        self.rank, self.world = (dist.get_rank(group), dist.get_world_size(group)) if live else (0, 1)
+        self.local = HeffOperator(shard_problem(problem, self.rank, self.world), device=device,
+                                  device_fill=device_fill, force_split=force_split)
+        self.psi_len = self.local.psi_len
+
+    @property
+    def info(self):
+        return self.local.info
+
+    def apply(self, psi, out=None):
+        import torch.distributed as dist
+        out = self.local.apply(psi, out)
+        if self.world > 1:
+            dist.all_reduce(out, op=dist.ReduceOp.SUM, group=self.group)   # on the current stream, after the kernels
+        return out

@@ -58,6 +58,48 @@ def test_synthetic_parity_full_oracle(name, force_split):
     assert _rel(f_gpu, f_ref) <= TOL
 
 
+@pytest.mark.parametrize("name", ["cfg1", "mini", "midi"])
+def test_small_bonds_through_the_large_tile_kernel(name, monkeypatch):
+    """Bonds whose sectors all hold <= 48 multiplets plan onto heff_small_kernel; SU2_HEFF_SMALL=0 keeps them on
+    heff_dmma_kernel, so the large-tile kernel stays covered on blocks of 1..17 rows (far smaller than a tile),
+    and the two kernels are checked against each other as well as against the oracle."""
+    torch = _torch()
+    prob = _cfg1() if name == "cfg1" else config_problem(name)
+    op_small = _operator(prob, force_split=True)
+    assert op_small.info["small_plan"] == 1
+    monkeypatch.setenv("SU2_HEFF_SMALL", "0")
+    op_big = _operator(prob, force_split=True)
+    monkeypatch.delenv("SU2_HEFF_SMALL")
+    assert op_big.info["small_plan"] == 0
+    x = random_psi(op_small.psi_len, seed=5)
+    f_ref = oracle_flat(prob, op_small.plan, x)
+    f_small = op_small.apply(torch.from_numpy(x).cuda()).cpu().numpy()
+    f_big = op_big.apply(torch.from_numpy(x).cuda()).cpu().numpy()
+    assert _rel(f_small, f_ref) <= TOL and _rel(f_big, f_ref) <= TOL
+    assert _rel(f_small, f_big) <= 1e-12
+
+
+@pytest.mark.parametrize("name,world", [("mini", 2), ("midi", 3)])
+def test_position_shards_add_up_on_the_gpu(name, world):
+    """Position-sharded apply (sharding.py): each rank's shard applied by the CUDA path, one after the
+    other on this GPU, summed in rank order (what the all-reduce does) = the oracle's full H_eff Psi."""
+    torch = _torch()
+    from paper_2309_16724_b200.sharding import ShardedHeffOperator, shard_problem
+    prob = config_problem(name)
+    full = _operator(prob)
+    x = random_psi(full.psi_len, seed=6)
+    f_ref = oracle_flat(prob, full.plan, x)
+    xd = torch.from_numpy(x).cuda()
+    total = torch.zeros_like(xd)
+    for rank in range(world):
+        op = _operator(shard_problem(prob, rank, world))
+        assert op.plan.labels == full.plan.labels
+        total += op.apply(xd)
+    assert _rel(total.cpu().numpy(), f_ref) <= TOL
+    single = ShardedHeffOperator(prob, "cuda:0")          # no process group: one rank, no exchange step
+    assert single.world == 1 and _rel(single.apply(xd).cpu().numpy(), f_ref) <= TOL
+
+
 def test_several_tiles_and_ragged_tail():
     """Blocks larger than one tile with ragged tails (L=16, D=500: dims 6..109)."""
     torch = _torch()
@@ -160,6 +202,7 @@ def test_gpu_result_is_hermitian_and_linear_midi():
                                            (16, 16, 16, 16, 20000), (32, 32, 32, 32, 3000), (7, 5, 9, 3, 501),
                                            (24, 46, 30, 40, 50), (33, 17, 25, 47, 20), (6, 46, 12, 31, 777),
                                            (48, 48, 48, 48, 40), (8, 8, 8, 8, 300000), (2, 64, 2, 5, 33),
+                                           (80, 80, 80, 80, 300), (64, 72, 79, 55, 11), (81, 80, 80, 80, 3),
                                            # too big for the small-block kernel, too narrow for the DMMA tiles
                                            (8, 512, 512, 8, 3)])
 def test_gemm_pair_batched(m, k, n, p, batch):
