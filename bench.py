@@ -325,7 +325,8 @@ def run_cfg5(args):
                       "roofline_small_blocks": {"bound": "hbm", "kernel": "gemm_pair_small_kernel",
                                                 "shape": best_hbm["m=k=n=p"], "achieved": best_hbm["operand_gbs"],
                                                 "peak": peaks["hbm_gbs"], "peak_source": peak_src, "unit": "GB/s",
-                                                "frac": best_hbm["hbm_frac"], "traffic": None}}))
+                                                "frac": best_hbm["hbm_frac"],
+                                                "traffic": ncu_traffic("cfg5_b%d" % best_hbm["m=k=n=p"])}}))
 
 
 def run_gpu(args):
