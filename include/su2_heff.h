@@ -181,7 +181,13 @@ su2_status su2_davidson_destroy(su2_davidson* dav);
 
 /* Strided-batched FP64 GEMM-pair microbenchmark entry (BASELINE.json configs[4]):
  * C_b (m x p) += alpha * A_b (m x k) * X_b (k x n) * B_b^T (n x p) for b < batch, all DEVICE,
- * row-major, dense strides (A_b = A + b*m*k, ...).  Uses the same fused kernel as the apply. */
+ * row-major, dense strides (A_b = A + b*m*k, ...); the paper's strided-batched GEMM sequences
+ * with T = A_b X_b kept on chip.  Items whose operands fit one SM's shared memory run one CTA per item on FP64
+ * tensor instructions (HBM-bound regime); larger items with >= 64 x 64 outputs use the fused kernel of the apply;
+ * anything else an FP64-FMA tile routine.  C_b blocks must not overlap; one CTA owns an output
+ * element, so results are bit-reproducible.  Errors: non-positive dimension, negative batch or null pointer ->
+ * SU2_ERR_INVALID_ARGUMENT; batch == 0 is a no-op.  SU2_GEMM_PAIR_SMALL="wpi,nbuf" ("0": off) in the environment
+ * overrides the small-item kernel's warps per item and input buffering (tuning aid). */
 su2_status su2_gemm_pair_batched(int32_t m, int32_t k, int32_t n, int32_t p, int64_t batch, double alpha,
                                  const double* A, const double* X, const double* B, double* C,
                                  void* cuda_stream);

@@ -54,6 +54,35 @@ def _sector_choice(prob, op, count):
     return sorted(pick)
 
 
+def test_cfg2_small_block_parity_and_properties():
+    """BASELINE.json configs[1]: L=20, D=256, blocks 6-46: the small-block kernel (heff_small_kernel, size classes
+    24/40/48) in the launch configuration bench.py times: sampled entries of 24 of the 138 sectors against the
+    oracle, every sector against the large-tile kernel on the same plan input, and the any-size properties."""
+    import os
+    from oracle.heff_sampled import numpy_block_rows
+    torch, prob, op = _setup("cfg2")
+    assert op.psi_len == 85126 and op.info["small_plan"] == 1
+    worst, f = _sampled_parity(torch, prob, op, _sector_choice(prob, op, 24), 5, numpy_block_rows(prob), seed=31)
+    assert worst <= TOL, worst
+    x = torch.from_numpy(random_psi(op.psi_len, seed=31)).cuda()
+    y = torch.from_numpy(random_psi(op.psi_len, seed=32)).cuda()
+    hx = op.apply(x).clone()
+    assert torch.equal(hx.cpu(), torch.from_numpy(f))                      # bitwise reproducible
+    os.environ["SU2_HEFF_SMALL"] = "0"
+    try:
+        _, _, op_big = _setup("cfg2")
+    finally:
+        del os.environ["SU2_HEFF_SMALL"]
+    assert op_big.info["small_plan"] == 0
+    hx_big = op_big.apply(x)
+    assert float((hx - hx_big).abs().max()) <= 1e-12 * float(hx.abs().max())   # all 85 126 elements, two kernels
+    hy = op.apply(y).clone()
+    a, b = float(torch.dot(y, hx)), float(torch.dot(x, hy))
+    assert abs(a - b) <= 1e-11 * float(hx.norm()) * float(y.norm())          # Hermiticity
+    hz = op.apply(2.0 * x - 0.5 * y)
+    assert float((hz - (2.0 * hx - 0.5 * hy)).abs().max()) <= 1e-12 * float(hx.abs().max())
+
+
 def test_cfg3_sampled_parity_and_properties():
     """BASELINE.json configs[2]: L=40, D=1024, blocks 30-131 (all operators built by the numpy generator)."""
     from oracle.heff_sampled import numpy_block_rows
