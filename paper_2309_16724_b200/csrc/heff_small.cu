@@ -138,15 +138,21 @@ heff_small_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __
 
   // dense rows x cols block -> shared rows of stride LD, one warp per row; pads untouched
   auto copy_rows = [&](double* dst, const double* __restrict__ src, int rows, int cols) {
+    uint32_t d = (uint32_t)__cvta_generic_to_shared(dst) + (uint32_t)(warp * LD) * 8u;
+    const double* s = src + (int64_t)warp * cols;
+    const int64_t s_step = (int64_t)WARPS * cols;
     if (!(cols & 1) && !((uintptr_t)src & 15)) {
-      const bool on = 2 * lane < cols;
-      for (int r = warp; r < rows; r += WARPS)
-        if (on) hs_cp16(dst + r * LD + 2 * lane, src + (int64_t)r * cols + 2 * lane, true);
+      if (2 * lane < cols) {
+        d += 16u * lane; s += 2 * lane;
+        for (int r = warp; r < rows; r += WARPS, d += WARPS * LD * 8, s += s_step)
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(s) : "memory");
+      }
     } else {
-      const bool on0 = lane < cols, on1 = lane + 32 < cols;
-      for (int r = warp; r < rows; r += WARPS) {
-        if (on0) hs_cp8(dst + r * LD + lane, src + (int64_t)r * cols + lane, true);
-        if (DM8 > 32 && on1) hs_cp8(dst + r * LD + lane + 32, src + (int64_t)r * cols + lane + 32, true);
+      d += 8u * lane; s += lane;
+      const bool on0 = lane < cols, on1 = DM8 > 32 && lane + 32 < cols;
+      for (int r = warp; r < rows; r += WARPS, d += WARPS * LD * 8, s += s_step) {
+        if (on0) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(s) : "memory");
+        if (on1) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d + 256u), "l"(s + 32) : "memory");
       }
     }
   };
