@@ -172,6 +172,15 @@ su2_status su2_heff_diag(const su2_plan* plan, double* diag_dev, void* cuda_stre
 int64_t su2_davidson_workspace_bytes(const su2_plan* plan, int32_t max_subspace);
 su2_status su2_davidson_create(su2_davidson** out, const su2_plan* plan, int32_t max_subspace,
                                const double* x0_dev, void* dav_workspace_dev, void* cuda_stream);
+/* The same for a POSITION-SHARDED plan (one rank's share of the operator positions; all ranks hold the same Psi
+ * layout and run the same Davidson algebra): `reduce` must sum vec_dev[0..n) (DEVICE) over the ranks, in place,
+ * ordered on cuda_stream, and leave identical bits on every rank (an NCCL all-reduce does); it is called once for
+ * the diagonal at create time and once per step on w = H_eff v, right after the local su2_heff_apply.  A non-zero
+ * return aborts the call with that status.  reduce == NULL is su2_davidson_create. */
+typedef int32_t (*su2_reduce_fn)(double* vec_dev, int64_t n, void* cuda_stream, void* user);   /* returns a su2_status */
+su2_status su2_davidson_create_sharded(su2_davidson** out, const su2_plan* plan, int32_t max_subspace,
+                                       const double* x0_dev, void* dav_workspace_dev, void* cuda_stream,
+                                       su2_reduce_fn reduce, void* reduce_user);
 /* One iteration: w = H_eff v (su2_heff_apply), Rayleigh-Ritz, residual, new direction.
  * theta: current Ritz value; resnorm: |H x - theta x|.  Synchronises for the two scalars. */
 su2_status su2_davidson_step(const su2_plan* plan, su2_davidson* dav, void* workspace_dev,

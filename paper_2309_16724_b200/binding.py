@@ -53,8 +53,10 @@ class su2_plan_info_t(C.Structure):
 
 EXPORTS = ["su2_status_string", "su2_last_cuda_error", "su2_kernel_launch_count", "su2_plan_create", "su2_plan_destroy", "su2_plan_info",
            "su2_plan_psi_layout", "su2_plan_export_tasks", "su2_heff_apply", "su2_heff_apply_host", "su2_heff_diag",
-           "su2_davidson_workspace_bytes", "su2_davidson_create", "su2_davidson_step", "su2_davidson_ritz_vector",
+           "su2_davidson_workspace_bytes", "su2_davidson_create", "su2_davidson_create_sharded", "su2_davidson_step", "su2_davidson_ritz_vector",
            "su2_davidson_destroy", "su2_gemm_pair_batched", "su2_probe_fp64_peak"]
+
+REDUCE_FN = C.CFUNCTYPE(C.c_int32, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p)   # su2_reduce_fn
 
 SU2_PLAN_HOST_ONLY = 1
 _lib = None
@@ -87,6 +89,8 @@ def load():
     lib.su2_davidson_workspace_bytes.restype = C.c_int64
     lib.su2_davidson_workspace_bytes.argtypes = [C.c_void_p, C.c_int32]
     lib.su2_davidson_create.argtypes = [C.POINTER(C.c_void_p), C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.su2_davidson_create_sharded.argtypes = [C.POINTER(C.c_void_p), C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p,
+                                                C.c_void_p, REDUCE_FN, C.c_void_p]
     lib.su2_davidson_step.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                       C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.su2_davidson_ritz_vector.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
@@ -225,10 +229,16 @@ class Plan:
 
 
 class Davidson:
-    def __init__(self, plan, max_subspace, x0_ptr, ws_ptr, stream=0):
+    def __init__(self, plan, max_subspace, x0_ptr, ws_ptr, stream=0, reduce=None):
+        """reduce(vec_ptr, n, stream) -> status: sum over ranks of a device vector (position-sharded plans)."""
         self.plan = plan
         self.handle = C.c_void_p()
-        check(load().su2_davidson_create(C.byref(self.handle), plan.handle, max_subspace, x0_ptr, ws_ptr, stream))
+        if reduce is None:
+            check(load().su2_davidson_create(C.byref(self.handle), plan.handle, max_subspace, x0_ptr, ws_ptr, stream))
+        else:
+            self._reduce = REDUCE_FN(lambda vec, n, st, user: int(reduce(vec, n, st) or 0))   # keep the thunk alive
+            check(load().su2_davidson_create_sharded(C.byref(self.handle), plan.handle, max_subspace, x0_ptr, ws_ptr,
+                                                     stream, self._reduce, None))
 
     @staticmethod
     def workspace_bytes(plan, max_subspace):

@@ -148,6 +148,8 @@ struct su2_davidson {
   std::vector<double> y;        // last Ritz vector in the subspace
   double diag_floor = 0.0;
   int32_t grid = 296;
+  su2_reduce_fn reduce = nullptr;   // position-sharded plans: sums a vector over the ranks (null: single GPU)
+  void* reduce_user = nullptr;
 };
 
 static su2_status dots(su2_davidson* d, const double* xs, int nx, const double* y, double* host_out, cudaStream_t st) {
@@ -187,12 +189,20 @@ extern "C" int64_t su2_davidson_workspace_bytes(const su2_plan* plan, int32_t ma
 
 extern "C" su2_status su2_davidson_create(su2_davidson** out, const su2_plan* plan, int32_t max_subspace, const double* x0_dev,
                                           void* ws, void* cuda_stream) {
+  return su2_davidson_create_sharded(out, plan, max_subspace, x0_dev, ws, cuda_stream, nullptr, nullptr);
+}
+
+extern "C" su2_status su2_davidson_create_sharded(su2_davidson** out, const su2_plan* plan, int32_t max_subspace,
+                                                  const double* x0_dev, void* ws, void* cuda_stream, su2_reduce_fn reduce,
+                                                  void* reduce_user) {
   if (!out || !plan || !x0_dev || !ws || max_subspace < 2 || max_subspace > MAX_SUB) return SU2_ERR_INVALID_ARGUMENT;
   if (plan->host_only) return SU2_ERR_NO_DEVICE_PLAN;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   su2_davidson* d = new su2_davidson();
   d->n = plan->psi_len;
   d->mmax = max_subspace;
+  d->reduce = reduce;
+  d->reduce_user = reduce_user;
   const int64_t n = plan->psi_len;
   double* base = (double*)ws;
   d->V = base;
@@ -209,6 +219,7 @@ extern "C" su2_status su2_davidson_create(su2_davidson** out, const su2_plan* pl
     return SU2_ERR_CUDA;
   }
   su2_status s = su2_heff_diag(plan, d->diag, cuda_stream);
+  if (s == SU2_OK && d->reduce) s = d->reduce(d->diag, d->n, cuda_stream, d->reduce_user);   // diag of a sum of shards
   if (s != SU2_OK) { su2_davidson_destroy(d); return s; }
   maxabs_stage1<<<RED_BLOCKS, RED_THREADS, 0, st>>>(d->diag, d->n, d->scratch); su2::count_launch();
   std::vector<double> part(RED_BLOCKS);
@@ -238,6 +249,12 @@ extern "C" su2_status su2_davidson_step(const su2_plan* plan, su2_davidson* d, v
   // 1. w = H_eff v for the newest basis vector
   su2_status s = su2_heff_apply(plan, d->V + (int64_t)(k - 1) * n, d->W + (int64_t)(k - 1) * n, workspace_dev, cuda_stream);
   if (s != SU2_OK) return s;
+  // 1b. position-sharded plan: this rank applied its share of the positions; sum F over the ranks (the path's one
+  //     exchange step).  Every rank receives the same bits, so the replicated algebra below stays in step.
+  if (d->reduce) {
+    s = d->reduce(d->W + (int64_t)(k - 1) * n, n, cuda_stream, d->reduce_user);
+    if (s != SU2_OK) return s;
+  }
   // 2. new column of the projected matrix G = V^T H V
   std::vector<double> col(k);
   s = dots(d, d->V, k, d->W + (int64_t)(k - 1) * n, col.data(), st);

@@ -95,3 +95,45 @@ class ShardedHeffOperator:
         if self.world > 1:
             dist.all_reduce(out, op=dist.ReduceOp.SUM, group=self.group)   # on the current stream, after the kernels
         return out
+
+    def davidson(self, x0, max_subspace=20):
+        """Davidson solver on the sharded operator: su2_davidson_create_sharded with an all-reduce hook (called on
+        the diagonal once and on w = H_eff v every step); everything else is replicated on the ranks."""
+        return ShardedDavidsonSolver(self, x0, max_subspace)
+
+
+class ShardedDavidsonSolver:
+    def __init__(self, op, x0, max_subspace=20):
+        import torch
+        import torch.distributed as dist
+        from .binding import Davidson
+        self.op, local = op, op.local
+        self.ws = torch.empty(Davidson.workspace_bytes(local.plan, max_subspace), dtype=torch.uint8, device=local.device)
+        self.stream = torch.cuda.current_stream(local.device).cuda_stream
+        self.reduce_calls = 0
+
+        def reduce(vec_ptr, n, stream):
+            # the vector lives inside self.ws (the Davidson workspace): view it as a tensor, no copy
+            off = vec_ptr - self.ws.data_ptr()
+            assert 0 <= off and off + 8 * n <= self.ws.numel() and (stream or 0) == self.stream
+            view = self.ws[off:off + 8 * n].view(torch.float64)
+            if op.world > 1:
+                dist.all_reduce(view, op=dist.ReduceOp.SUM, group=op.group)
+            self.reduce_calls += 1
+            return 0
+
+        self.dav = Davidson(local.plan, max_subspace, x0.data_ptr(), self.ws.data_ptr(), self.stream, reduce=reduce)
+        self.history = []
+
+    def step(self):
+        theta, res = self.dav.step(self.op.local.workspace.data_ptr(), self.stream)
+        self.history.append((theta, res))
+        return theta, res
+
+    def ritz_vector(self):
+        x = self.op.local.new_vector()
+        self.dav.ritz_vector(x.data_ptr(), self.stream)
+        return x
+
+    def close(self):
+        self.dav.close()

@@ -100,6 +100,81 @@ def test_position_shards_add_up_on_the_gpu(name, world):
     assert single.world == 1 and _rel(single.apply(xd).cpu().numpy(), f_ref) <= TOL
 
 
+def test_sharded_davidson_reduce_hook():
+    """su2_davidson_create_sharded: the reduce hook is called once for the diagonal and once per step, on vectors
+    inside the Davidson workspace; with one rank (nothing to add) the iteration is bit-identical to the plain
+    solver.  A hook that returns an error aborts the step with that status."""
+    torch = _torch()
+    from paper_2309_16724_b200 import Su2Error
+    from paper_2309_16724_b200.binding import Davidson
+    from paper_2309_16724_b200.sharding import ShardedHeffOperator
+    prob = config_problem("midi")
+    op = ShardedHeffOperator(prob, "cuda:0")
+    x0 = torch.from_numpy(random_psi(op.psi_len, seed=8)).cuda()
+    plain = op.local.davidson(x0, max_subspace=6)
+    sharded = op.davidson(x0, max_subspace=6)
+    assert sharded.reduce_calls == 1
+    h0 = [plain.step() for _ in range(8)]
+    h1 = [sharded.step() for _ in range(8)]
+    assert h0 == h1 and sharded.reduce_calls == 9
+    assert torch.equal(plain.ritz_vector(), sharded.ritz_vector())
+    plain.close(); sharded.close()
+    ws = torch.empty(Davidson.workspace_bytes(op.local.plan, 4), dtype=torch.uint8, device="cuda")
+    calls = []
+    bad = Davidson(op.local.plan, 4, x0.data_ptr(), ws.data_ptr(), torch.cuda.current_stream().cuda_stream,
+                   reduce=lambda vec, n, st: calls.append(n) or (-1 if len(calls) > 1 else 0))
+    with pytest.raises(Su2Error):
+        bad.step(op.local.workspace.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    assert calls == [op.psi_len, op.psi_len]
+    bad.close()
+
+
+def test_sharded_davidson_two_shards_on_one_gpu():
+    """Two position shards, both resident on this GPU.  The solver runs on shard 0; its reduce hook adds shard 1's
+    share (what the all-reduce delivers): the diagonal at create time, then H_1 v for the vector the step just
+    applied (w = W[i] and v = V[i] sit max_subspace * n doubles apart in the Davidson workspace).  Ritz values and
+    residuals follow the unsharded solver through a restart."""
+    torch = _torch()
+    from paper_2309_16724_b200.binding import Davidson
+    from paper_2309_16724_b200.sharding import shard_problem
+    prob = config_problem("midi")
+    full = _operator(prob)
+    op0, op1 = _operator(shard_problem(prob, 0, 2)), _operator(shard_problem(prob, 1, 2))
+    n, mm = full.psi_len, 5
+    x0 = torch.from_numpy(random_psi(n, seed=13)).cuda()
+    ws = torch.empty(Davidson.workspace_bytes(op0.plan, mm), dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream().cuda_stream
+    calls = []
+
+    def reduce(vec, nn, st):
+        off = vec - ws.data_ptr()
+        w = ws[off:off + 8 * nn].view(torch.float64)
+        if not calls:
+            w += op1.diag()
+        else:
+            v = ws[off - 8 * mm * nn:off - 8 * mm * nn + 8 * nn].view(torch.float64)
+            w += op1.apply(v.clone())
+        calls.append(nn)
+        return 0
+
+    dav = Davidson(op0.plan, mm, x0.data_ptr(), ws.data_ptr(), stream, reduce=reduce)
+    ref = full.davidson(x0, max_subspace=mm)
+    for it in range(9):
+        th, rn = dav.step(op0.workspace.data_ptr(), stream)
+        th_ref, rn_ref = ref.step()
+        if it < 3:   # same trajectory while the different summation order of F (shard sums) has not been amplified
+            assert abs(th - th_ref) <= 1e-9 * max(1.0, abs(th_ref)) and abs(rn - rn_ref) <= 1e-7 * max(1.0, rn_ref)
+    # whatever the trajectory: the reported Ritz pair is one of the FULL operator
+    x = full.new_vector()
+    dav.ritz_vector(x.data_ptr(), stream)
+    hx = full.apply(x)
+    assert abs(float(torch.dot(x, x)) - 1.0) <= 1e-10
+    assert abs(float(torch.dot(x, hx)) - th) <= 1e-10 * max(1.0, abs(th))
+    assert abs(float((hx - th * x).norm()) - rn) <= 1e-8 * max(1.0, rn)
+    assert calls == [n] * 10
+    dav.close(); ref.close()
+
+
 def test_several_tiles_and_ragged_tail():
     """Blocks larger than one tile with ragged tails (L=16, D=500: dims 6..109)."""
     torch = _torch()
