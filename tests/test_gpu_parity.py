@@ -294,6 +294,25 @@ def test_gemm_pair_batched(m, k, n, p, batch):
     assert _rel(dC.cpu().numpy(), ref) <= 1e-12
 
 
+def test_gemm_pair_batched_degenerate_calls():
+    """batch == 0 is a no-op that leaves C untouched; non-positive dimensions and null pointers are rejected with
+    SU2_ERR_INVALID_ARGUMENT before anything is launched."""
+    torch = _torch()
+    from paper_2309_16724_b200 import Su2Error, gemm_pair_batched
+    from paper_2309_16724_b200.binding import kernel_launch_count
+    buf = torch.full((64,), 3.0, dtype=torch.float64, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    l0 = kernel_launch_count()
+    gemm_pair_batched(8, 8, 8, 8, 0, 0.5, buf.data_ptr(), buf.data_ptr(), buf.data_ptr(), buf.data_ptr(), st)
+    for bad in ((0, 8, 8, 8, 1), (8, -1, 8, 8, 1), (8, 8, 8, 8, -2)):
+        with pytest.raises(Su2Error):
+            gemm_pair_batched(*bad, 0.5, buf.data_ptr(), buf.data_ptr(), buf.data_ptr(), buf.data_ptr(), st)
+    with pytest.raises(Su2Error):
+        gemm_pair_batched(8, 8, 8, 8, 1, 0.5, buf.data_ptr(), None, buf.data_ptr(), buf.data_ptr(), st)
+    torch.cuda.synchronize()
+    assert kernel_launch_count() == l0 and bool((buf == 3.0).all())
+
+
 @pytest.mark.gpu
 def test_gemm_pair_batched_unaligned_and_repeatable():
     """Operands that start 8 bytes off a 16-byte boundary take the 8-byte copy path of the small-block kernel;
