@@ -87,6 +87,17 @@ lincomb(double* __restrict__ out, const double* __restrict__ a, const double* __
 __global__ void __launch_bounds__(256) axpy(double* __restrict__ y, const double* __restrict__ x, double a, int64_t n) {
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) y[i] += a * x[i];
 }
+// the same two with the scalar left on the device by dot_stage2 (no host round trip inside Gram-Schmidt):
+// y -= c[0] x, and y = x / sqrt(c[0]) (0 if c[0] == 0); same operations, same bits as the host-scalar versions
+__global__ void __launch_bounds__(256) axpy_neg_dev(double* __restrict__ y, const double* __restrict__ x, const double* __restrict__ c, int64_t n) {
+  const double a = -c[0];
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) y[i] += a * x[i];
+}
+__global__ void __launch_bounds__(256) scale_copy_rnorm_dev(double* __restrict__ y, const double* __restrict__ x, const double* __restrict__ c, int64_t n) {
+  const double nrm = sqrt(c[0]);
+  const double a = nrm > 0 ? 1.0 / nrm : 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) y[i] = a * x[i];
+}
 __global__ void __launch_bounds__(256) scale_copy(double* __restrict__ y, const double* __restrict__ x, double a, int64_t n) {
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) y[i] = a * x[i];
 }
@@ -165,17 +176,20 @@ static su2_status dots(su2_davidson* d, const double* xs, int nx, const double* 
 
 // orthogonalise d->t against V[0..k) (modified Gram-Schmidt, twice), normalise into V[k]
 static su2_status orthonormalise_into_basis(su2_davidson* d, cudaStream_t st) {
-  double c = 0.0;
+  // every scalar (projection, norm) stays on the device: the loop is stream-ordered, no synchronisation
+  double* res = d->scratch + (int64_t)MAX_SUB * RED_BLOCKS;
+  auto dot_dev = [&](const double* x, const double* y) {
+    dim3 g1(RED_BLOCKS, 1);
+    dot_stage1<<<g1, RED_THREADS, 0, st>>>(x, d->n, y, d->n, d->scratch); su2::count_launch();
+    dot_stage2<<<1, RED_THREADS, 0, st>>>(d->scratch, res); su2::count_launch();
+  };
   for (int pass = 0; pass < 2; ++pass)
     for (int i = 0; i < d->k; ++i) {
-      su2_status s = dots(d, d->V + (int64_t)i * d->n, 1, d->t, &c, st);
-      if (s != SU2_OK) return s;
-      axpy<<<d->grid, 256, 0, st>>>(d->t, d->V + (int64_t)i * d->n, -c, d->n); su2::count_launch();
+      dot_dev(d->V + (int64_t)i * d->n, d->t);
+      axpy_neg_dev<<<d->grid, 256, 0, st>>>(d->t, d->V + (int64_t)i * d->n, res, d->n); su2::count_launch();
     }
-  su2_status s = dots(d, d->t, 1, d->t, &c, st);
-  if (s != SU2_OK) return s;
-  const double nrm = std::sqrt(c);
-  scale_copy<<<d->grid, 256, 0, st>>>(d->V + (int64_t)d->k * d->n, d->t, nrm > 0 ? 1.0 / nrm : 0.0, d->n); su2::count_launch();
+  dot_dev(d->t, d->t);
+  scale_copy_rnorm_dev<<<d->grid, 256, 0, st>>>(d->V + (int64_t)d->k * d->n, d->t, res, d->n); su2::count_launch();
   SU2_CUDA(cudaGetLastError());
   d->k += 1;
   return SU2_OK;
