@@ -35,7 +35,7 @@
 #include "tile_config.h"
 // L2 eviction hints of the producers' 16-byte tile copies (0 none, 1 evict_last, 2 evict_first).  Measured at cfg4:
 // D tiles evict_first (a D_pos tile is streamed once per sibling CTA and never again) +0.5 %; E tiles evict_last
-// -0.4 %; both: no change.
+// -0.4 %; both: no change; A tiles evict_first as well: -0.4 % (two more producer registers spill).
 #ifndef SU2_HINT_E
 #define SU2_HINT_E 0
 #define SU2_HINT_D 2
