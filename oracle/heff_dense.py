@@ -206,32 +206,23 @@ def apply_full(problem, psi_full, terms=None):
 
 
 def _sum_over_positions(fl, lb, ltr, fr, rb, rtr, alpha, e):
-    """sum_pos alpha_pos * A_pos E D_pos^T  (the paper's sum over the position index,
-    PAPER.md:58-60); A, D = the applied l / r operator blocks (transposed if adjoint); a
-    family with a single position (or the identity) is the same for every pos.
+    """sum_pos alpha_pos * A_pos E D_pos^T, written out as the paper's innermost loop over the
+    position index ("three nested loops", the third over the positions); A, D = the
+    applied l / r operator blocks (transposed if adjoint).  A family with a single position (or the
+    identity: family None) contributes the same block at every pos.  Nothing is folded, factored
+    or reordered here: one term alpha_pos * (A_pos @ E) @ D_pos^T per position, added in index order.
     E may carry leading batch axes (..., k, n)."""
-    npos = len(alpha)
-    a = None if fl is None else (np.swapaxes(fl.data[lb], 1, 2) if ltr else fl.data[lb])
-    d = None if fr is None else (np.swapaxes(fr.data[rb], 1, 2) if rtr else fr.data[rb])
-    a_varies = a is not None and a.shape[0] == npos and npos > 1
-    d_varies = d is not None and d.shape[0] == npos and npos > 1
-    if a_varies and d_varies:
-        t = np.einsum("p,pmk,...kn->p...mn", alpha, a, e, optimize=True)      # T_pos = alpha_pos A_pos E
-        return np.einsum("p...mn,pqn->...mq", t, d, optimize=True)            # sum_pos T_pos D_pos^T
-    scale = 1.0
-    if a_varies:
-        a0 = np.tensordot(alpha, a, axes=(0, 0))
-    else:
-        a0 = None if a is None else a[0]
-    if d_varies:
-        d0 = np.tensordot(alpha, d, axes=(0, 0))
-    else:
-        d0 = None if d is None else d[0]
-    if not a_varies and not d_varies:
-        scale = alpha.sum()
-    out = e if a0 is None else np.matmul(a0, e)
-    out = out if d0 is None else np.matmul(out, d0.T)
-    return scale * out
+    acc = 0.0
+    for pos in range(len(alpha)):
+        x = e
+        if fl is not None:
+            a = fl.data[lb][pos if fl.data[lb].shape[0] > 1 else 0]
+            x = np.matmul(a.T if ltr else a, x)
+        if fr is not None:
+            d = fr.data[rb][pos if fr.data[rb].shape[0] > 1 else 0]
+            x = np.matmul(x, d if rtr else d.T)
+        acc = acc + alpha[pos] * x
+    return acc
 
 
 def heff_apply(problem, psi_red, check_leak=True, terms=None):

@@ -13,8 +13,9 @@ Every operator-table row, every input sector and every position contributes; not
 along the contraction.  Operator values are obtained through a callback so that blocks resident on a
 device (92 GB at configs[3]) need not be staged through host memory in full.
 
-Pin: tests/test_oracle_heff.py::test_sampled_equals_full_oracle (equality with heff_dense.heff_apply
-on workloads small enough for both).
+Pins: tests/test_oracle_heff.py::test_sampled_equals_full_oracle (equality with heff_dense.heff_apply
+on workloads small enough for both) and ::test_sampled_sum_equals_position_loop (the position sum against
+scalar loops, every varying / fixed / identity operand combination, non-trivial alpha).
 """
 import numpy as np
 
@@ -125,16 +126,21 @@ def heff_sample(problem, psi_red, label, rows_a, rows_b, block_rows, psi_full=No
 
 def _sampled_sum(a, d, alpha, e, rows_a, rows_b):
     """sum_pos alpha_pos A_pos[rows_a, :] E D_pos[rows_b, :]^T; a: [npos or 1, |rows_a|, k] or None
-    (identity), d: [npos or 1, |rows_b|, n] or None (identity)."""
+    (identity), d: [npos or 1, |rows_b|, n] or None (identity).
+
+    The same per-position terms as heff_dense._sum_over_positions, evaluated for all
+    positions by ONE stacked call per product (np.matmul over a leading position axis) and then added
+    with their alpha_pos: a family with a single position (or the identity) is repeated along that
+    axis, never folded into the sum.  Pinned against the explicit position loop, for every
+    combination of varying / fixed / identity operands and non-trivial alpha, by
+    tests/test_oracle_heff.py::test_sampled_sum_equals_position_loop."""
     npos = len(alpha)
-    a_varies = a is not None and a.shape[0] == npos and npos > 1
-    d_varies = d is not None and d.shape[0] == npos and npos > 1
-    if a_varies and d_varies:
-        t = np.einsum("p,pak,kn->pan", alpha, a, e, optimize=True)
-        return np.einsum("pan,pbn->ab", t, d, optimize=True)
-    a0 = None if a is None else (np.tensordot(alpha, a, axes=(0, 0)) if a_varies else a[0])
-    d0 = None if d is None else (np.tensordot(alpha, d, axes=(0, 0)) if d_varies else d[0])
-    scale = 1.0 if (a_varies or d_varies) else alpha.sum()
-    te = e[rows_a, :] if a0 is None else a0 @ e
-    out = te[:, rows_b] if d0 is None else te @ d0.T
-    return scale * out
+    if a is None:
+        te = np.broadcast_to(e[rows_a, :], (npos,) + e[rows_a, :].shape)           # (1 E)[rows_a, :]
+    else:
+        te = np.matmul(np.broadcast_to(a, (npos,) + a.shape[1:]), e)                # T_pos = A_pos[rows_a, :] E
+    if d is None:
+        ted = te[:, :, rows_b]                                                      # (T_pos 1^T)[:, rows_b]
+    else:
+        ted = np.matmul(te, np.swapaxes(np.broadcast_to(d, (npos,) + d.shape[1:]), 1, 2))   # T_pos D_pos[rows_b, :]^T
+    return np.tensordot(np.asarray(alpha, dtype=np.float64), ted, axes=(0, 0))      # sum_pos alpha_pos (...)

@@ -157,3 +157,56 @@ def test_sampled_equals_full_oracle():
             assert np.abs(got - want).max() <= 1e-13 * max(1.0, np.abs(flatten(prob, ref, labels)).max())
             checked += got.size
         assert checked > 20
+
+
+def _position_loop(a, d, alpha, e, rows_a, rows_b):
+    """sum_pos alpha_pos A_pos[rows_a, :] E D_pos[rows_b, :]^T with python loops over every index
+    (PAPER.md:58-60); a / d: [npos or 1, m, k] / [npos or 1, p, n] full applied blocks or None (identity)."""
+    out = np.zeros((len(rows_a), len(rows_b)))
+    k, n = e.shape
+    for pos in range(len(alpha)):
+        ap = np.eye(k) if a is None else a[pos if a.shape[0] > 1 else 0]
+        dp = np.eye(n) if d is None else d[pos if d.shape[0] > 1 else 0]
+        for ia, ra in enumerate(rows_a):
+            for ib, rb in enumerate(rows_b):
+                s = 0.0
+                for x in range(k):
+                    for y in range(n):
+                        s += ap[ra, x] * e[x, y] * dp[rb, y]
+                out[ia, ib] += alpha[pos] * s
+    return out
+
+
+def test_sampled_sum_equals_position_loop():
+    """Pins the position sum of BOTH oracles (heff_dense._sum_over_positions, heff_sampled._sampled_sum) against
+    scalar loops on random blocks with non-trivial alpha, for every combination of operands that varies with
+    the position, is fixed (one position), or is the identity -- including len(alpha) > 1 with neither varying."""
+    from types import SimpleNamespace
+    from oracle.heff_dense import _sum_over_positions
+    from oracle.heff_sampled import _sampled_sum
+    rng = np.random.default_rng(5)
+    m, k, n, p, npos = 4, 5, 3, 6, 7
+    e = rng.normal(size=(k, n))
+    alpha = rng.normal(size=npos) + 0.3
+    rows = {"m": np.array([0, 2, 3]), "p": np.array([1, 4])}
+    kinds = ("varies", "fixed", "identity")
+    for ka in kinds:
+        for kd in kinds:
+            for tr in (False, True):
+                mm = k if ka == "identity" else m
+                pp = n if kd == "identity" else p
+                a = None if ka == "identity" else rng.normal(size=(npos if ka == "varies" else 1, mm, k))
+                d = None if kd == "identity" else rng.normal(size=(npos if kd == "varies" else 1, pp, n))
+                ra = rows["m"][rows["m"] < mm]
+                rb = rows["p"][rows["p"] < pp]
+                want = _position_loop(a, d, alpha, e, ra, rb)
+                got_s = _sampled_sum(None if a is None else a[:, ra, :], None if d is None else d[:, rb, :], alpha, e, ra, rb)
+                assert np.abs(got_s - want).max() < 1e-13
+                # the dense oracle takes STORED blocks + adjoint flags: store the transposes when tr is set
+                fl = None if a is None else SimpleNamespace(data=[np.swapaxes(a, 1, 2).copy() if tr else a])
+                fr = None if d is None else SimpleNamespace(data=[np.swapaxes(d, 1, 2).copy() if tr else d])
+                got_d = _sum_over_positions(fl, 0, tr, fr, 0, tr, alpha, e)
+                assert np.abs(got_d[np.ix_(ra, rb)] - want).max() < 1e-13
+                # batched E (heff_matrix pushes all unit vectors of a sector at once)
+                got_b = _sum_over_positions(fl, 0, tr, fr, 0, tr, alpha, np.stack([e, 2.0 * e]))
+                assert np.abs(got_b[1][np.ix_(ra, rb)] - 2.0 * want).max() < 1e-13

@@ -155,12 +155,61 @@ def test_c_hat_and_9j_against_brute_force_cg():
         done += 1
 
 
+def _el_mirrored(j, m, k, q, jp, mp):
+    """Matrix element of a unit-reduced tensor operator in the MIRRORED Wigner-Eckart convention (bra and operator
+    couple to the ket): <j m|T^k_q|j' m'> = (-1)^(k-q) <j m; k -q|j' m'> <j||T||j'>  (reading G1)."""
+    return (-1) ** ((k - q) // 2) * cg(j, m, k, -q, jp, mp)
+
+
+def _c_tilde_brute_mirrored(j1, j2, j, k1, k2, k, j1p, j2p, jp):
+    """<(j1 j2)j||[T x U]^k||(j1' j2')j'> with unit reduced elements, from Clebsch-Gordan sums only, every
+    Wigner-Eckart step taken in the mirrored convention of _el_mirrored."""
+    for m in range(-j, j + 1, 2):
+        for q in range(-k, k + 1, 2):
+            mp = m - q
+            if abs(mp) > jp:
+                continue
+            den = _el_mirrored(j, m, k, q, jp, mp)
+            if abs(den) < 1e-6:
+                continue
+            tot = 0.0
+            for m1 in range(-j1, j1 + 1, 2):
+                m2 = m - m1
+                if abs(m2) > j2:
+                    continue
+                for q1 in range(-k1, k1 + 1, 2):
+                    q2 = q - q1
+                    if abs(q2) > k2:
+                        continue
+                    m1p, m2p = m1 - q1, m2 - q2
+                    if abs(m1p) > j1p or abs(m2p) > j2p:
+                        continue
+                    tot += (cg(j1, m1, j2, m2, j, m) * cg(k1, q1, k2, q2, k, q) * cg(j1p, m1p, j2p, m2p, jp, mp)
+                            * _el_mirrored(j1, m1, k1, q1, j1p, m1p) * _el_mirrored(j2, m2, k2, q2, j2p, m2p))
+            return tot / den
+    return 0.0
+
+
 def test_printed_prefactor_is_the_mirrored_convention():
-    """Eq. (5) as printed equals C-hat times sqrt((2j1'+1)(2j2'+1)(2j+1)/((2j1+1)(2j2+1)(2j'+1)))."""
-    args = (2, 1, 3, 1, 1, 2, 1, 2, 1)
-    j1, j2, j, k1, k2, k, j1p, j2p, jp = args
-    ratio = sqrt((j1p + 1) * (j2p + 1) * (j + 1) / ((j1 + 1) * (j2 + 1) * (jp + 1)))
-    assert abs(c_tilde_paper(*args) - ratio * c_hat(*args)) < 1e-14
+    """G1: Eq. (5)/(9) exactly as printed (prefactor sqrt((2j1'+1)(2j2'+1)(2j+1)(2k+1))) is the
+    product formula of the mirrored Wigner-Eckart convention -- brute-force Clebsch-Gordan sums, no 6j/9j on the
+    reference side -- and it is NOT the formula of the convention the code uses (where c_hat holds)."""
+    rnd = random.Random(11)
+    done = differs = 0
+    while done < 250:
+        j1, j2, j1p, j2p = (rnd.randrange(0, 4) for _ in range(4))
+        k1, k2 = rnd.randrange(0, 3), rnd.randrange(0, 3)
+        j = rnd.choice(range(abs(j1 - j2), j1 + j2 + 1, 2))
+        jp = rnd.choice(range(abs(j1p - j2p), j1p + j2p + 1, 2))
+        k = rnd.choice(range(abs(k1 - k2), k1 + k2 + 1, 2))
+        if not (_tri(j1, k1, j1p) and _tri(j2, k2, j2p) and _tri(j, k, jp)):
+            continue
+        ref = _c_tilde_brute_mirrored(j1, j2, j, k1, k2, k, j1p, j2p, jp)
+        got = c_tilde_paper(j1, j2, j, k1, k2, k, j1p, j2p, jp)
+        assert abs(got - ref) < 1e-12
+        differs += abs(got - _c_hat_brute(j1, j2, j, k1, k2, k, j1p, j2p, jp)) > 1e-6
+        done += 1
+    assert differs > 50          # the two conventions really differ: the printed form must not be mixed with B
 
 
 def test_9j_orthogonality_and_k0_reduction():
