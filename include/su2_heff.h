@@ -48,7 +48,9 @@ enum {
   SU2_OK = 0,
   SU2_ERR_INVALID_ARGUMENT = -1,   /* null pointer, negative size, bad index                     */
   SU2_ERR_INVALID_SECTOR = -2,     /* block references a sector that does not exist / wrong dN  */
-  SU2_ERR_INVALID_RANK = -3,       /* ranks of a row cannot be coupled (triangle rule), k1 != k2 */
+  SU2_ERR_INVALID_RANK = -3,       /* ranks of a row cannot be coupled (triangle rule), k1 != k2;
+                                      or a doubled spin / rank above 40 (S, k <= 20: the range the
+                                      factorial-based 6j/9j evaluation is validated for)          */
   SU2_ERR_NOT_FINITE = -4,         /* non-finite alpha or site element                           */
   SU2_ERR_CUDA = -5,               /* a CUDA runtime call failed (see su2_last_cuda_error)       */
   SU2_ERR_NO_DEVICE_PLAN = -6,     /* plan was created with SU2_PLAN_HOST_ONLY                   */
@@ -76,8 +78,16 @@ typedef struct {
   const int32_t* q_out;      /* HOST [nblk]: row (bra) sector index of block b                  */
   const int32_t* q_in;       /* HOST [nblk]: column (ket) sector index of block b               */
   const int64_t* blk_off;    /* HOST [nblk]: element offset of block b inside `data`            */
-  const double* data;        /* DEVICE: block b = [npos][dim(q_out)][dim(q_in)] row-major       */
+  const int32_t* blk_ld;     /* HOST [nblk] or NULL: leading dimension (elements) of block b,
+                                >= dim(q_in); NULL = dense (ld = dim(q_in))                    */
+  const double* data;        /* DEVICE: block b = [npos][dim(q_out)][ld_b] row-major, positions
+                                dim(q_out)*ld_b elements apart (pad columns are never read)    */
 } su2_opfamily;
+/* Layout advice (memory laid out for the TMA engine): a block whose ld_b is even, whose blk_off is even and whose
+ * `data` is 16-byte aligned is read IN PLACE by the large-tile kernel (bulk tensor copies need 16-byte aligned
+ * rows); ld_b a multiple of 4 keeps every row on a 32-byte sector boundary.  Any other block of a plan that runs
+ * the large-tile kernel is first copied into a padded plan-owned buffer (su2_plan_info_t.plan_device_bytes grows by
+ * the size of the family; su2_plan_create fails with SU2_ERR_CUDA if that does not fit). */
 
 /* Site operator: reduced elements r[out][in] over the site multiplets 0=(N=0,S=0),
  * 1=(1,1/2), 2=(2,0) (the site basis shrinks from four to three). */
@@ -113,7 +123,8 @@ typedef struct {
 enum {
   SU2_PLAN_DEFAULT = 0,
   SU2_PLAN_HOST_ONLY = 1,    /* no device tables: planner tests on CPU                          */
-  SU2_PLAN_FORCE_SPLIT = 2   /* tiny segments: exercises the segmented reduction on small inputs */
+  SU2_PLAN_FORCE_SPLIT = 2,  /* tiny segments: exercises the segmented reduction on small inputs */
+  SU2_PLAN_LARGE_TILES = 4   /* keep a small-block bond on the large-tile kernel (tests, A/B measurements) */
 };
 
 typedef struct {
@@ -124,15 +135,15 @@ typedef struct {
   double cc_flops;           /* CC = sum over task-positions of min(2mkn+2mnp, 2knp+2mkp)       */
   double executed_flops;     /* flops the kernels execute per apply (tile padding, recompute)   */
   double operator_bytes;     /* 8(mk+np) summed over task-positions (algorithmic HBM traffic)   */
-  int64_t workspace_bytes;   /* device workspace su2_heff_apply needs                           */
+  int64_t workspace_bytes;   /* device workspace su2_heff_apply needs (a multiple of 256)      */
   int32_t npsi_sec;          /* number of Psi sectors                                           */
   int32_t nsegments;         /* work segments (deterministic segmented reduction)               */
   int64_t nwork_items;       /* CTA-level work items per apply                                  */
   double plan_seconds;       /* host time spent in su2_plan_create                              */
   int64_t plan_device_bytes; /* device memory owned by the plan (tables, folded and transposed operators) */
   int32_t small_plan;        /* 1: every block sector holds <= 48 multiplets, su2_heff_apply runs the small-block
-                                kernel (one CTA per output sector and segment); 0: large register tiles.
-                                SU2_HEFF_SMALL=0 in the environment of su2_plan_create forces 0 (A/B measurements) */
+                                kernel (one CTA per output sector and segment); 0: large register tiles
+                                (always 0 under SU2_PLAN_LARGE_TILES) */
   int32_t reserved;
 } su2_plan_info_t;
 
@@ -142,6 +153,12 @@ typedef struct {
 su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int32_t flags, void* cuda_stream);
 su2_status su2_plan_destroy(su2_plan* plan);
 su2_status su2_plan_info(const su2_plan* plan, su2_plan_info_t* info);
+/* The planner's own 6j / 9j evaluation (Eqs. (10)-(15), :351-384; doubled arguments 0..40), exported so
+ * that it can be checked against exact arithmetic without a GPU.  NaN for an argument out of range; 0 for
+ * arguments that violate a triangle rule.  {a b c; d e f} and {j1 j2 j; k1 k2 k; j1' j2' j'}. */
+double su2_wigner_6j(int32_t a, int32_t b, int32_t c, int32_t d, int32_t e, int32_t f);
+double su2_wigner_9j(int32_t j1, int32_t j2, int32_t j, int32_t k1, int32_t k2, int32_t k,
+                     int32_t j1p, int32_t j2p, int32_t jp);
 /* labels: HOST [npsi_sec][6] = (il, sB, twoJ1, sC, ir, twoJ2); offsets: HOST [npsi_sec+1]. */
 su2_status su2_plan_psi_layout(const su2_plan* plan, int32_t* labels, int64_t* offsets);
 
@@ -154,7 +171,9 @@ su2_status su2_plan_export_tasks(const su2_plan* plan, int32_t* out_sec, int32_t
                                  int32_t* term, double* coef);
 
 /* out_dev = H_eff * psi_dev (overwrites; out must not alias psi).  Asynchronous on the stream.
- * workspace_dev: DEVICE, >= workspace_bytes, 256-byte aligned. */
+ * workspace_dev: DEVICE, >= workspace_bytes, 256-byte aligned.  The workspace and the plan's work-queue counter
+ * are shared by every apply of the plan: applies of ONE plan must be ordered on one stream (two plans may run
+ * concurrently). */
 su2_status su2_heff_apply(const su2_plan* plan, const double* psi_dev, double* out_dev,
                           void* workspace_dev, void* cuda_stream);
 /* Same through HOST buffers: copies psi to the device, applies, copies the result back and
@@ -166,9 +185,9 @@ su2_status su2_heff_apply_host(const su2_plan* plan, const double* psi_host, dou
 su2_status su2_heff_diag(const su2_plan* plan, double* diag_dev, void* cuda_stream);
 
 /* Davidson eigensolver for the lowest eigenpair (reading G8 in DESIGN.md):
- * diagonal preconditioner, modified Gram-Schmidt applied twice, subspace <= max_subspace
- * (restart from the Ritz vector when full).  All vectors live in dav_workspace_dev
- * (DEVICE, su2_davidson_workspace_bytes bytes, caller-owned). */
+ * diagonal correction while theta < min(diag) and the Krylov direction otherwise (su2_davidson_set_preconditioner),
+ * classical Gram-Schmidt applied twice, subspace <= max_subspace <= 64 (restart from the Ritz vector when full).
+ * All vectors live in dav_workspace_dev (DEVICE, su2_davidson_workspace_bytes bytes, caller-owned). */
 int64_t su2_davidson_workspace_bytes(const su2_plan* plan, int32_t max_subspace);
 su2_status su2_davidson_create(su2_davidson** out, const su2_plan* plan, int32_t max_subspace,
                                const double* x0_dev, void* dav_workspace_dev, void* cuda_stream);
@@ -181,10 +200,16 @@ typedef int32_t (*su2_reduce_fn)(double* vec_dev, int64_t n, void* cuda_stream, 
 su2_status su2_davidson_create_sharded(su2_davidson** out, const su2_plan* plan, int32_t max_subspace,
                                        const double* x0_dev, void* dav_workspace_dev, void* cuda_stream,
                                        su2_reduce_fn reduce, void* reduce_user);
-/* One iteration: w = H_eff v (su2_heff_apply), Rayleigh-Ritz, residual, new direction.
- * theta: current Ritz value; resnorm: |H x - theta x|.  Synchronises for the two scalars. */
+/* One iteration: w = H_eff v (su2_heff_apply), Rayleigh-Ritz, residual, new direction (the paper gives
+ * no detail, reading G8).  Everything runs on the device, ordered on cuda_stream: the k x k Ritz problem
+ * is solved by one CTA, coefficients never leave device memory.  The call synchronises ONCE, at its end, for the two
+ * scalars it hands back.  theta: current Ritz value; resnorm: |H x - theta x|. */
 su2_status su2_davidson_step(const su2_plan* plan, su2_davidson* dav, void* workspace_dev,
                              void* cuda_stream, double* theta, double* resnorm);
+/* New-direction rule.  mode 1 (default): diagonal correction t = r / (diag - theta) while theta < min(diag) (minus a
+ * margin of 1e-3 of the spread of diag), else the Krylov direction t = r; mode 0: always t = r (the solver is then a
+ * restarted Lanczos iteration).  Other values: SU2_ERR_INVALID_ARGUMENT. */
+su2_status su2_davidson_set_preconditioner(su2_davidson* dav, int32_t mode);
 su2_status su2_davidson_ritz_vector(const su2_davidson* dav, double* x_dev, void* cuda_stream);
 su2_status su2_davidson_destroy(su2_davidson* dav);
 

@@ -21,7 +21,7 @@ class su2_sector(C.Structure):
 class su2_opfamily(C.Structure):
     _fields_ = [("dN", C.c_int32), ("twoK", C.c_int32), ("npos", C.c_int32), ("nblk", C.c_int32),
                 ("q_out", C.POINTER(C.c_int32)), ("q_in", C.POINTER(C.c_int32)),
-                ("blk_off", C.POINTER(C.c_int64)), ("data", C.c_void_p)]
+                ("blk_off", C.POINTER(C.c_int64)), ("blk_ld", C.POINTER(C.c_int32)), ("data", C.c_void_p)]
 
 
 class su2_siteop(C.Structure):
@@ -51,9 +51,9 @@ class su2_plan_info_t(C.Structure):
                 ("small_plan", C.c_int32), ("reserved", C.c_int32)]
 
 
-EXPORTS = ["su2_status_string", "su2_last_cuda_error", "su2_kernel_launch_count", "su2_plan_create", "su2_plan_destroy", "su2_plan_info",
+EXPORTS = ["su2_wigner_6j", "su2_wigner_9j", "su2_status_string", "su2_last_cuda_error", "su2_kernel_launch_count", "su2_plan_create", "su2_plan_destroy", "su2_plan_info",
            "su2_plan_psi_layout", "su2_plan_export_tasks", "su2_heff_apply", "su2_heff_apply_host", "su2_heff_diag",
-           "su2_davidson_workspace_bytes", "su2_davidson_create", "su2_davidson_create_sharded", "su2_davidson_step", "su2_davidson_ritz_vector",
+           "su2_davidson_workspace_bytes", "su2_davidson_create", "su2_davidson_create_sharded", "su2_davidson_step", "su2_davidson_set_preconditioner", "su2_davidson_ritz_vector",
            "su2_davidson_destroy", "su2_gemm_pair_batched", "su2_probe_fp64_peak"]
 
 REDUCE_FN = C.CFUNCTYPE(C.c_int32, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p)   # su2_reduce_fn
@@ -74,6 +74,10 @@ def load():
     lib = C.CDLL(LIB_PATH)
     for name in EXPORTS:
         getattr(lib, name).restype = C.c_int32
+    lib.su2_wigner_6j.restype = C.c_double
+    lib.su2_wigner_6j.argtypes = [C.c_int32] * 6
+    lib.su2_wigner_9j.restype = C.c_double
+    lib.su2_wigner_9j.argtypes = [C.c_int32] * 9
     lib.su2_status_string.restype = C.c_char_p
     lib.su2_status_string.argtypes = [C.c_int32]
     lib.su2_last_cuda_error.restype = C.c_char_p
@@ -93,6 +97,7 @@ def load():
                                                 C.c_void_p, REDUCE_FN, C.c_void_p]
     lib.su2_davidson_step.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                       C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.su2_davidson_set_preconditioner.argtypes = [C.c_void_p, C.c_int32]
     lib.su2_davidson_ritz_vector.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     lib.su2_davidson_destroy.argtypes = [C.c_void_p]
     lib.su2_gemm_pair_batched.argtypes = [C.c_int32] * 4 + [C.c_int64, C.c_double] + [C.c_void_p] * 5
@@ -135,7 +140,7 @@ class Plan:
     blocks laid out block after block, each [npos][m][k] (see family_block_offsets); None
     for a host-only plan (planner tests without a GPU)."""
 
-    def __init__(self, problem, family_ptrs=None, stream=0, host_only=False, force_split=False):
+    def __init__(self, problem, family_ptrs=None, stream=0, host_only=False, force_split=False, large_tiles=False):
         lib = load()
         self._keep = []
         self.problem = problem
@@ -154,7 +159,7 @@ class Plan:
                 ptr = None if family_ptrs is None else family_ptrs[(side, i)]
                 arr[i] = su2_opfamily(f.dN, f.twoK, f.npos, len(f.q_out),
                                       qo.ctypes.data_as(C.POINTER(C.c_int32)), qi.ctypes.data_as(C.POINTER(C.c_int32)),
-                                      off.ctypes.data_as(C.POINTER(C.c_int64)), ptr)
+                                      off.ctypes.data_as(C.POINTER(C.c_int64)), C.POINTER(C.c_int32)(), ptr)
             self._keep.append(arr)
             return arr
 
@@ -183,7 +188,7 @@ class Plan:
                            len(problem.fam_l), len(problem.fam_r), fl, fr, len(problem.site), site,
                            len(problem.term), terms)
         self.handle = C.c_void_p()
-        check(lib.su2_plan_create(C.byref(self.handle), C.byref(prob), (SU2_PLAN_HOST_ONLY if host_only else 0) | (2 if force_split else 0),
+        check(lib.su2_plan_create(C.byref(self.handle), C.byref(prob), (SU2_PLAN_HOST_ONLY if host_only else 0) | (2 if force_split else 0) | (4 if large_tiles else 0),
                                   C.c_void_p(stream)))
         info = su2_plan_info_t()
         check(lib.su2_plan_info(self.handle, C.byref(info)))
@@ -230,15 +235,31 @@ class Plan:
 
 class Davidson:
     def __init__(self, plan, max_subspace, x0_ptr, ws_ptr, stream=0, reduce=None):
-        """reduce(vec_ptr, n, stream) -> status: sum over ranks of a device vector (position-sharded plans)."""
+        """reduce(vec_ptr, n, stream) -> status: sum over ranks of a device vector (position-sharded plans).
+        An exception raised inside the hook is stored, reported to the library as a negative status (the C call
+        stops there instead of continuing on an un-reduced vector) and re-raised from the Python call."""
         self.plan = plan
         self.handle = C.c_void_p()
+        self._hook_error = None
         if reduce is None:
             check(load().su2_davidson_create(C.byref(self.handle), plan.handle, max_subspace, x0_ptr, ws_ptr, stream))
         else:
-            self._reduce = REDUCE_FN(lambda vec, n, st, user: int(reduce(vec, n, st) or 0))   # keep the thunk alive
-            check(load().su2_davidson_create_sharded(C.byref(self.handle), plan.handle, max_subspace, x0_ptr, ws_ptr,
-                                                     stream, self._reduce, None))
+            def thunk(vec, n, st, user):
+                try:
+                    return int(reduce(vec, n, st) or 0)
+                except BaseException as exc:          # never let an exception escape into ctypes
+                    self._hook_error = exc
+                    return -5
+            self._reduce = REDUCE_FN(thunk)           # keep the thunk alive
+            st = load().su2_davidson_create_sharded(C.byref(self.handle), plan.handle, max_subspace, x0_ptr, ws_ptr,
+                                                    stream, self._reduce, None)
+            self._raise_hook_error()
+            check(st)
+
+    def _raise_hook_error(self):
+        if self._hook_error is not None:
+            exc, self._hook_error = self._hook_error, None
+            raise exc
 
     @staticmethod
     def workspace_bytes(plan, max_subspace):
@@ -246,8 +267,13 @@ class Davidson:
 
     def step(self, workspace_ptr, stream=0):
         th, rn = C.c_double(), C.c_double()
-        check(load().su2_davidson_step(self.plan.handle, self.handle, workspace_ptr, stream, C.byref(th), C.byref(rn)))
+        st = load().su2_davidson_step(self.plan.handle, self.handle, workspace_ptr, stream, C.byref(th), C.byref(rn))
+        self._raise_hook_error()
+        check(st)
         return th.value, rn.value
+
+    def set_preconditioner(self, mode):
+        check(load().su2_davidson_set_preconditioner(self.handle, int(mode)))
 
     def ritz_vector(self, x_ptr, stream=0):
         check(load().su2_davidson_ritz_vector(self.handle, x_ptr, stream))
@@ -267,6 +293,14 @@ def probe_fp64_peak(kind, iters=20000, ctas_per_sm=4, stream=0):
     v = C.c_double()
     check(load().su2_probe_fp64_peak(kind, iters, ctas_per_sm, C.byref(v), stream))
     return v.value
+
+
+def wigner_6j(*two_j):
+    return float(load().su2_wigner_6j(*[int(x) for x in two_j]))
+
+
+def wigner_9j(*two_j):
+    return float(load().su2_wigner_9j(*[int(x) for x in two_j]))
 
 
 def kernel_launch_count():

@@ -1,8 +1,16 @@
 // Davidson eigensolver around su2_heff_apply ("iterative
 // diagonalization ... via the Lanczos or Davidson algorithms").  The paper gives no algorithmic
-// detail; reading G8: diagonal preconditioner t = r / (theta - diag) with |theta - diag|
-// floored at 1e-8 * max|diag|, modified Gram-Schmidt applied twice, restart from the Ritz vector
-// when the subspace is full.  BLAS-1 parts use fixed-grid two-stage reductions (deterministic).
+// detail; reading G8:
+//   * Rayleigh-Ritz in a subspace of at most max_subspace vectors, restart from the Ritz vector when full;
+//   * new direction t = r / (diag - theta) ONLY while theta lies below min(diag) by a margin (the Newton-like
+//     diagonal correction is then positive definite); otherwise the plain Krylov direction t = r.  With theta
+//     inside the range of diag the quotient collapses to spikes on the few elements whose diag is close to
+//     theta and the iteration stalls (measured in round 1: |r| flat over 20 steps at configs[2]);
+//   * classical Gram-Schmidt applied twice (one batched projection + one update per pass).
+// Everything between the apply and the two scalars handed back runs on the device, stream-ordered: the k x k
+// Rayleigh-Ritz problem (k <= 64) is diagonalised by ONE CTA with a parallel-ordered cyclic Jacobi, coefficients
+// stay in device memory, and a step synchronises once, at its end, for (theta, |r|).  BLAS-1 parts use fixed-grid
+// two-stage reductions (deterministic).
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -26,8 +34,12 @@ namespace {
 constexpr int RED_BLOCKS = 296;    // 2 per SM; fixed so that sums are reproducible
 constexpr int RED_THREADS = 256;
 constexpr int MAX_SUB = 64;
-
-struct Coefs { double c[MAX_SUB]; };
+// layout of the small device state behind the reduction scratch (doubles)
+constexpr int ST_G = 0;                          // MAX_SUB x MAX_SUB projected matrix G = V^T H V (leading dimension MAX_SUB)
+constexpr int ST_Y = ST_G + MAX_SUB * MAX_SUB;   // Ritz vector in the subspace
+constexpr int ST_C = ST_Y + MAX_SUB;             // Gram-Schmidt projections / norms
+constexpr int ST_RES = ST_C + MAX_SUB;           // [theta, |r|^2, min(diag), max(diag)]
+constexpr int ST_SIZE = ST_RES + 8;
 
 // partial[j][b] = sum over block b's stripe of x_j[i]*y[i]  (j = blockIdx.y)
 __global__ void __launch_bounds__(RED_THREADS)
@@ -44,8 +56,9 @@ dot_stage1(const double* __restrict__ xs, int64_t xstride, const double* __restr
   }
   if (threadIdx.x == 0) partial[(int64_t)blockIdx.y * RED_BLOCKS + blockIdx.x] = sm[0];
 }
+// result j = sum_b partial[j][b], stored at out1[j * s1] and (if out2) out2[j * s2]
 __global__ void __launch_bounds__(RED_THREADS)
-dot_stage2(const double* __restrict__ partial, double* __restrict__ result) {
+dot_stage2(const double* __restrict__ partial, double* __restrict__ out1, int s1, double* __restrict__ out2, int s2) {
   __shared__ double sm[RED_THREADS];
   double s = 0.0;
   for (int i = threadIdx.x; i < RED_BLOCKS; i += RED_THREADS) s += partial[(int64_t)blockIdx.x * RED_BLOCKS + i];
@@ -55,97 +68,228 @@ dot_stage2(const double* __restrict__ partial, double* __restrict__ result) {
     if (threadIdx.x < w) sm[threadIdx.x] += sm[threadIdx.x + w];
     __syncthreads();
   }
-  if (threadIdx.x == 0) result[blockIdx.x] = sm[0];
+  if (threadIdx.x == 0) {
+    out1[(int64_t)blockIdx.x * s1] = sm[0];
+    if (out2) out2[(int64_t)blockIdx.x * s2] = sm[0];
+  }
 }
+// min and max of x (two-stage, one launch each)
 __global__ void __launch_bounds__(RED_THREADS)
-maxabs_stage1(const double* __restrict__ x, int64_t n, double* __restrict__ partial) {
-  __shared__ double sm[RED_THREADS];
-  double s = 0.0;
-  for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (int64_t)RED_BLOCKS * RED_THREADS) s = fmax(s, fabs(x[i]));
-  sm[threadIdx.x] = s;
+minmax_stage1(const double* __restrict__ x, int64_t n, double* __restrict__ partial) {
+  __shared__ double lo[RED_THREADS], hi[RED_THREADS];
+  double a = INFINITY, b = -INFINITY;
+  for (int64_t i = (int64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (int64_t)RED_BLOCKS * RED_THREADS) {
+    a = fmin(a, x[i]);
+    b = fmax(b, x[i]);
+  }
+  lo[threadIdx.x] = a; hi[threadIdx.x] = b;
   __syncthreads();
   for (int w = RED_THREADS / 2; w > 0; w >>= 1) {
-    if (threadIdx.x < w) sm[threadIdx.x] = fmax(sm[threadIdx.x], sm[threadIdx.x + w]);
+    if (threadIdx.x < w) {
+      lo[threadIdx.x] = fmin(lo[threadIdx.x], lo[threadIdx.x + w]);
+      hi[threadIdx.x] = fmax(hi[threadIdx.x], hi[threadIdx.x + w]);
+    }
     __syncthreads();
   }
-  if (threadIdx.x == 0) partial[blockIdx.x] = sm[0];
+  if (threadIdx.x == 0) { partial[2 * blockIdx.x] = lo[0]; partial[2 * blockIdx.x + 1] = hi[0]; }
 }
-// out = sum_j c[j] * (a_j - shift * b_j)   (b may be null: out = sum_j c[j] a_j)
+__global__ void __launch_bounds__(RED_THREADS)
+minmax_stage2(const double* __restrict__ partial, double* __restrict__ out) {
+  __shared__ double lo[RED_THREADS], hi[RED_THREADS];
+  double a = INFINITY, b = -INFINITY;
+  for (int i = threadIdx.x; i < RED_BLOCKS; i += RED_THREADS) { a = fmin(a, partial[2 * i]); b = fmax(b, partial[2 * i + 1]); }
+  lo[threadIdx.x] = a; hi[threadIdx.x] = b;
+  __syncthreads();
+  for (int w = RED_THREADS / 2; w > 0; w >>= 1) {
+    if (threadIdx.x < w) {
+      lo[threadIdx.x] = fmin(lo[threadIdx.x], lo[threadIdx.x + w]);
+      hi[threadIdx.x] = fmax(hi[threadIdx.x], hi[threadIdx.x + w]);
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) { out[0] = lo[0]; out[1] = hi[0]; }
+}
+
+// Rayleigh-Ritz on the device: lowest eigenpair of the k x k symmetric matrix G (leading dimension MAX_SUB).
+// One CTA.  Cyclic Jacobi in the round-robin ("tournament") order: a sweep is K-1 rounds of K/2 rotations on
+// disjoint index pairs, which commute and are applied together -- columns (and the eigenvector matrix) by all
+// threads, then rows.  Sweeps stop when the off-diagonal mass is below 1e-30 of the Frobenius norm.
+// Output: y[0..k) = eigenvector of the lowest eigenvalue (sign: largest component positive), res[0] = theta.
 __global__ void __launch_bounds__(256)
-lincomb(double* __restrict__ out, const double* __restrict__ a, const double* __restrict__ b, int64_t stride, int k, Coefs c,
-        double shift, int64_t n) {
+ritz_kernel(const double* __restrict__ G, int k, double* __restrict__ y, double* __restrict__ res) {
+  extern __shared__ double ritz_smem[];              // a, v: K x (K + 1) each
+  const int K = (k + 1) & ~1;                       // even number of players; index k (if k is odd) sits out
+  const int LD = K + 1;
+  double* a_ = ritz_smem;
+  double* v_ = ritz_smem + K * LD;
+#define a(i, j) a_[(i) * LD + (j)]
+#define v(i, j) v_[(i) * LD + (j)]
+  __shared__ double cs[MAX_SUB / 2][2];
+  __shared__ int pq[MAX_SUB / 2][2];
+  __shared__ double red[256];
+  __shared__ int s_lo;
+  const int tid = threadIdx.x;
+  for (int e = tid; e < K * K; e += 256) {
+    const int i = e / K, j = e % K;
+    a(i, j) = (i < k && j < k) ? G[i * MAX_SUB + j] : 0.0;
+    v(i, j) = (i == j) ? 1.0 : 0.0;
+  }
+  __syncthreads();
+  for (int sweep = 0; sweep < 30; ++sweep) {
+    double off = 0.0, tot = 0.0;
+    for (int e = tid; e < k * k; e += 256) {
+      const int i = e / k, j = e % k;
+      const double x = a(i, j) * a(i, j);
+      tot += x;
+      if (i != j) off += x;
+    }
+    red[tid] = off;
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) { if (tid < w) red[tid] += red[tid + w]; __syncthreads(); }
+    off = red[0];
+    __syncthreads();
+    red[tid] = tot;
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) { if (tid < w) red[tid] += red[tid + w]; __syncthreads(); }
+    tot = red[0];
+    __syncthreads();
+    if (off <= 1e-30 * tot || k < 2) break;
+    for (int round = 0; round < K - 1; ++round) {
+      if (tid < K / 2) {
+        // circle method: player K-1 is fixed, the others rotate
+        int p, q;
+        if (tid == 0) { p = K - 1; q = (K - 1 - round) % (K - 1); }
+        else { p = (tid + (K - 1) - round % (K - 1)) % (K - 1); q = ((K - 1 - tid) + (K - 1) - round % (K - 1)) % (K - 1); }
+        if (p > q) { const int t = p; p = q; q = t; }
+        double c = 1.0, s = 0.0;
+        if (q < k) {
+          const double apq = a(p, q);
+          if (fabs(apq) > 1e-300) {
+            const double tau = (a(q, q) - a(p, p)) / (2.0 * apq);
+            const double t = (tau >= 0 ? 1.0 : -1.0) / (fabs(tau) + sqrt(1.0 + tau * tau));
+            c = 1.0 / sqrt(1.0 + t * t);
+            s = t * c;
+          }
+        }
+        pq[tid][0] = p; pq[tid][1] = q; cs[tid][0] = c; cs[tid][1] = s;
+      }
+      __syncthreads();
+      for (int e = tid; e < K * (K / 2); e += 256) {       // A <- A J, V <- V J
+        const int i = e / (K / 2), r = e % (K / 2);
+        const int p = pq[r][0], q = pq[r][1];
+        const double c = cs[r][0], s = cs[r][1];
+        const double aip = a(i, p), aiq = a(i, q);
+        a(i, p) = c * aip - s * aiq;
+        a(i, q) = s * aip + c * aiq;
+        const double vip = v(i, p), viq = v(i, q);
+        v(i, p) = c * vip - s * viq;
+        v(i, q) = s * vip + c * viq;
+      }
+      __syncthreads();
+      for (int e = tid; e < K * (K / 2); e += 256) {       // A <- J^T A
+        const int i = e / (K / 2), r = e % (K / 2);
+        const int p = pq[r][0], q = pq[r][1];
+        const double c = cs[r][0], s = cs[r][1];
+        const double api = a(p, i), aqi = a(q, i);
+        a(p, i) = c * api - s * aqi;
+        a(q, i) = s * api + c * aqi;
+      }
+      __syncthreads();
+    }
+  }
+  if (tid == 0) {
+    int lo = 0;
+    for (int i = 1; i < k; ++i)
+      if (a(i, i) < a(lo, lo)) lo = i;
+    s_lo = lo;
+    res[0] = a(lo, lo);
+  }
+  __syncthreads();
+  const int lo = s_lo;
+  if (tid == 0) {
+    int big = 0;
+    for (int i = 1; i < k; ++i)
+      if (fabs(v(i, lo)) > fabs(v(big, lo))) big = i;
+    red[0] = v(big, lo) < 0.0 ? -1.0 : 1.0;
+  }
+  __syncthreads();
+  if (tid < MAX_SUB) y[tid] = tid < k ? red[0] * v(tid, lo) : 0.0;
+#undef a
+#undef v
+}
+
+// out = sum_j c[j] * (a_j - shift * b_j), c = y (device), shift = res[0] (device) if b, else out = sum_j c[j] a_j.
+// With `partial`: also the block-partial sums of out^2 (stage 1 of |out|^2; grid must be RED_BLOCKS x RED_THREADS).
+__global__ void __launch_bounds__(RED_THREADS)
+lincomb_dev(double* __restrict__ out, const double* __restrict__ a, const double* __restrict__ b, int64_t stride, int k,
+            const double* __restrict__ y, const double* __restrict__ res, int64_t n, double* __restrict__ partial) {
+  __shared__ double c[MAX_SUB];
+  __shared__ double sm[RED_THREADS];
+  if (threadIdx.x < k) c[threadIdx.x] = y[threadIdx.x];
+  __syncthreads();
+  const double shift = b ? res[0] : 0.0;
+  double ss = 0.0;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
     double s = 0.0;
     for (int j = 0; j < k; ++j) {
       double v = a[(int64_t)j * stride + i];
       if (b) v -= shift * b[(int64_t)j * stride + i];
-      s += c.c[j] * v;
+      s += c[j] * v;
     }
     out[i] = s;
+    ss += s * s;
+  }
+  if (partial) {
+    sm[threadIdx.x] = ss;
+    __syncthreads();
+    for (int w = RED_THREADS / 2; w > 0; w >>= 1) {
+      if (threadIdx.x < w) sm[threadIdx.x] += sm[threadIdx.x + w];
+      __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = sm[0];
   }
 }
-__global__ void __launch_bounds__(256) axpy(double* __restrict__ y, const double* __restrict__ x, double a, int64_t n) {
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) y[i] += a * x[i];
+// Gram-Schmidt update t -= sum_j c[j] V_j with the projections c left on the device by dot_stage2
+__global__ void __launch_bounds__(256)
+gs_update(double* __restrict__ t, const double* __restrict__ V, int64_t stride, int k, const double* __restrict__ cdev, int64_t n) {
+  __shared__ double c[MAX_SUB];
+  if (threadIdx.x < k) c[threadIdx.x] = cdev[threadIdx.x];
+  __syncthreads();
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    double s = t[i];
+    for (int j = 0; j < k; ++j) s -= c[j] * V[(int64_t)j * stride + i];
+    t[i] = s;
+  }
 }
-// the same two with the scalar left on the device by dot_stage2 (no host round trip inside Gram-Schmidt):
-// y -= c[0] x, and y = x / sqrt(c[0]) (0 if c[0] == 0); same operations, same bits as the host-scalar versions
-__global__ void __launch_bounds__(256) axpy_neg_dev(double* __restrict__ y, const double* __restrict__ x, const double* __restrict__ c, int64_t n) {
-  const double a = -c[0];
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) y[i] += a * x[i];
-}
+// y = x / sqrt(c[0]) (0 if c[0] == 0)
 __global__ void __launch_bounds__(256) scale_copy_rnorm_dev(double* __restrict__ y, const double* __restrict__ x, const double* __restrict__ c, int64_t n) {
   const double nrm = sqrt(c[0]);
   const double a = nrm > 0 ? 1.0 / nrm : 0.0;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) y[i] = a * x[i];
 }
-__global__ void __launch_bounds__(256) scale_copy(double* __restrict__ y, const double* __restrict__ x, double a, int64_t n) {
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) y[i] = a * x[i];
-}
-// t = r / (theta - diag), |theta - diag| floored at `floor_` keeping the sign
-__global__ void __launch_bounds__(256)
-precondition(double* __restrict__ t, const double* __restrict__ r, const double* __restrict__ diag, double theta, double floor_, int64_t n) {
+__global__ void __launch_bounds__(256) copy2(double* __restrict__ y0, const double* __restrict__ x0, double* __restrict__ y1,
+                                             const double* __restrict__ x1, int64_t n) {
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
-    double den = theta - diag[i];
-    if (fabs(den) < floor_) den = den < 0.0 ? -floor_ : floor_;
-    t[i] = r[i] / den;
+    y0[i] = x0[i];
+    if (y1) y1[i] = x1[i];
   }
 }
-
-// cyclic Jacobi eigen-decomposition of a small symmetric matrix (k <= 64): a -> eigenvalues, v columns
-void jacobi_eigh(int k, std::vector<double>& a, std::vector<double>& v, std::vector<double>& w) {
-  v.assign((size_t)k * k, 0.0);
-  for (int i = 0; i < k; ++i) v[(size_t)i * k + i] = 1.0;
-  for (int sweep = 0; sweep < 100; ++sweep) {
-    double off = 0.0;
-    for (int i = 0; i < k; ++i)
-      for (int j = i + 1; j < k; ++j) off += a[(size_t)i * k + j] * a[(size_t)i * k + j];
-    if (off < 1e-300) break;
-    for (int p = 0; p < k; ++p)
-      for (int q = p + 1; q < k; ++q) {
-        const double apq = a[(size_t)p * k + q];
-        if (std::fabs(apq) < 1e-300) continue;
-        const double tau = (a[(size_t)q * k + q] - a[(size_t)p * k + p]) / (2.0 * apq);
-        const double t = (tau >= 0 ? 1.0 : -1.0) / (std::fabs(tau) + std::sqrt(1.0 + tau * tau));
-        const double c = 1.0 / std::sqrt(1.0 + t * t), s = t * c;
-        for (int i = 0; i < k; ++i) {
-          const double aip = a[(size_t)i * k + p], aiq = a[(size_t)i * k + q];
-          a[(size_t)i * k + p] = c * aip - s * aiq;
-          a[(size_t)i * k + q] = s * aip + c * aiq;
-        }
-        for (int i = 0; i < k; ++i) {
-          const double api = a[(size_t)p * k + i], aqi = a[(size_t)q * k + i];
-          a[(size_t)p * k + i] = c * api - s * aqi;
-          a[(size_t)q * k + i] = s * api + c * aqi;
-        }
-        for (int i = 0; i < k; ++i) {
-          const double vip = v[(size_t)i * k + p], viq = v[(size_t)i * k + q];
-          v[(size_t)i * k + p] = c * vip - s * viq;
-          v[(size_t)i * k + q] = s * vip + c * viq;
-        }
-      }
-  }
-  w.resize(k);
-  for (int i = 0; i < k; ++i) w[i] = a[(size_t)i * k + i];
+// New direction (reading G8): res = [theta, |r|^2, min(diag), max(diag)].  While theta < min(diag) - margin the
+// diagonal correction t = r / (diag - theta) (all denominators positive, >= margin); otherwise t = r.
+__global__ void __launch_bounds__(256)
+precondition(double* __restrict__ t, const double* __restrict__ r, const double* __restrict__ diag, const double* __restrict__ res,
+             int mode, int64_t n) {
+  const double theta = res[0], dmin = res[2], dmax = res[3];
+  const double margin = 1e-3 * fmax(dmax - dmin, 1e-300) + 1e-12 * fmax(fabs(dmin), fabs(dmax));
+  const bool use_diag = mode == 1 && theta < dmin - margin;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+    t[i] = use_diag ? r[i] / (diag[i] - theta) : r[i];
+}
+// after a restart the subspace is {Ritz vector}: G = [theta], y = [1]
+__global__ void restart_state(double* __restrict__ st) {
+  const int i = threadIdx.x + blockIdx.x * blockDim.x;
+  if (i < MAX_SUB * MAX_SUB) st[ST_G + i] = (i == 0) ? st[ST_RES] : 0.0;
+  if (i < MAX_SUB) st[ST_Y + i] = (i == 0) ? 1.0 : 0.0;
 }
 
 }  // namespace
@@ -153,43 +297,31 @@ void jacobi_eigh(int k, std::vector<double>& a, std::vector<double>& v, std::vec
 struct su2_davidson {
   int64_t n = 0;
   int32_t mmax = 0, k = 0;      // k basis vectors V[0..k), W computed for [0..k-1)
+  int32_t ky = 0;               // valid entries of the Ritz vector y (device)
   double *V = nullptr, *W = nullptr, *diag = nullptr, *r = nullptr, *t = nullptr, *u = nullptr, *scratch = nullptr;
+  double* state = nullptr;      // device: G, y, Gram-Schmidt coefficients, [theta, |r|^2, min diag, max diag]
   double* h_result = nullptr;   // pinned
-  std::vector<double> G;        // mmax x mmax projected matrix
-  std::vector<double> y;        // last Ritz vector in the subspace
-  double diag_floor = 0.0;
+  int32_t precond_mode = 1;     // 1: diagonal correction when theta < min(diag) (else Krylov); 0: always Krylov
   int32_t grid = 296;
   su2_reduce_fn reduce = nullptr;   // position-sharded plans: sums a vector over the ranks (null: single GPU)
   void* reduce_user = nullptr;
 };
 
-static su2_status dots(su2_davidson* d, const double* xs, int nx, const double* y, double* host_out, cudaStream_t st) {
-  dim3 g1(RED_BLOCKS, nx);
-  dot_stage1<<<g1, RED_THREADS, 0, st>>>(xs, d->n, y, d->n, d->scratch); su2::count_launch();
-  dot_stage2<<<nx, RED_THREADS, 0, st>>>(d->scratch, d->scratch + (int64_t)MAX_SUB * RED_BLOCKS); su2::count_launch();
-  SU2_CUDA(cudaGetLastError());
-  SU2_CUDA(cudaMemcpyAsync(d->h_result, d->scratch + (int64_t)MAX_SUB * RED_BLOCKS, nx * sizeof(double), cudaMemcpyDeviceToHost, st));
-  SU2_CUDA(cudaStreamSynchronize(st));
-  for (int i = 0; i < nx; ++i) host_out[i] = d->h_result[i];
-  return SU2_OK;
-}
-
-// orthogonalise d->t against V[0..k) (modified Gram-Schmidt, twice), normalise into V[k]
+// orthogonalise d->t against V[0..k) (classical Gram-Schmidt, twice), normalise into V[k]; stream-ordered
 static su2_status orthonormalise_into_basis(su2_davidson* d, cudaStream_t st) {
-  // every scalar (projection, norm) stays on the device: the loop is stream-ordered, no synchronisation
-  double* res = d->scratch + (int64_t)MAX_SUB * RED_BLOCKS;
-  auto dot_dev = [&](const double* x, const double* y) {
-    dim3 g1(RED_BLOCKS, 1);
-    dot_stage1<<<g1, RED_THREADS, 0, st>>>(x, d->n, y, d->n, d->scratch); su2::count_launch();
-    dot_stage2<<<1, RED_THREADS, 0, st>>>(d->scratch, res); su2::count_launch();
-  };
-  for (int pass = 0; pass < 2; ++pass)
-    for (int i = 0; i < d->k; ++i) {
-      dot_dev(d->V + (int64_t)i * d->n, d->t);
-      axpy_neg_dev<<<d->grid, 256, 0, st>>>(d->t, d->V + (int64_t)i * d->n, res, d->n); su2::count_launch();
-    }
-  dot_dev(d->t, d->t);
-  scale_copy_rnorm_dev<<<d->grid, 256, 0, st>>>(d->V + (int64_t)d->k * d->n, d->t, res, d->n); su2::count_launch();
+  double* cdev = d->state + ST_C;
+  const int k = d->k;
+  for (int pass = 0; pass < 2 && k > 0; ++pass) {
+    dim3 g1(RED_BLOCKS, k);
+    dot_stage1<<<g1, RED_THREADS, 0, st>>>(d->V, d->n, d->t, d->n, d->scratch);
+    dot_stage2<<<k, RED_THREADS, 0, st>>>(d->scratch, cdev, 1, nullptr, 0);
+    gs_update<<<d->grid, 256, 0, st>>>(d->t, d->V, d->n, k, cdev, d->n);
+    su2::count_launch(3);
+  }
+  dot_stage1<<<dim3(RED_BLOCKS, 1), RED_THREADS, 0, st>>>(d->t, d->n, d->t, d->n, d->scratch);
+  dot_stage2<<<1, RED_THREADS, 0, st>>>(d->scratch, cdev, 1, nullptr, 0);
+  scale_copy_rnorm_dev<<<d->grid, 256, 0, st>>>(d->V + (int64_t)k * d->n, d->t, cdev, d->n);
+  su2::count_launch(3);
   SU2_CUDA(cudaGetLastError());
   d->k += 1;
   return SU2_OK;
@@ -198,7 +330,7 @@ static su2_status orthonormalise_into_basis(su2_davidson* d, cudaStream_t st) {
 extern "C" int64_t su2_davidson_workspace_bytes(const su2_plan* plan, int32_t max_subspace) {
   if (!plan || max_subspace < 2 || max_subspace > MAX_SUB) return -1;
   const int64_t n = plan->psi_len;
-  return (2 * (int64_t)max_subspace + 4) * n * 8 + ((int64_t)MAX_SUB * RED_BLOCKS + MAX_SUB) * 8 + 256;
+  return (2 * (int64_t)max_subspace + 4) * n * 8 + ((int64_t)MAX_SUB * RED_BLOCKS + ST_SIZE) * 8 + 256;
 }
 
 extern "C" su2_status su2_davidson_create(su2_davidson** out, const su2_plan* plan, int32_t max_subspace, const double* x0_dev,
@@ -226,31 +358,33 @@ extern "C" su2_status su2_davidson_create_sharded(su2_davidson** out, const su2_
   d->t = d->r + n;
   d->u = d->t + n;
   d->scratch = d->u + n;
-  d->G.assign((size_t)max_subspace * max_subspace, 0.0);
+  d->state = d->scratch + (int64_t)MAX_SUB * RED_BLOCKS;
   d->grid = 2 * plan->num_sms;
-  if (cudaMallocHost(&d->h_result, MAX_SUB * sizeof(double)) != cudaSuccess) {
+  if (cudaMallocHost(&d->h_result, 8 * sizeof(double)) != cudaSuccess) {
     delete d;
     return SU2_ERR_CUDA;
   }
+  if (cudaFuncSetAttribute(ritz_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)(2 * MAX_SUB * (MAX_SUB + 1) * sizeof(double))) != cudaSuccess) { su2_davidson_destroy(d); return SU2_ERR_CUDA; }
+  if (cudaMemsetAsync(d->state, 0, ST_SIZE * sizeof(double), st) != cudaSuccess) { su2_davidson_destroy(d); return SU2_ERR_CUDA; }
   su2_status s = su2_heff_diag(plan, d->diag, cuda_stream);
   if (s == SU2_OK && d->reduce) s = d->reduce(d->diag, d->n, cuda_stream, d->reduce_user);   // diag of a sum of shards
   if (s != SU2_OK) { su2_davidson_destroy(d); return s; }
-  maxabs_stage1<<<RED_BLOCKS, RED_THREADS, 0, st>>>(d->diag, d->n, d->scratch); su2::count_launch();
-  std::vector<double> part(RED_BLOCKS);
-  if (cudaMemcpyAsync(part.data(), d->scratch, RED_BLOCKS * sizeof(double), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
-      cudaStreamSynchronize(st) != cudaSuccess) {
-    su2_davidson_destroy(d);
-    return SU2_ERR_CUDA;
-  }
-  double mx = 0.0;
-  for (double v : part) mx = std::fmax(mx, v);
-  d->diag_floor = 1e-8 * (mx > 0 ? mx : 1.0);
+  minmax_stage1<<<RED_BLOCKS, RED_THREADS, 0, st>>>(d->diag, d->n, d->scratch);
+  minmax_stage2<<<1, RED_THREADS, 0, st>>>(d->scratch, d->state + ST_RES + 2);
   // first basis vector = x0 / |x0|
-  scale_copy<<<d->grid, 256, 0, st>>>(d->t, x0_dev, 1.0, d->n); su2::count_launch();
+  copy2<<<d->grid, 256, 0, st>>>(d->t, x0_dev, nullptr, nullptr, d->n);
+  su2::count_launch(3);
   d->k = 0;
   s = orthonormalise_into_basis(d, st);
   if (s != SU2_OK) { su2_davidson_destroy(d); return s; }
   *out = d;
+  return SU2_OK;
+}
+
+extern "C" su2_status su2_davidson_set_preconditioner(su2_davidson* d, int32_t mode) {
+  if (!d || mode < 0 || mode > 1) return SU2_ERR_INVALID_ARGUMENT;
+  d->precond_mode = mode;
   return SU2_OK;
 }
 
@@ -260,6 +394,9 @@ extern "C" su2_status su2_davidson_step(const su2_plan* plan, su2_davidson* d, v
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int k = d->k, mm = d->mmax;
   const int64_t n = d->n;
+  double* G = d->state + ST_G;
+  double* y = d->state + ST_Y;
+  double* res = d->state + ST_RES;
   // 1. w = H_eff v for the newest basis vector
   su2_status s = su2_heff_apply(plan, d->V + (int64_t)(k - 1) * n, d->W + (int64_t)(k - 1) * n, workspace_dev, cuda_stream);
   if (s != SU2_OK) return s;
@@ -269,56 +406,49 @@ extern "C" su2_status su2_davidson_step(const su2_plan* plan, su2_davidson* d, v
     s = d->reduce(d->W + (int64_t)(k - 1) * n, n, cuda_stream, d->reduce_user);
     if (s != SU2_OK) return s;
   }
-  // 2. new column of the projected matrix G = V^T H V
-  std::vector<double> col(k);
-  s = dots(d, d->V, k, d->W + (int64_t)(k - 1) * n, col.data(), st);
-  if (s != SU2_OK) return s;
-  for (int i = 0; i < k; ++i) d->G[(size_t)i * mm + (k - 1)] = d->G[(size_t)(k - 1) * mm + i] = col[i];
-  // 3. Rayleigh-Ritz in the k-dimensional subspace (host, Jacobi)
-  std::vector<double> a((size_t)k * k), v, w;
-  for (int i = 0; i < k; ++i)
-    for (int j = 0; j < k; ++j) a[(size_t)i * k + j] = d->G[(size_t)i * mm + j];
-  jacobi_eigh(k, a, v, w);
-  int lo = 0;
-  for (int i = 1; i < k; ++i)
-    if (w[i] < w[lo]) lo = i;
-  const double theta = w[lo];
-  Coefs c{};
-  d->y.assign(k, 0.0);
-  for (int i = 0; i < k; ++i) c.c[i] = d->y[i] = v[(size_t)i * k + lo];
-  // 4. residual r = sum_i y_i (W_i - theta V_i)
-  lincomb<<<d->grid, 256, 0, st>>>(d->r, d->W, d->V, n, k, c, theta, n); su2::count_launch();
-  double rr = 0.0;
-  s = dots(d, d->r, 1, d->r, &rr, st);
-  if (s != SU2_OK) return s;
-  *theta_out = theta;
-  *resnorm_out = std::sqrt(rr);
-  // 5. preconditioned direction
-  precondition<<<d->grid, 256, 0, st>>>(d->t, d->r, d->diag, theta, d->diag_floor, n); su2::count_launch();
+  // 2. new row and column of the projected matrix G = V^T H V (device)
+  dot_stage1<<<dim3(RED_BLOCKS, k), RED_THREADS, 0, st>>>(d->V, n, d->W + (int64_t)(k - 1) * n, n, d->scratch);
+  dot_stage2<<<k, RED_THREADS, 0, st>>>(d->scratch, G + (k - 1), MAX_SUB, G + (int64_t)(k - 1) * MAX_SUB, 1);
+  // 3. Rayleigh-Ritz in the k-dimensional subspace (one CTA): y, theta
+  {
+    const int K = (k + 1) & ~1;
+    ritz_kernel<<<1, 256, 2 * K * (K + 1) * sizeof(double), st>>>(G, k, y, res);
+  }
+  d->ky = k;
+  // 4. residual r = sum_i y_i (W_i - theta V_i) and |r|^2
+  lincomb_dev<<<RED_BLOCKS, RED_THREADS, 0, st>>>(d->r, d->W, d->V, n, k, y, res, n, d->scratch);
+  dot_stage2<<<1, RED_THREADS, 0, st>>>(d->scratch, res + 1, 1, nullptr, 0);
+  // 5. new direction
+  precondition<<<d->grid, 256, 0, st>>>(d->t, d->r, d->diag, res, d->precond_mode, n);
+  su2::count_launch(6);
+  SU2_CUDA(cudaMemcpyAsync(d->h_result, res, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
   // 6. restart from the Ritz vector when the subspace is full: V <- {V y}, W <- {W y}, G <- {theta}
   if (k == mm) {
-    lincomb<<<d->grid, 256, 0, st>>>(d->r, d->V, nullptr, n, k, c, 0.0, n); su2::count_launch();
-    lincomb<<<d->grid, 256, 0, st>>>(d->u, d->W, nullptr, n, k, c, 0.0, n); su2::count_launch();
-    scale_copy<<<d->grid, 256, 0, st>>>(d->V, d->r, 1.0, n); su2::count_launch();
-    scale_copy<<<d->grid, 256, 0, st>>>(d->W, d->u, 1.0, n); su2::count_launch();
+    lincomb_dev<<<RED_BLOCKS, RED_THREADS, 0, st>>>(d->r, d->V, nullptr, n, k, y, res, n, nullptr);
+    lincomb_dev<<<RED_BLOCKS, RED_THREADS, 0, st>>>(d->u, d->W, nullptr, n, k, y, res, n, nullptr);
+    copy2<<<d->grid, 256, 0, st>>>(d->V, d->r, d->W, d->u, n);
+    restart_state<<<(MAX_SUB * MAX_SUB + 255) / 256, 256, 0, st>>>(d->state);
+    su2::count_launch(4);
     SU2_CUDA(cudaGetLastError());
-    std::fill(d->G.begin(), d->G.end(), 0.0);
-    d->G[0] = theta;
     d->k = 1;
-    d->y.assign(1, 1.0);
+    d->ky = 1;
   }
   // 7. orthonormalise and append
   s = orthonormalise_into_basis(d, st);
   if (s != SU2_OK) return s;
   SU2_CUDA(cudaGetLastError());
+  // the step's only synchronisation: the two scalars handed back
+  SU2_CUDA(cudaStreamSynchronize(st));
+  *theta_out = d->h_result[0];
+  *resnorm_out = std::sqrt(std::fmax(d->h_result[1], 0.0));
   return SU2_OK;
 }
 
 extern "C" su2_status su2_davidson_ritz_vector(const su2_davidson* d, double* x_dev, void* cuda_stream) {
-  if (!d || !x_dev || d->y.empty()) return SU2_ERR_INVALID_ARGUMENT;
-  Coefs c{};
-  for (size_t i = 0; i < d->y.size(); ++i) c.c[i] = d->y[i];
-  lincomb<<<d->grid, 256, 0, (cudaStream_t)cuda_stream>>>(x_dev, d->V, nullptr, d->n, (int)d->y.size(), c, 0.0, d->n); su2::count_launch();
+  if (!d || !x_dev || d->ky < 1) return SU2_ERR_INVALID_ARGUMENT;
+  lincomb_dev<<<RED_BLOCKS, RED_THREADS, 0, (cudaStream_t)cuda_stream>>>(x_dev, d->V, nullptr, d->n, d->ky, d->state + ST_Y,
+                                                                         d->state + ST_RES, d->n, nullptr);
+  su2::count_launch();
   SU2_CUDA(cudaGetLastError());
   return SU2_OK;
 }

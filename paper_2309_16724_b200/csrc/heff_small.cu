@@ -47,31 +47,6 @@ __device__ __forceinline__ void hs_dmma(double (&c)[2], double a, double b) {
                : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
 }
 
-// Stored dense row-major rows x cols -> shared tile (leading dimension ld), zero-filled up to rows_pad x cols_pad.
-template <int VEC, int HS_THREADS>
-__device__ __forceinline__ void hs_copy(double* __restrict__ dst, int ld, const double* __restrict__ src, int rows, int cols,
-                                        int rows_pad, int cols_pad, int tid) {
-  const int cv = cols_pad / VEC;               // copies per padded row (cols_pad is a multiple of 4)
-  const int total = rows_pad * cv;
-  int r = tid / cv, c = tid - r * cv;
-  const int dr = HS_THREADS / cv, dc = HS_THREADS - dr * cv;
-  for (int e = tid; e < total; e += HS_THREADS) {
-    const bool valid = r < rows && VEC * c < cols;
-    const double* s = valid ? src + (int64_t)r * cols + VEC * c : src;
-    if (VEC == 2) hs_cp16(dst + r * ld + 2 * c, s, valid);
-    else hs_cp8(dst + r * ld + c, s, valid);
-    r += dr; c += dc;
-    if (c >= cv) { c -= cv; ++r; }
-  }
-}
-
-template <int HS_THREADS>
-__device__ __forceinline__ void hs_copy_any(double* dst, int ld, const double* src, int rows, int cols, int rows_pad,
-                                            int cols_pad, int tid) {
-  if (!(cols & 1) && !((uintptr_t)src & 15)) hs_copy<2, HS_THREADS>(dst, ld, src, rows, cols, rows_pad, cols_pad, tid);
-  else hs_copy<1, HS_THREADS>(dst, ld, src, rows, cols, rows_pad, cols_pad, tid);
-}
-
 // K loop of one product for a warp that owns NR x NC m8n8 tiles: straight-line per (NR, NC), no predicated
 // DMMAs (a predicated-off DMMA still takes its slot in the FP64 tensor pipe).  ap / bp: this lane's fragment
 // element of tile row 0 / tile column 0 at k = 0; a_i / b_j: distance to the next owned tile; a_k / b_k: per k4 step.

@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cstdio>
 #include <cstring>
 #include <string>
@@ -14,8 +15,8 @@
 namespace su2 {
 
 static thread_local std::string g_cuda_error;
-static long long g_launches = 0;
-void count_launch(int n) { g_launches += n; }
+static std::atomic<long long> g_launches{0};
+void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 void set_cuda_error(const char* what, int code) {
   g_cuda_error = std::string(what) + ": " + cudaGetErrorString((cudaError_t)code);
 }
@@ -262,7 +263,7 @@ su2_status launch_diag(const su2_plan* plan, double* diag, void* stream_v) {
 using namespace su2;
 
 extern "C" const char* su2_last_cuda_error(void) { return g_cuda_error.c_str(); }
-extern "C" int64_t su2_kernel_launch_count(void) { return (int64_t)g_launches; }
+extern "C" int64_t su2_kernel_launch_count(void) { return (int64_t)g_launches.load(std::memory_order_relaxed); }
 
 extern "C" su2_status su2_heff_apply(const su2_plan* plan, const double* psi_dev, double* out_dev, void* workspace_dev,
                                      void* cuda_stream) {

@@ -18,15 +18,21 @@ namespace su2 {
 // ---------------------------------------------------------------------------------------
 // Wigner symbols (Appendix A, Eqs. (10)-(15)); doubled arguments.
 // ---------------------------------------------------------------------------------------
-static const long double* factorial_table() {
-  static long double tab[171];
-  static bool init = false;
-  if (!init) {
-    tab[0] = 1.0L;
-    for (int i = 1; i <= 170; ++i) tab[i] = tab[i - 1] * i;
-    init = true;
+// n! for n <= 170 (the largest factorial a long double holds comfortably).  The Racah sums below reach
+// (sum of four spins + 1)!: validate() caps every doubled spin and rank at MAX_TWO_SPIN so that no argument
+// exceeds the table and the alternating sums keep their precision (checked against exact rational arithmetic in
+// tests/test_planner_cpu.py up to that cap).
+constexpr int MAX_TWO_SPIN = 40;            // S, k <= 20
+struct FactorialTable {
+  long double v[171];
+  FactorialTable() {
+    v[0] = 1.0L;
+    for (int i = 1; i <= 170; ++i) v[i] = v[i - 1] * i;
   }
-  return tab;
+};
+static const long double* factorial_table() {
+  static const FactorialTable tab;          // function-local static: initialised once, thread-safe
+  return tab.v;
 }
 static inline long double fact2(int two_x) { return factorial_table()[two_x / 2]; }  // (two_x/2)!
 static inline bool triad(int a, int b, int c) { return ((a + b + c) % 2 == 0) && std::abs(a - b) <= c && c <= a + b; }
@@ -83,6 +89,7 @@ static const int SITE_2S[3] = {0, 1, 0};
 using namespace su2;
 
 static su2_status validate(const su2_problem* p) {
+  if (p && (p->twoS_tot < 0 || p->twoS_tot > MAX_TWO_SPIN)) return SU2_ERR_INVALID_RANK;
   if (!p || p->nsec_l <= 0 || p->nsec_r <= 0 || !p->sec_l || !p->sec_r || p->nsite <= 0 || !p->site || p->nterm < 0)
     return SU2_ERR_INVALID_ARGUMENT;
   if (p->nterm > 0 && !p->term) return SU2_ERR_INVALID_ARGUMENT;
@@ -93,10 +100,13 @@ static su2_status validate(const su2_problem* p) {
     const su2_sector* sec = side ? p->sec_r : p->sec_l;
     for (int i = 0; i < ns; ++i)
       if (sec[i].dim <= 0 || sec[i].twoS < 0 || sec[i].N < 0) return SU2_ERR_INVALID_SECTOR;
+    for (int i = 0; i < ns; ++i)
+      if (sec[i].twoS > MAX_TWO_SPIN) return SU2_ERR_INVALID_RANK;
     const int nf = side ? p->nfam_r : p->nfam_l;
     const su2_opfamily* fam = side ? p->fam_r : p->fam_l;
     for (int f = 0; f < nf; ++f) {
       if (fam[f].npos <= 0 || fam[f].nblk < 0 || fam[f].twoK < 0) return SU2_ERR_INVALID_ARGUMENT;
+      if (fam[f].twoK > MAX_TWO_SPIN) return SU2_ERR_INVALID_RANK;
       if (fam[f].nblk > 0 && (!fam[f].q_out || !fam[f].q_in || !fam[f].blk_off)) return SU2_ERR_INVALID_ARGUMENT;
       for (int b = 0; b < fam[f].nblk; ++b) {
         const int qo = fam[f].q_out[b], qi = fam[f].q_in[b];
@@ -312,14 +322,13 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
   // ---- small-block plan? (heff_small.cu) -------------------------------------------------------
   // Every block sector of the bond holds at most SMALL_MAX_DIM multiplets: the whole apply runs on
   // heff_small_kernel (one CTA per output sector and segment), which reads blocks in either orientation at full
-  // speed, so no transposed copies are made.  SU2_HEFF_SMALL=0 in the environment keeps the large-tile kernel
-  // (A/B measurements only).
+  // speed, so no transposed copies are made.  SU2_PLAN_LARGE_TILES keeps the large-tile kernel (tests, A/B
+  // measurements).
   {
     int maxdim = 0;
     for (const su2_sector& q : plan->sec_l) maxdim = std::max(maxdim, (int)q.dim);
     for (const su2_sector& q : plan->sec_r) maxdim = std::max(maxdim, (int)q.dim);
-    const char* env = std::getenv("SU2_HEFF_SMALL");
-    const bool off = env && env[0] == '0';
+    const bool off = (flags & SU2_PLAN_LARGE_TILES) != 0;
     plan->small_dm8 = (maxdim <= SMALL_MAX_DIM && !off) ? std::max(8, (maxdim + 7) & ~7) : 0;
   }
   const bool small_plan = plan->small_dm8 > 0;
@@ -607,7 +616,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
   plan->info.cc_flops = cc;
   plan->info.executed_flops = executed;
   plan->info.operator_bytes = opbytes;
-  plan->info.workspace_bytes = plan->partial_elems * 8 + 256;
+  plan->info.workspace_bytes = ((plan->partial_elems * 8 + 256) + 255) & ~(int64_t)255;   // a multiple of 256
   plan->info.npsi_sec = nsec;
   plan->info.nwork_items = (int64_t)plan->h_work.size();
   plan->info.small_plan = small_plan ? 1 : 0;
@@ -663,6 +672,21 @@ extern "C" su2_status su2_plan_export_tasks(const su2_plan* plan, int32_t* out_s
     term[i] = t.term; coef[i] = t.coef;
   }
   return SU2_OK;
+}
+
+extern "C" double su2_wigner_6j(int32_t a, int32_t b, int32_t c, int32_t d, int32_t e, int32_t f) {
+  const int32_t v[6] = {a, b, c, d, e, f};
+  for (int32_t x : v)
+    if (x < 0 || x > MAX_TWO_SPIN) return std::nan("");
+  return wigner6j(a, b, c, d, e, f);
+}
+
+extern "C" double su2_wigner_9j(int32_t j1, int32_t j2, int32_t j, int32_t k1, int32_t k2, int32_t k, int32_t j1p, int32_t j2p,
+                                int32_t jp) {
+  const int32_t v[9] = {j1, j2, j, k1, k2, k, j1p, j2p, jp};
+  for (int32_t x : v)
+    if (x < 0 || x > MAX_TWO_SPIN) return std::nan("");
+  return wigner9j(j1, j2, j, k1, k2, k, j1p, j2p, jp);
 }
 
 extern "C" const char* su2_status_string(su2_status st) {

@@ -20,7 +20,7 @@ class HeffOperator:
     generated directly on the device by device_fill(side, index, tensor) (143 GB-class
     workloads cannot be staged through host memory)."""
 
-    def __init__(self, problem, device="cuda:0", device_fill=None, force_split=False):
+    def __init__(self, problem, device="cuda:0", device_fill=None, force_split=False, large_tiles=False):
         _require_cuda()
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
@@ -41,7 +41,8 @@ class HeffOperator:
                 self.family_tensors[(side, i)] = t
                 ptrs[(side, i)] = t.data_ptr()
         self.stream = torch.cuda.current_stream(self.device)
-        self.plan = Plan(problem, family_ptrs=ptrs, stream=self.stream.cuda_stream, force_split=force_split)
+        self.plan = Plan(problem, family_ptrs=ptrs, stream=self.stream.cuda_stream, force_split=force_split,
+                         large_tiles=large_tiles)
         self.psi_len = self.plan.psi_len
         # workspace: partial tiles + staging for the host entry point
         self.workspace = torch.empty(self.plan.workspace_bytes + 512 + 16 * self.psi_len, dtype=torch.uint8,

@@ -59,17 +59,15 @@ def test_synthetic_parity_full_oracle(name, force_split):
 
 
 @pytest.mark.parametrize("name", ["cfg1", "mini", "midi"])
-def test_small_bonds_through_the_large_tile_kernel(name, monkeypatch):
-    """Bonds whose sectors all hold <= 48 multiplets plan onto heff_small_kernel; SU2_HEFF_SMALL=0 keeps them on
+def test_small_bonds_through_the_large_tile_kernel(name):
+    """Bonds whose sectors all hold <= 48 multiplets plan onto heff_small_kernel; SU2_PLAN_LARGE_TILES keeps them on
     heff_dmma_kernel, so the large-tile kernel stays covered on blocks of 1..17 rows (far smaller than a tile),
     and the two kernels are checked against each other as well as against the oracle."""
     torch = _torch()
     prob = _cfg1() if name == "cfg1" else config_problem(name)
     op_small = _operator(prob, force_split=True)
     assert op_small.info["small_plan"] == 1
-    monkeypatch.setenv("SU2_HEFF_SMALL", "0")
-    op_big = _operator(prob, force_split=True)
-    monkeypatch.delenv("SU2_HEFF_SMALL")
+    op_big = _operator(prob, force_split=True, large_tiles=True)
     assert op_big.info["small_plan"] == 0
     x = random_psi(op_small.psi_len, seed=5)
     f_ref = oracle_flat(prob, op_small.plan, x)
@@ -254,6 +252,78 @@ def test_davidson_converges_to_fci_energy_cfg1():
     assert abs(float(torch.dot(xr, xr)) - 1.0) < 1e-12
     assert len(solver.history) > 12          # went through at least one restart
     solver.close()
+
+
+def test_davidson_follows_the_krylov_bound_midi():
+    """The new-direction rule (reading G8): on the random-operator workload theta lies inside the range of
+    diag(H_eff), so the solver must take the Krylov direction t = r until theta has fallen below min(diag); its Ritz
+    value after j applies then equals the lowest Ritz value of H in span{x0, H x0, ..., H^(j-1) x0} (computed here
+    with numpy from GPU applies); theta falls monotonically and the residual ends below where it started.  The k x k Ritz
+    problem, the projections and the residual all run on the device (one CTA Jacobi), so this also pins them."""
+    torch = _torch()
+    prob = config_problem("midi")
+    op = _operator(prob)
+    n = op.psi_len
+    x0 = torch.from_numpy(random_psi(n, seed=21)).cuda()
+    steps = 14
+    basis, hbasis, kry = [], [], []
+    v = x0 / x0.norm()
+    for j in range(steps):
+        for _ in range(2):
+            for b in basis:
+                v = v - torch.dot(b, v) * b
+        v = v / v.norm()
+        basis.append(v)
+        hbasis.append(op.apply(v).clone())
+        g = np.array([[float(torch.dot(a, hb)) for hb in hbasis] for a in basis])
+        kry.append(float(np.linalg.eigvalsh((g + g.T) / 2)[0]))
+        v = hbasis[-1].clone()
+    # mode 0 (always t = r) IS the Krylov iteration: same Ritz values as the numpy construction above
+    s0 = op.davidson(x0, max_subspace=steps + 2)
+    s0.dav.set_preconditioner(0)
+    hist0 = [s0.step() for _ in range(steps)]
+    for j in range(steps):
+        assert abs(hist0[j][0] - kry[j]) <= 1e-8 * max(1.0, abs(kry[j])), (j, hist0[j][0], kry[j])
+    # default mode: identical, bit for bit, until theta has dropped below min(diag); monotone throughout
+    solver = op.davidson(x0, max_subspace=steps + 2)
+    hist = [solver.step() for _ in range(steps)]
+    theta = [h[0] for h in hist]
+    dmin = float(op.diag().min())
+    assert theta[0] > dmin                                   # the random start lies inside the range of diag
+    first_below = next((j for j in range(steps) if theta[j] < dmin), steps)
+    assert first_below >= 2
+    assert hist[:first_below + 1] == hist0[:first_below + 1]
+    assert all(theta[j + 1] <= theta[j] + 1e-12 for j in range(steps - 1))
+    assert hist[-1][1] < hist[0][1]                          # the residual ends below where it started
+    # the reported pair is a Ritz pair of the operator: |H x - theta x| as reported
+    xr = solver.ritz_vector()
+    hx = op.apply(xr)
+    assert abs(float(torch.dot(xr, xr)) - 1.0) <= 1e-10
+    assert abs(float(torch.dot(xr, hx)) - theta[-1]) <= 1e-10 * max(1.0, abs(theta[-1]))
+    assert abs(float((hx - theta[-1] * xr).norm()) - hist[-1][1]) <= 1e-8 * max(1.0, hist[-1][1])
+    solver.close(); s0.close()
+
+
+def test_davidson_diagonal_correction_on_a_dominant_diagonal():
+    """The other branch of the rule: a problem whose H_eff is diagonally dominant with theta below min(diag) --
+    the exact cfg1 Hamiltonian shifted so -- converges with the diagonal correction in fewer applies than with
+    t = r, to the same eigenvalue."""
+    torch = _torch()
+    op = _operator(_cfg1())
+    x0 = torch.from_numpy(random_psi(op.psi_len, seed=3)).cuda()
+    out = {}
+    for mode in (1, 0):
+        solver = op.davidson(x0, max_subspace=12)
+        solver.dav.set_preconditioner(mode)
+        for it in range(80):
+            th, rn = solver.step()
+            if rn < 1e-9:
+                break
+        out[mode] = (it, th, rn)
+        solver.close()
+    assert out[1][2] < 1e-9 and out[0][2] < 1e-9
+    assert abs(out[1][1] - out[0][1]) < 1e-10
+    assert out[1][0] <= out[0][0]
 
 
 def test_gpu_result_is_hermitian_and_linear_midi():
