@@ -27,10 +27,11 @@
  * Ownership: the caller owns every device buffer and the CUDA stream.  Host arrays handed to
  * su2_plan_create are copied and may be freed afterwards; operator-family `data` pointers are
  * DEVICE pointers that must stay valid and unchanged while the plan is used.  The library
- * allocates on the device only what belongs to the plan (freed by su2_plan_destroy): its task
- * tables, the position-folded operators of one-sided rows (sum_pos alpha_pos A_pos, formed once per
- * plan) and, if they fit, transposed copies of the right-block families used by position-batched
- * rows (su2_plan_info_t.plan_device_bytes; +50 % of the right-block operator bytes).
+ * allocates on the device only what belongs to the plan (freed by su2_plan_destroy): its task tables and tensor
+ * maps, the position-folded operators of one-sided rows (sum_pos alpha_pos A_pos, formed once per plan), a padded
+ * copy of Psi refreshed by every apply (the large-tile kernel loads its tiles with bulk-tensor copies, which need
+ * 16-byte aligned rows) and, only for operator families whose stored layout is not 16-byte aligned, a padded copy
+ * of the family (su2_plan_info_t.padded_copy_bytes; see su2_opfamily.blk_ld).
  * Errors: every entry point returns 0 on success and a negative su2_status otherwise; no
  * exceptions, no aborts, no partial state.  Results are bit-reproducible for a fixed plan.
  */
@@ -140,11 +141,12 @@ typedef struct {
   int32_t nsegments;         /* work segments (deterministic segmented reduction)               */
   int64_t nwork_items;       /* CTA-level work items per apply                                  */
   double plan_seconds;       /* host time spent in su2_plan_create                              */
-  int64_t plan_device_bytes; /* device memory owned by the plan (tables, folded and transposed operators) */
+  int64_t plan_device_bytes; /* device memory owned by the plan (tables, tensor maps, folded operators, padded copies) */
   int32_t small_plan;        /* 1: every block sector holds <= 48 multiplets, su2_heff_apply runs the small-block
                                 kernel (one CTA per output sector and segment); 0: large register tiles
                                 (always 0 under SU2_PLAN_LARGE_TILES) */
   int32_t reserved;
+  int64_t padded_copy_bytes; /* part of plan_device_bytes: padded copies of families that could not be read in place */
 } su2_plan_info_t;
 
 /* Build the plan: enumerate the sector tasks (Eq. (3)), compute the coefficient of each
@@ -217,14 +219,20 @@ su2_status su2_davidson_destroy(su2_davidson* dav);
  * C_b (m x p) += alpha * A_b (m x k) * X_b (k x n) * B_b^T (n x p) for b < batch, all DEVICE,
  * row-major, dense strides (A_b = A + b*m*k, ...); the paper's strided-batched GEMM sequences
  * with T = A_b X_b kept on chip.  Items whose operands fit one SM's shared memory run one CTA per item on FP64
- * tensor instructions (HBM-bound regime); larger items with >= 64 x 64 outputs use the fused kernel of the apply;
- * anything else an FP64-FMA tile routine.  C_b blocks must not overlap; one CTA owns an output
- * element, so results are bit-reproducible.  Errors: non-positive dimension, negative batch or null pointer ->
- * SU2_ERR_INVALID_ARGUMENT; batch == 0 is a no-op.  SU2_GEMM_PAIR_SMALL="wpi,nbuf" ("0": off) in the environment
- * overrides the small-item kernel's warps per item and input buffering (tuning aid). */
+ * tensor instructions (HBM-bound regime); all other items whose rows are 16-byte aligned (even k and n, 16-byte
+ * aligned A, X, B) use the fused kernel of the apply (three rank-3 tensor maps {columns, rows, batch} describe the
+ * whole call); only odd-k / odd-n items too large for shared memory fall to an FP64-FMA tile routine.  C_b blocks
+ * must not overlap; one CTA owns an output element, so results are bit-reproducible.  Errors:
+ * non-positive dimension, negative batch or null pointer -> SU2_ERR_INVALID_ARGUMENT; batch == 0 is a no-op. */
 su2_status su2_gemm_pair_batched(int32_t m, int32_t k, int32_t n, int32_t p, int64_t batch, double alpha,
                                  const double* A, const double* X, const double* B, double* C,
                                  void* cuda_stream);
+/* The same with the kernel chosen by the caller (tests, tuning): route 0 automatic, 1 small-block kernel, 2 fused
+ * large-tile kernel, 3 FP64-FMA tile routine; SU2_ERR_INVALID_ARGUMENT if the shape does not fit the route.  wpi /
+ * nbuf (0 = heuristics) override the small-block kernel's warps per item and input buffering. */
+su2_status su2_gemm_pair_batched_route(int32_t m, int32_t k, int32_t n, int32_t p, int64_t batch, double alpha,
+                                       const double* A, const double* X, const double* B, double* C,
+                                       void* cuda_stream, int32_t route, int32_t wpi, int32_t nbuf);
 
 /* Measurement aid, not on the hot path: register-resident FP64 throughput of the current device
  * in TFLOP/s (best of 3 timed launches, CUDA events on cuda_stream; synchronises).

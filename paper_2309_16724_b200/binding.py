@@ -48,13 +48,13 @@ class su2_plan_info_t(C.Structure):
                 ("cc_flops", C.c_double), ("executed_flops", C.c_double), ("operator_bytes", C.c_double),
                 ("workspace_bytes", C.c_int64), ("npsi_sec", C.c_int32), ("nsegments", C.c_int32),
                 ("nwork_items", C.c_int64), ("plan_seconds", C.c_double), ("plan_device_bytes", C.c_int64),
-                ("small_plan", C.c_int32), ("reserved", C.c_int32)]
+                ("small_plan", C.c_int32), ("reserved", C.c_int32), ("padded_copy_bytes", C.c_int64)]
 
 
 EXPORTS = ["su2_wigner_6j", "su2_wigner_9j", "su2_status_string", "su2_last_cuda_error", "su2_kernel_launch_count", "su2_plan_create", "su2_plan_destroy", "su2_plan_info",
            "su2_plan_psi_layout", "su2_plan_export_tasks", "su2_heff_apply", "su2_heff_apply_host", "su2_heff_diag",
            "su2_davidson_workspace_bytes", "su2_davidson_create", "su2_davidson_create_sharded", "su2_davidson_step", "su2_davidson_set_preconditioner", "su2_davidson_ritz_vector",
-           "su2_davidson_destroy", "su2_gemm_pair_batched", "su2_probe_fp64_peak"]
+           "su2_davidson_destroy", "su2_gemm_pair_batched", "su2_gemm_pair_batched_route", "su2_probe_fp64_peak"]
 
 REDUCE_FN = C.CFUNCTYPE(C.c_int32, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p)   # su2_reduce_fn
 
@@ -101,6 +101,7 @@ def load():
     lib.su2_davidson_ritz_vector.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     lib.su2_davidson_destroy.argtypes = [C.c_void_p]
     lib.su2_gemm_pair_batched.argtypes = [C.c_int32] * 4 + [C.c_int64, C.c_double] + [C.c_void_p] * 5
+    lib.su2_gemm_pair_batched_route.argtypes = [C.c_int32] * 4 + [C.c_int64, C.c_double] + [C.c_void_p] * 5 + [C.c_int32] * 3
     lib.su2_probe_fp64_peak.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_double), C.c_void_p]
     _lib = lib
     return lib
@@ -119,28 +120,41 @@ def _i32(a):
     return np.ascontiguousarray(a, dtype=np.int32)
 
 
-def family_block_offsets(fam, secs):
-    """Element offset of each block inside the family's buffer: blocks in order, each
-    [npos][dim(q_out)][dim(q_in)] row-major."""
-    offs, cur = [], 0
+def family_layout(fam, secs, ld_align=1):
+    """Layout of a family's device buffer: block b = [npos][dim(q_out)][ld_b] row-major with ld_b = dim(q_in) rounded up
+    to a multiple of ld_align, blocks one after the other, every block starting on a multiple of 16 elements when
+    ld_align > 1.  Returns (offsets, lds, total_elements).  ld_align = 1 is the dense layout; ld_align = 4 puts every
+    row on a 32-byte boundary, which lets the large-tile kernel read the family in place (su2_heff.h)."""
+    offs, lds, cur = [], [], 0
     for qo, qi in zip(fam.q_out, fam.q_in):
         offs.append(cur)
         if 0 <= qo < len(secs) and 0 <= qi < len(secs):      # bad indices are rejected by su2_plan_create
-            cur += fam.npos * secs[qo].dim * secs[qi].dim
-    return offs
+            ld = -(-secs[qi].dim // ld_align) * ld_align
+            lds.append(ld)
+            cur += fam.npos * secs[qo].dim * ld
+            if ld_align > 1:
+                cur = -(-cur // 16) * 16
+        else:
+            lds.append(1)
+    return offs, lds, cur
+
+
+def family_block_offsets(fam, secs):
+    return family_layout(fam, secs)[0]
 
 
 def family_elems(fam, secs):
-    return sum(fam.npos * secs[qo].dim * secs[qi].dim for qo, qi in zip(fam.q_out, fam.q_in))
+    return family_layout(fam, secs)[2]
 
 
 class Plan:
     """su2_plan wrapper.  `problem` is a gen.problem.Problem-like object (plain data);
     `family_ptrs` maps ("l"|"r", family index) -> DEVICE base pointer (int) of the family's
-    blocks laid out block after block, each [npos][m][k] (see family_block_offsets); None
-    for a host-only plan (planner tests without a GPU)."""
+    blocks laid out as family_layout(fam, secs, ld_align) says; None for a host-only plan (planner tests
+    without a GPU)."""
 
-    def __init__(self, problem, family_ptrs=None, stream=0, host_only=False, force_split=False, large_tiles=False):
+    def __init__(self, problem, family_ptrs=None, stream=0, host_only=False, force_split=False, large_tiles=False,
+                 ld_align=1):
         lib = load()
         self._keep = []
         self.problem = problem
@@ -154,12 +168,14 @@ class Plan:
             arr = (su2_opfamily * max(len(fams), 1))()
             for i, f in enumerate(fams):
                 qo, qi = _i32(f.q_out), _i32(f.q_in)
-                off = np.asarray(family_block_offsets(f, secs), dtype=np.int64)
-                self._keep += [qo, qi, off]
+                offs, lds, _ = family_layout(f, secs, ld_align)
+                off, ld = np.asarray(offs, dtype=np.int64), _i32(lds)
+                self._keep += [qo, qi, off, ld]
                 ptr = None if family_ptrs is None else family_ptrs[(side, i)]
+                ldp = C.POINTER(C.c_int32)() if ld_align == 1 else ld.ctypes.data_as(C.POINTER(C.c_int32))
                 arr[i] = su2_opfamily(f.dN, f.twoK, f.npos, len(f.q_out),
                                       qo.ctypes.data_as(C.POINTER(C.c_int32)), qi.ctypes.data_as(C.POINTER(C.c_int32)),
-                                      off.ctypes.data_as(C.POINTER(C.c_int64)), C.POINTER(C.c_int32)(), ptr)
+                                      off.ctypes.data_as(C.POINTER(C.c_int64)), ldp, ptr)
             self._keep.append(arr)
             return arr
 
@@ -284,8 +300,12 @@ class Davidson:
             self.handle = C.c_void_p()
 
 
-def gemm_pair_batched(m, k, n, p, batch, alpha, a_ptr, x_ptr, b_ptr, c_ptr, stream=0):
-    check(load().su2_gemm_pair_batched(m, k, n, p, batch, alpha, a_ptr, x_ptr, b_ptr, c_ptr, stream))
+def gemm_pair_batched(m, k, n, p, batch, alpha, a_ptr, x_ptr, b_ptr, c_ptr, stream=0, route=0, wpi=0, nbuf=0):
+    """route 0: automatic; 1: small-block kernel; 2: fused large-tile kernel; 3: FP64-FMA tile routine."""
+    if route == 0 and wpi == 0 and nbuf == 0:
+        check(load().su2_gemm_pair_batched(m, k, n, p, batch, alpha, a_ptr, x_ptr, b_ptr, c_ptr, stream))
+    else:
+        check(load().su2_gemm_pair_batched_route(m, k, n, p, batch, alpha, a_ptr, x_ptr, b_ptr, c_ptr, stream, route, wpi, nbuf))
 
 
 def probe_fp64_peak(kind, iters=20000, ctas_per_sm=4, stream=0):

@@ -1,10 +1,11 @@
 // Strided-batched FP64 GEMM-pair microbenchmark entry (BASELINE.json configs[4]):
 //   C_b += alpha * A_b X_b B_b^T, one independent item per batch index.
-// Larger items with at least 64 x 64 outputs run on the fused DMMA kernel of the hot path (heff_dmma.cu): a small
-// kernel writes one task / unit / work-item record per batch item (and output tile) and the persistent
-// kernel consumes them with the accumulate flag.  Items whose operands fit an SM's shared memory are tried first
-// on the small-block kernel (gemm_pair_small.cu, whole items per CTA, many in flight per SM).  What is left
-// (e.g. 8 x 512 x 512 x 8) uses the FP64-FMA tile routine below.
+// Items whose operands fit an SM's shared memory run on the small-block kernel (gemm_pair_small.cu, whole items per
+// CTA, many in flight per SM).  Everything else whose rows are 16-byte aligned (even k and n) runs on the fused DMMA
+// kernel of the hot path (heff_tma.cu): A, X and B are rank-3 tensors {columns, rows, batch}, three tensor maps
+// describe the whole call, a small kernel writes one task / unit / work-item record per batch item (and output
+// tile), and the persistent kernel consumes them with the accumulate flag.  Only odd-k / odd-n items too large for
+// the small-block kernel fall to the FP64-FMA tile routine below.
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -54,7 +55,7 @@ __device__ __forceinline__ void accumulate_task(const DevTask& t, const double* 
           if (!ta) { i = e / KC; kk = e % KC; } else { kk = e / TILE_M; i = e % TILE_M; }
           const int r = row0 + i, c = k0 + kk;
           double v = 0.0;
-          if (r < t.m && c < t.k) v = ta ? A[(int64_t)c * t.m + r] : A[(int64_t)r * t.k + c];
+          if (r < t.m && c < t.k) v = ta ? A[(int64_t)c * t.ldA + r] : A[(int64_t)r * t.ldA + c];
           sm.As[i][kk] = v;
         }
         for (int e = tid; e < KC * NC; e += GP_THREADS) {
@@ -87,7 +88,7 @@ __device__ __forceinline__ void accumulate_task(const DevTask& t, const double* 
         if (!td) { c = e / NC; j = e % NC; } else { j = e / TILE_P; c = e % TILE_P; }
         const int r = col0 + c, q = n0 + j;
         double v = 0.0;
-        if (r < t.p && q < t.n) v = td ? D[(int64_t)q * t.p + r] : D[(int64_t)r * t.n + q];
+        if (r < t.p && q < t.n) v = td ? D[(int64_t)q * t.ldD + r] : D[(int64_t)r * t.ldD + q];
         sm.Ds[c][j] = v;
       }
       __syncthreads();
@@ -120,7 +121,7 @@ gemm_pair_kernel(int m, int k, int n, int p, int64_t batch, double alpha, const 
   for (int64_t b = blockIdx.y; b < batch; b += gridDim.y) {
     DevTask t;
     t.A = A + b * (int64_t)m * k; t.D = B + b * (int64_t)p * n; t.alpha = nullptr; t.coef = alpha; t.e_off = 0;
-    t.m = m; t.k = k; t.n = n; t.p = p; t.strideA = 0; t.strideD = 0; t.npos = 1; t.flags = 0;
+    t.m = m; t.k = k; t.n = n; t.p = p; t.strideA = 0; t.strideD = 0; t.ldA = k; t.ldD = n; t.npos = 1; t.flags = 0;
     double acc[4][4];
 #pragma unroll
     for (int i = 0; i < 4; ++i)
@@ -139,18 +140,20 @@ gemm_pair_kernel(int m, int k, int n, int p, int64_t batch, double alpha, const 
 }
 
 
-// one task, one unit and ntile work items per batch index
-__global__ void gemm_pair_tables_kernel(int m, int k, int n, int p, int64_t batch, double alpha, const double* A,
-                                        const double* B, int wr, int tm, int tp, DevTask* tasks, DevUnit* units,
-                                        DevWork* work, int* counter) {
+// one task, one unit and ntile work items per batch index; the batch index is the item coordinate of the three
+// tensor maps (A, X, B are rank-3 tensors {columns, rows, batch})
+__global__ void gemm_pair_tables_kernel(int m, int k, int n, int p, int64_t batch, double alpha, int wr, int tm, int tp,
+                                        DevTask* tasks, DevUnit* units, DevWork* work, int* counter) {
   const int tr = (m + tm - 1) / tm, tc = (p + tp - 1) / tp;
   if (blockIdx.x == 0 && threadIdx.x == 0) *counter = 0;
   for (int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; b < batch; b += (int64_t)gridDim.x * blockDim.x) {
     DevTask t;
-    t.A = A + b * (int64_t)m * k; t.D = B + b * (int64_t)p * n; t.alpha = nullptr; t.coef = alpha;
-    t.e_off = b * (int64_t)k * n; t.m = m; t.k = k; t.n = n; t.p = p; t.strideA = 0; t.strideD = 0; t.npos = 1; t.flags = 0;
+    t.A = nullptr; t.D = nullptr; t.alpha = nullptr; t.coef = alpha;
+    t.e_off = b * (int64_t)k * n; t.m = m; t.k = k; t.n = n; t.p = p;
+    t.strideA = m * k; t.strideD = p * n; t.ldA = k; t.ldD = n; t.npos = 1; t.flags = 0;
+    t.mapA = 0; t.mapD = 1; t.mapE = 2; t.e_item = (int32_t)b;
     tasks[b] = t;
-    units[b] = DevUnit{(int32_t)b, 0, 1, 0};
+    units[b] = DevUnit{(int32_t)b, (int32_t)b, (int32_t)b + 1, 0};     // "position" b = the item coordinate of A and B
     for (int i = 0; i < tr * tc; ++i) {
       DevWork w;
       w.dst_off = b * (int64_t)m * p; w.unit0 = (int32_t)b; w.unit1 = (int32_t)b + 1;
@@ -161,50 +164,69 @@ __global__ void gemm_pair_tables_kernel(int m, int k, int n, int p, int64_t batc
 }
 
 su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double alpha, const double* A, const double* X,
-                            const double* B, double* C, void* stream_v) {
+                            const double* B, double* C, void* stream_v, int route, int wpi, int nbuf) {
   if (batch == 0) return SU2_OK;
   cudaStream_t stream = (cudaStream_t)stream_v;
-  {
+  if (route == 0 || route == 1) {
     // items whose operands fit one SM's shared memory (all dims <= 80 for square shapes): one CTA of 1-16 warps per
-    // item, shared memory sized by the item shape (gemm_pair_small.cu).
-    // SU2_GEMM_PAIR_SMALL="wpi,nbuf" overrides the heuristics (tuning aid; "0" disables the kernel).
-    int wpi = 0, nbuf = 0;
-    bool off = false;
-    if (const char* env = std::getenv("SU2_GEMM_PAIR_SMALL")) {
-      if (std::sscanf(env, "%d,%d", &wpi, &nbuf) >= 1 && wpi == 0) off = true;
-    }
-    if (!off) {
-      su2_status st = launch_gemm_pair_small(m, k, n, p, batch, alpha, A, X, B, C, stream_v, wpi, nbuf);
-      if (st != 1) return st;
-    }
+    // item, shared memory sized by the item shape (gemm_pair_small.cu)
+    su2_status st = launch_gemm_pair_small(m, k, n, p, batch, alpha, A, X, B, C, stream_v, wpi, nbuf);
+    if (st != 1) return st;
+    if (route == 1) return SU2_ERR_INVALID_ARGUMENT;
   }
-  if (m >= 64 && p >= 64 && batch < (int64_t)1 << 24) {
-    // smallest tile class whose width covers p (no recomputation of the first product), like the planner
-    const int wr = p <= 144 ? 4 : (p <= 288 ? 2 : 1);
+  // anything else whose rows are 16-byte aligned runs on the fused kernel of the apply (heff_tma.cu): the three
+  // operands are rank-3 tensors {columns, rows, batch}, so three tensor maps describe the whole call
+  const bool aligned = !(k & 1) && !(n & 1) && !((uintptr_t)A & 15) && !((uintptr_t)X & 15) && !((uintptr_t)B & 15);
+  const int64_t max_items = (int64_t)1 << 24;
+  if ((route == 0 || route == 2) && aligned && batch < max_items) {
+    // tile class with the lowest modelled cost, like the planner
+    int wr = 1;
+    double best = -1.0;
+    for (int cand : {1, 2, 4}) {
+      const TileShape ts = tile_shape(cand);
+      double c = 0.0;
+      for (int r0 = 0; r0 < m; r0 += ts.tm)
+        for (int c0 = 0; c0 < p; c0 += ts.tp) c += tile_pos_cost(cand, std::min(ts.tm, m - r0), std::min(ts.tp, p - c0), k, n);
+      if (best < 0.0 || c < best) { best = c; wr = cand; }
+    }
     const TileShape ts = tile_shape(wr);
     const int64_t ntile = (int64_t)((m + ts.tm - 1) / ts.tm) * ((p + ts.tp - 1) / ts.tp);
-    const size_t b_task = ((size_t)batch * sizeof(DevTask) + 255) & ~(size_t)255;
-    const size_t b_unit = ((size_t)batch * sizeof(DevUnit) + 255) & ~(size_t)255;
-    const size_t b_work = ((size_t)(batch * ntile) * sizeof(DevWork) + 255) & ~(size_t)255;
-    char* buf = nullptr;
-    cudaError_t e = cudaMallocAsync((void**)&buf, b_task + b_unit + b_work + 256, stream);
-    if (e != cudaSuccess) { set_cuda_error("cudaMallocAsync(gemm_pair tables)", (int)e); return SU2_ERR_CUDA; }
-    DevTask* tasks = (DevTask*)buf;
-    DevUnit* units = (DevUnit*)(buf + b_task);
-    DevWork* work = (DevWork*)(buf + b_task + b_unit);
-    int* counter = (int*)(buf + b_task + b_unit + b_work);
-    gemm_pair_tables_kernel<<<(unsigned)std::min<int64_t>((batch + 127) / 128, 1024), 128, 0, stream>>>(
-        m, k, n, p, batch, alpha, A, B, wr, ts.tm, ts.tp, tasks, units, work, counter);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) { set_cuda_error("gemm_pair_tables_kernel launch", (int)e); return SU2_ERR_CUDA; }
-    count_launch();
-    int dev = 0, sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    su2_status st = launch_heff_dmma_tables(work, (int)(batch * ntile), units, tasks, X, C, nullptr, counter, sms, stream_v);
-    cudaFreeAsync(buf, stream);
-    return st;
+    if (batch * ntile < ((int64_t)1 << 31)) {
+      alignas(128) unsigned char h_maps[3 * 128];
+      const int nb = (int)batch;
+      su2_status st;
+      if ((st = encode_tensor_map(h_maps, MapKey{A, m, k, k, nb, (int64_t)m * k, KS1, ts.tm})) != SU2_OK) return st;
+      if ((st = encode_tensor_map(h_maps + 128, MapKey{B, p, n, n, nb, (int64_t)p * n, KS2, DBOX_C})) != SU2_OK) return st;
+      if ((st = encode_tensor_map(h_maps + 256, MapKey{X, k, n, n, nb, (int64_t)k * n, EBOX_LD, KS1})) != SU2_OK) return st;
+      const size_t b_maps = 512;
+      const size_t b_task = ((size_t)batch * sizeof(DevTask) + 255) & ~(size_t)255;
+      const size_t b_unit = ((size_t)batch * sizeof(DevUnit) + 255) & ~(size_t)255;
+      const size_t b_work = ((size_t)(batch * ntile) * sizeof(DevWork) + 255) & ~(size_t)255;
+      char* buf = nullptr;
+      cudaError_t e = cudaMallocAsync((void**)&buf, b_maps + b_task + b_unit + b_work + 256, stream);
+      if (e != cudaSuccess) { set_cuda_error("cudaMallocAsync(gemm_pair tables)", (int)e); return SU2_ERR_CUDA; }
+      DevTask* tasks = (DevTask*)(buf + b_maps);
+      DevUnit* units = (DevUnit*)(buf + b_maps + b_task);
+      DevWork* work = (DevWork*)(buf + b_maps + b_task + b_unit);
+      int* counter = (int*)(buf + b_maps + b_task + b_unit + b_work);
+      // pageable source: the runtime stages the 384 bytes before the call returns
+      e = cudaMemcpyAsync(buf, h_maps, sizeof(h_maps), cudaMemcpyHostToDevice, stream);
+      if (e != cudaSuccess) { set_cuda_error("cudaMemcpyAsync(gemm_pair tensor maps)", (int)e); cudaFreeAsync(buf, stream); return SU2_ERR_CUDA; }
+      gemm_pair_tables_kernel<<<(unsigned)std::min<int64_t>((batch + 127) / 128, 1024), 128, 0, stream>>>(
+          m, k, n, p, batch, alpha, wr, ts.tm, ts.tp, tasks, units, work, counter);
+      e = cudaGetLastError();
+      if (e != cudaSuccess) { set_cuda_error("gemm_pair_tables_kernel launch", (int)e); cudaFreeAsync(buf, stream); return SU2_ERR_CUDA; }
+      count_launch();
+      int dev = 0, sms = 148;
+      cudaGetDevice(&dev);
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+      st = launch_heff_tma_tables(work, (int)(batch * ntile), units, tasks, buf, C, nullptr, counter, sms, stream_v);
+      cudaFreeAsync(buf, stream);
+      return st;
+    }
   }
+  if (route == 2) return SU2_ERR_INVALID_ARGUMENT;
+  // rows that are not 16-byte aligned (odd k or n) and too large for the small-block kernel: FP64-FMA tile routine
   const int tiles = ((m + TILE_M - 1) / TILE_M) * ((p + TILE_P - 1) / TILE_P);
   dim3 grid(tiles, (unsigned)std::min<int64_t>(batch, 65535));
   gemm_pair_kernel<<<grid, GP_THREADS, 0, stream>>>(m, k, n, p, batch, alpha, A, X, B, C);
@@ -220,5 +242,13 @@ extern "C" su2_status su2_gemm_pair_batched(int32_t m, int32_t k, int32_t n, int
                                             const double* A, const double* X, const double* B, double* C,
                                             void* cuda_stream) {
   if (m <= 0 || k <= 0 || n <= 0 || p <= 0 || batch < 0 || !A || !X || !B || !C) return SU2_ERR_INVALID_ARGUMENT;
-  return su2::launch_gemm_pair(m, k, n, p, batch, alpha, A, X, B, C, cuda_stream);
+  return su2::launch_gemm_pair(m, k, n, p, batch, alpha, A, X, B, C, cuda_stream, 0, 0, 0);
+}
+
+extern "C" su2_status su2_gemm_pair_batched_route(int32_t m, int32_t k, int32_t n, int32_t p, int64_t batch, double alpha,
+                                                  const double* A, const double* X, const double* B, double* C,
+                                                  void* cuda_stream, int32_t route, int32_t wpi, int32_t nbuf) {
+  if (m <= 0 || k <= 0 || n <= 0 || p <= 0 || batch < 0 || !A || !X || !B || !C || route < 0 || route > 3)
+    return SU2_ERR_INVALID_ARGUMENT;
+  return su2::launch_gemm_pair(m, k, n, p, batch, alpha, A, X, B, C, cuda_stream, route, wpi, nbuf);
 }

@@ -111,12 +111,12 @@ heff_small_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __
   double* const Ts = smem + 3 * SZ;
   for (int e = tid; e < 4 * SZ; e += THREADS) smem[e] = 0.0;   // whatever sits in a pad must be finite
 
-  // dense rows x cols block -> shared rows of stride LD, one warp per row; pads untouched
-  auto copy_rows = [&](double* dst, const double* __restrict__ src, int rows, int cols) {
+  // stored rows x cols block (leading dimension lds) -> shared rows of stride LD, one warp per row; pads untouched
+  auto copy_rows = [&](double* dst, const double* __restrict__ src, int rows, int cols, int lds) {
     uint32_t d = (uint32_t)__cvta_generic_to_shared(dst) + (uint32_t)(warp * LD) * 8u;
-    const double* s = src + (int64_t)warp * cols;
-    const int64_t s_step = (int64_t)WARPS * cols;
-    if (!(cols & 1) && !((uintptr_t)src & 15)) {
+    const double* s = src + (int64_t)warp * lds;
+    const int64_t s_step = (int64_t)WARPS * lds;
+    if (!(cols & 1) && !(lds & 1) && !((uintptr_t)src & 15)) {
       if (2 * lane < cols) {
         d += 16u * lane; s += 2 * lane;
         for (int r = warp; r < rows; r += WARPS, d += WARPS * LD * 8, s += s_step)
@@ -141,14 +141,14 @@ heff_small_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __
   };
   auto issue_AE = [&](const DevTask& t, int pos, bool with_e) {
     const double* A = t.A + (int64_t)pos * t.strideA;
-    if (t.flags & TASK_TRANS_A) copy_rows(As, A, t.k, t.m);
-    else copy_rows(As, A, t.m, t.k);
+    if (t.flags & TASK_TRANS_A) copy_rows(As, A, t.k, t.m, t.ldA);
+    else copy_rows(As, A, t.m, t.k, t.ldA);
     if (with_e) copy_e(psi + t.e_off, t.k, t.n, (t.k + 3) & ~3, (t.n + 7) & ~7);
   };
   auto issue_D = [&](const DevTask& t, int pos) {
     const double* D = t.D + (int64_t)pos * t.strideD;
-    if (t.flags & TASK_TRANS_D) copy_rows(Ds, D, t.n, t.p);
-    else copy_rows(Ds, D, t.p, t.n);
+    if (t.flags & TASK_TRANS_D) copy_rows(Ds, D, t.n, t.p, t.ldD);
+    else copy_rows(Ds, D, t.p, t.n, t.ldD);
   };
 
   for (;;) {

@@ -10,7 +10,10 @@
 #include <cstring>
 #include <string>
 
+#include <map>
+
 #include "su2_internal.h"
+#include "tile_config.h"
 
 namespace su2 {
 
@@ -20,6 +23,7 @@ void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 void set_cuda_error(const char* what, int code) {
   g_cuda_error = std::string(what) + ": " + cudaGetErrorString((cudaError_t)code);
 }
+void set_error_text(const char* what) { g_cuda_error = what; }
 #define SU2_CUDA(call)                              \
   do {                                              \
     cudaError_t _e = (call);                        \
@@ -41,43 +45,47 @@ reduce_kernel(const DevReduce* __restrict__ red, const double* __restrict__ part
   }
 }
 
-// Plan-time position folding (the paper's pre-contraction): dst[e] = sum_pos alpha_pos src[pos][e],
+// Plan-time position folding (the paper's pre-contraction): dst[r][c] = sum_pos alpha_pos src[pos][r][c],
 // positions summed in index order (deterministic).  HBM-bound, runs once per plan.
 __global__ void __launch_bounds__(256)
 fold_kernel(const FoldJob* __restrict__ jobs, const double* __restrict__ alpha, double* __restrict__ fold) {
   const FoldJob j = jobs[blockIdx.y];
   const double* __restrict__ al = j.alpha_off >= 0 ? alpha + j.alpha_off : nullptr;
-  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < j.nelem; e += (int64_t)gridDim.x * blockDim.x) {
+  const int64_t nelem = (int64_t)j.rows * j.cols, pstride = (int64_t)j.rows * j.ld_src;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < nelem; e += (int64_t)gridDim.x * blockDim.x) {
+    const int r = (int)(e / j.cols), c = (int)(e % j.cols);
+    const double* __restrict__ src = j.src + (int64_t)r * j.ld_src + c;
     double s = 0.0;
-    for (int pos = 0; pos < j.npos; ++pos) s += (al ? al[pos] : 1.0) * j.src[(int64_t)pos * j.nelem + e];
-    fold[j.dst_off + e] = s;
+    for (int pos = 0; pos < j.npos; ++pos) s += (al ? al[pos] : 1.0) * src[(int64_t)pos * pstride];
+    fold[j.dst_off + (int64_t)r * j.ld_dst + c] = s;
   }
 }
 
-// Plan-time transposed copy of a right-block operator block, 32x32 tiles through shared memory:
-// dst[pos][j][c] = src[pos][c][j].  blockIdx.x = tile, blockIdx.y = job, blockIdx.z strides positions.
+// Plan-time padded copy of a block whose rows are not 16-byte aligned (see plan.cpp): leading dimension ld_src -> ld_dst,
+// pad columns zeroed.  blockIdx.y = job, blockIdx.z strides positions.
 __global__ void __launch_bounds__(256)
-transpose_kernel(const TransposeJob* __restrict__ jobs, double* __restrict__ trans) {
-  __shared__ double tile[32][33];
-  const TransposeJob j = jobs[blockIdx.y];
-  const int tc = (j.cols + 31) / 32, tr = (j.rows + 31) / 32;
-  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+copy_kernel(const CopyJob* __restrict__ jobs, double* __restrict__ buf) {
+  const CopyJob j = jobs[blockIdx.y];
+  const int64_t nelem = (int64_t)j.rows * j.ld_dst;
   for (int pos = blockIdx.z; pos < j.npos; pos += gridDim.z) {
-    const double* __restrict__ src = j.src + (int64_t)pos * j.rows * j.cols;
-    double* __restrict__ dst = trans + j.dst_off + (int64_t)pos * j.rows * j.cols;
-    for (int t = blockIdx.x; t < tr * tc; t += gridDim.x) {
-      const int r0 = (t / tc) * 32, c0 = (t % tc) * 32;
-      for (int i = ty; i < 32; i += 8) {
-        const int r = r0 + i, c = c0 + tx;
-        tile[i][tx] = (r < j.rows && c < j.cols) ? src[(int64_t)r * j.cols + c] : 0.0;
-      }
-      __syncthreads();
-      for (int i = ty; i < 32; i += 8) {
-        const int c = c0 + i, r = r0 + tx;
-        if (c < j.cols && r < j.rows) dst[(int64_t)c * j.rows + r] = tile[tx][i];
-      }
-      __syncthreads();
+    const double* __restrict__ src = j.src + (int64_t)pos * j.rows * j.ld_src;
+    double* __restrict__ dst = buf + j.dst_off + (int64_t)pos * nelem;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < nelem; e += (int64_t)gridDim.x * blockDim.x) {
+      const int r = (int)(e / j.ld_dst), c = (int)(e % j.ld_dst);
+      dst[e] = c < j.cols ? src[(int64_t)r * j.ld_src + c] : 0.0;
     }
+  }
+}
+
+// Every apply of a large-tile plan: Psi -> the plan's padded private copy (rows on 32-byte boundaries) the E boxes
+// are loaded from.  HBM-bound, 16 bytes per element of Psi: 0.05 ms at configs[3] against seconds of compute.
+__global__ void __launch_bounds__(256)
+psi_pad_kernel(const PsiPadJob* __restrict__ jobs, const double* __restrict__ psi, double* __restrict__ pad) {
+  const PsiPadJob j = jobs[blockIdx.y];
+  const int64_t nelem = (int64_t)j.rows * j.ld_dst;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < nelem; e += (int64_t)gridDim.x * blockDim.x) {
+    const int r = (int)(e / j.ld_dst), c = (int)(e % j.ld_dst);
+    pad[j.dst_off + e] = c < j.cols ? psi[j.src_off + (int64_t)r * j.cols + c] : 0.0;
   }
 }
 
@@ -96,7 +104,7 @@ diag_kernel(const DevDiagTask* __restrict__ dt, const int32_t* __restrict__ begi
       double v = 0.0;
       for (int pos = 0; pos < t.npos; ++pos) {
         const double al = t.alpha ? t.alpha[pos] : 1.0;
-        v += al * t.A[(int64_t)pos * t.strideA + (int64_t)a * m + a] * t.D[(int64_t)pos * t.strideD + (int64_t)b * p + b];
+        v += al * t.A[(int64_t)pos * t.strideA + (int64_t)a * t.ldA + a] * t.D[(int64_t)pos * t.strideD + (int64_t)b * t.ldD + b];
       }
       acc += t.coef * v;
     }
@@ -109,14 +117,56 @@ diag_kernel(const DevDiagTask* __restrict__ dt, const int32_t* __restrict__ begi
 // ---------------------------------------------------------------------------------------
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, const std::vector<double>& ident_host,
-                       const std::vector<int64_t>& alpha_off_of_task, const std::vector<int64_t>& identA,
-                       const std::vector<int64_t>& identD, const std::vector<int64_t>& foldA,
-                       const std::vector<int64_t>& foldD, const std::vector<int64_t>& transD, void* stream_v) {
+namespace {
+struct DeviceFree {   // frees on scope exit (error paths of upload_plan)
+  void* p = nullptr;
+  ~DeviceFree() { if (p) cudaFree(p); }
+};
+}  // namespace
+
+su2_status upload_plan(su2_plan* plan, void* stream_v) {
   cudaStream_t stream = (cudaStream_t)stream_v;
   int dev = 0;
   SU2_CUDA(cudaGetDevice(&dev));
   SU2_CUDA(cudaDeviceGetAttribute(&plan->num_sms, cudaDevAttrMultiProcessorCount, dev));
+  const bool large = plan->small_dm8 == 0;
+  // ---- plan-owned operator buffers -------------------------------------------------------------
+  auto big_alloc = [&](double** ptr, int64_t elems, const char* what) -> su2_status {
+    if (elems <= 0) return SU2_OK;
+    cudaError_t e = cudaMalloc((void**)ptr, (size_t)elems * sizeof(double));
+    if (e != cudaSuccess) {   // fail loudly: there is no slower layout to fall back to
+      *ptr = nullptr;
+      char buf[200];
+      std::snprintf(buf, sizeof(buf), "cudaMalloc of %.2f GB for %s", elems * 8.0 / 1e9, what);
+      set_cuda_error(buf, (int)e);
+      (void)cudaGetLastError();
+      return SU2_ERR_CUDA;
+    }
+    plan->info.plan_device_bytes += elems * (int64_t)sizeof(double);
+    return SU2_OK;
+  };
+  plan->info.plan_device_bytes = 0;
+  su2_status st;
+  if ((st = big_alloc(&plan->d_fold, plan->fold_elems, "the position-folded operators")) != SU2_OK) return st;
+  if ((st = big_alloc(&plan->d_copy, plan->copy_elems,
+                      "padded copies of operator families whose rows are not 16-byte aligned (pass blk_ld with even "
+                      "leading dimensions to have them read in place)")) != SU2_OK) return st;
+  if ((st = big_alloc(&plan->d_psi_pad, plan->psipad_elems, "the padded copy of Psi")) != SU2_OK) return st;
+
+  // ---- resolve operand pointers; tensor maps of the large-tile kernel ------------------------------
+  std::vector<unsigned char> h_maps;       // 128-byte records
+  std::map<MapKey, int32_t> map_index;
+  auto map_for = [&](const MapKey& key, int32_t* out) -> su2_status {
+    auto it = map_index.find(key);
+    if (it != map_index.end()) { *out = it->second; return SU2_OK; }
+    const int32_t idx = (int32_t)map_index.size();
+    h_maps.resize((size_t)(idx + 1) * 128);
+    su2_status s2 = encode_tensor_map(h_maps.data() + (size_t)idx * 128, key);
+    if (s2 != SU2_OK) return s2;
+    map_index[key] = idx;
+    *out = idx;
+    return SU2_OK;
+  };
   const size_t b_tasks = align256(plan->h_tasks.size() * sizeof(DevTask));
   const size_t b_units = align256(plan->h_units.size() * sizeof(DevUnit));
   const size_t b_work = align256(plan->h_work.size() * sizeof(DevWork));
@@ -124,34 +174,19 @@ su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, co
   const size_t b_diag = align256(plan->h_diag.size() * sizeof(DevDiagTask));
   const size_t b_dbeg = align256(plan->h_diag_begin.size() * sizeof(int32_t));
   const size_t b_psi = align256(plan->psi.size() * sizeof(PsiSector));
-  const size_t b_alpha = align256(alpha_host.size() * sizeof(double));
-  const size_t b_ident = align256(ident_host.size() * sizeof(double));
-  const size_t total = b_tasks + b_units + b_work + b_red + b_diag + b_dbeg + b_psi + b_alpha + b_ident + 256;
+  const size_t b_pad = align256(plan->h_psipad.size() * sizeof(PsiPadJob));
+  const size_t b_alpha = align256(plan->h_alpha.size() * sizeof(double));
+  const size_t b_ident = align256(plan->h_ident.size() * sizeof(double));
+  // the identity blocks must exist before their tensor maps are encoded: allocate the blob first (maps are
+  // appended to it in a second allocation-free step: their count is bounded by 3 per task)
+  const size_t b_maps = align256(large ? (3 * plan->h_tasks.size() + 1) * 128 : 0);
+  const size_t total = b_tasks + b_units + b_work + b_red + b_diag + b_dbeg + b_psi + b_pad + b_alpha + b_ident + b_maps + 256;
   SU2_CUDA(cudaMalloc(&plan->d_blob, total));
-  plan->info.plan_device_bytes = (int64_t)total;
-  TransposeJob* d_tjobs = nullptr;
-  if (plan->trans_elems > 0) {
-    bool ok = true;
-    for (const TransposeJob& j : plan->h_trans) ok = ok && j.src != nullptr;
-    // optional: when the copy does not fit, the tasks keep reading the stored layout
-    if (ok && cudaMalloc(&plan->d_trans, (size_t)plan->trans_elems * sizeof(double)) != cudaSuccess) {
-      plan->d_trans = nullptr;
-      (void)cudaGetLastError();
-    }
-    if (plan->d_trans) {
-      SU2_CUDA(cudaMalloc(&d_tjobs, plan->h_trans.size() * sizeof(TransposeJob)));
-      plan->info.plan_device_bytes += plan->trans_elems * (int64_t)sizeof(double);
-    }
-  }
-  FoldJob* d_jobs = nullptr;
-  if (plan->fold_elems > 0) {
-    SU2_CUDA(cudaMalloc(&plan->d_fold, (size_t)plan->fold_elems * sizeof(double)));
-    plan->info.plan_device_bytes += plan->fold_elems * (int64_t)sizeof(double);
-    SU2_CUDA(cudaMalloc(&d_jobs, plan->h_fold.size() * sizeof(FoldJob)));
-  }
+  plan->info.plan_device_bytes += (int64_t)total;
   char* base = (char*)plan->d_blob;
   size_t off = 0;
-  auto carve = [&](size_t bytes) { char* p = base + off; off += bytes; return p; };
+  auto carve = [&](size_t bytes) { char* q = base + off; off += bytes; return q; };
+  plan->d_maps = carve(b_maps);            // first: 256-byte aligned records
   plan->d_tasks = (DevTask*)carve(b_tasks);
   plan->d_units = (DevUnit*)carve(b_units);
   plan->d_work = (DevWork*)carve(b_work);
@@ -159,23 +194,39 @@ su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, co
   plan->d_diag = (DevDiagTask*)carve(b_diag);
   plan->d_diag_begin = (int32_t*)carve(b_dbeg);
   char* d_psi = carve(b_psi);
+  plan->d_psipad = (PsiPadJob*)carve(b_pad);
   plan->d_alpha = (double*)carve(b_alpha);
   plan->d_identity = (double*)carve(b_ident);
   plan->d_counter = (int32_t*)carve(256);
-  // patch device pointers into the host images
+
+  auto resolve = [&](const OperandRef& r) -> const double* {
+    switch (r.kind) {
+      case 0: { const double* b0 = plan->fam_ptr[r.side][r.fam]; return b0 ? b0 + r.off : nullptr; }
+      case 1: return plan->d_copy ? plan->d_copy + r.off : nullptr;
+      case 2: return plan->d_fold ? plan->d_fold + r.off : nullptr;
+      default: return plan->d_identity + r.off;
+    }
+  };
   for (size_t i = 0; i < plan->h_tasks.size(); ++i) {
     DevTask& t = plan->h_tasks[i];
-    if (alpha_off_of_task[i] >= 0) t.alpha = plan->d_alpha + alpha_off_of_task[i];
-    if (identA[i] >= 0) t.A = plan->d_identity + identA[i];
-    if (identD[i] >= 0) t.D = plan->d_identity + identD[i];
-    if (foldA[i] >= 0) t.A = plan->d_fold + foldA[i];
-    if (foldD[i] >= 0) t.D = plan->d_fold + foldD[i];
-    if (transD[i] >= 0 && plan->d_trans) {
-      t.D = plan->d_trans + transD[i];
-      t.flags |= TASK_TRANS_D;
-    }
+    const OperandRef &ra = plan->h_opA[i], &rd = plan->h_opD[i];
+    t.A = resolve(ra);
+    t.D = resolve(rd);
     if (!t.A || !t.D) return SU2_ERR_INVALID_ARGUMENT;   // family without device data
+    if (plan->h_alpha_off[i] >= 0) t.alpha = plan->d_alpha + plan->h_alpha_off[i];
+    if (!large) continue;
+    const int wr = plan->tasks[i].wr;
+    const int tm = 32 * wr;
+    MapKey ka{t.A, ra.rows, ra.cols, ra.ld, ra.npos, (int64_t)ra.rows * ra.ld,
+              (t.flags & TASK_TRANS_A) ? tm + 4 : KS1, (t.flags & TASK_TRANS_A) ? KS1 : tm};
+    MapKey kd{t.D, rd.rows, rd.cols, rd.ld, rd.npos, (int64_t)rd.rows * rd.ld,
+              (t.flags & TASK_TRANS_D) ? DBOX_LD : KS2, (t.flags & TASK_TRANS_D) ? KS2 : DBOX_C};
+    const PsiPadJob& pj = plan->h_psipad[plan->tasks[i].in_sec];
+    MapKey ke{plan->d_psi_pad + pj.dst_off, pj.rows, pj.cols, pj.ld_dst, 1, (int64_t)pj.rows * pj.ld_dst, EBOX_LD, KS1};
+    if ((st = map_for(ka, &t.mapA)) != SU2_OK || (st = map_for(kd, &t.mapD)) != SU2_OK || (st = map_for(ke, &t.mapE)) != SU2_OK) return st;
+    t.e_item = 0;
   }
+  plan->nmaps = (int32_t)map_index.size();
   for (auto& d : plan->h_diag) {
     const DevTask& t = plan->h_tasks[d.pad];
     d.A = t.A; d.D = t.D; d.alpha = t.alpha;
@@ -184,6 +235,7 @@ su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, co
     if (bytes == 0) return cudaSuccess;
     return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, stream);
   };
+  SU2_CUDA(up(plan->d_maps, h_maps.data(), h_maps.size()));
   SU2_CUDA(up(plan->d_tasks, plan->h_tasks.data(), plan->h_tasks.size() * sizeof(DevTask)));
   SU2_CUDA(up(plan->d_units, plan->h_units.data(), plan->h_units.size() * sizeof(DevUnit)));
   SU2_CUDA(up(plan->d_work, plan->h_work.data(), plan->h_work.size() * sizeof(DevWork)));
@@ -191,51 +243,58 @@ su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, co
   SU2_CUDA(up(plan->d_diag, plan->h_diag.data(), plan->h_diag.size() * sizeof(DevDiagTask)));
   SU2_CUDA(up(plan->d_diag_begin, plan->h_diag_begin.data(), plan->h_diag_begin.size() * sizeof(int32_t)));
   SU2_CUDA(up(d_psi, plan->psi.data(), plan->psi.size() * sizeof(PsiSector)));
-  SU2_CUDA(up(plan->d_alpha, alpha_host.data(), alpha_host.size() * sizeof(double)));
-  SU2_CUDA(up(plan->d_identity, ident_host.data(), ident_host.size() * sizeof(double)));
+  SU2_CUDA(up(plan->d_psipad, plan->h_psipad.data(), plan->h_psipad.size() * sizeof(PsiPadJob)));
+  SU2_CUDA(up(plan->d_alpha, plan->h_alpha.data(), plan->h_alpha.size() * sizeof(double)));
+  SU2_CUDA(up(plan->d_identity, plan->h_ident.data(), plan->h_ident.size() * sizeof(double)));
+  DeviceFree d_fjobs, d_cjobs;
   if (plan->fold_elems > 0) {
     for (const FoldJob& j : plan->h_fold)
-      if (!j.src) { cudaFree(d_jobs); return SU2_ERR_INVALID_ARGUMENT; }   // family without device data
-    SU2_CUDA(cudaMemcpyAsync(d_jobs, plan->h_fold.data(), plan->h_fold.size() * sizeof(FoldJob), cudaMemcpyHostToDevice, stream));
+      if (!j.src) return SU2_ERR_INVALID_ARGUMENT;   // family without device data
+    SU2_CUDA(cudaMalloc(&d_fjobs.p, plan->h_fold.size() * sizeof(FoldJob)));
+    SU2_CUDA(cudaMemcpyAsync(d_fjobs.p, plan->h_fold.data(), plan->h_fold.size() * sizeof(FoldJob), cudaMemcpyHostToDevice, stream));
+    SU2_CUDA(cudaMemsetAsync(plan->d_fold, 0, (size_t)plan->fold_elems * sizeof(double), stream));   // pad columns
     dim3 grid(64, (unsigned)plan->h_fold.size());
-    fold_kernel<<<grid, 256, 0, stream>>>(d_jobs, plan->d_alpha, plan->d_fold);
+    fold_kernel<<<grid, 256, 0, stream>>>((const FoldJob*)d_fjobs.p, plan->d_alpha, plan->d_fold);
     SU2_CUDA(cudaGetLastError());
     count_launch();
   }
-  if (plan->d_trans) {
-    SU2_CUDA(cudaMemcpyAsync(d_tjobs, plan->h_trans.data(), plan->h_trans.size() * sizeof(TransposeJob), cudaMemcpyHostToDevice, stream));
-    dim3 grid(64, (unsigned)plan->h_trans.size(), 16);
-    transpose_kernel<<<grid, 256, 0, stream>>>(d_tjobs, plan->d_trans);
+  if (plan->copy_elems > 0) {
+    for (const CopyJob& j : plan->h_copy)
+      if (!j.src) return SU2_ERR_INVALID_ARGUMENT;
+    SU2_CUDA(cudaMalloc(&d_cjobs.p, plan->h_copy.size() * sizeof(CopyJob)));
+    SU2_CUDA(cudaMemcpyAsync(d_cjobs.p, plan->h_copy.data(), plan->h_copy.size() * sizeof(CopyJob), cudaMemcpyHostToDevice, stream));
+    dim3 grid(64, (unsigned)plan->h_copy.size(), 16);
+    copy_kernel<<<grid, 256, 0, stream>>>((const CopyJob*)d_cjobs.p, plan->d_copy);
     SU2_CUDA(cudaGetLastError());
     count_launch();
   }
   SU2_CUDA(cudaStreamSynchronize(stream));
-  if (d_jobs) cudaFree(d_jobs);
-  if (d_tjobs) cudaFree(d_tjobs);
   plan->d_psi_sec = d_psi;
+  plan->info.padded_copy_bytes = plan->copy_elems * (int64_t)sizeof(double);
   return SU2_OK;
 }
 
 void free_plan_device(su2_plan* plan) {
-  if (plan && plan->d_blob) {
-    cudaFree(plan->d_blob);
-    plan->d_blob = nullptr;
-  }
-  if (plan && plan->d_fold) {
-    cudaFree(plan->d_fold);
-    plan->d_fold = nullptr;
-  }
-  if (plan && plan->d_trans) {
-    cudaFree(plan->d_trans);
-    plan->d_trans = nullptr;
-  }
+  if (!plan) return;
+  for (void** q : {(void**)&plan->d_blob, (void**)&plan->d_fold, (void**)&plan->d_copy, (void**)&plan->d_psi_pad})
+    if (*q) { cudaFree(*q); *q = nullptr; }
 }
 
 su2_status launch_apply(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream_v) {
   cudaStream_t stream = (cudaStream_t)stream_v;
   SU2_CUDA(cudaMemsetAsync(plan->d_counter, 0, 8 * sizeof(int32_t), stream));   // [0]: work queue; small plans: one per size class
-  su2_status st = plan->small_dm8 > 0 ? launch_heff_small(plan, psi, out, partial, stream_v)
-                                      : launch_heff_dmma(plan, psi, out, partial, stream_v);
+  su2_status st;
+  if (plan->small_dm8 > 0) {
+    st = launch_heff_small(plan, psi, out, partial, stream_v);
+  } else {
+    if (!plan->h_psipad.empty()) {
+      dim3 grid(16, (unsigned)plan->h_psipad.size());
+      psi_pad_kernel<<<grid, 256, 0, stream>>>(plan->d_psipad, psi, plan->d_psi_pad);
+      SU2_CUDA(cudaGetLastError());
+      count_launch();
+    }
+    st = launch_heff_tma(plan, out, partial, stream_v);
+  }
   if (st != SU2_OK) return st;
   const int nsec = (int)plan->h_reduce.size();
   if (nsec > 0) {

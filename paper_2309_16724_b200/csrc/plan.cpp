@@ -276,13 +276,31 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
     return std::tie(x.out_sec, x.in_sec, x.term, x.blk_l, x.blk_r) < std::tie(y.out_sec, y.in_sec, y.term, y.blk_l, y.blk_r);
   });
 
-  // ---- device task images ---------------------------------------------------------------
+  // ---- operand layout ---------------------------------------------------------------------
+  // Leading dimension of every stored block (su2_opfamily.blk_ld; dense if absent).
+  auto blk_ld = [&](int side, int f, int b) {
+    const su2_opfamily& fam = side ? p->fam_r[f] : p->fam_l[f];
+    const auto& sec = side ? sr : sl;
+    return fam.blk_ld ? (int)fam.blk_ld[b] : (int)sec[fam.q_in[b]].dim;
+  };
+  for (int side = 0; side < 2; ++side) {
+    const int nf = side ? p->nfam_r : p->nfam_l;
+    plan->fam_ptr[side].resize(nf);
+    for (int f = 0; f < nf; ++f) {
+      const su2_opfamily& fam = side ? p->fam_r[f] : p->fam_l[f];
+      const auto& sec = side ? sr : sl;
+      plan->fam_ptr[side][f] = fam.data;
+      for (int b = 0; b < fam.nblk; ++b)
+        if (blk_ld(side, f, b) < sec[fam.q_in[b]].dim) { delete plan; return SU2_ERR_INVALID_ARGUMENT; }
+    }
+  }
+  auto pad4 = [](int x) { return (x + 3) & ~3; };
+
   // ---- position folding (the paper's pre-contraction) -----------------------------
   // A row whose positions enter through ONE block only (the other factor is the identity or has a
   // single position) is sum_pos alpha_pos A_pos applied once: that sum does not depend on Psi, so it
   // is formed at plan time (fold_kernel) and the row's tasks become one-position tasks.
   std::vector<int> fold_side(p->nterm, -1);          // -1: not folded, 0: l family folded, 1: r family folded
-  std::vector<int64_t> fold_base(p->nterm, -1);      // element offset of the term's folded family in plan->d_fold
   std::vector<std::vector<int64_t>> fold_blk_off(p->nterm);
   int64_t fold_elems = 0;
   for (int t = 0; t < p->nterm; ++t) {
@@ -291,39 +309,32 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
     const int npr = tm.fam_r >= 0 ? p->fam_r[tm.fam_r].npos : 1;
     if (tm.npos <= 1 || (npl > 1) == (npr > 1)) continue;
     const int side = npl > 1 ? 0 : 1;
-    const su2_opfamily& f = side ? p->fam_r[tm.fam_r] : p->fam_l[tm.fam_l];
+    const int fi = side ? tm.fam_r : tm.fam_l;
+    const su2_opfamily& f = side ? p->fam_r[fi] : p->fam_l[fi];
     const auto& sec = side ? sr : sl;
     fold_side[t] = side;
-    fold_base[t] = fold_elems;
     fold_blk_off[t].resize(f.nblk);
     for (int b = 0; b < f.nblk; ++b) {
       fold_blk_off[t][b] = fold_elems;
-      const int64_t nelem = (int64_t)sec[f.q_out[b]].dim * sec[f.q_in[b]].dim;
       FoldJob job{};
       job.src = f.data ? f.data + f.blk_off[b] : nullptr;
       job.dst_off = fold_elems;
-      job.nelem = nelem;
+      job.rows = sec[f.q_out[b]].dim; job.cols = sec[f.q_in[b]].dim;
+      job.ld_src = blk_ld(side, fi, b); job.ld_dst = pad4(job.cols);
       job.npos = f.npos;
       job.alpha_off = alpha_off_of_term[t];
       plan->h_fold.push_back(job);
-      fold_elems += nelem;
+      fold_elems += (int64_t)job.rows * job.ld_dst;
     }
   }
   plan->fold_elems = fold_elems;
   for (HostTask& ht : plan->tasks)
     if (fold_side[ht.term] >= 0) ht.npos = 1;
 
-  // ---- transposed copies of the right-block families ------------------------------------------
-  // The second product stages D_pos[cols, chunk]: for a row-major block used as stored that is a
-  // gather of 64-byte runs (measured 6.2 TB/s per GPU into shared memory), for a block read transposed it
-  // is one contiguous run per k row (16-byte cp.async, 11-19 TB/s).  Families that are used as stored by
-  // position-batched rows therefore get a transposed copy at plan time (transpose_kernel); if the copy
-  // does not fit in device memory the plan falls back to the stored layout.
   // ---- small-block plan? (heff_small.cu) -------------------------------------------------------
   // Every block sector of the bond holds at most SMALL_MAX_DIM multiplets: the whole apply runs on
-  // heff_small_kernel (one CTA per output sector and segment), which reads blocks in either orientation at full
-  // speed, so no transposed copies are made.  SU2_PLAN_LARGE_TILES keeps the large-tile kernel (tests, A/B
-  // measurements).
+  // heff_small_kernel (one CTA per output sector and segment), which reads blocks of any layout with plain
+  // cp.async.  SU2_PLAN_LARGE_TILES keeps the large-tile kernel (tests, A/B measurements).
   {
     int maxdim = 0;
     for (const su2_sector& q : plan->sec_l) maxdim = std::max(maxdim, (int)q.dim);
@@ -333,44 +344,94 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
   }
   const bool small_plan = plan->small_dm8 > 0;
 
-  std::vector<std::vector<int64_t>> trans_blk_off(p->nfam_r);
+  // ---- padded copies for the bulk-tensor engine ---------------------------------------------------
+  // heff_tma_kernel stages every operand tile with cp.async.bulk.tensor, which needs 16-byte aligned rows.  A
+  // family whose device pointer is 16-byte aligned and whose blocks all have an even offset and an even leading
+  // dimension is read in place; any other family used by a non-folded row is copied once, at plan time, into a
+  // plan-owned buffer with leading dimensions padded to a multiple of 4 (copy_kernel).
+  std::vector<std::vector<int64_t>> copy_blk_off[2];
+  copy_blk_off[0].resize(p->nfam_l);
+  copy_blk_off[1].resize(p->nfam_r);
   if (!small_plan) {
-    std::vector<char> need(p->nfam_r, 0);
-    for (const HostTask& ht : plan->tasks)
-      if (ht.fam_r >= 0 && !ht.adj_r && fold_side[ht.term] != 1 && p->fam_r[ht.fam_r].npos > 1) need[ht.fam_r] = 1;
+    std::vector<char> used[2];
+    used[0].assign(p->nfam_l, 0);
+    used[1].assign(p->nfam_r, 0);
+    for (const HostTask& ht : plan->tasks) {
+      if (ht.fam_l >= 0 && fold_side[ht.term] != 0) used[0][ht.fam_l] = 1;
+      if (ht.fam_r >= 0 && fold_side[ht.term] != 1) used[1][ht.fam_r] = 1;
+    }
     int64_t off = 0;
-    for (int f = 0; f < p->nfam_r; ++f) {
-      if (!need[f]) continue;
-      const su2_opfamily& fam = p->fam_r[f];
-      trans_blk_off[f].resize(fam.nblk);
-      for (int b = 0; b < fam.nblk; ++b) {
-        trans_blk_off[f][b] = off;
-        TransposeJob job{};
-        job.src = fam.data ? fam.data + fam.blk_off[b] : nullptr;
-        job.dst_off = off;
-        job.rows = sr[fam.q_out[b]].dim; job.cols = sr[fam.q_in[b]].dim; job.npos = fam.npos;
-        plan->h_trans.push_back(job);
-        off += (int64_t)fam.npos * job.rows * job.cols;
+    for (int side = 0; side < 2; ++side) {
+      const int nf = side ? p->nfam_r : p->nfam_l;
+      for (int f = 0; f < nf; ++f) {
+        if (!used[side][f]) continue;
+        const su2_opfamily& fam = side ? p->fam_r[f] : p->fam_l[f];
+        const auto& sec = side ? sr : sl;
+        bool aligned = ((uintptr_t)fam.data & 15) == 0;
+        for (int b = 0; b < fam.nblk && aligned; ++b) aligned = !(fam.blk_off[b] & 1) && !(blk_ld(side, f, b) & 1);
+        if (aligned) continue;
+        copy_blk_off[side][f].resize(fam.nblk);
+        for (int b = 0; b < fam.nblk; ++b) {
+          copy_blk_off[side][f][b] = off;
+          CopyJob job{};
+          job.src = fam.data ? fam.data + fam.blk_off[b] : nullptr;
+          job.dst_off = off;
+          job.rows = sec[fam.q_out[b]].dim; job.cols = sec[fam.q_in[b]].dim;
+          job.ld_src = blk_ld(side, f, b); job.ld_dst = pad4(job.cols); job.npos = fam.npos;
+          plan->h_copy.push_back(job);
+          off += (int64_t)fam.npos * job.rows * job.ld_dst;
+        }
       }
     }
-    plan->trans_elems = off;
+    plan->copy_elems = off;
+    // padded private copy of Psi: the E tiles are bulk-tensor loads too
+    int64_t poff = 0;
+    for (const PsiSector& ps : plan->psi) {
+      PsiPadJob j{};
+      j.src_off = ps.off; j.dst_off = poff; j.rows = ps.m; j.cols = ps.p; j.ld_dst = pad4(ps.p);
+      plan->h_psipad.push_back(j);
+      poff += (int64_t)ps.m * j.ld_dst;
+    }
+    plan->psipad_elems = poff;
   }
 
+  // ---- task records: where the two operator blocks of every task live ----------------------------------
   const int64_t ntask = (int64_t)plan->tasks.size();
   plan->h_tasks.resize(ntask);
-  std::vector<int64_t> transD(ntask, -1);
-  std::vector<int64_t> alpha_off_of_task(ntask, -1), identA(ntask, -1), identD(ntask, -1), foldA(ntask, -1), foldD(ntask, -1);
-  // identity blocks: one (dim x dim) identity per distinct dim, concatenated
+  plan->h_opA.resize(ntask);
+  plan->h_opD.resize(ntask);
+  plan->h_alpha_off.assign(ntask, -1);
+  plan->h_alpha = alpha_host;
+  // identity blocks: one (dim x pad4(dim)) identity per distinct dim, concatenated
   std::map<int, int64_t> ident_off;
-  std::vector<double> ident_host;
   auto ident_for = [&](int dim) {
     auto it = ident_off.find(dim);
     if (it != ident_off.end()) return it->second;
-    const int64_t off = (int64_t)ident_host.size();
-    ident_host.resize(off + (int64_t)dim * dim, 0.0);
-    for (int i = 0; i < dim; ++i) ident_host[off + (int64_t)i * dim + i] = 1.0;
+    const int ld = pad4(dim);
+    const int64_t off = (int64_t)plan->h_ident.size();
+    plan->h_ident.resize(off + (int64_t)dim * ld, 0.0);
+    for (int i = 0; i < dim; ++i) plan->h_ident[off + (int64_t)i * ld + i] = 1.0;
     ident_off[dim] = off;
     return off;
+  };
+  auto operand = [&](int side, int fam, int blk, int term, int dim) {
+    OperandRef r{};
+    const auto& sec = side ? sr : sl;
+    if (fam < 0) {
+      r.kind = 3; r.off = ident_for(dim); r.rows = dim; r.cols = dim; r.ld = pad4(dim); r.npos = 1;
+      return r;
+    }
+    const su2_opfamily& f = side ? p->fam_r[fam] : p->fam_l[fam];
+    r.side = side; r.fam = fam;
+    r.rows = sec[f.q_out[blk]].dim; r.cols = sec[f.q_in[blk]].dim;
+    if (fold_side[term] == side) {
+      r.kind = 2; r.off = fold_blk_off[term][blk]; r.ld = pad4(r.cols); r.npos = 1;
+    } else if (!copy_blk_off[side][fam].empty()) {
+      r.kind = 1; r.off = copy_blk_off[side][fam][blk]; r.ld = pad4(r.cols); r.npos = f.npos;
+    } else {
+      r.kind = 0; r.off = f.blk_off[blk]; r.ld = blk_ld(side, fam, blk); r.npos = f.npos;
+    }
+    return r;
   };
   double cc = 0.0, opbytes = 0.0;
   int64_t ntp = 0;
@@ -382,31 +443,16 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
     d.e_off = plan->psi[ht.in_sec].off;
     d.m = ht.m; d.k = ht.k; d.n = ht.n; d.p = ht.p; d.npos = ht.npos;
     d.flags = (ht.adj_l ? TASK_TRANS_A : 0u) | (ht.adj_r ? TASK_TRANS_D : 0u);
+    d.mapA = d.mapD = d.mapE = -1;
+    const OperandRef ra = operand(0, ht.fam_l, ht.blk_l, ht.term, ht.m);
+    const OperandRef rd = operand(1, ht.fam_r, ht.blk_r, ht.term, ht.p);
+    plan->h_opA[i] = ra;
+    plan->h_opD[i] = rd;
+    d.ldA = ra.ld; d.ldD = rd.ld;
+    d.strideA = ra.npos > 1 ? ra.rows * ra.ld : 0;
+    d.strideD = rd.npos > 1 ? rd.rows * rd.ld : 0;
     const int fs = fold_side[ht.term];
-    if (ht.fam_l >= 0 && fs == 0) {
-      foldA[i] = fold_blk_off[ht.term][ht.blk_l];
-      d.strideA = 0;
-    } else if (ht.fam_l >= 0) {
-      const su2_opfamily& f = p->fam_l[ht.fam_l];
-      d.A = f.data ? f.data + f.blk_off[ht.blk_l] : nullptr;
-      d.strideA = f.npos > 1 ? ht.m * ht.k : 0;
-    } else {
-      identA[i] = ident_for(ht.m);
-      d.strideA = 0;
-    }
-    if (ht.fam_r >= 0 && fs == 1) {
-      foldD[i] = fold_blk_off[ht.term][ht.blk_r];
-      d.strideD = 0;
-    } else if (ht.fam_r >= 0) {
-      const su2_opfamily& f = p->fam_r[ht.fam_r];
-      d.D = f.data ? f.data + f.blk_off[ht.blk_r] : nullptr;
-      d.strideD = f.npos > 1 ? ht.p * ht.n : 0;
-      if (!ht.adj_r && !trans_blk_off[ht.fam_r].empty()) transD[i] = trans_blk_off[ht.fam_r][ht.blk_r];
-    } else {
-      identD[i] = ident_for(ht.p);
-      d.strideD = 0;
-    }
-    alpha_off_of_task[i] = fs >= 0 ? -1 : alpha_off_of_term[ht.term];   // folded rows carry alpha inside the block
+    plan->h_alpha_off[i] = fs >= 0 ? -1 : alpha_off_of_term[ht.term];   // folded rows carry alpha inside the block
     const double m = ht.m, k = ht.k, n = ht.n, pp = ht.p;
     cc += ht.npos * std::min(2 * m * k * n + 2 * m * n * pp, 2 * k * n * pp + 2 * m * k * pp);
     opbytes += ht.npos * 8.0 * (m * k + n * pp);
@@ -450,12 +496,17 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
     sec_cost[s] = best;
     total_cost += best;
   }
-  double executed = total_cost * NWARPS * 512.0;   // DMMA issue slots x 8 warps x 2*8*8*4 flop
-  if (small_plan) {   // heff_small_kernel: m8n8k4 tiles over (m8, k4, n8) and (m8, n8, p8)
-    executed = 0.0;
-    for (const HostTask& ht : plan->tasks) {
+  for (HostTask& ht : plan->tasks) ht.wr = sec_wr[ht.out_sec];
+  // FP64 tensor flops the kernels issue per apply (m8 / n8 / k4 padding of both products; the first product is
+  // always A E, and a sector wider than its tile class forms T once per column tile); agrees with ncu's
+  // sm__ops_path_tensor_src_fp64 up to the DMMAs of the predicated ragged-edge code paths
+  double executed = 0.0;
+  for (const HostTask& ht : plan->tasks) {
+    if (small_plan) {   // heff_small_kernel: m8n8k4 tiles over (m8, k4, n8) and (m8, n8, p8)
       const double m8 = (ht.m + 7) & ~7, k4 = (ht.k + 3) & ~3, n8 = (ht.n + 7) & ~7, p8 = (ht.p + 7) & ~7;
       executed += ht.npos * 2.0 * (m8 * k4 * n8 + m8 * n8 * p8);
+    } else {
+      executed += ht.npos * tile_pos_executed_flops(ht.wr, ht.m, ht.p, ht.k, ht.n);
     }
   }
   // target cost of one work item: ~24 items per SM, but never so small that the pipeline fill dominates
@@ -604,6 +655,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
       d.A = plan->h_tasks[i].A; d.D = plan->h_tasks[i].D; d.alpha = nullptr;
       d.coef = ht.coef; d.f_off = plan->psi[s].off; d.m = ht.m; d.p = ht.p;
       d.strideA = plan->h_tasks[i].strideA; d.strideD = plan->h_tasks[i].strideD; d.npos = ht.npos;
+      d.ldA = plan->h_tasks[i].ldA; d.ldD = plan->h_tasks[i].ldD;
       d.pad = (int32_t)i;   // index of the full task: upload_plan copies its patched pointers
       plan->h_diag.push_back(d);
     }
@@ -622,7 +674,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
   plan->info.small_plan = small_plan ? 1 : 0;
 
   if (!plan->host_only) {
-    st = upload_plan(plan, alpha_host, ident_host, alpha_off_of_task, identA, identD, foldA, foldD, transD, cuda_stream);
+    st = upload_plan(plan, cuda_stream);
     if (st != SU2_OK) {
       free_plan_device(plan);
       delete plan;

@@ -19,13 +19,16 @@ struct DevTask {
   int64_t e_off;          // offset of the input sector E_s' in psi
   int32_t m, k, n, p;
   int32_t strideA, strideD;   // elements between positions (0: same block for all positions)
+  int32_t ldA, ldD;           // leading dimensions of the STORED blocks
   int32_t npos;
   uint32_t flags;
+  int32_t mapA, mapD, mapE;   // large-tile kernel: indices of the operands' tensor maps (su2_plan::d_maps)
+  int32_t e_item;             // third coordinate of the E map (0 inside H_eff; the batch index of a GEMM-pair item)
 };
 enum : uint32_t { TASK_TRANS_A = 1u, TASK_TRANS_D = 2u };
 
 // A bond whose block sectors all hold at most this many multiplets runs on heff_small_kernel (heff_small.cu)
-// instead of the 128 x 144 / 64 x 288 / 32 x 576 register tiles of heff_dmma_kernel.
+// instead of the 128 x 144 / 64 x 288 / 32 x 576 register tiles of heff_tma_kernel.
 constexpr int SMALL_MAX_DIM = 48;
 
 // A run of positions of one task inside one segment.
@@ -50,20 +53,36 @@ struct DevReduce {
   int32_t pad;
 };
 
-// Plan-time position folding: dst[e] = sum_pos alpha[pos] * src[pos * nelem + e].
+// Plan-time position folding: dst[r][c] = sum_pos alpha[pos] * src[pos][r][c]  (dst leading dimension ld_dst).
 struct FoldJob {
-  const double* src;      // block of the family: [npos][nelem]
+  const double* src;      // block of the family: [npos][rows][ld_src]
   int64_t dst_off;        // element offset inside the plan's folded-operator buffer
-  int64_t nelem;
   int64_t alpha_off;      // offset into the plan's alpha array, -1: all ones
+  int32_t rows, cols, ld_src, ld_dst;
   int32_t npos, pad;
 };
 
-// Plan-time transposition of a right-block operator block: dst[pos][j][c] = src[pos][c][j].
-struct TransposeJob {
-  const double* src;      // [npos][rows][cols]
-  int64_t dst_off;        // element offset inside the plan's transposed-operator buffer
-  int32_t rows, cols, npos, pad;
+// Plan-time padded copy of a block whose stored layout the bulk-tensor engine cannot read (rows not 16-byte
+// aligned): dst[pos][r][c] = src[pos][r][c], leading dimension ld_src -> ld_dst.
+struct CopyJob {
+  const double* src;
+  int64_t dst_off;        // element offset inside the plan's padded-operator buffer
+  int32_t rows, cols, ld_src, ld_dst, npos, pad;
+};
+
+// One Psi sector of the padded private copy the E tiles are read from (psi_pad_kernel, every apply).
+struct PsiPadJob {
+  int64_t src_off, dst_off;
+  int32_t rows, cols, ld_dst, pad;
+};
+
+// Where an operand block of a task lives (resolved to a device pointer by upload_plan).
+struct OperandRef {
+  int32_t kind;           // 0: caller's family memory, 1: plan's padded copy, 2: folded operators, 3: identity blocks
+  int32_t side, fam;      // kind 0: family (side 0 = l, 1 = r)
+  int64_t off;            // element offset inside that buffer
+  int32_t rows, cols, ld; // STORED block: rows x cols, leading dimension ld
+  int32_t npos;           // positions stored (1: the same block for every position)
 };
 
 // Diagonal tasks (s == s') for su2_heff_diag.
@@ -73,7 +92,7 @@ struct DevDiagTask {
   const double* alpha;
   double coef;
   int64_t f_off;
-  int32_t m, p, strideA, strideD, npos, pad;
+  int32_t m, p, strideA, strideD, ldA, ldD, npos, pad;   // pad: index of the full task (host side)
 };
 
 // ---- host-side plan --------------------------------------------------------------------
@@ -84,6 +103,7 @@ struct HostTask {
   int32_t term;
   double coef;
   int32_t m, k, n, p, npos;
+  int32_t wr;             // tile class of the output sector (large-tile plans)
 };
 
 struct PsiSector {
@@ -106,14 +126,18 @@ struct su2_plan {
   bool host_only = false;
   // host images of the device tables
   std::vector<su2::DevTask> h_tasks;
+  std::vector<su2::OperandRef> h_opA, h_opD;   // per task: where its two operator blocks live
+  std::vector<int64_t> h_alpha_off;            // per task: offset into the alpha array, -1: none
+  std::vector<double> h_alpha, h_ident;        // alpha arrays of the rows; identity blocks (padded leading dimension)
+  std::vector<const double*> fam_ptr[2];       // caller's family base pointers (device)
   std::vector<su2::DevUnit> h_units;
   std::vector<su2::DevWork> h_work;
   std::vector<su2::DevReduce> h_reduce;
   std::vector<su2::DevDiagTask> h_diag;
-  std::vector<su2::FoldJob> h_fold;    // plan-time folding jobs
-  std::vector<su2::TransposeJob> h_trans;   // plan-time transposition jobs
-  int64_t trans_elems = 0;
-  int64_t fold_elems = 0;
+  std::vector<su2::FoldJob> h_fold;            // plan-time folding jobs
+  std::vector<su2::CopyJob> h_copy;            // plan-time padded copies
+  std::vector<su2::PsiPadJob> h_psipad;        // per Psi sector: its place in the padded private copy
+  int64_t copy_elems = 0, fold_elems = 0, psipad_elems = 0;
   std::vector<int32_t> h_diag_begin;   // per psi sector: range into h_diag
   // device tables (owned)
   void* d_blob = nullptr;              // one allocation holding everything below
@@ -122,11 +146,15 @@ struct su2_plan {
   su2::DevWork* d_work = nullptr;
   su2::DevReduce* d_reduce = nullptr;
   su2::DevDiagTask* d_diag = nullptr;
+  su2::PsiPadJob* d_psipad = nullptr;
   int32_t* d_diag_begin = nullptr;
   double* d_alpha = nullptr;
   double* d_identity = nullptr;
+  void* d_maps = nullptr;              // CUtensorMap[] of the large-tile kernel (128 bytes each)
+  int32_t nmaps = 0;
   double* d_fold = nullptr;            // folded operators (own allocation, freed with the plan)
-  double* d_trans = nullptr;           // transposed copies of right-block families (own allocation; null if it did not fit)
+  double* d_copy = nullptr;            // padded copies of families whose stored rows are not 16-byte aligned
+  double* d_psi_pad = nullptr;         // padded private copy of Psi (E tiles are bulk-tensor loads from it)
   int32_t* d_counter = nullptr;
   void* d_psi_sec = nullptr;           // device copy of `psi` (PsiSector[])
   int64_t partial_elems = 0;
@@ -136,26 +164,31 @@ struct su2_plan {
 };
 
 namespace su2 {
-// kernels.cu
-su2_status launch_heff_dmma(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream);   // heff_dmma.cu
-// the same kernel on caller-built tables (gemm_pair.cu); counter = zeroed device int
-su2_status launch_heff_dmma_tables(const DevWork* work, int nwork, const DevUnit* units, const DevTask* tasks, const double* psi,
-                                   double* out, double* partial, int* counter, int num_sms, void* stream);
+// heff_tma.cu: the large-tile kernel on a plan, and on caller-built tables (gemm_pair.cu; counter = zeroed device int)
+su2_status launch_heff_tma(const su2_plan* plan, double* out, double* partial, void* stream);
+su2_status launch_heff_tma_tables(const DevWork* work, int nwork, const DevUnit* units, const DevTask* tasks, const void* maps,
+                                  double* out, double* partial, int* counter, int num_sms, void* stream);
+// Tensor maps (tensor_maps.cpp).  box kinds of an operand block stored [npos][rows][ld] (cols valid per row):
+//   cmajor: box {KSX along the columns, CT rows}  -- the block used as stored (k runs along the contiguous direction)
+//   kmajor: box {CT + 4 along the columns, KSX rows} -- the block read transposed
+struct MapKey {
+  const void* base; int32_t rows, cols, ld, nitems; int64_t item_stride; int32_t box_c, box_r;
+  bool operator<(const MapKey& o) const;
+};
+su2_status encode_tensor_map(void* out128, const MapKey& key);   // host; SU2_ERR_CUDA if the driver refuses
 su2_status launch_heff_small(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream);   // heff_small.cu
 su2_status launch_apply(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream);
 su2_status launch_diag(const su2_plan* plan, double* diag, void* stream);
-su2_status upload_plan(su2_plan* plan, const std::vector<double>& alpha_host, const std::vector<double>& ident_host,
-                       const std::vector<int64_t>& alpha_off_of_task, const std::vector<int64_t>& identA_off_of_task,
-                       const std::vector<int64_t>& identD_off_of_task, const std::vector<int64_t>& foldA_off_of_task,
-                       const std::vector<int64_t>& foldD_off_of_task, const std::vector<int64_t>& transD_off_of_task,
-                       void* stream);
+su2_status upload_plan(su2_plan* plan, void* stream);
 void free_plan_device(su2_plan* plan);
+// route 0: automatic; 1: small-block kernel only; 2: fused large-tile kernel only; 3: FP64-FMA tile routine only
 su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double alpha, const double* A, const double* X,
-                            const double* B, double* C, void* stream);
+                            const double* B, double* C, void* stream, int route, int wpi, int nbuf);
 // gemm_pair_small.cu: returns SU2_OK after launching, 1 if the item shape does not fit the small-block kernel
 su2_status launch_gemm_pair_small(int m, int k, int n, int p, int64_t batch, double alpha, const double* A, const double* X,
                                   const double* B, double* C, void* stream, int wpi_force, int nbuf_force);
 void set_cuda_error(const char* what, int code);
+void set_error_text(const char* what);
 void count_launch(int n = 1);   // kernels launched by this library since load (bench.py's gpu_launches)
 // wigner (plan.cpp)
 double wigner6j(int a2, int b2, int c2, int d2, int e2, int f2);

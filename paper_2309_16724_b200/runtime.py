@@ -4,7 +4,7 @@ and the Davidson steps run inside libsu2heff.so; a missing extension or GPU rais
 import numpy as np
 import torch
 
-from .binding import Davidson, Plan, Su2Error, family_elems
+from .binding import Davidson, Plan, Su2Error, family_layout
 
 
 def _require_cuda():
@@ -20,32 +20,40 @@ class HeffOperator:
     generated directly on the device by device_fill(side, index, tensor) (143 GB-class
     workloads cannot be staged through host memory)."""
 
-    def __init__(self, problem, device="cuda:0", device_fill=None, force_split=False, large_tiles=False):
+    def __init__(self, problem, device="cuda:0", device_fill=None, force_split=False, large_tiles=False, ld_align=4):
+        """ld_align: leading dimensions of the operator blocks in device memory are rounded up to this multiple
+        (binding.family_layout).  4 (default) puts every row on a 32-byte boundary, so that the large-tile kernel
+        reads the operators in place with bulk-tensor copies; 1 is the dense layout, of which the plan makes a
+        padded copy when it needs one."""
         _require_cuda()
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
         self.problem = problem
+        self.ld_align = ld_align
         self.family_tensors = {}
+        self.family_layouts = {}
         ptrs = {}
         for side, fams, secs in (("l", problem.fam_l, problem.sec_l), ("r", problem.fam_r, problem.sec_r)):
             for i, f in enumerate(fams):
-                n = family_elems(f, secs)
+                offs, lds, n = family_layout(f, secs, ld_align)
+                self.family_layouts[(side, i)] = (offs, lds)
                 if device_fill is not None:
                     t = torch.empty(max(n, 1), dtype=torch.float64, device=self.device)
-                    device_fill(side, i, t)
+                    device_fill(side, i, t, offs, lds)
                 else:
-                    host = np.concatenate([np.ascontiguousarray(b, dtype=np.float64).ravel() for b in f.data]) \
-                        if len(f.data) else np.zeros(1)
-                    assert host.size == max(n, 1) or n == host.size
+                    host = np.zeros(max(n, 1))
+                    for b, (off, ld) in zip(f.data, zip(offs, lds)):
+                        npos, m, k = b.shape
+                        host[off:off + npos * m * ld].reshape(npos, m, ld)[:, :, :k] = b
                     t = torch.from_numpy(host).to(self.device)
                 self.family_tensors[(side, i)] = t
                 ptrs[(side, i)] = t.data_ptr()
         self.stream = torch.cuda.current_stream(self.device)
         self.plan = Plan(problem, family_ptrs=ptrs, stream=self.stream.cuda_stream, force_split=force_split,
-                         large_tiles=large_tiles)
+                         large_tiles=large_tiles, ld_align=ld_align)
         self.psi_len = self.plan.psi_len
         # workspace: partial tiles + staging for the host entry point
-        self.workspace = torch.empty(self.plan.workspace_bytes + 512 + 16 * self.psi_len, dtype=torch.uint8,
+        self.workspace = torch.empty(self.plan.workspace_bytes + 16 * self.psi_len, dtype=torch.uint8,
                                      device=self.device)
         self.operator_bytes_resident = sum(t.numel() * 8 for t in self.family_tensors.values())
 

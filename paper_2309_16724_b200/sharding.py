@@ -46,7 +46,8 @@ def shard_problem(problem, rank, world):
                 continue
             g = copy.copy(f)
             g.npos = hi - lo
-            g.data = [np.ascontiguousarray(b[lo:hi]) for b in f.data] if f.data is not None else None
+            g.pos0, g.npos_full = lo, f.npos       # where the slice sits in the full family (device-side generators)
+            g.data = [None if b is None else np.ascontiguousarray(b[lo:hi]) for b in f.data] if f.data is not None else None
             out.append(g)
         return out
 

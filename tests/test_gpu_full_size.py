@@ -107,6 +107,6 @@ def test_cfg4_sampled_parity():
     from gen.device_ops import device_block_rows
     torch, prob, op = _setup("cfg4")
     assert op.psi_len == 19728348
-    rows = device_block_rows(prob, op.family_tensors)
+    rows = device_block_rows(prob, op.family_tensors, op.family_layouts)
     worst, _ = _sampled_parity(torch, prob, op, _sector_choice(prob, op, 5), 3, rows, seed=21)
     assert worst <= TOL, worst

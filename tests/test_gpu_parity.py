@@ -58,6 +58,25 @@ def test_synthetic_parity_full_oracle(name, force_split):
     assert _rel(f_gpu, f_ref) <= TOL
 
 
+@pytest.mark.parametrize("ld_align", [1, 2, 4])
+def test_operator_layouts_dense_and_padded(ld_align):
+    """su2_opfamily.blk_ld: the same operator in the dense layout (ld = dim; the plan makes padded copies for the
+    bulk-tensor engine and reports them), with even and with 4-aligned leading dimensions (read in place), through
+    both kernels."""
+    torch = _torch()
+    prob = config_problem("midi")
+    x = random_psi(_operator(prob).psi_len, seed=2)
+    f_ref = oracle_flat(prob, _operator(prob).plan, x)
+    for large in (False, True):
+        op = _operator(prob, ld_align=ld_align, large_tiles=large, force_split=True)
+        f = op.apply(torch.from_numpy(x).cuda()).cpu().numpy()
+        assert _rel(f, f_ref) <= TOL
+        if large:
+            assert (op.info["padded_copy_bytes"] > 0) == (ld_align == 1)
+        d = op.diag().cpu().numpy()
+        assert np.abs(d - _operator(prob).diag().cpu().numpy()).max() <= 1e-13 * np.abs(d).max()
+
+
 @pytest.mark.parametrize("name", ["cfg1", "mini", "midi"])
 def test_small_bonds_through_the_large_tile_kernel(name):
     """Bonds whose sectors all hold <= 48 multiplets plan onto heff_small_kernel; SU2_PLAN_LARGE_TILES keeps them on
