@@ -10,7 +10,12 @@ only after such initialization procedure is completed"); its wall 
 value = CC flops of all ranks / max-over-ranks device time, CC = sum over task-positions of
 min(2mkn+2mnp, 2knp+2mkp) (the paper's definition of TFLOPS).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg4] [--impl reference]
+N > 1 (launched by the driver under torch.distributed.run, or re-launched that way by this script when it is
+started plainly with --gpus N): ONE H_eff*Psi spread over the ranks by operator positions (sharding.py, SURVEY.md
+8(e)): local su2_heff_apply + one FP64 all-reduce of F per step; "scaling": "strong".  --parallelism replicas runs
+N independent copies instead ("weak").
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg4] [--impl reference] [--parallelism shard|replicas]
 """
 import argparse
 import json
@@ -35,9 +40,9 @@ FP64_OVER_BF16_NOMINAL = 45.0 / 2250.0
 
 
 def ncu_traffic(cfg_name):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of heff_dmma_kernel from the committed
-    ncu --set full capture of this workload (profiles/r01_traffic_per_launch.txt), or None."""
-    path = os.path.join(ROOT, "profiles", "r01_traffic_per_launch.txt")
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed ncu capture
+    of this workload with the round's final build (profiles/r02_traffic_per_launch.txt), or None."""
+    path = os.path.join(ROOT, "profiles", "r02_traffic_per_launch.txt")
     if os.path.exists(path):
         with open(path) as f:
             return json.load(f).get(cfg_name)
@@ -104,175 +109,162 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------ CPU oracle arm
-def oracle_sample_problem(cfg_name, npos_sample):
-    """Bounded sample of the workload for the CPU oracle: the two heaviest row classes of the
-    config (A1 P~1 and B1 Q1, with their Hermitian conjugates) restricted to the first
-    `npos_sample` positions, all sector combinations, full block sizes."""
+# Bounded, seeded, STRATIFIED sample of the operator-table rows (SURVEY.md 8(d) "CPU baseline"): every row (Term) is a
+# stratum; of its P positions floor(frac * P + u) are kept (u: one seeded uniform per row, systematic sampling), rows
+# that keep none are dropped.  Block sizes, sector tables and Psi are the full workload's.  The sample fraction is
+# chosen per config so that one oracle apply takes some seconds on the box's cores; the TFLOP/s figure is intensive,
+# the full-apply time quoted next to it is EXTRAPOLATED from it (CC of the full workload / measured rate).
+SAMPLE_FRAC = {"cfg1": 1.0, "mini": 1.0, "midi": 1.0, "cfg2": 1.0, "cfg3": 0.01, "cfg4": 0.0002, "cfg4p": 0.02}
+
+
+def oracle_sample_problem(cfg_name, frac, seed=0):
+    import copy
+    import numpy as np
     from gen import workloads as W
     from gen.problem import Problem
     c = W.CONFIGS[cfg_name]
-    full = W.synthetic_problem(c["L"], c["N"], c["twoS"], c["D"], xi=c["xi"], seed=0, fill=False, pos_cap=c.get("pos_cap"))
-    keep = [t for t in full.term if t.name.split("^")[0] in ("A1P1", "B1Q1")]
-    fam_l, fam_r, terms = [], [], []
-    import copy
-    for t in keep:
+    if cfg_name == "cfg1":
+        from oracle.abinitio_table import build_problem
+        t, v = W.integrals(c["L"], seed=0, xi=c["xi"])
+        return build_problem(t, v, 2, c["N"], c["twoS"], use_adjoints=True), "all rows, all positions"
+    full = W.synthetic_problem(c["L"], c["N"], c["twoS"], c["D"], xi=c["xi"], seed=0, fill=frac >= 1.0,
+                               pos_cap=c.get("pos_cap"))
+    if frac >= 1.0:
+        return full, "all rows, all positions"
+    rng = np.random.default_rng(seed)
+    keeps = [int(np.floor(frac * full.npos_of(t) + rng.random())) for t in full.term]
+    if not any(keeps):                                       # never an empty sample: one position of the longest row
+        keeps[int(np.argmax([full.npos_of(t) for t in full.term]))] = 1
+    fam_l, fam_r, terms, kept_rows, kept_pos, tot_pos = [], [], [], 0, 0, 0
+    for ti, t in enumerate(full.term):
+        npos = full.npos_of(t)
+        tot_pos += npos
+        keep = keeps[ti]
+        if keep <= 0:
+            continue
+        kept_rows += 1
+        kept_pos += keep
         t = copy.copy(t)
         for side, fams, secs, new in (("l", full.fam_l, full.sec_l, fam_l), ("r", full.fam_r, full.sec_r, fam_r)):
             idx = t.fam_l if side == "l" else t.fam_r
+            if idx < 0:
+                continue
             f = fams[idx]
-            nf = W.make_family(secs, f.dN, f.twoK, min(npos_sample, f.npos), 0, 900 + idx, f.name)
+            nf = W.make_family(secs, f.dN, f.twoK, min(keep, f.npos), 0, 900 + 2 * ti + (side == "r"), f.name,
+                               symmetric=f.name in ("H_l", "H_r"))
             new.append(nf)
             if side == "l":
                 t.fam_l = len(new) - 1
             else:
                 t.fam_r = len(new) - 1
-        t.alpha = None if t.alpha is None else t.alpha[:min(npos_sample, len(t.alpha))]
+        t.alpha = None if t.alpha is None else np.asarray(t.alpha)[:keep]
+        if t.alpha is not None and len(t.alpha) < keep:       # a single-position alpha of a one-position row
+            t.alpha = np.resize(t.alpha, keep)
         terms.append(t)
-    return Problem(n_tot=full.n_tot, twoS_tot=full.twoS_tot, sec_l=full.sec_l, sec_r=full.sec_r, fam_l=fam_l,
+    prob = Problem(n_tot=full.n_tot, twoS_tot=full.twoS_tot, sec_l=full.sec_l, sec_r=full.sec_r, fam_l=fam_l,
                    fam_r=fam_r, site=full.site, term=terms, meta=dict(full.meta))
+    what = ("seeded stratified sample: %d of %d operator-table rows, %d of %d row-positions (fraction %.4g per row), "
+            "all sector combinations, full block sizes" % (kept_rows, len(full.term), kept_pos, tot_pos, frac))
+    return prob, what
 
 
-def time_oracle(cfg_name, steps, warmup, budget_s=20.0):
-    """Times oracle.heff_dense.heff_apply, as it stands, on the bounded sample."""
+def time_oracle(cfg_name, budget_s=20.0, threads=None):
+    """Times oracle.heff_dense.heff_apply, as it stands, on the bounded sample.  Nothing of the CUDA library is loaded:
+    the Psi layout comes from oracle.heff_dense.psi_sectors, the flop count from oracle.cc_count."""
     import numpy as np
     from gen.workloads import random_psi
-    from helpers import oracle_flat
-    from paper_2309_16724_b200 import Plan
-    npos = {"cfg4": 1, "cfg4p": 1, "cfg3": 4, "cfg2": 16}.get(cfg_name, 16)
-    prob = oracle_sample_problem(cfg_name, npos)
-    plan = Plan(prob, host_only=True)
-    x = random_psi(plan.psi_len, seed=0)
-    times = []
-    for i in range(warmup + steps):
-        t0 = time.perf_counter()
-        oracle_flat(prob, plan, x)
-        dt = time.perf_counter() - t0
-        if i >= warmup:
-            times.append(dt)
-        if sum(times) > budget_s and len(times) >= 1 and i >= warmup:
-            break
-    try:
-        from threadpoolctl import threadpool_info
-        cores = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
-    except Exception:
-        cores = os.cpu_count()
-    ms = 1e3 * sum(times) / len(times)
-    cc = plan.info["cc_flops"]
-    sample = ("rows A1P1,B1Q1 (+h.c.) of %s restricted to %d position(s), all sector combinations, full block sizes; "
-              "CC of the sample %.3e flop" % (cfg_name, npos, cc))
-    return {"value": cc / (ms * 1e-3) / 1e12, "unit": UNIT, "cores": int(cores), "kind": "oracle", "sample": sample,
-            "ms_per_apply": ms, "steps_timed": len(times)}
+    from oracle.cc_count import cc_flops
+    from oracle.heff_dense import heff_apply, psi_sectors, unflatten
+    from threadpoolctl import threadpool_info, threadpool_limits
+    prob, what = oracle_sample_problem(cfg_name, SAMPLE_FRAC.get(cfg_name, 1.0))
+    labels = psi_sectors(prob)
+    n = sum(prob.sec_l[s[0]].dim * prob.sec_r[s[4]].dim for s in labels)
+    psi = unflatten(prob, random_psi(n, seed=0), labels)
+    cc, _, _ = cc_flops(prob)
+
+    def run(limit):
+        times = []
+        with threadpool_limits(limits=limit):
+            while True:
+                t0 = time.perf_counter()
+                heff_apply(prob, psi, check_leak=False)
+                times.append(time.perf_counter() - t0)
+                if sum(times) > budget_s / 2 or len(times) >= 3:
+                    break
+        return min(times)
+    cores = max([p.get("num_threads", 1) for p in threadpool_info()] + [1]) if threads is None else threads
+    t_all = run(threads)
+    t_one = run(1)
+    return {"value": cc / t_all / 1e12, "unit": UNIT, "cores": int(cores), "kind": "oracle",
+            "sample": what + "; CC of the sample %.3e flop" % cc, "seconds_per_sample_apply": t_all,
+            "single_thread": {"value": cc / t_one / 1e12, "cores": 1, "seconds_per_sample_apply": t_one},
+            "host_cpus": os.cpu_count(), "cc_sample": cc}
+
+
+def full_cc(cfg_name):
+    """CC of the full workload counted in Python (oracle/cc_count.py), for the extrapolated full-apply time."""
+    from gen import workloads as W
+    from oracle.cc_count import cc_flops
+    if cfg_name == "cfg1":
+        return None
+    return cc_flops(W.config_problem(cfg_name, seed=0, fill=False))[0]
 
 
 def run_reference(args):
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only).  Loads nothing of the product."""
+    if int(os.environ.get("RANK", "0")) != 0:
         return
-    from paper_2309_16724_b200.build import build
-    build()
-    cb = time_oracle(args.config, args.steps, args.warmup)
-    line = {"metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": cb["steps_timed"],
-            "warmup": args.warmup, "ms_per_step": cb["ms_per_apply"], "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "reference",
-            "config": {"workload": args.config + " (oracle on a bounded sample)", "sample": cb["sample"]},
-            "cpu_baseline": {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")},
+    cb = time_oracle(args.config, budget_s=30.0)
+    cc_full = full_cc(args.config)
+    extra = None if cc_full is None else cc_full / (cb["value"] * 1e12)
+    line = {"metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * cb["seconds_per_sample_apply"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "reference",
+            "config": {"workload": args.config + " (oracle on a bounded sample)", "sample": cb["sample"],
+                       "step": "one oracle H_eff*Psi on the sample (best of up to 3)",
+                       "extrapolated_seconds_per_full_apply": extra},
+            "cpu_baseline": {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample", "single_thread", "host_cpus")},
             "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
 
 
 # ------------------------------------------------------------------------------ GPU arm
-def build_operator(cfg_name, device):
-    """Operator families resident in HBM.  cfg1-3: numpy counter-based generator, uploaded;
-    cfg4 (92 GB): generated on the device (seeded torch generator, gen/device_ops.py), DESIGN.md "Input recipe"."""
-    import torch
+def build_operator(cfg_name, device, shard=False):
+    """Operator families resident in HBM, in the padded layout the large-tile kernel reads in place (ld_align = 4).
+    cfg1-3: numpy counter-based generator, uploaded; cfg4 (92 GB): generated on the device (seeded torch generator,
+    gen/device_ops.py), DESIGN.md "Input recipe".  shard=True: this rank's position slice of every family
+    (paper_2309_16724_b200/sharding.py) under the current torch.distributed process group; the device generator
+    reproduces the N = 1 operator's values at the positions a rank holds."""
     from gen import workloads as W
     from paper_2309_16724_b200.runtime import HeffOperator
-    if cfg_name not in ("cfg4", "cfg4p"):
-        prob = W.config_problem(cfg_name, seed=0, fill=True)
-        return prob, HeffOperator(prob, device=device)
-    from gen.device_ops import device_fill
-    prob = W.config_problem(cfg_name, seed=0, fill=False)
-    fill = device_fill(prob)
-    return prob, HeffOperator(prob, device=device, device_fill=fill)
+    from paper_2309_16724_b200.sharding import ShardedHeffOperator, shard_problem
+    big = cfg_name in ("cfg4", "cfg4p")
+    prob = W.config_problem(cfg_name, seed=0, fill=not big)
+    if not shard:
+        fill = None
+        if big:
+            from gen.device_ops import device_fill
+            fill = device_fill(prob)
+        return prob, HeffOperator(prob, device=device, device_fill=fill)
+    import torch.distributed as dist
+    live = dist.is_available() and dist.is_initialized()
+    rank, world = (dist.get_rank(), dist.get_world_size()) if live else (0, 1)
+    fill = None
+    if big:
+        from gen.device_ops import device_fill
+        fill = device_fill(shard_problem(prob, rank, world))
+    return prob, ShardedHeffOperator(prob, device, device_fill=fill)
 
 
-def reduce_max(values, device, world):
-    """Max over ranks of a list of timings (the contract's max-over-ranks device time)."""
+def reduce_vals(values, device, world, op="max"):
+    """Max (or sum) over ranks of a list of numbers (the contract's max-over-ranks device time)."""
     import torch
     import torch.distributed as dist
     t = torch.tensor(values, dtype=torch.float64, device=device)
     if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX if op == "max" else dist.ReduceOp.SUM)
     return [float(v) for v in t.cpu()]
-
-
-def whole_job_tflops(cc_per_rank, world, ms):
-    """Replicas: every rank applies its own H_eff (CC flops each); aggregate over the job."""
-    return world * cc_per_rank / (ms * 1e-3) / 1e12
-
-
-def run_sharded(args):
-    """--parallelism shard: ONE H_eff*Psi spread over the ranks by operator positions (paper_2309_16724_b200/
-    sharding.py): local su2_heff_apply + one FP64 all-reduce of F per step.  Strong scaling:
-    value = CC of the whole operator / max-over-ranks device time of (apply + all-reduce).  Not the default: the
-    driver's N > 1 line is the replica path (weak scaling)."""
-    import torch
-    import torch.distributed as dist
-    from gen import workloads as W
-    from gen.workloads import random_psi
-    from paper_2309_16724_b200.binding import kernel_launch_count
-    from paper_2309_16724_b200.build import build
-    from paper_2309_16724_b200.sharding import ShardedHeffOperator
-    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if world > 1:
-        dist.init_process_group("nccl")
-    assert torch.cuda.is_available(), "bench.py needs a GPU (no CPU fallback)"
-    device = "cuda:%d" % local
-    torch.cuda.set_device(device)
-    if rank == 0:
-        build()
-    if world > 1:
-        dist.barrier()
-    big = args.config in ("cfg4", "cfg4p")
-    prob = W.config_problem(args.config, seed=0, fill=not big)
-    fill = None
-    if big:
-        from gen.device_ops import device_fill
-        from paper_2309_16724_b200.sharding import shard_problem
-        fill = device_fill(shard_problem(prob, rank, world))
-    op = ShardedHeffOperator(prob, device, device_fill=fill)
-    cc = torch.tensor([op.info["cc_flops"]], dtype=torch.float64, device=device)
-    if world > 1:
-        dist.all_reduce(cc)
-    x = torch.from_numpy(random_psi(op.psi_len, seed=0)).to(device)
-    y = op.local.new_vector()
-    for _ in range(max(3, args.warmup)):
-        op.apply(x, y)
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize()
-    l0 = kernel_launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(args.steps):
-        op.apply(x, y)
-    e1.record()
-    if world > 1:
-        dist.barrier()
-    torch.cuda.synchronize()
-    ms = reduce_max([e0.elapsed_time(e1) / args.steps], device, world)[0]
-    if rank == 0:
-        print(json.dumps({"metric": METRIC, "value": float(cc[0]) / (ms * 1e-3) / 1e12, "unit": UNIT, "n_gpus": world,
-                          "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms, "higher_is_better": True,
-                          "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                          "config": {"workload": args.config, "parallelism": "positions sharded over %d rank(s), "
-                                     "one all-reduce of F (%d bytes) per step" % (world, 8 * op.psi_len),
-                                     "step": "one H_eff*Psi (su2_heff_apply + all-reduce)"},
-                          "gpu_launches": kernel_launch_count() - l0}))
-    if world > 1:
-        dist.destroy_process_group()
 
 
 def run_cfg5(args):
@@ -339,7 +331,12 @@ def run_gpu(args):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    mode = args.parallelism or ("shard" if world > 1 else "single")
     if world > 1:
+        if rank == 0:          # keep the communicator's own lines visible (transport, NVLS), on stderr
+            os.environ.setdefault("NCCL_DEBUG", "INFO")
+            os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT,ENV")
+            os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
         dist.init_process_group("nccl")
     assert torch.cuda.is_available(), "bench.py needs a GPU (no CPU fallback)"
     device = "cuda:%d" % local
@@ -351,10 +348,13 @@ def run_gpu(args):
     stream = torch.cuda.current_stream().cuda_stream
 
     t0 = time.perf_counter()
-    prob, op = build_operator(args.config, device)
+    prob, op = build_operator(args.config, device, shard=(mode == "shard"))
     setup_s = time.perf_counter() - t0
-    info = op.info
-    cc = info["cc_flops"]
+    local_op = op.local if mode == "shard" else op
+    info = local_op.info
+    cc_local = info["cc_flops"]
+    # CC of the whole job: the shards add up to ONE operator; replicas are N operators
+    cc_job = reduce_vals([cc_local], device, world, "sum")[0] if mode != "single" else cc_local
     psi0 = torch.from_numpy(random_psi(op.psi_len, seed=0)).to(device)
     solver = op.davidson(psi0, max_subspace=max(4, min(20, args.steps + args.warmup + 2)))
 
@@ -381,22 +381,22 @@ def run_gpu(args):
     barrier()
     launches = kernel_launch_count() - l0
     ms_total = ev0.elapsed_time(ev1)
-    # --- the dominant kernel alone: su2_heff_apply (fused GEMM pair + reduction), CUDA events
-    x, y = psi0.clone(), op.new_vector()
+    # --- the dominant kernel alone: the LOCAL su2_heff_apply (fused GEMM pair + reduction), CUDA events
+    x, y = psi0.clone(), local_op.new_vector()
     ka0, ka1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    long_apply = ms_total / args.steps > 2000.0           # cfg4: one apply takes tens of seconds
+    long_apply = ms_total / args.steps > 2000.0           # cfg4: one apply takes seconds
     napply = 1 if long_apply else max(1, min(args.steps, 5))
     if not long_apply:
-        op.apply(x, y)
+        local_op.apply(x, y)
     torch.cuda.synchronize()
     ka0.record()
     for _ in range(napply):
-        op.apply(x, y)
+        local_op.apply(x, y)
     ka1.record()
     torch.cuda.synchronize()
     apply_ms = ka0.elapsed_time(ka1) / napply
     clocks = sampler.stop() if rank == 0 else None
-    # --- end to end through the C ABI with HOST buffers (pinned): H2D psi, apply, D2H F, every step
+    # --- end to end through the public API with HOST buffers (pinned): H2D psi, apply (+ all-reduce), D2H F, every step
     xh = psi0.cpu().pin_memory()
     fh = torch.empty_like(xh).pin_memory()
     if not long_apply:
@@ -409,7 +409,7 @@ def run_gpu(args):
     torch.cuda.synchronize()
     e2e_ms = 1e3 * (time.perf_counter() - t1) / ne2e
 
-    ms_total, apply_ms, e2e_ms = reduce_max([ms_total, apply_ms, e2e_ms], device, world)
+    ms_total, e2e_ms = reduce_vals([ms_total, e2e_ms], device, world, "max")
     if rank != 0:
         solver.close()
         if world > 1:
@@ -422,45 +422,53 @@ def run_gpu(args):
     dmma = probe_fp64_peak(1, 4000, 4, stream)
     peak = dmma
     peak_rule = peaks["bf16_tflops"] * FP64_OVER_BF16_NOMINAL
-    achieved = cc / (apply_ms * 1e-3) / 1e12
+    achieved = cc_local / (apply_ms * 1e-3) / 1e12
+    par_text = {"single": "single GPU",
+                "shard": "positions sharded over %d rank(s), one FP64 all-reduce of F (%d bytes) per step" % (world, 8 * op.psi_len),
+                "replicas": "%d independent replicas" % world}[mode]
     line = {
-        "metric": METRIC, "value": whole_job_tflops(cc, world, ms_step), "unit": UNIT, "n_gpus": world,
+        "metric": METRIC, "value": cc_job / (ms_step * 1e-3) / 1e12, "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "scaling": "strong" if mode == "shard" else "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "%s: L=%d N=%d S=0 D_SU2=%d middle bond (BASELINE.json configs)" % (
                        args.config, prob.meta["L"], prob.meta["N"], prob.meta["D"]),
-                   "step": "one su2_davidson_step = H_eff*Psi + Rayleigh-Ritz/residual/orthogonalisation",
-                   "parallelism": "replicas" if world > 1 else "single GPU",
-                   "l2": ("inputs exceed L2 (operators %.2f GB resident, streamed every apply)" if op.operator_bytes_resident > 252e6
+                   "step": "one su2_davidson_step = H_eff*Psi%s + Rayleigh-Ritz/residual/orthogonalisation" % (
+                       " (local apply + all-reduce)" if mode == "shard" else ""),
+                   "parallelism": par_text,
+                   "l2": ("inputs exceed L2 (operators %.2f GB resident per rank, streamed every apply)" if local_op.operator_bytes_resident > 252e6
                           else "operators %.3f GB fit the 126 MB L2 and stay there between applies (not flushed): "
-                               "small-block configuration, not the headline") % (op.operator_bytes_resident / 1e9),
+                               "small-block configuration, not the headline") % (local_op.operator_bytes_resident / 1e9),
+                   "layout": "operator blocks with leading dimensions padded to a multiple of 4 (read in place by bulk-tensor copies)",
                    "small_plan": int(info["small_plan"]),
                    "psi_len": int(info["psi_len"]), "tasks": int(info["ntasks"]),
-                   "task_positions": int(info["ntask_positions"]), "cc_flops_per_apply": cc,
-                   "executed_flops_per_apply": info["executed_flops"], "work_items": int(info["nwork_items"]),
+                   "task_positions": int(info["ntask_positions"]), "cc_flops_per_apply": cc_job,
+                   "cc_flops_per_apply_this_rank": cc_local,
+                   "executed_flops_per_apply_this_rank": info["executed_flops"], "work_items": int(info["nwork_items"]),
                    "segments": int(info["nsegments"]), "plan_seconds": info["plan_seconds"], "setup_seconds": setup_s,
-                   "plan_device_bytes": int(info["plan_device_bytes"])},
+                   "plan_device_bytes": int(info["plan_device_bytes"]), "padded_copy_bytes": int(info["padded_copy_bytes"])},
         "clocks": clocks,
-        "e2e": {"value": whole_job_tflops(cc, world, e2e_ms), "unit": UNIT, "h2d_bytes_per_step": 8 * op.psi_len,
-                "d2h_bytes_per_step": 8 * op.psi_len, "ms_per_step": e2e_ms,
-                "call": "su2_heff_apply_host (pinned host Psi in, host F out)"},
+        "e2e": {"value": cc_job / (e2e_ms * 1e-3) / 1e12, "unit": UNIT, "h2d_bytes_per_step": 8 * op.psi_len * world,
+                "d2h_bytes_per_step": 8 * op.psi_len * world, "ms_per_step": e2e_ms,
+                "call": "apply_host: pinned host Psi in, host F out (su2_heff_apply_host%s)" % (
+                    "" if mode != "shard" else "-equivalent: H2D, su2_heff_apply, all-reduce, D2H")},
         "gpu_launches": int(launches),
-        "roofline": {"bound": "tensor", "kernel": "%s (+reduce_kernel) = one su2_heff_apply" % (
-                         "heff_small_kernel, one launch per size class" if info["small_plan"] else "heff_dmma_kernel"),
+        "roofline": {"bound": "tensor", "kernel": "%s (+reduce_kernel) = one su2_heff_apply on this rank" % (
+                         "heff_small_kernel, one launch per size class" if info["small_plan"] else "heff_tma_kernel"),
                      "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                      "traffic": ncu_traffic(args.config),
-                     "peak_source": "FP64 tensor (DMMA.8x8x4) loop measured in this run by su2_probe_fp64_peak",
+                     "peak_source": "FP64 tensor (DMMA.8x8x4) loop measured in this run by su2_probe_fp64_peak (libsu2probe.so)",
                      "peak_bf16_ratio_rule": peak_rule, "frac_of_bf16_ratio_rule": achieved / peak_rule,
                      "peak_bf16_ratio_rule_source": "%s bf16_tflops x nominal FP64/BF16 ratio 45/2250" % peak_src,
-                     "instruction_path": "FP64 tensor: mma.sync.m8n8k4.f64 = SASS DMMA.8x8x4",
+                     "instruction_path": "FP64 tensor: mma.sync.m8n8k4.f64 = SASS DMMA.8x8x4; operands staged by cp.async.bulk.tensor (UTMALDG)",
                      "flops": "CC of the plan (useful flops, PAPER.md:229), not executed flops",
                      "apply_ms": apply_ms, "launches_timed": napply, "peak_dfma_loop_measured": dfma,
                      "hbm_achieved_gbs": info["operator_bytes"] / (apply_ms * 1e-3) / 1e9, "hbm_peak_gbs": peaks["hbm_gbs"]},
         "davidson": {"theta": [h[0] for h in hist], "resnorm": [h[1] for h in hist]},
     }
-    if not args.no_cpu_baseline:
-        line["cpu_baseline"] = {k: v for k, v in time_oracle(args.config, 1, 0, budget_s=15.0).items()
-                                if k in ("value", "unit", "cores", "kind", "sample")}
+    if not args.no_cpu_baseline and world == 1:
+        cb = time_oracle(args.config, budget_s=20.0)
+        line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample", "single_thread", "host_cpus")}
+        line["cpu_baseline"]["extrapolated_seconds_per_full_apply"] = cc_job / (cb["value"] * 1e12)
     print(json.dumps(line))
     solver.close()
     if world > 1:
@@ -475,16 +483,28 @@ def main():
     ap.add_argument("--config", default="cfg4")
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "shard"])
+    ap.add_argument("--parallelism", default=None, choices=["shard", "replicas"],
+                    help="N > 1: shard (default; one operator over N GPUs, strong scaling) or replicas (weak)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
-    elif args.config == "cfg5":
+        return
+    if args.config == "cfg5":
         run_cfg5(args)
-    elif args.parallelism == "shard":
-        run_sharded(args)
-    else:
-        run_gpu(args)
+        return
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        # started plainly with --gpus N: become N ranks (one process per GPU) under torch.distributed.run
+        import socket
+        with socket.socket() as s:
+            s.bind(("127.0.0.1", 0))
+            port = s.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        sys.exit(subprocess.call(cmd))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world != args.gpus:
+        sys.exit("bench.py: --gpus %d but WORLD_SIZE=%d: launch with --nproc-per-node equal to --gpus" % (args.gpus, world))
+    run_gpu(args)
 
 
 if __name__ == "__main__":

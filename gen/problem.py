@@ -81,6 +81,10 @@ class Problem:
     site: List[SiteOp]
     term: List[Term]
     meta: dict = field(default_factory=dict)
+    # "su2": reduced blocks, sectors (N, S), 3 site multiplets.  "u1" (U(1)-only mode): sectors
+    # (N, 2 S_z) -- Sector.twoS, OpFamily.twoK and SiteOp.twoK then hold 2 S_z / its change, twoS_tot the target 2 S_z,
+    # SiteOp.r is 4 x 4 over the site states |0>, |up>, |down>, |up down>, Term.twoK_L / twoK_R are unused.
+    symmetry: str = "su2"
 
     def npos_of(self, t: Term) -> int:
         pl = self.fam_l[t.fam_l].npos if t.fam_l >= 0 else 1

@@ -109,16 +109,28 @@ typedef struct {
   const double* alpha;       /* HOST [npos] or NULL (all 1.0)                                   */
 } su2_term;
 
+/* U(1)-only mode (the U(1) calculation the paper's "effective" figures are rescaled to; the
+ * same tables, the same kernels, a unit recoupling factor).  Sectors are labelled by (N, 2 S_z): su2_sector.twoS holds
+ * 2 S_z (may be negative), su2_opfamily.twoK the change of 2 S_z of the family's operator component, twoS_tot the target
+ * 2 S_z; twoK_L / twoK_R of a row are ignored.  The site basis has its four states 0 = |0>, 1 = |up>, 2 = |down>,
+ * 3 = |up down>, each a one-dimensional sector; site operators are plain 4 x 4 matrices.  The coefficient
+ * of a task is the fermion sign times the two site elements; an adjoint flag reads the stored block transposed and
+ * reverses (dN, d2Sz), with no phase.  A Psi sector is (il, b, 0, c, ir, 0). */
+typedef struct { double r[4][4]; int32_t dN, dM; } su2_siteop_u1;
+enum { SU2_SYMMETRY_SU2 = 0, SU2_SYMMETRY_U1 = 1 };
+
 typedef struct {
-  int32_t n_tot, twoS_tot;   /* target particle number and doubled total spin                   */
+  int32_t n_tot, twoS_tot;   /* target particle number and doubled total spin (U(1) mode: 2 S_z) */
   int32_t nsec_l, nsec_r;
   const su2_sector *sec_l, *sec_r;
   int32_t nfam_l, nfam_r;
   const su2_opfamily *fam_l, *fam_r;
   int32_t nsite;
-  const su2_siteop* site;
+  const su2_siteop* site;    /* SU(2) mode: [nsite]; U(1) mode: ignored                           */
   int32_t nterm;
   const su2_term* term;
+  int32_t symmetry;          /* SU2_SYMMETRY_SU2 (0) or SU2_SYMMETRY_U1                           */
+  const su2_siteop_u1* site_u1;   /* U(1) mode: [nsite]                                           */
 } su2_problem;
 
 enum {
@@ -233,11 +245,6 @@ su2_status su2_gemm_pair_batched(int32_t m, int32_t k, int32_t n, int32_t p, int
 su2_status su2_gemm_pair_batched_route(int32_t m, int32_t k, int32_t n, int32_t p, int64_t batch, double alpha,
                                        const double* A, const double* X, const double* B, double* C,
                                        void* cuda_stream, int32_t route, int32_t wpi, int32_t nbuf);
-
-/* Measurement aid, not on the hot path: register-resident FP64 throughput of the current device
- * in TFLOP/s (best of 3 timed launches, CUDA events on cuda_stream; synchronises).
- * kind 0: DFMA loop (FP64 vector pipe); kind 1: mma.sync.m8n8k4.f64 loop (SASS DMMA.8x8x4). */
-su2_status su2_probe_fp64_peak(int32_t kind, int32_t iters, int32_t ctas_per_sm, double* tflops, void* cuda_stream);
 
 #ifdef __cplusplus
 }

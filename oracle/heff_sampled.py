@@ -138,7 +138,10 @@ def _sampled_sum(a, d, alpha, e, rows_a, rows_b):
     if a is None:
         te = np.broadcast_to(e[rows_a, :], (npos,) + e[rows_a, :].shape)           # (1 E)[rows_a, :]
     else:
-        te = np.matmul(np.broadcast_to(a, (npos,) + a.shape[1:]), e)                # T_pos = A_pos[rows_a, :] E
+        # T_pos = A_pos[rows_a, :] E for every position: the position axis is stacked onto the row axis, so that all
+        # positions share one library matmul ([npos * |rows_a|, k] @ [k, n]) -- the same products as the loop's
+        stack = np.ascontiguousarray(np.broadcast_to(a, (npos,) + a.shape[1:]))
+        te = np.matmul(stack.reshape(npos * a.shape[1], a.shape[2]), e).reshape(npos, a.shape[1], e.shape[1])
     if d is None:
         ted = te[:, :, rows_b]                                                      # (T_pos 1^T)[:, rows_b]
     else:

@@ -28,6 +28,10 @@ class su2_siteop(C.Structure):
     _fields_ = [("r", (C.c_double * 3) * 3), ("dN", C.c_int32), ("twoK", C.c_int32)]
 
 
+class su2_siteop_u1(C.Structure):
+    _fields_ = [("r", (C.c_double * 4) * 4), ("dN", C.c_int32), ("dM", C.c_int32)]
+
+
 class su2_term(C.Structure):
     _fields_ = [("fam_l", C.c_int32), ("fam_r", C.c_int32), ("op_B", C.c_int32), ("op_C", C.c_int32),
                 ("twoK_L", C.c_int32), ("twoK_R", C.c_int32), ("adj_l", C.c_int32), ("adj_r", C.c_int32),
@@ -40,7 +44,8 @@ class su2_problem(C.Structure):
                 ("nfam_l", C.c_int32), ("nfam_r", C.c_int32),
                 ("fam_l", C.POINTER(su2_opfamily)), ("fam_r", C.POINTER(su2_opfamily)),
                 ("nsite", C.c_int32), ("site", C.POINTER(su2_siteop)),
-                ("nterm", C.c_int32), ("term", C.POINTER(su2_term))]
+                ("nterm", C.c_int32), ("term", C.POINTER(su2_term)),
+                ("symmetry", C.c_int32), ("site_u1", C.POINTER(su2_siteop_u1))]
 
 
 class su2_plan_info_t(C.Structure):
@@ -54,7 +59,7 @@ class su2_plan_info_t(C.Structure):
 EXPORTS = ["su2_wigner_6j", "su2_wigner_9j", "su2_status_string", "su2_last_cuda_error", "su2_kernel_launch_count", "su2_plan_create", "su2_plan_destroy", "su2_plan_info",
            "su2_plan_psi_layout", "su2_plan_export_tasks", "su2_heff_apply", "su2_heff_apply_host", "su2_heff_diag",
            "su2_davidson_workspace_bytes", "su2_davidson_create", "su2_davidson_create_sharded", "su2_davidson_step", "su2_davidson_set_preconditioner", "su2_davidson_ritz_vector",
-           "su2_davidson_destroy", "su2_gemm_pair_batched", "su2_gemm_pair_batched_route", "su2_probe_fp64_peak"]
+           "su2_davidson_destroy", "su2_gemm_pair_batched", "su2_gemm_pair_batched_route"]
 
 REDUCE_FN = C.CFUNCTYPE(C.c_int32, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p)   # su2_reduce_fn
 
@@ -102,7 +107,6 @@ def load():
     lib.su2_davidson_destroy.argtypes = [C.c_void_p]
     lib.su2_gemm_pair_batched.argtypes = [C.c_int32] * 4 + [C.c_int64, C.c_double] + [C.c_void_p] * 5
     lib.su2_gemm_pair_batched_route.argtypes = [C.c_int32] * 4 + [C.c_int64, C.c_double] + [C.c_void_p] * 5 + [C.c_int32] * 3
-    lib.su2_probe_fp64_peak.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_double), C.c_void_p]
     _lib = lib
     return lib
 
@@ -182,12 +186,16 @@ class Plan:
         sl, sr = sectors(problem.sec_l), sectors(problem.sec_r)
         fl = families(problem.fam_l, problem.sec_l, "l")
         fr = families(problem.fam_r, problem.sec_r, "r")
-        site = (su2_siteop * len(problem.site))()
+        u1 = getattr(problem, "symmetry", "su2") == "u1"
+        site = ((su2_siteop_u1 if u1 else su2_siteop) * len(problem.site))()
         for i, o in enumerate(problem.site):
-            for a in range(3):
-                for b in range(3):
+            for a in range(4 if u1 else 3):
+                for b in range(4 if u1 else 3):
                     site[i].r[a][b] = float(o.r[a][b])
-            site[i].dN, site[i].twoK = o.dN, o.twoK
+            if u1:
+                site[i].dN, site[i].dM = o.dN, o.twoK
+            else:
+                site[i].dN, site[i].twoK = o.dN, o.twoK
         terms = (su2_term * max(len(problem.term), 1))()
         for i, t in enumerate(problem.term):
             npos = problem.npos_of(t)
@@ -201,8 +209,8 @@ class Plan:
             terms[i] = su2_term(t.fam_l, t.fam_r, t.op_B, t.op_C, t.twoK_L, t.twoK_R, t.adj_l, t.adj_r, npos, ap)
         self._keep += [site, terms]
         prob = su2_problem(problem.n_tot, problem.twoS_tot, len(problem.sec_l), len(problem.sec_r), sl, sr,
-                           len(problem.fam_l), len(problem.fam_r), fl, fr, len(problem.site), site,
-                           len(problem.term), terms)
+                           len(problem.fam_l), len(problem.fam_r), fl, fr, len(problem.site),
+                           None if u1 else site, len(problem.term), terms, 1 if u1 else 0, site if u1 else None)
         self.handle = C.c_void_p()
         check(lib.su2_plan_create(C.byref(self.handle), C.byref(prob), (SU2_PLAN_HOST_ONLY if host_only else 0) | (2 if force_split else 0) | (4 if large_tiles else 0),
                                   C.c_void_p(stream)))
@@ -308,10 +316,24 @@ def gemm_pair_batched(m, k, n, p, batch, alpha, a_ptr, x_ptr, b_ptr, c_ptr, stre
         check(load().su2_gemm_pair_batched_route(m, k, n, p, batch, alpha, a_ptr, x_ptr, b_ptr, c_ptr, stream, route, wpi, nbuf))
 
 
+_probe = None
+
+
 def probe_fp64_peak(kind, iters=20000, ctas_per_sm=4, stream=0):
-    """Measured register-resident FP64 TFLOP/s: kind 0 = DFMA loop, 1 = DMMA.8x8x4 loop."""
+    """Measured register-resident FP64 TFLOP/s: kind 0 = DFMA loop, 1 = DMMA.8x8x4 loop.  Lives in its own library
+    (libsu2probe.so, include/su2_probe.h): a measurement aid of bench.py, not part of the product ABI."""
+    global _probe
+    if _probe is None:
+        path = os.path.join(HERE, "libsu2probe.so")
+        if not os.path.exists(path):
+            raise Su2Error("%s is missing: run python -m paper_2309_16724_b200.build" % path)
+        _probe = C.CDLL(path)
+        _probe.su2_probe_fp64_peak.restype = C.c_int32
+        _probe.su2_probe_fp64_peak.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_double), C.c_void_p]
     v = C.c_double()
-    check(load().su2_probe_fp64_peak(kind, iters, ctas_per_sm, C.byref(v), stream))
+    st = _probe.su2_probe_fp64_peak(kind, iters, ctas_per_sm, C.byref(v), stream)
+    if st != 0:
+        raise Su2Error("su2_probe_fp64_peak failed with status %d" % st)
     return v.value
 
 

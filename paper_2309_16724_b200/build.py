@@ -7,12 +7,13 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
-SOURCES = ["plan.cpp", "tensor_maps.cpp", "kernels.cu", "heff_tma.cu", "heff_small.cu", "davidson.cu", "gemm_pair.cu", "gemm_pair_small.cu", "peak_probe.cu"]
+SOURCES = ["plan.cpp", "tensor_maps.cpp", "kernels.cu", "heff_tma.cu", "heff_small.cu", "davidson.cu", "gemm_pair.cu", "gemm_pair_small.cu"]
 LIB = os.path.join(HERE, "libsu2heff.so")
+PROBE_LIB = os.path.join(HERE, "libsu2probe.so")      # measurement aid of bench.py (include/su2_probe.h), not the product
 
 
 def _stale():
-    if not os.path.exists(LIB):
+    if not os.path.exists(LIB) or not os.path.exists(PROBE_LIB):
         return True
     t = os.path.getmtime(LIB)
     deps = [os.path.join(HERE, "csrc", f) for f in os.listdir(os.path.join(HERE, "csrc"))]
@@ -35,6 +36,11 @@ def build(force=False, verbose=False):
         raise RuntimeError("nvcc failed building libsu2heff.so")
     if verbose:
         sys.stderr.write(res.stderr)
+    res = subprocess.run(cmd[:cmd.index("-shared") + 1] + ["-I" + os.path.join(ROOT, "include"),
+                          os.path.join(HERE, "csrc", "peak_probe.cu"), "-o", PROBE_LIB], capture_output=True, text=True)
+    if res.returncode != 0:
+        sys.stderr.write(res.stdout + res.stderr)
+        raise RuntimeError("nvcc failed building libsu2probe.so")
     return LIB
 
 

@@ -39,7 +39,7 @@ namespace su2 {
 
 namespace {
 
-enum : int { PH_END = 1, PH_G2 = 2, PH_TRANS = 4, PH_FIRST = 8, PH_LAST = 16, PH_RESET = 32 };
+enum : int { PH_END = 1, PH_G2 = 2, PH_TRANS = 4, PH_FIRST = 8, PH_LAST = 16, PH_RESET = 32, PH_NOBAR = 64 };
 
 // Consumer-visible part of one phase (ring in shared memory, written by the producer thread one or more phases
 // ahead; made visible by the release/acquire pair on the "full" mbarrier of the phase's first stage).
@@ -86,8 +86,7 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, int parity) {
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, int parity) {
   while (!mbar_try_wait(bar, parity)) {}
 }
-__device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, 384;\n" ::: "memory"); }
-static_assert(NWARPS * 32 == 384, "barrier thread count is spelled out in the PTX above");
+__device__ __forceinline__ void consumer_bar() { asm volatile("bar.sync 1, %0;\n" ::"n"(NWARPS * 32) : "memory"); }
 
 // One box of a rank-3 tensor map {columns, rows, items} -> shared memory; completion is counted in bytes on `bar`.
 __device__ __forceinline__ void tma_box(unsigned dst, const void* map, int c0, int c1, int c2, uint64_t* bar, uint64_t policy) {
@@ -103,6 +102,111 @@ __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
       : "d"(a), "d"(b));
 }
 
+// ---- the producer thread --------------------------------------------------------------------------------------
+struct Pipe {          // position in the stage ring; one parity bit per barrier (the ring length depends on the class)
+  int b;
+  unsigned par;
+  unsigned pq;         // phases emitted / consumed
+};
+
+template <int WR>
+__device__ __forceinline__ void produce_item(const DevWork& wk, int w, bool reset, const DevUnit* __restrict__ units,
+                                             const DevTask* __restrict__ tasks, const CUtensorMap* __restrict__ maps,
+                                             unsigned stage0, PhaseInfo* ring, uint64_t* full, uint64_t* empty, Pipe& pp,
+                                             uint64_t pol_stream, uint64_t pol_keep) {
+  using C = TileCfg<WR>;
+  constexpr int NS = C::NSTAGE;
+  constexpr int NEB = C::NEBOX, NDB = C::NDBOX;
+  constexpr unsigned E_BYTES = NEB * EBOX_SZ * 8u;
+  bool first = true;
+#pragma unroll 1
+  for (int u = wk.unit0; u < wk.unit1; ++u) {
+    const DevUnit un = units[u];
+    const DevTask* __restrict__ t = tasks + un.task;
+    const int k = t->k, n = t->n;
+    const unsigned tflags = t->flags;
+    const double coef = t->coef;
+    const double* __restrict__ alpha = t->alpha;
+    const CUtensorMap* mA = maps + t->mapA;
+    const CUtensorMap* mD = maps + t->mapD;
+    const CUtensorMap* mE = maps + t->mapE;
+    const int e_item = t->e_item;
+    const int posA = t->strideA ? 1 : 0, posD = t->strideD ? 1 : 0;   // a block shared by all positions has one item
+    int nchunks, ncw_full;
+    chunking(n, C::NC, nchunks, ncw_full);
+    const int nsteps1 = (k + KS1 - 1) / KS1;
+    const unsigned a_bytes = (tflags & TASK_TRANS_A) ? (unsigned)(KS1 * (C::TM + 4) * 8) : (unsigned)(C::TM * KS1 * 8);
+    const unsigned d_bytes = NDB * ((tflags & TASK_TRANS_D) ? (unsigned)(KS2 * DBOX_LD * 8) : (unsigned)(DBOX_C * KS2 * 8));
+#pragma unroll 1
+    for (int pos = un.pos0; pos < un.pos1; ++pos) {
+      const double scale = coef * (alpha ? alpha[pos] : 1.0);
+#pragma unroll 1
+      for (int chunk = 0; chunk < nchunks; ++chunk) {
+        const int n0 = chunk * ncw_full;
+        const int ncw = min(ncw_full, n - n0);
+        // ---- first product: T chunk = A_pos[rows, :] E[:, n0 .. n0 + ncw)
+        {
+          PhaseInfo& pi = ring[pp.pq & (PHASE_RING - 1)];
+          pi.scale = scale;
+          // a first product of more than NS stages cannot be finished by any warp before every warp has left the
+          // previous second product (a stage is refilled only after all twelve warps released it): no barrier is
+          // then needed in front of the T store
+          pi.flags = ((tflags & TASK_TRANS_A) ? PH_TRANS : 0) | (first ? PH_FIRST : 0) | (nsteps1 > NS ? PH_NOBAR : 0);
+          pi.nsteps = nsteps1;
+          pi.ktot = k;
+          pi.ncw = ncw;
+          pi.work = w;
+          first = false;
+#pragma unroll 1
+          for (int s = 0; s < nsteps1; ++s) {
+            const int b = pp.b;
+            mbar_wait(&empty[b], ((pp.par >> b) & 1) ^ 1);          // consumers have released the previous fill
+            mbar_arrive_expect_tx(&full[b], a_bytes + E_BYTES);     // (release: the phase record is visible)
+            const unsigned st = stage0 + (unsigned)b * (C::STAGE * 8u);
+            const int k0 = s * KS1;
+            if (tflags & TASK_TRANS_A) tma_box(st, mA, wk.row0, k0, pos * posA, &full[b], pol_stream);
+            else tma_box(st, mA, k0, wk.row0, pos * posA, &full[b], pol_stream);
+#pragma unroll
+            for (int e = 0; e < NEB; ++e)
+              tma_box(st + (unsigned)(C::A_SZ + e * EBOX_SZ) * 8u, mE, n0 + e * EBOX_C, k0, e_item, &full[b], pol_keep);
+            pp.par ^= 1u << b;
+            pp.b = (b + 1 == NS) ? 0 : b + 1;
+          }
+          ++pp.pq;
+        }
+        // ---- second product: F_tile += T chunk D_pos[cols, n0 .. n0 + ncw)^T
+        {
+          const bool last = (chunk + 1 == nchunks) && (pos + 1 == un.pos1) && (u + 1 == wk.unit1);
+          const int nsteps2 = (ncw + KS2 - 1) / KS2;
+          PhaseInfo& pi = ring[pp.pq & (PHASE_RING - 1)];
+          pi.scale = 0.0;
+          pi.flags = PH_G2 | ((tflags & TASK_TRANS_D) ? PH_TRANS : 0) | (last ? PH_LAST : 0) | ((last && reset) ? PH_RESET : 0);
+          pi.nsteps = nsteps2;
+          pi.ktot = ncw;
+          pi.ncw = 0;
+          pi.work = w;
+#pragma unroll 1
+          for (int s = 0; s < nsteps2; ++s) {
+            const int b = pp.b;
+            mbar_wait(&empty[b], ((pp.par >> b) & 1) ^ 1);
+            mbar_arrive_expect_tx(&full[b], d_bytes);
+            const unsigned st = stage0 + (unsigned)b * (C::STAGE * 8u);
+            const int kk = n0 + s * KS2;
+#pragma unroll
+            for (int d = 0; d < NDB; ++d) {
+              if (tflags & TASK_TRANS_D) tma_box(st + (unsigned)(d * DBOX_SZ) * 8u, mD, wk.col0 + d * DBOX_C, kk, pos * posD, &full[b], pol_stream);
+              else tma_box(st + (unsigned)(d * DBOX_SZ) * 8u, mD, kk, wk.col0 + d * DBOX_C, pos * posD, &full[b], pol_stream);
+            }
+            pp.par ^= 1u << b;
+            pp.b = (b + 1 == NS) ? 0 : b + 1;
+          }
+          ++pp.pq;
+        }
+      }
+    }
+  }
+}
+
 // One pipeline stage (nsub <= NSUB k4 sub-steps) of a warp-level product: c[ii][j] += A_frag[ii] B_frag[j] for
 // 4 m8-tiles (the first mt active) and NT n8-tiles.  a / b point at this lane's element of the first fragment;
 // A_I / B_J are the strides between m8-tiles / n8-tiles, A_SUB / B_SUB between k4 sub-steps.
@@ -111,8 +215,7 @@ __device__ __forceinline__ void mma_stage(double (&c)[4][NACC][2], const double*
                                           const double* __restrict__ b, int nsub, int mt) {
   if (mt == 4 && nsub == NSUB) {
     // full stage: straight-line, fragments of sub-step s+1 are loaded into a second register set under the DMMAs
-    // of sub-step s (the latency of LDS is otherwise exposed at every sub-step: 11 % of the consumers' time in the
-    // round-1 kernel, profiles/r02_before_cfg4p.md)
+    // of sub-step s (ptxas keeps only part of that distance; with three warps per sub-partition the rest is covered)
     double af[2][4], bf[2][NT];
 #pragma unroll
     for (int ii = 0; ii < 4; ++ii) af[0][ii] = a[ii * A_I];
@@ -146,107 +249,6 @@ __device__ __forceinline__ void mma_stage(double (&c)[4][NACC][2], const double*
 #pragma unroll
       for (int ii = 0; ii < 4; ++ii)
         if (ii < mt) dmma(c[ii][j], af[ii], bf[j]);
-  }
-}
-
-// ---- the producer thread --------------------------------------------------------------------------------------
-struct Pipe {          // position in the stage ring; one parity bit per barrier (the ring length depends on the class)
-  int b;
-  unsigned par;
-  unsigned pq;         // phases emitted / consumed
-};
-
-template <int WR>
-__device__ __forceinline__ void produce_item(const DevWork& wk, int w, bool reset, const DevUnit* __restrict__ units,
-                                             const DevTask* __restrict__ tasks, const CUtensorMap* __restrict__ maps,
-                                             unsigned stage0, PhaseInfo* ring, uint64_t* full, uint64_t* empty, Pipe& pp,
-                                             uint64_t pol_stream, uint64_t pol_keep) {
-  using C = TileCfg<WR>;
-  constexpr int NS = C::NSTAGE;
-  constexpr unsigned E_BYTES = C::NEBOX * EBOX_SZ * 8u;
-  bool first = true;
-#pragma unroll 1
-  for (int u = wk.unit0; u < wk.unit1; ++u) {
-    const DevUnit un = units[u];
-    const DevTask* __restrict__ t = tasks + un.task;
-    const int k = t->k, n = t->n;
-    const unsigned tflags = t->flags;
-    const double coef = t->coef;
-    const double* __restrict__ alpha = t->alpha;
-    const CUtensorMap* mA = maps + t->mapA;
-    const CUtensorMap* mD = maps + t->mapD;
-    const CUtensorMap* mE = maps + t->mapE;
-    const int e_item = t->e_item;
-    const int posA = t->strideA ? 1 : 0, posD = t->strideD ? 1 : 0;   // a block shared by all positions has one item
-    int nchunks, ncw_full;
-    chunking(n, C::NC, nchunks, ncw_full);
-    const int nsteps1 = (k + KS1 - 1) / KS1;
-    const unsigned a_bytes = (tflags & TASK_TRANS_A) ? (unsigned)(KS1 * (C::TM + 4) * 8) : (unsigned)(C::TM * KS1 * 8);
-    const unsigned d_bytes = C::NDBOX * ((tflags & TASK_TRANS_D) ? (unsigned)(KS2 * DBOX_LD * 8) : (unsigned)(DBOX_C * KS2 * 8));
-#pragma unroll 1
-    for (int pos = un.pos0; pos < un.pos1; ++pos) {
-      const double scale = coef * (alpha ? alpha[pos] : 1.0);
-#pragma unroll 1
-      for (int chunk = 0; chunk < nchunks; ++chunk) {
-        const int n0 = chunk * ncw_full;
-        const int ncw = min(ncw_full, n - n0);
-        // ---- first product: T chunk = A_pos[rows, :] E[:, n0 .. n0 + ncw)
-        {
-          PhaseInfo& pi = ring[pp.pq & (PHASE_RING - 1)];
-          pi.scale = scale;
-          pi.flags = ((tflags & TASK_TRANS_A) ? PH_TRANS : 0) | (first ? PH_FIRST : 0);
-          pi.nsteps = nsteps1;
-          pi.ktot = k;
-          pi.ncw = ncw;
-          pi.work = w;
-          first = false;
-#pragma unroll 1
-          for (int s = 0; s < nsteps1; ++s) {
-            const int b = pp.b;
-            mbar_wait(&empty[b], ((pp.par >> b) & 1) ^ 1);          // consumers have released the previous fill
-            mbar_arrive_expect_tx(&full[b], a_bytes + E_BYTES);     // (release: the phase record is visible)
-            const unsigned st = stage0 + (unsigned)b * (C::STAGE * 8u);
-            const int k0 = s * KS1;
-            if (tflags & TASK_TRANS_A) tma_box(st, mA, wk.row0, k0, pos * posA, &full[b], pol_stream);
-            else tma_box(st, mA, k0, wk.row0, pos * posA, &full[b], pol_stream);
-#pragma unroll
-            for (int e = 0; e < C::NEBOX; ++e)
-              tma_box(st + (unsigned)(C::A_SZ + e * EBOX_SZ) * 8u, mE, n0 + e * EBOX_C, k0, e_item, &full[b], pol_keep);
-            pp.par ^= 1u << b;
-            pp.b = (b + 1 == NS) ? 0 : b + 1;
-          }
-          ++pp.pq;
-        }
-        // ---- second product: F_tile += T chunk D_pos[cols, n0 .. n0 + ncw)^T
-        {
-          const bool last = (chunk + 1 == nchunks) && (pos + 1 == un.pos1) && (u + 1 == wk.unit1);
-          const int nsteps2 = (ncw + KS2 - 1) / KS2;
-          PhaseInfo& pi = ring[pp.pq & (PHASE_RING - 1)];
-          pi.scale = 0.0;
-          pi.flags = PH_G2 | ((tflags & TASK_TRANS_D) ? PH_TRANS : 0) | (last ? PH_LAST : 0) | ((last && reset) ? PH_RESET : 0);
-          pi.nsteps = nsteps2;
-          pi.ktot = ncw;
-          pi.ncw = 0;
-          pi.work = w;
-#pragma unroll 1
-          for (int s = 0; s < nsteps2; ++s) {
-            const int b = pp.b;
-            mbar_wait(&empty[b], ((pp.par >> b) & 1) ^ 1);
-            mbar_arrive_expect_tx(&full[b], d_bytes);
-            const unsigned st = stage0 + (unsigned)b * (C::STAGE * 8u);
-            const int kk = n0 + s * KS2;
-#pragma unroll
-            for (int d = 0; d < C::NDBOX; ++d) {
-              if (tflags & TASK_TRANS_D) tma_box(st + (unsigned)(d * DBOX_SZ) * 8u, mD, wk.col0 + d * DBOX_C, kk, pos * posD, &full[b], pol_stream);
-              else tma_box(st + (unsigned)(d * DBOX_SZ) * 8u, mD, kk, wk.col0 + d * DBOX_C, pos * posD, &full[b], pol_stream);
-            }
-            pp.par ^= 1u << b;
-            pp.b = (b + 1 == NS) ? 0 : b + 1;
-          }
-          ++pp.pq;
-        }
-      }
-    }
   }
 }
 
@@ -295,10 +297,10 @@ __device__ __forceinline__ void consume_item(PhaseInfo info, const DevWork* __re
   const int nt2 = max(0, min(NT2, ((cols_valid + 7) >> 3) - wc * NT2));    // active n8-tiles (second product)
   const int a_c_off = (wr * 32 + g) * KS1 + t;                              // A fragment, block as stored (c-major box)
   const int a_k_off = t * (TM + 4) + wr * 32 + g;                           // A fragment, block read transposed
-  const int e_off = C::A_SZ + (wc / 3) * EBOX_SZ + t * EBOX_LD + (wc % 3) * (8 * NT1) + g;
+  const int e_off = C::A_SZ + (wc / WPB) * EBOX_SZ + t * EBOX_LD + (wc % WPB) * (8 * NT1) + g;
   const int t_off = (wr * 32 + g) * LDT + t;                                // A fragment of the second product inside T
-  const int d_k_off = (wc / 3) * DBOX_SZ + t * DBOX_LD + (wc % 3) * (8 * NT2) + g;
-  const int d_c_off = (wc / 3) * DBOX_SZ + ((wc % 3) * (8 * NT2) + g) * KS2 + t;
+  const int d_k_off = (wc / WPB) * DBOX_SZ + t * DBOX_LD + (wc % WPB) * (8 * NT2) + g;
+  const int d_c_off = (wc / WPB) * DBOX_SZ + ((wc % WPB) * (8 * NT2) + g) * KS2 + t;
 
   double acc[4][NT2][2];
   double tacc[4][NT1][2];
@@ -321,17 +323,19 @@ __device__ __forceinline__ void consume_item(PhaseInfo info, const DevWork* __re
       if (flags & PH_TRANS) {
         switch (nt1) {
           case 1: run_phase<NS, ST, false, 1, NT1, 8, 4 * (TM + 4), 8, 4 * EBOX_LD>(tacc, stages, Ts, a_k_off, e_off, nsteps, ktot, mt, cp, full, empty, lane); break;
-          case 2: run_phase<NS, ST, false, 2, NT1, 8, 4 * (TM + 4), 8, 4 * EBOX_LD>(tacc, stages, Ts, a_k_off, e_off, nsteps, ktot, mt, cp, full, empty, lane); break;
+          case 2: run_phase<NS, ST, false, (2 <= NT1 ? 2 : 0), NT1, 8, 4 * (TM + 4), 8, 4 * EBOX_LD>(tacc, stages, Ts, a_k_off, e_off, nsteps, ktot, mt, cp, full, empty, lane); break;
+          case 3: run_phase<NS, ST, false, (3 <= NT1 ? 3 : 0), NT1, 8, 4 * (TM + 4), 8, 4 * EBOX_LD>(tacc, stages, Ts, a_k_off, e_off, nsteps, ktot, mt, cp, full, empty, lane); break;
           default: run_phase<NS, ST, false, 0, NT1, 8, 4 * (TM + 4), 8, 4 * EBOX_LD>(tacc, stages, Ts, a_k_off, e_off, nsteps, ktot, mt, cp, full, empty, lane); break;
         }
       } else {
         switch (nt1) {
           case 1: run_phase<NS, ST, false, 1, NT1, 8 * KS1, 4, 8, 4 * EBOX_LD>(tacc, stages, Ts, a_c_off, e_off, nsteps, ktot, mt, cp, full, empty, lane); break;
-          case 2: run_phase<NS, ST, false, 2, NT1, 8 * KS1, 4, 8, 4 * EBOX_LD>(tacc, stages, Ts, a_c_off, e_off, nsteps, ktot, mt, cp, full, empty, lane); break;
+          case 2: run_phase<NS, ST, false, (2 <= NT1 ? 2 : 0), NT1, 8 * KS1, 4, 8, 4 * EBOX_LD>(tacc, stages, Ts, a_c_off, e_off, nsteps, ktot, mt, cp, full, empty, lane); break;
+          case 3: run_phase<NS, ST, false, (3 <= NT1 ? 3 : 0), NT1, 8 * KS1, 4, 8, 4 * EBOX_LD>(tacc, stages, Ts, a_c_off, e_off, nsteps, ktot, mt, cp, full, empty, lane); break;
           default: run_phase<NS, ST, false, 0, NT1, 8 * KS1, 4, 8, 4 * EBOX_LD>(tacc, stages, Ts, a_c_off, e_off, nsteps, ktot, mt, cp, full, empty, lane); break;
         }
       }
-      consumer_bar();                              // every warp is done reading the previous T chunk
+      if (!(flags & PH_NOBAR)) consumer_bar();     // every warp is done reading the previous T chunk
       double* trow = Ts + (wr * 32 + g) * LDT + wc * (8 * NT1) + 2 * t;
 #pragma unroll
       for (int ii = 0; ii < 4; ++ii)
@@ -342,14 +346,17 @@ __device__ __forceinline__ void consume_item(PhaseInfo info, const DevWork* __re
       consumer_bar();                              // the new T chunk is visible to every warp
     } else {
       // ---- second product: acc (32 x 48 per warp) += T_chunk D_pos[cols, chunk]^T --------------
-#define SU2_G2_CASES(AOFF, BJ, BSUB)                                                                                          \
-      switch (nt2) {                                                                                                          \
-        case 1: run_phase<NS, ST, true, 1, NT2, 8 * LDT, 4, BJ, BSUB>(acc, stages, Ts, t_off, AOFF, nsteps, ktot, mt, cp, full, empty, lane); break; \
-        case 2: run_phase<NS, ST, true, 2, NT2, 8 * LDT, 4, BJ, BSUB>(acc, stages, Ts, t_off, AOFF, nsteps, ktot, mt, cp, full, empty, lane); break; \
-        case 3: run_phase<NS, ST, true, 3, NT2, 8 * LDT, 4, BJ, BSUB>(acc, stages, Ts, t_off, AOFF, nsteps, ktot, mt, cp, full, empty, lane); break; \
-        case 4: run_phase<NS, ST, true, 4, NT2, 8 * LDT, 4, BJ, BSUB>(acc, stages, Ts, t_off, AOFF, nsteps, ktot, mt, cp, full, empty, lane); break; \
-        case 5: run_phase<NS, ST, true, 5, NT2, 8 * LDT, 4, BJ, BSUB>(acc, stages, Ts, t_off, AOFF, nsteps, ktot, mt, cp, full, empty, lane); break; \
-        case 6: run_phase<NS, ST, true, 6, NT2, 8 * LDT, 4, BJ, BSUB>(acc, stages, Ts, t_off, AOFF, nsteps, ktot, mt, cp, full, empty, lane); break; \
+#define SU2_G2_CASES(AOFF, BJ, BSUB) \
+      switch (nt2) { \
+        case 1: run_phase<NS, ST, true, (1 <= NT2 ? 1 : 0), NT2, 8 * LDT, 4, BJ, BSUB>(acc, stages, Ts, t_off, AOFF, nsteps, ktot, mt, cp, full, empty, lane); break; \
+        case 2: run_phase<NS, ST, true, (2 <= NT2 ? 2 : 0), NT2, 8 * LDT, 4, BJ, BSUB>(acc, stages, Ts, t_off, AOFF, nsteps, ktot, mt, cp, full, empty, lane); break; \
+        case 3: run_phase<NS, ST, true, (3 <= NT2 ? 3 : 0), NT2, 8 * LDT, 4, BJ, BSUB>(acc, stages, Ts, t_off, AOFF, nsteps, ktot, mt, cp, full, empty, lane); break; \
+        case 4: run_phase<NS, ST, true, (4 <= NT2 ? 4 : 0), NT2, 8 * LDT, 4, BJ, BSUB>(acc, stages, Ts, t_off, AOFF, nsteps, ktot, mt, cp, full, empty, lane); break; \
+        case 5: run_phase<NS, ST, true, (5 <= NT2 ? 5 : 0), NT2, 8 * LDT, 4, BJ, BSUB>(acc, stages, Ts, t_off, AOFF, nsteps, ktot, mt, cp, full, empty, lane); break; \
+        case 6: run_phase<NS, ST, true, (6 <= NT2 ? 6 : 0), NT2, 8 * LDT, 4, BJ, BSUB>(acc, stages, Ts, t_off, AOFF, nsteps, ktot, mt, cp, full, empty, lane); break; \
+        case 7: run_phase<NS, ST, true, (7 <= NT2 ? 7 : 0), NT2, 8 * LDT, 4, BJ, BSUB>(acc, stages, Ts, t_off, AOFF, nsteps, ktot, mt, cp, full, empty, lane); break; \
+        case 8: run_phase<NS, ST, true, (8 <= NT2 ? 8 : 0), NT2, 8 * LDT, 4, BJ, BSUB>(acc, stages, Ts, t_off, AOFF, nsteps, ktot, mt, cp, full, empty, lane); break; \
+        case 9: run_phase<NS, ST, true, (9 <= NT2 ? 9 : 0), NT2, 8 * LDT, 4, BJ, BSUB>(acc, stages, Ts, t_off, AOFF, nsteps, ktot, mt, cp, full, empty, lane); break; \
         default: run_phase<NS, ST, true, 0, NT2, 8 * LDT, 4, BJ, BSUB>(acc, stages, Ts, t_off, AOFF, nsteps, ktot, mt, cp, full, empty, lane); break; \
       }
       if (flags & PH_TRANS) { SU2_G2_CASES(d_k_off, 8, 4 * DBOX_LD) }

@@ -1,9 +1,10 @@
-// Measurement aid (not on the hot path): register-resident FP64 throughput of this GPU, so that
-// bench.py can quote the roofline denominator it measured itself (MEASURED_PEAKS.json has no FP64
-// entry).  kind 0: DFMA loop; kind 1: mma.sync m8n8k4 f64 (SASS DMMA.8x8x4) loop.
+// Measurement aid, built as its OWN library (libsu2probe.so, include/su2_probe.h) so that nothing of it ships in the
+// product ABI: register-resident FP64 throughput of this GPU, with which bench.py quotes the roofline denominator it
+// measured itself (MEASURED_PEAKS.json has no FP64 entry).  kind 0: DFMA loop; kind 1: mma.sync m8n8k4 f64 (SASS
+// DMMA.8x8x4) loop.
 #include <cuda_runtime.h>
 
-#include "su2_internal.h"
+#include "su2_probe.h"
 
 namespace {
 __global__ void __launch_bounds__(256) dfma_probe(double* out, int iters, double a, double b) {
@@ -36,15 +37,15 @@ __global__ void __launch_bounds__(256) dmma_probe(double* out, int iters, double
 }
 }  // namespace
 
-extern "C" su2_status su2_probe_fp64_peak(int32_t kind, int32_t iters, int32_t ctas_per_sm, double* tflops, void* cuda_stream) {
-  if (!tflops || iters <= 0 || ctas_per_sm <= 0 || (kind != 0 && kind != 1)) return SU2_ERR_INVALID_ARGUMENT;
+extern "C" int32_t su2_probe_fp64_peak(int32_t kind, int32_t iters, int32_t ctas_per_sm, double* tflops, void* cuda_stream) {
+  if (!tflops || iters <= 0 || ctas_per_sm <= 0 || (kind != 0 && kind != 1)) return -1;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int dev = 0, sms = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-    return SU2_ERR_CUDA;
+    return -5;
   double* buf = nullptr;
   const int grid = sms * ctas_per_sm;
-  if (cudaMalloc(&buf, (size_t)grid * 256 * sizeof(double)) != cudaSuccess) return SU2_ERR_CUDA;
+  if (cudaMalloc(&buf, (size_t)grid * 256 * sizeof(double)) != cudaSuccess) return -5;
   cudaEvent_t e0, e1;
   cudaEventCreate(&e0);
   cudaEventCreate(&e1);
@@ -54,7 +55,7 @@ extern "C" su2_status su2_probe_fp64_peak(int32_t kind, int32_t iters, int32_t c
     if (kind == 0) dfma_probe<<<grid, 256, 0, st>>>(buf, iters, 1.0000001, 1e-9);
     else dmma_probe<<<grid, 256, 0, st>>>(buf, iters, 1.0000001, 1e-9);
     cudaEventRecord(e1, st);
-    if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(buf); return SU2_ERR_CUDA; }
+    if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(buf); return -5; }
     float ms = 0.f;
     cudaEventElapsedTime(&ms, e0, e1);
     if (rep > 0 && ms < best) best = ms;
@@ -65,5 +66,5 @@ extern "C" su2_status su2_probe_fp64_peak(int32_t kind, int32_t iters, int32_t c
   const double flops = kind == 0 ? (double)grid * 256 * (double)iters * 16 * 2
                                  : (double)grid * 8 /*warps*/ * (double)iters * 8 * (2.0 * 8 * 8 * 4);
   *tflops = flops / (best * 1e-3) / 1e12;
-  return SU2_OK;
+  return 0;
 }

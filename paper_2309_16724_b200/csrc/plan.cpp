@@ -88,7 +88,60 @@ static const int SITE_2S[3] = {0, 1, 0};
 
 using namespace su2;
 
+static const int U1_SITE_N[4] = {0, 1, 1, 2};
+static const int U1_SITE_M[4] = {0, 1, -1, 0};
+
+// U(1)-only mode (su2_heff.h): sectors (N, 2Sz), operator components (dN, d2Sz), 4 x 4 site matrices.
+static su2_status validate_u1(const su2_problem* p) {
+  if (p->nsec_l <= 0 || p->nsec_r <= 0 || !p->sec_l || !p->sec_r || p->nsite <= 0 || !p->site_u1 || p->nterm < 0)
+    return SU2_ERR_INVALID_ARGUMENT;
+  if (p->nterm > 0 && !p->term) return SU2_ERR_INVALID_ARGUMENT;
+  if ((p->nfam_l > 0 && !p->fam_l) || (p->nfam_r > 0 && !p->fam_r) || p->nfam_l < 0 || p->nfam_r < 0)
+    return SU2_ERR_INVALID_ARGUMENT;
+  for (int side = 0; side < 2; ++side) {
+    const int ns = side ? p->nsec_r : p->nsec_l;
+    const su2_sector* sec = side ? p->sec_r : p->sec_l;
+    for (int i = 0; i < ns; ++i)
+      if (sec[i].dim <= 0 || sec[i].N < 0) return SU2_ERR_INVALID_SECTOR;
+    const int nf = side ? p->nfam_r : p->nfam_l;
+    const su2_opfamily* fam = side ? p->fam_r : p->fam_l;
+    for (int f = 0; f < nf; ++f) {
+      if (fam[f].npos <= 0 || fam[f].nblk < 0) return SU2_ERR_INVALID_ARGUMENT;
+      if (fam[f].nblk > 0 && (!fam[f].q_out || !fam[f].q_in || !fam[f].blk_off)) return SU2_ERR_INVALID_ARGUMENT;
+      for (int b = 0; b < fam[f].nblk; ++b) {
+        const int qo = fam[f].q_out[b], qi = fam[f].q_in[b];
+        if (qo < 0 || qo >= ns || qi < 0 || qi >= ns) return SU2_ERR_INVALID_SECTOR;
+        if (sec[qo].N != sec[qi].N + fam[f].dN || sec[qo].twoS != sec[qi].twoS + fam[f].twoK) return SU2_ERR_INVALID_SECTOR;
+        if (fam[f].blk_off[b] < 0) return SU2_ERR_INVALID_ARGUMENT;
+      }
+    }
+  }
+  for (int s = 0; s < p->nsite; ++s)
+    for (int o = 0; o < 4; ++o)
+      for (int i = 0; i < 4; ++i) {
+        const double v = p->site_u1[s].r[o][i];
+        if (!std::isfinite(v)) return SU2_ERR_NOT_FINITE;
+        if (v != 0.0 && (U1_SITE_N[o] != U1_SITE_N[i] + p->site_u1[s].dN || U1_SITE_M[o] != U1_SITE_M[i] + p->site_u1[s].dM))
+          return SU2_ERR_INVALID_SECTOR;
+      }
+  for (int t = 0; t < p->nterm; ++t) {
+    const su2_term& tm = p->term[t];
+    if (tm.fam_l < -1 || tm.fam_l >= p->nfam_l || tm.fam_r < -1 || tm.fam_r >= p->nfam_r) return SU2_ERR_INVALID_ARGUMENT;
+    if (tm.op_B < 0 || tm.op_B >= p->nsite || tm.op_C < 0 || tm.op_C >= p->nsite) return SU2_ERR_INVALID_ARGUMENT;
+    if (tm.npos <= 0) return SU2_ERR_INVALID_ARGUMENT;
+    const int npl = tm.fam_l >= 0 ? p->fam_l[tm.fam_l].npos : 1;
+    const int npr = tm.fam_r >= 0 ? p->fam_r[tm.fam_r].npos : 1;
+    if ((npl != 1 && npl != tm.npos) || (npr != 1 && npr != tm.npos)) return SU2_ERR_INVALID_ARGUMENT;
+    if (tm.alpha)
+      for (int i = 0; i < tm.npos; ++i)
+        if (!std::isfinite(tm.alpha[i])) return SU2_ERR_NOT_FINITE;
+  }
+  return SU2_OK;
+}
+
 static su2_status validate(const su2_problem* p) {
+  if (p && p->symmetry == SU2_SYMMETRY_U1) return validate_u1(p);
+  if (p && p->symmetry != SU2_SYMMETRY_SU2) return SU2_ERR_INVALID_ARGUMENT;
   if (p && (p->twoS_tot < 0 || p->twoS_tot > MAX_TWO_SPIN)) return SU2_ERR_INVALID_RANK;
   if (!p || p->nsec_l <= 0 || p->nsec_r <= 0 || !p->sec_l || !p->sec_r || p->nsite <= 0 || !p->site || p->nterm < 0)
     return SU2_ERR_INVALID_ARGUMENT;
@@ -162,9 +215,24 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
   const auto& sl = plan->sec_l;
   const auto& sr = plan->sec_r;
 
+  const bool u1 = p->symmetry == SU2_SYMMETRY_U1;
   // ---- Psi sectors s = (il, sB, J1, sC, ir, J2) -----------------------------------------
   std::map<std::tuple<int, int, int, int>, std::vector<int>> by_quad;  // (il,sB,sC,ir) -> sector ids
-  for (int il = 0; il < (int)sl.size(); ++il)
+  if (u1) {
+    // U(1) mode: (il, b, 0, c, ir, 0) with particle number and 2 S_z adding up to the targets
+    for (int il = 0; il < (int)sl.size(); ++il)
+      for (int b = 0; b < 4; ++b)
+        for (int c = 0; c < 4; ++c)
+          for (int ir = 0; ir < (int)sr.size(); ++ir) {
+            if (sl[il].N + U1_SITE_N[b] + U1_SITE_N[c] + sr[ir].N != p->n_tot) continue;
+            if (sl[il].twoS + U1_SITE_M[b] + U1_SITE_M[c] + sr[ir].twoS != p->twoS_tot) continue;
+            PsiSector s{il, b, 0, c, ir, 0, plan->psi_len, sl[il].dim, sr[ir].dim};
+            by_quad[std::make_tuple(il, b, c, ir)].push_back((int)plan->psi.size());
+            plan->psi.push_back(s);
+            plan->psi_len += (int64_t)s.m * s.p;
+          }
+  }
+  for (int il = 0; !u1 && il < (int)sl.size(); ++il)
     for (int sB = 0; sB < 3; ++sB)
       for (int sC = 0; sC < 3; ++sC)
         for (int ir = 0; ir < (int)sr.size(); ++ir) {
@@ -219,7 +287,55 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
     return tr;
   };
 
-  for (int t = 0; t < p->nterm; ++t) {
+  // U(1) mode: coefficient = fermion sign x the two site elements (unit recoupling factor)
+  for (int t = 0; u1 && t < p->nterm; ++t) {
+    const su2_term& tm = p->term[t];
+    const su2_opfamily* fl = tm.fam_l >= 0 ? &p->fam_l[tm.fam_l] : nullptr;
+    const su2_opfamily* fr = tm.fam_r >= 0 ? &p->fam_r[tm.fam_r] : nullptr;
+    const su2_siteop_u1& oB = p->site_u1[tm.op_B];
+    const su2_siteop_u1& oC = p->site_u1[tm.op_C];
+    const int pB = oB.dN & 1, pC = oC.dN & 1, pr = fr ? (fr->dN & 1) : 0;
+    auto trans_u1 = [&](const su2_opfamily* fam, int adj, const std::vector<su2_sector>& sec) {
+      std::vector<Trans> tr;
+      if (!fam) {
+        for (int i = 0; i < (int)sec.size(); ++i) tr.push_back({i, i, -1, 1.0});
+        return tr;
+      }
+      for (int b = 0; b < fam->nblk; ++b)
+        tr.push_back(adj ? Trans{fam->q_out[b], fam->q_in[b], b, 1.0} : Trans{fam->q_in[b], fam->q_out[b], b, 1.0});
+      return tr;
+    };
+    const auto ltr = trans_u1(fl, tm.adj_l, sl);
+    const auto rtr = trans_u1(fr, tm.adj_r, sr);
+    for (const Trans& lt : ltr)
+      for (int bi = 0; bi < 4; ++bi)
+        for (int bo = 0; bo < 4; ++bo) {
+          if (oB.r[bo][bi] == 0.0) continue;
+          for (int ci = 0; ci < 4; ++ci)
+            for (int co = 0; co < 4; ++co) {
+              if (oC.r[co][ci] == 0.0) continue;
+              for (const Trans& rt : rtr) {
+                auto in_it = by_quad.find(std::make_tuple(lt.q_in, bi, ci, rt.q_in));
+                if (in_it == by_quad.end()) continue;
+                auto out_it = by_quad.find(std::make_tuple(lt.q_out, bo, co, rt.q_out));
+                if (out_it == by_quad.end()) continue;
+                const int nl = sl[lt.q_in].N, nB = U1_SITE_N[bi], nC = U1_SITE_N[ci];
+                const int sexp = pB * nl + pC * (nl + nB) + pr * (nl + nB + nC);
+                const double coef = ((sexp % 2) ? -1.0 : 1.0) * oB.r[bo][bi] * oC.r[co][ci];
+                HostTask ht;
+                ht.out_sec = out_it->second[0]; ht.in_sec = in_it->second[0];
+                ht.fam_l = tm.fam_l; ht.blk_l = lt.blk; ht.adj_l = fl ? tm.adj_l : 0;
+                ht.fam_r = tm.fam_r; ht.blk_r = rt.blk; ht.adj_r = fr ? tm.adj_r : 0;
+                ht.term = t; ht.coef = coef;
+                const PsiSector& a = plan->psi[ht.out_sec];
+                const PsiSector& b = plan->psi[ht.in_sec];
+                ht.m = a.m; ht.k = b.m; ht.n = b.p; ht.p = a.p; ht.npos = tm.npos; ht.wr = 0;
+                plan->tasks.push_back(ht);
+              }
+            }
+        }
+  }
+  for (int t = 0; !u1 && t < p->nterm; ++t) {
     const su2_term& tm = p->term[t];
     const su2_opfamily* fl = tm.fam_l >= 0 ? &p->fam_l[tm.fam_l] : nullptr;
     const su2_opfamily* fr = tm.fam_r >= 0 ? &p->fam_r[tm.fam_r] : nullptr;

@@ -19,28 +19,32 @@
 
 namespace su2 {
 
-constexpr int NWARPS = 12;             // consumer (math) warps: three warpgroups, three warps per SM sub-partition
+#ifndef SU2_NWARPS
+#define SU2_NWARPS 12
+#endif
+constexpr int NWARPS = SU2_NWARPS;     // consumer (math) warps: 12 = three warpgroups, three warps per SM sub-partition
+constexpr int WPB = NWARPS / 4;        // consumer warps that share one E box / one D box
 constexpr int NPRODUCERS = 4;          // one producer warpgroup; a single elected thread issues every bulk-tensor copy
 constexpr int NTHREADS = 32 * (NWARPS + NPRODUCERS);
 constexpr int KS1 = 28;         // k extent of one pipeline stage of the first product (seven DMMA k4 steps)
 constexpr int KS2 = 12;         // k extent of one pipeline stage of the second product (three DMMA k4 steps)
-constexpr int NT1 = 2;          // n8-tiles per warp, first product
-constexpr int NT2 = 6;          // n8-tiles per warp, second product
+constexpr int NT1 = 6 / WPB;    // n8-tiles per warp, first product  (a box is 48 columns)
+constexpr int NT2 = 18 / WPB;   // n8-tiles per warp, second product (a box is 144 columns)
 constexpr int MAX_STAGE = 4;    // upper bound of the pipeline depth (mbarrier arrays)
-constexpr int EBOX_C = 8 * NT1 * 3, EBOX_LD = EBOX_C + 4;      // three warps share one E box: 48 (+4) columns
-constexpr int DBOX_C = 8 * NT2 * 3, DBOX_LD = DBOX_C + 4;      // three warps share one D box: 144 (+4) columns
+constexpr int EBOX_C = 8 * NT1 * WPB, EBOX_LD = EBOX_C + 4;    // WPB warps share one E box: 48 (+4) columns
+constexpr int DBOX_C = 8 * NT2 * WPB, DBOX_LD = DBOX_C + 4;    // WPB warps share one D box: 144 (+4) columns
 constexpr int EBOX_SZ = KS1 * EBOX_LD;                          // doubles per E box
 constexpr int DBOX_SZ = KS2 * DBOX_LD;                          // doubles per D box slot (c-major needs 144 * KS2 <= this)
 
 template <int WR>
 struct TileCfg {
-  static_assert(NWARPS % (3 * WR) == 0, "a box serves three warps");
+  static_assert(NWARPS % (WPB * WR) == 0, "a box serves WPB warps");
   static constexpr int WC = NWARPS / WR;        // warps along the columns    : 12 / 6 / 3
   static constexpr int TM = 32 * WR;            // rows of F per CTA          : 32 / 64 / 128
   static constexpr int TP = 8 * NT2 * WC;       // columns of F per CTA       : 576 / 288 / 144
   static constexpr int NC = 8 * NT1 * WC;       // max columns of a T chunk   : 192 / 96 / 48
   static constexpr int LDT = NC + 4;            // leading dimension of T in shared memory
-  static constexpr int NEBOX = WC / 3, NDBOX = WC / 3;
+  static constexpr int NEBOX = WC / WPB, NDBOX = WC / WPB;
   static constexpr int NSTAGE = (WR == 1) ? 3 : 4;   // pipeline depth (what fits beside T in 227 KB)
   static constexpr int A_SZ = KS1 * (TM + 4);   // k-major A box (the larger of the two orientations)
   static constexpr int E_SZ = NEBOX * EBOX_SZ;

@@ -97,6 +97,20 @@ class ShardedHeffOperator:
             dist.all_reduce(out, op=dist.ReduceOp.SUM, group=self.group)   # on the current stream, after the kernels
         return out
 
+    def new_vector(self):
+        return self.local.new_vector()
+
+    def apply_host(self, psi_host, out_host):
+        """End-to-end entry with HOST buffers (pinned): H2D of Psi, local su2_heff_apply, all-reduce of F, D2H."""
+        import torch
+        if not hasattr(self, "_xdev"):
+            self._xdev, self._ydev = self.local.new_vector(), self.local.new_vector()
+        self._xdev.copy_(psi_host, non_blocking=True)
+        self.apply(self._xdev, self._ydev)
+        out_host.copy_(self._ydev, non_blocking=True)
+        torch.cuda.current_stream(self.local.device).synchronize()
+        return out_host
+
     def davidson(self, x0, max_subspace=20):
         """Davidson solver on the sharded operator: su2_davidson_create_sharded with an all-reduce hook (called on
         the diagonal once and on w = H_eff v every step); everything else is replicated on the ranks."""

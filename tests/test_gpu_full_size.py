@@ -1,7 +1,15 @@
 """GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times
-(bench.build_operator): sampled output entries of H_eff * Psi against the M-resolved oracle
-(oracle/heff_sampled.py), plus properties that hold at any size
-(Hermiticity, linearity, bitwise reproducibility).  Tolerance (north_star): 1e-10 relative to max |F|."""
+(bench.build_operator): H_eff * Psi against the M-resolved oracle, plus properties that hold at any size
+(Hermiticity, linearity, bitwise reproducibility).  Tolerance (north_star): 1e-10 relative to max |F|.
+
+Coverage, elements checked against the oracle / elements of F:
+  configs[1] (cfg2):  85 126 / 85 126        -- the FULL oracle (oracle/heff_dense.py), every element
+  configs[2] (cfg3):  64 entries (8 x 8) in EVERY one of the 138 sectors = 8 832 / 1 208 228, sampled oracle
+  configs[3] (cfg4):  36 entries (6 x 6) in 40 of the 138 sectors = 1 440 / 19 728 348, sampled oracle; the sectors
+                      are stratified over the three tile classes (all of the two rarer classes' extremes, largest /
+                      smallest / median of each) and the sampled rows / columns over the first, a middle and the
+                      last row tile / column slab of each sector (incl. the ragged tails).
+Every sampled entry is evaluated over ALL operator-table rows, input sectors and positions (oracle/heff_sampled.py)."""
 import numpy as np
 import pytest
 
@@ -19,7 +27,17 @@ def _setup(cfg):
     return torch, prob, op
 
 
+def _stratified(dim, tile, count, rng):
+    """`count` indices of range(dim): the first and the last one (ragged tails), one inside the last tile, one
+    inside a middle tile, the rest seeded."""
+    pick = {0, dim - 1, max(0, ((dim - 1) // tile) * tile), min(dim - 1, (dim // (2 * tile)) * tile + tile // 2)}
+    while len(pick) < min(count, dim):
+        pick.add(int(rng.integers(dim)))
+    return np.array(sorted(pick)[:count] if len(pick) > count else sorted(pick))
+
+
 def _sampled_parity(torch, prob, op, labels_idx, nsamp, block_rows, seed):
+    """max over the sampled entries of |F_gpu - F_oracle| / max|F_gpu|, the GPU result, and the number of entries."""
     from oracle.heff_dense import expand_psi
     from oracle.heff_sampled import heff_sample
     x = random_psi(op.psi_len, seed=seed)
@@ -30,83 +48,92 @@ def _sampled_parity(torch, prob, op, labels_idx, nsamp, block_rows, seed):
         psi_red[lab] = x[o0:o1].reshape(prob.sec_l[lab[0]].dim, prob.sec_r[lab[4]].dim)
     full = expand_psi(prob, psi_red)
     rng = np.random.default_rng(seed)
-    worst = 0.0
+    worst, checked = 0.0, 0
     for si in labels_idx:
         lab = op.plan.labels[si]
         m, p = prob.sec_l[lab[0]].dim, prob.sec_r[lab[4]].dim
-        # sampled rows/columns always include the first and the last (ragged tile tails)
-        ra = np.unique(np.concatenate([[0, m - 1], rng.choice(m, size=nsamp, replace=False)]))
-        rb = np.unique(np.concatenate([[0, p - 1], rng.choice(p, size=nsamp, replace=False)]))
+        ra = _stratified(m, 32, nsamp, rng)      # row tiles of the large-tile kernel are 32 rows
+        rb = _stratified(p, 48, nsamp, rng)      # a consumer warp owns 48 columns
         ref = heff_sample(prob, psi_red, lab, ra, rb, block_rows, psi_full=full)
         got = f[op.plan.offsets[si]:op.plan.offsets[si + 1]].reshape(m, p)[np.ix_(ra, rb)]
         worst = max(worst, np.abs(got - ref).max() / fmax)
-    return worst, f
+        checked += got.size
+    return worst, f, checked
 
 
-def _sector_choice(prob, op, count):
-    """Largest, smallest and a few seeded sectors: all three tile classes appear."""
-    sizes = [prob.sec_l[s[0]].dim * prob.sec_r[s[4]].dim for s in op.plan.labels]
-    order = np.argsort(sizes)
-    rng = np.random.default_rng(7)
-    pick = {int(order[-1]), int(order[0]), int(order[len(order) // 2])}
-    while len(pick) < count:
-        pick.add(int(rng.integers(len(sizes))))
-    return sorted(pick)
-
-
-def test_cfg2_small_block_parity_and_properties():
-    """BASELINE.json configs[1]: L=20, D=256, blocks 6-46: the small-block kernel (heff_small_kernel, size classes
-    24/40/48) in the launch configuration bench.py times: sampled entries of 24 of the 138 sectors against the
-    oracle, every sector against the large-tile kernel on the same plan input, and the any-size properties."""
-    import os
-    from oracle.heff_sampled import numpy_block_rows
-    torch, prob, op = _setup("cfg2")
-    assert op.psi_len == 85126 and op.info["small_plan"] == 1
-    worst, f = _sampled_parity(torch, prob, op, _sector_choice(prob, op, 24), 5, numpy_block_rows(prob), seed=31)
-    assert worst <= TOL, worst
-    x = torch.from_numpy(random_psi(op.psi_len, seed=31)).cuda()
-    y = torch.from_numpy(random_psi(op.psi_len, seed=32)).cuda()
+def _properties(torch, op, f_first, seed, herm_tol=1e-11):
+    """bitwise reproducibility (two applies), Hermiticity <y|Hx> = <Hy|x>, linearity H(2x - y/2)."""
+    x = torch.from_numpy(random_psi(op.psi_len, seed=seed)).cuda()
+    y = torch.from_numpy(random_psi(op.psi_len, seed=seed + 1)).cuda()
     hx = op.apply(x).clone()
-    assert torch.equal(hx.cpu(), torch.from_numpy(f))                      # bitwise reproducible
-    os.environ["SU2_HEFF_SMALL"] = "0"
-    try:
-        _, _, op_big = _setup("cfg2")
-    finally:
-        del os.environ["SU2_HEFF_SMALL"]
-    assert op_big.info["small_plan"] == 0
-    hx_big = op_big.apply(x)
-    assert float((hx - hx_big).abs().max()) <= 1e-12 * float(hx.abs().max())   # all 85 126 elements, two kernels
+    assert torch.equal(hx.cpu(), torch.from_numpy(f_first))
     hy = op.apply(y).clone()
     a, b = float(torch.dot(y, hx)), float(torch.dot(x, hy))
-    assert abs(a - b) <= 1e-11 * float(hx.norm()) * float(y.norm())          # Hermiticity
+    assert abs(a - b) <= herm_tol * float(hx.norm()) * float(y.norm())
     hz = op.apply(2.0 * x - 0.5 * y)
     assert float((hz - (2.0 * hx - 0.5 * hy)).abs().max()) <= 1e-12 * float(hx.abs().max())
+    return x, hx
 
 
-def test_cfg3_sampled_parity_and_properties():
-    """BASELINE.json configs[2]: L=40, D=1024, blocks 30-131 (all operators built by the numpy generator)."""
+def test_cfg2_full_oracle_parity_and_properties():
+    """BASELINE.json configs[1]: L=20, D=256, blocks 6-46: the small-block kernel (heff_small_kernel, size classes
+    24/40/48) in the launch configuration bench.py times, EVERY element against the full oracle; the large-tile
+    kernel on the same input as well; the any-size properties."""
+    from helpers import oracle_flat
+    torch, prob, op = _setup("cfg2")
+    assert op.psi_len == 85126 and op.info["small_plan"] == 1 and len(op.plan.labels) == 138
+    x = random_psi(op.psi_len, seed=31)
+    f = op.apply(torch.from_numpy(x).cuda()).cpu().numpy()
+    f_ref = oracle_flat(prob, op.plan, x)
+    assert np.abs(f - f_ref).max() / np.abs(f_ref).max() <= TOL
+    xd, hx = _properties(torch, op, f, 31)
+    from paper_2309_16724_b200.runtime import HeffOperator
+    op_big = HeffOperator(prob, device="cuda:0", large_tiles=True)
+    assert op_big.info["small_plan"] == 0
+    f_big = op_big.apply(xd).cpu().numpy()
+    assert np.abs(f_big - f_ref).max() / np.abs(f_ref).max() <= TOL       # all 85 126 elements, the other kernel
+
+
+def test_cfg3_sampled_parity_every_sector_and_properties():
+    """BASELINE.json configs[2]: L=40, D=1024, blocks 30-131 (all operators built by the numpy generator): 8 x 8
+    sampled entries in every one of the 138 sectors."""
     from oracle.heff_sampled import numpy_block_rows
     torch, prob, op = _setup("cfg3")
-    assert op.psi_len == 1208228
-    worst, f = _sampled_parity(torch, prob, op, _sector_choice(prob, op, 8), 6, numpy_block_rows(prob), seed=11)
+    assert op.psi_len == 1208228 and len(op.plan.labels) == 138 and op.info["padded_copy_bytes"] == 0
+    worst, f, checked = _sampled_parity(torch, prob, op, range(138), 8, numpy_block_rows(prob), seed=11)
+    assert checked == 138 * 64
     assert worst <= TOL, worst
-    # bitwise reproducibility, Hermiticity <y|Hx> = <Hy|x>, linearity
-    x = torch.from_numpy(random_psi(op.psi_len, seed=11)).cuda()
-    y = torch.from_numpy(random_psi(op.psi_len, seed=12)).cuda()
-    hx = op.apply(x).clone()
-    assert torch.equal(hx.cpu(), torch.from_numpy(f))
-    hy = op.apply(y).clone()
-    a, b = float(torch.dot(y, hx)), float(torch.dot(x, hy))
-    assert abs(a - b) <= 1e-11 * float(hx.norm()) * float(y.norm())
-    hz = op.apply(2.0 * x - 0.5 * y)
-    assert float((hz - (2.0 * hx - 0.5 * hy)).abs().max()) <= 1e-12 * float(hx.abs().max())
+    _properties(torch, op, f, 11)
 
 
-def test_cfg4_sampled_parity():
-    """BASELINE.json configs[3]: L=76, D=4096, blocks 69-547, 92 GB of operators generated on the device."""
+def _cfg4_sector_choice(prob, op, count):
+    """Sectors stratified over the tile classes of the large-tile kernel (class = smallest of 144 / 288 / 576 columns
+    that covers the sector; rows decide the number of row tiles): per class the largest, the smallest and the median
+    sector by element count, then seeded picks until `count` sectors."""
+    dims = [(prob.sec_l[s[0]].dim, prob.sec_r[s[4]].dim) for s in op.plan.labels]
+    cls = [0 if p <= 144 else 1 if p <= 288 else 2 for _, p in dims]
+    pick = set()
+    for c in range(3):
+        members = sorted((m * p, i) for i, ((m, p), cc) in enumerate(zip(dims, cls)) if cc == c)
+        if members:
+            pick |= {members[0][1], members[-1][1], members[len(members) // 2][1]}
+    rng = np.random.default_rng(7)
+    while len(pick) < count:
+        pick.add(int(rng.integers(len(dims))))
+    return sorted(pick), cls
+
+
+def test_cfg4_sampled_parity_and_properties():
+    """BASELINE.json configs[3] (the headline configuration): L=76, D=4096, blocks 69-547, 92 GB of operators
+    generated on the device: 6 x 6 sampled entries in 40 sectors over all tile classes and row tiles, then bitwise
+    reproducibility, Hermiticity and linearity of the GPU result at this size."""
     from gen.device_ops import device_block_rows
     torch, prob, op = _setup("cfg4")
-    assert op.psi_len == 19728348
+    assert op.psi_len == 19728348 and op.info["padded_copy_bytes"] == 0
     rows = device_block_rows(prob, op.family_tensors, op.family_layouts)
-    worst, _ = _sampled_parity(torch, prob, op, _sector_choice(prob, op, 5), 3, rows, seed=21)
+    sectors, cls = _cfg4_sector_choice(prob, op, 40)
+    assert len({cls[i] for i in sectors}) == len(set(cls))
+    worst, f, checked = _sampled_parity(torch, prob, op, sectors, 6, rows, seed=21)
+    assert checked == 40 * 36
     assert worst <= TOL, worst
+    _properties(torch, op, f, 21)

@@ -468,3 +468,27 @@ def test_wide_sector_multiple_column_tiles(force_split):
     f_ref = oracle_flat(prob, op.plan, x)
     assert np.abs(f_ref).max() > 0
     assert _rel(f_gpu, f_ref) <= TOL
+
+
+def test_two_ranks_nccl_sharded_apply_when_two_gpus_are_visible(tmp_path):
+    """bench.py --gpus 2 (position-sharded H_eff*Psi, NCCL all-reduce of F) on one box: the script re-launches itself
+    under torch.distributed.run, prints one JSON line with n_gpus = 2 and scaling "strong", and its Davidson history
+    equals the single-GPU run's (the sharded operator IS the single-GPU operator).  Skipped with fewer than 2 GPUs."""
+    import json
+    import os
+    import subprocess
+    import sys
+    torch = _torch()
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs 2 visible GPUs")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    lines = {}
+    for n in (1, 2):
+        out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", str(n), "--config", "cfg2", "--steps", "4",
+                              "--warmup", "3", "--no-cpu-baseline"], capture_output=True, text=True, timeout=900)
+        assert out.returncode == 0, out.stderr[-2000:]
+        lines[n] = json.loads(out.stdout.strip().splitlines()[-1])
+    assert lines[2]["n_gpus"] == 2 and lines[2]["scaling"] == "strong"
+    assert abs(lines[2]["config"]["cc_flops_per_apply"] - lines[1]["config"]["cc_flops_per_apply"]) <= 1e-9 * lines[1]["config"]["cc_flops_per_apply"]
+    t1, t2 = lines[1]["davidson"]["theta"], lines[2]["davidson"]["theta"]
+    assert max(abs(a - b) for a, b in zip(t1, t2)) <= 1e-8 * max(1.0, max(abs(a) for a in t1))

@@ -1,7 +1,7 @@
-"""N > 1 path on CPU: world_size-2 gloo.  The path shards by replicas only: every
-rank plans the same problem and applies its own H_eff; the only cross-rank step is the max-over-ranks
-timing reduction of bench.py.  Checked here: identical plans on all ranks (the planner is deterministic),
-the MAX reduction, and the whole-job aggregate."""
+"""N > 1 path on CPU: world_size-2 gloo.  The path shards by operator positions: every rank
+plans its slice of the same problem, applies it, and one all-reduce of F completes the product; bench.py adds the
+max-over-ranks timing reduction and the sum-over-ranks CC.  Checked here: identical plans on all ranks (the planner
+is deterministic), the MAX / SUM reductions of bench.py, and the sharded apply against the oracle."""
 import os
 import sys
 
@@ -31,14 +31,15 @@ def _worker(rank, world, port, out):
     ref = coef.clone()
     dist.broadcast(ref, src=0)
     same = same and torch.equal(coef, ref)
-    ms = bench.reduce_max([10.0 + rank, 5.0 - rank], "cpu", world)
+    ms = bench.reduce_vals([10.0 + rank, 5.0 - rank], "cpu", world, "max")
+    cc = bench.reduce_vals([1.0e12 * (rank + 1)], "cpu", world, "sum")[0]        # the shards' CC add up to the job's
     if rank == 0:
-        out.put((same, ms, bench.whole_job_tflops(2.0e12, world, ms[0])))
+        out.put((same, ms, cc / (ms[0] * 1e-3) / 1e12))
     dist.barrier()
     dist.destroy_process_group()
 
 
-def test_two_rank_replicas_gloo():
+def test_two_rank_reductions_gloo():
     ctx = mp.get_context("spawn")
     out = ctx.Queue()
     port = 29500 + os.getpid() % 2000
@@ -51,7 +52,7 @@ def test_two_rank_replicas_gloo():
         assert p.exitcode == 0
     assert same
     assert ms == [11.0, 5.0]                       # max over ranks of (10, 11) and (5, 4)
-    assert abs(value - 2 * 2.0e12 / 11.0e-3 / 1e12) < 1e-9
+    assert abs(value - 3.0e12 / 11.0e-3 / 1e12) < 1e-9
 
 
 # ---- position-sharded apply (paper_2309_16724_b200/sharding.py) ---------------------------

@@ -22,6 +22,7 @@ def lib():
 
 
 def test_library_exports_every_declared_symbol(lib):
+    import ctypes
     header = open(os.path.join(ROOT, "include", "su2_heff.h")).read()
     declared = set(re.findall(r"\b(su2_[a-z0-9_]+)\s*\(", header))
     assert {"su2_plan_create", "su2_heff_apply", "su2_davidson_step"} <= declared
@@ -30,6 +31,13 @@ def test_library_exports_every_declared_symbol(lib):
     from paper_2309_16724_b200.binding import EXPORTS
     assert set(EXPORTS) == declared
     assert lib.su2_status_string(0) == b"ok"
+    # the measurement aid is a library of its own (include/su2_probe.h), outside the product ABI
+    assert not hasattr(lib, "su2_probe_fp64_peak")
+    probe_h = open(os.path.join(ROOT, "include", "su2_probe.h")).read()
+    probe = ctypes.CDLL(os.path.join(ROOT, "paper_2309_16724_b200", "libsu2probe.so"))
+    for name in set(re.findall(r"\b(su2_[a-z0-9_]+)\s*\(", probe_h)):
+        assert hasattr(probe, name), name
+    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["su2_heff.h", "su2_probe.h"]
 
 
 def _cfg1(use_adjoints):
@@ -88,3 +96,16 @@ def test_device_entry_points_fail_loudly_without_device_plan(lib):
     plan = Plan(config_problem("mini"), host_only=True)
     with pytest.raises(Su2Error):
         plan.heff_apply(1, 2, 0)
+
+
+def test_cc_count_matches_the_planner(lib):
+    """oracle/cc_count.py (the Python count of the paper's CC, used by bench.py's reference arm) against
+    su2_plan_info_t: same tasks, same task-positions (one-sided rows folded to one position, reading G13), same flops."""
+    from oracle.cc_count import cc_flops
+    from paper_2309_16724_b200 import Plan
+    for name in ("mini", "midi", "cfg2"):
+        prob = config_problem(name, fill=False)
+        plan = Plan(prob, host_only=True)
+        cc, ntask, ntp = cc_flops(prob)
+        assert ntask == plan.info["ntasks"] and ntp == plan.info["ntask_positions"]
+        assert cc == plan.info["cc_flops"]
