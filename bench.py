@@ -210,6 +210,24 @@ def full_cc(cfg_name):
     return cc_flops(W.config_problem(cfg_name, seed=0, fill=False))[0]
 
 
+def u1_equivalent(cfg_name):
+    """The paper's rescaling to a U(1) calculation of the same accuracy (PAPER.md:231-241 Table I, :255): R_CC = CC of the
+    operator written out in the (N, 2 S_z) basis with merged sectors / CC of the SU(2) plan, R_D = ratio of the bond
+    dimensions.  The expansion is oracle-side (oracle/heff_u1.py, structure only); both CCs come from host-only plans."""
+    from gen import workloads as W
+    from oracle.heff_u1 import expand_problem
+    from paper_2309_16724_b200 import Plan
+    if cfg_name == "cfg1":
+        return None
+    prob = W.config_problem(cfg_name, seed=0, fill=False)
+    u1, _ = expand_problem(prob, merged=True, with_data=False)
+    cc_su2, cc_u1 = Plan(prob, host_only=True).info["cc_flops"], Plan(u1, host_only=True).info["cc_flops"]
+    d_su2, d_u1 = sum(s.dim for s in prob.sec_l), sum(s.dim for s in u1.sec_l)
+    return {"R_CC": cc_u1 / cc_su2, "R_D": d_u1 / d_su2, "D_SU2": d_su2, "D_U1": d_u1, "cc_flops_u1": cc_u1,
+            "note": "U(1)-only mode of the same planner (SU2_SYMMETRY_U1) on the (N, 2Sz) expansion with merged sectors; "
+                    "synthetic sector tables (windowed rule, S <= 2), so the ratios are those of this workload, not the paper's"}
+
+
 def run_reference(args):
     """--impl reference: the oracle, as it stands, on the host cores (rank 0 only).  Loads nothing of the product."""
     if int(os.environ.get("RANK", "0")) != 0:
@@ -469,6 +487,10 @@ def run_gpu(args):
         cb = time_oracle(args.config, budget_s=20.0)
         line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample", "single_thread", "host_cpus")}
         line["cpu_baseline"]["extrapolated_seconds_per_full_apply"] = cc_job / (cb["value"] * 1e12)
+        u1 = u1_equivalent(args.config)
+        if u1 is not None:       # reported NEXT TO the plain figure, never instead of it
+            u1["u1_equivalent_tflops"] = line["value"] * u1["R_CC"]
+            line["u1_equivalent"] = u1
     print(json.dumps(line))
     solver.close()
     if world > 1:

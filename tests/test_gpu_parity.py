@@ -470,6 +470,36 @@ def test_wide_sector_multiple_column_tiles(force_split):
     assert _rel(f_gpu, f_ref) <= TOL
 
 
+@pytest.mark.parametrize("name,merged", [("mini", False), ("mini", True), ("midi", True)])
+def test_u1_mode_parity_and_equivalence(name, merged):
+    """U(1)-only mode (SU2_SYMMETRY_U1): the SAME kernels on a plan whose sectors are
+    (N, 2 S_z) and whose recoupling factor is one, against the plain U(1) oracle (oracle/heff_u1.py) on the expansion of
+    the SU(2) workload -- through the small-block kernel, the large-tile kernel and with split segments -- and, projected
+    back onto the coupled basis, against the SU(2)-mode GPU result (the same numbers up to scalars)."""
+    torch = _torch()
+    from oracle.heff_dense import psi_sectors, unflatten
+    from oracle.heff_u1 import (expand_problem, expand_psi_u1, flatten_u1, heff_apply_u1, project_psi_u1, psi_sectors_u1,
+                                unflatten_u1)
+    prob = config_problem(name)
+    u1, maps = expand_problem(prob, merged=merged)
+    labels_u1 = psi_sectors_u1(u1)
+    op_su2 = _operator(prob)
+    x_red = random_psi(op_su2.psi_len, seed=12)
+    psi_u1 = expand_psi_u1(prob, u1, maps, unflatten(prob, x_red, psi_sectors(prob)))
+    x = flatten_u1(u1, psi_u1, labels_u1)
+    f_ref = flatten_u1(u1, heff_apply_u1(u1, psi_u1), labels_u1)
+    f_su2 = op_su2.apply(torch.from_numpy(x_red).cuda()).cpu().numpy()
+    for kw in (dict(), dict(large_tiles=True), dict(large_tiles=True, force_split=True), dict(force_split=True)):
+        op = _operator(u1, **kw)
+        assert op.plan.labels == labels_u1
+        f = op.apply(torch.from_numpy(x).cuda()).cpu().numpy()
+        assert _rel(f, f_ref) <= TOL
+        back = project_psi_u1(prob, maps, unflatten_u1(u1, f, labels_u1))
+        f_back = np.concatenate([back[lab].ravel() for lab in op_su2.plan.labels])
+        assert _rel(f_back, f_su2) <= TOL
+    assert op.info["cc_flops"] > op_su2.info["cc_flops"]          # R_CC > 1: what the SU(2) adaptation saves
+
+
 def test_two_ranks_nccl_sharded_apply_when_two_gpus_are_visible(tmp_path):
     """bench.py --gpus 2 (position-sharded H_eff*Psi, NCCL all-reduce of F) on one box: the script re-launches itself
     under torch.distributed.run, prints one JSON line with n_gpus = 2 and scaling "strong", and its Davidson history

@@ -38,9 +38,8 @@ def test_u1_oracle_spectrum_equals_fci_in_the_sz_sector(merged):
     assert np.abs(h - h.T).max() < 1e-12
     fs = FockSpace(L)
     hfull = fs.hamiltonian(t, v)
-    nop, szop = fs.number_operator(), fs.sz_operator()
-    sel = [i for i in range(hfull.shape[0]) if abs(nop[i, i] - N) < 1e-9 and abs(2 * szop[i, i] - twoS) < 1e-9]
-    ref = np.linalg.eigvalsh(hfull[np.ix_(sel, sel)])
+    sel = fs.sector_indices(N, twoS)
+    ref = np.linalg.eigvalsh(np.asarray(hfull[np.ix_(sel, sel)].todense()))
     assert h.shape[0] == len(ref)
     assert np.abs(np.linalg.eigvalsh((h + h.T) / 2) - ref).max() < 1e-10
 
