@@ -227,6 +227,20 @@ su2_status su2_davidson_set_preconditioner(su2_davidson* dav, int32_t mode);
 su2_status su2_davidson_ritz_vector(const su2_davidson* dav, double* x_dev, void* cuda_stream);
 su2_status su2_davidson_destroy(su2_davidson* dav);
 
+/* Pre-contraction of an operator family on the device ("we form pre-contracted operators to reduce the
+ * N^4 terms to N^2"): a complementary family is a linear combination over the positions of a normal
+ * family of the same block with weights made of the two-electron integrals,
+ *     out[b][pos'][r][c] = sum_pos W[pos'][pos] * in[b][pos][r][c]     for every sector block b,
+ * i.e. per block ONE row-major GEMM (npos_out x E_b) = W (npos_out x npos_in) . IN (npos_in x E_b) with E_b = rows * ld
+ * of the block (positions are contiguous per block), on FP64 tensor instructions.
+ * block_elems / in_off / out_off: HOST [nblk] -- E_b and the element offsets of block b inside in_dev / out_dev (the
+ * family layouts of su2_opfamily: [npos][rows][ld]); w_dev: DEVICE [npos_out][npos_in] row-major; in_dev / out_dev:
+ * DEVICE, caller-owned, must not overlap.  Asynchronous on the stream, bit-reproducible.  Errors: negative sizes or
+ * null pointers -> SU2_ERR_INVALID_ARGUMENT. */
+su2_status su2_precontract(int32_t nblk, const int64_t* block_elems, const int64_t* in_off, const int64_t* out_off,
+                           int32_t npos_in, int32_t npos_out, const double* w_dev, const double* in_dev,
+                           double* out_dev, void* cuda_stream);
+
 /* Strided-batched FP64 GEMM-pair microbenchmark entry (BASELINE.json configs[4]):
  * C_b (m x p) += alpha * A_b (m x k) * X_b (k x n) * B_b^T (n x p) for b < batch, all DEVICE,
  * row-major, dense strides (A_b = A + b*m*k, ...); the paper's strided-batched GEMM sequences

@@ -210,8 +210,15 @@ def _site_canonical(red):
     return r / lam, lam
 
 
-def build_problem(t, v, n_left, n_elec, two_s_tot, keep_l=None, keep_r=None, use_adjoints=False, drop_tol=1e-14):
-    """Exact `Problem` for the superblock l=[0,n_left) | B=n_left | C=n_left+1 | r=rest."""
+def build_problem(t, v, n_left, n_elec, two_s_tot, keep_l=None, keep_r=None, use_adjoints=False, drop_tol=1e-14,
+                  decomposition=None):
+    """Exact `Problem` for the superblock l=[0,n_left) | B=n_left | C=n_left+1 | r=rest.
+
+    decomposition: if a dict is passed, it receives for every pre-contracted ("complementary") family the ingredients of
+    its pre-contraction, decomposition[(side, family index)] = (normal, W): `normal` is the family of the
+    NORMAL operators of that block the complementary ones are made of (one position per distinct coupled product of
+    elementary operators), W[pos', pos] the integral-dependent weight of normal operator pos in complementary operator
+    pos' -- so that family[pos'] = sum_pos W[pos', pos] normal[pos], which is how this module itself accumulates them."""
     t = np.asarray(t, dtype=float)
     v = np.asarray(v, dtype=float)
     n_orb = t.shape[0]
@@ -240,7 +247,7 @@ def build_problem(t, v, n_left, n_elec, two_s_tot, keep_l=None, keep_r=None, use
         return site_index[key], lam
 
     # groups[(side, normal desc, opB, opC, k1, (dN, two_k) of contracted op)] -> reduced blocks
-    groups = {}
+    groups, raw = {}, {}
     for (descs, k1), alpha in merged.items():
         if abs(alpha) < drop_tol:
             continue
@@ -255,6 +262,7 @@ def build_problem(t, v, n_left, n_elec, two_s_tot, keep_l=None, keep_r=None, use
         cdn = sum(+1 if kd == "+" else -1 for kd in cd_[0])
         gkey = ("r" if contract_r else "l", nd, ob, oc, k1, (cdn, cd_[3]))
         _add_blocks(groups.setdefault(gkey, {}), subs[cx].reduced(cd_), a)
+        raw.setdefault(gkey, []).append((cd_, a))
 
     # step 5: families.  Normal operators of one type (kinds, S, k) form a family whose
     # positions are the orbital tuples; each group contributes one position of a
@@ -315,6 +323,18 @@ def build_problem(t, v, n_left, n_elec, two_s_tot, keep_l=None, keep_r=None, use
         cfam = make_family(pos_blocks, ck[0], ck[1], secs[side], "C%s%s" % (side, (tkey, ob, oc, k1)))
         cid = len(fams[side])
         fams[side].append(cfam)
+        if decomposition is not None:
+            orbs_list = [()] if tkey is None else normal_pos[nside][tkey]
+            lists = [raw.get((side, (() if tkey is None else tkey[0], o, 0 if tkey is None else tkey[1],
+                                     0 if tkey is None else tkey[2]), ob, oc, k1, ck), []) for o in orbs_list]
+            descs_in = sorted({d for lst in lists for d, _ in lst}, key=repr)
+            w = np.zeros((len(orbs_list), len(descs_in)))
+            for p, lst in enumerate(lists):
+                for d, a in lst:
+                    w[p, descs_in.index(d)] += a
+            cx = 3 if side == "r" else 0
+            normal = make_family([subs[cx].reduced(d) for d in descs_in], ck[0], ck[1], secs[side], "normal of " + cfam.name)
+            decomposition[(side, cid)] = (normal, w)
         fam_l, fam_r = (nfam, cid) if side == "r" else (cid, nfam)
         terms.append(Term(fam_l=fam_l, fam_r=fam_r, op_B=ob, op_C=oc, twoK_L=k1, twoK_R=k1,
                           name="%s|%s" % (side, tkey)))

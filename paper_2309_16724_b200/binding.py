@@ -59,7 +59,7 @@ class su2_plan_info_t(C.Structure):
 EXPORTS = ["su2_wigner_6j", "su2_wigner_9j", "su2_status_string", "su2_last_cuda_error", "su2_kernel_launch_count", "su2_plan_create", "su2_plan_destroy", "su2_plan_info",
            "su2_plan_psi_layout", "su2_plan_export_tasks", "su2_heff_apply", "su2_heff_apply_host", "su2_heff_diag",
            "su2_davidson_workspace_bytes", "su2_davidson_create", "su2_davidson_create_sharded", "su2_davidson_step", "su2_davidson_set_preconditioner", "su2_davidson_ritz_vector",
-           "su2_davidson_destroy", "su2_gemm_pair_batched", "su2_gemm_pair_batched_route"]
+           "su2_davidson_destroy", "su2_gemm_pair_batched", "su2_gemm_pair_batched_route", "su2_precontract"]
 
 REDUCE_FN = C.CFUNCTYPE(C.c_int32, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p)   # su2_reduce_fn
 
@@ -107,6 +107,8 @@ def load():
     lib.su2_davidson_destroy.argtypes = [C.c_void_p]
     lib.su2_gemm_pair_batched.argtypes = [C.c_int32] * 4 + [C.c_int64, C.c_double] + [C.c_void_p] * 5
     lib.su2_gemm_pair_batched_route.argtypes = [C.c_int32] * 4 + [C.c_int64, C.c_double] + [C.c_void_p] * 5 + [C.c_int32] * 3
+    lib.su2_precontract.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p,
+                                    C.c_void_p, C.c_void_p, C.c_void_p]
     _lib = lib
     return lib
 
@@ -335,6 +337,15 @@ def probe_fp64_peak(kind, iters=20000, ctas_per_sm=4, stream=0):
     if st != 0:
         raise Su2Error("su2_probe_fp64_peak failed with status %d" % st)
     return v.value
+
+
+def precontract(block_elems, in_off, out_off, npos_in, npos_out, w_ptr, in_ptr, out_ptr, stream=0):
+    """out[b][pos'] = sum_pos W[pos'][pos] in[b][pos] for every block b (su2_precontract): host offset arrays, device data."""
+    be = np.ascontiguousarray(block_elems, dtype=np.int64)
+    io = np.ascontiguousarray(in_off, dtype=np.int64)
+    oo = np.ascontiguousarray(out_off, dtype=np.int64)
+    check(load().su2_precontract(len(be), be.ctypes.data, io.ctypes.data, oo.ctypes.data, npos_in, npos_out, w_ptr, in_ptr,
+                                 out_ptr, stream))
 
 
 def wigner_6j(*two_j):

@@ -110,3 +110,35 @@ class DavidsonSolver:
 
     def close(self):
         self.dav.close()
+
+
+def precontract_family(fam, secs, weights, device="cuda:0", ld_align=4):
+    """Complementary family from a normal one on the device (su2_precontract): `fam` is a gen.problem.OpFamily-like object
+    with numpy blocks [npos, m, k], `weights` a (npos_out x npos) array.  Returns the list of output blocks
+    [npos_out, m, k] as numpy arrays (marshalling only: the contraction runs in the library)."""
+    from .binding import family_layout, precontract
+    _require_cuda()
+    dev = torch.device(device)
+    w = np.ascontiguousarray(weights, dtype=np.float64)
+    npos_out, npos_in = w.shape
+    assert npos_in == fam.npos
+    offs_in, lds, n_in = family_layout(fam, secs, ld_align)
+    host = np.zeros(max(n_in, 1))
+    elems, offs_out, cur = [], [], 0
+    for b, (blk, off, ld) in enumerate(zip(fam.data, offs_in, lds)):
+        _, m, k = blk.shape
+        host[off:off + npos_in * m * ld].reshape(npos_in, m, ld)[:, :, :k] = blk
+        elems.append(m * ld)
+        offs_out.append(cur)
+        cur += -(-npos_out * m * ld // 16) * 16
+    d_in = torch.from_numpy(host).to(dev)
+    d_w = torch.from_numpy(w).to(dev)
+    d_out = torch.zeros(max(cur, 1), dtype=torch.float64, device=dev)
+    precontract(elems, offs_in, offs_out, npos_in, npos_out, d_w.data_ptr(), d_in.data_ptr(), d_out.data_ptr(),
+                torch.cuda.current_stream(dev).cuda_stream)
+    out_host = d_out.cpu().numpy()
+    out = []
+    for blk, off, ld in zip(fam.data, offs_out, lds):
+        _, m, k = blk.shape
+        out.append(out_host[off:off + npos_out * m * ld].reshape(npos_out, m, ld)[:, :, :k].copy())
+    return out
