@@ -241,6 +241,37 @@ su2_status su2_precontract(int32_t nblk, const int64_t* block_elems, const int64
                            int32_t npos_in, int32_t npos_out, const double* w_dev, const double* in_dev,
                            double* out_dev, void* cuda_stream);
 
+/* Renormalisation (blocking) step on the device (Eq. (6)-(7), :311-315): the block l
+ * is enlarged by the site, l' = l + B, and the operator [O_l x O_B]^{k'} is carried into the new (rotated, truncated)
+ * basis of l'.  A new sector q' = (N', J) is spanned, before the rotation, by its CHANNELS (q_l, sigma) -- block sector
+ * and site multiplet coupled to J -- each contributing dim(q_l) coupled rows; U[q'] (coupled rows x D'(q'), orthonormal
+ * columns) is the rotation kept by the truncation.  Per new block, position and channel pair
+ *   R'[pos][q'_o <- q'_i] += weight (-1)^(p_B N_l') <sigma||O_B||sigma'> C^(S_l,s,J | k_l,k_B,k' | S_l',s',J')
+ *                            U[q'_o][rows c_o]^T R_l[pos][q_l <- q_l'] U[q'_i][rows c_i]
+ * (C^ = Eq. (5)/(9) in this header's convention): the same fused GEMM pair as the eigensolver's, on the same kernels. */
+typedef struct {
+  int32_t nsec_old; const su2_sector* sec_old;   /* HOST: sectors (N, 2S, dim) of block l                           */
+  int32_t nsec_new; const su2_sector* sec_new;   /* HOST: sectors (N', 2J, D') of l' in the NEW basis               */
+  int32_t nchan;                                 /* channels of all new sectors                                      */
+  const int32_t* chan_new;   /* HOST [nchan]: new sector of the channel                                              */
+  const int32_t* chan_old;   /* HOST [nchan]: block sector q_l                                                       */
+  const int32_t* chan_site;  /* HOST [nchan]: site multiplet 0 = (0,0), 1 = (1,1/2), 2 = (2,0)                       */
+  const int32_t* chan_row0;  /* HOST [nchan]: first coupled row of the channel inside U[chan_new]                    */
+  const int64_t* u_off;      /* HOST [nsec_new]: element offset of U[q'] inside u                                    */
+  const int32_t* u_ld;       /* HOST [nsec_new]: leading dimension of U[q'] (>= D'(q'); even, with even u_off and a
+                                16-byte aligned u, for blocks of more than 48 rows: bulk-tensor copies)             */
+  const double* u;           /* DEVICE: U[q'] = [coupled rows][u_ld] row-major                                       */
+} su2_blocking;
+/* op_old: operator family on l (NULL = identity); op_site: site operator (NULL = identity); twoK_new: rank k' of the
+ * product; op_new: layout of the new family (q_out / q_in index sec_new, blk_off, blk_ld, npos = op_old's, dN and twoK
+ * of the product) whose DEVICE `data` is WRITTEN (accumulate = 0: overwritten, blocks without contribution zeroed;
+ * 1: added to, which is how sums of several products -- complementary operators -- are composed).  Families of more
+ * than 48-row blocks must be 16-byte aligned (su2_opfamily layout advice).  Asynchronous on the stream; table memory is
+ * stream-ordered.  Errors: SU2_ERR_INVALID_ARGUMENT / _SECTOR / _RANK as for su2_plan_create, SU2_ERR_CUDA. */
+su2_status su2_renormalize(const su2_blocking* blocking, const su2_opfamily* op_old, const su2_siteop* op_site,
+                           int32_t twoK_new, double weight, int32_t accumulate, const su2_opfamily* op_new,
+                           void* cuda_stream);
+
 /* Strided-batched FP64 GEMM-pair microbenchmark entry (BASELINE.json configs[4]):
  * C_b (m x p) += alpha * A_b (m x k) * X_b (k x n) * B_b^T (n x p) for b < batch, all DEVICE,
  * row-major, dense strides (A_b = A + b*m*k, ...); the paper's strided-batched GEMM sequences

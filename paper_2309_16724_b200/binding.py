@@ -32,6 +32,13 @@ class su2_siteop_u1(C.Structure):
     _fields_ = [("r", (C.c_double * 4) * 4), ("dN", C.c_int32), ("dM", C.c_int32)]
 
 
+class su2_blocking(C.Structure):
+    _fields_ = [("nsec_old", C.c_int32), ("sec_old", C.POINTER(su2_sector)), ("nsec_new", C.c_int32),
+                ("sec_new", C.POINTER(su2_sector)), ("nchan", C.c_int32), ("chan_new", C.POINTER(C.c_int32)),
+                ("chan_old", C.POINTER(C.c_int32)), ("chan_site", C.POINTER(C.c_int32)), ("chan_row0", C.POINTER(C.c_int32)),
+                ("u_off", C.POINTER(C.c_int64)), ("u_ld", C.POINTER(C.c_int32)), ("u", C.c_void_p)]
+
+
 class su2_term(C.Structure):
     _fields_ = [("fam_l", C.c_int32), ("fam_r", C.c_int32), ("op_B", C.c_int32), ("op_C", C.c_int32),
                 ("twoK_L", C.c_int32), ("twoK_R", C.c_int32), ("adj_l", C.c_int32), ("adj_r", C.c_int32),
@@ -59,7 +66,7 @@ class su2_plan_info_t(C.Structure):
 EXPORTS = ["su2_wigner_6j", "su2_wigner_9j", "su2_status_string", "su2_last_cuda_error", "su2_kernel_launch_count", "su2_plan_create", "su2_plan_destroy", "su2_plan_info",
            "su2_plan_psi_layout", "su2_plan_export_tasks", "su2_heff_apply", "su2_heff_apply_host", "su2_heff_diag",
            "su2_davidson_workspace_bytes", "su2_davidson_create", "su2_davidson_create_sharded", "su2_davidson_step", "su2_davidson_set_preconditioner", "su2_davidson_ritz_vector",
-           "su2_davidson_destroy", "su2_gemm_pair_batched", "su2_gemm_pair_batched_route", "su2_precontract"]
+           "su2_davidson_destroy", "su2_gemm_pair_batched", "su2_gemm_pair_batched_route", "su2_precontract", "su2_renormalize"]
 
 REDUCE_FN = C.CFUNCTYPE(C.c_int32, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p)   # su2_reduce_fn
 
@@ -109,6 +116,8 @@ def load():
     lib.su2_gemm_pair_batched_route.argtypes = [C.c_int32] * 4 + [C.c_int64, C.c_double] + [C.c_void_p] * 5 + [C.c_int32] * 3
     lib.su2_precontract.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p,
                                     C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.su2_renormalize.argtypes = [C.POINTER(su2_blocking), C.POINTER(su2_opfamily), C.POINTER(su2_siteop), C.c_int32,
+                                    C.c_double, C.c_int32, C.POINTER(su2_opfamily), C.c_void_p]
     _lib = lib
     return lib
 
@@ -346,6 +355,38 @@ def precontract(block_elems, in_off, out_off, npos_in, npos_out, w_ptr, in_ptr, 
     oo = np.ascontiguousarray(out_off, dtype=np.int64)
     check(load().su2_precontract(len(be), be.ctypes.data, io.ctypes.data, oo.ctypes.data, npos_in, npos_out, w_ptr, in_ptr,
                                  out_ptr, stream))
+
+
+def _family_struct(dN, twoK, npos, q_out, q_in, offs, lds, ptr, keep):
+    qo, qi, off, ld = _i32(q_out), _i32(q_in), np.ascontiguousarray(offs, dtype=np.int64), _i32(lds)
+    keep += [qo, qi, off, ld]
+    return su2_opfamily(dN, twoK, npos, len(qo), qo.ctypes.data_as(C.POINTER(C.c_int32)), qi.ctypes.data_as(C.POINTER(C.c_int32)),
+                        off.ctypes.data_as(C.POINTER(C.c_int64)), ld.ctypes.data_as(C.POINTER(C.c_int32)), ptr)
+
+
+def renormalize(sec_old, sec_new, channels, u_off, u_ld, u_ptr, old, site, twoK_new, weight, accumulate, new, stream=0):
+    """su2_renormalize.  sec_old / sec_new: lists of (N, twoS, dim); channels: list of (new sector, block sector, site
+    multiplet, first row); old / new: None or dict(dN, twoK, npos, q_out, q_in, offs, lds, ptr) describing a family in
+    DEVICE memory; site: None or (r 3x3, dN, twoK)."""
+    keep = []
+    so = (su2_sector * len(sec_old))(*[su2_sector(*s) for s in sec_old])
+    sn = (su2_sector * len(sec_new))(*[su2_sector(*s) for s in sec_new])
+    ch = [_i32([c[i] for c in channels]) for i in range(4)]
+    uo, ul = np.ascontiguousarray(u_off, dtype=np.int64), _i32(u_ld)
+    blk = su2_blocking(len(sec_old), so, len(sec_new), sn, len(channels), *[a.ctypes.data_as(C.POINTER(C.c_int32)) for a in ch],
+                       uo.ctypes.data_as(C.POINTER(C.c_int64)), ul.ctypes.data_as(C.POINTER(C.c_int32)), u_ptr)
+    f_old = None if old is None else _family_struct(old["dN"], old["twoK"], old["npos"], old["q_out"], old["q_in"], old["offs"],
+                                                    old["lds"], old["ptr"], keep)
+    f_new = _family_struct(new["dN"], new["twoK"], new["npos"], new["q_out"], new["q_in"], new["offs"], new["lds"], new["ptr"], keep)
+    s_op = None
+    if site is not None:
+        s_op = su2_siteop()
+        for a in range(3):
+            for b in range(3):
+                s_op.r[a][b] = float(site[0][a][b])
+        s_op.dN, s_op.twoK = site[1], site[2]
+    check(load().su2_renormalize(C.byref(blk), None if f_old is None else C.byref(f_old), None if s_op is None else C.byref(s_op),
+                                 twoK_new, weight, 1 if accumulate else 0, C.byref(f_new), stream))
 
 
 def wigner_6j(*two_j):

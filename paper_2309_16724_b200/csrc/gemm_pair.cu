@@ -151,13 +151,13 @@ __global__ void gemm_pair_tables_kernel(int m, int k, int n, int p, int64_t batc
     t.A = nullptr; t.D = nullptr; t.alpha = nullptr; t.coef = alpha;
     t.e_off = b * (int64_t)k * n; t.m = m; t.k = k; t.n = n; t.p = p;
     t.strideA = m * k; t.strideD = p * n; t.ldA = k; t.ldD = n; t.npos = 1; t.flags = 0;
-    t.mapA = 0; t.mapD = 1; t.mapE = 2; t.e_item = (int32_t)b;
+    t.mapA = 0; t.mapD = 1; t.mapE = 2; t.e_item = (int32_t)b; t.ldE = n; t.pad = 0;
     tasks[b] = t;
     units[b] = DevUnit{(int32_t)b, (int32_t)b, (int32_t)b + 1, 0};     // "position" b = the item coordinate of A and B
     for (int i = 0; i < tr * tc; ++i) {
       DevWork w;
       w.dst_off = b * (int64_t)m * p; w.unit0 = (int32_t)b; w.unit1 = (int32_t)b + 1;
-      w.row0 = (i / tc) * tm; w.col0 = (i % tc) * tp; w.m = m; w.p = p; w.to_partial = 2; w.wr = wr;
+      w.row0 = (i / tc) * tm; w.col0 = (i % tc) * tp; w.m = m; w.p = p; w.to_partial = 2; w.wr = wr; w.ldo = p; w.pad = 0;
       work[b * (int64_t)(tr * tc) + i] = w;
     }
   }

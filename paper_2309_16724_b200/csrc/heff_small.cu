@@ -132,18 +132,18 @@ heff_small_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __
     }
   };
   // E: the same with zero fill up to rows_pad x cols_pad
-  auto copy_e = [&](const double* __restrict__ src, int rows, int cols, int rows_pad, int cols_pad) {
+  auto copy_e = [&](const double* __restrict__ src, int rows, int cols, int lde, int rows_pad, int cols_pad) {
     for (int r = warp; r < rows_pad; r += WARPS)
       for (int c = lane; c < cols_pad; c += 32) {
         const bool valid = r < rows && c < cols;
-        hs_cp8(Es + r * LD + c, valid ? src + (int64_t)r * cols + c : src, valid);
+        hs_cp8(Es + r * LD + c, valid ? src + (int64_t)r * lde + c : src, valid);
       }
   };
   auto issue_AE = [&](const DevTask& t, int pos, bool with_e) {
     const double* A = t.A + (int64_t)pos * t.strideA;
     if (t.flags & TASK_TRANS_A) copy_rows(As, A, t.k, t.m, t.ldA);
     else copy_rows(As, A, t.m, t.k, t.ldA);
-    if (with_e) copy_e(psi + t.e_off, t.k, t.n, (t.k + 3) & ~3, (t.n + 7) & ~7);
+    if (with_e) copy_e(psi + t.e_off, t.k, t.n, t.ldE, (t.k + 3) & ~3, (t.n + 7) & ~7);
   };
   auto issue_D = [&](const DevTask& t, int pos) {
     const double* D = t.D + (int64_t)pos * t.strideD;
@@ -239,7 +239,7 @@ heff_small_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __
       for (int j = 0; j < TCM; ++j) {
         const int r = 8 * (wr + WR * i) + fr, c = 8 * (wc + WC * j) + 2 * fc;
         if (i < nr && j < np && r < w.m) {
-          double* q = dst + (int64_t)r * w.p + c;
+          double* q = dst + (int64_t)r * w.ldo + c;
           if (w.to_partial & 2) {
             if (c < w.p) q[0] += acc[i][j][0];
             if (c + 1 < w.p) q[1] += acc[i][j][1];

@@ -383,7 +383,7 @@ __device__ __forceinline__ void consume_item(PhaseInfo info, const DevWork* __re
         const int r = wk.row0 + wr * 32 + ii * 8 + g;
         const int q = wk.col0 + (wc * NT2 + j) * 8 + 2 * t;
         if (r < wk.m) {
-          double* o = dst + (int64_t)r * wk.p + q;
+          double* o = dst + (int64_t)r * wk.ldo + q;
           if (q < wk.p) o[0] = accumulate ? o[0] + acc[ii][j][0] : acc[ii][j][0];
           if (q + 1 < wk.p) o[1] = accumulate ? o[1] + acc[ii][j][1] : acc[ii][j][1];
         }

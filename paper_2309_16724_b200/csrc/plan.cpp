@@ -560,6 +560,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
     d.m = ht.m; d.k = ht.k; d.n = ht.n; d.p = ht.p; d.npos = ht.npos;
     d.flags = (ht.adj_l ? TASK_TRANS_A : 0u) | (ht.adj_r ? TASK_TRANS_D : 0u);
     d.mapA = d.mapD = d.mapE = -1;
+    d.ldE = ht.n;
     const OperandRef ra = operand(0, ht.fam_l, ht.blk_l, ht.term, ht.m);
     const OperandRef rd = operand(1, ht.fam_r, ht.blk_r, ht.term, ht.p);
     plan->h_opA[i] = ra;
@@ -706,7 +707,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
           }
           DevWork wk{};
           wk.unit0 = segs[g].first; wk.unit1 = segs[g].second;
-          wk.row0 = r0; wk.col0 = c0; wk.m = ps.m; wk.p = ps.p;
+          wk.row0 = r0; wk.col0 = c0; wk.m = ps.m; wk.p = ps.p; wk.ldo = ps.p;
           wk.to_partial = nseg > 1 ? 1 : 0;
           wk.dst_off = nseg > 1 ? red.part_off + (int64_t)g * sz : ps.off;
           wk.wr = small_plan ? 0 : wr;

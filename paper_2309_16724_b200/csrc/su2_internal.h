@@ -24,6 +24,7 @@ struct DevTask {
   uint32_t flags;
   int32_t mapA, mapD, mapE;   // large-tile kernel: indices of the operands' tensor maps (su2_plan::d_maps)
   int32_t e_item;             // third coordinate of the E map (0 inside H_eff; the batch index of a GEMM-pair item)
+  int32_t ldE, pad;           // leading dimension of the stored E block (n inside H_eff: Psi sectors are dense)
 };
 enum : uint32_t { TASK_TRANS_A = 1u, TASK_TRANS_D = 2u };
 
@@ -44,6 +45,8 @@ struct DevWork {
   int32_t m, p;           // output block dims (p = leading dimension)
   int32_t to_partial;     // bit 0: dst_off refers to the partial buffer; bit 1: accumulate into dst (dst += tile)
   int32_t wr;             // tile class: warp rows WR of TileCfg<WR> (1, 2 or 4); 0 = whole sector (heff_small_kernel)
+  int32_t ldo;            // leading dimension of the output block (p for Psi sectors; padded for operator blocks)
+  int32_t pad;
 };
 
 // Second pass of the deterministic segmented reduction: F_s = sum_{seg} partial[seg] in index order.

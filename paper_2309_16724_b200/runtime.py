@@ -142,3 +142,58 @@ def precontract_family(fam, secs, weights, device="cuda:0", ld_align=4):
         _, m, k = blk.shape
         out.append(out_host[off:off + npos_out * m * ld].reshape(npos_out, m, ld)[:, :, :k].copy())
     return out
+
+
+def renormalize_family(sec_old, sec_new, channels, rotation, fam_old, site, twoK_new, new_blocks, weight=1.0,
+                       device="cuda:0", ld_align=4):
+    """Blocking step on the device (su2_renormalize): the operator [O_l x O_B]^{k'} of the enlarged block in its new basis.
+
+    sec_old / sec_new: lists of (N, twoS, dim); channels[q'] = [(block sector, site multiplet, first row)] (the coupled
+    rows of new sector q'); rotation[q'] = numpy (coupled rows x D') matrix; fam_old: OpFamily-like with numpy blocks
+    [npos, m, k] over sec_old, or None (identity); site: SiteOp-like (r, dN, twoK) or None; new_blocks: list of
+    (q'_out, q'_in) to compute.  Returns the list of new blocks [npos, D'_out, D'_in] as numpy arrays (marshalling only)."""
+    from types import SimpleNamespace
+    from .binding import family_layout, renormalize
+    _require_cuda()
+    dev = torch.device(device)
+    stream = torch.cuda.current_stream(dev).cuda_stream
+    # rotation matrices, padded leading dimensions, one buffer
+    u_off, u_ld, cur = [], [], 0
+    for q, (_, _, d) in enumerate(sec_new):
+        ld = -(-d // ld_align) * ld_align
+        u_off.append(cur)
+        u_ld.append(ld)
+        cur += -(-rotation[q].shape[0] * ld // 16) * 16
+    u_host = np.zeros(max(cur, 1))
+    for q, (_, _, d) in enumerate(sec_new):
+        rows = rotation[q].shape[0]
+        u_host[u_off[q]:u_off[q] + rows * u_ld[q]].reshape(rows, u_ld[q])[:, :d] = rotation[q]
+    d_u = torch.from_numpy(u_host).to(dev)
+    chan = [(q, il, sg, r0) for q, lst in enumerate(channels) for (il, sg, r0) in lst]
+    old = None
+    npos, dN, kl = 1, 0, 0
+    if fam_old is not None:
+        secs = [SimpleNamespace(N=s[0], twoS=s[1], dim=s[2]) for s in sec_old]
+        offs, lds, n = family_layout(fam_old, secs, ld_align)
+        host = np.zeros(max(n, 1))
+        for blk, off, ld in zip(fam_old.data, offs, lds):
+            p_, m, k = blk.shape
+            host[off:off + p_ * m * ld].reshape(p_, m, ld)[:, :, :k] = blk
+        d_old = torch.from_numpy(host).to(dev)
+        npos, dN, kl = fam_old.npos, fam_old.dN, fam_old.twoK
+        old = dict(dN=dN, twoK=kl, npos=npos, q_out=fam_old.q_out, q_in=fam_old.q_in, offs=offs, lds=lds, ptr=d_old.data_ptr())
+    dN_new = dN + (site.dN if site is not None else 0)
+    secs_new = [SimpleNamespace(N=s[0], twoS=s[1], dim=s[2]) for s in sec_new]
+    new_fam = SimpleNamespace(npos=npos, q_out=[b[0] for b in new_blocks], q_in=[b[1] for b in new_blocks])
+    offs_n, lds_n, n_new = family_layout(new_fam, secs_new, ld_align)
+    d_new = torch.full((max(n_new, 1),), float("nan"), dtype=torch.float64, device=dev)   # must be overwritten / zeroed
+    new = dict(dN=dN_new, twoK=twoK_new, npos=npos, q_out=new_fam.q_out, q_in=new_fam.q_in, offs=offs_n, lds=lds_n,
+               ptr=d_new.data_ptr())
+    renormalize(sec_old, sec_new, chan, u_off, u_ld, d_u.data_ptr(), old,
+                None if site is None else (site.r, site.dN, site.twoK), twoK_new, weight, False, new, stream)
+    host_new = d_new.cpu().numpy()
+    out = []
+    for (qo, qi), off, ld in zip(new_blocks, offs_n, lds_n):
+        m, k = sec_new[qo][2], sec_new[qi][2]
+        out.append(host_new[off:off + npos * m * ld].reshape(npos, m, ld)[:, :, :k].copy())
+    return out

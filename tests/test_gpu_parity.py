@@ -467,6 +467,76 @@ def test_precontracted_operators_give_the_fci_energy():
     solver.close()
 
 
+@pytest.mark.parametrize("n,big", [(2, False), (3, False), (3, True)])
+def test_renormalize_against_the_fock_space_blocking(n, big):
+    """su2_renormalize (Eq. (6)-(7), :311-315): block of n orbitals + site -> new block in a
+    rotated, truncated basis, for normal operators of the block (position-indexed families), site operators and coupled
+    block x site products, against oracle/blocking.py -- Jordan-Wigner matrices of the joint Fock space reduced in the
+    coupled multiplet basis, no 6j / 9j.  big: every multiplet is replicated so that sectors exceed 48 rows and the step
+    runs on the large-tile (bulk-tensor) kernel instead of the small-block one."""
+    torch = _torch()
+    from types import SimpleNamespace
+    from gen.workloads import site_table
+    from oracle.blocking import blocked_basis
+    from oracle.fock import FockSpace, couple
+    from oracle.multiplets import full_multiplet_basis, reduce_tensor
+    from paper_2309_16724_b200.runtime import renormalize_family
+    fs, fsj = FockSpace(n), FockSpace(n + 1)
+    bl = full_multiplet_basis(fs)
+    _, sectors, channels = blocked_basis(bl, fs)
+    rng = np.random.default_rng(8)
+    rot = {}
+    for isec, (_, _, d) in enumerate(sectors):
+        q, _ = np.linalg.qr(rng.normal(size=(d, d)))
+        rot[isec] = q[:, :max(1, (2 * d + 2) // 3)]
+    bj, _, _ = blocked_basis(bl, fs, rotation=rot)
+    site = {o.name: o for o in site_table()[0]}
+    rep = 1
+    if big:
+        # replicate every multiplet `rep` times (block-diagonal copies): R -> R (x) 1_rep, U -> U (x) 1_rep, results likewise
+        rep = 9
+    sec_old = [(a, b, d * rep) for a, b, d in bl.sectors]
+    sec_new = [(a, b, d * rep) for a, b, d in bj.sectors]
+    chans = [[(il, sg, r0 * rep) for il, sg, r0 in lst] for lst in channels]
+    eye = np.eye(rep)
+    rotation = {q: np.kron(rot[q], eye) for q in rot}
+    assert (max(d for _, _, d in sec_old + sec_new) > 48) == big
+
+    def family(ops):
+        """position-indexed family of block operators (same rank and dN) reduced in the block's basis"""
+        reds = [reduce_tensor(o, bl) for o in ops]
+        keys = sorted({k for r in reds for k in r})
+        data = [np.stack([np.kron(r.get(k, np.zeros((bl.sectors[k[0]][2], bl.sectors[k[1]][2]))), eye) for r in reds]) for k in keys]
+        return SimpleNamespace(dN=ops[0].dN, twoK=ops[0].two_k, npos=len(ops), q_out=[k[0] for k in keys], q_in=[k[1] for k in keys], data=data)
+
+    cases = [([fs.t_cd(i) for i in range(n)], [fsj.t_cd(i) for i in range(n)], None, None, 1),
+             ([couple(fs.t_cd(i), fs.t_ct(j), 2) for i in range(n) for j in range(n)],
+              [couple(fsj.t_cd(i), fsj.t_ct(j), 2) for i in range(n) for j in range(n)], None, None, 2),
+             (None, None, "c~", fsj.t_ct(n), 1),
+             ([fs.t_cd(i) for i in range(n)], [fsj.t_cd(i) for i in range(n)], "c+", fsj.t_cd(n), 0),
+             ([fs.t_cd(i) for i in range(n)], [fsj.t_cd(i) for i in range(n)], "c~", fsj.t_ct(n), 2),
+             ([couple(fs.t_cd(i), fs.t_ct(j), 2) for i in range(n) for j in range(n)],
+              [couple(fsj.t_cd(i), fsj.t_ct(j), 2) for i in range(n) for j in range(n)], "c+", fsj.t_cd(n), 3)]
+    checked = 0
+    for ops_l, ops_lj, sname, op_sj, two_k in cases:
+        npos = 1 if ops_l is None else len(ops_l)
+        joint = [op_sj] if ops_lj is None else [(o if op_sj is None else couple(o, op_sj, two_k)) for o in ops_lj]
+        want = [reduce_tensor(o, bj) for o in joint]
+        dN = joint[0].dN
+        blocks = [(io, ii) for io, so in enumerate(sec_new) for ii, si in enumerate(sec_new)
+                  if so[0] == si[0] + dN and abs(si[1] - two_k) <= so[1] <= si[1] + two_k]
+        got = renormalize_family(sec_old, sec_new, chans, rotation, None if ops_l is None else family(ops_l),
+                                 site[sname] if sname else None, two_k, blocks)
+        scale = max(np.abs(m).max() for w in want for m in w.values())
+        for (io, ii), g in zip(blocks, got):
+            assert g.shape == (npos, sec_new[io][2], sec_new[ii][2]) and np.isfinite(g).all()
+            for pos in range(npos):
+                ref = np.kron(want[pos].get((io, ii), np.zeros((bj.sectors[io][2], bj.sectors[ii][2]))), eye)
+                assert np.abs(g[pos] - ref).max() <= 1e-12 * scale, (sname, two_k, io, ii, pos)
+                checked += 1
+    assert checked > 100
+
+
 def test_gpu_result_is_hermitian_and_linear_midi():
     torch = _torch()
     prob = config_problem("midi")
