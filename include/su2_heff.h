@@ -55,7 +55,9 @@ enum {
   SU2_ERR_NOT_FINITE = -4,         /* non-finite alpha or site element                           */
   SU2_ERR_CUDA = -5,               /* a CUDA runtime call failed (see su2_last_cuda_error)       */
   SU2_ERR_NO_DEVICE_PLAN = -6,     /* plan was created with SU2_PLAN_HOST_ONLY                   */
-  SU2_ERR_WORKSPACE = -7           /* workspace pointer null although workspace_bytes > 0        */
+  SU2_ERR_WORKSPACE = -7,          /* workspace pointer null although workspace_bytes > 0        */
+  SU2_ERR_SCRATCH_LIMIT = -8       /* su2_heff_apply_noalloc: the plan needs more scratch than the
+                                      library's static array holds (see su2_last_cuda_error)      */
 };
 const char* su2_status_string(su2_status st);
 const char* su2_last_cuda_error(void);
@@ -190,6 +192,18 @@ su2_status su2_plan_export_tasks(const su2_plan* plan, int32_t* out_sec, int32_t
  * concurrently). */
 su2_status su2_heff_apply(const su2_plan* plan, const double* psi_dev, double* out_dev,
                           void* workspace_dev, void* cuda_stream);
+/* The same for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): out_dev = H_eff * psi_dev with NO workspace argument.  The partial tiles of the
+ * segmented reduction live in a static device array of SU2_NOALLOC_SCRATCH_BYTES = 64 MiB inside the library (held by
+ * every GPU that loads it until the process exits); the call allocates and frees nothing and is bit-identical to
+ * su2_heff_apply.  A plan whose partial tiles exceed that size (workspace_bytes - 256 > SU2_NOALLOC_SCRATCH_BYTES;
+ * BASELINE.json configs[2..3]) is rejected with SU2_ERR_SCRATCH_LIMIT and a message in su2_last_cuda_error.  The array is
+ * shared by ALL calls on a device and keeps the last call's contents (no element is read before the same call wrote it,
+ * so nothing needs clearing): calls that overlap on the GPU -- two streams, two plans -- race; order them on one stream.
+ * psi_dev / out_dev: DEVICE, caller-owned, out must not alias psi.  Asynchronous on the stream. */
+#define SU2_NOALLOC_SCRATCH_BYTES (64 * 1024 * 1024)
+su2_status su2_heff_apply_noalloc(const su2_plan* plan, const double* psi_dev, double* out_dev, void* cuda_stream);
+int64_t su2_noalloc_scratch_bytes(void);   /* = SU2_NOALLOC_SCRATCH_BYTES, as compiled into the library */
 /* Same through HOST buffers: copies psi to the device, applies, copies the result back and
  * synchronises (the end-to-end entry point; device staging buffers inside workspace_dev, which
  * must hold workspace_bytes + 2*8*psi_len bytes). */

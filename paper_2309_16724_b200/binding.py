@@ -66,7 +66,8 @@ class su2_plan_info_t(C.Structure):
 EXPORTS = ["su2_wigner_6j", "su2_wigner_9j", "su2_status_string", "su2_last_cuda_error", "su2_kernel_launch_count", "su2_plan_create", "su2_plan_destroy", "su2_plan_info",
            "su2_plan_psi_layout", "su2_plan_export_tasks", "su2_heff_apply", "su2_heff_apply_host", "su2_heff_diag",
            "su2_davidson_workspace_bytes", "su2_davidson_create", "su2_davidson_create_sharded", "su2_davidson_step", "su2_davidson_set_preconditioner", "su2_davidson_ritz_vector",
-           "su2_davidson_destroy", "su2_gemm_pair_batched", "su2_gemm_pair_batched_route", "su2_precontract", "su2_renormalize"]
+           "su2_davidson_destroy", "su2_gemm_pair_batched", "su2_gemm_pair_batched_route", "su2_precontract", "su2_renormalize", "su2_heff_apply_noalloc",
+           "su2_noalloc_scratch_bytes"]
 
 REDUCE_FN = C.CFUNCTYPE(C.c_int32, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p)   # su2_reduce_fn
 
@@ -100,6 +101,9 @@ def load():
     lib.su2_plan_psi_layout.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     lib.su2_plan_export_tasks.argtypes = [C.c_void_p] + [C.c_void_p] * 10
     lib.su2_heff_apply.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.su2_heff_apply_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.su2_noalloc_scratch_bytes.restype = C.c_int64
+    lib.su2_noalloc_scratch_bytes.argtypes = []
     lib.su2_heff_apply_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.su2_heff_diag.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     lib.su2_davidson_workspace_bytes.restype = C.c_int64
@@ -126,7 +130,7 @@ def check(st):
     if st != 0:
         lib = load()
         msg = lib.su2_status_string(st).decode()
-        if st == -5:
+        if st in (-5, -8):
             msg += " (" + lib.su2_last_cuda_error().decode() + ")"
         raise Su2Error("su2 status %d: %s" % (st, msg))
 
@@ -249,6 +253,10 @@ class Plan:
     # --- device entry points (pointers are plain ints) ---
     def heff_apply(self, psi_ptr, out_ptr, workspace_ptr, stream=0):
         check(load().su2_heff_apply(self.handle, psi_ptr, out_ptr, workspace_ptr, stream))
+
+    def heff_apply_noalloc(self, psi_ptr, out_ptr, stream=0):
+        """su2_heff_apply_noalloc: scratch in the library's static device array (<= 64 MiB), nothing allocated."""
+        check(load().su2_heff_apply_noalloc(self.handle, psi_ptr, out_ptr, stream))
 
     def heff_apply_host(self, psi_host_ptr, out_host_ptr, workspace_ptr, stream=0):
         check(load().su2_heff_apply_host(self.handle, psi_host_ptr, out_host_ptr, workspace_ptr, stream))
@@ -395,6 +403,10 @@ def wigner_6j(*two_j):
 
 def wigner_9j(*two_j):
     return float(load().su2_wigner_9j(*[int(x) for x in two_j]))
+
+
+def noalloc_scratch_bytes():
+    return int(load().su2_noalloc_scratch_bytes())
 
 
 def kernel_launch_count():

@@ -868,6 +868,7 @@ extern "C" const char* su2_status_string(su2_status st) {
     case SU2_ERR_CUDA: return "CUDA runtime error";
     case SU2_ERR_NO_DEVICE_PLAN: return "plan has no device tables (SU2_PLAN_HOST_ONLY)";
     case SU2_ERR_WORKSPACE: return "workspace missing";
+    case SU2_ERR_SCRATCH_LIMIT: return "plan needs more scratch than the library's static no-alloc array holds";
     default: return "unknown status";
   }
 }

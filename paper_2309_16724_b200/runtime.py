@@ -73,6 +73,13 @@ class HeffOperator:
                              torch.cuda.current_stream(self.device).cuda_stream)
         return out
 
+    def apply_noalloc(self, psi, out):
+        """out = H_eff psi through su2_heff_apply_noalloc: no workspace, nothing allocated (caller passes both tensors)."""
+        assert psi.dtype == torch.float64 and psi.is_cuda and psi.is_contiguous() and psi.numel() == self.psi_len
+        assert out.dtype == torch.float64 and out.is_cuda and out.is_contiguous() and out.numel() == self.psi_len
+        self.plan.heff_apply_noalloc(psi.data_ptr(), out.data_ptr(), torch.cuda.current_stream(self.device).cuda_stream)
+        return out
+
     def apply_host(self, psi_host, out_host):
         """End-to-end entry: pinned host tensors in and out (copies inside the C call)."""
         assert psi_host.dtype == torch.float64 and not psi_host.is_cuda and psi_host.numel() == self.psi_len
