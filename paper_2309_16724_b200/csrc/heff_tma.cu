@@ -207,6 +207,23 @@ __device__ __forceinline__ void produce_item(const DevWork& wk, int w, bool rese
   }
 }
 
+template <int MT, int NT, int NACC, int A_I, int A_SUB, int B_J, int B_SUB>
+__device__ __forceinline__ void mma_ragged(double (&c)[4][NACC][2], const double* __restrict__ a,
+                                           const double* __restrict__ b, int nsub) {
+#pragma unroll 1
+  for (int sub = 0; sub < nsub; ++sub) {
+    double af[MT], bf[NT];
+#pragma unroll
+    for (int ii = 0; ii < MT; ++ii) af[ii] = a[sub * A_SUB + ii * A_I];
+#pragma unroll
+    for (int j = 0; j < NT; ++j) bf[j] = b[sub * B_SUB + j * B_J];
+#pragma unroll
+    for (int j = 0; j < NT; ++j)
+#pragma unroll
+      for (int ii = 0; ii < MT; ++ii) dmma(c[ii][j], af[ii], bf[j]);
+  }
+}
+
 // One pipeline stage (nsub <= NSUB k4 sub-steps) of a warp-level product: c[ii][j] += A_frag[ii] B_frag[j] for
 // 4 m8-tiles (the first mt active) and NT n8-tiles.  a / b point at this lane's element of the first fragment;
 // A_I / B_J are the strides between m8-tiles / n8-tiles, A_SUB / B_SUB between k4 sub-steps.
@@ -237,18 +254,15 @@ __device__ __forceinline__ void mma_stage(double (&c)[4][NACC][2], const double*
     }
     return;
   }
-#pragma unroll 1
-  for (int sub = 0; sub < nsub; ++sub) {
-    double af[4], bf[NT];
-#pragma unroll
-    for (int ii = 0; ii < 4; ++ii) af[ii] = a[sub * A_SUB + ii * A_I];
-#pragma unroll
-    for (int j = 0; j < NT; ++j) bf[j] = b[sub * B_SUB + j * B_J];
-#pragma unroll
-    for (int j = 0; j < NT; ++j)
-#pragma unroll
-      for (int ii = 0; ii < 4; ++ii)
-        if (ii < mt) dmma(c[ii][j], af[ii], bf[j]);
+  // ragged stage (k tail of a phase, or a row tile with fewer than 32 valid rows): rolled loop over the sub-steps,
+  // instantiated per number of active m8-tiles -- a predicated-off DMMA still occupies its slot in the FP64 tensor pipe
+  // (sm__ops_path_tensor_src_fp64 counts it), so `if (ii < mt) dmma(...)` made the last row tile of every sector pay
+  // for four m8-tiles whatever it held
+  switch (mt) {
+    case 1: mma_ragged<1, NT, NACC, A_I, A_SUB, B_J, B_SUB>(c, a, b, nsub); break;
+    case 2: mma_ragged<2, NT, NACC, A_I, A_SUB, B_J, B_SUB>(c, a, b, nsub); break;
+    case 3: mma_ragged<3, NT, NACC, A_I, A_SUB, B_J, B_SUB>(c, a, b, nsub); break;
+    default: mma_ragged<4, NT, NACC, A_I, A_SUB, B_J, B_SUB>(c, a, b, nsub); break;
   }
 }
 
