@@ -365,6 +365,9 @@ def run_gpu(args):
         dist.barrier()
     stream = torch.cuda.current_stream().cuda_stream
 
+    # FP64 tensor peak of this GPU, measured before the load (and again after it: the higher reading is the denominator;
+    # right after a 1 kW run the short probe can catch a power-cap clock dip and read low, which would flatter frac)
+    dmma_cold = probe_fp64_peak(1, 4000, 4, stream) if rank == 0 else 0.0
     t0 = time.perf_counter()
     prob, op = build_operator(args.config, device, shard=(mode == "shard"))
     setup_s = time.perf_counter() - t0
@@ -437,7 +440,8 @@ def run_gpu(args):
     ms_step = ms_total / args.steps
     peaks, peak_src = measured_peaks()
     dfma = probe_fp64_peak(0, 20000, 4, stream)
-    dmma = probe_fp64_peak(1, 4000, 4, stream)
+    dmma_hot = probe_fp64_peak(1, 4000, 4, stream)
+    dmma = max(dmma_cold, dmma_hot)
     peak = dmma
     peak_rule = peaks["bf16_tflops"] * FP64_OVER_BF16_NOMINAL
     achieved = cc_local / (apply_ms * 1e-3) / 1e12
@@ -474,7 +478,10 @@ def run_gpu(args):
                          "heff_small_kernel, one launch per size class" if info["small_plan"] else "heff_tma_kernel"),
                      "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                      "traffic": ncu_traffic(args.config),
-                     "peak_source": "FP64 tensor (DMMA.8x8x4) loop measured in this run by su2_probe_fp64_peak (libsu2probe.so)",
+                     "peak_source": "FP64 tensor (DMMA.8x8x4) loop measured in this run by su2_probe_fp64_peak (libsu2probe.so): "
+                                    "max of the reading before the load (%.2f) and after it (%.2f)" % (dmma_cold, dmma_hot),
+                     "peak_nominal": torch.cuda.get_device_properties(device).multi_processor_count * 128 *
+                                     ((clocks or {}).get("sm_max_mhz") or 1965.0) * 1e-6,
                      "peak_bf16_ratio_rule": peak_rule, "frac_of_bf16_ratio_rule": achieved / peak_rule,
                      "peak_bf16_ratio_rule_source": "%s bf16_tflops x nominal FP64/BF16 ratio 45/2250" % peak_src,
                      "instruction_path": "FP64 tensor: mma.sync.m8n8k4.f64 = SASS DMMA.8x8x4; operands staged by cp.async.bulk.tensor (UTMALDG)",

@@ -96,6 +96,24 @@ __device__ __forceinline__ void tma_box(unsigned dst, const void* map, int c0, i
       : "memory");
 }
 
+// L2 eviction priority of the A / D / E boxes (0 evict_normal, 1 evict_last, 2 evict_first).  Measured at cfg4's block sizes
+// (DESIGN.md section 7): the apply time is the same for every combination (the kernel is not bound by its loads); DRAM
+// reads are lowest with E evict_last (every sibling CTA and every position re-reads it) and A, D left alone --
+// evict_first on the D boxes, round 1's choice, costs 20 % more DRAM traffic here because sibling row-tile CTAs arrive late.
+#ifndef SU2_POL_A
+#define SU2_POL_A 0
+#define SU2_POL_D 0
+#define SU2_POL_E 1
+#endif
+template <int KIND>
+__device__ __forceinline__ uint64_t l2_policy() {
+  uint64_t pol;
+  if (KIND == 1) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(pol));
+  else if (KIND == 2) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(pol));
+  else asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;\n" : "=l"(pol));
+  return pol;
+}
+
 __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
   asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
       : "+d"(c[0]), "+d"(c[1])
@@ -113,7 +131,7 @@ template <int WR>
 __device__ __forceinline__ void produce_item(const DevWork& wk, int w, bool reset, const DevUnit* __restrict__ units,
                                              const DevTask* __restrict__ tasks, const CUtensorMap* __restrict__ maps,
                                              unsigned stage0, PhaseInfo* ring, uint64_t* full, uint64_t* empty, Pipe& pp,
-                                             uint64_t pol_stream, uint64_t pol_keep) {
+                                             uint64_t pol_a, uint64_t pol_d, uint64_t pol_e) {
   using C = TileCfg<WR>;
   constexpr int NS = C::NSTAGE;
   constexpr int NEB = C::NEBOX, NDB = C::NDBOX;
@@ -148,10 +166,11 @@ __device__ __forceinline__ void produce_item(const DevWork& wk, int w, bool rese
         {
           PhaseInfo& pi = ring[pp.pq & (PHASE_RING - 1)];
           pi.scale = scale;
-          // a first product of more than NS stages cannot be finished by any warp before every warp has left the
-          // previous second product (a stage is refilled only after all twelve warps released it): no barrier is
-          // then needed in front of the T store
-          pi.flags = ((tflags & TASK_TRANS_A) ? PH_TRANS : 0) | (first ? PH_FIRST : 0) | (nsteps1 > NS ? PH_NOBAR : 0);
+          // No barrier is needed in front of the T store when the first product has at least NS stages: its stage NS-1
+          // refills the ring slot of the LAST stage of the previous second product, and a slot is refilled only after all
+          // twelve warps have released it -- so a warp that has consumed the whole first product knows that every warp has
+          // left the previous second product (has stopped reading T)
+          pi.flags = ((tflags & TASK_TRANS_A) ? PH_TRANS : 0) | (first ? PH_FIRST : 0) | ((nsteps1 >= NS && !first) ? PH_NOBAR : 0);
           pi.nsteps = nsteps1;
           pi.ktot = k;
           pi.ncw = ncw;
@@ -164,11 +183,11 @@ __device__ __forceinline__ void produce_item(const DevWork& wk, int w, bool rese
             mbar_arrive_expect_tx(&full[b], a_bytes + E_BYTES);     // (release: the phase record is visible)
             const unsigned st = stage0 + (unsigned)b * (C::STAGE * 8u);
             const int k0 = s * KS1;
-            if (tflags & TASK_TRANS_A) tma_box(st, mA, wk.row0, k0, pos * posA, &full[b], pol_stream);
-            else tma_box(st, mA, k0, wk.row0, pos * posA, &full[b], pol_stream);
+            if (tflags & TASK_TRANS_A) tma_box(st, mA, wk.row0, k0, pos * posA, &full[b], pol_a);
+            else tma_box(st, mA, k0, wk.row0, pos * posA, &full[b], pol_a);
 #pragma unroll
             for (int e = 0; e < NEB; ++e)
-              tma_box(st + (unsigned)(C::A_SZ + e * EBOX_SZ) * 8u, mE, n0 + e * EBOX_C, k0, e_item, &full[b], pol_keep);
+              tma_box(st + (unsigned)(C::A_SZ + e * EBOX_SZ) * 8u, mE, n0 + e * EBOX_C, k0, e_item, &full[b], pol_e);
             pp.par ^= 1u << b;
             pp.b = (b + 1 == NS) ? 0 : b + 1;
           }
@@ -194,8 +213,8 @@ __device__ __forceinline__ void produce_item(const DevWork& wk, int w, bool rese
             const int kk = n0 + s * KS2;
 #pragma unroll
             for (int d = 0; d < NDB; ++d) {
-              if (tflags & TASK_TRANS_D) tma_box(st + (unsigned)(d * DBOX_SZ) * 8u, mD, wk.col0 + d * DBOX_C, kk, pos * posD, &full[b], pol_stream);
-              else tma_box(st + (unsigned)(d * DBOX_SZ) * 8u, mD, kk, wk.col0 + d * DBOX_C, pos * posD, &full[b], pol_stream);
+              if (tflags & TASK_TRANS_D) tma_box(st + (unsigned)(d * DBOX_SZ) * 8u, mD, wk.col0 + d * DBOX_C, kk, pos * posD, &full[b], pol_d);
+              else tma_box(st + (unsigned)(d * DBOX_SZ) * 8u, mD, kk, wk.col0 + d * DBOX_C, pos * posD, &full[b], pol_d);
             }
             pp.par ^= 1u << b;
             pp.b = (b + 1 == NS) ? 0 : b + 1;
@@ -424,9 +443,7 @@ heff_tma_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __re
   if (warp < NPRODUCERS) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(PRODUCER_REGS));
     if (tid != 0) return;
-    uint64_t pol_stream, pol_keep;
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(pol_stream));
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(pol_keep));
+    const uint64_t pol_a = l2_policy<SU2_POL_A>(), pol_d = l2_policy<SU2_POL_D>(), pol_e = l2_policy<SU2_POL_E>();
     Pipe pp{0, 0u, 0u};
     int w = atomicAdd(counter, 1);
 #pragma unroll 1
@@ -442,9 +459,9 @@ heff_tma_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __re
       const int wn = atomicAdd(counter, 1);
       const bool reset = wn >= nwork || work[wn].wr != wk.wr;
       const unsigned stage0 = smem_u32(smem + (wk.wr == 1 ? TileCfg<1>::T_SZ : wk.wr == 2 ? TileCfg<2>::T_SZ : TileCfg<4>::T_SZ));
-      if (wk.wr == 1) produce_item<1>(wk, w, reset, units, tasks, maps, stage0, ring, full, empty, pp, pol_stream, pol_keep);
-      else if (wk.wr == 2) produce_item<2>(wk, w, reset, units, tasks, maps, stage0, ring, full, empty, pp, pol_stream, pol_keep);
-      else produce_item<4>(wk, w, reset, units, tasks, maps, stage0, ring, full, empty, pp, pol_stream, pol_keep);
+      if (wk.wr == 1) produce_item<1>(wk, w, reset, units, tasks, maps, stage0, ring, full, empty, pp, pol_a, pol_d, pol_e);
+      else if (wk.wr == 2) produce_item<2>(wk, w, reset, units, tasks, maps, stage0, ring, full, empty, pp, pol_a, pol_d, pol_e);
+      else produce_item<4>(wk, w, reset, units, tasks, maps, stage0, ring, full, empty, pp, pol_a, pol_d, pol_e);
       if (reset) {
         // the stage geometry changes (or the stream ends): wait until every stage in flight has been released
         for (int i = 0; i < MAX_STAGE; ++i) mbar_wait(&empty[i], ((pp.par >> i) & 1) ^ 1);
