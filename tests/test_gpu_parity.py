@@ -146,6 +146,35 @@ def test_sharded_davidson_reduce_hook():
     bad.close()
 
 
+def test_reduce_hook_that_raises_stops_the_step_and_is_re_raised():
+    """a Python exception inside the all-reduce hook (an NCCL error, a failed assert) must not be swallowed by
+    ctypes: the C call stops with a negative status instead of continuing on an un-reduced vector, and the original
+    exception comes out of step() / of the constructor."""
+    torch = _torch()
+    from paper_2309_16724_b200.binding import Davidson
+    op = _operator(config_problem("mini"))
+    x0 = torch.from_numpy(random_psi(op.psi_len, seed=8)).cuda()
+    ws = torch.empty(Davidson.workspace_bytes(op.plan, 4), dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream().cuda_stream
+    calls = []
+
+    def hook(vec, n, st):
+        calls.append(n)
+        if len(calls) == 2:
+            raise RuntimeError("collective failed")
+        return 0
+    dav = Davidson(op.plan, 4, x0.data_ptr(), ws.data_ptr(), stream, reduce=hook)
+    with pytest.raises(RuntimeError, match="collective failed"):
+        dav.step(op.workspace.data_ptr(), stream)
+    assert len(calls) == 2
+    dav.close()
+
+    def bad_from_the_start(vec, n, st):
+        raise ValueError("no communicator")
+    with pytest.raises(ValueError, match="no communicator"):
+        Davidson(op.plan, 4, x0.data_ptr(), ws.data_ptr(), stream, reduce=bad_from_the_start)
+
+
 def test_sharded_davidson_two_shards_on_one_gpu():
     """Two position shards, both resident on this GPU.  The solver runs on shard 0; its reduce hook adds shard 1's
     share (what the all-reduce delivers): the diagonal at create time, then H_1 v for the vector the step just

@@ -109,3 +109,33 @@ def test_cc_count_matches_the_planner(lib):
         cc, ntask, ntp = cc_flops(prob)
         assert ntask == plan.info["ntasks"] and ntp == plan.info["ntask_positions"]
         assert cc == plan.info["cc_flops"]
+
+
+def test_planner_wigner_symbols_equal_exact_arithmetic_up_to_the_spin_cap(lib):
+    """the planner's factorial-based 6j / 9j (long double) against oracle/wigner.py (exact rational arithmetic)
+    over the whole admitted range (doubled arguments <= 40); arguments beyond the cap give NaN from the exported symbol and
+    SU2_ERR_INVALID_RANK from su2_plan_create instead of silently wrong coefficients."""
+    import random
+    from oracle.wigner import w6j, w9j
+    from paper_2309_16724_b200 import Plan, Su2Error
+    from paper_2309_16724_b200.binding import wigner_6j, wigner_9j
+    rnd = random.Random(3)
+    n = 0
+    while n < 1500:
+        a, b, d, e = (rnd.randrange(0, 41) for _ in range(4))
+        cs = [c for c in range(abs(a - b), min(a + b, 40) + 1, 2) if abs(d - e) <= c <= d + e and (c + d + e) % 2 == 0]
+        fs = [f for f in range(abs(a - e), min(a + e, 40) + 1, 2) if abs(b - d) <= f <= b + d and (b + d + f) % 2 == 0]
+        if not cs or not fs:
+            continue
+        c, f = rnd.choice(cs), rnd.choice(fs)
+        assert abs(wigner_6j(a, b, c, d, e, f) - w6j(a, b, c, d, e, f)) <= 1e-14
+        n += 1
+    for args in [(1, 1, 0, 1, 1, 0, 0, 0, 0), (1, 1, 2, 1, 1, 2, 2, 2, 0), (4, 3, 5, 2, 1, 3, 4, 2, 4), (2, 1, 3, 1, 1, 2, 1, 2, 1)]:
+        assert abs(wigner_9j(*args) - w9j(*args)) <= 1e-14
+    assert wigner_6j(1, 1, 1, 1, 1, 1) == 0.0                       # violates a triangle rule
+    assert np.isnan(wigner_6j(42, 2, 42, 2, 42, 2)) and np.isnan(wigner_9j(*([42] * 9)))
+    prob = config_problem("mini", fill=False)
+    prob.sec_l[0].twoS = 42
+    with pytest.raises(Su2Error) as info:
+        Plan(prob, host_only=True)
+    assert "status -3" in str(info.value)
