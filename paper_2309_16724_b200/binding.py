@@ -411,3 +411,54 @@ def noalloc_scratch_bytes():
 
 def kernel_launch_count():
     return int(load().su2_kernel_launch_count())
+
+
+# ---- include/su2_ozaki.h: the GEMM pair on the INT8 tensor path (libsu2ozaki.so) ----------------------------
+OZAKI_LIB_PATH = os.path.join(HERE, "libsu2ozaki.so")
+_ozaki = None
+
+
+def load_ozaki():
+    global _ozaki
+    if _ozaki is None:
+        if not os.path.exists(OZAKI_LIB_PATH):
+            raise Su2Error("%s is missing: run python -m paper_2309_16724_b200.build" % OZAKI_LIB_PATH)
+        lib = C.CDLL(OZAKI_LIB_PATH)
+        dp = C.c_void_p
+        lib.su2_gemm_pair_batched_i8.restype = C.c_int32
+        lib.su2_gemm_pair_batched_i8.argtypes = [C.c_int32] * 4 + [C.c_int64, C.c_double, dp, dp, dp, dp, C.c_int32, dp, C.c_size_t, dp]
+        lib.su2_matmul_batched_i8.restype = C.c_int32
+        lib.su2_matmul_batched_i8.argtypes = [C.c_int32] * 3 + [C.c_int64, dp, dp, dp, C.c_int32, dp, C.c_size_t, dp]
+        lib.su2_ozaki_workspace_bytes.restype = C.c_size_t
+        lib.su2_ozaki_workspace_bytes.argtypes = [C.c_int32] * 4 + [C.c_int64, C.c_int32]
+        lib.su2_ozaki_launch_count.restype = C.c_int64
+        lib.su2_ozaki_launch_count.argtypes = []
+        lib.su2_ozaki_last_error.restype = C.c_char_p
+        lib.su2_ozaki_last_error.argtypes = []
+        _ozaki = lib
+    return _ozaki
+
+
+def _check_ozaki(st):
+    if st != 0:
+        raise Su2Error("su2_ozaki status %d: %s" % (st, load_ozaki().su2_ozaki_last_error().decode()))
+
+
+def gemm_pair_batched_i8(m, k, n, p, batch, alpha, a_ptr, x_ptr, b_ptr, c_ptr, stream=0, nslices=0, workspace_ptr=None,
+                         workspace_bytes=0):
+    """C_b += alpha A_b X_b B_b^T on the INT8 tensor path (su2_gemm_pair_batched_i8): device pointers, dense strides."""
+    _check_ozaki(load_ozaki().su2_gemm_pair_batched_i8(m, k, n, p, batch, alpha, a_ptr, x_ptr, b_ptr, c_ptr, nslices, workspace_ptr,
+                                                       workspace_bytes, stream))
+
+
+def matmul_batched_i8(m, k, n, batch, a_ptr, x_ptr, c_ptr, stream=0, nslices=0, workspace_ptr=None, workspace_bytes=0):
+    """C_b = A_b X_b on the INT8 tensor path (su2_matmul_batched_i8)."""
+    _check_ozaki(load_ozaki().su2_matmul_batched_i8(m, k, n, batch, a_ptr, x_ptr, c_ptr, nslices, workspace_ptr, workspace_bytes, stream))
+
+
+def ozaki_workspace_bytes(m, k, n, p, items, nslices=0):
+    return int(load_ozaki().su2_ozaki_workspace_bytes(m, k, n, p, items, nslices))
+
+
+def ozaki_launch_count():
+    return int(load_ozaki().su2_ozaki_launch_count())

@@ -1,6 +1,7 @@
 """Build step: compiles the CUDA kernels + C-ABI into paper_2309_16724_b200/libsu2heff.so
-(in-tree, sm_100a) with nvcc.  Used by __graft_entry__.build() and by `python -m
-paper_2309_16724_b200.build`."""
+(in-tree, sm_100a) with nvcc, the measurement probe into libsu2probe.so and the INT8-sliced GEMM pair
+(include/su2_ozaki.h, needs the CUTLASS/CuTe header tree vendored in site-packages) into libsu2ozaki.so.
+Used by __graft_entry__.build() and by `python -m paper_2309_16724_b200.build`."""
 import os
 import subprocess
 import sys
@@ -10,18 +11,58 @@ ROOT = os.path.dirname(HERE)
 SOURCES = ["plan.cpp", "tensor_maps.cpp", "kernels.cu", "heff_tma.cu", "heff_small.cu", "davidson.cu", "gemm_pair.cu", "gemm_pair_small.cu", "precontract.cu", "renorm.cu", "apply_noalloc.cu"]
 LIB = os.path.join(HERE, "libsu2heff.so")
 PROBE_LIB = os.path.join(HERE, "libsu2probe.so")      # measurement aid of bench.py (include/su2_probe.h), not the product
+OZAKI_LIB = os.path.join(HERE, "libsu2ozaki.so")      # include/su2_ozaki.h: GEMM pair on the INT8 tensor path (row f4)
+OZAKI_SOURCES = ["ozaki.cu"]
+
+
+def cutlass_root():
+    """The CUTLASS/CuTe header tree this image vendors (header-only; versions 4.x carry the sm_100 collective builder)."""
+    env = os.environ.get("CUTLASS_ROOT")
+    cands = [env] if env else []
+    for sp in sys.path:
+        cands += [os.path.join(sp, "flashinfer", "data", "cutlass"), os.path.join(sp, "tilelang", "3rdparty", "cutlass")]
+    for c in cands:
+        if c and os.path.exists(os.path.join(c, "include", "cutlass", "gemm", "collective", "collective_builder.hpp")):
+            return c
+    raise RuntimeError("no CUTLASS header tree found (set CUTLASS_ROOT): libsu2ozaki.so cannot be built")
 
 
 def _stale():
     if not os.path.exists(LIB) or not os.path.exists(PROBE_LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(HERE, "csrc", f) for f in os.listdir(os.path.join(HERE, "csrc"))]
+    deps = [os.path.join(HERE, "csrc", f) for f in os.listdir(os.path.join(HERE, "csrc")) if f not in OZAKI_SOURCES]
     deps.append(os.path.join(ROOT, "include", "su2_heff.h"))
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+def _ozaki_stale():
+    if not os.path.exists(OZAKI_LIB):
+        return True
+    t = os.path.getmtime(OZAKI_LIB)
+    deps = [os.path.join(HERE, "csrc", f) for f in OZAKI_SOURCES] + [os.path.join(ROOT, "include", "su2_ozaki.h")]
+    return any(os.path.getmtime(d) > t for d in deps)
+
+
+def build_ozaki(force=False):
+    """libsu2ozaki.so: a few minutes of template instantiation, so it is rebuilt only when its own sources changed."""
+    if not force and not _ozaki_stale():
+        return OZAKI_LIB
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    cr = cutlass_root()
+    cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--expt-relaxed-constexpr",
+           "-Xcompiler", "-fPIC", "-shared", "-I" + os.path.join(ROOT, "include"), "-I" + os.path.join(cr, "include"),
+           "-I" + os.path.join(cr, "tools", "util", "include")]
+    cmd += [os.path.join(HERE, "csrc", s) for s in OZAKI_SOURCES] + ["-o", OZAKI_LIB]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if res.returncode != 0:
+        sys.stderr.write(res.stdout + res.stderr)
+        raise RuntimeError("nvcc failed building libsu2ozaki.so")
+    return OZAKI_LIB
+
+
 def build(force=False, verbose=False):
+    build_ozaki(force)
     if not force and not _stale():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")

@@ -1,0 +1,401 @@
+// libsu2ozaki.so (include/su2_ozaki.h): the strided-batched FP64 GEMM pair on the INT8 tensor path
+// (the FP64 ceiling the paper's headline is quoted against).
+//
+// tcgen05.mma has no f64 kind and DMMA runs at the DFMA rate on sm_100a (37 TFLOP/s), so the road past that ceiling with
+// tensor units is exact integer arithmetic on tcgen05.mma kind::i8 (int32 accumulators in TMEM).  Per product L (M x K) . R (K x N),
+// following oracle/ozaki.py step by step:
+//   1. every row of L and every column of R is scaled by a power of two to |v| < 1 (exponents e_i, f_j);
+//   2. and cut into S slices of 7 bits by truncation (INT8 in [-127, 127]);
+//   3. the slice pairs (s, t) with s + t = d are ONE exact INT8 GEMM with int32 accumulation over the concatenated
+//      contraction index of length (d+1) K: L's slices are stored 0..S-1 along its rows, R's slices S-1..0 along its
+//      contraction index, so a diagonal is a prefix window of one and a suffix window of the other -- S GEMMs, S(S+1)/2 pairs;
+//   4. the S integer planes are recombined in FP64, smallest first, and scaled by 2^(e_i + f_j).
+// The pair C += alpha (A X) B^T runs product 1 with R = X as stored (rows = contraction index: an MN-major INT8 operand, no
+// transposition) and product 2 with R = B^T (B's rows are K-major as stored).  Recombining product 1 and slicing its result T for
+// product 2 is one kernel (T is never written in FP64).
+//
+// The INT8 GEMM is generated from the CUTLASS 4.x sm_100 collective builder (vendored CuTe/CUTLASS header templates: TMA loads,
+// tcgen05.mma.cta_group::1.kind::i8 issued by one thread, TMEM accumulators, SASS UTCIMMA); everything else here is hand-written.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <atomic>
+#include <cstdio>
+#include <cstring>
+
+#include "cutlass/cutlass.h"
+#include "cute/tensor.hpp"
+#include "cutlass/gemm/device/gemm_universal_adapter.h"
+#include "cutlass/gemm/kernel/gemm_universal.hpp"
+#include "cutlass/gemm/collective/collective_builder.hpp"
+#include "cutlass/epilogue/collective/collective_builder.hpp"
+
+#include "su2_ozaki.h"
+
+namespace su2oz {
+
+constexpr int OZ_W = 7;                     // bits per slice
+constexpr int OZ_SMAX = SU2_OZAKI_MAX_SLICES;
+constexpr int OZ_OK = 0, OZ_INVALID = -1, OZ_CUDA = -5;
+
+thread_local char g_err[256] = "";
+std::atomic<int64_t> g_launches{0};
+
+int fail(int code, const char* what, cudaError_t e = cudaSuccess) {
+  if (e != cudaSuccess) snprintf(g_err, sizeof(g_err), "%s: %s", what, cudaGetErrorString(e));
+  else snprintf(g_err, sizeof(g_err), "%s", what);
+  return code;
+}
+
+// 2^e for any int e reachable from finite doubles (two exact factors keep each inside the normal range)
+__device__ __forceinline__ double scale2(double v, int e) { return ldexp(v, e); }
+
+// exponent of the scaling of a line with largest magnitude amax: amax 2^-e in [0.5, 1), 0 for a zero line
+__device__ __forceinline__ int line_exponent(double amax) {
+  int e = 0;
+  if (amax > 0.0) (void)frexp(amax, &e);
+  return e;
+}
+
+// the S slices of v (|v| < 1), truncation toward zero; exact in FP64 (oracle/ozaki.py step 2)
+template <int S>
+__device__ __forceinline__ void slices_of(double v, int8_t (&q)[OZ_SMAX]) {
+#pragma unroll
+  for (int s = 0; s < S; ++s) {
+    v *= (double)(1 << OZ_W);
+    const double t = trunc(v);
+    q[s] = (int8_t)(int)t;
+    v -= t;
+  }
+}
+
+// ---- slicing of a K-major operand: one warp per row --------------------------------------------------------------------------------
+// src: nlines rows of `len` FP64 (len % 4 == 0), row pitch ld.  Slice s of row r goes to q[r * (S len) + slot(s) * len + j],
+// slot(s) = s (left operand) or S-1-s (REVERSED: right operand); expo[r] = the row's exponent.  Each lane owns 4 consecutive
+// elements (two 16-byte loads, one 4-byte store per slice: a warp writes 128 contiguous bytes).
+template <int S, bool REVERSED>
+__global__ void __launch_bounds__(256)
+slice_rows_kernel(const double* __restrict__ src, int64_t ld, int len, int64_t nlines, int8_t* __restrict__ q, int32_t* __restrict__ expo) {
+  const int lane = threadIdx.x & 31;
+  const int64_t line = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (line >= nlines) return;
+  const double* __restrict__ row = src + line * ld;
+  double amax = 0.0;
+  for (int j = lane * 4; j < len; j += 128) {
+    const double2 a = *(const double2*)(row + j), b = *(const double2*)(row + j + 2);
+    amax = fmax(fmax(amax, fmax(fabs(a.x), fabs(a.y))), fmax(fabs(b.x), fabs(b.y)));
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) amax = fmax(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+  const int e = line_exponent(amax);
+  if (lane == 0) expo[line] = e;
+  int8_t* __restrict__ out = q + line * (int64_t)S * len;
+  for (int j = lane * 4; j < len; j += 128) {
+    const double2 a = *(const double2*)(row + j), b = *(const double2*)(row + j + 2);
+    int8_t q0[OZ_SMAX], q1[OZ_SMAX], q2[OZ_SMAX], q3[OZ_SMAX];
+    slices_of<S>(scale2(a.x, -e), q0); slices_of<S>(scale2(a.y, -e), q1);
+    slices_of<S>(scale2(b.x, -e), q2); slices_of<S>(scale2(b.y, -e), q3);
+#pragma unroll
+    for (int s = 0; s < S; ++s)
+      *(char4*)(out + (int64_t)(REVERSED ? S - 1 - s : s) * len + j) = make_char4(q0[s], q1[s], q2[s], q3[s]);
+  }
+}
+
+// ---- slicing of an MN-major right operand (X: k x n as stored, contraction index along its rows): one CTA per (128-column strip, item)
+// expo[item * n + c] = exponent of column c; slice s of element (j, c) goes to q[item][(S-1-s) * k + j][c] (row pitch n).
+template <int S>
+__global__ void __launch_bounds__(256)
+slice_cols_kernel(const double* __restrict__ src, int k, int n, int8_t* __restrict__ q, int32_t* __restrict__ expo) {
+  __shared__ double s_amax[8][128];
+  __shared__ int s_e[128];
+  const int lane = threadIdx.x & 31, wy = threadIdx.x >> 5;
+  const int64_t item = blockIdx.y;
+  const int c = blockIdx.x * 128 + lane * 4;
+  const bool live = c < n;                                   // n % 4 == 0: a thread's 4 columns are all inside or all outside
+  const double* __restrict__ x = src + item * (int64_t)k * n;
+  double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+  if (live)
+    for (int j = wy; j < k; j += 8) {
+      const double2 u = *(const double2*)(x + (int64_t)j * n + c), v = *(const double2*)(x + (int64_t)j * n + c + 2);
+      a0 = fmax(a0, fabs(u.x)); a1 = fmax(a1, fabs(u.y)); a2 = fmax(a2, fabs(v.x)); a3 = fmax(a3, fabs(v.y));
+    }
+  s_amax[wy][lane * 4 + 0] = a0; s_amax[wy][lane * 4 + 1] = a1; s_amax[wy][lane * 4 + 2] = a2; s_amax[wy][lane * 4 + 3] = a3;
+  __syncthreads();
+  if (threadIdx.x < 128) {
+    double a = 0.0;
+#pragma unroll
+    for (int y = 0; y < 8; ++y) a = fmax(a, s_amax[y][threadIdx.x]);
+    const int e = line_exponent(a);
+    s_e[threadIdx.x] = e;
+    if (blockIdx.x * 128 + threadIdx.x < n) expo[item * n + blockIdx.x * 128 + threadIdx.x] = e;
+  }
+  __syncthreads();
+  if (!live) return;
+  const int e0 = s_e[lane * 4], e1 = s_e[lane * 4 + 1], e2 = s_e[lane * 4 + 2], e3 = s_e[lane * 4 + 3];
+  int8_t* __restrict__ out = q + item * (int64_t)S * k * n;
+  for (int j = wy; j < k; j += 8) {
+    const double2 u = *(const double2*)(x + (int64_t)j * n + c), v = *(const double2*)(x + (int64_t)j * n + c + 2);
+    int8_t q0[OZ_SMAX], q1[OZ_SMAX], q2[OZ_SMAX], q3[OZ_SMAX];
+    slices_of<S>(scale2(u.x, -e0), q0); slices_of<S>(scale2(u.y, -e1), q1);
+    slices_of<S>(scale2(v.x, -e2), q2); slices_of<S>(scale2(v.y, -e3), q3);
+#pragma unroll
+    for (int s = 0; s < S; ++s)
+      *(char4*)(out + ((int64_t)(S - 1 - s) * k + j) * n + c) = make_char4(q0[s], q1[s], q2[s], q3[s]);
+  }
+}
+
+// ---- recombination -----------------------------------------------------------------------------------------------------------------
+// value of entry idx of the product from its S integer planes (plane d at planes + d * plane_stride), before the 2^(e+f) scaling:
+//   sum_{d = S-1 .. 0} P_d 2^(-W (d+2)),  smallest first (oracle/ozaki.py step 5); the weights are powers of two, so multiplying is exact.
+template <int S>
+__device__ __forceinline__ void combine4(const int32_t* __restrict__ planes, int64_t plane_stride, int64_t idx, double (&v)[4]) {
+  v[0] = v[1] = v[2] = v[3] = 0.0;
+#pragma unroll
+  for (int d = S - 1; d >= 0; --d) {
+    const int4 pl = *(const int4*)(planes + d * plane_stride + idx);
+    const double w = __hiloint2double((1023 - OZ_W * (d + 2)) << 20, 0);
+    v[0] += (double)pl.x * w; v[1] += (double)pl.y * w; v[2] += (double)pl.z * w; v[3] += (double)pl.w * w;
+  }
+}
+
+// product 1's planes -> slices of T for product 2 (left operand), one warp per row of T (n % 4 == 0):
+// T_ij = 2^(e_i + f_j) sum_d ...; row exponent g_i from max_j |T_ij|; slices of T_ij 2^(-g_i) at qT[row * (S n) + s * n + j].
+// The row is recombined twice (exponent pass, slicing pass; the second read of the planes hits L1/L2) instead of being stored in FP64.
+template <int S>
+__global__ void __launch_bounds__(256)
+combine_slice_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, int rows, int n, int64_t nlines,
+                     const int32_t* __restrict__ e_row, const int32_t* __restrict__ f_col, int8_t* __restrict__ qT,
+                     int32_t* __restrict__ g_row) {
+  const int lane = threadIdx.x & 31;
+  const int64_t line = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (line >= nlines) return;
+  const int64_t item = line / rows;
+  const int e = e_row[line];
+  const int32_t* __restrict__ f = f_col + item * n;
+  double amax = 0.0;
+  for (int j = lane * 4; j < n; j += 128) {
+    double v[4];
+    combine4<S>(planes, plane_stride, line * n + j, v);
+    const int4 fj = *(const int4*)(f + j);
+    amax = fmax(fmax(amax, fmax(fabs(scale2(v[0], e + fj.x)), fabs(scale2(v[1], e + fj.y)))),
+                fmax(fabs(scale2(v[2], e + fj.z)), fabs(scale2(v[3], e + fj.w))));
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) amax = fmax(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+  const int g = line_exponent(amax);
+  if (lane == 0) g_row[line] = g;
+  int8_t* __restrict__ out = qT + line * (int64_t)S * n;
+  for (int j = lane * 4; j < n; j += 128) {
+    double v[4];
+    combine4<S>(planes, plane_stride, line * n + j, v);
+    const int4 fj = *(const int4*)(f + j);
+    int8_t q0[OZ_SMAX], q1[OZ_SMAX], q2[OZ_SMAX], q3[OZ_SMAX];
+    // T_ij 2^-g = v 2^(e + f_j - g): one exact scaling of the recombined sum, as in the oracle (ldexp of T, then ldexp by -g)
+    slices_of<S>(scale2(scale2(v[0], e + fj.x), -g), q0); slices_of<S>(scale2(scale2(v[1], e + fj.y), -g), q1);
+    slices_of<S>(scale2(scale2(v[2], e + fj.z), -g), q2); slices_of<S>(scale2(scale2(v[3], e + fj.w), -g), q3);
+#pragma unroll
+    for (int s = 0; s < S; ++s) *(char4*)(out + (int64_t)s * n + j) = make_char4(q0[s], q1[s], q2[s], q3[s]);
+  }
+}
+
+// planes of a product -> FP64 result: dst = (ACCUMULATE ? dst : 0) + alpha 2^(e_i + f_j) sum_d ...; 4 consecutive columns per thread
+template <int S, bool ACCUMULATE>
+__global__ void __launch_bounds__(256)
+combine_out_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, int rows, int cols, int64_t nquad,
+                   const int32_t* __restrict__ e_row, const int32_t* __restrict__ f_col, double alpha, double* __restrict__ dst) {
+  const int cq = cols >> 2;
+  for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < nquad; t += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t line = t / cq;                              // item * rows + i
+    const int j = (int)(t - line * cq) * 4;
+    const int64_t item = line / rows;
+    double v[4];
+    combine4<S>(planes, plane_stride, line * cols + j, v);
+    const int e = e_row[line];
+    const int4 fj = *(const int4*)(f_col + item * cols + j);
+    double2* o = (double2*)(dst + line * cols + j);
+    double2 lo = ACCUMULATE ? o[0] : make_double2(0.0, 0.0), hi = ACCUMULATE ? o[1] : make_double2(0.0, 0.0);
+    lo.x += alpha * scale2(v[0], e + fj.x); lo.y += alpha * scale2(v[1], e + fj.y);
+    hi.x += alpha * scale2(v[2], e + fj.z); hi.y += alpha * scale2(v[3], e + fj.w);
+    o[0] = lo; o[1] = hi;
+  }
+}
+
+// ---- the exact INT8 GEMM: D (M x N, int32, row-major) = L (M x K, int8, K-major) . R, batched; R is K x N with N contiguous
+// (RMajorN = true: X as stored) or N x K with K contiguous (false: B as stored) -------------------------------------------------------
+using I8Tile = cute::Shape<cute::_128, cute::_128, cute::_128>;
+using I8Cluster = cute::Shape<cute::_1, cute::_1, cute::_1>;
+using I8Epilogue = typename cutlass::epilogue::collective::CollectiveBuilder<
+    cutlass::arch::Sm100, cutlass::arch::OpClassTensorOp, I8Tile, I8Cluster, cutlass::epilogue::collective::EpilogueTileAuto,
+    int32_t, int32_t, int32_t, cutlass::layout::RowMajor, 4, int32_t, cutlass::layout::RowMajor, 4,
+    cutlass::epilogue::collective::EpilogueScheduleAuto>::CollectiveOp;
+template <class LayoutR>
+using I8Mainloop = typename cutlass::gemm::collective::CollectiveBuilder<
+    cutlass::arch::Sm100, cutlass::arch::OpClassTensorOp, int8_t, cutlass::layout::RowMajor, 16, int8_t, LayoutR, 16, int32_t, I8Tile,
+    I8Cluster, cutlass::gemm::collective::StageCountAutoCarveout<static_cast<int>(sizeof(typename I8Epilogue::SharedStorage))>,
+    cutlass::gemm::collective::KernelScheduleAuto>::CollectiveOp;
+template <class LayoutR>
+using I8Gemm = cutlass::gemm::device::GemmUniversalAdapter<
+    cutlass::gemm::kernel::GemmUniversal<cute::Shape<int, int, int, int>, I8Mainloop<LayoutR>, I8Epilogue>>;
+
+template <bool RMajorN>
+int i8_gemm(int M, int N, int K, int L, const int8_t* Lp, int64_t ldl, int64_t batchL, const int8_t* Rp, int64_t ldr, int64_t batchR,
+            int32_t* D, int64_t batchD, cudaStream_t stream) {
+  using Gemm = I8Gemm<std::conditional_t<RMajorN, cutlass::layout::RowMajor, cutlass::layout::ColumnMajor>>;
+  typename Gemm::GemmKernel::StrideA sa = cute::make_stride(ldl, cute::Int<1>{}, batchL);
+  typename Gemm::GemmKernel::StrideB sb;
+  if constexpr (RMajorN) sb = cute::make_stride(cute::Int<1>{}, ldr, batchR);       // (N, K, L): N contiguous
+  else sb = cute::make_stride(ldr, cute::Int<1>{}, batchR);                          // (N, K, L): K contiguous
+  typename Gemm::GemmKernel::StrideD sd = cute::make_stride((int64_t)N, cute::Int<1>{}, batchD);
+  typename Gemm::Arguments args{cutlass::gemm::GemmUniversalMode::kGemm, {M, N, K, L}, {Lp, sa, Rp, sb}, {{1, 0}, D, sd, D, sd}};
+  Gemm gemm;
+  if (gemm.can_implement(args) != cutlass::Status::kSuccess) return fail(OZ_INVALID, "INT8 GEMM: extents or alignment not supported");
+  if (Gemm::get_workspace_size(args) != 0) return fail(OZ_CUDA, "INT8 GEMM: unexpected workspace request");
+  if (gemm.initialize(args, nullptr, stream) != cutlass::Status::kSuccess) return fail(OZ_CUDA, "INT8 GEMM: initialize", cudaGetLastError());
+  if (gemm.run(stream) != cutlass::Status::kSuccess) return fail(OZ_CUDA, "INT8 GEMM: launch", cudaGetLastError());
+  g_launches.fetch_add(1, std::memory_order_relaxed);
+  return OZ_OK;
+}
+
+inline size_t up256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// workspace of a chunk of `c` items (p = 0: single product)
+struct Workspace {
+  size_t qA, qX, planes, qT, qB, eA, fX, gT, hB, total;
+  Workspace(int64_t c, int m, int k, int n, int p, int S) {
+    size_t o = 0;
+    auto take = [&](size_t bytes) { const size_t at = o; o += up256(bytes); return at; };
+    qA = take((size_t)c * m * S * k);
+    qX = take((size_t)c * S * k * n);
+    planes = take((size_t)c * S * 4 * m * std::max(n, p));
+    qT = take(p ? (size_t)c * m * S * n : 0);
+    qB = take(p ? (size_t)c * p * S * n : 0);
+    eA = take((size_t)c * m * 4); fX = take((size_t)c * n * 4);
+    gT = take(p ? (size_t)c * m * 4 : 0); hB = take(p ? (size_t)c * p * 4 : 0);
+    total = o;
+  }
+};
+
+#define OZ_LAUNCH_CHECK(what)                                                    \
+  do {                                                                           \
+    cudaError_t e_ = cudaGetLastError();                                         \
+    if (e_ != cudaSuccess) return fail(OZ_CUDA, what, e_);                       \
+    g_launches.fetch_add(1, std::memory_order_relaxed);                          \
+  } while (0)
+
+// one chunk of c items; p == 0: C (m x n) = A X, else C (m x p) += alpha (A X) B^T
+template <int S>
+int run_chunk(int m, int k, int n, int p, int c, double alpha, const double* A, const double* X, const double* B, double* C,
+              char* ws, cudaStream_t st) {
+  const Workspace w(c, m, k, n, p, S);
+  int8_t *qA = (int8_t*)(ws + w.qA), *qX = (int8_t*)(ws + w.qX), *qT = (int8_t*)(ws + w.qT), *qB = (int8_t*)(ws + w.qB);
+  int32_t *planes = (int32_t*)(ws + w.planes), *eA = (int32_t*)(ws + w.eA), *fX = (int32_t*)(ws + w.fX), *gT = (int32_t*)(ws + w.gT),
+          *hB = (int32_t*)(ws + w.hB);
+  const int64_t rowsA = (int64_t)c * m;
+  slice_rows_kernel<S, false><<<(unsigned)((rowsA + 7) / 8), 256, 0, st>>>(A, k, k, rowsA, qA, eA);
+  OZ_LAUNCH_CHECK("slice_rows_kernel(A) launch");
+  slice_cols_kernel<S><<<dim3((n + 127) / 128, c), 256, 0, st>>>(X, k, n, qX, fX);
+  OZ_LAUNCH_CHECK("slice_cols_kernel(X) launch");
+  const int64_t ps1 = (int64_t)c * m * n;
+  for (int d = 0; d < S; ++d) {                               // diagonal d: L slices 0..d, R slices d..0 = slots S-1-d..S-1
+    const int rc = i8_gemm<true>(m, n, (d + 1) * k, c, qA, (int64_t)S * k, (int64_t)m * S * k, qX + (int64_t)(S - 1 - d) * k * n, n,
+                                 (int64_t)S * k * n, planes + d * ps1, (int64_t)m * n, st);
+    if (rc != OZ_OK) return rc;
+  }
+  if (p == 0) {
+    const int64_t nquad = ps1 / 4;
+    combine_out_kernel<S, false><<<(unsigned)std::min<int64_t>((nquad + 255) / 256, 148 * 16), 256, 0, st>>>(planes, ps1, m, n, nquad, eA, fX, 1.0, C);
+    OZ_LAUNCH_CHECK("combine_out_kernel launch");
+    return OZ_OK;
+  }
+  combine_slice_kernel<S><<<(unsigned)((rowsA + 7) / 8), 256, 0, st>>>(planes, ps1, m, n, rowsA, eA, fX, qT, gT);
+  OZ_LAUNCH_CHECK("combine_slice_kernel launch");
+  const int64_t rowsB = (int64_t)c * p;
+  slice_rows_kernel<S, true><<<(unsigned)((rowsB + 7) / 8), 256, 0, st>>>(B, n, n, rowsB, qB, hB);
+  OZ_LAUNCH_CHECK("slice_rows_kernel(B) launch");
+  const int64_t ps2 = (int64_t)c * m * p;
+  for (int d = 0; d < S; ++d) {
+    const int rc = i8_gemm<false>(m, p, (d + 1) * n, c, qT, (int64_t)S * n, (int64_t)m * S * n, qB + (int64_t)(S - 1 - d) * n,
+                                  (int64_t)S * n, (int64_t)p * S * n, planes + d * ps2, (int64_t)m * p, st);
+    if (rc != OZ_OK) return rc;
+  }
+  const int64_t nquad = ps2 / 4;
+  combine_out_kernel<S, true><<<(unsigned)std::min<int64_t>((nquad + 255) / 256, 148 * 16), 256, 0, st>>>(planes, ps2, m, p, nquad, gT, hB, alpha, C);
+  OZ_LAUNCH_CHECK("combine_out_kernel launch");
+  return OZ_OK;
+}
+
+int run_chunk_s(int S, int m, int k, int n, int p, int c, double alpha, const double* A, const double* X, const double* B, double* C,
+                char* ws, cudaStream_t st) {
+  switch (S) {
+    case 2: return run_chunk<2>(m, k, n, p, c, alpha, A, X, B, C, ws, st);
+    case 3: return run_chunk<3>(m, k, n, p, c, alpha, A, X, B, C, ws, st);
+    case 4: return run_chunk<4>(m, k, n, p, c, alpha, A, X, B, C, ws, st);
+    case 5: return run_chunk<5>(m, k, n, p, c, alpha, A, X, B, C, ws, st);
+    case 6: return run_chunk<6>(m, k, n, p, c, alpha, A, X, B, C, ws, st);
+    default: return run_chunk<7>(m, k, n, p, c, alpha, A, X, B, C, ws, st);
+  }
+}
+
+int run(int m, int k, int n, int p, int64_t batch, double alpha, const double* A, const double* X, const double* B, double* C, int S,
+        void* workspace, size_t workspace_bytes, cudaStream_t st) {
+  g_err[0] = 0;
+  const bool pair = p != 0;
+  if (m <= 0 || k <= 0 || n <= 0 || p < 0 || batch < 0 || !A || !X || !C || (pair && !B)) return fail(OZ_INVALID, "null pointer, non-positive dimension or negative batch");
+  if (S == 0) S = OZ_SMAX;
+  if (S < 2 || S > OZ_SMAX) return fail(OZ_INVALID, "nslices must be 0 or 2..7");
+  if ((k & 15) || (n & 15) || (p & 3)) return fail(OZ_INVALID, "k and n must be multiples of 16 and p a multiple of 4 (INT8 rows are moved by TMA)");
+  if ((int64_t)S * std::max(k, n) * 127 * 127 >= ((int64_t)1 << 31)) return fail(OZ_INVALID, "contraction too long for exact int32 accumulation");
+  if (((uintptr_t)A | (uintptr_t)X | (uintptr_t)B | (uintptr_t)C) & 15) return fail(OZ_INVALID, "operands must be 16-byte aligned");
+  if (workspace && ((uintptr_t)workspace & 255)) return fail(OZ_INVALID, "workspace must be 256-byte aligned");
+  if (batch == 0) return OZ_OK;
+  if (workspace_bytes == 0) {
+    if (workspace) return fail(OZ_INVALID, "workspace given without its size");
+    workspace_bytes = (size_t)2 << 30;
+  }
+  // largest chunk that fits (the table sizes are monotone in c and at most 9 * 256 bytes above linear)
+  const size_t per_item = Workspace(1, m, k, n, p, S).total;
+  if (per_item > workspace_bytes) return fail(OZ_INVALID, "workspace limit below one item");
+  int64_t c = std::min<int64_t>({batch, 65535, (int64_t)(workspace_bytes / per_item) + 1});
+  while (c > 1 && Workspace(c, m, k, n, p, S).total > workspace_bytes) --c;
+  if ((int64_t)c * m * std::max({k, n, p}) * S >= ((int64_t)1 << 40)) return fail(OZ_INVALID, "chunk too large");
+  char* ws = (char*)workspace;
+  if (!ws) {
+    cudaError_t e = cudaMallocAsync((void**)&ws, Workspace(c, m, k, n, p, S).total, st);
+    if (e != cudaSuccess) return fail(OZ_CUDA, "cudaMallocAsync(workspace)", e);
+  }
+  int rc = OZ_OK;
+  const int pp = pair ? p : n;
+  for (int64_t b0 = 0; b0 < batch && rc == OZ_OK; b0 += c) {
+    const int cc = (int)std::min<int64_t>(c, batch - b0);
+    rc = run_chunk_s(S, m, k, n, p, cc, alpha, A + b0 * m * k, X + b0 * k * n, pair ? B + b0 * p * n : nullptr, C + b0 * m * pp, ws, st);
+  }
+  if (!workspace) cudaFreeAsync(ws, st);
+  return rc;
+}
+
+}  // namespace su2oz
+
+using namespace su2oz;
+
+extern "C" int32_t su2_gemm_pair_batched_i8(int32_t m, int32_t k, int32_t n, int32_t p, int64_t batch, double alpha, const double* A,
+                                            const double* X, const double* B, double* C, int32_t nslices, void* workspace,
+                                            size_t workspace_bytes, void* cuda_stream) {
+  if (p <= 0) { g_err[0] = 0; return fail(OZ_INVALID, "null pointer, non-positive dimension or negative batch"); }
+  return run(m, k, n, p, batch, alpha, A, X, B, C, nslices, workspace, workspace_bytes, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int32_t su2_matmul_batched_i8(int32_t m, int32_t k, int32_t n, int64_t batch, const double* A, const double* X, double* C,
+                                         int32_t nslices, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  return run(m, k, n, 0, batch, 1.0, A, X, nullptr, C, nslices, workspace, workspace_bytes, (cudaStream_t)cuda_stream);
+}
+
+extern "C" size_t su2_ozaki_workspace_bytes(int32_t m, int32_t k, int32_t n, int32_t p, int64_t items, int32_t nslices) {
+  if (m <= 0 || k <= 0 || n <= 0 || p < 0 || items <= 0) return 0;
+  if (nslices == 0) nslices = OZ_SMAX;
+  if (nslices < 2 || nslices > OZ_SMAX) return 0;
+  return Workspace(items, m, k, n, p, nslices).total;
+}
+
+extern "C" int64_t su2_ozaki_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+extern "C" const char* su2_ozaki_last_error(void) { return g_err; }

@@ -37,7 +37,18 @@ def test_library_exports_every_declared_symbol(lib):
     probe = ctypes.CDLL(os.path.join(ROOT, "paper_2309_16724_b200", "libsu2probe.so"))
     for name in set(re.findall(r"\b(su2_[a-z0-9_]+)\s*\(", probe_h)):
         assert hasattr(probe, name), name
-    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["su2_heff.h", "su2_probe.h"]
+    # the GEMM pair on the INT8 tensor path is a third library (include/su2_ozaki.h); argument checks run without a GPU
+    ozaki_h = open(os.path.join(ROOT, "include", "su2_ozaki.h")).read()
+    from paper_2309_16724_b200.binding import load_ozaki, ozaki_workspace_bytes
+    oz = load_ozaki()
+    declared_oz = set(re.findall(r"\b(su2_[a-z0-9_]+)\s*\(", ozaki_h))
+    assert {"su2_gemm_pair_batched_i8", "su2_matmul_batched_i8", "su2_ozaki_workspace_bytes"} <= declared_oz
+    for name in declared_oz:
+        assert hasattr(oz, name), name
+    assert oz.su2_gemm_pair_batched_i8(16, 24, 16, 16, 1, 1.0, 16, 16, 16, 16, 0, None, 0, None) == -1
+    assert b"multiples of 16" in oz.su2_ozaki_last_error()
+    assert ozaki_workspace_bytes(512, 512, 512, 512, 1) == 14688256 and ozaki_workspace_bytes(512, 512, 512, 512, 1, 9) == 0
+    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["su2_heff.h", "su2_ozaki.h", "su2_probe.h"]
 
 
 def _cfg1(use_adjoints):
