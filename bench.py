@@ -316,8 +316,47 @@ def run_cfg5(args):
         sweep.append({"m=k=n=p": b, "batch": batch, "ms": ms, "tflops": flops / ms / 1e9,
                       "operand_gbs": 8.0 * 5 * b * b * batch / ms / 1e6})
         del A, X, B, Cm
+    # The same operation on the INT8 tensor path (include/su2_ozaki.h), next to the FP64 tensor route
+    # on the same operands; 1024 and 2048 extend BASELINE.json's shape list to where the FP64 ceiling is passed.
+    from paper_2309_16724_b200.binding import gemm_pair_batched_i8, ozaki_launch_count, ozaki_workspace_bytes
+    sweep_i8 = []
+    li0 = ozaki_launch_count()
+    ws_bytes = 4 << 30
+    ws = torch.empty(ws_bytes, dtype=torch.uint8, device="cuda")
+    for b in (128, 256, 512, 1024, 2048):
+        batch = int(max(8, 1.5e9 / (4 * b * b * 8)))
+        A, X, B, C8, C64 = (torch.randn(batch, b, b, dtype=torch.float64, device="cuda", generator=gen) for _ in range(5))
+        C64.copy_(C8)
+        row = {"m=k=n=p": b, "batch": batch, "nslices": 7,
+               "items_per_chunk": min(batch, max(1, ws_bytes // ozaki_workspace_bytes(b, b, b, b, 1)))}
+        for name, Cm, call in (("i8", C8, lambda: gemm_pair_batched_i8(b, b, b, b, batch, 0.5, A.data_ptr(), X.data_ptr(), B.data_ptr(),
+                                                                      C8.data_ptr(), stream, 7, ws.data_ptr(), ws_bytes)),
+                               ("fp64", C64, lambda: gemm_pair_batched(b, b, b, b, batch, 0.5, A.data_ptr(), X.data_ptr(), B.data_ptr(),
+                                                                      C64.data_ptr(), stream))):
+            call()                                     # the first call of each route on identical C: compared below
+            if name == "fp64":
+                row["max_diff_over_max_abs"] = float((C8 - C64).abs().max() / C64.abs().max())
+            for _ in range(max(3, args.warmup)):
+                call()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(args.steps):
+                call()
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / args.steps
+            row["ms_" + name], row["tflops_" + name] = ms, 4.0 * b ** 3 * batch / ms / 1e9
+            if name == "i8":                           # put C8 back to one call's worth for the comparison
+                C8.copy_(C64)
+                call()
+        sweep_i8.append(row)
+        del A, X, B, C8, C64
+    del ws
+    launches_i8 = ozaki_launch_count() - li0
     dmma = probe_fp64_peak(1, 4000, 4, stream)
     peaks, peak_src = measured_peaks()
+    for r in sweep_i8:
+        r["i8_over_fp64_tensor_peak"] = r["tflops_i8"] / dmma
     for r in sweep:   # algorithmic bytes per item: A, X, B read, C read + written (8 * 5 b^2)
         r["hbm_frac"] = r["operand_gbs"] / peaks["hbm_gbs"]
         r["tensor_frac"] = r["tflops"] / dmma
@@ -329,7 +368,11 @@ def run_cfg5(args):
                       "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                       "config": {"workload": "cfg5: strided-batched GEMM-pair microbenchmark (BASELINE.json configs[4]), square shapes; "
                                              "value = best shape", "l2": "operands 1.5 GB per shape exceed L2"},
-                      "gpu_launches": kernel_launch_count() - l0, "sweep": sweep,
+                      "gpu_launches": kernel_launch_count() - l0 + launches_i8, "sweep": sweep,
+                      "int8_path": {"what": "the same GEMM pair by su2_gemm_pair_batched_i8: 7 INT8 slices of 7 bits, exact "
+                                            "tcgen05 kind::i8 products, FP64 recombination (oracle/ozaki.py); tflops = 4 b^3 "
+                                            "batch / time, the FP64-equivalent rate; NOT the line's value",
+                                    "fp64_tensor_peak_measured": dmma, "gpu_launches": launches_i8, "sweep": sweep_i8},
                       "roofline": {"bound": "tensor", "achieved": best["tflops"], "peak": dmma, "unit": UNIT,
                                    "frac": best["tflops"] / dmma, "traffic": None},
                       "roofline_small_blocks": {"bound": "hbm", "kernel": "gemm_pair_small_kernel",

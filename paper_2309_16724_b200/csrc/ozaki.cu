@@ -15,7 +15,7 @@
 // product 2 is one kernel (T is never written in FP64).
 //
 // The INT8 GEMM is generated from the CUTLASS 4.x sm_100 collective builder (vendored CuTe/CUTLASS header templates: TMA loads,
-// tcgen05.mma.cta_group::1.kind::i8 issued by one thread, TMEM accumulators, SASS UTCIMMA); everything else here is hand-written.
+// tcgen05.mma.cta_group::{1,2}.kind::i8 issued by one thread, TMEM accumulators, SASS UTCIMMA); everything else here is hand-written.
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -47,26 +47,41 @@ int fail(int code, const char* what, cudaError_t e = cudaSuccess) {
   return code;
 }
 
-// 2^e for any int e reachable from finite doubles (two exact factors keep each inside the normal range)
-__device__ __forceinline__ double scale2(double v, int e) { return ldexp(v, e); }
+// v 2^e, exact (ldexp); the factor 2^e is built from its bits when it is a normal number, which gives ldexp's result in one
+// multiplication (a power-of-two factor is exact, and where the product is subnormal both round the same way)
+__device__ __forceinline__ double scale2(double v, int e) {
+  return (e >= -1022 && e <= 1023) ? v * __hiloint2double((1023 + e) << 20, 0) : ldexp(v, e);
+}
 
-// exponent of the scaling of a line with largest magnitude amax: amax 2^-e in [0.5, 1), 0 for a zero line
-__device__ __forceinline__ int line_exponent(double amax) {
-  int e = 0;
-  if (amax > 0.0) (void)frexp(amax, &e);
+// |a| as an ordered integer: for finite doubles the order of the bit patterns of |a| is the order of the magnitudes
+__device__ __forceinline__ unsigned long long abs_bits(double a) { return (unsigned long long)__double_as_longlong(a) & 0x7fffffffffffffffull; }
+
+// exponent of the scaling of a line whose largest magnitude has the bit pattern amax: amax 2^-e in [0.5, 1); 0 for a zero line
+// (oracle/ozaki.py step 1: floor(log2 amax) + 1).  Normal numbers read it off the exponent field.
+__device__ __forceinline__ int line_exponent(unsigned long long amax) {
+  if (amax == 0) return 0;
+  const int E = (int)(amax >> 52);
+  if (E) return E - 1022;
+  int e;
+  (void)frexp(__longlong_as_double((long long)amax), &e);      // subnormal maximum
   return e;
 }
 
-// the S slices of v (|v| < 1), truncation toward zero; exact in FP64 (oracle/ozaki.py step 2)
+// The S slices of v = a 2^-e (|v| < 1) by truncation toward zero (oracle/ozaki.py step 2: t = 128 v; q = trunc(t); t -= q; ...).
+// Every step of that recurrence is exact, so the slices are the base-128 digits of |v|, signed: with a = +-M 2^(E-1075)
+// (M the 53-bit significand), floor(|v| 2^(7S)) = M >> (1075 - 7S + e - E) and q_s = +-((that >> 7(S-1-s)) & 127) -- integer
+// shifts instead of 4 S dependent FP64 operations per element (the slicing kernels were bound by the FP64 pipe).
 template <int S>
-__device__ __forceinline__ void slices_of(double v, int8_t (&q)[OZ_SMAX]) {
+__device__ __forceinline__ void slices_of(double a, int e, int8_t (&q)[OZ_SMAX]) {
+  const long long bits = __double_as_longlong(a);
+  int E = (int)((bits >> 52) & 0x7ff);
+  unsigned long long M = (unsigned long long)bits & 0xfffffffffffffull;
+  if (E) M |= 1ull << 52; else E = 1;                           // subnormal: no hidden bit, exponent of the smallest normal
+  const int sh = 1075 - OZ_W * S + e - E;                       // >= 53 - 7 S > 0 because |v| < 1
+  const unsigned long long fx = sh < 64 ? M >> sh : 0ull;
+  const int sgn = bits < 0 ? -1 : 1;
 #pragma unroll
-  for (int s = 0; s < S; ++s) {
-    v *= (double)(1 << OZ_W);
-    const double t = trunc(v);
-    q[s] = (int8_t)(int)t;
-    v -= t;
-  }
+  for (int s = 0; s < S; ++s) q[s] = (int8_t)(sgn * (int)((fx >> (OZ_W * (S - 1 - s))) & 127));
 }
 
 // ---- slicing of a K-major operand: one warp per row --------------------------------------------------------------------------------
@@ -80,21 +95,21 @@ slice_rows_kernel(const double* __restrict__ src, int64_t ld, int len, int64_t n
   const int64_t line = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (line >= nlines) return;
   const double* __restrict__ row = src + line * ld;
-  double amax = 0.0;
+  unsigned long long amax = 0;
   for (int j = lane * 4; j < len; j += 128) {
     const double2 a = *(const double2*)(row + j), b = *(const double2*)(row + j + 2);
-    amax = fmax(fmax(amax, fmax(fabs(a.x), fabs(a.y))), fmax(fabs(b.x), fabs(b.y)));
+    amax = max(max(amax, max(abs_bits(a.x), abs_bits(a.y))), max(abs_bits(b.x), abs_bits(b.y)));
   }
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) amax = fmax(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+  for (int o = 16; o > 0; o >>= 1) amax = max(amax, __shfl_xor_sync(0xffffffffu, amax, o));
   const int e = line_exponent(amax);
   if (lane == 0) expo[line] = e;
   int8_t* __restrict__ out = q + line * (int64_t)S * len;
   for (int j = lane * 4; j < len; j += 128) {
     const double2 a = *(const double2*)(row + j), b = *(const double2*)(row + j + 2);
     int8_t q0[OZ_SMAX], q1[OZ_SMAX], q2[OZ_SMAX], q3[OZ_SMAX];
-    slices_of<S>(scale2(a.x, -e), q0); slices_of<S>(scale2(a.y, -e), q1);
-    slices_of<S>(scale2(b.x, -e), q2); slices_of<S>(scale2(b.y, -e), q3);
+    slices_of<S>(a.x, e, q0); slices_of<S>(a.y, e, q1);
+    slices_of<S>(b.x, e, q2); slices_of<S>(b.y, e, q3);
 #pragma unroll
     for (int s = 0; s < S; ++s)
       *(char4*)(out + (int64_t)(REVERSED ? S - 1 - s : s) * len + j) = make_char4(q0[s], q1[s], q2[s], q3[s]);
@@ -106,25 +121,25 @@ slice_rows_kernel(const double* __restrict__ src, int64_t ld, int len, int64_t n
 template <int S>
 __global__ void __launch_bounds__(256)
 slice_cols_kernel(const double* __restrict__ src, int k, int n, int8_t* __restrict__ q, int32_t* __restrict__ expo) {
-  __shared__ double s_amax[8][128];
+  __shared__ unsigned long long s_amax[8][128];
   __shared__ int s_e[128];
   const int lane = threadIdx.x & 31, wy = threadIdx.x >> 5;
   const int64_t item = blockIdx.y;
   const int c = blockIdx.x * 128 + lane * 4;
   const bool live = c < n;                                   // n % 4 == 0: a thread's 4 columns are all inside or all outside
   const double* __restrict__ x = src + item * (int64_t)k * n;
-  double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+  unsigned long long a0 = 0, a1 = 0, a2 = 0, a3 = 0;
   if (live)
     for (int j = wy; j < k; j += 8) {
       const double2 u = *(const double2*)(x + (int64_t)j * n + c), v = *(const double2*)(x + (int64_t)j * n + c + 2);
-      a0 = fmax(a0, fabs(u.x)); a1 = fmax(a1, fabs(u.y)); a2 = fmax(a2, fabs(v.x)); a3 = fmax(a3, fabs(v.y));
+      a0 = max(a0, abs_bits(u.x)); a1 = max(a1, abs_bits(u.y)); a2 = max(a2, abs_bits(v.x)); a3 = max(a3, abs_bits(v.y));
     }
   s_amax[wy][lane * 4 + 0] = a0; s_amax[wy][lane * 4 + 1] = a1; s_amax[wy][lane * 4 + 2] = a2; s_amax[wy][lane * 4 + 3] = a3;
   __syncthreads();
   if (threadIdx.x < 128) {
-    double a = 0.0;
+    unsigned long long a = 0;
 #pragma unroll
-    for (int y = 0; y < 8; ++y) a = fmax(a, s_amax[y][threadIdx.x]);
+    for (int y = 0; y < 8; ++y) a = max(a, s_amax[y][threadIdx.x]);
     const int e = line_exponent(a);
     s_e[threadIdx.x] = e;
     if (blockIdx.x * 128 + threadIdx.x < n) expo[item * n + blockIdx.x * 128 + threadIdx.x] = e;
@@ -136,8 +151,8 @@ slice_cols_kernel(const double* __restrict__ src, int k, int n, int8_t* __restri
   for (int j = wy; j < k; j += 8) {
     const double2 u = *(const double2*)(x + (int64_t)j * n + c), v = *(const double2*)(x + (int64_t)j * n + c + 2);
     int8_t q0[OZ_SMAX], q1[OZ_SMAX], q2[OZ_SMAX], q3[OZ_SMAX];
-    slices_of<S>(scale2(u.x, -e0), q0); slices_of<S>(scale2(u.y, -e1), q1);
-    slices_of<S>(scale2(v.x, -e2), q2); slices_of<S>(scale2(v.y, -e3), q3);
+    slices_of<S>(u.x, e0, q0); slices_of<S>(u.y, e1, q1);
+    slices_of<S>(v.x, e2, q2); slices_of<S>(v.y, e3, q3);
 #pragma unroll
     for (int s = 0; s < S; ++s)
       *(char4*)(out + ((int64_t)(S - 1 - s) * k + j) * n + c) = make_char4(q0[s], q1[s], q2[s], q3[s]);
@@ -160,8 +175,9 @@ __device__ __forceinline__ void combine4(const int32_t* __restrict__ planes, int
 
 // product 1's planes -> slices of T for product 2 (left operand), one warp per row of T (n % 4 == 0):
 // T_ij = 2^(e_i + f_j) sum_d ...; row exponent g_i from max_j |T_ij|; slices of T_ij 2^(-g_i) at qT[row * (S n) + s * n + j].
-// The row is recombined twice (exponent pass, slicing pass; the second read of the planes hits L1/L2) instead of being stored in FP64.
-template <int S>
+// T is never stored in FP64: rows of up to 128 NSTEP columns stay in registers between the exponent pass and the slicing pass
+// (NSTEP = 1, 2, 4); longer rows (NSTEP = 0) are recombined twice, the second read of the planes coming from L1/L2.
+template <int S, int NSTEP>
 __global__ void __launch_bounds__(256)
 combine_slice_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, int rows, int n, int64_t nlines,
                      const int32_t* __restrict__ e_row, const int32_t* __restrict__ f_col, int8_t* __restrict__ qT,
@@ -172,29 +188,54 @@ combine_slice_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, i
   const int64_t item = line / rows;
   const int e = e_row[line];
   const int32_t* __restrict__ f = f_col + item * n;
-  double amax = 0.0;
-  for (int j = lane * 4; j < n; j += 128) {
-    double v[4];
-    combine4<S>(planes, plane_stride, line * n + j, v);
-    const int4 fj = *(const int4*)(f + j);
-    amax = fmax(fmax(amax, fmax(fabs(scale2(v[0], e + fj.x)), fabs(scale2(v[1], e + fj.y)))),
-                fmax(fabs(scale2(v[2], e + fj.z)), fabs(scale2(v[3], e + fj.w))));
-  }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) amax = fmax(amax, __shfl_xor_sync(0xffffffffu, amax, o));
-  const int g = line_exponent(amax);
-  if (lane == 0) g_row[line] = g;
   int8_t* __restrict__ out = qT + line * (int64_t)S * n;
-  for (int j = lane * 4; j < n; j += 128) {
-    double v[4];
-    combine4<S>(planes, plane_stride, line * n + j, v);
+  // T_ij for the 4 columns at j, exactly as the oracle forms it: the recombined sum, then one scaling by 2^(e_i + f_j)
+  auto t_at = [&](int j, double (&t)[4]) {
+    combine4<S>(planes, plane_stride, line * n + j, t);
     const int4 fj = *(const int4*)(f + j);
+    t[0] = scale2(t[0], e + fj.x); t[1] = scale2(t[1], e + fj.y); t[2] = scale2(t[2], e + fj.z); t[3] = scale2(t[3], e + fj.w);
+  };
+  auto put = [&](int j, const double (&t)[4], int g) {
     int8_t q0[OZ_SMAX], q1[OZ_SMAX], q2[OZ_SMAX], q3[OZ_SMAX];
-    // T_ij 2^-g = v 2^(e + f_j - g): one exact scaling of the recombined sum, as in the oracle (ldexp of T, then ldexp by -g)
-    slices_of<S>(scale2(scale2(v[0], e + fj.x), -g), q0); slices_of<S>(scale2(scale2(v[1], e + fj.y), -g), q1);
-    slices_of<S>(scale2(scale2(v[2], e + fj.z), -g), q2); slices_of<S>(scale2(scale2(v[3], e + fj.w), -g), q3);
+    slices_of<S>(t[0], g, q0); slices_of<S>(t[1], g, q1); slices_of<S>(t[2], g, q2); slices_of<S>(t[3], g, q3);
 #pragma unroll
     for (int s = 0; s < S; ++s) *(char4*)(out + (int64_t)s * n + j) = make_char4(q0[s], q1[s], q2[s], q3[s]);
+  };
+  unsigned long long amax = 0;
+  if constexpr (NSTEP > 0) {
+    double t[NSTEP][4];
+#pragma unroll
+    for (int u = 0; u < NSTEP; ++u) {
+      const int j = lane * 4 + u * 128;
+      if (j < n) {
+        t_at(j, t[u]);
+        amax = max(max(amax, max(abs_bits(t[u][0]), abs_bits(t[u][1]))), max(abs_bits(t[u][2]), abs_bits(t[u][3])));
+      }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) amax = max(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+    const int g = line_exponent(amax);
+    if (lane == 0) g_row[line] = g;
+#pragma unroll
+    for (int u = 0; u < NSTEP; ++u) {
+      const int j = lane * 4 + u * 128;
+      if (j < n) put(j, t[u], g);
+    }
+  } else {
+    for (int j = lane * 4; j < n; j += 128) {
+      double t[4];
+      t_at(j, t);
+      amax = max(max(amax, max(abs_bits(t[0]), abs_bits(t[1]))), max(abs_bits(t[2]), abs_bits(t[3])));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) amax = max(amax, __shfl_xor_sync(0xffffffffu, amax, o));
+    const int g = line_exponent(amax);
+    if (lane == 0) g_row[line] = g;
+    for (int j = lane * 4; j < n; j += 128) {
+      double t[4];
+      t_at(j, t);
+      put(j, t, g);
+    }
   }
 }
 
@@ -221,26 +262,32 @@ combine_out_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, int
 }
 
 // ---- the exact INT8 GEMM: D (M x N, int32, row-major) = L (M x K, int8, K-major) . R, batched; R is K x N with N contiguous
-// (RMajorN = true: X as stored) or N x K with K contiguous (false: B as stored) -------------------------------------------------------
-using I8Tile = cute::Shape<cute::_128, cute::_128, cute::_128>;
-using I8Cluster = cute::Shape<cute::_1, cute::_1, cute::_1>;
-using I8Epilogue = typename cutlass::epilogue::collective::CollectiveBuilder<
-    cutlass::arch::Sm100, cutlass::arch::OpClassTensorOp, I8Tile, I8Cluster, cutlass::epilogue::collective::EpilogueTileAuto,
-    int32_t, int32_t, int32_t, cutlass::layout::RowMajor, 4, int32_t, cutlass::layout::RowMajor, 4,
-    cutlass::epilogue::collective::EpilogueScheduleAuto>::CollectiveOp;
-template <class LayoutR>
-using I8Mainloop = typename cutlass::gemm::collective::CollectiveBuilder<
-    cutlass::arch::Sm100, cutlass::arch::OpClassTensorOp, int8_t, cutlass::layout::RowMajor, 16, int8_t, LayoutR, 16, int32_t, I8Tile,
-    I8Cluster, cutlass::gemm::collective::StageCountAutoCarveout<static_cast<int>(sizeof(typename I8Epilogue::SharedStorage))>,
-    cutlass::gemm::collective::KernelScheduleAuto>::CollectiveOp;
-template <class LayoutR>
-using I8Gemm = cutlass::gemm::device::GemmUniversalAdapter<
-    cutlass::gemm::kernel::GemmUniversal<cute::Shape<int, int, int, int>, I8Mainloop<LayoutR>, I8Epilogue>>;
+// (RMajorN = true: X as stored) or N x K with K contiguous (false: B as stored).  Two tile configurations: 256 x 256 x 128 on a
+// pair of SMs (cta_group::2, cluster 2 x 1) for outputs of at least 256 x 256, 128 x 128 x 128 on one SM below that.
+template <int TM, int TN, int CM>
+struct I8Config {
+  using Tile = cute::Shape<cute::Int<TM>, cute::Int<TN>, cute::_128>;
+  using Cluster = cute::Shape<cute::Int<CM>, cute::_1, cute::_1>;
+  using Epilogue = typename cutlass::epilogue::collective::CollectiveBuilder<
+      cutlass::arch::Sm100, cutlass::arch::OpClassTensorOp, Tile, Cluster, cutlass::epilogue::collective::EpilogueTileAuto, int32_t,
+      int32_t, int32_t, cutlass::layout::RowMajor, 4, int32_t, cutlass::layout::RowMajor, 4,
+      cutlass::epilogue::collective::EpilogueScheduleAuto>::CollectiveOp;
+  template <class LayoutR>
+  using Mainloop = typename cutlass::gemm::collective::CollectiveBuilder<
+      cutlass::arch::Sm100, cutlass::arch::OpClassTensorOp, int8_t, cutlass::layout::RowMajor, 16, int8_t, LayoutR, 16, int32_t, Tile,
+      Cluster, cutlass::gemm::collective::StageCountAutoCarveout<static_cast<int>(sizeof(typename Epilogue::SharedStorage))>,
+      cutlass::gemm::collective::KernelScheduleAuto>::CollectiveOp;
+  template <class LayoutR>
+  using Gemm = cutlass::gemm::device::GemmUniversalAdapter<
+      cutlass::gemm::kernel::GemmUniversal<cute::Shape<int, int, int, int>, Mainloop<LayoutR>, Epilogue>>;
+};
+using I8Small = I8Config<128, 128, 1>;
+using I8Large = I8Config<256, 256, 2>;
 
-template <bool RMajorN>
-int i8_gemm(int M, int N, int K, int L, const int8_t* Lp, int64_t ldl, int64_t batchL, const int8_t* Rp, int64_t ldr, int64_t batchR,
-            int32_t* D, int64_t batchD, cudaStream_t stream) {
-  using Gemm = I8Gemm<std::conditional_t<RMajorN, cutlass::layout::RowMajor, cutlass::layout::ColumnMajor>>;
+template <class Cfg, bool RMajorN>
+int i8_gemm_cfg(int M, int N, int K, int L, const int8_t* Lp, int64_t ldl, int64_t batchL, const int8_t* Rp, int64_t ldr, int64_t batchR,
+                int32_t* D, int64_t batchD, cudaStream_t stream) {
+  using Gemm = typename Cfg::template Gemm<std::conditional_t<RMajorN, cutlass::layout::RowMajor, cutlass::layout::ColumnMajor>>;
   typename Gemm::GemmKernel::StrideA sa = cute::make_stride(ldl, cute::Int<1>{}, batchL);
   typename Gemm::GemmKernel::StrideB sb;
   if constexpr (RMajorN) sb = cute::make_stride(cute::Int<1>{}, ldr, batchR);       // (N, K, L): N contiguous
@@ -254,6 +301,13 @@ int i8_gemm(int M, int N, int K, int L, const int8_t* Lp, int64_t ldl, int64_t b
   if (gemm.run(stream) != cutlass::Status::kSuccess) return fail(OZ_CUDA, "INT8 GEMM: launch", cudaGetLastError());
   g_launches.fetch_add(1, std::memory_order_relaxed);
   return OZ_OK;
+}
+
+template <bool RMajorN>
+int i8_gemm(int M, int N, int K, int L, const int8_t* Lp, int64_t ldl, int64_t batchL, const int8_t* Rp, int64_t ldr, int64_t batchR,
+            int32_t* D, int64_t batchD, cudaStream_t stream) {
+  if (M >= 256 && N >= 256) return i8_gemm_cfg<I8Large, RMajorN>(M, N, K, L, Lp, ldl, batchL, Rp, ldr, batchR, D, batchD, stream);
+  return i8_gemm_cfg<I8Small, RMajorN>(M, N, K, L, Lp, ldl, batchL, Rp, ldr, batchR, D, batchD, stream);
 }
 
 inline size_t up256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -307,7 +361,13 @@ int run_chunk(int m, int k, int n, int p, int c, double alpha, const double* A, 
     OZ_LAUNCH_CHECK("combine_out_kernel launch");
     return OZ_OK;
   }
-  combine_slice_kernel<S><<<(unsigned)((rowsA + 7) / 8), 256, 0, st>>>(planes, ps1, m, n, rowsA, eA, fX, qT, gT);
+  {
+    const unsigned grid = (unsigned)((rowsA + 7) / 8);
+    if (n <= 128) combine_slice_kernel<S, 1><<<grid, 256, 0, st>>>(planes, ps1, m, n, rowsA, eA, fX, qT, gT);
+    else if (n <= 256) combine_slice_kernel<S, 2><<<grid, 256, 0, st>>>(planes, ps1, m, n, rowsA, eA, fX, qT, gT);
+    else if (n <= 512) combine_slice_kernel<S, 4><<<grid, 256, 0, st>>>(planes, ps1, m, n, rowsA, eA, fX, qT, gT);
+    else combine_slice_kernel<S, 0><<<grid, 256, 0, st>>>(planes, ps1, m, n, rowsA, eA, fX, qT, gT);
+  }
   OZ_LAUNCH_CHECK("combine_slice_kernel launch");
   const int64_t rowsB = (int64_t)c * p;
   slice_rows_kernel<S, true><<<(unsigned)((rowsB + 7) / 8), 256, 0, st>>>(B, n, n, rowsB, qB, hB);
