@@ -176,7 +176,7 @@ __device__ __forceinline__ void combine4(const int32_t* __restrict__ planes, int
 // product 1's planes -> slices of T for product 2 (left operand), one warp per row of T (n % 4 == 0):
 // T_ij = 2^(e_i + f_j) sum_d ...; row exponent g_i from max_j |T_ij|; slices of T_ij 2^(-g_i) at qT[row * (S n) + s * n + j].
 // T is never stored in FP64: rows of up to 128 NSTEP columns stay in registers between the exponent pass and the slicing pass
-// (NSTEP = 1, 2, 4); longer rows (NSTEP = 0) are recombined twice, the second read of the planes coming from L1/L2.
+// (NSTEP = 1, 2, 4, 8, 16); longer rows (NSTEP = 0) are recombined twice, the second read of the planes coming from L1/L2.
 template <int S, int NSTEP>
 __global__ void __launch_bounds__(256)
 combine_slice_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, int rows, int n, int64_t nlines,
@@ -366,6 +366,8 @@ int run_chunk(int m, int k, int n, int p, int c, double alpha, const double* A, 
     if (n <= 128) combine_slice_kernel<S, 1><<<grid, 256, 0, st>>>(planes, ps1, m, n, rowsA, eA, fX, qT, gT);
     else if (n <= 256) combine_slice_kernel<S, 2><<<grid, 256, 0, st>>>(planes, ps1, m, n, rowsA, eA, fX, qT, gT);
     else if (n <= 512) combine_slice_kernel<S, 4><<<grid, 256, 0, st>>>(planes, ps1, m, n, rowsA, eA, fX, qT, gT);
+    else if (n <= 1024) combine_slice_kernel<S, 8><<<grid, 256, 0, st>>>(planes, ps1, m, n, rowsA, eA, fX, qT, gT);
+    else if (n <= 2048) combine_slice_kernel<S, 16><<<grid, 256, 0, st>>>(planes, ps1, m, n, rowsA, eA, fX, qT, gT);
     else combine_slice_kernel<S, 0><<<grid, 256, 0, st>>>(planes, ps1, m, n, rowsA, eA, fX, qT, gT);
   }
   OZ_LAUNCH_CHECK("combine_slice_kernel launch");
