@@ -139,7 +139,12 @@ enum {
   SU2_PLAN_DEFAULT = 0,
   SU2_PLAN_HOST_ONLY = 1,    /* no device tables: planner tests on CPU                          */
   SU2_PLAN_FORCE_SPLIT = 2,  /* tiny segments: exercises the segmented reduction on small inputs */
-  SU2_PLAN_LARGE_TILES = 4   /* keep a small-block bond on the large-tile kernel (tests, A/B measurements) */
+  SU2_PLAN_LARGE_TILES = 4,  /* keep a small-block bond on the large-tile kernel (tests, A/B measurements) */
+  SU2_PLAN_GANG_PACING = 8   /* large-tile kernel: the row tiles of an output sector, which stream the same right-block
+                                operators, keep within two positions of each other, so that L2 serves them to all but
+                                the first (DRAM reads -70 %, L2 hit rate 60 -> 84 % at configs[3]'s blocks); costs 2-5 %
+                                of the time because a row tile on a faster SM waits -- off by default, for callers that
+                                share HBM bandwidth or power with something else.  Same result bit for bit. */
 };
 
 typedef struct {

@@ -172,7 +172,7 @@ class Plan:
     blocks laid out as family_layout(fam, secs, ld_align) says; None for a host-only plan (planner tests
     without a GPU)."""
 
-    def __init__(self, problem, family_ptrs=None, stream=0, host_only=False, force_split=False, large_tiles=False,
+    def __init__(self, problem, family_ptrs=None, stream=0, host_only=False, force_split=False, large_tiles=False, gang_pacing=False,
                  ld_align=1):
         lib = load()
         self._keep = []
@@ -227,7 +227,7 @@ class Plan:
                            len(problem.fam_l), len(problem.fam_r), fl, fr, len(problem.site),
                            None if u1 else site, len(problem.term), terms, 1 if u1 else 0, site if u1 else None)
         self.handle = C.c_void_p()
-        check(lib.su2_plan_create(C.byref(self.handle), C.byref(prob), (SU2_PLAN_HOST_ONLY if host_only else 0) | (2 if force_split else 0) | (4 if large_tiles else 0),
+        check(lib.su2_plan_create(C.byref(self.handle), C.byref(prob), (SU2_PLAN_HOST_ONLY if host_only else 0) | (2 if force_split else 0) | (4 if large_tiles else 0) | (8 if gang_pacing else 0),
                                   C.c_void_p(stream)))
         info = su2_plan_info_t()
         check(lib.su2_plan_info(self.handle, C.byref(info)))

@@ -157,7 +157,7 @@ __global__ void gemm_pair_tables_kernel(int m, int k, int n, int p, int64_t batc
     for (int i = 0; i < tr * tc; ++i) {
       DevWork w;
       w.dst_off = b * (int64_t)m * p; w.unit0 = (int32_t)b; w.unit1 = (int32_t)b + 1;
-      w.row0 = (i / tc) * tm; w.col0 = (i % tc) * tp; w.m = m; w.p = p; w.to_partial = 2; w.wr = wr; w.ldo = p; w.pad = 0;
+      w.row0 = (i / tc) * tm; w.col0 = (i % tc) * tp; w.m = m; w.p = p; w.to_partial = 2; w.wr = wr; w.ldo = p; w.gang = -1;
       work[b * (int64_t)(tr * tc) + i] = w;
     }
   }
@@ -220,7 +220,7 @@ su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double al
       int dev = 0, sms = 148;
       cudaGetDevice(&dev);
       cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-      st = launch_heff_tma_tables(work, (int)(batch * ntile), units, tasks, buf, C, nullptr, counter, sms, stream_v);
+      st = launch_heff_tma_tables(work, (int)(batch * ntile), units, tasks, buf, C, nullptr, counter, nullptr, sms, stream_v);
       cudaFreeAsync(buf, stream);
       return st;
     }

@@ -100,6 +100,10 @@ __device__ __forceinline__ void tma_box(unsigned dst, const void* map, int c0, i
 // (DESIGN.md section 7): the apply time is the same for every combination (the kernel is not bound by its loads); DRAM
 // reads are lowest with E evict_last (every sibling CTA and every position re-reads it) and A, D left alone --
 // evict_first on the D boxes, round 1's choice, costs 20 % more DRAM traffic here because sibling row-tile CTAs arrive late.
+#ifndef SU2_GANG_AHEAD
+#define SU2_GANG_AHEAD 2      // positions a gang member may run in front of a running member behind it (< 0: no pacing)
+#define SU2_GANG_NEAR 48      // members further behind than this are another wave of the queue: ignored
+#endif
 #ifndef SU2_POL_A
 #define SU2_POL_A 0
 #define SU2_POL_D 0
@@ -131,12 +135,23 @@ template <int WR>
 __device__ __forceinline__ void produce_item(const DevWork& wk, int w, bool reset, const DevUnit* __restrict__ units,
                                              const DevTask* __restrict__ tasks, const CUtensorMap* __restrict__ maps,
                                              unsigned stage0, PhaseInfo* ring, uint64_t* full, uint64_t* empty, Pipe& pp,
-                                             uint64_t pol_a, uint64_t pol_d, uint64_t pol_e) {
+                                             uint64_t pol_a, uint64_t pol_d, uint64_t pol_e, int* __restrict__ gangs) {
   using C = TileCfg<WR>;
   constexpr int NS = C::NSTAGE;
   constexpr int NEB = C::NEBOX, NDB = C::NDBOX;
   constexpr unsigned E_BYTES = NEB * EBOX_SZ * 8u;
   bool first = true;
+  // Pacing of a gang: the row tiles of one (sector, segment, column tile) walk through the same tasks and positions and read
+  // the same D_pos and E boxes.  Left alone they drift apart by more positions than their share of L2 holds and every one of
+  // them streams D from DRAM again (68 % of the DRAM reads, profiles/r02_traffic_cfg4.md).  Each member publishes the number
+  // of positions it has issued; a member more than GANG_AHEAD positions in front of another RUNNING member that is less than
+  // GANG_NEAR behind holds its loads until that one has caught up.  Members that started much later (another wave of the
+  // queue) are out of reach of L2 anyway and are ignored; finished members publish INT_MAX.  Nobody waits for a member that
+  // has not started, and the hindmost running member never waits: no deadlock.  Only this thread (the producer) polls.
+  constexpr int GANG_AHEAD = SU2_GANG_AHEAD, GANG_NEAR = SU2_GANG_NEAR;
+  volatile int* gang = (GANG_AHEAD >= 0 && gangs != nullptr && wk.gang >= 0) ? gangs + wk.gang : nullptr;
+  const int gang_n = wk.m / C::TM, gang_me = wk.row0 / C::TM;      // full row tiles only (plan.cpp)
+  int gang_step = 0;
 #pragma unroll 1
   for (int u = wk.unit0; u < wk.unit1; ++u) {
     const DevUnit un = units[u];
@@ -158,6 +173,19 @@ __device__ __forceinline__ void produce_item(const DevWork& wk, int w, bool rese
 #pragma unroll 1
     for (int pos = un.pos0; pos < un.pos1; ++pos) {
       const double scale = coef * (alpha ? alpha[pos] : 1.0);
+      if (gang) {
+        gang[gang_me] = gang_step;
+        for (;;) {
+          bool hold = false;
+          for (int j = 0; j < gang_n; ++j) {
+            const int pj = gang[j];
+            if (pj >= 0 && pj < gang_step - GANG_AHEAD && pj > gang_step - GANG_NEAR) { hold = true; break; }
+          }
+          if (!hold) break;
+          __nanosleep(500);
+        }
+        ++gang_step;
+      }
 #pragma unroll 1
       for (int chunk = 0; chunk < nchunks; ++chunk) {
         const int n0 = chunk * ncw_full;
@@ -224,6 +252,7 @@ __device__ __forceinline__ void produce_item(const DevWork& wk, int w, bool rese
       }
     }
   }
+  if (gang) gang[gang_me] = 0x7fffffff;          // finished: out of every member's window
 }
 
 template <int MT, int NT, int NACC, int A_I, int A_SUB, int B_J, int B_SUB>
@@ -426,7 +455,7 @@ __device__ __forceinline__ void consume_item(PhaseInfo info, const DevWork* __re
 __global__ void __launch_bounds__(NTHREADS, 1)
 heff_tma_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __restrict__ units,
                 const DevTask* __restrict__ tasks, const CUtensorMap* __restrict__ maps, double* __restrict__ out,
-                double* __restrict__ partial, int* __restrict__ counter) {
+                double* __restrict__ partial, int* __restrict__ counter, int* __restrict__ gangs) {
   extern __shared__ __align__(1024) double smem[];
   __shared__ PhaseInfo ring[PHASE_RING];
   __shared__ __align__(8) uint64_t full[MAX_STAGE];
@@ -459,9 +488,9 @@ heff_tma_kernel(const DevWork* __restrict__ work, int nwork, const DevUnit* __re
       const int wn = atomicAdd(counter, 1);
       const bool reset = wn >= nwork || work[wn].wr != wk.wr;
       const unsigned stage0 = smem_u32(smem + (wk.wr == 1 ? TileCfg<1>::T_SZ : wk.wr == 2 ? TileCfg<2>::T_SZ : TileCfg<4>::T_SZ));
-      if (wk.wr == 1) produce_item<1>(wk, w, reset, units, tasks, maps, stage0, ring, full, empty, pp, pol_a, pol_d, pol_e);
-      else if (wk.wr == 2) produce_item<2>(wk, w, reset, units, tasks, maps, stage0, ring, full, empty, pp, pol_a, pol_d, pol_e);
-      else produce_item<4>(wk, w, reset, units, tasks, maps, stage0, ring, full, empty, pp, pol_a, pol_d, pol_e);
+      if (wk.wr == 1) produce_item<1>(wk, w, reset, units, tasks, maps, stage0, ring, full, empty, pp, pol_a, pol_d, pol_e, gangs);
+      else if (wk.wr == 2) produce_item<2>(wk, w, reset, units, tasks, maps, stage0, ring, full, empty, pp, pol_a, pol_d, pol_e, gangs);
+      else produce_item<4>(wk, w, reset, units, tasks, maps, stage0, ring, full, empty, pp, pol_a, pol_d, pol_e, gangs);
       if (reset) {
         // the stage geometry changes (or the stream ends): wait until every stage in flight has been released
         for (int i = 0; i < MAX_STAGE; ++i) mbar_wait(&empty[i], ((pp.par >> i) & 1) ^ 1);
@@ -503,14 +532,14 @@ static su2_status ensure_smem_attr() {
 }
 
 su2_status launch_heff_tma_tables(const DevWork* work, int nwork, const DevUnit* units, const DevTask* tasks, const void* maps,
-                                  double* out, double* partial, int* counter, int num_sms, void* stream_v) {
+                                  double* out, double* partial, int* counter, int* gangs, int num_sms, void* stream_v) {
   cudaStream_t stream = (cudaStream_t)stream_v;
   if (nwork == 0) return SU2_OK;
   su2_status st = ensure_smem_attr();
   if (st != SU2_OK) return st;
   const int grid = std::min(nwork, num_sms);
   heff_tma_kernel<<<grid, NTHREADS, SMEM_DOUBLES_MAX * sizeof(double), stream>>>(work, nwork, units, tasks, (const CUtensorMap*)maps,
-                                                                               out, partial, counter);
+                                                                               out, partial, counter, gangs);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { set_cuda_error("heff_tma_kernel launch", (int)e); return SU2_ERR_CUDA; }
   count_launch();
@@ -519,7 +548,7 @@ su2_status launch_heff_tma_tables(const DevWork* work, int nwork, const DevUnit*
 
 su2_status launch_heff_tma(const su2_plan* plan, double* out, double* partial, void* stream_v) {
   return launch_heff_tma_tables(plan->d_work, (int)plan->h_work.size(), plan->d_units, plan->d_tasks, plan->d_maps, out, partial,
-                                plan->d_counter, plan->num_sms, stream_v);
+                                plan->d_counter, plan->d_gang, plan->num_sms, stream_v);
 }
 
 }  // namespace su2

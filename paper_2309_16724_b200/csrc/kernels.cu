@@ -180,7 +180,8 @@ su2_status upload_plan(su2_plan* plan, void* stream_v) {
   // the identity blocks must exist before their tensor maps are encoded: allocate the blob first (maps are
   // appended to it in a second allocation-free step: their count is bounded by 3 per task)
   const size_t b_maps = align256(large ? (3 * plan->h_tasks.size() + 1) * 128 : 0);
-  const size_t total = b_tasks + b_units + b_work + b_red + b_diag + b_dbeg + b_psi + b_pad + b_alpha + b_ident + b_maps + 256;
+  const size_t b_gang = align256((size_t)plan->n_gang_slots * sizeof(int32_t));
+  const size_t total = b_tasks + b_units + b_work + b_red + b_diag + b_dbeg + b_psi + b_pad + b_alpha + b_ident + b_maps + b_gang + 256;
   SU2_CUDA(cudaMalloc(&plan->d_blob, total));
   plan->info.plan_device_bytes += (int64_t)total;
   char* base = (char*)plan->d_blob;
@@ -198,6 +199,7 @@ su2_status upload_plan(su2_plan* plan, void* stream_v) {
   plan->d_alpha = (double*)carve(b_alpha);
   plan->d_identity = (double*)carve(b_ident);
   plan->d_counter = (int32_t*)carve(256);
+  plan->d_gang = b_gang ? (int32_t*)carve(b_gang) : nullptr;
 
   auto resolve = [&](const OperandRef& r) -> const double* {
     switch (r.kind) {
@@ -293,6 +295,8 @@ su2_status launch_apply(const su2_plan* plan, const double* psi, double* out, do
       SU2_CUDA(cudaGetLastError());
       count_launch();
     }
+    if (plan->d_gang)   // pacing slots: -1 = member not started
+      SU2_CUDA(cudaMemsetAsync(plan->d_gang, 0xff, (size_t)plan->n_gang_slots * sizeof(int32_t), stream));
     st = launch_heff_tma(plan, out, partial, stream_v);
   }
   if (st != SU2_OK) return st;

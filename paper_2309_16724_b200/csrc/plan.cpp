@@ -208,6 +208,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
 
   su2_plan* plan = new su2_plan();
   plan->host_only = (flags & SU2_PLAN_HOST_ONLY) != 0;
+  plan->gang_pacing = (flags & SU2_PLAN_GANG_PACING) != 0;
   plan->n_tot = p->n_tot;
   plan->twoS_tot = p->twoS_tot;
   plan->sec_l.assign(p->sec_l, p->sec_l + p->nsec_l);
@@ -696,7 +697,18 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
       plan->partial_elems += (int64_t)nseg * sz;
     }
     plan->h_reduce.push_back(red);
+    // Gangs (large-tile kernel, SU2_PLAN_GANG_PACING): the FULL row tiles of one (segment, column tile) read the same D_pos
+    // and E boxes in the same order and get one pacing slot each (heff_tma.cu produce_item).  A ragged last row tile stays
+    // outside: it has less work per position, and paced to the others it would idle its SM for the difference.
+    const int nrow_full = ps.m / ts.tm;
+    const int ncol = (ps.p + ts.tp - 1) / ts.tp;
     for (int g = 0; g < nseg; ++g) {
+      std::vector<int32_t> gang_of(ncol, -1);
+      if (plan->gang_pacing && !small_plan && nrow_full > 1)
+        for (int c = 0; c < ncol; ++c) {
+          gang_of[c] = (int32_t)plan->n_gang_slots;
+          plan->n_gang_slots += nrow_full;
+        }
       for (int r0 = 0; r0 < ps.m; r0 += ts.tm)
         for (int c0 = 0; c0 < ps.p; c0 += ts.tp) {
           double w = 0.0;
@@ -711,6 +723,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
           wk.to_partial = nseg > 1 ? 1 : 0;
           wk.dst_off = nseg > 1 ? red.part_off + (int64_t)g * sz : ps.off;
           wk.wr = small_plan ? 0 : wr;
+          wk.gang = (r0 + ts.tm <= ps.m) ? gang_of[c0 / ts.tp] : -1;
           plan->h_work.push_back(wk);
           work_cost.push_back(w);
         }

@@ -270,7 +270,7 @@ extern "C" su2_status su2_renormalize(const su2_blocking* bk, const su2_opfamily
       const double* psi = op_old ? op_old->data : d_ident;
       st = launch_heff_small(&tmp, psi, out, nullptr, cuda_stream);
     } else {
-      st = launch_heff_tma_tables(d_work, (int)h_work.size(), d_units, d_tasks, d_maps, out, nullptr, d_counter, sms, cuda_stream);
+      st = launch_heff_tma_tables(d_work, (int)h_work.size(), d_units, d_tasks, d_maps, out, nullptr, d_counter, nullptr, sms, cuda_stream);
     }
   }
   cudaFreeAsync(blob, stream);

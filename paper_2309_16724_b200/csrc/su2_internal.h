@@ -46,7 +46,8 @@ struct DevWork {
   int32_t to_partial;     // bit 0: dst_off refers to the partial buffer; bit 1: accumulate into dst (dst += tile)
   int32_t wr;             // tile class: warp rows WR of TileCfg<WR> (1, 2 or 4); 0 = whole sector (heff_small_kernel)
   int32_t ldo;            // leading dimension of the output block (p for Psi sectors; padded for operator blocks)
-  int32_t pad;
+  int32_t gang;           // first slot of this item's gang in the pacing array (heff_tma.cu produce_item), -1 = none;
+                          // the member index is row0 / TM, the member count floor(m / TM) (full row tiles)
 };
 
 // Second pass of the deterministic segmented reduction: F_s = sum_{seg} partial[seg] in index order.
@@ -159,6 +160,9 @@ struct su2_plan {
   double* d_copy = nullptr;            // padded copies of families whose stored rows are not 16-byte aligned
   double* d_psi_pad = nullptr;         // padded private copy of Psi (E tiles are bulk-tensor loads from it)
   int32_t* d_counter = nullptr;
+  int32_t* d_gang = nullptr;       // pacing slots of the large-tile kernel's gangs (reset to -1 before every launch)
+  int64_t n_gang_slots = 0;
+  bool gang_pacing = false;        // SU2_PLAN_GANG_PACING
   void* d_psi_sec = nullptr;           // device copy of `psi` (PsiSector[])
   int64_t partial_elems = 0;
   int32_t num_sms = 148;
@@ -170,7 +174,7 @@ namespace su2 {
 // heff_tma.cu: the large-tile kernel on a plan, and on caller-built tables (gemm_pair.cu; counter = zeroed device int)
 su2_status launch_heff_tma(const su2_plan* plan, double* out, double* partial, void* stream);
 su2_status launch_heff_tma_tables(const DevWork* work, int nwork, const DevUnit* units, const DevTask* tasks, const void* maps,
-                                  double* out, double* partial, int* counter, int num_sms, void* stream);
+                                  double* out, double* partial, int* counter, int* gangs, int num_sms, void* stream);
 // Tensor maps (tensor_maps.cpp).  box kinds of an operand block stored [npos][rows][ld] (cols valid per row):
 //   cmajor: box {KSX along the columns, CT rows}  -- the block used as stored (k runs along the contiguous direction)
 //   kmajor: box {CT + 4 along the columns, KSX rows} -- the block read transposed

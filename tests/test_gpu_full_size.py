@@ -104,6 +104,14 @@ def test_cfg3_sampled_parity_every_sector_and_properties():
     assert checked == 138 * 64
     assert worst <= TOL, worst
     _properties(torch, op, f, 11)
+    # SU2_PLAN_GANG_PACING (row tiles of a sector paced by the producer threads for L2 reuse) changes when loads are issued,
+    # never what is computed: same bits, also on a second apply (the pacing slots are reset per launch)
+    from paper_2309_16724_b200.runtime import HeffOperator
+    paced = HeffOperator(prob, device="cuda:0", gang_pacing=True)
+    assert paced.info["nwork_items"] == op.info["nwork_items"]
+    x = torch.from_numpy(random_psi(op.psi_len, seed=11)).cuda()
+    for _ in range(2):
+        assert torch.equal(paced.apply(x), torch.from_numpy(f).cuda())
 
 
 def _cfg4_sector_choice(prob, op, count):
