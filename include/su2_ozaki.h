@@ -35,13 +35,15 @@ extern "C" {
  * is within 1e-12 of max|C| of the FP64 product; the result is bit-reproducible (integer sums are exact, the FP64
  * recombination has a fixed order).
  *
- * Restrictions (the INT8 operand rows are moved by TMA): k and n multiples of 16, p a multiple of 4, 16-byte aligned
- * operands, nslices * max(k, n) * 127^2 < 2^31.  Inf / NaN operands are not supported (the result is unspecified).
+ * Shapes are arbitrary (the INT8 copies are padded inside: contraction lengths and MN-major rows to 16 bytes, integer
+ * plane rows to 4 entries, pads zero); operands 8-byte aligned (lines that start on a 16-byte boundary are read with
+ * 16-byte loads).  Restriction: nslices * roundup16(max(k, n)) * 127^2 < 2^31 (exact int32 sums: k, n <= 19008 at 7
+ * slices).  Inf / NaN operands are not supported (the result is unspecified).
  *
  * Memory: slices and integer planes of a chunk of items live in `workspace` (DEVICE, 256-byte aligned, workspace_bytes
  * long, owned by the caller, free for reuse once the stream has passed the call); the batch is processed in chunks of
  * as many items as fit (su2_ozaki_workspace_bytes(m, k, n, p, items, nslices) says how much `items` items need: about
- * nslices (m k + k n + m n + p n) + 4 nslices m max(n, p) bytes each).  workspace == NULL: a stream-ordered allocation
+ * nslices (m k + k n + m n + p n) + 4 nslices m max(n, p) bytes each, with k and n rounded up to 16 and p to 4).  workspace == NULL: a stream-ordered allocation
  * (cudaMallocAsync on cuda_stream) of at most workspace_bytes (0 = 2 GiB), freed in stream order before the call
  * returns.  Asynchronous on cuda_stream.
  *
@@ -52,7 +54,7 @@ int32_t su2_gemm_pair_batched_i8(int32_t m, int32_t k, int32_t n, int32_t p, int
                                  void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* One product on its own, C_b (m x n) = A_b (m x k) * X_b (k x n) (overwritten, no alpha): the unit the oracle's
- * emulated_matmul defines, for element-by-element parity.  Same restrictions with p := n. */
+ * emulated_matmul defines, for element-by-element parity.  Same restriction. */
 int32_t su2_matmul_batched_i8(int32_t m, int32_t k, int32_t n, int64_t batch, const double* A, const double* X,
                               double* C, int32_t nslices, void* workspace, size_t workspace_bytes, void* cuda_stream);
 

@@ -84,84 +84,120 @@ __device__ __forceinline__ void slices_of(double a, int e, int8_t (&q)[OZ_SMAX])
   for (int s = 0; s < S; ++s) q[s] = (int8_t)(sgn * (int)((fx >> (OZ_W * (S - 1 - s))) & 127));
 }
 
-// ---- slicing of a K-major operand: one warp per row --------------------------------------------------------------------------------
-// src: nlines rows of `len` FP64 (len % 4 == 0), row pitch ld.  Slice s of row r goes to q[r * (S len) + slot(s) * len + j],
-// slot(s) = s (left operand) or S-1-s (REVERSED: right operand); expo[r] = the row's exponent.  Each lane owns 4 consecutive
-// elements (two 16-byte loads, one 4-byte store per slice: a warp writes 128 contiguous bytes).
+// 4 consecutive elements of a line from element j on, zeros from `len` on; vec: the line starts on a 16-byte boundary
+__device__ __forceinline__ void load4(const double* __restrict__ row, int j, int len, bool vec, double (&v)[4]) {
+  if (vec && j + 3 < len) {
+    const double2 a = *(const double2*)(row + j), b = *(const double2*)(row + j + 2);
+    v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+  } else {
+#pragma unroll
+    for (int q = 0; q < 4; ++q) v[q] = (j + q < len) ? row[j + q] : 0.0;
+  }
+}
+
+__device__ __forceinline__ unsigned long long amax4(unsigned long long a, const double (&v)[4]) {
+  return max(max(a, max(abs_bits(v[0]), abs_bits(v[1]))), max(abs_bits(v[2]), abs_bits(v[3])));
+}
+
+// Shapes need not be multiples of anything: the INT8 copies are this file's own, so their extents are padded (contraction
+// lengths and MN-major rows to 16 bytes for TMA, int32 plane rows to 16 bytes) and the pads are written as zeros, which add
+// nothing to the integer sums.  FP64 operands are read with 16-byte loads where a line is aligned, element-wise otherwise.
+
+// ---- slicing of a K-major operand: one warp per line ------------------------------------------------------------------------------
+// src: items of `rows` lines of `len` FP64 (line pitch ld, items istride apart).  The INT8 copy has rowsP >= rows lines per item
+// (lines beyond `rows` are zero: B's rows are padded to a multiple of 4) of S slots of lenP >= len bytes: slice s of element j
+// of line r of item b goes to q[((b rowsP + r) S + slot(s)) lenP + j], slot(s) = s (left operand) or S-1-s (REVERSED: right
+// operand); expo[b rowsP + r] = the line's exponent.  Each lane owns 4 consecutive elements (one 4-byte store per slice).
 template <int S, bool REVERSED>
 __global__ void __launch_bounds__(256)
-slice_rows_kernel(const double* __restrict__ src, int64_t ld, int len, int64_t nlines, int8_t* __restrict__ q, int32_t* __restrict__ expo) {
+slice_rows_kernel(const double* __restrict__ src, int64_t istride, int64_t ld, int rows, int rowsP, int len, int lenP, int64_t nlines,
+                  int8_t* __restrict__ q, int32_t* __restrict__ expo) {
   const int lane = threadIdx.x & 31;
   const int64_t line = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (line >= nlines) return;
-  const double* __restrict__ row = src + line * ld;
+  const int64_t item = line / rowsP;
+  const int r = (int)(line - item * rowsP);
+  int8_t* __restrict__ out = q + line * (int64_t)S * lenP;
+  if (r >= rows) {                                            // padding line
+    if (lane == 0) expo[line] = 0;
+    for (int j = lane * 4; j < S * lenP; j += 128) *(char4*)(out + j) = make_char4(0, 0, 0, 0);
+    return;
+  }
+  const double* __restrict__ row = src + item * istride + (int64_t)r * ld;
+  const bool vec = ((uintptr_t)row & 15) == 0;
   unsigned long long amax = 0;
   for (int j = lane * 4; j < len; j += 128) {
-    const double2 a = *(const double2*)(row + j), b = *(const double2*)(row + j + 2);
-    amax = max(max(amax, max(abs_bits(a.x), abs_bits(a.y))), max(abs_bits(b.x), abs_bits(b.y)));
+    double v[4];
+    load4(row, j, len, vec, v);
+    amax = amax4(amax, v);
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) amax = max(amax, __shfl_xor_sync(0xffffffffu, amax, o));
   const int e = line_exponent(amax);
   if (lane == 0) expo[line] = e;
-  int8_t* __restrict__ out = q + line * (int64_t)S * len;
-  for (int j = lane * 4; j < len; j += 128) {
-    const double2 a = *(const double2*)(row + j), b = *(const double2*)(row + j + 2);
+  for (int j = lane * 4; j < lenP; j += 128) {
+    double v[4];
+    load4(row, j, len, vec, v);
     int8_t q0[OZ_SMAX], q1[OZ_SMAX], q2[OZ_SMAX], q3[OZ_SMAX];
-    slices_of<S>(a.x, e, q0); slices_of<S>(a.y, e, q1);
-    slices_of<S>(b.x, e, q2); slices_of<S>(b.y, e, q3);
+    slices_of<S>(v[0], e, q0); slices_of<S>(v[1], e, q1); slices_of<S>(v[2], e, q2); slices_of<S>(v[3], e, q3);
 #pragma unroll
     for (int s = 0; s < S; ++s)
-      *(char4*)(out + (int64_t)(REVERSED ? S - 1 - s : s) * len + j) = make_char4(q0[s], q1[s], q2[s], q3[s]);
+      *(char4*)(out + (int64_t)(REVERSED ? S - 1 - s : s) * lenP + j) = make_char4(q0[s], q1[s], q2[s], q3[s]);
   }
 }
 
 // ---- slicing of an MN-major right operand (X: k x n as stored, contraction index along its rows): one CTA per (128-column strip, item)
-// expo[item * n + c] = exponent of column c; slice s of element (j, c) goes to q[item][(S-1-s) * k + j][c] (row pitch n).
+// expo[item nP + c] = exponent of column c (0 for the padding columns); slice s of element (j, c) goes to
+// q[item][(S-1-s) kP + j][c] (row pitch nP); rows k..kP-1 and columns n..nP-1 are zero.
 template <int S>
 __global__ void __launch_bounds__(256)
-slice_cols_kernel(const double* __restrict__ src, int k, int n, int8_t* __restrict__ q, int32_t* __restrict__ expo) {
+slice_cols_kernel(const double* __restrict__ src, int k, int n, int kP, int nP, int8_t* __restrict__ q, int32_t* __restrict__ expo) {
   __shared__ unsigned long long s_amax[8][128];
   __shared__ int s_e[128];
   const int lane = threadIdx.x & 31, wy = threadIdx.x >> 5;
   const int64_t item = blockIdx.y;
   const int c = blockIdx.x * 128 + lane * 4;
-  const bool live = c < n;                                   // n % 4 == 0: a thread's 4 columns are all inside or all outside
+  const bool live = c < nP;                                  // nP % 4 == 0: a thread's 4 columns are all inside or all outside
   const double* __restrict__ x = src + item * (int64_t)k * n;
-  unsigned long long a0 = 0, a1 = 0, a2 = 0, a3 = 0;
+  const bool vec = !(n & 1) && ((uintptr_t)x & 15) == 0;     // every row of this item starts on a 16-byte boundary
+  unsigned long long a[4] = {0, 0, 0, 0};
   if (live)
     for (int j = wy; j < k; j += 8) {
-      const double2 u = *(const double2*)(x + (int64_t)j * n + c), v = *(const double2*)(x + (int64_t)j * n + c + 2);
-      a0 = max(a0, abs_bits(u.x)); a1 = max(a1, abs_bits(u.y)); a2 = max(a2, abs_bits(v.x)); a3 = max(a3, abs_bits(v.y));
+      double v[4];
+      load4(x + (int64_t)j * n, c, n, vec, v);
+#pragma unroll
+      for (int u = 0; u < 4; ++u) a[u] = max(a[u], abs_bits(v[u]));
     }
-  s_amax[wy][lane * 4 + 0] = a0; s_amax[wy][lane * 4 + 1] = a1; s_amax[wy][lane * 4 + 2] = a2; s_amax[wy][lane * 4 + 3] = a3;
+#pragma unroll
+  for (int u = 0; u < 4; ++u) s_amax[wy][lane * 4 + u] = a[u];
   __syncthreads();
   if (threadIdx.x < 128) {
-    unsigned long long a = 0;
+    unsigned long long m = 0;
 #pragma unroll
-    for (int y = 0; y < 8; ++y) a = max(a, s_amax[y][threadIdx.x]);
-    const int e = line_exponent(a);
+    for (int y = 0; y < 8; ++y) m = max(m, s_amax[y][threadIdx.x]);
+    const int e = line_exponent(m);
     s_e[threadIdx.x] = e;
-    if (blockIdx.x * 128 + threadIdx.x < n) expo[item * n + blockIdx.x * 128 + threadIdx.x] = e;
+    if (blockIdx.x * 128 + threadIdx.x < nP) expo[item * nP + blockIdx.x * 128 + threadIdx.x] = e;
   }
   __syncthreads();
   if (!live) return;
   const int e0 = s_e[lane * 4], e1 = s_e[lane * 4 + 1], e2 = s_e[lane * 4 + 2], e3 = s_e[lane * 4 + 3];
-  int8_t* __restrict__ out = q + item * (int64_t)S * k * n;
-  for (int j = wy; j < k; j += 8) {
-    const double2 u = *(const double2*)(x + (int64_t)j * n + c), v = *(const double2*)(x + (int64_t)j * n + c + 2);
+  int8_t* __restrict__ out = q + item * (int64_t)S * kP * nP;
+  for (int j = wy; j < kP; j += 8) {
+    double v[4] = {0.0, 0.0, 0.0, 0.0};
+    if (j < k) load4(x + (int64_t)j * n, c, n, vec, v);
     int8_t q0[OZ_SMAX], q1[OZ_SMAX], q2[OZ_SMAX], q3[OZ_SMAX];
-    slices_of<S>(u.x, e0, q0); slices_of<S>(u.y, e1, q1);
-    slices_of<S>(v.x, e2, q2); slices_of<S>(v.y, e3, q3);
+    slices_of<S>(v[0], e0, q0); slices_of<S>(v[1], e1, q1); slices_of<S>(v[2], e2, q2); slices_of<S>(v[3], e3, q3);
 #pragma unroll
     for (int s = 0; s < S; ++s)
-      *(char4*)(out + ((int64_t)(S - 1 - s) * k + j) * n + c) = make_char4(q0[s], q1[s], q2[s], q3[s]);
+      *(char4*)(out + ((int64_t)(S - 1 - s) * kP + j) * nP + c) = make_char4(q0[s], q1[s], q2[s], q3[s]);
   }
 }
 
 // ---- recombination -----------------------------------------------------------------------------------------------------------------
-// value of entry idx of the product from its S integer planes (plane d at planes + d * plane_stride), before the 2^(e+f) scaling:
-//   sum_{d = S-1 .. 0} P_d 2^(-W (d+2)),  smallest first (oracle/ozaki.py step 5); the weights are powers of two, so multiplying is exact.
+// value of 4 consecutive entries of the product from their S integer planes (plane d at planes + d * plane_stride), before the
+// 2^(e+f) scaling:  sum_{d = S-1 .. 0} P_d 2^(-W (d+2)),  smallest first (oracle/ozaki.py step 5); the weights are powers of two, so
+// multiplying is exact.  idx is a multiple of 4 (plane rows are padded to 4 entries).
 template <int S>
 __device__ __forceinline__ void combine4(const int32_t* __restrict__ planes, int64_t plane_stride, int64_t idx, double (&v)[4]) {
   v[0] = v[1] = v[2] = v[3] = 0.0;
@@ -173,13 +209,15 @@ __device__ __forceinline__ void combine4(const int32_t* __restrict__ planes, int
   }
 }
 
-// product 1's planes -> slices of T for product 2 (left operand), one warp per row of T (n % 4 == 0):
-// T_ij = 2^(e_i + f_j) sum_d ...; row exponent g_i from max_j |T_ij|; slices of T_ij 2^(-g_i) at qT[row * (S n) + s * n + j].
-// T is never stored in FP64: rows of up to 128 NSTEP columns stay in registers between the exponent pass and the slicing pass
-// (NSTEP = 1, 2, 4, 8, 16); longer rows (NSTEP = 0) are recombined twice, the second read of the planes coming from L1/L2.
+// product 1's planes -> slices of T for product 2 (left operand), one warp per row of T.  Plane rows, the column exponents and
+// the INT8 rows all have the padded pitch nP; the padding columns hold zero planes and zero exponents, so they come out as zero
+// slices without a special case.  T_ij = 2^(e_i + f_j) sum_d ...; row exponent g_i from max_j |T_ij|; slices of T_ij 2^(-g_i) at
+// qT[(row S + s) nP + j].  T is never stored in FP64: rows of up to 128 NSTEP columns stay in registers between the exponent
+// pass and the slicing pass (NSTEP = 1, 2, 4, 8, 16); longer rows (NSTEP = 0) are recombined twice, the second read of the
+// planes coming from L1/L2.
 template <int S, int NSTEP>
 __global__ void __launch_bounds__(256)
-combine_slice_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, int rows, int n, int64_t nlines,
+combine_slice_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, int rows, int nP, int64_t nlines,
                      const int32_t* __restrict__ e_row, const int32_t* __restrict__ f_col, int8_t* __restrict__ qT,
                      int32_t* __restrict__ g_row) {
   const int lane = threadIdx.x & 31;
@@ -187,11 +225,11 @@ combine_slice_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, i
   if (line >= nlines) return;
   const int64_t item = line / rows;
   const int e = e_row[line];
-  const int32_t* __restrict__ f = f_col + item * n;
-  int8_t* __restrict__ out = qT + line * (int64_t)S * n;
+  const int32_t* __restrict__ f = f_col + item * nP;
+  int8_t* __restrict__ out = qT + line * (int64_t)S * nP;
   // T_ij for the 4 columns at j, exactly as the oracle forms it: the recombined sum, then one scaling by 2^(e_i + f_j)
   auto t_at = [&](int j, double (&t)[4]) {
-    combine4<S>(planes, plane_stride, line * n + j, t);
+    combine4<S>(planes, plane_stride, line * nP + j, t);
     const int4 fj = *(const int4*)(f + j);
     t[0] = scale2(t[0], e + fj.x); t[1] = scale2(t[1], e + fj.y); t[2] = scale2(t[2], e + fj.z); t[3] = scale2(t[3], e + fj.w);
   };
@@ -199,7 +237,7 @@ combine_slice_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, i
     int8_t q0[OZ_SMAX], q1[OZ_SMAX], q2[OZ_SMAX], q3[OZ_SMAX];
     slices_of<S>(t[0], g, q0); slices_of<S>(t[1], g, q1); slices_of<S>(t[2], g, q2); slices_of<S>(t[3], g, q3);
 #pragma unroll
-    for (int s = 0; s < S; ++s) *(char4*)(out + (int64_t)s * n + j) = make_char4(q0[s], q1[s], q2[s], q3[s]);
+    for (int s = 0; s < S; ++s) *(char4*)(out + (int64_t)s * nP + j) = make_char4(q0[s], q1[s], q2[s], q3[s]);
   };
   unsigned long long amax = 0;
   if constexpr (NSTEP > 0) {
@@ -207,9 +245,9 @@ combine_slice_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, i
 #pragma unroll
     for (int u = 0; u < NSTEP; ++u) {
       const int j = lane * 4 + u * 128;
-      if (j < n) {
+      if (j < nP) {
         t_at(j, t[u]);
-        amax = max(max(amax, max(abs_bits(t[u][0]), abs_bits(t[u][1]))), max(abs_bits(t[u][2]), abs_bits(t[u][3])));
+        amax = amax4(amax, t[u]);
       }
     }
 #pragma unroll
@@ -219,19 +257,19 @@ combine_slice_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, i
 #pragma unroll
     for (int u = 0; u < NSTEP; ++u) {
       const int j = lane * 4 + u * 128;
-      if (j < n) put(j, t[u], g);
+      if (j < nP) put(j, t[u], g);
     }
   } else {
-    for (int j = lane * 4; j < n; j += 128) {
+    for (int j = lane * 4; j < nP; j += 128) {
       double t[4];
       t_at(j, t);
-      amax = max(max(amax, max(abs_bits(t[0]), abs_bits(t[1]))), max(abs_bits(t[2]), abs_bits(t[3])));
+      amax = amax4(amax, t);
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) amax = max(amax, __shfl_xor_sync(0xffffffffu, amax, o));
     const int g = line_exponent(amax);
     if (lane == 0) g_row[line] = g;
-    for (int j = lane * 4; j < n; j += 128) {
+    for (int j = lane * 4; j < nP; j += 128) {
       double t[4];
       t_at(j, t);
       put(j, t, g);
@@ -239,25 +277,35 @@ combine_slice_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, i
   }
 }
 
-// planes of a product -> FP64 result: dst = (ACCUMULATE ? dst : 0) + alpha 2^(e_i + f_j) sum_d ...; 4 consecutive columns per thread
+// planes of a product -> FP64 result: dst = (ACCUMULATE ? dst : 0) + alpha 2^(e_i + f_j) sum_d ...; 4 consecutive columns per
+// thread.  Plane rows and column exponents have the padded pitch colsP; dst is dense (pitch cols).
 template <int S, bool ACCUMULATE>
 __global__ void __launch_bounds__(256)
-combine_out_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, int rows, int cols, int64_t nquad,
+combine_out_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, int rows, int cols, int colsP, int64_t nquad,
                    const int32_t* __restrict__ e_row, const int32_t* __restrict__ f_col, double alpha, double* __restrict__ dst) {
-  const int cq = cols >> 2;
+  const int cq = colsP >> 2;
+  const bool vec = !(cols & 3) && ((uintptr_t)dst & 15) == 0;
   for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < nquad; t += (int64_t)gridDim.x * blockDim.x) {
     const int64_t line = t / cq;                              // item * rows + i
     const int j = (int)(t - line * cq) * 4;
+    if (j >= cols) continue;
     const int64_t item = line / rows;
     double v[4];
-    combine4<S>(planes, plane_stride, line * cols + j, v);
+    combine4<S>(planes, plane_stride, line * colsP + j, v);
     const int e = e_row[line];
-    const int4 fj = *(const int4*)(f_col + item * cols + j);
-    double2* o = (double2*)(dst + line * cols + j);
-    double2 lo = ACCUMULATE ? o[0] : make_double2(0.0, 0.0), hi = ACCUMULATE ? o[1] : make_double2(0.0, 0.0);
-    lo.x += alpha * scale2(v[0], e + fj.x); lo.y += alpha * scale2(v[1], e + fj.y);
-    hi.x += alpha * scale2(v[2], e + fj.z); hi.y += alpha * scale2(v[3], e + fj.w);
-    o[0] = lo; o[1] = hi;
+    const int4 fj = *(const int4*)(f_col + item * colsP + j);
+    v[0] = alpha * scale2(v[0], e + fj.x); v[1] = alpha * scale2(v[1], e + fj.y);
+    v[2] = alpha * scale2(v[2], e + fj.z); v[3] = alpha * scale2(v[3], e + fj.w);
+    double* o = dst + line * cols + j;
+    if (vec) {
+      double2 lo = ACCUMULATE ? ((double2*)o)[0] : make_double2(0.0, 0.0), hi = ACCUMULATE ? ((double2*)o)[1] : make_double2(0.0, 0.0);
+      lo.x += v[0]; lo.y += v[1]; hi.x += v[2]; hi.y += v[3];
+      ((double2*)o)[0] = lo; ((double2*)o)[1] = hi;
+    } else {
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+        if (j + u < cols) o[u] = ACCUMULATE ? o[u] + v[u] : v[u];
+    }
   }
 }
 
@@ -312,19 +360,23 @@ int i8_gemm(int M, int N, int K, int L, const int8_t* Lp, int64_t ldl, int64_t b
 
 inline size_t up256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-// workspace of a chunk of `c` items (p = 0: single product)
+inline int up16(int x) { return (x + 15) & ~15; }
+inline int up4(int x) { return (x + 3) & ~3; }
+
+// workspace of a chunk of `c` items (p = 0: single product); padded extents kP, nP (16), pP (4)
 struct Workspace {
   size_t qA, qX, planes, qT, qB, eA, fX, gT, hB, total;
   Workspace(int64_t c, int m, int k, int n, int p, int S) {
+    const size_t kP = up16(k), nP = up16(n), pP = up4(p);
     size_t o = 0;
     auto take = [&](size_t bytes) { const size_t at = o; o += up256(bytes); return at; };
-    qA = take((size_t)c * m * S * k);
-    qX = take((size_t)c * S * k * n);
-    planes = take((size_t)c * S * 4 * m * std::max(n, p));
-    qT = take(p ? (size_t)c * m * S * n : 0);
-    qB = take(p ? (size_t)c * p * S * n : 0);
-    eA = take((size_t)c * m * 4); fX = take((size_t)c * n * 4);
-    gT = take(p ? (size_t)c * m * 4 : 0); hB = take(p ? (size_t)c * p * 4 : 0);
+    qA = take((size_t)c * m * S * kP);
+    qX = take((size_t)c * S * kP * nP);
+    planes = take((size_t)c * S * 4 * m * std::max(nP, pP));
+    qT = take(p ? (size_t)c * m * S * nP : 0);
+    qB = take(p ? (size_t)c * pP * S * nP : 0);
+    eA = take((size_t)c * m * 4); fX = take((size_t)c * nP * 4);
+    gT = take(p ? (size_t)c * m * 4 : 0); hB = take(p ? (size_t)c * pP * 4 : 0);
     total = o;
   }
 };
@@ -341,47 +393,50 @@ template <int S>
 int run_chunk(int m, int k, int n, int p, int c, double alpha, const double* A, const double* X, const double* B, double* C,
               char* ws, cudaStream_t st) {
   const Workspace w(c, m, k, n, p, S);
+  const int kP = up16(k), nP = up16(n), pP = up4(p);
   int8_t *qA = (int8_t*)(ws + w.qA), *qX = (int8_t*)(ws + w.qX), *qT = (int8_t*)(ws + w.qT), *qB = (int8_t*)(ws + w.qB);
   int32_t *planes = (int32_t*)(ws + w.planes), *eA = (int32_t*)(ws + w.eA), *fX = (int32_t*)(ws + w.fX), *gT = (int32_t*)(ws + w.gT),
           *hB = (int32_t*)(ws + w.hB);
   const int64_t rowsA = (int64_t)c * m;
-  slice_rows_kernel<S, false><<<(unsigned)((rowsA + 7) / 8), 256, 0, st>>>(A, k, k, rowsA, qA, eA);
+  slice_rows_kernel<S, false><<<(unsigned)((rowsA + 7) / 8), 256, 0, st>>>(A, (int64_t)m * k, k, m, m, k, kP, rowsA, qA, eA);
   OZ_LAUNCH_CHECK("slice_rows_kernel(A) launch");
-  slice_cols_kernel<S><<<dim3((n + 127) / 128, c), 256, 0, st>>>(X, k, n, qX, fX);
+  slice_cols_kernel<S><<<dim3((nP + 127) / 128, c), 256, 0, st>>>(X, k, n, kP, nP, qX, fX);
   OZ_LAUNCH_CHECK("slice_cols_kernel(X) launch");
-  const int64_t ps1 = (int64_t)c * m * n;
+  const int64_t ps1 = (int64_t)c * m * nP;
   for (int d = 0; d < S; ++d) {                               // diagonal d: L slices 0..d, R slices d..0 = slots S-1-d..S-1
-    const int rc = i8_gemm<true>(m, n, (d + 1) * k, c, qA, (int64_t)S * k, (int64_t)m * S * k, qX + (int64_t)(S - 1 - d) * k * n, n,
-                                 (int64_t)S * k * n, planes + d * ps1, (int64_t)m * n, st);
+    const int rc = i8_gemm<true>(m, nP, (d + 1) * kP, c, qA, (int64_t)S * kP, (int64_t)m * S * kP, qX + (int64_t)(S - 1 - d) * kP * nP,
+                                 nP, (int64_t)S * kP * nP, planes + d * ps1, (int64_t)m * nP, st);
     if (rc != OZ_OK) return rc;
   }
   if (p == 0) {
     const int64_t nquad = ps1 / 4;
-    combine_out_kernel<S, false><<<(unsigned)std::min<int64_t>((nquad + 255) / 256, 148 * 16), 256, 0, st>>>(planes, ps1, m, n, nquad, eA, fX, 1.0, C);
+    combine_out_kernel<S, false><<<(unsigned)std::min<int64_t>((nquad + 255) / 256, 148 * 16), 256, 0, st>>>(planes, ps1, m, n, nP, nquad, eA,
+                                                                                                        fX, 1.0, C);
     OZ_LAUNCH_CHECK("combine_out_kernel launch");
     return OZ_OK;
   }
   {
     const unsigned grid = (unsigned)((rowsA + 7) / 8);
-    if (n <= 128) combine_slice_kernel<S, 1><<<grid, 256, 0, st>>>(planes, ps1, m, n, rowsA, eA, fX, qT, gT);
-    else if (n <= 256) combine_slice_kernel<S, 2><<<grid, 256, 0, st>>>(planes, ps1, m, n, rowsA, eA, fX, qT, gT);
-    else if (n <= 512) combine_slice_kernel<S, 4><<<grid, 256, 0, st>>>(planes, ps1, m, n, rowsA, eA, fX, qT, gT);
-    else if (n <= 1024) combine_slice_kernel<S, 8><<<grid, 256, 0, st>>>(planes, ps1, m, n, rowsA, eA, fX, qT, gT);
-    else if (n <= 2048) combine_slice_kernel<S, 16><<<grid, 256, 0, st>>>(planes, ps1, m, n, rowsA, eA, fX, qT, gT);
-    else combine_slice_kernel<S, 0><<<grid, 256, 0, st>>>(planes, ps1, m, n, rowsA, eA, fX, qT, gT);
+    if (nP <= 128) combine_slice_kernel<S, 1><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, fX, qT, gT);
+    else if (nP <= 256) combine_slice_kernel<S, 2><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, fX, qT, gT);
+    else if (nP <= 512) combine_slice_kernel<S, 4><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, fX, qT, gT);
+    else if (nP <= 1024) combine_slice_kernel<S, 8><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, fX, qT, gT);
+    else if (nP <= 2048) combine_slice_kernel<S, 16><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, fX, qT, gT);
+    else combine_slice_kernel<S, 0><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, fX, qT, gT);
   }
   OZ_LAUNCH_CHECK("combine_slice_kernel launch");
-  const int64_t rowsB = (int64_t)c * p;
-  slice_rows_kernel<S, true><<<(unsigned)((rowsB + 7) / 8), 256, 0, st>>>(B, n, n, rowsB, qB, hB);
+  const int64_t rowsB = (int64_t)c * pP;
+  slice_rows_kernel<S, true><<<(unsigned)((rowsB + 7) / 8), 256, 0, st>>>(B, (int64_t)p * n, n, p, pP, n, nP, rowsB, qB, hB);
   OZ_LAUNCH_CHECK("slice_rows_kernel(B) launch");
-  const int64_t ps2 = (int64_t)c * m * p;
+  const int64_t ps2 = (int64_t)c * m * pP;
   for (int d = 0; d < S; ++d) {
-    const int rc = i8_gemm<false>(m, p, (d + 1) * n, c, qT, (int64_t)S * n, (int64_t)m * S * n, qB + (int64_t)(S - 1 - d) * n,
-                                  (int64_t)S * n, (int64_t)p * S * n, planes + d * ps2, (int64_t)m * p, st);
+    const int rc = i8_gemm<false>(m, pP, (d + 1) * nP, c, qT, (int64_t)S * nP, (int64_t)m * S * nP, qB + (int64_t)(S - 1 - d) * nP,
+                                  (int64_t)S * nP, (int64_t)pP * S * nP, planes + d * ps2, (int64_t)m * pP, st);
     if (rc != OZ_OK) return rc;
   }
   const int64_t nquad = ps2 / 4;
-  combine_out_kernel<S, true><<<(unsigned)std::min<int64_t>((nquad + 255) / 256, 148 * 16), 256, 0, st>>>(planes, ps2, m, p, nquad, gT, hB, alpha, C);
+  combine_out_kernel<S, true><<<(unsigned)std::min<int64_t>((nquad + 255) / 256, 148 * 16), 256, 0, st>>>(planes, ps2, m, p, pP, nquad, gT, hB,
+                                                                                                     alpha, C);
   OZ_LAUNCH_CHECK("combine_out_kernel launch");
   return OZ_OK;
 }
@@ -405,9 +460,8 @@ int run(int m, int k, int n, int p, int64_t batch, double alpha, const double* A
   if (m <= 0 || k <= 0 || n <= 0 || p < 0 || batch < 0 || !A || !X || !C || (pair && !B)) return fail(OZ_INVALID, "null pointer, non-positive dimension or negative batch");
   if (S == 0) S = OZ_SMAX;
   if (S < 2 || S > OZ_SMAX) return fail(OZ_INVALID, "nslices must be 0 or 2..7");
-  if ((k & 15) || (n & 15) || (p & 3)) return fail(OZ_INVALID, "k and n must be multiples of 16 and p a multiple of 4 (INT8 rows are moved by TMA)");
-  if ((int64_t)S * std::max(k, n) * 127 * 127 >= ((int64_t)1 << 31)) return fail(OZ_INVALID, "contraction too long for exact int32 accumulation");
-  if (((uintptr_t)A | (uintptr_t)X | (uintptr_t)B | (uintptr_t)C) & 15) return fail(OZ_INVALID, "operands must be 16-byte aligned");
+  if ((int64_t)S * up16(std::max(k, n)) * 127 * 127 >= ((int64_t)1 << 31)) return fail(OZ_INVALID, "contraction too long for exact int32 accumulation");
+  if (((uintptr_t)A | (uintptr_t)X | (uintptr_t)B | (uintptr_t)C) & 7) return fail(OZ_INVALID, "operands must be 8-byte aligned");
   if (workspace && ((uintptr_t)workspace & 255)) return fail(OZ_INVALID, "workspace must be 256-byte aligned");
   if (batch == 0) return OZ_OK;
   if (workspace_bytes == 0) {

@@ -39,7 +39,11 @@ def _operands(seed, batch, m, k, n, p=None, spread=0.0):
     (257, 272, 144, 2, 7, 20.0),      # three row tiles, two column tiles, rows / columns of wildly different magnitude
     (128, 128, 128, 5, 4, 0.0),       # fewer slices (the template parameter)
     (64, 512, 256, 2, 2, 3.0),
-    (5, 16, 16, 7, 7, 0.0),           # the smallest contraction the INT8 rows allow
+    (5, 16, 16, 7, 7, 0.0),
+    (70, 33, 45, 3, 7, 0.0),          # nothing a multiple of 16, 4 or 2: padded INT8 copies, element-wise FP64 loads
+    (131, 577, 100, 2, 7, 4.0),       # a block of BASELINE.json configs[2] / [3]: 131 rows, contraction 577
+    (1, 1, 1, 5, 7, 0.0),
+    (9, 130, 7, 2, 3, 0.0),
 ])
 def test_i8_matmul_equals_the_oracle_bit_for_bit(m, k, n, batch, nslices, spread):
     torch = _torch()
@@ -62,7 +66,9 @@ def test_i8_matmul_equals_the_oracle_bit_for_bit(m, k, n, batch, nslices, spread
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("m,k,n,p,batch", [(48, 32, 64, 20, 3), (130, 144, 80, 132, 2), (256, 256, 256, 256, 3),
-                                           (100, 16, 16, 4, 9), (200, 80, 304, 600, 2)])
+                                           (100, 16, 16, 4, 9), (200, 80, 304, 600, 2),
+                                           # ragged in every extent (odd row lengths: element-wise loads and stores)
+                                           (70, 33, 45, 129, 5), (7, 5, 9, 3, 11), (131, 577, 99, 250, 2), (1, 1, 1, 1, 4)])
 def test_i8_gemm_pair_equals_the_oracle_chain_and_the_fp64_definition(m, k, n, p, batch):
     """C += alpha (A X) B^T: the oracle's emulated product applied twice (alpha a power of two, so that alpha * v is exact
     and the final sum is one rounding on both sides): bit for bit; against the plain FP64 definition: 1e-10 of max|C|."""
@@ -123,7 +129,7 @@ def test_i8_gemm_pair_rejects_what_it_cannot_run():
     buf = torch.zeros(1 << 16, dtype=torch.float64, device="cuda")
     q, st = buf.data_ptr(), _stream(torch)
     gemm_pair_batched_i8(16, 16, 16, 16, 0, 1.0, q, q, q, q, st)                       # batch 0: no-op
-    for bad in [(16, 24, 16, 16), (16, 16, 8, 16), (16, 16, 16, 6), (0, 16, 16, 16), (16, 16, 16, 0)]:
+    for bad in [(0, 16, 16, 16), (16, 0, 16, 16), (16, 16, -1, 16), (16, 16, 16, 0)]:
         with pytest.raises(Su2Error):
             gemm_pair_batched_i8(*bad, 1, 1.0, q, q, q, q, st)
     with pytest.raises(Su2Error):
@@ -133,7 +139,7 @@ def test_i8_gemm_pair_rejects_what_it_cannot_run():
     with pytest.raises(Su2Error):
         gemm_pair_batched_i8(16, 16, 16, 16, 1, 1.0, q, q, q, q, st, 8)                # nslices out of range
     with pytest.raises(Su2Error):
-        gemm_pair_batched_i8(16, 16, 16, 16, 1, 1.0, q, q + 8, q, q, st)               # misaligned operand
+        gemm_pair_batched_i8(16, 16, 16, 16, 1, 1.0, q, q + 4, q, q, st)               # operand not 8-byte aligned
     with pytest.raises(Su2Error) as info:
         gemm_pair_batched_i8(16, 16, 16, 16, 1, 1.0, q, q, q, q, st, 0, q, 256)        # workspace below one item
     assert "workspace limit below one item" in str(info.value)

@@ -45,8 +45,9 @@ def test_library_exports_every_declared_symbol(lib):
     assert {"su2_gemm_pair_batched_i8", "su2_matmul_batched_i8", "su2_ozaki_workspace_bytes"} <= declared_oz
     for name in declared_oz:
         assert hasattr(oz, name), name
-    assert oz.su2_gemm_pair_batched_i8(16, 24, 16, 16, 1, 1.0, 16, 16, 16, 16, 0, None, 0, None) == -1
-    assert b"multiples of 16" in oz.su2_ozaki_last_error()
+    assert oz.su2_gemm_pair_batched_i8(16, 24, 16, 16, 1, 1.0, 16, 16, 16, 16, 9, None, 0, None) == -1
+    assert b"nslices" in oz.su2_ozaki_last_error()
+    assert ozaki_workspace_bytes(70, 33, 45, 129, 1) == ozaki_workspace_bytes(70, 48, 48, 132, 1)      # padded extents
     assert ozaki_workspace_bytes(512, 512, 512, 512, 1) == 14688256 and ozaki_workspace_bytes(512, 512, 512, 512, 1, 9) == 0
     assert sorted(os.listdir(os.path.join(ROOT, "include"))) == ["su2_heff.h", "su2_ozaki.h", "su2_probe.h"]
 
