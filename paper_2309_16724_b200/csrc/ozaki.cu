@@ -213,8 +213,8 @@ __device__ __forceinline__ void combine4(const int32_t* __restrict__ planes, int
 // the INT8 rows all have the padded pitch nP; the padding columns hold zero planes and zero exponents, so they come out as zero
 // slices without a special case.  T_ij = 2^(e_i + f_j) sum_d ...; row exponent g_i from max_j |T_ij|; slices of T_ij 2^(-g_i) at
 // qT[(row S + s) nP + j].  T is never stored in FP64: rows of up to 128 NSTEP columns stay in registers between the exponent
-// pass and the slicing pass (NSTEP = 1, 2, 4, 8, 16); longer rows (NSTEP = 0) are recombined twice, the second read of the
-// planes coming from L1/L2.
+// pass and the slicing pass (NSTEP = 1, 2, 4, 8); longer rows (NSTEP = 0) are recombined twice, the second read of the planes
+// coming from L1/L2 (64 FP64 registers per lane for 2048 columns measured slower than the second read).
 template <int S, int NSTEP>
 __global__ void __launch_bounds__(256)
 combine_slice_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, int rows, int nP, int64_t nlines,
@@ -421,7 +421,6 @@ int run_chunk(int m, int k, int n, int p, int c, double alpha, const double* A, 
     else if (nP <= 256) combine_slice_kernel<S, 2><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, fX, qT, gT);
     else if (nP <= 512) combine_slice_kernel<S, 4><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, fX, qT, gT);
     else if (nP <= 1024) combine_slice_kernel<S, 8><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, fX, qT, gT);
-    else if (nP <= 2048) combine_slice_kernel<S, 16><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, fX, qT, gT);
     else combine_slice_kernel<S, 0><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, fX, qT, gT);
   }
   OZ_LAUNCH_CHECK("combine_slice_kernel launch");
