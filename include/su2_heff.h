@@ -191,6 +191,25 @@ su2_status su2_plan_export_tasks(const su2_plan* plan, int32_t* out_sec, int32_t
                                  int32_t* fam_r, int32_t* blk_r, int32_t* adj_r,
                                  int32_t* term, double* coef);
 
+/* Device view of the task table after upload (sector-task-table with resolved operands): one record per task
+ * F_s += coef * sum_pos alpha[pos] * Aop_pos * E_s' * Dop_pos^T (Eq. (3)).  Aop_pos is the m x k block at
+ * A + pos * strideA (row pitch ldA), or its transpose if transA (the block is then stored k x m); Dop_pos the p x n block
+ * at D + pos * strideD (row pitch ldD), or stored n x p if transD; stride 0 = one block for all positions.  alpha: DEVICE
+ * [npos] or NULL (all 1).  E_s' is the dense k x n block at psi + e_off, F_s the dense m x p block at out + f_off.  One-sided
+ * rows appear with their operators already folded over the positions (npos = 1).  The pointers belong to the plan. */
+typedef struct {
+  const double* A;
+  const double* D;
+  const double* alpha;
+  double coef;
+  int64_t strideA, strideD, e_off, f_off;
+  int32_t ldA, ldD, transA, transD;
+  int32_t m, k, n, p, npos, pad;
+} su2_task_view;
+/* Writes min(capacity, ntasks) records to tasks (HOST) and returns ntasks; -1 for a NULL or host-only plan.  This is what
+ * an alternative execution of the same plan needs (su2_ozaki.h: H_eff * Psi on the INT8 tensor path). */
+int64_t su2_plan_export_task_views(const su2_plan* plan, su2_task_view* tasks, int64_t capacity);
+
 /* out_dev = H_eff * psi_dev (overwrites; out must not alias psi).  Asynchronous on the stream.
  * workspace_dev: DEVICE, >= workspace_bytes, 256-byte aligned.  The workspace and the plan's work-queue counter
  * are shared by every apply of the plan: applies of ONE plan must be ordered on one stream (two plans may run

@@ -18,6 +18,8 @@
 #include <stddef.h>
 #include <stdint.h>
 
+#include "su2_heff.h"   /* su2_task_view */
+
 #ifdef __cplusplus
 extern "C" {
 #endif
@@ -57,6 +59,21 @@ int32_t su2_gemm_pair_batched_i8(int32_t m, int32_t k, int32_t n, int32_t p, int
  * emulated_matmul defines, for element-by-element parity.  Same restriction. */
 int32_t su2_matmul_batched_i8(int32_t m, int32_t k, int32_t n, int64_t batch, const double* A, const double* X,
                               double* C, int32_t nslices, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* out = H_eff * psi with every task of a plan executed on the INT8 tensor path (row f4 inside the hot path):
+ * tasks: HOST [ntask], the records that su2_heff.h's export of task views hands out (device operands of the plan).
+ * Per task F_s += coef * sum_pos alpha_pos * Aop_pos * E * Dop_pos^T (Eq. (3)) runs as two batched sliced
+ * products over the positions: E is sliced once per task, A_pos / D_pos on the fly (operators stored transposed become
+ * MN-major INT8 operands, no transposed copy; a block shared by all positions is sliced once), the second product's
+ * integer planes are recombined and summed over the positions in index order (deterministic) into F_s.
+ * psi, out: DEVICE [psi_len] (out is overwritten; must not alias psi).  workspace: DEVICE, 256-byte aligned; a task is
+ * processed in chunks of as many positions as fit (about 7 (m k + p n + m n) + 28 m max(n, p) bytes per position).
+ * Accuracy: each product within the bound above with K = k or n; 7 slices give <= 1e-12 of max|F| on the synthetic
+ * workloads (tests: 1e-10 against the oracle, the tolerance of su2_heff_apply).  Launch-bound for small blocks: one task
+ * costs 17 + 2 kernel launches, so this pays for bonds whose blocks hold several hundred multiplets.
+ * Returns 0, -1 (invalid argument, a contraction too long for exact int32 sums, workspace below one position) or -5. */
+int32_t su2_heff_apply_i8(const su2_task_view* tasks, int64_t ntask, const double* psi, double* out, int64_t psi_len,
+                          int32_t nslices, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* Bytes of workspace `items` items need (p = 0: the single product); 0 for invalid arguments. */
 size_t su2_ozaki_workspace_bytes(int32_t m, int32_t k, int32_t n, int32_t p, int64_t items, int32_t nslices);

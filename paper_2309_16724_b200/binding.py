@@ -55,6 +55,13 @@ class su2_problem(C.Structure):
                 ("symmetry", C.c_int32), ("site_u1", C.POINTER(su2_siteop_u1))]
 
 
+class su2_task_view(C.Structure):
+    _fields_ = [("A", C.c_void_p), ("D", C.c_void_p), ("alpha", C.c_void_p), ("coef", C.c_double),
+                ("strideA", C.c_int64), ("strideD", C.c_int64), ("e_off", C.c_int64), ("f_off", C.c_int64),
+                ("ldA", C.c_int32), ("ldD", C.c_int32), ("transA", C.c_int32), ("transD", C.c_int32),
+                ("m", C.c_int32), ("k", C.c_int32), ("n", C.c_int32), ("p", C.c_int32), ("npos", C.c_int32), ("pad", C.c_int32)]
+
+
 class su2_plan_info_t(C.Structure):
     _fields_ = [("psi_len", C.c_int64), ("ntasks", C.c_int64), ("ntask_positions", C.c_int64),
                 ("cc_flops", C.c_double), ("executed_flops", C.c_double), ("operator_bytes", C.c_double),
@@ -67,7 +74,7 @@ EXPORTS = ["su2_wigner_6j", "su2_wigner_9j", "su2_status_string", "su2_last_cuda
            "su2_plan_psi_layout", "su2_plan_export_tasks", "su2_heff_apply", "su2_heff_apply_host", "su2_heff_diag",
            "su2_davidson_workspace_bytes", "su2_davidson_create", "su2_davidson_create_sharded", "su2_davidson_step", "su2_davidson_set_preconditioner", "su2_davidson_ritz_vector",
            "su2_davidson_destroy", "su2_gemm_pair_batched", "su2_gemm_pair_batched_route", "su2_precontract", "su2_renormalize", "su2_heff_apply_noalloc",
-           "su2_noalloc_scratch_bytes"]
+           "su2_noalloc_scratch_bytes", "su2_plan_export_task_views"]
 
 REDUCE_FN = C.CFUNCTYPE(C.c_int32, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p)   # su2_reduce_fn
 
@@ -100,6 +107,8 @@ def load():
     lib.su2_plan_info.argtypes = [C.c_void_p, C.POINTER(su2_plan_info_t)]
     lib.su2_plan_psi_layout.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     lib.su2_plan_export_tasks.argtypes = [C.c_void_p] + [C.c_void_p] * 10
+    lib.su2_plan_export_task_views.restype = C.c_int64
+    lib.su2_plan_export_task_views.argtypes = [C.c_void_p, C.POINTER(su2_task_view), C.c_int64]
     lib.su2_heff_apply.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.su2_heff_apply_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.su2_noalloc_scratch_bytes.restype = C.c_int64
@@ -249,6 +258,16 @@ class Plan:
         check(load().su2_plan_export_tasks(self.handle, *[arrs[k].ctypes.data for k in names], coef.ctypes.data))
         arrs["coef"] = coef
         return arrs
+
+    def export_task_views(self):
+        """The uploaded task table with resolved device operands (su2_plan_export_task_views): a ctypes array of
+        su2_task_view, valid as long as the plan lives."""
+        n = int(load().su2_plan_export_task_views(self.handle, None, 0))
+        if n < 0:
+            raise Su2Error("su2_plan_export_task_views: host-only plan")
+        views = (su2_task_view * n)()
+        load().su2_plan_export_task_views(self.handle, views, n)
+        return views
 
     # --- device entry points (pointers are plain ints) ---
     def heff_apply(self, psi_ptr, out_ptr, workspace_ptr, stream=0):
@@ -429,6 +448,8 @@ def load_ozaki():
         lib.su2_gemm_pair_batched_i8.argtypes = [C.c_int32] * 4 + [C.c_int64, C.c_double, dp, dp, dp, dp, C.c_int32, dp, C.c_size_t, dp]
         lib.su2_matmul_batched_i8.restype = C.c_int32
         lib.su2_matmul_batched_i8.argtypes = [C.c_int32] * 3 + [C.c_int64, dp, dp, dp, C.c_int32, dp, C.c_size_t, dp]
+        lib.su2_heff_apply_i8.restype = C.c_int32
+        lib.su2_heff_apply_i8.argtypes = [C.POINTER(su2_task_view), C.c_int64, dp, dp, C.c_int64, C.c_int32, dp, C.c_size_t, dp]
         lib.su2_ozaki_workspace_bytes.restype = C.c_size_t
         lib.su2_ozaki_workspace_bytes.argtypes = [C.c_int32] * 4 + [C.c_int64, C.c_int32]
         lib.su2_ozaki_launch_count.restype = C.c_int64
@@ -462,3 +483,9 @@ def ozaki_workspace_bytes(m, k, n, p, items, nslices=0):
 
 def ozaki_launch_count():
     return int(load_ozaki().su2_ozaki_launch_count())
+
+
+def heff_apply_i8(task_views, psi_ptr, out_ptr, psi_len, workspace_ptr, workspace_bytes, stream=0, nslices=0):
+    """out = H_eff psi with every task on the INT8 tensor path (su2_heff_apply_i8); task_views: Plan.export_task_views()."""
+    _check_ozaki(load_ozaki().su2_heff_apply_i8(task_views, len(task_views), psi_ptr, out_ptr, psi_len, nslices, workspace_ptr,
+                                                workspace_bytes, stream))

@@ -146,25 +146,28 @@ slice_rows_kernel(const double* __restrict__ src, int64_t istride, int64_t ld, i
   }
 }
 
-// ---- slicing of an MN-major right operand (X: k x n as stored, contraction index along its rows): one CTA per (128-column strip, item)
-// expo[item nP + c] = exponent of column c (0 for the padding columns); slice s of element (j, c) goes to
-// q[item][(S-1-s) kP + j][c] (row pitch nP); rows k..kP-1 and columns n..nP-1 are zero.
-template <int S>
+// ---- slicing of an MN-major operand (the contraction index runs down the rows of the stored block): one CTA per (128-column strip, item)
+// src: items (istride apart) of k rows of n FP64, row pitch ld.  expo[item nP + c] = exponent of column c (0 for the padding
+// columns); slice s of element (j, c) goes to q[item][slot(s) kP + j][c] (row pitch nP), slot(s) = S-1-s for a right operand
+// (REVERSED: X as stored, D stored transposed) or s for a left operand (A stored transposed: an M-major left operand); rows
+// k..kP-1 and columns n..nP-1 are zero.
+template <int S, bool REVERSED>
 __global__ void __launch_bounds__(256)
-slice_cols_kernel(const double* __restrict__ src, int k, int n, int kP, int nP, int8_t* __restrict__ q, int32_t* __restrict__ expo) {
+slice_cols_kernel(const double* __restrict__ src, int64_t istride, int64_t ld, int k, int n, int kP, int nP, int8_t* __restrict__ q,
+                  int32_t* __restrict__ expo) {
   __shared__ unsigned long long s_amax[8][128];
   __shared__ int s_e[128];
   const int lane = threadIdx.x & 31, wy = threadIdx.x >> 5;
   const int64_t item = blockIdx.y;
   const int c = blockIdx.x * 128 + lane * 4;
   const bool live = c < nP;                                  // nP % 4 == 0: a thread's 4 columns are all inside or all outside
-  const double* __restrict__ x = src + item * (int64_t)k * n;
-  const bool vec = !(n & 1) && ((uintptr_t)x & 15) == 0;     // every row of this item starts on a 16-byte boundary
+  const double* __restrict__ x = src + item * istride;
+  const bool vec = !(ld & 1) && ((uintptr_t)x & 15) == 0;    // every row of this item starts on a 16-byte boundary
   unsigned long long a[4] = {0, 0, 0, 0};
   if (live)
     for (int j = wy; j < k; j += 8) {
       double v[4];
-      load4(x + (int64_t)j * n, c, n, vec, v);
+      load4(x + (int64_t)j * ld, c, n, vec, v);
 #pragma unroll
       for (int u = 0; u < 4; ++u) a[u] = max(a[u], abs_bits(v[u]));
     }
@@ -185,12 +188,12 @@ slice_cols_kernel(const double* __restrict__ src, int k, int n, int kP, int nP, 
   int8_t* __restrict__ out = q + item * (int64_t)S * kP * nP;
   for (int j = wy; j < kP; j += 8) {
     double v[4] = {0.0, 0.0, 0.0, 0.0};
-    if (j < k) load4(x + (int64_t)j * n, c, n, vec, v);
+    if (j < k) load4(x + (int64_t)j * ld, c, n, vec, v);
     int8_t q0[OZ_SMAX], q1[OZ_SMAX], q2[OZ_SMAX], q3[OZ_SMAX];
     slices_of<S>(v[0], e0, q0); slices_of<S>(v[1], e1, q1); slices_of<S>(v[2], e2, q2); slices_of<S>(v[3], e3, q3);
 #pragma unroll
     for (int s = 0; s < S; ++s)
-      *(char4*)(out + ((int64_t)(S - 1 - s) * kP + j) * nP + c) = make_char4(q0[s], q1[s], q2[s], q3[s]);
+      *(char4*)(out + ((int64_t)(REVERSED ? S - 1 - s : s) * kP + j) * nP + c) = make_char4(q0[s], q1[s], q2[s], q3[s]);
   }
 }
 
@@ -218,14 +221,14 @@ __device__ __forceinline__ void combine4(const int32_t* __restrict__ planes, int
 template <int S, int NSTEP>
 __global__ void __launch_bounds__(256)
 combine_slice_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, int rows, int nP, int64_t nlines,
-                     const int32_t* __restrict__ e_row, const int32_t* __restrict__ f_col, int8_t* __restrict__ qT,
-                     int32_t* __restrict__ g_row) {
+                     const int32_t* __restrict__ e_row, int e_pitch, const int32_t* __restrict__ f_col, int f_pitch,
+                     int8_t* __restrict__ qT, int32_t* __restrict__ g_row) {
   const int lane = threadIdx.x & 31;
   const int64_t line = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (line >= nlines) return;
   const int64_t item = line / rows;
-  const int e = e_row[line];
-  const int32_t* __restrict__ f = f_col + item * nP;
+  const int e = e_row[item * e_pitch + (line - item * rows)];      // pitch 0: one operand shared by all items
+  const int32_t* __restrict__ f = f_col + item * f_pitch;
   int8_t* __restrict__ out = qT + line * (int64_t)S * nP;
   // T_ij for the 4 columns at j, exactly as the oracle forms it: the recombined sum, then one scaling by 2^(e_i + f_j)
   auto t_at = [&](int j, double (&t)[4]) {
@@ -309,9 +312,10 @@ combine_out_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, int
   }
 }
 
-// ---- the exact INT8 GEMM: D (M x N, int32, row-major) = L (M x K, int8, K-major) . R, batched; R is K x N with N contiguous
-// (RMajorN = true: X as stored) or N x K with K contiguous (false: B as stored).  Two tile configurations: 256 x 256 x 128 on a
-// pair of SMs (cta_group::2, cluster 2 x 1) for outputs of at least 256 x 256, 128 x 128 x 128 on one SM below that.
+// ---- the exact INT8 GEMM: D (M x N, int32, row-major) = L . R, batched.  L is M x K with K contiguous (LMajorM = false: slices of
+// rows) or K x M with M contiguous (true: slices of an operand stored transposed); R is K x N with N contiguous (RMajorN = true:
+// X as stored) or N x K with K contiguous (false: B as stored).  Two tile configurations: 256 x 256 x 128 on a pair of SMs
+// (cta_group::2, cluster 2 x 1) for outputs of at least 256 x 256, 128 x 128 x 128 on one SM below that.
 template <int TM, int TN, int CM>
 struct I8Config {
   using Tile = cute::Shape<cute::Int<TM>, cute::Int<TN>, cute::_128>;
@@ -320,23 +324,26 @@ struct I8Config {
       cutlass::arch::Sm100, cutlass::arch::OpClassTensorOp, Tile, Cluster, cutlass::epilogue::collective::EpilogueTileAuto, int32_t,
       int32_t, int32_t, cutlass::layout::RowMajor, 4, int32_t, cutlass::layout::RowMajor, 4,
       cutlass::epilogue::collective::EpilogueScheduleAuto>::CollectiveOp;
-  template <class LayoutR>
+  template <class LayoutL, class LayoutR>
   using Mainloop = typename cutlass::gemm::collective::CollectiveBuilder<
-      cutlass::arch::Sm100, cutlass::arch::OpClassTensorOp, int8_t, cutlass::layout::RowMajor, 16, int8_t, LayoutR, 16, int32_t, Tile,
+      cutlass::arch::Sm100, cutlass::arch::OpClassTensorOp, int8_t, LayoutL, 16, int8_t, LayoutR, 16, int32_t, Tile,
       Cluster, cutlass::gemm::collective::StageCountAutoCarveout<static_cast<int>(sizeof(typename Epilogue::SharedStorage))>,
       cutlass::gemm::collective::KernelScheduleAuto>::CollectiveOp;
-  template <class LayoutR>
+  template <class LayoutL, class LayoutR>
   using Gemm = cutlass::gemm::device::GemmUniversalAdapter<
-      cutlass::gemm::kernel::GemmUniversal<cute::Shape<int, int, int, int>, Mainloop<LayoutR>, Epilogue>>;
+      cutlass::gemm::kernel::GemmUniversal<cute::Shape<int, int, int, int>, Mainloop<LayoutL, LayoutR>, Epilogue>>;
 };
 using I8Small = I8Config<128, 128, 1>;
 using I8Large = I8Config<256, 256, 2>;
 
-template <class Cfg, bool RMajorN>
+template <class Cfg, bool LMajorM, bool RMajorN>
 int i8_gemm_cfg(int M, int N, int K, int L, const int8_t* Lp, int64_t ldl, int64_t batchL, const int8_t* Rp, int64_t ldr, int64_t batchR,
                 int32_t* D, int64_t batchD, cudaStream_t stream) {
-  using Gemm = typename Cfg::template Gemm<std::conditional_t<RMajorN, cutlass::layout::RowMajor, cutlass::layout::ColumnMajor>>;
-  typename Gemm::GemmKernel::StrideA sa = cute::make_stride(ldl, cute::Int<1>{}, batchL);
+  using Gemm = typename Cfg::template Gemm<std::conditional_t<LMajorM, cutlass::layout::ColumnMajor, cutlass::layout::RowMajor>,
+                                           std::conditional_t<RMajorN, cutlass::layout::RowMajor, cutlass::layout::ColumnMajor>>;
+  typename Gemm::GemmKernel::StrideA sa;
+  if constexpr (LMajorM) sa = cute::make_stride(cute::Int<1>{}, ldl, batchL);       // (M, K, L): M contiguous
+  else sa = cute::make_stride(ldl, cute::Int<1>{}, batchL);                          // (M, K, L): K contiguous
   typename Gemm::GemmKernel::StrideB sb;
   if constexpr (RMajorN) sb = cute::make_stride(cute::Int<1>{}, ldr, batchR);       // (N, K, L): N contiguous
   else sb = cute::make_stride(ldr, cute::Int<1>{}, batchR);                          // (N, K, L): K contiguous
@@ -351,11 +358,11 @@ int i8_gemm_cfg(int M, int N, int K, int L, const int8_t* Lp, int64_t ldl, int64
   return OZ_OK;
 }
 
-template <bool RMajorN>
+template <bool LMajorM, bool RMajorN>
 int i8_gemm(int M, int N, int K, int L, const int8_t* Lp, int64_t ldl, int64_t batchL, const int8_t* Rp, int64_t ldr, int64_t batchR,
             int32_t* D, int64_t batchD, cudaStream_t stream) {
-  if (M >= 256 && N >= 256) return i8_gemm_cfg<I8Large, RMajorN>(M, N, K, L, Lp, ldl, batchL, Rp, ldr, batchR, D, batchD, stream);
-  return i8_gemm_cfg<I8Small, RMajorN>(M, N, K, L, Lp, ldl, batchL, Rp, ldr, batchR, D, batchD, stream);
+  if (M >= 256 && N >= 256) return i8_gemm_cfg<I8Large, LMajorM, RMajorN>(M, N, K, L, Lp, ldl, batchL, Rp, ldr, batchR, D, batchD, stream);
+  return i8_gemm_cfg<I8Small, LMajorM, RMajorN>(M, N, K, L, Lp, ldl, batchL, Rp, ldr, batchR, D, batchD, stream);
 }
 
 inline size_t up256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -400,11 +407,11 @@ int run_chunk(int m, int k, int n, int p, int c, double alpha, const double* A, 
   const int64_t rowsA = (int64_t)c * m;
   slice_rows_kernel<S, false><<<(unsigned)((rowsA + 7) / 8), 256, 0, st>>>(A, (int64_t)m * k, k, m, m, k, kP, rowsA, qA, eA);
   OZ_LAUNCH_CHECK("slice_rows_kernel(A) launch");
-  slice_cols_kernel<S><<<dim3((nP + 127) / 128, c), 256, 0, st>>>(X, k, n, kP, nP, qX, fX);
+  slice_cols_kernel<S, true><<<dim3((nP + 127) / 128, c), 256, 0, st>>>(X, (int64_t)k * n, n, k, n, kP, nP, qX, fX);
   OZ_LAUNCH_CHECK("slice_cols_kernel(X) launch");
   const int64_t ps1 = (int64_t)c * m * nP;
   for (int d = 0; d < S; ++d) {                               // diagonal d: L slices 0..d, R slices d..0 = slots S-1-d..S-1
-    const int rc = i8_gemm<true>(m, nP, (d + 1) * kP, c, qA, (int64_t)S * kP, (int64_t)m * S * kP, qX + (int64_t)(S - 1 - d) * kP * nP,
+    const int rc = i8_gemm<false, true>(m, nP, (d + 1) * kP, c, qA, (int64_t)S * kP, (int64_t)m * S * kP, qX + (int64_t)(S - 1 - d) * kP * nP,
                                  nP, (int64_t)S * kP * nP, planes + d * ps1, (int64_t)m * nP, st);
     if (rc != OZ_OK) return rc;
   }
@@ -417,11 +424,11 @@ int run_chunk(int m, int k, int n, int p, int c, double alpha, const double* A, 
   }
   {
     const unsigned grid = (unsigned)((rowsA + 7) / 8);
-    if (nP <= 128) combine_slice_kernel<S, 1><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, fX, qT, gT);
-    else if (nP <= 256) combine_slice_kernel<S, 2><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, fX, qT, gT);
-    else if (nP <= 512) combine_slice_kernel<S, 4><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, fX, qT, gT);
-    else if (nP <= 1024) combine_slice_kernel<S, 8><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, fX, qT, gT);
-    else combine_slice_kernel<S, 0><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, fX, qT, gT);
+    if (nP <= 128) combine_slice_kernel<S, 1><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, m, fX, nP, qT, gT);
+    else if (nP <= 256) combine_slice_kernel<S, 2><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, m, fX, nP, qT, gT);
+    else if (nP <= 512) combine_slice_kernel<S, 4><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, m, fX, nP, qT, gT);
+    else if (nP <= 1024) combine_slice_kernel<S, 8><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, m, fX, nP, qT, gT);
+    else combine_slice_kernel<S, 0><<<grid, 256, 0, st>>>(planes, ps1, m, nP, rowsA, eA, m, fX, nP, qT, gT);
   }
   OZ_LAUNCH_CHECK("combine_slice_kernel launch");
   const int64_t rowsB = (int64_t)c * pP;
@@ -429,7 +436,7 @@ int run_chunk(int m, int k, int n, int p, int c, double alpha, const double* A, 
   OZ_LAUNCH_CHECK("slice_rows_kernel(B) launch");
   const int64_t ps2 = (int64_t)c * m * pP;
   for (int d = 0; d < S; ++d) {
-    const int rc = i8_gemm<false>(m, pP, (d + 1) * nP, c, qT, (int64_t)S * nP, (int64_t)m * S * nP, qB + (int64_t)(S - 1 - d) * nP,
+    const int rc = i8_gemm<false, false>(m, pP, (d + 1) * nP, c, qT, (int64_t)S * nP, (int64_t)m * S * nP, qB + (int64_t)(S - 1 - d) * nP,
                                   (int64_t)S * nP, (int64_t)pP * S * nP, planes + d * ps2, (int64_t)m * pP, st);
     if (rc != OZ_OK) return rc;
   }
@@ -437,6 +444,125 @@ int run_chunk(int m, int k, int n, int p, int c, double alpha, const double* A, 
   combine_out_kernel<S, true><<<(unsigned)std::min<int64_t>((nquad + 255) / 256, 148 * 16), 256, 0, st>>>(planes, ps2, m, p, pP, nquad, gT, hB,
                                                                                                      alpha, C);
   OZ_LAUNCH_CHECK("combine_out_kernel launch");
+  return OZ_OK;
+}
+
+// ---- one task of H_eff * Psi (su2_task_view): F += coef sum_pos alpha_pos Aop_pos E Dop_pos^T -----------------------------------------
+// recombination of product 2 with the sum over the positions of a chunk:
+//   dst[i][j] += coef sum_b alpha_b 2^(g_(b,i) + h_(b,j)) sum_d P_d[b][i][j] 2^(-W (d+2)),   b in index order (deterministic)
+// planes: [S][items][rowsT][colsP]; g: [items][rowsT]; h: [items or 1][colsP] (h_pitch 0: D is the same block for all positions)
+template <int S>
+__global__ void __launch_bounds__(256)
+combine_reduce_kernel(const int32_t* __restrict__ planes, int64_t plane_stride, int items, int rowsT, int rows, int cols, int colsP,
+                      const int32_t* __restrict__ g_row, const int32_t* __restrict__ h_col, int h_pitch,
+                      const double* __restrict__ alpha, double coef, double* __restrict__ dst) {
+  const int cq = (cols + 3) >> 2;
+  const int64_t nquad = (int64_t)rows * cq;
+  for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < nquad; t += (int64_t)gridDim.x * blockDim.x) {
+    const int i = (int)(t / cq), j = (int)(t - (int64_t)i * cq) * 4;
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    for (int b = 0; b < items; ++b) {
+      double v[4];
+      combine4<S>(planes, plane_stride, ((int64_t)b * rowsT + i) * colsP + j, v);
+      const int g = g_row[(int64_t)b * rowsT + i];
+      const int4 hj = *(const int4*)(h_col + (int64_t)b * h_pitch + j);
+      const double a = coef * (alpha ? alpha[b] : 1.0);
+      acc[0] += a * scale2(v[0], g + hj.x); acc[1] += a * scale2(v[1], g + hj.y);
+      acc[2] += a * scale2(v[2], g + hj.z); acc[3] += a * scale2(v[3], g + hj.w);
+    }
+    double* o = dst + (int64_t)i * cols + j;
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (j + u < cols) o[u] += acc[u];
+  }
+}
+
+// bytes of workspace a chunk of c positions of this task needs, and the carve-up
+struct TaskSpace {
+  size_t qA, qX, planes, qT, qB, eA, fX, gT, hB, total;
+  int kP, nP, mP, pP, rowsT;
+  TaskSpace(const su2_task_view& t, int64_t c, int S) {
+    kP = up16(t.k); nP = up16(t.n); mP = up16(t.m);
+    pP = t.transD ? up16(t.p) : up4(t.p);
+    rowsT = t.transA ? mP : t.m;                    // an M-major left operand brings its padded rows along
+    const int64_t cA = t.strideA ? c : 1, cD = t.strideD ? c : 1;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { const size_t at = o; o += up256(bytes); return at; };
+    qA = take((size_t)cA * rowsT * S * kP);
+    qX = take((size_t)S * kP * nP);
+    planes = take((size_t)c * S * 4 * rowsT * std::max(nP, pP));
+    qT = take((size_t)c * rowsT * S * nP);
+    qB = take((size_t)cD * pP * S * nP);
+    eA = take((size_t)cA * rowsT * 4); fX = take((size_t)nP * 4);
+    gT = take((size_t)c * rowsT * 4); hB = take((size_t)cD * pP * 4);
+    total = o;
+  }
+};
+
+template <int S>
+int run_task(const su2_task_view& t, const double* psi, double* out, char* ws, size_t ws_bytes, cudaStream_t st) {
+  if ((int64_t)S * up16(std::max(t.k, t.n)) * 127 * 127 >= ((int64_t)1 << 31)) return fail(OZ_INVALID, "task: contraction too long for exact int32 accumulation");
+  int64_t c = t.npos;
+  while (c > 1 && TaskSpace(t, c, S).total > ws_bytes) c = (c + 1) / 2;
+  const TaskSpace w(t, c, S);
+  if (w.total > ws_bytes) return fail(OZ_INVALID, "task: workspace below one position");
+  const int kP = w.kP, nP = w.nP, mP = w.mP, pP = w.pP, rowsT = w.rowsT;
+  int8_t *qA = (int8_t*)(ws + w.qA), *qX = (int8_t*)(ws + w.qX), *qT = (int8_t*)(ws + w.qT), *qB = (int8_t*)(ws + w.qB);
+  int32_t *planes = (int32_t*)(ws + w.planes), *eA = (int32_t*)(ws + w.eA), *fX = (int32_t*)(ws + w.fX), *gT = (int32_t*)(ws + w.gT),
+          *hB = (int32_t*)(ws + w.hB);
+  // E is the same for every position: sliced once per task
+  slice_cols_kernel<S, true><<<dim3((nP + 127) / 128, 1), 256, 0, st>>>(psi + t.e_off, 0, t.n, t.k, t.n, kP, nP, qX, fX);
+  OZ_LAUNCH_CHECK("slice_cols_kernel(E) launch");
+  for (int64_t pos0 = 0; pos0 < t.npos; pos0 += c) {
+    const int cc = (int)std::min<int64_t>(c, t.npos - pos0);
+    const int cA = t.strideA ? cc : 1, cD = t.strideD ? cc : 1;
+    const double* A = t.A + pos0 * t.strideA;
+    const double* D = t.D + pos0 * t.strideD;
+    if (pos0 == 0 || t.strideA) {
+      if (t.transA) slice_cols_kernel<S, false><<<dim3((mP + 127) / 128, cA), 256, 0, st>>>(A, t.strideA, t.ldA, t.k, t.m, kP, mP, qA, eA);
+      else slice_rows_kernel<S, false><<<(unsigned)(((int64_t)cA * t.m + 7) / 8), 256, 0, st>>>(A, t.strideA, t.ldA, t.m, t.m, t.k, kP, (int64_t)cA * t.m, qA, eA);
+      OZ_LAUNCH_CHECK("slice kernel (A) launch");
+    }
+    if (pos0 == 0 || t.strideD) {
+      if (t.transD) slice_cols_kernel<S, true><<<dim3((pP + 127) / 128, cD), 256, 0, st>>>(D, t.strideD, t.ldD, t.n, t.p, nP, pP, qB, hB);
+      else slice_rows_kernel<S, true><<<(unsigned)(((int64_t)cD * pP + 7) / 8), 256, 0, st>>>(D, t.strideD, t.ldD, t.p, pP, t.n, nP, (int64_t)cD * pP, qB, hB);
+      OZ_LAUNCH_CHECK("slice kernel (D) launch");
+    }
+    const int64_t ps1 = (int64_t)cc * rowsT * nP;
+    for (int d = 0; d < S; ++d) {
+      int rc;
+      if (t.transA) rc = i8_gemm<true, true>(rowsT, nP, (d + 1) * kP, cc, qA, mP, t.strideA ? (int64_t)S * kP * mP : 0, qX + (int64_t)(S - 1 - d) * kP * nP,
+                                             nP, 0, planes + d * ps1, (int64_t)rowsT * nP, st);
+      else rc = i8_gemm<false, true>(rowsT, nP, (d + 1) * kP, cc, qA, (int64_t)S * kP, t.strideA ? (int64_t)rowsT * S * kP : 0,
+                                     qX + (int64_t)(S - 1 - d) * kP * nP, nP, 0, planes + d * ps1, (int64_t)rowsT * nP, st);
+      if (rc != OZ_OK) return rc;
+    }
+    {
+      const int64_t lines = (int64_t)cc * rowsT;
+      const unsigned grid = (unsigned)((lines + 7) / 8);
+      const int ep = t.strideA ? rowsT : 0;
+      if (nP <= 128) combine_slice_kernel<S, 1><<<grid, 256, 0, st>>>(planes, ps1, rowsT, nP, lines, eA, ep, fX, 0, qT, gT);
+      else if (nP <= 256) combine_slice_kernel<S, 2><<<grid, 256, 0, st>>>(planes, ps1, rowsT, nP, lines, eA, ep, fX, 0, qT, gT);
+      else if (nP <= 512) combine_slice_kernel<S, 4><<<grid, 256, 0, st>>>(planes, ps1, rowsT, nP, lines, eA, ep, fX, 0, qT, gT);
+      else if (nP <= 1024) combine_slice_kernel<S, 8><<<grid, 256, 0, st>>>(planes, ps1, rowsT, nP, lines, eA, ep, fX, 0, qT, gT);
+      else combine_slice_kernel<S, 0><<<grid, 256, 0, st>>>(planes, ps1, rowsT, nP, lines, eA, ep, fX, 0, qT, gT);
+      OZ_LAUNCH_CHECK("combine_slice_kernel launch");
+    }
+    const int64_t ps2 = (int64_t)cc * rowsT * pP;
+    for (int d = 0; d < S; ++d) {
+      int rc;
+      if (t.transD) rc = i8_gemm<false, true>(rowsT, pP, (d + 1) * nP, cc, qT, (int64_t)S * nP, (int64_t)rowsT * S * nP,
+                                              qB + (int64_t)(S - 1 - d) * nP * pP, pP, t.strideD ? (int64_t)S * nP * pP : 0, planes + d * ps2,
+                                              (int64_t)rowsT * pP, st);
+      else rc = i8_gemm<false, false>(rowsT, pP, (d + 1) * nP, cc, qT, (int64_t)S * nP, (int64_t)rowsT * S * nP, qB + (int64_t)(S - 1 - d) * nP,
+                                      (int64_t)S * nP, t.strideD ? (int64_t)pP * S * nP : 0, planes + d * ps2, (int64_t)rowsT * pP, st);
+      if (rc != OZ_OK) return rc;
+    }
+    const int64_t nquad = (int64_t)t.m * ((t.p + 3) / 4);
+    combine_reduce_kernel<S><<<(unsigned)std::min<int64_t>((nquad + 255) / 256, 148 * 16), 256, 0, st>>>(
+        planes, ps2, cc, rowsT, t.m, t.p, pP, gT, hB, t.strideD ? pP : 0, t.alpha ? t.alpha + pos0 : nullptr, t.coef, out + t.f_off);
+    OZ_LAUNCH_CHECK("combine_reduce_kernel launch");
+  }
   return OZ_OK;
 }
 
@@ -502,6 +628,33 @@ extern "C" int32_t su2_gemm_pair_batched_i8(int32_t m, int32_t k, int32_t n, int
 extern "C" int32_t su2_matmul_batched_i8(int32_t m, int32_t k, int32_t n, int64_t batch, const double* A, const double* X, double* C,
                                          int32_t nslices, void* workspace, size_t workspace_bytes, void* cuda_stream) {
   return run(m, k, n, 0, batch, 1.0, A, X, nullptr, C, nslices, workspace, workspace_bytes, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int32_t su2_heff_apply_i8(const su2_task_view* tasks, int64_t ntask, const double* psi, double* out, int64_t psi_len,
+                                     int32_t nslices, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  g_err[0] = 0;
+  if (!tasks || ntask < 0 || !psi || !out || psi == out || psi_len < 0 || !workspace || ((uintptr_t)workspace & 255))
+    return fail(OZ_INVALID, "null pointer, out aliasing psi, or a workspace that is not 256-byte aligned");
+  if (nslices == 0) nslices = OZ_SMAX;
+  if (nslices < 2 || nslices > OZ_SMAX) return fail(OZ_INVALID, "nslices must be 0 or 2..7");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  cudaError_t e = cudaMemsetAsync(out, 0, (size_t)psi_len * sizeof(double), st);
+  if (e != cudaSuccess) return fail(OZ_CUDA, "cudaMemsetAsync(out)", e);
+  for (int64_t i = 0; i < ntask; ++i) {
+    const su2_task_view& t = tasks[i];
+    if (!t.A || !t.D || t.m <= 0 || t.k <= 0 || t.n <= 0 || t.p <= 0 || t.npos <= 0) return fail(OZ_INVALID, "task: null operand or non-positive extent");
+    int rc;
+    switch (nslices) {
+      case 2: rc = run_task<2>(t, psi, out, (char*)workspace, workspace_bytes, st); break;
+      case 3: rc = run_task<3>(t, psi, out, (char*)workspace, workspace_bytes, st); break;
+      case 4: rc = run_task<4>(t, psi, out, (char*)workspace, workspace_bytes, st); break;
+      case 5: rc = run_task<5>(t, psi, out, (char*)workspace, workspace_bytes, st); break;
+      case 6: rc = run_task<6>(t, psi, out, (char*)workspace, workspace_bytes, st); break;
+      default: rc = run_task<7>(t, psi, out, (char*)workspace, workspace_bytes, st); break;
+    }
+    if (rc != OZ_OK) return rc;
+  }
+  return OZ_OK;
 }
 
 extern "C" size_t su2_ozaki_workspace_bytes(int32_t m, int32_t k, int32_t n, int32_t p, int64_t items, int32_t nslices) {

@@ -885,3 +885,22 @@ extern "C" const char* su2_status_string(su2_status st) {
     default: return "unknown status";
   }
 }
+
+extern "C" int64_t su2_plan_export_task_views(const su2_plan* plan, su2_task_view* tasks, int64_t capacity) {
+  if (!plan || plan->host_only) return -1;
+  const int64_t n = (int64_t)plan->h_tasks.size();
+  if (!tasks) return n;
+  for (int64_t i = 0; i < std::min(n, capacity); ++i) {
+    const su2::DevTask& t = plan->h_tasks[i];          // operands resolved by upload_plan
+    const su2::HostTask& h = plan->tasks[i];
+    su2_task_view v{};
+    v.A = t.A; v.D = t.D; v.alpha = t.alpha; v.coef = t.coef;
+    v.strideA = t.strideA; v.strideD = t.strideD;
+    v.e_off = plan->psi[h.in_sec].off; v.f_off = plan->psi[h.out_sec].off;
+    v.ldA = t.ldA; v.ldD = t.ldD;
+    v.transA = (t.flags & su2::TASK_TRANS_A) ? 1 : 0; v.transD = (t.flags & su2::TASK_TRANS_D) ? 1 : 0;
+    v.m = t.m; v.k = t.k; v.n = t.n; v.p = t.p; v.npos = t.npos; v.pad = 0;
+    tasks[i] = v;
+  }
+  return n;
+}

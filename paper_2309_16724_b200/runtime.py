@@ -80,6 +80,21 @@ class HeffOperator:
         self.plan.heff_apply_noalloc(psi.data_ptr(), out.data_ptr(), torch.cuda.current_stream(self.device).cuda_stream)
         return out
 
+    def apply_i8(self, psi, out=None, nslices=0, workspace_bytes=4 << 30):
+        """out = H_eff psi with every task on the INT8 tensor path (su2_heff_apply_i8, include/su2_ozaki.h): the same
+        plan and operands, executed as sliced exact integer products; the workspace is allocated on first use."""
+        from .binding import heff_apply_i8
+        assert psi.dtype == torch.float64 and psi.is_cuda and psi.is_contiguous() and psi.numel() == self.psi_len
+        if out is None:
+            out = torch.empty(self.psi_len, dtype=torch.float64, device=self.device)
+        if getattr(self, "_i8_views", None) is None:
+            self._i8_views = self.plan.export_task_views()
+        if getattr(self, "_i8_ws", None) is None or self._i8_ws.numel() < workspace_bytes:
+            self._i8_ws = torch.empty(workspace_bytes, dtype=torch.uint8, device=self.device)
+        heff_apply_i8(self._i8_views, psi.data_ptr(), out.data_ptr(), self.psi_len, self._i8_ws.data_ptr(), workspace_bytes,
+                      torch.cuda.current_stream(self.device).cuda_stream, nslices)
+        return out
+
     def apply_host(self, psi_host, out_host):
         """End-to-end entry: pinned host tensors in and out (copies inside the C call)."""
         assert psi_host.dtype == torch.float64 and not psi_host.is_cuda and psi_host.numel() == self.psi_len

@@ -172,3 +172,32 @@ def test_i8_gemm_pair_at_microbenchmark_size_on_sampled_entries():
         want = C0[b, ii, jj] + 0.5 * np.einsum("sk,kn,sn->s", A[b, ii], X[b], B[b, jj])
         worst = max(worst, np.abs(got[b, ii, jj] - want).max())
     assert worst <= TOL * scale, worst
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfg,large_tiles", [("mini", False), ("midi", False), ("midi", True)])
+def test_heff_apply_i8_equals_the_oracle_and_the_fp64_path(cfg, large_tiles):
+    """su2_heff_apply_i8: every task of the plan (adjoint operands, identity sides, folded one-sided rows, alpha arrays,
+    shared and per-position blocks, ragged sectors) on the INT8 tensor path, against the M-resolved oracle (1e-10, the
+    tolerance of the FP64 path) and against su2_heff_apply; bit-reproducible."""
+    torch = _torch()
+    from gen.workloads import config_problem, random_psi
+    from helpers import oracle_flat
+    from paper_2309_16724_b200.runtime import HeffOperator
+    prob = config_problem(cfg)
+    op = HeffOperator(prob, large_tiles=large_tiles)
+    x = random_psi(op.psi_len, seed=3)
+    dx = torch.from_numpy(x).cuda()
+    got = op.apply_i8(dx, workspace_bytes=256 << 20).clone()
+    again = op.apply_i8(dx, workspace_bytes=256 << 20)
+    torch.cuda.synchronize()
+    assert torch.equal(got, again)
+    f_ref = oracle_flat(prob, op.plan, x)
+    scale = np.abs(f_ref).max()
+    assert np.abs(got.cpu().numpy() - f_ref).max() / scale <= TOL
+    f64 = op.apply(dx)
+    assert float((got - f64).abs().max()) / scale <= 1e-11
+    # a workspace that holds only a few positions of a task: chunks over the positions; the per-position terms are the same
+    # and they are added in the same order, so the bits are the same
+    small = op.apply_i8(dx, workspace_bytes=(2 << 20) if cfg == "midi" else (256 << 10))
+    assert torch.equal(small, got)
