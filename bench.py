@@ -462,6 +462,29 @@ def run_gpu(args):
     ka1.record()
     torch.cuda.synchronize()
     apply_ms = ka0.elapsed_time(ka1) / napply
+    # --- the same apply on the INT8 tensor path (su2_heff_apply_i8), on request: reported next to
+    # the FP64 figure, never instead of it
+    int8_path = None
+    if args.int8_apply and mode == "single":
+        from paper_2309_16724_b200.binding import ozaki_launch_count
+        wsb = int(args.int8_workspace_gb * (1 << 30))
+        y8 = local_op.apply_i8(x, workspace_bytes=wsb)          # warm-up (workspace allocation, first launches)
+        torch.cuda.synchronize()
+        diff = float((y8 - y).abs().max() / y.abs().max())
+        n8 = 1 if long_apply else max(1, min(args.steps, 5))
+        li0 = ozaki_launch_count()
+        k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        k0.record()
+        for _ in range(n8):
+            local_op.apply_i8(x, y8, workspace_bytes=wsb)
+        k1.record()
+        torch.cuda.synchronize()
+        ms8 = k0.elapsed_time(k1) / n8
+        int8_path = {"what": "su2_heff_apply_i8: every task of the same plan as sliced exact INT8 products (7 slices), FP64 "
+                             "recombination; FP64-equivalent rate = CC / time", "apply_ms": ms8,
+                     "tflops": cc_local / (ms8 * 1e-3) / 1e12, "speedup_over_fp64_apply": apply_ms / ms8,
+                     "max_diff_over_max_abs_vs_fp64_apply": diff, "gpu_launches_per_apply": (ozaki_launch_count() - li0) // n8,
+                     "workspace_bytes": wsb}
     clocks = sampler.stop() if rank == 0 else None
     # --- end to end through the public API with HOST buffers (pinned): H2D psi, apply (+ all-reduce), D2H F, every step
     xh = psi0.cpu().pin_memory()
@@ -537,6 +560,9 @@ def run_gpu(args):
                      "hbm_achieved_gbs": info["operator_bytes"] / (apply_ms * 1e-3) / 1e9, "hbm_peak_gbs": peaks["hbm_gbs"]},
         "davidson": {"theta": [h[0] for h in hist], "resnorm": [h[1] for h in hist]},
     }
+    if int8_path is not None:
+        int8_path["over_fp64_tensor_peak"] = int8_path["tflops"] / peak
+        line["int8_path"] = int8_path
     if not args.no_cpu_baseline and world == 1:
         cb = time_oracle(args.config, budget_s=20.0)
         line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample", "single_thread", "host_cpus")}
@@ -559,6 +585,9 @@ def main():
     ap.add_argument("--config", default="cfg4")
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--int8-apply", action="store_true",
+                    help="also time H_eff*Psi on the INT8 tensor path (su2_heff_apply_i8) and report it as int8_path")
+    ap.add_argument("--int8-workspace-gb", type=float, default=8.0)
     ap.add_argument("--gang-pacing", action="store_true",
                     help="plan with SU2_PLAN_GANG_PACING (row tiles of a sector paced for L2 reuse: less DRAM traffic, 2-5 %% slower)")
     ap.add_argument("--parallelism", default=None, choices=["shard", "replicas"],
