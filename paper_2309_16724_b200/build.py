@@ -62,7 +62,17 @@ def build_ozaki(force=False):
 
 
 def build(force=False, verbose=False):
-    build_ozaki(force)
+    """All three libraries; libsu2ozaki.so (minutes of template instantiation) compiles next to the other two."""
+    import concurrent.futures
+    with concurrent.futures.ThreadPoolExecutor(max_workers=1) as pool:
+        ozaki = pool.submit(build_ozaki, force)
+        try:
+            return _build_main(force, verbose)
+        finally:
+            ozaki.result()
+
+
+def _build_main(force=False, verbose=False):
     if not force and not _stale():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
