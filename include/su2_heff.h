@@ -164,7 +164,7 @@ typedef struct {
   int32_t small_plan;        /* 1: every block sector holds <= 48 multiplets, su2_heff_apply runs the small-block
                                 kernel (one CTA per output sector and segment); 0: large register tiles
                                 (always 0 under SU2_PLAN_LARGE_TILES) */
-  int32_t reserved;
+  int32_t gang_slots;        /* row tiles that take part in gang pacing (0 without SU2_PLAN_GANG_PACING)            */
   int64_t padded_copy_bytes; /* part of plan_device_bytes: padded copies of families that could not be read in place */
 } su2_plan_info_t;
 

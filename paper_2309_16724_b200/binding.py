@@ -67,7 +67,7 @@ class su2_plan_info_t(C.Structure):
                 ("cc_flops", C.c_double), ("executed_flops", C.c_double), ("operator_bytes", C.c_double),
                 ("workspace_bytes", C.c_int64), ("npsi_sec", C.c_int32), ("nsegments", C.c_int32),
                 ("nwork_items", C.c_int64), ("plan_seconds", C.c_double), ("plan_device_bytes", C.c_int64),
-                ("small_plan", C.c_int32), ("reserved", C.c_int32), ("padded_copy_bytes", C.c_int64)]
+                ("small_plan", C.c_int32), ("gang_slots", C.c_int32), ("padded_copy_bytes", C.c_int64)]
 
 
 EXPORTS = ["su2_wigner_6j", "su2_wigner_9j", "su2_status_string", "su2_last_cuda_error", "su2_kernel_launch_count", "su2_plan_create", "su2_plan_destroy", "su2_plan_info",

@@ -802,6 +802,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
   plan->info.npsi_sec = nsec;
   plan->info.nwork_items = (int64_t)plan->h_work.size();
   plan->info.small_plan = small_plan ? 1 : 0;
+  plan->info.gang_slots = (int32_t)plan->n_gang_slots;
 
   if (!plan->host_only) {
     st = upload_plan(plan, cuda_stream);

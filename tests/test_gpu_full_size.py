@@ -5,6 +5,7 @@
 Coverage, elements checked against the oracle / elements of F:
   configs[1] (cfg2):  85 126 / 85 126        -- the FULL oracle (oracle/heff_dense.py), every element
   configs[2] (cfg3):  64 entries (8 x 8) in EVERY one of the 138 sectors = 8 832 / 1 208 228, sampled oracle
+  cfg4p (cfg4's blocks, 24 positions): 16 entries in 12 sectors; gang pacing bit-equal, INT8 apply within 1e-12
   configs[3] (cfg4):  36 entries (6 x 6) in 40 of the 138 sectors = 1 440 / 19 728 348, sampled oracle; the sectors
                       are stratified over the three tile classes (all of the two rarer classes' extremes, largest /
                       smallest / median of each) and the sampled rows / columns over the first, a middle and the
@@ -104,14 +105,6 @@ def test_cfg3_sampled_parity_every_sector_and_properties():
     assert checked == 138 * 64
     assert worst <= TOL, worst
     _properties(torch, op, f, 11)
-    # SU2_PLAN_GANG_PACING (row tiles of a sector paced by the producer threads for L2 reuse) changes when loads are issued,
-    # never what is computed: same bits, also on a second apply (the pacing slots are reset per launch)
-    from paper_2309_16724_b200.runtime import HeffOperator
-    paced = HeffOperator(prob, device="cuda:0", gang_pacing=True)
-    assert paced.info["nwork_items"] == op.info["nwork_items"]
-    x = torch.from_numpy(random_psi(op.psi_len, seed=11)).cuda()
-    for _ in range(2):
-        assert torch.equal(paced.apply(x), torch.from_numpy(f).cuda())
 
 
 def _cfg4_sector_choice(prob, op, count):
@@ -145,3 +138,28 @@ def test_cfg4_sampled_parity_and_properties():
     assert checked == 40 * 36
     assert worst <= TOL, worst
     _properties(torch, op, f, 21)
+
+
+def test_cfg4p_gang_pacing_and_int8_apply_equal_the_default_apply():
+    """cfg4p = the blocks of BASELINE.json configs[3] (69-547 multiplets) with 24 positions per family (5.8 GB): the plan
+    flag SU2_PLAN_GANG_PACING (1 908 row tiles in gangs here) gives the bits of the default plan, twice in a row; the same
+    plan executed on the INT8 tensor path (su2_heff_apply_i8) agrees with it to 1e-12 of max|F|; sampled entries of the
+    default result against the oracle (the other two inherit that parity)."""
+    from gen.device_ops import device_block_rows, device_fill
+    from paper_2309_16724_b200.runtime import HeffOperator
+    torch, prob, op = _setup("cfg4p")
+    assert op.info["gang_slots"] == 0
+    rows = device_block_rows(prob, op.family_tensors, op.family_layouts)
+    sectors, _ = _cfg4_sector_choice(prob, op, 12)
+    worst, f, checked = _sampled_parity(torch, prob, op, sectors, 4, rows, seed=31)
+    assert checked == 12 * 16 and worst <= TOL, worst
+    x = torch.from_numpy(random_psi(op.psi_len, seed=31)).cuda()
+    want = torch.from_numpy(f).cuda()
+    f8 = op.apply_i8(x, workspace_bytes=4 << 30)
+    assert float((f8 - want).abs().max() / want.abs().max()) <= 1e-12
+    del f8
+    op._i8_ws = None
+    paced = HeffOperator(prob, device="cuda:0", device_fill=device_fill(prob), gang_pacing=True)
+    assert paced.info["gang_slots"] > 1000 and paced.info["nwork_items"] == op.info["nwork_items"]
+    for _ in range(2):
+        assert torch.equal(paced.apply(x), want)
