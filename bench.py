@@ -288,6 +288,44 @@ def reduce_vals(values, device, world, op="max"):
     return [float(v) for v in t.cpu()]
 
 
+def cublas_two_step(torch, A, X, B, Cm, alpha, args):
+    """ms per call of T = A X; C += alpha T B^T as two strided-batched cuBLAS DGEMMs (torch.bmm / baddbmm_): the paper's scheme,
+    timed as a yardstick beside su2_gemm_pair_batched (never on the product path)."""
+    T = torch.empty(A.shape[0], A.shape[1], X.shape[2], dtype=torch.float64, device=A.device)
+    Bt = B.transpose(1, 2)
+
+    def call():
+        torch.bmm(A, X, out=T)
+        Cm.baddbmm_(T, Bt, alpha=alpha)
+    for _ in range(2):
+        call()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        call()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / args.steps
+
+
+def heavy_shapes(cfg, top=12):
+    """The `top` most flop-heavy task shapes (m, k, n, p) of a configuration (cfg5 sweeps them next to the
+    square shapes): flops = positions x min(2mkn + 2mnp, 2knp + 2mkp) summed over the tasks of a host-only plan."""
+    from gen.workloads import config_problem
+    from paper_2309_16724_b200 import Plan
+    prob = config_problem(cfg, fill=False)
+    plan = Plan(prob, host_only=True)
+    t = plan.export_tasks()
+    dims = [(prob.sec_l[lab[0]].dim, prob.sec_r[lab[4]].dim) for lab in plan.labels]
+    acc = {}
+    for o, i, fl, fr in zip(t["out_sec"], t["in_sec"], t["fam_l"], t["fam_r"]):
+        (m, p), (k, n) = dims[o], dims[i]
+        npos = max(prob.fam_l[fl].npos if fl >= 0 else 1, prob.fam_r[fr].npos if fr >= 0 else 1)
+        acc[(m, k, n, p)] = acc.get((m, k, n, p), 0.0) + npos * min(2.0 * m * k * n + 2.0 * m * n * p, 2.0 * k * n * p + 2.0 * m * k * p)
+    total = sum(acc.values())
+    return [(shape, f / total) for shape, f in sorted(acc.items(), key=lambda kv: -kv[1])[:top]]
+
+
 def run_cfg5(args):
     """BASELINE.json configs[4]: strided-batched FP64 GEMM-pair microbenchmark, C_b += alpha A_b X_b B_b^T,
     square shapes 8..512, batch sized to ~1.5 GB of operands, through su2_gemm_pair_batched."""
@@ -317,8 +355,43 @@ def run_cfg5(args):
         ms = e0.elapsed_time(e1) / args.steps
         flops = 4.0 * b ** 3 * batch
         sweep.append({"m=k=n=p": b, "batch": batch, "ms": ms, "tflops": flops / ms / 1e9,
-                      "operand_gbs": 8.0 * 5 * b * b * batch / ms / 1e6})
+                      "operand_gbs": 8.0 * 5 * b * b * batch / ms / 1e6,
+                      # yardstick, not part of the product: the paper's own scheme, two strided-batched vendor DGEMMs with
+                      # T written to memory in between, through torch.bmm / baddbmm (cuBLAS)
+                      "tflops_cublas_two_step": flops / cublas_two_step(torch, A, X, B, Cm, 0.5, args) / 1e9})
         del A, X, B, Cm
+    # the most flop-heavy task shapes of configs[1..3]: FP64 route, the vendor yardstick, and for the
+    # shapes of configs[2..3] the INT8 route
+    from paper_2309_16724_b200.binding import gemm_pair_batched_i8
+    heavy = []
+    hws = torch.empty(2 << 30, dtype=torch.uint8, device="cuda")
+    for cfg in ("cfg2", "cfg3", "cfg4"):
+        for (m, k, n, p), share in heavy_shapes(cfg, args.heavy_shapes):
+            batch = int(max(4, min(100000, 0.75e9 / (8.0 * (m * k + k * n + p * n + m * p)))))
+            A = torch.randn(batch, m, k, dtype=torch.float64, device="cuda", generator=gen)
+            X = torch.randn(batch, k, n, dtype=torch.float64, device="cuda", generator=gen)
+            B = torch.randn(batch, p, n, dtype=torch.float64, device="cuda", generator=gen)
+            Cm = torch.randn(batch, m, p, dtype=torch.float64, device="cuda", generator=gen)
+            flops = (2.0 * m * k * n + 2.0 * m * n * p) * batch
+            row = {"config": cfg, "m,k,n,p": [m, k, n, p], "flop_share_of_config": share, "batch": batch}
+            routes = [("fp64", lambda: gemm_pair_batched(m, k, n, p, batch, 0.5, A.data_ptr(), X.data_ptr(), B.data_ptr(), Cm.data_ptr(), stream))]
+            if cfg != "cfg2":
+                routes.append(("i8", lambda: gemm_pair_batched_i8(m, k, n, p, batch, 0.5, A.data_ptr(), X.data_ptr(), B.data_ptr(),
+                                                                  Cm.data_ptr(), stream, 7, hws.data_ptr(), hws.numel())))
+            for name, call in routes:
+                for _ in range(3):
+                    call()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                for _ in range(args.steps):
+                    call()
+                e1.record()
+                torch.cuda.synchronize()
+                row["tflops_" + name] = flops / (e0.elapsed_time(e1) / args.steps) / 1e9
+            row["tflops_cublas_two_step"] = flops / cublas_two_step(torch, A, X, B, Cm, 0.5, args) / 1e9
+            heavy.append(row)
+            del A, X, B, Cm
+    del hws
     # The same operation on the INT8 tensor path (include/su2_ozaki.h), next to the FP64 tensor route
     # on the same operands; 1024 and 2048 extend BASELINE.json's shape list to where the FP64 ceiling is passed.
     from paper_2309_16724_b200.binding import gemm_pair_batched_i8, ozaki_launch_count, ozaki_workspace_bytes
@@ -371,7 +444,7 @@ def run_cfg5(args):
                       "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                       "config": {"workload": "cfg5: strided-batched GEMM-pair microbenchmark (BASELINE.json configs[4]), square shapes; "
                                              "value = best shape", "l2": "operands 1.5 GB per shape exceed L2"},
-                      "gpu_launches": kernel_launch_count() - l0 + launches_i8, "sweep": sweep,
+                      "gpu_launches": kernel_launch_count() - l0 + launches_i8, "sweep": sweep, "heavy_task_shapes": heavy,
                       "int8_path": {"what": "the same GEMM pair by su2_gemm_pair_batched_i8: 7 INT8 slices of 7 bits, exact "
                                             "tcgen05 kind::i8 products, FP64 recombination (oracle/ozaki.py); tflops = 4 b^3 "
                                             "batch / time, the FP64-equivalent rate; NOT the line's value",
@@ -510,6 +583,19 @@ def run_gpu(args):
     peaks, peak_src = measured_peaks()
     dfma = probe_fp64_peak(0, 20000, 4, stream)
     dmma_hot = probe_fp64_peak(1, 4000, 4, stream)
+    # third yardstick of SURVEY.md 8(d): the vendor DGEMM at 8192^3 (torch.matmul = cuBLAS; not part of the product)
+    ga = torch.randn(8192, 8192, dtype=torch.float64, device=device)
+    gb = torch.randn(8192, 8192, dtype=torch.float64, device=device)
+    gc = torch.empty_like(ga)
+    torch.matmul(ga, gb, out=gc)
+    g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    g0.record()
+    for _ in range(3):
+        torch.matmul(ga, gb, out=gc)
+    g1.record()
+    torch.cuda.synchronize()
+    cublas_dgemm = 3 * 2.0 * 8192.0 ** 3 / (g0.elapsed_time(g1) * 1e-3) / 1e12
+    del ga, gb, gc
     dmma = max(dmma_cold, dmma_hot)
     peak = dmma
     peak_rule = peaks["bf16_tflops"] * FP64_OVER_BF16_NOMINAL
@@ -557,6 +643,7 @@ def run_gpu(args):
                      "instruction_path": "FP64 tensor: mma.sync.m8n8k4.f64 = SASS DMMA.8x8x4; operands staged by cp.async.bulk.tensor (UTMALDG)",
                      "flops": "CC of the plan (useful flops, PAPER.md:229), not executed flops",
                      "apply_ms": apply_ms, "launches_timed": napply, "peak_dfma_loop_measured": dfma,
+                     "cublas_dgemm_8192_measured": cublas_dgemm,
                      "hbm_achieved_gbs": info["operator_bytes"] / (apply_ms * 1e-3) / 1e9, "hbm_peak_gbs": peaks["hbm_gbs"]},
         "davidson": {"theta": [h[0] for h in hist], "resnorm": [h[1] for h in hist]},
     }
@@ -585,6 +672,7 @@ def main():
     ap.add_argument("--config", default="cfg4")
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--heavy-shapes", type=int, default=12, help="cfg5: task shapes per configuration in the non-square sweep")
     ap.add_argument("--int8-apply", action="store_true",
                     help="also time H_eff*Psi on the INT8 tensor path (su2_heff_apply_i8) and report it as int8_path")
     ap.add_argument("--int8-workspace-gb", type=float, default=8.0)
