@@ -347,7 +347,7 @@ class Davidson:
 
 
 def gemm_pair_batched(m, k, n, p, batch, alpha, a_ptr, x_ptr, b_ptr, c_ptr, stream=0, route=0, wpi=0, nbuf=0):
-    """route 0: automatic; 1: small-block kernel; 2: fused large-tile kernel; 3: FP64-FMA tile routine."""
+    """route 0: automatic; 1: small-block kernel; 2: fused large-tile kernel; 3: FP64-FMA tile routine; 4: un-fused two-pass kernel."""
     if route == 0 and wpi == 0 and nbuf == 0:
         check(load().su2_gemm_pair_batched(m, k, n, p, batch, alpha, a_ptr, x_ptr, b_ptr, c_ptr, stream))
     else:

@@ -604,6 +604,28 @@ def test_gemm_pair_batched(m, k, n, p, batch):
     assert _rel(dC.cpu().numpy(), ref) <= 1e-12
 
 
+@pytest.mark.parametrize("m,k,n,p,batch", [(64, 20, 128, 128, 2), (256, 256, 256, 256, 3), (300, 260, 258, 384, 2), (70, 33, 45, 129, 5),
+                                           (131, 577, 99, 250, 2), (1, 1, 1, 1, 3), (65, 21, 129, 2, 4), (512, 512, 512, 512, 2)])
+def test_gemm_pair_two_pass_route(m, k, n, p, batch):
+    """Route 4 (gemm_two_pass.cu): T = A X through a scratch, C += alpha T B^T, both on dgemm_tma_kernel (K-major and N-major
+    right operands, ragged tiles, K tails, odd leading dimensions re-pitched, beta epilogue), against numpy; the automatic
+    route (which picks it for items >= 256) gives the same bits as the explicit one."""
+    torch = _torch()
+    from paper_2309_16724_b200 import gemm_pair_batched
+    rng = np.random.default_rng(m * 1000 + p + 1)
+    A, X = rng.normal(size=(batch, m, k)), rng.normal(size=(batch, k, n))
+    B, C0 = rng.normal(size=(batch, p, n)), rng.normal(size=(batch, m, p))
+    dA, dX, dB, dC = (torch.from_numpy(a).cuda() for a in (A, X, B, C0))
+    st = torch.cuda.current_stream().cuda_stream
+    gemm_pair_batched(m, k, n, p, batch, 0.5, dA.data_ptr(), dX.data_ptr(), dB.data_ptr(), dC.data_ptr(), st, 4)
+    ref = C0 + 0.5 * np.matmul(np.matmul(A, X), np.swapaxes(B, 1, 2))
+    assert _rel(dC.cpu().numpy(), ref) <= 1e-12
+    if min(m, k, n, p) >= 256 and not (k % 2 or n % 2 or p % 2):
+        auto = torch.from_numpy(C0).cuda()
+        gemm_pair_batched(m, k, n, p, batch, 0.5, dA.data_ptr(), dX.data_ptr(), dB.data_ptr(), auto.data_ptr(), st)
+        assert torch.equal(auto, dC)
+
+
 def test_gemm_pair_batched_degenerate_calls():
     """batch == 0 is a no-op that leaves C untouched; non-positive dimensions and null pointers are rejected with
     SU2_ERR_INVALID_ARGUMENT before anything is launched."""
