@@ -194,7 +194,13 @@ su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double al
   const int64_t max_items = (int64_t)1 << 24;
   // automatic choice: items of at least 256 in every extent with 16-byte aligned rows are faster un-fused (512^4: 28.1 against
   // 26.1 TFLOP/s, 256^4: 23.0 against 22.1; below that, and for operands that need re-pitching, the fused kernel wins)
-  if (route == 0 && std::min(std::min(m, k), std::min(n, p)) >= 256 && !padA && !padX && !padB && !(p & 1) && batch <= 65535) route = 4;
+  // -- provided its 64 x 128 tiles fit the two outputs (516^4 pads to 576 x 640: 23.7 against 25.2 fused; 446^4: 26.6 against 20.9)
+  if (route == 0 && std::min(std::min(m, k), std::min(n, p)) >= 256 && !padA && !padX && !padB && !(p & 1) && batch <= 65535) {
+    auto fit = [](int rows, int cols) {
+      return ((double)rows * cols) / ((double)((rows + 63) / 64 * 64) * ((cols + 127) / 128 * 128));
+    };
+    if (fit(m, n) >= 0.8 && fit(m, p) >= 0.8) route = 4;
+  }
   if (route == 4) {
     // un-fused form (gemm_two_pass.cu): T through a scratch, both passes with 32 x 64 warp tiles and two CTAs per SM
     const size_t b_padA = padA ? (((size_t)batch * m * ldA * 8 + 255) & ~(size_t)255) : 0;
