@@ -249,6 +249,7 @@ def run_reference(args):
 
 # ------------------------------------------------------------------------------ GPU arm
 GANG_PACING = False      # --gang-pacing: plan flag SU2_PLAN_GANG_PACING (single-GPU operator)
+TWO_PASS = {}            # --two-pass ...: plan flag SU2_PLAN_TWO_PASS and its options (single-GPU operator)
 
 
 def build_operator(cfg_name, device, shard=False):
@@ -267,7 +268,7 @@ def build_operator(cfg_name, device, shard=False):
         if big:
             from gen.device_ops import device_fill
             fill = device_fill(prob)
-        return prob, HeffOperator(prob, device=device, device_fill=fill, gang_pacing=GANG_PACING)
+        return prob, HeffOperator(prob, device=device, device_fill=fill, gang_pacing=GANG_PACING, **TWO_PASS)
     import torch.distributed as dist
     live = dist.is_available() and dist.is_initialized()
     rank, world = (dist.get_rank(), dist.get_world_size()) if live else (0, 1)
@@ -617,6 +618,8 @@ def run_gpu(args):
                                "small-block configuration, not the headline") % (local_op.operator_bytes_resident / 1e9),
                    "layout": "operator blocks with leading dimensions padded to a multiple of 4 (read in place by bulk-tensor copies)",
                    "gang_pacing": bool(GANG_PACING),
+                   "two_pass": {"tasks": int(info["two_pass_tasks"]), "groups": int(info["two_pass_groups"]),
+                                "scratch_bytes": int(info["two_pass_scratch_bytes"]), "options": TWO_PASS},
                    "small_plan": int(info["small_plan"]),
                    "psi_len": int(info["psi_len"]), "tasks": int(info["ntasks"]),
                    "task_positions": int(info["ntask_positions"]), "cc_flops_per_apply": cc_job,
@@ -678,11 +681,19 @@ def main():
     ap.add_argument("--int8-workspace-gb", type=float, default=8.0)
     ap.add_argument("--gang-pacing", action="store_true",
                     help="plan with SU2_PLAN_GANG_PACING (row tiles of a sector paced for L2 reuse: less DRAM traffic, 2-5 %% slower)")
+    ap.add_argument("--two-pass", action="store_true",
+                    help="plan with SU2_PLAN_TWO_PASS: tasks with all four extents >= --two-pass-min-dim run un-fused through a plan-owned scratch")
+    ap.add_argument("--two-pass-min-dim", type=int, default=0)
+    ap.add_argument("--two-pass-chunk-k", type=int, default=0)
+    ap.add_argument("--two-pass-scratch-gb", type=float, default=0.0)
     ap.add_argument("--parallelism", default=None, choices=["shard", "replicas"],
                     help="N > 1: shard (default; one operator over N GPUs, strong scaling) or replicas (weak)")
     args = ap.parse_args()
     global GANG_PACING
     GANG_PACING = bool(args.gang_pacing)
+    if args.two_pass:
+        TWO_PASS.update(two_pass=True, two_pass_min_dim=args.two_pass_min_dim, two_pass_chunk_k=args.two_pass_chunk_k,
+                        two_pass_scratch_bytes=int(args.two_pass_scratch_gb * 2**30))
     if args.impl == "reference":
         run_reference(args)
         return

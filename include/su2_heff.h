@@ -140,12 +140,30 @@ enum {
   SU2_PLAN_HOST_ONLY = 1,    /* no device tables: planner tests on CPU                          */
   SU2_PLAN_FORCE_SPLIT = 2,  /* tiny segments: exercises the segmented reduction on small inputs */
   SU2_PLAN_LARGE_TILES = 4,  /* keep a small-block bond on the large-tile kernel (tests, A/B measurements) */
-  SU2_PLAN_GANG_PACING = 8   /* large-tile kernel: the row tiles of an output sector, which stream the same right-block
+  SU2_PLAN_GANG_PACING = 8,  /* large-tile kernel: the row tiles of an output sector, which stream the same right-block
                                 operators, keep within two positions of each other, so that L2 serves them to all but
                                 the first (DRAM reads -70 %, L2 hit rate 60 -> 84 % at configs[3]'s blocks); costs 2-5 %
                                 of the time because a row tile on a faster SM waits -- off by default, for callers that
                                 share HBM bandwidth or power with something else.  Same result bit for bit. */
+  SU2_PLAN_TWO_PASS = 16     /* tasks whose four extents m, k, n, p all reach su2_plan_options.two_pass_min_dim leave the fused
+                                kernel and run UN-FUSED, the way the paper executes them (one batched GEMM
+                                per product, the position sum as the inner dimension of the second): pass 1
+                                writes T_pos = coef alpha_pos A_pos E (or E D_pos^T, whichever product order is cheaper -- the
+                                order the paper's CC counts) to a plan-owned scratch, pass 2 contracts it over
+                                (position, inner index) into partial slabs, a fixed-order reduction adds the slabs to F_s.
+                                Both passes run on 64 x 128 tiles, 32 x 64 per warp, two CTAs per SM, which the FP64 tensor
+                                pipe of sm_100a rewards.  Ignored by small-block plans.  Deterministic;
+                                the summation order differs from the fused kernel's, so results agree to rounding, not bit
+                                for bit. */
 };
+
+/* Tuning of SU2_PLAN_TWO_PASS (su2_plan_create_opts; 0 = default for every field). */
+typedef struct {
+  int32_t two_pass_min_dim;        /* smallest extent of a task that takes the two-pass route (default 192)                  */
+  int32_t two_pass_chunk_k;        /* target length of the inner (position, index) loop of one pass-2 CTA (default 8192)      */
+  int64_t two_pass_scratch_bytes;  /* upper bound of the plan-owned scratch for T (default 8 GiB; never less than one
+                                      position of the largest task; su2_plan_info_t.two_pass_scratch_bytes = what was taken) */
+} su2_plan_options;
 
 typedef struct {
   int64_t psi_len;           /* number of doubles in Psi / F                                    */
@@ -166,12 +184,19 @@ typedef struct {
                                 (always 0 under SU2_PLAN_LARGE_TILES) */
   int32_t gang_slots;        /* row tiles that take part in gang pacing (0 without SU2_PLAN_GANG_PACING)            */
   int64_t padded_copy_bytes; /* part of plan_device_bytes: padded copies of families that could not be read in place */
+  int64_t two_pass_tasks;    /* tasks on the two-pass route (0 without SU2_PLAN_TWO_PASS)                              */
+  int64_t two_pass_scratch_bytes;   /* part of plan_device_bytes: the scratch the intermediates T_pos go through       */
+  int32_t two_pass_groups;   /* launch groups of the two-pass route per apply (three launches each)                    */
+  int32_t pad;
 } su2_plan_info_t;
 
 /* Build the plan: enumerate the sector tasks (Eq. (3)), compute the coefficient of each
  * (sector-value-table), sort them by output sector, cut the lists into
  * load-balanced segments and upload the tables on `cuda_stream` (synchronises). */
 su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int32_t flags, void* cuda_stream);
+/* The same with tuning options (HOST, may be NULL = defaults); negative fields: SU2_ERR_INVALID_ARGUMENT. */
+su2_status su2_plan_create_opts(su2_plan** out, const su2_problem* p, int32_t flags, const su2_plan_options* opts,
+                                void* cuda_stream);
 su2_status su2_plan_destroy(su2_plan* plan);
 su2_status su2_plan_info(const su2_plan* plan, su2_plan_info_t* info);
 /* The planner's own 6j / 9j evaluation (Eqs. (10)-(15), :351-384; doubled arguments 0..40), exported so

@@ -67,10 +67,15 @@ class su2_plan_info_t(C.Structure):
                 ("cc_flops", C.c_double), ("executed_flops", C.c_double), ("operator_bytes", C.c_double),
                 ("workspace_bytes", C.c_int64), ("npsi_sec", C.c_int32), ("nsegments", C.c_int32),
                 ("nwork_items", C.c_int64), ("plan_seconds", C.c_double), ("plan_device_bytes", C.c_int64),
-                ("small_plan", C.c_int32), ("gang_slots", C.c_int32), ("padded_copy_bytes", C.c_int64)]
+                ("small_plan", C.c_int32), ("gang_slots", C.c_int32), ("padded_copy_bytes", C.c_int64),
+                ("two_pass_tasks", C.c_int64), ("two_pass_scratch_bytes", C.c_int64), ("two_pass_groups", C.c_int32), ("pad", C.c_int32)]
 
 
-EXPORTS = ["su2_wigner_6j", "su2_wigner_9j", "su2_status_string", "su2_last_cuda_error", "su2_kernel_launch_count", "su2_plan_create", "su2_plan_destroy", "su2_plan_info",
+class su2_plan_options(C.Structure):
+    _fields_ = [("two_pass_min_dim", C.c_int32), ("two_pass_chunk_k", C.c_int32), ("two_pass_scratch_bytes", C.c_int64)]
+
+
+EXPORTS = ["su2_wigner_6j", "su2_wigner_9j", "su2_status_string", "su2_last_cuda_error", "su2_kernel_launch_count", "su2_plan_create", "su2_plan_create_opts", "su2_plan_destroy", "su2_plan_info",
            "su2_plan_psi_layout", "su2_plan_export_tasks", "su2_heff_apply", "su2_heff_apply_host", "su2_heff_diag",
            "su2_davidson_workspace_bytes", "su2_davidson_create", "su2_davidson_create_sharded", "su2_davidson_step", "su2_davidson_set_preconditioner", "su2_davidson_ritz_vector",
            "su2_davidson_destroy", "su2_gemm_pair_batched", "su2_gemm_pair_batched_route", "su2_precontract", "su2_renormalize", "su2_heff_apply_noalloc",
@@ -103,6 +108,7 @@ def load():
     lib.su2_last_cuda_error.restype = C.c_char_p
     lib.su2_kernel_launch_count.restype = C.c_int64
     lib.su2_plan_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(su2_problem), C.c_int32, C.c_void_p]
+    lib.su2_plan_create_opts.argtypes = [C.POINTER(C.c_void_p), C.POINTER(su2_problem), C.c_int32, C.POINTER(su2_plan_options), C.c_void_p]
     lib.su2_plan_destroy.argtypes = [C.c_void_p]
     lib.su2_plan_info.argtypes = [C.c_void_p, C.POINTER(su2_plan_info_t)]
     lib.su2_plan_psi_layout.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
@@ -182,7 +188,7 @@ class Plan:
     without a GPU)."""
 
     def __init__(self, problem, family_ptrs=None, stream=0, host_only=False, force_split=False, large_tiles=False, gang_pacing=False,
-                 ld_align=1):
+                 ld_align=1, two_pass=False, two_pass_min_dim=0, two_pass_chunk_k=0, two_pass_scratch_bytes=0):
         lib = load()
         self._keep = []
         self.problem = problem
@@ -236,8 +242,10 @@ class Plan:
                            len(problem.fam_l), len(problem.fam_r), fl, fr, len(problem.site),
                            None if u1 else site, len(problem.term), terms, 1 if u1 else 0, site if u1 else None)
         self.handle = C.c_void_p()
-        check(lib.su2_plan_create(C.byref(self.handle), C.byref(prob), (SU2_PLAN_HOST_ONLY if host_only else 0) | (2 if force_split else 0) | (4 if large_tiles else 0) | (8 if gang_pacing else 0),
-                                  C.c_void_p(stream)))
+        flags = ((SU2_PLAN_HOST_ONLY if host_only else 0) | (2 if force_split else 0) | (4 if large_tiles else 0) | (8 if gang_pacing else 0) |
+                 (16 if two_pass else 0))
+        opts = su2_plan_options(int(two_pass_min_dim), int(two_pass_chunk_k), int(two_pass_scratch_bytes))
+        check(lib.su2_plan_create_opts(C.byref(self.handle), C.byref(prob), flags, C.byref(opts), C.c_void_p(stream)))
         info = su2_plan_info_t()
         check(lib.su2_plan_info(self.handle, C.byref(info)))
         self.info = {k: getattr(info, k) for k, _ in su2_plan_info_t._fields_}

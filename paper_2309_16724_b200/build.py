@@ -8,7 +8,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
-SOURCES = ["plan.cpp", "tensor_maps.cpp", "kernels.cu", "heff_tma.cu", "heff_small.cu", "davidson.cu", "gemm_pair.cu", "gemm_pair_small.cu", "gemm_two_pass.cu", "precontract.cu", "renorm.cu", "apply_noalloc.cu"]
+SOURCES = ["plan.cpp", "tensor_maps.cpp", "kernels.cu", "heff_tma.cu", "heff_two_pass.cu", "heff_small.cu", "davidson.cu", "gemm_pair.cu", "gemm_pair_small.cu", "gemm_two_pass.cu", "precontract.cu", "renorm.cu", "apply_noalloc.cu"]
 LIB = os.path.join(HERE, "libsu2heff.so")
 PROBE_LIB = os.path.join(HERE, "libsu2probe.so")      # measurement aid of bench.py (include/su2_probe.h), not the product
 OZAKI_LIB = os.path.join(HERE, "libsu2ozaki.so")      # include/su2_ozaki.h: GEMM pair on the INT8 tensor path (row f4)

@@ -1,0 +1,346 @@
+// Two-pass route of H_eff * Psi (row a4 of SURVEY.md section 8; plan flag SU2_PLAN_TWO_PASS): the task
+//     F_s (m x p) += coef sum_pos alpha_pos Aop_pos (m x k) E_s' (k x n) Dop_pos^T (n x p)          (Eq. (3))
+// executed the way the paper does it (a strided-batched GEMM per product, the sum over positions as the
+// inner dimension of the second one -- the "stripe" trick), but with both products on this library's own
+// TMA-fed DMMA.8x8x4 GEMM and the intermediate T in a plan-owned scratch:
+//   pass 1:  T_pos = coef alpha_pos Aop_pos E           for every position of a slice        (order 1: T_pos = coef alpha_pos E Dop_pos^T)
+//   pass 2:  partial[chunk] = sum_{pos in chunk} T_pos Dop_pos^T   (K loop over (pos, n))     (order 1: sum_pos Aop_pos T_pos)
+//   reduce:  F_s += partial slabs in index order (deterministic, no atomics; row a5)
+// Why: on sm_100a what decides DMMA throughput is the register tile of a warp and the number of independent CTAs per SM
+// (profiles/r02_cfg5_shapes.md, r02_two_pass_kernel.md): four warps of 32 x 64, two CTAs per SM reach 90-95 % of the pipe, the
+// fused kernel (heff_tma.cu: both products' accumulators in registers, T chunk in shared memory, one CTA per SM) 79 %.  T costs
+// 16 bytes of HBM traffic per entry against 2 (k + p) flops.
+//
+// One kernel serves both passes (tp_gemm_kernel): D (M x N) = scale * sum_pos L_pos (M x K) R_pos (K x N), CTA tile 64 x 128,
+// k stages of 20 staged by one elected thread with bulk-tensor copies (true extents in the tensor maps: ragged edges and the
+// k tail arrive as zeros), 4 consumer warps (2 x 2).  Ragged last row / column tiles run a narrower instantiation
+// (warp tile 8 NI x 8 NJ) instead of multiplying zeros.
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdint>
+#include <cstdio>
+
+#include "su2_internal.h"
+
+namespace su2 {
+
+namespace {
+
+constexpr int TP_NS = 3;                                   // pipeline stages
+constexpr int TP_CONSUMERS = 4, TP_THREADS = 32 * (TP_CONSUMERS + 1);
+constexpr int TP_LBOX_K = TP_TM * TP_KS;                   // L as stored (rows x k, pitch 20)
+constexpr int TP_LBOX_M = TP_KS * TP_LLD;                  // L read transposed (k x rows, pitch 68)
+constexpr int TP_LREG = TP_LBOX_M > TP_LBOX_K ? TP_LBOX_M : TP_LBOX_K;
+constexpr int TP_RBOX_K = TP_TN * TP_KS;                   // R with k contiguous (columns x k, pitch 20)
+constexpr int TP_RBOX_N = TP_KS * TP_RLD;                  // R with the columns contiguous (k x columns, pitch 132)
+constexpr int TP_RREG = TP_RBOX_N > TP_RBOX_K ? TP_RBOX_N : TP_RBOX_K;
+constexpr int TP_STAGE = TP_LREG + TP_RREG;
+static_assert(TP_LREG % 16 == 0 && TP_STAGE % 16 == 0, "boxes land on 128-byte boundaries");
+constexpr size_t TP_SMEM = (size_t)TP_NS * TP_STAGE * sizeof(double);
+
+__device__ __forceinline__ unsigned tp_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void tp_mbar_init(uint64_t* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(tp_smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void tp_mbar_arrive(uint64_t* bar) {
+  asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"(tp_smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tp_mbar_expect(uint64_t* bar, unsigned bytes) {
+  asm volatile("{\n.reg .b64 st;\nmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n}\n" ::"r"(tp_smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tp_mbar_wait(uint64_t* bar, int parity) {
+  unsigned ok = 0;
+  while (!ok)
+    asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
+                 : "=r"(ok) : "r"(tp_smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tp_tma_box(unsigned dst, const void* map, int c0, int c1, int c2, uint64_t* bar) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];\n"
+               ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(tp_smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tp_dmma(double (&c)[2], double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n" : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
+}
+
+// What one CTA does, decoded from its slice by every thread.
+struct TpItem {
+  const CUtensorMap *mapL, *mapR;
+  int M, N, K;              // extents of the product
+  int row0, col0;           // tile origin
+  int npl;                  // positions summed by this item (pass 1: one)
+  int lt, rn;               // L read transposed; R with the columns contiguous
+  int l_row, l_row_step;    // L row coordinate offset of the first position and its step per position (T as L)
+  int l_item, l_item_step;  // third coordinate of the L boxes
+  int r_k, r_k_step;        // R k-coordinate offset (T as R)
+  int r_item, r_item_step;
+  int ni, nj;               // warp tile: 8 ni rows x 8 nj columns
+  double* dst;
+  int ldd;
+  double scale;
+};
+
+// consumer warp (wr, wc) of a 2 x 2 grid: rows [8 NI wr, +8 NI) x columns [8 NJ wc, +8 NJ) of the CTA tile
+template <int NI, int NJ, bool LT, bool RN>
+__device__ __forceinline__ void tp_consume(const TpItem& it, const double* __restrict__ smem, uint64_t* full, uint64_t* empty, int warp, int lane) {
+  const int wr = warp >> 1, wc = warp & 1;
+  const int g = lane >> 2, t = lane & 3;
+  double acc[NI][NJ][2];
+#pragma unroll
+  for (int i = 0; i < NI; ++i)
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+  constexpr int LI = LT ? 8 : 8 * TP_KS, LS = LT ? 4 * TP_LLD : 4;          // element steps: next m8 tile, next k4 sub-step
+  constexpr int RJ = RN ? 8 : 8 * TP_KS, RS = RN ? 4 * TP_RLD : 4;
+  const int l_off = LT ? t * TP_LLD + wr * 8 * NI + g : (wr * 8 * NI + g) * TP_KS + t;
+  const int r_off = TP_LREG + (RN ? t * TP_RLD + wc * 8 * NJ + g : (wc * 8 * NJ + g) * TP_KS + t);
+  const int nsteps = (it.K + TP_KS - 1) / TP_KS;
+  const int nsub_last = (it.K - (nsteps - 1) * TP_KS + 3) >> 2;            // k4 sub-steps of the last stage that hold data
+  int step = 0;
+  for (int pl = 0; pl < it.npl; ++pl)
+    for (int s = 0; s < nsteps; ++s, ++step) {
+      const int b = step % TP_NS;
+      tp_mbar_wait(&full[b], (step / TP_NS) & 1);
+      const double* __restrict__ st = smem + (size_t)b * TP_STAGE;
+      if (s != nsteps - 1 || nsub_last == TP_KS / 4) {
+        // full stage: straight-line, the fragments of sub-step + 1 are fetched before the DMMAs of this one are issued
+        double af[2][NI], bf[2][NJ];
+#pragma unroll
+        for (int i = 0; i < NI; ++i) af[0][i] = st[l_off + i * LI];
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) bf[0][j] = st[r_off + j * RJ];
+#pragma unroll
+        for (int sub = 0; sub < TP_KS / 4; ++sub) {
+          const int cur = sub & 1, nxt = cur ^ 1;
+          if (sub + 1 < TP_KS / 4) {
+#pragma unroll
+            for (int i = 0; i < NI; ++i) af[nxt][i] = st[l_off + i * LI + (sub + 1) * LS];
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) bf[nxt][j] = st[r_off + j * RJ + (sub + 1) * RS];
+          }
+#pragma unroll
+          for (int j = 0; j < NJ; ++j)
+#pragma unroll
+            for (int i = 0; i < NI; ++i) tp_dmma(acc[i][j], af[cur][i], bf[cur][j]);
+        }
+      } else {
+        // ragged last stage of a position: only the k4 sub-steps that hold data (the rest of the box is zero fill)
+#pragma unroll 1
+        for (int sub = 0; sub < nsub_last; ++sub) {
+          double af[NI], bf[NJ];
+#pragma unroll
+          for (int i = 0; i < NI; ++i) af[i] = st[l_off + i * LI + sub * LS];
+#pragma unroll
+          for (int j = 0; j < NJ; ++j) bf[j] = st[r_off + j * RJ + sub * RS];
+#pragma unroll
+          for (int j = 0; j < NJ; ++j)
+#pragma unroll
+            for (int i = 0; i < NI; ++i) tp_dmma(acc[i][j], af[i], bf[j]);
+        }
+      }
+      __syncwarp();
+      if (lane == 0) tp_mbar_arrive(&empty[b]);
+    }
+  // epilogue: dst = scale * acc (accumulator layout: row g, columns 2t, 2t + 1 of every m8n8 tile), guarded
+  const bool vec = !(it.ldd & 1);
+  const int cbase = it.col0 + wc * 8 * NJ + 2 * t;
+#pragma unroll
+  for (int i = 0; i < NI; ++i) {
+    const int r = it.row0 + wr * 8 * NI + i * 8 + g;
+    if (r >= it.M) continue;
+#pragma unroll
+    for (int j = 0; j < NJ; ++j) {
+      const int c = cbase + j * 8;
+      double* o = it.dst + (int64_t)r * it.ldd + c;
+      const double v0 = it.scale * acc[i][j][0], v1 = it.scale * acc[i][j][1];
+      if (vec && c + 1 < it.N) *(double2*)o = make_double2(v0, v1);
+      else {
+        if (c < it.N) o[0] = v0;
+        if (c + 1 < it.N) o[1] = v1;
+      }
+    }
+  }
+}
+
+template <int NI, bool LT, bool RN>
+__device__ __forceinline__ void tp_consume_nj(const TpItem& it, const double* smem, uint64_t* full, uint64_t* empty, int warp, int lane) {
+  switch (it.nj) {
+    case 1: tp_consume<NI, 1, LT, RN>(it, smem, full, empty, warp, lane); break;
+    case 2: tp_consume<NI, 2, LT, RN>(it, smem, full, empty, warp, lane); break;
+    case 3: tp_consume<NI, 3, LT, RN>(it, smem, full, empty, warp, lane); break;
+    case 4: tp_consume<NI, 4, LT, RN>(it, smem, full, empty, warp, lane); break;
+    case 6: tp_consume<NI, 6, LT, RN>(it, smem, full, empty, warp, lane); break;
+    default: tp_consume<NI, 8, LT, RN>(it, smem, full, empty, warp, lane); break;
+  }
+}
+template <bool LT, bool RN>
+__device__ __forceinline__ void tp_consume_ni(const TpItem& it, const double* smem, uint64_t* full, uint64_t* empty, int warp, int lane) {
+  switch (it.ni) {
+    case 1: tp_consume_nj<1, LT, RN>(it, smem, full, empty, warp, lane); break;
+    case 2: tp_consume_nj<2, LT, RN>(it, smem, full, empty, warp, lane); break;
+    case 3: tp_consume_nj<3, LT, RN>(it, smem, full, empty, warp, lane); break;
+    default: tp_consume_nj<4, LT, RN>(it, smem, full, empty, warp, lane); break;
+  }
+}
+
+// warp-tile heights / widths of a ragged last tile with `rem` valid rows / columns (the instantiated sizes)
+__host__ __device__ __forceinline__ int tp_ni_for(int rem) { return rem >= TP_TM ? 4 : (rem + 15) / 16; }
+__host__ __device__ __forceinline__ int tp_nj_for(int rem) {
+  if (rem >= TP_TN) return 8;
+  const int nj = (rem + 15) / 16;
+  return nj == 5 ? 6 : nj == 7 ? 8 : nj;
+}
+
+// pass = 0: T_pos of every position of the group's slices; pass = 1: the partial slabs.  grid = items of the group.
+__global__ void __launch_bounds__(TP_THREADS, 2)
+tp_gemm_kernel(const TpSlice* __restrict__ slices, int nslices, int pass, const DevTask* __restrict__ tasks,
+               const CUtensorMap* __restrict__ maps, double* __restrict__ scratch, double* __restrict__ partial) {
+  extern __shared__ __align__(1024) double smem[];
+  __shared__ __align__(8) uint64_t full[TP_NS];
+  __shared__ __align__(8) uint64_t empty[TP_NS];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  if (tid == 0) {
+    for (int i = 0; i < TP_NS; ++i) {
+      tp_mbar_init(&full[i], 1);
+      tp_mbar_init(&empty[i], TP_CONSUMERS);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  // ---- which slice, which item of it (binary search over the slices' first items)
+  const int item = blockIdx.x;
+  int lo = 0, hi = nslices - 1;
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if ((pass ? slices[mid].item2 : slices[mid].item1) <= item) lo = mid; else hi = mid - 1;
+  }
+  const TpSlice sl = slices[lo];
+  const DevTask* __restrict__ tk = tasks + sl.task;
+  const int m = tk->m, k = tk->k, n = tk->n, p = tk->p;
+  const bool transA = tk->flags & TASK_TRANS_A, transD = tk->flags & TASK_TRANS_D;
+  const int stepA = tk->strideA != 0, stepD = tk->strideD != 0;
+  const int local = item - (pass ? sl.item2 : sl.item1);
+  TpItem it;
+  int pl0;   // first position (relative to the slice) of the item
+  if (pass == 0) {
+    it.M = sl.order ? k : m;
+    it.N = sl.order ? p : n;
+    it.K = sl.order ? n : k;
+  } else {
+    it.M = m; it.N = p;
+    it.K = sl.order ? k : n;
+  }
+  const int ntr = (it.M + TP_TM - 1) / TP_TM, ntc = (it.N + TP_TN - 1) / TP_TN;
+  const int tile = local % (ntr * ntc), outer = local / (ntr * ntc);
+  it.row0 = (tile / ntc) * TP_TM;
+  it.col0 = (tile % ntc) * TP_TN;
+  it.ni = tp_ni_for(it.M - it.row0);
+  it.nj = tp_nj_for(it.N - it.col0);
+  it.l_row = it.l_row_step = it.l_item = it.l_item_step = it.r_k = it.r_k_step = it.r_item = it.r_item_step = 0;
+  const int rowsT = sl.order ? k : m;          // rows of one T_pos
+  if (pass == 0) {
+    pl0 = outer;
+    it.npl = 1;
+    const double al = tk->alpha ? tk->alpha[sl.pos0 + pl0] : 1.0;
+    it.scale = tk->coef * al;
+    it.dst = scratch + ((int64_t)sl.t_row0 + (int64_t)pl0 * rowsT) * sl.ldt;
+    it.ldd = sl.ldt;
+    if (sl.order == 0) {   // T = Aop E
+      it.mapL = maps + sl.mapA; it.lt = transA; it.l_item = stepA ? sl.pos0 + pl0 : 0;
+      it.mapR = maps + sl.mapE; it.rn = 1;
+    } else {               // T = E Dop^T
+      it.mapL = maps + sl.mapE; it.lt = 0;
+      it.mapR = maps + sl.mapD; it.rn = transD; it.r_item = stepD ? sl.pos0 + pl0 : 0;
+    }
+  } else {
+    pl0 = outer * sl.chunk;
+    it.npl = min(sl.chunk, sl.npos - pl0);
+    it.scale = 1.0;
+    const int64_t slab = ((int64_t)m * p + 1) & ~(int64_t)1;
+    it.dst = partial + sl.part_off + (int64_t)outer * slab;
+    it.ldd = p;
+    if (sl.order == 0) {   // partial = sum_pos T_pos Dop_pos^T
+      it.mapL = maps + sl.mapT; it.lt = 0; it.l_row = sl.t_row0 + pl0 * rowsT; it.l_row_step = rowsT;
+      it.mapR = maps + sl.mapD; it.rn = transD; it.r_item = stepD ? sl.pos0 + pl0 : 0; it.r_item_step = stepD;
+    } else {               // partial = sum_pos Aop_pos T_pos
+      it.mapL = maps + sl.mapA; it.lt = transA; it.l_item = stepA ? sl.pos0 + pl0 : 0; it.l_item_step = stepA;
+      it.mapR = maps + sl.mapT; it.rn = 1; it.r_k = sl.t_row0 + pl0 * rowsT; it.r_k_step = rowsT;
+    }
+  }
+  __syncthreads();
+  if (warp == TP_CONSUMERS) {
+    // ---- producer: one thread, two boxes per stage
+    if (lane != 0) return;
+    const unsigned bytes = (unsigned)(((it.lt ? TP_LBOX_M : TP_LBOX_K) + (it.rn ? TP_RBOX_N : TP_RBOX_K)) * sizeof(double));
+    const int nsteps = (it.K + TP_KS - 1) / TP_KS;
+    int step = 0;
+    for (int pl = 0; pl < it.npl; ++pl) {
+      const int lrow = it.row0 + it.l_row + pl * it.l_row_step, litem = it.l_item + pl * it.l_item_step;
+      const int rk = it.r_k + pl * it.r_k_step, ritem = it.r_item + pl * it.r_item_step;
+      for (int s = 0; s < nsteps; ++s, ++step) {
+        const int b = step % TP_NS, round = step / TP_NS;
+        if (round > 0) tp_mbar_wait(&empty[b], (round - 1) & 1);
+        tp_mbar_expect(&full[b], bytes);
+        const unsigned st = tp_smem_u32(smem + (size_t)b * TP_STAGE);
+        if (it.lt) tp_tma_box(st, it.mapL, lrow, s * TP_KS, litem, &full[b]);
+        else tp_tma_box(st, it.mapL, s * TP_KS, lrow, litem, &full[b]);
+        if (it.rn) tp_tma_box(st + TP_LREG * 8u, it.mapR, it.col0, rk + s * TP_KS, ritem, &full[b]);
+        else tp_tma_box(st + TP_LREG * 8u, it.mapR, s * TP_KS, it.col0, ritem, &full[b]);
+      }
+    }
+    return;
+  }
+  if (it.lt) tp_consume_ni<true, true>(it, smem, full, empty, warp, lane);     // Aop read transposed: R is E or T (columns contiguous)
+  else if (it.rn) tp_consume_ni<false, true>(it, smem, full, empty, warp, lane);
+  else tp_consume_ni<false, false>(it, smem, full, empty, warp, lane);
+}
+
+// F_s += partial slabs in index order: fixed order, one thread per element (row a5).
+__global__ void __launch_bounds__(256)
+tp_reduce_kernel(const TpReduce* __restrict__ red, const double* __restrict__ partial, double* __restrict__ out) {
+  const TpReduce r = red[blockIdx.y];
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < r.size; i += (int64_t)gridDim.x * blockDim.x) {
+    double s = out[r.f_off + i];
+    for (int g = 0; g < r.nslab; ++g) s += partial[r.part_off + (int64_t)g * r.slab + i];
+    out[r.f_off + i] = s;
+  }
+}
+
+}  // namespace
+
+int tp_tile_rows_executed(int M) {   // rows the row tiles of an M-row output multiply (host: executed flops)
+  const int full = M / TP_TM, rem = M % TP_TM;
+  return full * TP_TM + (rem ? 16 * tp_ni_for(rem) : 0);
+}
+int tp_tile_cols_executed(int N) {
+  const int full = N / TP_TN, rem = N % TP_TN;
+  return full * TP_TN + (rem ? 16 * tp_nj_for(rem) : 0);
+}
+
+su2_status launch_heff_two_pass(const su2_plan* plan, double* out, double* tp_partial, void* stream_v) {
+  cudaStream_t stream = (cudaStream_t)stream_v;
+  if (plan->h_tp_groups.empty()) return SU2_OK;
+  static bool attr_done[64] = {};
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (!attr_done[dev & 63]) {
+    cudaError_t e = cudaFuncSetAttribute(tp_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TP_SMEM);
+    if (e != cudaSuccess) { set_cuda_error("cudaFuncSetAttribute(tp_gemm_kernel)", (int)e); return SU2_ERR_CUDA; }
+    attr_done[dev & 63] = true;
+  }
+  for (const TpGroup& g : plan->h_tp_groups) {
+    const int ns = g.slice1 - g.slice0;
+    tp_gemm_kernel<<<g.items1, TP_THREADS, TP_SMEM, stream>>>(plan->d_tp_slices + g.slice0, ns, 0, plan->d_tasks, (const CUtensorMap*)plan->d_maps,
+                                                             plan->d_tp_scratch, tp_partial);
+    tp_gemm_kernel<<<g.items2, TP_THREADS, TP_SMEM, stream>>>(plan->d_tp_slices + g.slice0, ns, 1, plan->d_tasks, (const CUtensorMap*)plan->d_maps,
+                                                             plan->d_tp_scratch, tp_partial);
+    dim3 grid(64, (unsigned)(g.red1 - g.red0));
+    tp_reduce_kernel<<<grid, 256, 0, stream>>>(plan->d_tp_reduce + g.red0, tp_partial, out);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { set_cuda_error("two-pass launch", (int)e); return SU2_ERR_CUDA; }
+    count_launch(3);
+  }
+  return SU2_OK;
+}
+
+}  // namespace su2

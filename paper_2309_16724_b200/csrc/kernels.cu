@@ -152,6 +152,11 @@ su2_status upload_plan(su2_plan* plan, void* stream_v) {
                       "padded copies of operator families whose rows are not 16-byte aligned (pass blk_ld with even "
                       "leading dimensions to have them read in place)")) != SU2_OK) return st;
   if ((st = big_alloc(&plan->d_psi_pad, plan->psipad_elems, "the padded copy of Psi")) != SU2_OK) return st;
+  if ((st = big_alloc(&plan->d_tp_scratch, plan->tp_scratch_elems,
+                      "the scratch of the two-pass route (su2_plan_options.two_pass_scratch_bytes)")) != SU2_OK) return st;
+  // a ragged k tail of T read as the right operand reaches into the rows of the next position: whatever is there is
+  // multiplied by exact zeros, so it only has to be finite -- zero once (later contents are finite products)
+  if (plan->d_tp_scratch) SU2_CUDA(cudaMemsetAsync(plan->d_tp_scratch, 0, (size_t)plan->tp_scratch_elems * sizeof(double), stream));
 
   // ---- resolve operand pointers; tensor maps of the large-tile kernel ------------------------------
   std::vector<unsigned char> h_maps;       // 128-byte records
@@ -179,9 +184,12 @@ su2_status upload_plan(su2_plan* plan, void* stream_v) {
   const size_t b_ident = align256(plan->h_ident.size() * sizeof(double));
   // the identity blocks must exist before their tensor maps are encoded: allocate the blob first (maps are
   // appended to it in a second allocation-free step: their count is bounded by 3 per task)
-  const size_t b_maps = align256(large ? (3 * plan->h_tasks.size() + 1) * 128 : 0);
+  // (+ the two-pass route: at most 4 per slice)
+  const size_t b_maps = align256(large ? (3 * plan->h_tasks.size() + 4 * plan->h_tp_slices.size() + 1) * 128 : 0);
+  const size_t b_tps = align256(plan->h_tp_slices.size() * sizeof(TpSlice));
+  const size_t b_tpr = align256(plan->h_tp_reduce.size() * sizeof(TpReduce));
   const size_t b_gang = align256((size_t)plan->n_gang_slots * sizeof(int32_t));
-  const size_t total = b_tasks + b_units + b_work + b_red + b_diag + b_dbeg + b_psi + b_pad + b_alpha + b_ident + b_maps + b_gang + 256;
+  const size_t total = b_tasks + b_units + b_work + b_red + b_diag + b_dbeg + b_psi + b_pad + b_alpha + b_ident + b_maps + b_gang + b_tps + b_tpr + 256;
   SU2_CUDA(cudaMalloc(&plan->d_blob, total));
   plan->info.plan_device_bytes += (int64_t)total;
   char* base = (char*)plan->d_blob;
@@ -200,6 +208,8 @@ su2_status upload_plan(su2_plan* plan, void* stream_v) {
   plan->d_identity = (double*)carve(b_ident);
   plan->d_counter = (int32_t*)carve(256);
   plan->d_gang = b_gang ? (int32_t*)carve(b_gang) : nullptr;
+  plan->d_tp_slices = (TpSlice*)carve(b_tps);
+  plan->d_tp_reduce = (TpReduce*)carve(b_tpr);
 
   auto resolve = [&](const OperandRef& r) -> const double* {
     switch (r.kind) {
@@ -216,7 +226,7 @@ su2_status upload_plan(su2_plan* plan, void* stream_v) {
     t.D = resolve(rd);
     if (!t.A || !t.D) return SU2_ERR_INVALID_ARGUMENT;   // family without device data
     if (plan->h_alpha_off[i] >= 0) t.alpha = plan->d_alpha + plan->h_alpha_off[i];
-    if (!large) continue;
+    if (!large || plan->tasks[i].two_pass) continue;
     const int wr = plan->tasks[i].wr;
     const int tm = 32 * wr;
     MapKey ka{t.A, ra.rows, ra.cols, ra.ld, ra.npos, (int64_t)ra.rows * ra.ld,
@@ -227,6 +237,28 @@ su2_status upload_plan(su2_plan* plan, void* stream_v) {
     MapKey ke{plan->d_psi_pad + pj.dst_off, pj.rows, pj.cols, pj.ld_dst, 1, (int64_t)pj.rows * pj.ld_dst, EBOX_LD, KS1};
     if ((st = map_for(ka, &t.mapA)) != SU2_OK || (st = map_for(kd, &t.mapD)) != SU2_OK || (st = map_for(ke, &t.mapE)) != SU2_OK) return st;
     t.e_item = 0;
+  }
+  // two-pass route: tensor maps with the boxes of tp_gemm_kernel (heff_two_pass.cu)
+  for (TpSlice& sl : plan->h_tp_slices) {
+    const DevTask& t = plan->h_tasks[sl.task];
+    const OperandRef &ra = plan->h_opA[sl.task], &rd = plan->h_opD[sl.task];
+    const bool ta = t.flags & TASK_TRANS_A, td = t.flags & TASK_TRANS_D;
+    // Aop is always the left operand: as stored (rows x k boxes) or read transposed (k x rows boxes)
+    MapKey ka{t.A, ra.rows, ra.cols, ra.ld, ra.npos, (int64_t)ra.rows * ra.ld, ta ? TP_LLD : TP_KS, ta ? TP_KS : TP_TM};
+    // Dop^T is always the right operand: D stored p x n has the inner index contiguous, stored n x p the columns
+    MapKey kd{t.D, rd.rows, rd.cols, rd.ld, rd.npos, (int64_t)rd.rows * rd.ld, td ? TP_RLD : TP_KS, td ? TP_KS : TP_TN};
+    // E (k x n): right operand of A E (columns contiguous), left operand of E D^T (as stored)
+    const PsiPadJob& pj = plan->h_psipad[plan->tasks[sl.task].in_sec];
+    MapKey ke{plan->d_psi_pad + pj.dst_off, pj.rows, pj.cols, pj.ld_dst, 1, (int64_t)pj.rows * pj.ld_dst, sl.order ? TP_KS : TP_RLD,
+              sl.order ? TP_TM : TP_KS};
+    // T: the scratch as one matrix of rows of ldt doubles, colsT of them valid; left operand of T D^T, right operand of A T
+    const int colsT = sl.order ? t.p : t.n;
+    const int64_t rows_all = plan->tp_scratch_elems / sl.ldt;
+    if (rows_all > 0x7fffffff) { set_error_text("two-pass scratch too large for 32-bit row coordinates"); return SU2_ERR_INVALID_ARGUMENT; }
+    MapKey kt{plan->d_tp_scratch, (int32_t)rows_all, colsT, sl.ldt, 1, rows_all * sl.ldt, sl.order ? TP_RLD : TP_KS, sl.order ? TP_KS : TP_TM};
+    if ((st = map_for(ka, &sl.mapA)) != SU2_OK || (st = map_for(kd, &sl.mapD)) != SU2_OK || (st = map_for(ke, &sl.mapE)) != SU2_OK ||
+        (st = map_for(kt, &sl.mapT)) != SU2_OK)
+      return st;
   }
   plan->nmaps = (int32_t)map_index.size();
   for (auto& d : plan->h_diag) {
@@ -248,6 +280,8 @@ su2_status upload_plan(su2_plan* plan, void* stream_v) {
   SU2_CUDA(up(plan->d_psipad, plan->h_psipad.data(), plan->h_psipad.size() * sizeof(PsiPadJob)));
   SU2_CUDA(up(plan->d_alpha, plan->h_alpha.data(), plan->h_alpha.size() * sizeof(double)));
   SU2_CUDA(up(plan->d_identity, plan->h_ident.data(), plan->h_ident.size() * sizeof(double)));
+  SU2_CUDA(up(plan->d_tp_slices, plan->h_tp_slices.data(), plan->h_tp_slices.size() * sizeof(TpSlice)));
+  SU2_CUDA(up(plan->d_tp_reduce, plan->h_tp_reduce.data(), plan->h_tp_reduce.size() * sizeof(TpReduce)));
   DeviceFree d_fjobs, d_cjobs;
   if (plan->fold_elems > 0) {
     for (const FoldJob& j : plan->h_fold)
@@ -278,7 +312,7 @@ su2_status upload_plan(su2_plan* plan, void* stream_v) {
 
 void free_plan_device(su2_plan* plan) {
   if (!plan) return;
-  for (void** q : {(void**)&plan->d_blob, (void**)&plan->d_fold, (void**)&plan->d_copy, (void**)&plan->d_psi_pad})
+  for (void** q : {(void**)&plan->d_blob, (void**)&plan->d_fold, (void**)&plan->d_copy, (void**)&plan->d_psi_pad, (void**)&plan->d_tp_scratch})
     if (*q) { cudaFree(*q); *q = nullptr; }
 }
 
@@ -307,6 +341,11 @@ su2_status launch_apply(const su2_plan* plan, const double* psi, double* out, do
     SU2_CUDA(cudaGetLastError());
     count_launch();
   }
+  // tasks on the two-pass route add their share to `out` (partial slabs behind the fused kernel's partial tiles)
+  if (!plan->h_tp_groups.empty()) {
+    double* tp_partial = (double*)((char*)partial + align256((size_t)plan->partial_elems * 8 + 256));
+    if ((st = launch_heff_two_pass(plan, out, tp_partial, stream_v)) != SU2_OK) return st;
+  }
   return SU2_OK;
 }
 
@@ -332,7 +371,7 @@ extern "C" su2_status su2_heff_apply(const su2_plan* plan, const double* psi_dev
                                      void* cuda_stream) {
   if (!plan || !psi_dev || !out_dev || psi_dev == out_dev) return SU2_ERR_INVALID_ARGUMENT;
   if (plan->host_only) return SU2_ERR_NO_DEVICE_PLAN;
-  if (plan->partial_elems > 0 && !workspace_dev) return SU2_ERR_WORKSPACE;
+  if ((plan->partial_elems > 0 || plan->tp_partial_elems > 0) && !workspace_dev) return SU2_ERR_WORKSPACE;
   return launch_apply(plan, psi_dev, out_dev, (double*)workspace_dev, cuda_stream);
 }
 

@@ -200,10 +200,21 @@ static su2_status validate(const su2_problem* p) {
 }
 
 extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int32_t flags, void* cuda_stream) {
+  return su2_plan_create_opts(out, p, flags, nullptr, cuda_stream);
+}
+
+extern "C" su2_status su2_plan_create_opts(su2_plan** out, const su2_problem* p, int32_t flags, const su2_plan_options* opts,
+                                           void* cuda_stream) {
   if (!out) return SU2_ERR_INVALID_ARGUMENT;
   *out = nullptr;
   su2_status st = validate(p);
   if (st != SU2_OK) return st;
+  su2_plan_options opt{};
+  if (opts) opt = *opts;
+  if (opt.two_pass_min_dim < 0 || opt.two_pass_scratch_bytes < 0 || opt.two_pass_chunk_k < 0) return SU2_ERR_INVALID_ARGUMENT;
+  if (opt.two_pass_min_dim == 0) opt.two_pass_min_dim = 192;
+  if (opt.two_pass_scratch_bytes == 0) opt.two_pass_scratch_bytes = (int64_t)8 << 30;
+  if (opt.two_pass_chunk_k == 0) opt.two_pass_chunk_k = 8192;
   const auto t_start = std::chrono::steady_clock::now();
 
   su2_plan* plan = new su2_plan();
@@ -577,6 +588,13 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
     ntp += ht.npos;
   }
 
+  // ---- two-pass route (heff_two_pass.cu) --------------------------------------------------------
+  // Tasks whose four extents all reach two_pass_min_dim leave the fused kernel: their intermediate T goes through a
+  // plan-owned scratch and both products run as plain GEMMs with 32 x 64 register tiles per warp, two CTAs per SM.
+  const bool two_pass_on = (flags & SU2_PLAN_TWO_PASS) != 0 && !small_plan;
+  for (HostTask& ht : plan->tasks)
+    ht.two_pass = two_pass_on && std::min(std::min(ht.m, ht.k), std::min(ht.n, ht.p)) >= opt.two_pass_min_dim ? 1 : 0;
+
   // ---- tile class per output sector, segments, work items ---------------------------------
   // Every output sector gets the tile class (TileCfg<WR>, tile_config.h) with the lowest modelled
   // cost.  Its task list (plan order) is cut into nseg segments of equal cost; each (segment, tile)
@@ -584,7 +602,11 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
   // copies that the reduce pass sums in index order: deterministic, no atomics (row a5).
   const int nsec = (int)plan->psi.size();
   std::vector<int64_t> first_task(nsec + 1, 0);
-  for (const HostTask& ht : plan->tasks) first_task[ht.out_sec + 1]++;
+  std::vector<int64_t> nfused(nsec, 0);           // tasks of the sector that run on the fused kernel
+  for (const HostTask& ht : plan->tasks) {
+    first_task[ht.out_sec + 1]++;
+    if (!ht.two_pass) nfused[ht.out_sec]++;
+  }
   for (int s = 0; s < nsec; ++s) first_task[s + 1] += first_task[s];
   // cost of one position of task ht summed over all tiles of its output sector
   auto pos_cost_all_tiles = [&](int wr, const HostTask& ht) {
@@ -599,12 +621,13 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
   std::vector<double> sec_cost(nsec, 0.0);        // summed over tiles
   double total_cost = 0.0;
   for (int s = 0; s < nsec; ++s) {
-    if (first_task[s + 1] == first_task[s]) continue;
+    if (nfused[s] == 0) continue;
     double best = -1.0;
     for (int wr : {1, 2, 4}) {
       if (small_plan && wr != 4) continue;   // cost unit of a small plan: the 128 x 144 class (one tile per sector)
       double c = 0.0;
-      for (int64_t i = first_task[s]; i < first_task[s + 1]; ++i) c += pos_cost_all_tiles(wr, plan->tasks[i]) * plan->tasks[i].npos;
+      for (int64_t i = first_task[s]; i < first_task[s + 1]; ++i)
+        if (!plan->tasks[i].two_pass) c += pos_cost_all_tiles(wr, plan->tasks[i]) * plan->tasks[i].npos;
       if (best < 0.0 || c < best * 0.97) {   // prefer the smaller tile unless the larger one is clearly cheaper
         if (best < 0.0 || c < best) { best = c; sec_wr[s] = wr; }
       }
@@ -620,6 +643,14 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
   // sm__ops_path_tensor_src_fp64 up to the DMMAs of the predicated ragged-edge code paths
   double executed = 0.0;
   for (const HostTask& ht : plan->tasks) {
+    if (ht.two_pass) {   // tp_gemm_kernel: 64 x 128 tiles with narrower ragged tiles, k padded to 4, the cheaper order
+      const bool o1 = 2.0 * ht.m * ht.k * ht.n + 2.0 * ht.m * ht.n * ht.p > 2.0 * ht.k * ht.n * ht.p + 2.0 * ht.m * ht.k * ht.p;
+      const double M1 = o1 ? ht.k : ht.m, N1 = o1 ? ht.p : ht.n, K1 = o1 ? ht.n : ht.k, K2 = o1 ? ht.k : ht.n;
+      auto k4 = [](double x) { return std::ceil(x / 4.0) * 4.0; };
+      executed += ht.npos * 2.0 * ((double)tp_tile_rows_executed((int)M1) * tp_tile_cols_executed((int)N1) * k4(K1) +
+                                   (double)tp_tile_rows_executed(ht.m) * tp_tile_cols_executed(ht.p) * k4(K2));
+      continue;
+    }
     if (small_plan) {   // heff_small_kernel: m8n8k4 tiles over (m8, k4, n8) and (m8, n8, p8)
       const double m8 = (ht.m + 7) & ~7, k4 = (ht.k + 3) & ~3, n8 = (ht.n + 7) & ~7, p8 = (ht.p + 7) & ~7;
       executed += ht.npos * 2.0 * (m8 * k4 * n8 + m8 * n8 * p8);
@@ -640,7 +671,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
     const int64_t t0 = first_task[s], t1 = first_task[s + 1];
     DevReduce red{};
     red.f_off = ps.off; red.size = sz; red.part_off = 0; red.nseg = 0;
-    if (t1 == t0) {
+    if (nfused[s] == 0) {   // nothing from the fused kernel: zero fill (the two-pass route adds to it)
       plan->h_reduce.push_back(red);
       continue;
     }
@@ -654,7 +685,8 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
       return step_cost + tile_pos_cost(wr, std::min(ts.tm, ht.m), std::min(ts.tp, ht.p), ht.k, ht.n);
     };
     double tile_work = 0.0;
-    for (int64_t i = t0; i < t1; ++i) tile_work += pos_cost(plan->tasks[i]) * plan->tasks[i].npos;
+    for (int64_t i = t0; i < t1; ++i)
+      if (!plan->tasks[i].two_pass) tile_work += pos_cost(plan->tasks[i]) * plan->tasks[i].npos;
     int nseg = (int)std::min<double>(64.0, std::max(1.0, std::ceil(tile_work / target)));
     (void)ntiles;
     std::vector<std::pair<int32_t, int32_t>> seg_units;   // unit ranges per segment
@@ -664,6 +696,7 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
       int32_t ustart = (int32_t)plan->h_units.size();
       for (int64_t i = t0; i < t1; ++i) {
         const HostTask& ht = plan->tasks[i];
+        if (ht.two_pass) continue;
         const double c = pos_cost(ht);
         int pos = 0;
         while (pos < ht.npos) {
@@ -774,6 +807,85 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
     plan->h_work.swap(sorted);
   }
 
+  // ---- two-pass route: slices, groups, partial slabs -----------------------------------------------------
+  // Tasks in plan order (sorted by output sector).  A task's positions are cut where the scratch of the current group is
+  // full; a group is one launch per pass.  Pass-2 items sum `chunk` positions each (a K loop of about two_pass_chunk_k)
+  // into a partial slab; consecutive slabs of one output sector inside a group form one reduce record.
+  if (two_pass_on) {
+    double need = 0.0;
+    int64_t min_need = 0;
+    for (const HostTask& ht : plan->tasks) {
+      if (!ht.two_pass) continue;
+      const bool o1 = 2.0 * ht.m * ht.k * ht.n + 2.0 * ht.m * ht.n * ht.p > 2.0 * ht.k * ht.n * ht.p + 2.0 * ht.m * ht.k * ht.p;
+      const int64_t per_pos = (int64_t)(o1 ? ht.k : ht.m) * pad4(o1 ? ht.p : ht.n);
+      need += (double)per_pos * ht.npos + 2.0 * pad4(o1 ? ht.p : ht.n);
+      min_need = std::max(min_need, per_pos + 2 * (int64_t)pad4(o1 ? ht.p : ht.n));
+    }
+    int64_t cap = std::max<int64_t>(opt.two_pass_scratch_bytes / 8, min_need);
+    if (need < (double)cap) cap = std::max<int64_t>((int64_t)need, min_need);
+    plan->tp_scratch_elems = need > 0.0 ? cap : 0;
+    int64_t cur = 0, part_cur = 0, items1 = 0, items2 = 0;
+    TpGroup grp{};
+    auto close_group = [&]() {
+      grp.slice1 = (int32_t)plan->h_tp_slices.size();
+      grp.red1 = (int32_t)plan->h_tp_reduce.size();
+      grp.items1 = (int32_t)items1; grp.items2 = (int32_t)items2;
+      if (grp.slice1 > grp.slice0) plan->h_tp_groups.push_back(grp);
+      plan->tp_partial_elems = std::max(plan->tp_partial_elems, part_cur);
+      grp.slice0 = grp.slice1; grp.red0 = grp.red1;
+      cur = 0; part_cur = 0; items1 = 0; items2 = 0;
+    };
+    int last_sec = -1;
+    for (int64_t i = 0; i < ntask; ++i) {
+      const HostTask& ht = plan->tasks[i];
+      if (!ht.two_pass) continue;
+      const bool o1 = 2.0 * ht.m * ht.k * ht.n + 2.0 * ht.m * ht.n * ht.p > 2.0 * ht.k * ht.n * ht.p + 2.0 * ht.m * ht.k * ht.p;
+      const int rowsT = o1 ? ht.k : ht.m, colsT = o1 ? ht.p : ht.n, ldt = pad4(colsT), K2 = o1 ? ht.k : ht.n;
+      const int64_t per_pos = (int64_t)rowsT * ldt;
+      const int64_t tiles1 = (int64_t)((rowsT + TP_TM - 1) / TP_TM) * ((colsT + TP_TN - 1) / TP_TN);
+      const int64_t tiles2 = (int64_t)((ht.m + TP_TM - 1) / TP_TM) * ((ht.p + TP_TN - 1) / TP_TN);
+      const int64_t slab = ((int64_t)ht.m * ht.p + 1) & ~(int64_t)1;
+      int pos = 0;
+      while (pos < ht.npos) {
+        int64_t start = (cur + ldt - 1) / ldt * ldt;
+        int64_t fit = (plan->tp_scratch_elems - start) / per_pos;
+        if (start > plan->tp_scratch_elems) fit = 0;
+        // a group's launches hold at most 2^30 items and its partial area at most 2^40 elements: never reached in practice
+        if (fit <= 0 || items1 > ((int64_t)1 << 30)) {
+          close_group();
+          last_sec = -1;
+          continue;
+        }
+        const int take = (int)std::min<int64_t>(ht.npos - pos, fit);
+        TpSlice sl{};
+        sl.task = (int32_t)i; sl.pos0 = pos; sl.npos = take; sl.order = o1 ? 1 : 0;
+        sl.t_row0 = (int32_t)(start / ldt); sl.ldt = ldt;
+        sl.mapA = sl.mapD = sl.mapE = sl.mapT = -1;
+        int chunk = std::max(1, (int)std::lround((double)opt.two_pass_chunk_k / K2));
+        const int nchunk = (take + chunk - 1) / chunk;
+        chunk = (take + nchunk - 1) / nchunk;
+        sl.chunk = chunk; sl.nchunk = (take + chunk - 1) / chunk;
+        sl.item1 = (int32_t)items1; sl.item2 = (int32_t)items2;
+        sl.part_off = part_cur;
+        items1 += tiles1 * take;
+        items2 += tiles2 * sl.nchunk;
+        if (last_sec == ht.out_sec) {
+          plan->h_tp_reduce.back().nslab += sl.nchunk;
+        } else {
+          TpReduce r{};
+          r.f_off = plan->psi[ht.out_sec].off; r.part_off = part_cur; r.slab = slab; r.size = (int64_t)ht.m * ht.p; r.nslab = sl.nchunk;
+          plan->h_tp_reduce.push_back(r);
+          last_sec = ht.out_sec;
+        }
+        part_cur += slab * sl.nchunk;
+        cur = start + per_pos * take;
+        pos += take;
+        plan->h_tp_slices.push_back(sl);
+      }
+    }
+    close_group();
+  }
+
   // ---- diagonal tasks (s == s') for the preconditioner -----------------------------------
   plan->h_diag_begin.assign(nsec + 1, 0);
   for (int s = 0; s < nsec; ++s) {
@@ -798,7 +910,12 @@ extern "C" su2_status su2_plan_create(su2_plan** out, const su2_problem* p, int3
   plan->info.cc_flops = cc;
   plan->info.executed_flops = executed;
   plan->info.operator_bytes = opbytes;
-  plan->info.workspace_bytes = ((plan->partial_elems * 8 + 256) + 255) & ~(int64_t)255;   // a multiple of 256
+  // a multiple of 256: the fused kernel's partial tiles, then the two-pass route's partial slabs
+  plan->info.workspace_bytes = (((plan->partial_elems * 8 + 256) + 255) & ~(int64_t)255) + ((plan->tp_partial_elems * 8 + 255) & ~(int64_t)255);
+  plan->info.two_pass_tasks = 0;
+  for (const HostTask& ht : plan->tasks) plan->info.two_pass_tasks += ht.two_pass;
+  plan->info.two_pass_groups = (int32_t)plan->h_tp_groups.size();
+  plan->info.two_pass_scratch_bytes = plan->tp_scratch_elems * 8;
   plan->info.npsi_sec = nsec;
   plan->info.nwork_items = (int64_t)plan->h_work.size();
   plan->info.small_plan = small_plan ? 1 : 0;

@@ -89,6 +89,32 @@ struct OperandRef {
   int32_t npos;           // positions stored (1: the same block for every position)
 };
 
+// ---- two-pass route of the apply (heff_two_pass.cu; plan flag SU2_PLAN_TWO_PASS) --------------------------------
+// A SLICE is a run of positions of one task whose intermediate T fits the plan's scratch together with the other slices
+// of its GROUP (one pass-1 launch, one pass-2 launch, one reduce launch per group).
+//   order 0: T_pos (m x n) = coef alpha_pos Aop_pos E,     partial[chunk] (m x p) = sum_{pos in chunk} T_pos Dop_pos^T
+//   order 1: T_pos (k x p) = coef alpha_pos E Dop_pos^T,   partial[chunk] (m x p) = sum_{pos in chunk} Aop_pos T_pos
+// (the cheaper of the two, which is what the paper's CC counts).  T_pos is stored row-major with pitch ldt in
+// the scratch, viewed as ONE matrix of rows of ldt doubles: T_pos starts at row t_row0 + (pos - pos0) * rowsT.
+struct TpSlice {
+  int32_t task, pos0, npos, order;
+  int32_t t_row0, ldt;
+  int32_t mapA, mapD, mapE, mapT;   // tensor maps with the boxes of tp_gemm_kernel (indices into su2_plan::d_maps)
+  int32_t item1, item2;             // first pass-1 / pass-2 item (CTA) of the slice inside its group
+  int32_t chunk, nchunk;            // positions per pass-2 item; number of chunks (= partial slabs) of the slice
+  int64_t part_off;                 // element offset of the slice's first partial slab in the workspace's two-pass area
+};
+struct TpGroup {                    // host only
+  int32_t slice0, slice1, items1, items2, red0, red1;
+};
+// F_s += sum of nslab partial slabs in index order (slabs of slab elements each, the first at part_off)
+struct TpReduce {
+  int64_t f_off, part_off, slab, size;
+  int32_t nslab, pad;
+};
+constexpr int TP_TM = 64, TP_TN = 128, TP_KS = 20;   // CTA tile and k depth of a stage (heff_two_pass.cu)
+constexpr int TP_LLD = TP_TM + 4, TP_RLD = TP_TN + 4; // row pitches of boxes read along the other direction
+
 // Diagonal tasks (s == s') for su2_heff_diag.
 struct DevDiagTask {
   const double* A;
@@ -108,6 +134,7 @@ struct HostTask {
   double coef;
   int32_t m, k, n, p, npos;
   int32_t wr;             // tile class of the output sector (large-tile plans)
+  int32_t two_pass;       // 1: executed by the two-pass route (heff_two_pass.cu), not by the fused kernel
 };
 
 struct PsiSector {
@@ -167,6 +194,15 @@ struct su2_plan {
   int64_t partial_elems = 0;
   int32_t num_sms = 148;
   int32_t small_dm8 = 0;               // > 0: small-block plan; largest sector dimension rounded up to 8
+  // two-pass route (SU2_PLAN_TWO_PASS)
+  std::vector<su2::TpSlice> h_tp_slices;
+  std::vector<su2::TpGroup> h_tp_groups;
+  std::vector<su2::TpReduce> h_tp_reduce;
+  int64_t tp_scratch_elems = 0;        // plan-owned T scratch (doubles)
+  int64_t tp_partial_elems = 0;        // two-pass area of the caller's workspace, behind the fused kernel's partial tiles
+  su2::TpSlice* d_tp_slices = nullptr;
+  su2::TpReduce* d_tp_reduce = nullptr;
+  double* d_tp_scratch = nullptr;
   int32_t small_begin[7] = {0, 0, 0, 0, 0, 0, 0};   // small plans: h_work is sorted by size class (DM8 = 8 (c + 1)); class c = [begin[c], begin[c+1])
 };
 
@@ -183,6 +219,9 @@ struct MapKey {
   bool operator<(const MapKey& o) const;
 };
 su2_status encode_tensor_map(void* out128, const MapKey& key);   // host; SU2_ERR_CUDA if the driver refuses
+int tp_tile_rows_executed(int M);   // rows / columns the tiles of tp_gemm_kernel multiply for an M-row / N-column output
+int tp_tile_cols_executed(int N);
+su2_status launch_heff_two_pass(const su2_plan* plan, double* out, double* tp_partial, void* stream);   // heff_two_pass.cu
 su2_status launch_heff_small(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream);   // heff_small.cu
 su2_status launch_apply(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream);
 su2_status launch_diag(const su2_plan* plan, double* diag, void* stream);
