@@ -249,7 +249,7 @@ def run_reference(args):
 
 # ------------------------------------------------------------------------------ GPU arm
 GANG_PACING = False      # --gang-pacing: plan flag SU2_PLAN_GANG_PACING (single-GPU operator)
-TWO_PASS = {}            # --two-pass ...: plan flag SU2_PLAN_TWO_PASS and its options (single-GPU operator)
+TWO_PASS = {}            # --fused / --two-pass-...: plan flag SU2_PLAN_FUSED, options of the two-pass route (single-GPU operator)
 
 
 def build_operator(cfg_name, device, shard=False):
@@ -633,8 +633,10 @@ def run_gpu(args):
                 "call": "apply_host: pinned host Psi in, host F out (su2_heff_apply_host%s)" % (
                     "" if mode != "shard" else "-equivalent: H2D, su2_heff_apply, all-reduce, D2H")},
         "gpu_launches": int(launches),
-        "roofline": {"bound": "tensor", "kernel": "%s (+reduce_kernel) = one su2_heff_apply on this rank" % (
-                         "heff_small_kernel, one launch per size class" if info["small_plan"] else "heff_tma_kernel"),
+        "roofline": {"bound": "tensor", "kernel": "%s = one su2_heff_apply on this rank" % (
+                         "heff_small_kernel, one launch per size class (+reduce_kernel)" if info["small_plan"] else
+                         "tp_gemm_kernel, %d launch groups of pass 1 + pass 2 (+tp_reduce_kernel)" % info["two_pass_groups"]
+                         if info["two_pass_tasks"] else "heff_tma_kernel (+reduce_kernel)"),
                      "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                      "traffic": ncu_traffic(args.config),
                      "peak_source": "FP64 tensor (DMMA.8x8x4) loop measured in this run by su2_probe_fp64_peak (libsu2probe.so): "
@@ -644,7 +646,8 @@ def run_gpu(args):
                      "peak_bf16_ratio_rule": peak_rule, "frac_of_bf16_ratio_rule": achieved / peak_rule,
                      "peak_bf16_ratio_rule_source": "%s bf16_tflops x nominal FP64/BF16 ratio 45/2250" % peak_src,
                      "instruction_path": "FP64 tensor: mma.sync.m8n8k4.f64 = SASS DMMA.8x8x4; operands staged by cp.async.bulk.tensor (UTMALDG)",
-                     "flops": "CC of the plan (useful flops, PAPER.md:229), not executed flops",
+                     "flops": "CC of the plan (useful flops, PAPER.md:229), not executed flops; achieved = CC / CUDA-event time of "
+                              "the whole apply (all launches of the dominant kernel, back to back on one stream)",
                      "apply_ms": apply_ms, "launches_timed": napply, "peak_dfma_loop_measured": dfma,
                      "cublas_dgemm_8192_measured": cublas_dgemm,
                      "hbm_achieved_gbs": info["operator_bytes"] / (apply_ms * 1e-3) / 1e9, "hbm_peak_gbs": peaks["hbm_gbs"]},
@@ -681,8 +684,8 @@ def main():
     ap.add_argument("--int8-workspace-gb", type=float, default=8.0)
     ap.add_argument("--gang-pacing", action="store_true",
                     help="plan with SU2_PLAN_GANG_PACING (row tiles of a sector paced for L2 reuse: less DRAM traffic, 2-5 %% slower)")
-    ap.add_argument("--two-pass", action="store_true",
-                    help="plan with SU2_PLAN_TWO_PASS: tasks with all four extents >= --two-pass-min-dim run un-fused through a plan-owned scratch")
+    ap.add_argument("--fused", action="store_true",
+                    help="plan with SU2_PLAN_FUSED: every task on the fused large-tile kernel (default: the two-pass route, T through a plan-owned scratch)")
     ap.add_argument("--two-pass-min-dim", type=int, default=0)
     ap.add_argument("--two-pass-chunk-k", type=int, default=0)
     ap.add_argument("--two-pass-scratch-gb", type=float, default=0.0)
@@ -691,8 +694,10 @@ def main():
     args = ap.parse_args()
     global GANG_PACING
     GANG_PACING = bool(args.gang_pacing)
-    if args.two_pass:
-        TWO_PASS.update(two_pass=True, two_pass_min_dim=args.two_pass_min_dim, two_pass_chunk_k=args.two_pass_chunk_k,
+    if args.fused:
+        TWO_PASS.update(fused=True)
+    elif args.two_pass_min_dim or args.two_pass_chunk_k or args.two_pass_scratch_gb:
+        TWO_PASS.update(two_pass_min_dim=args.two_pass_min_dim, two_pass_chunk_k=args.two_pass_chunk_k,
                         two_pass_scratch_bytes=int(args.two_pass_scratch_gb * 2**30))
     if args.impl == "reference":
         run_reference(args)

@@ -145,23 +145,28 @@ enum {
                                 the first (DRAM reads -70 %, L2 hit rate 60 -> 84 % at configs[3]'s blocks); costs 2-5 %
                                 of the time because a row tile on a faster SM waits -- off by default, for callers that
                                 share HBM bandwidth or power with something else.  Same result bit for bit. */
-  SU2_PLAN_TWO_PASS = 16     /* tasks whose four extents m, k, n, p all reach su2_plan_options.two_pass_min_dim leave the fused
-                                kernel and run UN-FUSED, the way the paper executes them (one batched GEMM
-                                per product, the position sum as the inner dimension of the second): pass 1
-                                writes T_pos = coef alpha_pos A_pos E (or E D_pos^T, whichever product order is cheaper -- the
-                                order the paper's CC counts) to a plan-owned scratch, pass 2 contracts it over
+  SU2_PLAN_TWO_PASS = 16,    /* (the default of every large-tile plan since round 2; accepted for clarity) the tasks run UN-FUSED,
+                                the way the paper executes them (one batched GEMM per product, the position
+                                sum as the inner dimension of the second): pass 1 writes
+                                T_pos = coef alpha_pos A_pos E (or E D_pos^T, whichever product order is cheaper -- the order
+                                the paper's CC counts) to a plan-owned scratch, pass 2 contracts it over
                                 (position, inner index) into partial slabs, a fixed-order reduction adds the slabs to F_s.
                                 Both passes run on 64 x 128 tiles, 32 x 64 per warp, two CTAs per SM, which the FP64 tensor
-                                pipe of sm_100a rewards.  Ignored by small-block plans.  Deterministic;
-                                the summation order differs from the fused kernel's, so results agree to rounding, not bit
-                                for bit. */
+                                pipe of sm_100a rewards (0.90 of the DMMA peak at configs[3] against 0.70 for
+                                the fused kernel).  Small-block plans (every sector <= 48 multiplets) are not affected.
+                                Deterministic; the summation order differs from the fused kernel's, so the two agree to
+                                rounding, not bit for bit. */
+  SU2_PLAN_FUSED = 32        /* keep the tasks on the fused kernel (T in shared memory, no scratch): tasks with an extent
+                                below su2_plan_options.two_pass_min_dim stay there anyway; with this flag all do.  For
+                                callers without memory for the scratch, and for A/B measurements.  Implied by
+                                SU2_PLAN_GANG_PACING. */
 };
 
 /* Tuning of SU2_PLAN_TWO_PASS (su2_plan_create_opts; 0 = default for every field). */
 typedef struct {
-  int32_t two_pass_min_dim;        /* smallest extent of a task that takes the two-pass route (default 192)                  */
+  int32_t two_pass_min_dim;        /* a task takes the two-pass route if its four extents all reach this (default 1: all do) */
   int32_t two_pass_chunk_k;        /* target length of the inner (position, index) loop of one pass-2 CTA (default 8192)      */
-  int64_t two_pass_scratch_bytes;  /* upper bound of the plan-owned scratch for T (default 8 GiB; never less than one
+  int64_t two_pass_scratch_bytes;  /* upper bound of the plan-owned scratch for T (default 16 GiB; never less than one
                                       position of the largest task; su2_plan_info_t.two_pass_scratch_bytes = what was taken) */
 } su2_plan_options;
 
@@ -245,7 +250,7 @@ su2_status su2_heff_apply(const su2_plan* plan, const double* psi_dev, double* o
  * harnesses that forbid cudaMalloc): out_dev = H_eff * psi_dev with NO workspace argument.  The partial tiles of the
  * segmented reduction live in a static device array of SU2_NOALLOC_SCRATCH_BYTES = 64 MiB inside the library (held by
  * every GPU that loads it until the process exits); the call allocates and frees nothing and is bit-identical to
- * su2_heff_apply.  A plan whose partial tiles exceed that size (workspace_bytes - 256 > SU2_NOALLOC_SCRATCH_BYTES;
+ * su2_heff_apply.  A plan whose partial tiles / partial slabs exceed that size (workspace_bytes - 256 > SU2_NOALLOC_SCRATCH_BYTES;
  * BASELINE.json configs[2..3]) is rejected with SU2_ERR_SCRATCH_LIMIT and a message in su2_last_cuda_error.  The array is
  * shared by ALL calls on a device and keeps the last call's contents (no element is read before the same call wrote it,
  * so nothing needs clearing): calls that overlap on the GPU -- two streams, two plans -- race; order them on one stream.

@@ -188,7 +188,7 @@ class Plan:
     without a GPU)."""
 
     def __init__(self, problem, family_ptrs=None, stream=0, host_only=False, force_split=False, large_tiles=False, gang_pacing=False,
-                 ld_align=1, two_pass=False, two_pass_min_dim=0, two_pass_chunk_k=0, two_pass_scratch_bytes=0):
+                 ld_align=1, fused=False, two_pass=False, two_pass_min_dim=0, two_pass_chunk_k=0, two_pass_scratch_bytes=0):
         lib = load()
         self._keep = []
         self.problem = problem
@@ -243,7 +243,7 @@ class Plan:
                            None if u1 else site, len(problem.term), terms, 1 if u1 else 0, site if u1 else None)
         self.handle = C.c_void_p()
         flags = ((SU2_PLAN_HOST_ONLY if host_only else 0) | (2 if force_split else 0) | (4 if large_tiles else 0) | (8 if gang_pacing else 0) |
-                 (16 if two_pass else 0))
+                 (16 if two_pass else 0) | (32 if fused else 0))
         opts = su2_plan_options(int(two_pass_min_dim), int(two_pass_chunk_k), int(two_pass_scratch_bytes))
         check(lib.su2_plan_create_opts(C.byref(self.handle), C.byref(prob), flags, C.byref(opts), C.c_void_p(stream)))
         info = su2_plan_info_t()

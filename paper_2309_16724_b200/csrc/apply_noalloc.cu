@@ -66,12 +66,15 @@ extern "C" int64_t su2_noalloc_scratch_bytes(void) { return (int64_t)SCRATCH_BYT
 
 extern "C" su2_status su2_heff_apply_noalloc(const su2_plan* plan, const double* psi_dev, double* out_dev, void* cuda_stream) {
   if (!plan || !psi_dev || !out_dev || psi_dev == out_dev) return SU2_ERR_INVALID_ARGUMENT;
-  if ((size_t)plan->partial_elems * sizeof(double) > SCRATCH_BYTES || (size_t)(plan->info.workspace_bytes - 256) > SCRATCH_BYTES) {
+  // what launch_apply touches behind the pointer it is given: the fused kernel's partial tiles, or -- two-pass plans -- all of
+  // the workspace (the partial slabs of the two-pass route start behind the fused kernel's area)
+  const size_t need = plan->tp_partial_elems > 0 ? (size_t)plan->info.workspace_bytes : (size_t)plan->partial_elems * sizeof(double);
+  if (need > SCRATCH_BYTES) {
     char buf[256];
     std::snprintf(buf, sizeof(buf),
                   "su2_heff_apply_noalloc: the plan needs %lld bytes of partial tiles, the static scratch holds %lld "
                   "(SU2_NOALLOC_SCRATCH_BYTES); use su2_heff_apply with a caller-owned workspace",
-                  (long long)(plan->info.workspace_bytes - 256), (long long)SCRATCH_BYTES);
+                  (long long)need, (long long)SCRATCH_BYTES);
     su2::set_error_text(buf);
     return SU2_ERR_SCRATCH_LIMIT;
   }

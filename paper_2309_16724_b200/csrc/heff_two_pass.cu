@@ -170,7 +170,9 @@ __device__ __forceinline__ void tp_consume_nj(const TpItem& it, const double* sm
     case 2: tp_consume<NI, 2, LT, RN>(it, smem, full, empty, warp, lane); break;
     case 3: tp_consume<NI, 3, LT, RN>(it, smem, full, empty, warp, lane); break;
     case 4: tp_consume<NI, 4, LT, RN>(it, smem, full, empty, warp, lane); break;
+    case 5: tp_consume<NI, 5, LT, RN>(it, smem, full, empty, warp, lane); break;
     case 6: tp_consume<NI, 6, LT, RN>(it, smem, full, empty, warp, lane); break;
+    case 7: tp_consume<NI, 7, LT, RN>(it, smem, full, empty, warp, lane); break;
     default: tp_consume<NI, 8, LT, RN>(it, smem, full, empty, warp, lane); break;
   }
 }
@@ -187,9 +189,7 @@ __device__ __forceinline__ void tp_consume_ni(const TpItem& it, const double* sm
 // warp-tile heights / widths of a ragged last tile with `rem` valid rows / columns (the instantiated sizes)
 __host__ __device__ __forceinline__ int tp_ni_for(int rem) { return rem >= TP_TM ? 4 : (rem + 15) / 16; }
 __host__ __device__ __forceinline__ int tp_nj_for(int rem) {
-  if (rem >= TP_TN) return 8;
-  const int nj = (rem + 15) / 16;
-  return nj == 5 ? 6 : nj == 7 ? 8 : nj;
+  return rem >= TP_TN ? 8 : (rem + 15) / 16;
 }
 
 // pass = 0: T_pos of every position of the group's slices; pass = 1: the partial slabs.  grid = items of the group.

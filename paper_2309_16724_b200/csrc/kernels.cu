@@ -331,7 +331,7 @@ su2_status launch_apply(const su2_plan* plan, const double* psi, double* out, do
     }
     if (plan->d_gang)   // pacing slots: -1 = member not started
       SU2_CUDA(cudaMemsetAsync(plan->d_gang, 0xff, (size_t)plan->n_gang_slots * sizeof(int32_t), stream));
-    st = launch_heff_tma(plan, out, partial, stream_v);
+    st = plan->h_work.empty() ? SU2_OK : launch_heff_tma(plan, out, partial, stream_v);   // nothing left on the fused kernel
   }
   if (st != SU2_OK) return st;
   const int nsec = (int)plan->h_reduce.size();

@@ -212,8 +212,8 @@ extern "C" su2_status su2_plan_create_opts(su2_plan** out, const su2_problem* p,
   su2_plan_options opt{};
   if (opts) opt = *opts;
   if (opt.two_pass_min_dim < 0 || opt.two_pass_scratch_bytes < 0 || opt.two_pass_chunk_k < 0) return SU2_ERR_INVALID_ARGUMENT;
-  if (opt.two_pass_min_dim == 0) opt.two_pass_min_dim = 192;
-  if (opt.two_pass_scratch_bytes == 0) opt.two_pass_scratch_bytes = (int64_t)8 << 30;
+  if (opt.two_pass_min_dim == 0) opt.two_pass_min_dim = 1;
+  if (opt.two_pass_scratch_bytes == 0) opt.two_pass_scratch_bytes = (int64_t)16 << 30;
   if (opt.two_pass_chunk_k == 0) opt.two_pass_chunk_k = 8192;
   const auto t_start = std::chrono::steady_clock::now();
 
@@ -589,9 +589,11 @@ extern "C" su2_status su2_plan_create_opts(su2_plan** out, const su2_problem* p,
   }
 
   // ---- two-pass route (heff_two_pass.cu) --------------------------------------------------------
-  // Tasks whose four extents all reach two_pass_min_dim leave the fused kernel: their intermediate T goes through a
-  // plan-owned scratch and both products run as plain GEMMs with 32 x 64 register tiles per warp, two CTAs per SM.
-  const bool two_pass_on = (flags & SU2_PLAN_TWO_PASS) != 0 && !small_plan;
+  // The default of a large-tile plan.  Tasks whose four extents all reach two_pass_min_dim (default: every task) leave the
+  // fused kernel: their intermediate T goes through a plan-owned scratch and both products run as plain GEMMs with
+  // 32 x 64 register tiles per warp, two CTAs per SM.  SU2_PLAN_FUSED (or gang pacing, which is the fused kernel's) keeps
+  // everything on the fused kernel.
+  const bool two_pass_on = !small_plan && !(flags & (SU2_PLAN_FUSED | SU2_PLAN_GANG_PACING));
   for (HostTask& ht : plan->tasks)
     ht.two_pass = two_pass_on && std::min(std::min(ht.m, ht.k), std::min(ht.n, ht.p)) >= opt.two_pass_min_dim ? 1 : 0;
 
@@ -917,7 +919,8 @@ extern "C" su2_status su2_plan_create_opts(su2_plan** out, const su2_problem* p,
   plan->info.two_pass_groups = (int32_t)plan->h_tp_groups.size();
   plan->info.two_pass_scratch_bytes = plan->tp_scratch_elems * 8;
   plan->info.npsi_sec = nsec;
-  plan->info.nwork_items = (int64_t)plan->h_work.size();
+  plan->info.nwork_items = (int64_t)plan->h_work.size();   // + the CTAs of the two-pass route's launches
+  for (const TpGroup& g : plan->h_tp_groups) plan->info.nwork_items += (int64_t)g.items1 + g.items2;
   plan->info.small_plan = small_plan ? 1 : 0;
   plan->info.gang_slots = (int32_t)plan->n_gang_slots;
 

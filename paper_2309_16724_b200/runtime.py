@@ -21,9 +21,10 @@ class HeffOperator:
     workloads cannot be staged through host memory)."""
 
     def __init__(self, problem, device="cuda:0", device_fill=None, force_split=False, large_tiles=False, ld_align=4, gang_pacing=False,
-                 two_pass=False, **two_pass_opts):
-        """two_pass: plan flag SU2_PLAN_TWO_PASS (large tasks un-fused through a plan-owned scratch); two_pass_opts:
-        two_pass_min_dim, two_pass_chunk_k, two_pass_scratch_bytes (su2_plan_options).
+                 fused=False, two_pass=False, **two_pass_opts):
+        """fused: plan flag SU2_PLAN_FUSED (every task on the fused kernel; default: large-tile plans run un-fused through a
+        plan-owned scratch, SU2_PLAN_TWO_PASS); two_pass_opts: two_pass_min_dim, two_pass_chunk_k, two_pass_scratch_bytes
+        (su2_plan_options).
         ld_align: leading dimensions of the operator blocks in device memory are rounded up to this multiple
         (binding.family_layout).  4 (default) puts every row on a 32-byte boundary, so that the large-tile kernel
         reads the operators in place with bulk-tensor copies; 1 is the dense layout, of which the plan makes a
@@ -53,7 +54,7 @@ class HeffOperator:
                 ptrs[(side, i)] = t.data_ptr()
         self.stream = torch.cuda.current_stream(self.device)
         self.plan = Plan(problem, family_ptrs=ptrs, stream=self.stream.cuda_stream, force_split=force_split,
-                         large_tiles=large_tiles, ld_align=ld_align, gang_pacing=gang_pacing, two_pass=two_pass, **two_pass_opts)
+                         large_tiles=large_tiles, ld_align=ld_align, gang_pacing=gang_pacing, fused=fused, two_pass=two_pass, **two_pass_opts)
         self.psi_len = self.plan.psi_len
         # workspace: partial tiles + staging for the host entry point
         self.workspace = torch.empty(self.plan.workspace_bytes + 16 * self.psi_len, dtype=torch.uint8,

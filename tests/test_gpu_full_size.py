@@ -10,6 +10,9 @@ Coverage, elements checked against the oracle / elem
                       are stratified over the three tile classes (all of the two rarer classes' extremes, largest /
                       smallest / median of each) and the sampled rows / columns over the first, a middle and the
                       last row tile / column slab of each sector (incl. the ragged tails).
+Launch configuration: bench.build_operator = the library's default plan, which for configs[2..3] / cfg4p is the two-pass
+route (SU2_PLAN_TWO_PASS: tp_gemm_kernel, 64 x 128 tiles) and for configs[1] the small-block kernel; the fused large-tile
+kernel (SU2_PLAN_FUSED) is compared with it at configs[1], configs[2] and cfg4p.
 Every sampled entry is evaluated over ALL operator-table rows, input sectors and positions (oracle/heff_sampled.py)."""
 import numpy as np
 import pytest
@@ -89,10 +92,11 @@ def test_cfg2_full_oracle_parity_and_properties():
     assert np.abs(f - f_ref).max() / np.abs(f_ref).max() <= TOL
     xd, hx = _properties(torch, op, f, 31)
     from paper_2309_16724_b200.runtime import HeffOperator
-    op_big = HeffOperator(prob, device="cuda:0", large_tiles=True)
-    assert op_big.info["small_plan"] == 0
-    f_big = op_big.apply(xd).cpu().numpy()
-    assert np.abs(f_big - f_ref).max() / np.abs(f_ref).max() <= TOL       # all 85 126 elements, the other kernel
+    for kw in (dict(fused=True), dict()):     # all 85 126 elements through the fused large-tile kernel and the two-pass route
+        op_big = HeffOperator(prob, device="cuda:0", large_tiles=True, **kw)
+        assert op_big.info["small_plan"] == 0 and (op_big.info["two_pass_tasks"] == 0) == bool(kw)
+        f_big = op_big.apply(xd).cpu().numpy()
+        assert np.abs(f_big - f_ref).max() / np.abs(f_ref).max() <= TOL
 
 
 def test_cfg3_sampled_parity_every_sector_and_properties():
@@ -104,7 +108,12 @@ def test_cfg3_sampled_parity_every_sector_and_properties():
     worst, f, checked = _sampled_parity(torch, prob, op, range(138), 8, numpy_block_rows(prob), seed=11)
     assert checked == 138 * 64
     assert worst <= TOL, worst
-    _properties(torch, op, f, 11)
+    assert op.info["two_pass_tasks"] == op.info["ntasks"]
+    x, hx = _properties(torch, op, f, 11)
+    from paper_2309_16724_b200.runtime import HeffOperator
+    fused = HeffOperator(prob, device="cuda:0", fused=True)      # every element: the fused kernel against the two-pass route
+    assert fused.info["two_pass_tasks"] == 0
+    assert float((fused.apply(x) - hx).abs().max() / hx.abs().max()) <= 1e-12
 
 
 def _cfg4_sector_choice(prob, op, count):
@@ -130,7 +139,7 @@ def test_cfg4_sampled_parity_and_properties():
     reproducibility, Hermiticity and linearity of the GPU result at this size."""
     from gen.device_ops import device_block_rows
     torch, prob, op = _setup("cfg4")
-    assert op.psi_len == 19728348 and op.info["padded_copy_bytes"] == 0
+    assert op.psi_len == 19728348 and op.info["padded_copy_bytes"] == 0 and op.info["two_pass_tasks"] == op.info["ntasks"]
     rows = device_block_rows(prob, op.family_tensors, op.family_layouts)
     sectors, cls = _cfg4_sector_choice(prob, op, 40)
     assert len({cls[i] for i in sectors}) == len(set(cls))
@@ -140,11 +149,11 @@ def test_cfg4_sampled_parity_and_properties():
     _properties(torch, op, f, 21)
 
 
-def test_cfg4p_gang_pacing_and_int8_apply_equal_the_default_apply():
-    """cfg4p = the blocks of BASELINE.json configs[3] (69-547 multiplets) with 24 positions per family (5.8 GB): the plan
-    flag SU2_PLAN_GANG_PACING (1 908 row tiles in gangs here) gives the bits of the default plan, twice in a row; the same
-    plan executed on the INT8 tensor path (su2_heff_apply_i8) agrees with it to 1e-12 of max|F|; sampled entries of the
-    default result against the oracle (the other two inherit that parity)."""
+def test_cfg4p_fused_kernel_gang_pacing_and_int8_apply_equal_the_default_apply():
+    """cfg4p = the blocks of BASELINE.json configs[3] (69-547 multiplets) with 24 positions per family (5.8 GB): sampled
+    entries of the default (two-pass) result against the oracle; the fused kernel (SU2_PLAN_FUSED) agrees with it to 1e-12
+    of max|F| on every element; the plan flag SU2_PLAN_GANG_PACING (1 908 row tiles in gangs here) gives the bits of the
+    fused plan, twice in a row; the same plan executed on the INT8 tensor path (su2_heff_apply_i8) agrees to 1e-12."""
     from gen.device_ops import device_block_rows, device_fill
     from paper_2309_16724_b200.runtime import HeffOperator
     torch, prob, op = _setup("cfg4p")
@@ -159,7 +168,12 @@ def test_cfg4p_gang_pacing_and_int8_apply_equal_the_default_apply():
     assert float((f8 - want).abs().max() / want.abs().max()) <= 1e-12
     del f8
     op._i8_ws = None
+    fused = HeffOperator(prob, device="cuda:0", device_fill=device_fill(prob), fused=True)
+    assert fused.info["two_pass_tasks"] == 0 and op.info["two_pass_tasks"] == op.info["ntasks"]
+    f_fused = fused.apply(x).clone()
+    assert float((f_fused - want).abs().max() / want.abs().max()) <= 1e-12
+    del fused
     paced = HeffOperator(prob, device="cuda:0", device_fill=device_fill(prob), gang_pacing=True)
-    assert paced.info["gang_slots"] > 1000 and paced.info["nwork_items"] == op.info["nwork_items"]
+    assert paced.info["gang_slots"] > 1000 and paced.info["two_pass_tasks"] == 0
     for _ in range(2):
-        assert torch.equal(paced.apply(x), want)
+        assert torch.equal(paced.apply(x), f_fused)

@@ -67,8 +67,9 @@ def test_operator_layouts_dense_and_padded(ld_align):
     prob = config_problem("midi")
     x = random_psi(_operator(prob).psi_len, seed=2)
     f_ref = oracle_flat(prob, _operator(prob).plan, x)
-    for large in (False, True):
-        op = _operator(prob, ld_align=ld_align, large_tiles=large, force_split=True)
+    for kw in (dict(), dict(large_tiles=True), dict(large_tiles=True, fused=True)):   # small-block, two-pass, fused kernels
+        large = bool(kw)
+        op = _operator(prob, ld_align=ld_align, force_split=True, **kw)
         f = op.apply(torch.from_numpy(x).cuda()).cpu().numpy()
         assert _rel(f, f_ref) <= TOL
         if large:
@@ -86,14 +87,17 @@ def test_small_bonds_through_the_large_tile_kernel(name):
     prob = _cfg1() if name == "cfg1" else config_problem(name)
     op_small = _operator(prob, force_split=True)
     assert op_small.info["small_plan"] == 1
-    op_big = _operator(prob, force_split=True, large_tiles=True)
-    assert op_big.info["small_plan"] == 0
+    op_big = _operator(prob, force_split=True, large_tiles=True, fused=True)
+    assert op_big.info["small_plan"] == 0 and op_big.info["two_pass_tasks"] == 0
+    op_tp = _operator(prob, force_split=True, large_tiles=True)          # the default of a large-tile plan: two-pass route
+    assert op_tp.info["two_pass_tasks"] == op_tp.info["ntasks"]
     x = random_psi(op_small.psi_len, seed=5)
     f_ref = oracle_flat(prob, op_small.plan, x)
     f_small = op_small.apply(torch.from_numpy(x).cuda()).cpu().numpy()
     f_big = op_big.apply(torch.from_numpy(x).cuda()).cpu().numpy()
-    assert _rel(f_small, f_ref) <= TOL and _rel(f_big, f_ref) <= TOL
-    assert _rel(f_small, f_big) <= 1e-12
+    f_tp = op_tp.apply(torch.from_numpy(x).cuda()).cpu().numpy()
+    assert _rel(f_small, f_ref) <= TOL and _rel(f_big, f_ref) <= TOL and _rel(f_tp, f_ref) <= TOL
+    assert _rel(f_small, f_big) <= 1e-12 and _rel(f_tp, f_big) <= 1e-12
 
 
 @pytest.mark.parametrize("name,world", [("mini", 2), ("midi", 3)])
@@ -221,13 +225,14 @@ def test_sharded_davidson_two_shards_on_one_gpu():
     dav.close(); ref.close()
 
 
-def test_several_tiles_and_ragged_tail():
-    """Blocks larger than one tile with ragged tails (L=16, D=500: dims 6..109)."""
+@pytest.mark.parametrize("fused", [False, True])
+def test_several_tiles_and_ragged_tail(fused):
+    """Blocks larger than one tile with ragged tails (L=16, D=500: dims 6..109), two-pass route and fused kernel."""
     torch = _torch()
     prob = synthetic_problem(16, 16, 0, 500, seed=3)
     dims = [s.dim for s in prob.sec_l]
     assert max(dims) > 64 and any(d % 8 for d in dims)
-    op = _operator(prob)
+    op = _operator(prob, fused=fused)
     x = random_psi(op.psi_len, seed=2)
     f_gpu = op.apply(torch.from_numpy(x).cuda()).cpu().numpy()
     f_ref = oracle_flat(prob, op.plan, x)
@@ -700,11 +705,11 @@ def _wide_problem():
                    meta=dict(L=0, N=4, D=0))
 
 
-@pytest.mark.parametrize("force_split", [False, True])
-def test_wide_sector_multiple_column_tiles(force_split):
+@pytest.mark.parametrize("force_split,fused", [(False, True), (True, True), (False, False)])
+def test_wide_sector_multiple_column_tiles(force_split, fused):
     torch = _torch()
     prob = _wide_problem()
-    op = _operator(prob, force_split=force_split)
+    op = _operator(prob, force_split=force_split, fused=fused)
     assert max(s.dim for s in prob.sec_r) > 576
     x = random_psi(op.psi_len, seed=8)
     f_gpu = op.apply(torch.from_numpy(x).cuda()).cpu().numpy()
@@ -732,7 +737,8 @@ def test_u1_mode_parity_and_equivalence(name, merged):
     x = flatten_u1(u1, psi_u1, labels_u1)
     f_ref = flatten_u1(u1, heff_apply_u1(u1, psi_u1), labels_u1)
     f_su2 = op_su2.apply(torch.from_numpy(x_red).cuda()).cpu().numpy()
-    for kw in (dict(), dict(large_tiles=True), dict(large_tiles=True, force_split=True), dict(force_split=True)):
+    for kw in (dict(), dict(large_tiles=True), dict(large_tiles=True, fused=True), dict(large_tiles=True, fused=True, force_split=True),
+               dict(force_split=True)):
         op = _operator(u1, **kw)
         assert op.plan.labels == labels_u1
         f = op.apply(torch.from_numpy(x).cuda()).cpu().numpy()

@@ -58,7 +58,7 @@ def test_hybrid_plan_ragged_tiles(min_dim):
     f_ref = oracle_flat(prob, op.plan, x)
     assert _rel(f_gpu, f_ref) <= TOL
     # against the fused kernel's result of the same operator
-    f_fused = _operator(prob).apply(torch.from_numpy(x).cuda()).cpu().numpy()
+    f_fused = _operator(prob, fused=True).apply(torch.from_numpy(x).cuda()).cpu().numpy()
     assert _rel(f_gpu, f_fused) <= 1e-12
 
 

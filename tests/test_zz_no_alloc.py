@@ -11,19 +11,19 @@ TOL = 1e-10          # the tolerance of the GPU parity tests (north_star)
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("large_tiles", [False, True])
-def test_noalloc_apply_equals_the_workspace_path_on_two_calls_in_a_row(large_tiles):
+@pytest.mark.parametrize("large_tiles,fused", [(False, False), (True, True), (True, False)])
+def test_noalloc_apply_equals_the_workspace_path_on_two_calls_in_a_row(large_tiles, fused):
     """Two calls in a row with different Psi (the second one finds the first one's partial tiles in the shared scratch),
     then the first input again: each equals su2_heff_apply's result (same kernels, same order of sums: bit for bit, and a
-    fortiori within 1e-10), through the small-block kernel and the large-tile (bulk-tensor) kernel, with split segments so
-    that the scratch really carries partial tiles."""
+    fortiori within 1e-10), through the small-block kernel, the fused large-tile (bulk-tensor) kernel and the two-pass route,
+    with split segments / partial slabs so that the scratch really carries partial results."""
     import torch
     assert torch.cuda.is_available(), "GPU tests need a CUDA device"
     from paper_2309_16724_b200.binding import noalloc_scratch_bytes
     from paper_2309_16724_b200.runtime import HeffOperator
     prob = config_problem("midi")
-    op = HeffOperator(prob, force_split=True, large_tiles=large_tiles)
-    assert op.info["nsegments"] > op.info["npsi_sec"]                       # partial tiles are in use
+    op = HeffOperator(prob, force_split=True, large_tiles=large_tiles, fused=fused)
+    assert op.info["nsegments"] > op.info["npsi_sec"] or op.info["two_pass_groups"] > 0      # partial tiles / slabs are in use
     assert 0 < op.plan.workspace_bytes - 256 <= noalloc_scratch_bytes() == 64 * 1024 * 1024
     xs = [torch.from_numpy(random_psi(op.psi_len, seed=s)).cuda() for s in (41, 42, 41)]
     ref = [op.apply(x).clone() for x in xs]                                 # existing path, caller-owned workspace
