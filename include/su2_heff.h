@@ -168,6 +168,9 @@ typedef struct {
   int32_t two_pass_chunk_k;        /* target length of the inner (position, index) loop of one pass-2 CTA (default 8192)      */
   int64_t two_pass_scratch_bytes;  /* upper bound of the plan-owned scratch for T (default 16 GiB; never less than one
                                       position of the largest task; su2_plan_info_t.two_pass_scratch_bytes = what was taken) */
+  int32_t two_pass_ipc_k;          /* pass 1: a CTA works through consecutive (position, tile) items until their inner
+                                      extents add up to about this (default 2048; 1 = one item per CTA)                     */
+  int32_t pad;
 } su2_plan_options;
 
 typedef struct {
@@ -342,20 +345,21 @@ su2_status su2_renormalize(const su2_blocking* blocking, const su2_opfamily* op_
 
 /* Strided-batched FP64 GEMM-pair microbenchmark entry (BASELINE.json configs[4]):
  * C_b (m x p) += alpha * A_b (m x k) * X_b (k x n) * B_b^T (n x p) for b < batch, all DEVICE,
- * row-major, dense strides (A_b = A + b*m*k, ...); the paper's strided-batched GEMM sequences
- * with T = A_b X_b kept on chip except for items of >= 256 in every extent (un-fused two-pass kernel: T through a
- * stream-ordered scratch).  Items whose operands fit one SM's shared memory run one CTA per item on FP64
- * tensor instructions (HBM-bound regime); all other items use the fused kernel of the apply (three rank-3 tensor maps
- * {columns, rows, batch} describe the whole call); an operand whose rows are not 16-byte aligned (odd k or n, odd base
- * address) is first copied into a stream-ordered buffer with an even row pitch.  C_b blocks must not overlap
- * (PAPER.md:132); one CTA owns an output element, so results are bit-reproducible.  Errors: non-positive dimension,
- * negative batch or null pointer -> SU2_ERR_INVALID_ARGUMENT; batch == 0 is a no-op. */
+ * row-major, dense strides (A_b = A + b*m*k, ...); the paper's strided-batched GEMM sequences.
+ * Items of at least 48 in every extent run UN-FUSED, as in the paper: T_b = alpha A_b X_b (or alpha X_b B_b^T, the cheaper
+ * order) through a stream-ordered scratch, then C_b += T_b B_b^T, both on the two-pass GEMM kernel of the apply (64 x 128
+ * tiles, narrower edge tiles, several consecutive tiles per CTA); an operand whose rows are not 16-byte aligned (odd k or n,
+ * odd base address) is first copied into a stream-ordered buffer with an even row pitch.  Smaller items whose operands fit one
+ * SM's shared memory run one CTA per item with T kept on chip (HBM-bound regime); items with one short extent use the fused
+ * large-tile kernel.  C_b blocks must not overlap; one CTA owns an output element, so results are
+ * bit-reproducible.  Errors: non-positive dimension, negative batch or null pointer -> SU2_ERR_INVALID_ARGUMENT; batch == 0
+ * is a no-op. */
 su2_status su2_gemm_pair_batched(int32_t m, int32_t k, int32_t n, int32_t p, int64_t batch, double alpha,
                                  const double* A, const double* X, const double* B, double* C,
                                  void* cuda_stream);
 /* The same with the kernel chosen by the caller (tests, tuning): route 0 automatic, 1 small-block kernel, 2 fused
- * large-tile kernel, 4 un-fused two-pass kernel (T = A X through a stream-ordered scratch, then C += alpha T B^T; 32 x 64
- * register tiles per warp, two CTAs per SM: chosen automatically for items of at least 256 in every extent), 3 FP64-FMA
+ * large-tile kernel, 4 un-fused two-pass kernel (T through a stream-ordered scratch; 32 x 64 register tiles per warp, two
+ * CTAs per SM: chosen automatically for items of at least 48 in every extent), 3 FP64-FMA
  * tile routine (a plain reference routine, never chosen automatically below 2^24 items); SU2_ERR_INVALID_ARGUMENT if
  * the shape does not fit the route.  wpi / nbuf (0 = heuristics) override the small-block kernel's warps per item and input buffering. */
 su2_status su2_gemm_pair_batched_route(int32_t m, int32_t k, int32_t n, int32_t p, int64_t batch, double alpha,

@@ -177,6 +177,12 @@ su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double al
                             const double* B, double* C, void* stream_v, int route, int wpi, int nbuf) {
   if (batch == 0) return SU2_OK;
   cudaStream_t stream = (cudaStream_t)stream_v;
+  // automatic choice: items of at least 48 in every extent run un-fused on the two-pass GEMM (gemm_two_pass.cu) -- measured on
+  // one B200, TFLOP/s un-fused / best other route: 48^4 16.5 / 13.4, 64^4 21.1 / 17.7, 96^4 25.8 / 12.6, 128^4 27.1 / 19.1,
+  // 192^4 29.6 / 21.1, 256^4 30.5 / 22.5, 512^4 32.7 / 26.2, 547^4 27.5 / 23.7 (odd row lengths re-pitched inside); 32^4
+  // 9.1 / 16.2 stays on the small-block kernel, and so do items with one short extent (8 x 512 x 512 x 8)
+  constexpr int TWO_PASS_MIN_EXTENT = 48;
+  if (route == 0 && std::min(std::min(m, k), std::min(n, p)) >= TWO_PASS_MIN_EXTENT) route = 4;
   if (route == 0 || route == 1) {
     // items whose operands fit one SM's shared memory (all dims <= 80 for square shapes): one CTA of 1-16 warps per
     // item, shared memory sized by the item shape (gemm_pair_small.cu)
@@ -192,15 +198,7 @@ su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double al
   const bool padA = (k & 1) || ((uintptr_t)A & 15), padX = (n & 1) || ((uintptr_t)X & 15), padB = (n & 1) || ((uintptr_t)B & 15);
   const int ldA = k + (k & 1), ldX = n + (n & 1), ldB = n + (n & 1);
   const int64_t max_items = (int64_t)1 << 24;
-  // automatic choice: items of at least 256 in every extent with 16-byte aligned rows are faster un-fused (512^4: 28.1 against
-  // 26.1 TFLOP/s, 256^4: 23.0 against 22.1; below that, and for operands that need re-pitching, the fused kernel wins)
-  // -- provided its 64 x 128 tiles fit the two outputs (516^4 pads to 576 x 640: 23.7 against 25.2 fused; 446^4: 26.6 against 20.9)
-  if (route == 0 && std::min(std::min(m, k), std::min(n, p)) >= 256 && !padA && !padX && !padB && !(p & 1) && batch <= 65535) {
-    auto fit = [](int rows, int cols) {
-      return ((double)rows * cols) / ((double)((rows + 63) / 64 * 64) * ((cols + 127) / 128 * 128));
-    };
-    if (fit(m, n) >= 0.8 && fit(m, p) >= 0.8) route = 4;
-  }
+  // (the automatic choice of route 4 is made at the top: every extent >= TWO_PASS_MIN_EXTENT)
   if (route == 4) {
     // un-fused form (gemm_two_pass.cu): T through a scratch, both passes with 32 x 64 warp tiles and two CTAs per SM
     const size_t b_padA = padA ? (((size_t)batch * m * ldA * 8 + 255) & ~(size_t)255) : 0;
@@ -220,12 +218,7 @@ su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double al
     if (padA) mA = repitch(A, pads, (int64_t)batch * m, k, ldA);
     if (padX) mX = repitch(X, pads + b_padA, (int64_t)batch * k, n, ldX);
     if (padB) mB = repitch(B, pads + b_padA + b_padX, (int64_t)batch * p, n, ldB);
-    su2_status st = SU2_OK;
-    for (int64_t b0 = 0; b0 < batch && st == SU2_OK; b0 += 65535) {      // grid.z
-      const int64_t nb = std::min<int64_t>(65535, batch - b0);
-      st = launch_gemm_two_pass(m, k, n, p, nb, alpha, mA + b0 * m * (padA ? ldA : k), padA ? ldA : k, mX + b0 * k * (padX ? ldX : n),
-                                padX ? ldX : n, mB + b0 * p * (padB ? ldB : n), padB ? ldB : n, C + b0 * m * p, stream_v);
-    }
+    su2_status st = launch_gemm_two_pass(m, k, n, p, batch, alpha, mA, padA ? ldA : k, mX, padX ? ldX : n, mB, padB ? ldB : n, C, stream_v);
     if (pads) cudaFreeAsync(pads, stream);
     return st;
   }

@@ -78,12 +78,13 @@ struct TpItem {
   int ni, nj;               // warp tile: 8 ni rows x 8 nj columns
   double* dst;
   int ldd;
+  int acc_init;             // 1: the accumulators start from dst (dst += ...), 0: from zero
   double scale;
 };
 
 // consumer warp (wr, wc) of a 2 x 2 grid: rows [8 NI wr, +8 NI) x columns [8 NJ wc, +8 NJ) of the CTA tile
 template <int NI, int NJ, bool LT, bool RN>
-__device__ __forceinline__ void tp_consume(const TpItem& it, const double* __restrict__ smem, uint64_t* full, uint64_t* empty, int warp, int lane) {
+__device__ __forceinline__ void tp_consume(const TpItem& it, const double* __restrict__ smem, uint64_t* full, uint64_t* empty, int warp, int lane, int& step) {
   const int wr = warp >> 1, wc = warp & 1;
   const int g = lane >> 2, t = lane & 3;
   double acc[NI][NJ][2];
@@ -91,13 +92,32 @@ __device__ __forceinline__ void tp_consume(const TpItem& it, const double* __res
   for (int i = 0; i < NI; ++i)
 #pragma unroll
     for (int j = 0; j < NJ; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+  if (it.acc_init) {   // dst += ...: start from the old values (fetched while the pipeline fills) instead of adding them at the end
+    const int cb = it.col0 + wc * 8 * NJ + 2 * t;
+#pragma unroll
+    for (int i = 0; i < NI; ++i) {
+      const int r = it.row0 + wr * 8 * NI + i * 8 + g;
+      if (r >= it.M) continue;
+#pragma unroll
+      for (int j = 0; j < NJ; ++j) {
+        const int c = cb + j * 8;
+        const double* o = it.dst + (int64_t)r * it.ldd + c;
+        if (!(it.ldd & 1) && !((uintptr_t)it.dst & 15) && c + 1 < it.N) {
+          const double2 v = *(const double2*)o;
+          acc[i][j][0] = v.x; acc[i][j][1] = v.y;
+        } else {
+          if (c < it.N) acc[i][j][0] = o[0];
+          if (c + 1 < it.N) acc[i][j][1] = o[1];
+        }
+      }
+    }
+  }
   constexpr int LI = LT ? 8 : 8 * TP_KS, LS = LT ? 4 * TP_LLD : 4;          // element steps: next m8 tile, next k4 sub-step
   constexpr int RJ = RN ? 8 : 8 * TP_KS, RS = RN ? 4 * TP_RLD : 4;
   const int l_off = LT ? t * TP_LLD + wr * 8 * NI + g : (wr * 8 * NI + g) * TP_KS + t;
   const int r_off = TP_LREG + (RN ? t * TP_RLD + wc * 8 * NJ + g : (wc * 8 * NJ + g) * TP_KS + t);
   const int nsteps = (it.K + TP_KS - 1) / TP_KS;
   const int nsub_last = (it.K - (nsteps - 1) * TP_KS + 3) >> 2;            // k4 sub-steps of the last stage that hold data
-  int step = 0;
   for (int pl = 0; pl < it.npl; ++pl)
     for (int s = 0; s < nsteps; ++s, ++step) {
       const int b = step % TP_NS;
@@ -143,7 +163,7 @@ __device__ __forceinline__ void tp_consume(const TpItem& it, const double* __res
       if (lane == 0) tp_mbar_arrive(&empty[b]);
     }
   // epilogue: dst = scale * acc (accumulator layout: row g, columns 2t, 2t + 1 of every m8n8 tile), guarded
-  const bool vec = !(it.ldd & 1);
+  const bool vec = !(it.ldd & 1) && !((uintptr_t)it.dst & 15);
   const int cbase = it.col0 + wc * 8 * NJ + 2 * t;
 #pragma unroll
   for (int i = 0; i < NI; ++i) {
@@ -164,25 +184,25 @@ __device__ __forceinline__ void tp_consume(const TpItem& it, const double* __res
 }
 
 template <int NI, bool LT, bool RN>
-__device__ __forceinline__ void tp_consume_nj(const TpItem& it, const double* smem, uint64_t* full, uint64_t* empty, int warp, int lane) {
+__device__ __forceinline__ void tp_consume_nj(const TpItem& it, const double* smem, uint64_t* full, uint64_t* empty, int warp, int lane, int& step) {
   switch (it.nj) {
-    case 1: tp_consume<NI, 1, LT, RN>(it, smem, full, empty, warp, lane); break;
-    case 2: tp_consume<NI, 2, LT, RN>(it, smem, full, empty, warp, lane); break;
-    case 3: tp_consume<NI, 3, LT, RN>(it, smem, full, empty, warp, lane); break;
-    case 4: tp_consume<NI, 4, LT, RN>(it, smem, full, empty, warp, lane); break;
-    case 5: tp_consume<NI, 5, LT, RN>(it, smem, full, empty, warp, lane); break;
-    case 6: tp_consume<NI, 6, LT, RN>(it, smem, full, empty, warp, lane); break;
-    case 7: tp_consume<NI, 7, LT, RN>(it, smem, full, empty, warp, lane); break;
-    default: tp_consume<NI, 8, LT, RN>(it, smem, full, empty, warp, lane); break;
+    case 1: tp_consume<NI, 1, LT, RN>(it, smem, full, empty, warp, lane, step); break;
+    case 2: tp_consume<NI, 2, LT, RN>(it, smem, full, empty, warp, lane, step); break;
+    case 3: tp_consume<NI, 3, LT, RN>(it, smem, full, empty, warp, lane, step); break;
+    case 4: tp_consume<NI, 4, LT, RN>(it, smem, full, empty, warp, lane, step); break;
+    case 5: tp_consume<NI, 5, LT, RN>(it, smem, full, empty, warp, lane, step); break;
+    case 6: tp_consume<NI, 6, LT, RN>(it, smem, full, empty, warp, lane, step); break;
+    case 7: tp_consume<NI, 7, LT, RN>(it, smem, full, empty, warp, lane, step); break;
+    default: tp_consume<NI, 8, LT, RN>(it, smem, full, empty, warp, lane, step); break;
   }
 }
 template <bool LT, bool RN>
-__device__ __forceinline__ void tp_consume_ni(const TpItem& it, const double* smem, uint64_t* full, uint64_t* empty, int warp, int lane) {
+__device__ __forceinline__ void tp_consume_ni(const TpItem& it, const double* smem, uint64_t* full, uint64_t* empty, int warp, int lane, int& step) {
   switch (it.ni) {
-    case 1: tp_consume_nj<1, LT, RN>(it, smem, full, empty, warp, lane); break;
-    case 2: tp_consume_nj<2, LT, RN>(it, smem, full, empty, warp, lane); break;
-    case 3: tp_consume_nj<3, LT, RN>(it, smem, full, empty, warp, lane); break;
-    default: tp_consume_nj<4, LT, RN>(it, smem, full, empty, warp, lane); break;
+    case 1: tp_consume_nj<1, LT, RN>(it, smem, full, empty, warp, lane, step); break;
+    case 2: tp_consume_nj<2, LT, RN>(it, smem, full, empty, warp, lane, step); break;
+    case 3: tp_consume_nj<3, LT, RN>(it, smem, full, empty, warp, lane, step); break;
+    default: tp_consume_nj<4, LT, RN>(it, smem, full, empty, warp, lane, step); break;
   }
 }
 
@@ -192,23 +212,11 @@ __host__ __device__ __forceinline__ int tp_nj_for(int rem) {
   return rem >= TP_TN ? 8 : (rem + 15) / 16;
 }
 
-// pass = 0: T_pos of every position of the group's slices; pass = 1: the partial slabs.  grid = items of the group.
-__global__ void __launch_bounds__(TP_THREADS, 2)
-tp_gemm_kernel(const TpSlice* __restrict__ slices, int nslices, int pass, const DevTask* __restrict__ tasks,
-               const CUtensorMap* __restrict__ maps, double* __restrict__ scratch, double* __restrict__ partial) {
-  extern __shared__ __align__(1024) double smem[];
-  __shared__ __align__(8) uint64_t full[TP_NS];
-  __shared__ __align__(8) uint64_t empty[TP_NS];
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  if (tid == 0) {
-    for (int i = 0; i < TP_NS; ++i) {
-      tp_mbar_init(&full[i], 1);
-      tp_mbar_init(&empty[i], TP_CONSUMERS);
-    }
-    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
-  }
+// What item `item` of a launch is: which slice (binary search over the slices' first items), which tile, which positions.
+__device__ __forceinline__ TpItem tp_decode(const TpSlice* __restrict__ slices, int nslices, int pass, const DevTask* __restrict__ tasks,
+                                            const CUtensorMap* __restrict__ maps, double* __restrict__ scratch,
+                                            double* __restrict__ partial, int item) {
   // ---- which slice, which item of it (binary search over the slices' first items)
-  const int item = blockIdx.x;
   int lo = 0, hi = nslices - 1;
   while (lo < hi) {
     const int mid = (lo + hi + 1) >> 1;
@@ -241,22 +249,24 @@ tp_gemm_kernel(const TpSlice* __restrict__ slices, int nslices, int pass, const 
   if (pass == 0) {
     pl0 = outer;
     it.npl = 1;
+    it.acc_init = 0;
     const double al = tk->alpha ? tk->alpha[sl.pos0 + pl0] : 1.0;
     it.scale = tk->coef * al;
     it.dst = scratch + ((int64_t)sl.t_row0 + (int64_t)pl0 * rowsT) * sl.ldt;
     it.ldd = sl.ldt;
     if (sl.order == 0) {   // T = Aop E
       it.mapL = maps + sl.mapA; it.lt = transA; it.l_item = stepA ? sl.pos0 + pl0 : 0;
-      it.mapR = maps + sl.mapE; it.rn = 1;
+      it.mapR = maps + sl.mapE; it.rn = 1; it.r_item = (sl.flags & TP_SLICE_E_PER_POS) ? sl.pos0 + pl0 : 0;
     } else {               // T = E Dop^T
-      it.mapL = maps + sl.mapE; it.lt = 0;
+      it.mapL = maps + sl.mapE; it.lt = 0; it.l_item = (sl.flags & TP_SLICE_E_PER_POS) ? sl.pos0 + pl0 : 0;
       it.mapR = maps + sl.mapD; it.rn = transD; it.r_item = stepD ? sl.pos0 + pl0 : 0;
     }
   } else {
     pl0 = outer * sl.chunk;
     it.npl = min(sl.chunk, sl.npos - pl0);
     it.scale = 1.0;
-    const int64_t slab = ((int64_t)m * p + 1) & ~(int64_t)1;
+    it.acc_init = (sl.flags & TP_SLICE_ACCUMULATE) ? 1 : 0;
+    const int64_t slab = it.acc_init ? (int64_t)m * p : ((int64_t)m * p + 1) & ~(int64_t)1;   // dense outputs / even-sized partial slabs
     it.dst = partial + sl.part_off + (int64_t)outer * slab;
     it.ldd = p;
     if (sl.order == 0) {   // partial = sum_pos T_pos Dop_pos^T
@@ -267,32 +277,60 @@ tp_gemm_kernel(const TpSlice* __restrict__ slices, int nslices, int pass, const 
       it.mapR = maps + sl.mapT; it.rn = 1; it.r_k = sl.t_row0 + pl0 * rowsT; it.r_k_step = rowsT;
     }
   }
+  return it;
+}
+
+// pass = 0: T_pos of every position of the group's slices; pass = 1: the partial slabs.  Items are numbered over the group;
+// CTA b works through items [b ipc, (b + 1) ipc) one after the other WITHOUT draining its pipeline in between: the producer
+// thread and the consumer warps decode the items independently and count the same stages, so the producer is already staging
+// the next item while the consumers store the current one (pass 1 of small blocks: a CTA's start-up is spread over ipc items).
+__global__ void __launch_bounds__(TP_THREADS, 2)
+tp_gemm_kernel(const TpSlice* __restrict__ slices, int nslices, int pass, int nitems, int ipc, const DevTask* __restrict__ tasks,
+               const CUtensorMap* __restrict__ maps, double* __restrict__ scratch, double* __restrict__ partial) {
+  extern __shared__ __align__(1024) double smem[];
+  __shared__ __align__(8) uint64_t full[TP_NS];
+  __shared__ __align__(8) uint64_t empty[TP_NS];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  if (tid == 0) {
+    for (int i = 0; i < TP_NS; ++i) {
+      tp_mbar_init(&full[i], 1);
+      tp_mbar_init(&empty[i], TP_CONSUMERS);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
   __syncthreads();
+  const int item0 = blockIdx.x * ipc, item1 = min(nitems, item0 + ipc);
+  int step = 0;
   if (warp == TP_CONSUMERS) {
     // ---- producer: one thread, two boxes per stage
     if (lane != 0) return;
-    const unsigned bytes = (unsigned)(((it.lt ? TP_LBOX_M : TP_LBOX_K) + (it.rn ? TP_RBOX_N : TP_RBOX_K)) * sizeof(double));
-    const int nsteps = (it.K + TP_KS - 1) / TP_KS;
-    int step = 0;
-    for (int pl = 0; pl < it.npl; ++pl) {
-      const int lrow = it.row0 + it.l_row + pl * it.l_row_step, litem = it.l_item + pl * it.l_item_step;
-      const int rk = it.r_k + pl * it.r_k_step, ritem = it.r_item + pl * it.r_item_step;
-      for (int s = 0; s < nsteps; ++s, ++step) {
-        const int b = step % TP_NS, round = step / TP_NS;
-        if (round > 0) tp_mbar_wait(&empty[b], (round - 1) & 1);
-        tp_mbar_expect(&full[b], bytes);
-        const unsigned st = tp_smem_u32(smem + (size_t)b * TP_STAGE);
-        if (it.lt) tp_tma_box(st, it.mapL, lrow, s * TP_KS, litem, &full[b]);
-        else tp_tma_box(st, it.mapL, s * TP_KS, lrow, litem, &full[b]);
-        if (it.rn) tp_tma_box(st + TP_LREG * 8u, it.mapR, it.col0, rk + s * TP_KS, ritem, &full[b]);
-        else tp_tma_box(st + TP_LREG * 8u, it.mapR, s * TP_KS, it.col0, ritem, &full[b]);
+    for (int item = item0; item < item1; ++item) {
+      const TpItem it = tp_decode(slices, nslices, pass, tasks, maps, scratch, partial, item);
+      const unsigned bytes = (unsigned)(((it.lt ? TP_LBOX_M : TP_LBOX_K) + (it.rn ? TP_RBOX_N : TP_RBOX_K)) * sizeof(double));
+      const int nsteps = (it.K + TP_KS - 1) / TP_KS;
+      for (int pl = 0; pl < it.npl; ++pl) {
+        const int lrow = it.row0 + it.l_row + pl * it.l_row_step, litem = it.l_item + pl * it.l_item_step;
+        const int rk = it.r_k + pl * it.r_k_step, ritem = it.r_item + pl * it.r_item_step;
+        for (int s = 0; s < nsteps; ++s, ++step) {
+          const int b = step % TP_NS, round = step / TP_NS;
+          if (round > 0) tp_mbar_wait(&empty[b], (round - 1) & 1);
+          tp_mbar_expect(&full[b], bytes);
+          const unsigned st = tp_smem_u32(smem + (size_t)b * TP_STAGE);
+          if (it.lt) tp_tma_box(st, it.mapL, lrow, s * TP_KS, litem, &full[b]);
+          else tp_tma_box(st, it.mapL, s * TP_KS, lrow, litem, &full[b]);
+          if (it.rn) tp_tma_box(st + TP_LREG * 8u, it.mapR, it.col0, rk + s * TP_KS, ritem, &full[b]);
+          else tp_tma_box(st + TP_LREG * 8u, it.mapR, s * TP_KS, it.col0, ritem, &full[b]);
+        }
       }
     }
     return;
   }
-  if (it.lt) tp_consume_ni<true, true>(it, smem, full, empty, warp, lane);     // Aop read transposed: R is E or T (columns contiguous)
-  else if (it.rn) tp_consume_ni<false, true>(it, smem, full, empty, warp, lane);
-  else tp_consume_ni<false, false>(it, smem, full, empty, warp, lane);
+  for (int item = item0; item < item1; ++item) {
+    const TpItem it = tp_decode(slices, nslices, pass, tasks, maps, scratch, partial, item);
+    if (it.lt) tp_consume_ni<true, true>(it, smem, full, empty, warp, lane, step);     // Aop read transposed: R is E or T (columns contiguous)
+    else if (it.rn) tp_consume_ni<false, true>(it, smem, full, empty, warp, lane, step);
+    else tp_consume_ni<false, false>(it, smem, full, empty, warp, lane, step);
+  }
 }
 
 // F_s += partial slabs in index order: fixed order, one thread per element (row a5).
@@ -317,6 +355,32 @@ int tp_tile_cols_executed(int N) {
   return full * TP_TN + (rem ? 16 * tp_nj_for(rem) : 0);
 }
 
+static su2_status tp_set_attr() {
+  static bool attr_done[64] = {};
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (!attr_done[dev & 63]) {
+    cudaError_t e = cudaFuncSetAttribute(tp_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TP_SMEM);
+    if (e != cudaSuccess) { set_cuda_error("cudaFuncSetAttribute(tp_gemm_kernel)", (int)e); return SU2_ERR_CUDA; }
+    attr_done[dev & 63] = true;
+  }
+  return SU2_OK;
+}
+
+su2_status launch_tp_gemm(const TpSlice* slices, int nslices, int pass, int nitems, int ipc, const DevTask* tasks, const void* maps,
+                          double* scratch, double* partial, void* stream_v) {
+  su2_status st = tp_set_attr();
+  if (st != SU2_OK) return st;
+  if (nitems <= 0) return SU2_OK;
+  ipc = std::max(1, ipc);
+  tp_gemm_kernel<<<(nitems + ipc - 1) / ipc, TP_THREADS, TP_SMEM, (cudaStream_t)stream_v>>>(slices, nslices, pass, nitems, ipc, tasks,
+                                                                                           (const CUtensorMap*)maps, scratch, partial);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { set_cuda_error("tp_gemm_kernel launch", (int)e); return SU2_ERR_CUDA; }
+  count_launch();
+  return SU2_OK;
+}
+
 su2_status launch_heff_two_pass(const su2_plan* plan, double* out, double* tp_partial, void* stream_v) {
   cudaStream_t stream = (cudaStream_t)stream_v;
   if (plan->h_tp_groups.empty()) return SU2_OK;
@@ -330,10 +394,10 @@ su2_status launch_heff_two_pass(const su2_plan* plan, double* out, double* tp_pa
   }
   for (const TpGroup& g : plan->h_tp_groups) {
     const int ns = g.slice1 - g.slice0;
-    tp_gemm_kernel<<<g.items1, TP_THREADS, TP_SMEM, stream>>>(plan->d_tp_slices + g.slice0, ns, 0, plan->d_tasks, (const CUtensorMap*)plan->d_maps,
-                                                             plan->d_tp_scratch, tp_partial);
-    tp_gemm_kernel<<<g.items2, TP_THREADS, TP_SMEM, stream>>>(plan->d_tp_slices + g.slice0, ns, 1, plan->d_tasks, (const CUtensorMap*)plan->d_maps,
-                                                             plan->d_tp_scratch, tp_partial);
+    tp_gemm_kernel<<<(g.items1 + g.ipc1 - 1) / g.ipc1, TP_THREADS, TP_SMEM, stream>>>(plan->d_tp_slices + g.slice0, ns, 0, g.items1, g.ipc1, plan->d_tasks,
+                                                                                     (const CUtensorMap*)plan->d_maps, plan->d_tp_scratch, tp_partial);
+    tp_gemm_kernel<<<g.items2, TP_THREADS, TP_SMEM, stream>>>(plan->d_tp_slices + g.slice0, ns, 1, g.items2, 1, plan->d_tasks,
+                                                             (const CUtensorMap*)plan->d_maps, plan->d_tp_scratch, tp_partial);
     dim3 grid(64, (unsigned)(g.red1 - g.red0));
     tp_reduce_kernel<<<grid, 256, 0, stream>>>(plan->d_tp_reduce + g.red0, tp_partial, out);
     cudaError_t e = cudaGetLastError();

@@ -215,6 +215,8 @@ extern "C" su2_status su2_plan_create_opts(su2_plan** out, const su2_problem* p,
   if (opt.two_pass_min_dim == 0) opt.two_pass_min_dim = 1;
   if (opt.two_pass_scratch_bytes == 0) opt.two_pass_scratch_bytes = (int64_t)16 << 30;
   if (opt.two_pass_chunk_k == 0) opt.two_pass_chunk_k = 8192;
+  if (opt.two_pass_ipc_k < 0) return SU2_ERR_INVALID_ARGUMENT;
+  if (opt.two_pass_ipc_k == 0) opt.two_pass_ipc_k = 2048;
   const auto t_start = std::chrono::steady_clock::now();
 
   su2_plan* plan = new su2_plan();
@@ -827,11 +829,20 @@ extern "C" su2_status su2_plan_create_opts(su2_plan** out, const su2_problem* p,
     if (need < (double)cap) cap = std::max<int64_t>((int64_t)need, min_need);
     plan->tp_scratch_elems = need > 0.0 ? cap : 0;
     int64_t cur = 0, part_cur = 0, items1 = 0, items2 = 0;
+    double k1_sum = 0.0;   // inner extent of the first product summed over the pass-1 items of the group
     TpGroup grp{};
     auto close_group = [&]() {
       grp.slice1 = (int32_t)plan->h_tp_slices.size();
       grp.red1 = (int32_t)plan->h_tp_reduce.size();
       grp.items1 = (int32_t)items1; grp.items2 = (int32_t)items2;
+      // pass-1 items per CTA: a K loop of about two_pass_ipc_k in total per CTA, at least ~8 waves of CTAs per launch
+      {
+        const double k1 = items1 > 0 ? k1_sum / (double)items1 : 1.0;
+        int64_t ipc = (int64_t)std::lround((double)opt.two_pass_ipc_k / std::max(1.0, k1));
+        ipc = std::min<int64_t>(ipc, items1 / (8 * 296));
+        grp.ipc1 = (int32_t)std::max<int64_t>(1, std::min<int64_t>(ipc, 64));
+      }
+      k1_sum = 0.0;
       if (grp.slice1 > grp.slice0) plan->h_tp_groups.push_back(grp);
       plan->tp_partial_elems = std::max(plan->tp_partial_elems, part_cur);
       grp.slice0 = grp.slice1; grp.red0 = grp.red1;
@@ -870,6 +881,7 @@ extern "C" su2_status su2_plan_create_opts(su2_plan** out, const su2_problem* p,
         sl.item1 = (int32_t)items1; sl.item2 = (int32_t)items2;
         sl.part_off = part_cur;
         items1 += tiles1 * take;
+        k1_sum += (double)(o1 ? ht.n : ht.k) * (double)(tiles1 * take);
         items2 += tiles2 * sl.nchunk;
         if (last_sec == ht.out_sec) {
           plan->h_tp_reduce.back().nslab += sl.nchunk;

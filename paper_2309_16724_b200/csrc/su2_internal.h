@@ -103,9 +103,15 @@ struct TpSlice {
   int32_t item1, item2;             // first pass-1 / pass-2 item (CTA) of the slice inside its group
   int32_t chunk, nchunk;            // positions per pass-2 item; number of chunks (= partial slabs) of the slice
   int64_t part_off;                 // element offset of the slice's first partial slab in the workspace's two-pass area
+  int32_t flags, pad;               // TP_SLICE_* (0 inside H_eff * Psi)
 };
+// su2_gemm_pair_batched on the same kernel (gemm_two_pass.cu): the "positions" are the batch items, each with its own E
+// (third coordinate of the E map = position) and its own output C_pos = C_pos + T_pos Dop_pos^T (chunk = 1, the accumulators
+// start from C_pos instead of zero, slabs are the dense m x p outputs themselves)
+enum : int32_t { TP_SLICE_E_PER_POS = 1, TP_SLICE_ACCUMULATE = 2 };
 struct TpGroup {                    // host only
   int32_t slice0, slice1, items1, items2, red0, red1;
+  int32_t ipc1;                     // pass-1 items per CTA (consecutive items, pipeline kept full across them)
 };
 // F_s += sum of nslab partial slabs in index order (slabs of slab elements each, the first at part_off)
 struct TpReduce {
@@ -221,6 +227,9 @@ struct MapKey {
 su2_status encode_tensor_map(void* out128, const MapKey& key);   // host; SU2_ERR_CUDA if the driver refuses
 int tp_tile_rows_executed(int M);   // rows / columns the tiles of tp_gemm_kernel multiply for an M-row / N-column output
 int tp_tile_cols_executed(int N);
+// one launch of tp_gemm_kernel on caller-built tables (device pointers): pass 0 / 1, nitems items, ipc items per CTA
+su2_status launch_tp_gemm(const TpSlice* slices, int nslices, int pass, int nitems, int ipc, const DevTask* tasks, const void* maps,
+                          double* scratch, double* partial, void* stream);
 su2_status launch_heff_two_pass(const su2_plan* plan, double* out, double* tp_partial, void* stream);   // heff_two_pass.cu
 su2_status launch_heff_small(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream);   // heff_small.cu
 su2_status launch_apply(const su2_plan* plan, const double* psi, double* out, double* partial, void* stream);

@@ -151,3 +151,36 @@ def test_planner_wigner_symbols_equal_exact_arithmetic_up_to_the_spin_cap(lib):
     with pytest.raises(Su2Error) as info:
         Plan(prob, host_only=True)
     assert "status -3" in str(info.value)
+
+
+def test_two_pass_route_planning(lib):
+    """Host side of the two-pass route (SU2_PLAN_TWO_PASS, the default of large-tile plans): which tasks take it, how the
+    scratch cap cuts them into launch groups, what it adds to the workspace, and that bad options are refused."""
+    from paper_2309_16724_b200 import Plan, Su2Error
+    prob = config_problem("midi")
+    small = Plan(prob, host_only=True)                                   # every sector <= 48 multiplets: small-block kernel
+    assert small.info["small_plan"] == 1 and small.info["two_pass_tasks"] == 0 and small.info["two_pass_groups"] == 0
+    tp = Plan(prob, host_only=True, large_tiles=True)
+    assert tp.info["small_plan"] == 0 and tp.info["two_pass_tasks"] == tp.info["ntasks"] and tp.info["two_pass_groups"] == 1
+    assert tp.info["cc_flops"] == small.info["cc_flops"] and tp.info["ntask_positions"] == small.info["ntask_positions"]
+    assert tp.info["two_pass_scratch_bytes"] > 0 and tp.workspace_bytes % 256 == 0
+    fused = Plan(prob, host_only=True, large_tiles=True, fused=True)
+    assert fused.info["two_pass_tasks"] == 0 and fused.info["two_pass_scratch_bytes"] == 0 and fused.info["nwork_items"] > 0
+    paced = Plan(prob, host_only=True, large_tiles=True, gang_pacing=True)       # pacing is the fused kernel's: implies it
+    assert paced.info["two_pass_tasks"] == 0
+    # a scratch of 16 KB: many groups, the same tasks, the same CC; never less than one position of the largest task
+    cut = Plan(prob, host_only=True, large_tiles=True, two_pass_scratch_bytes=16384, two_pass_chunk_k=24)
+    assert cut.info["two_pass_groups"] > 100 and cut.info["two_pass_tasks"] == tp.info["ntasks"]
+    assert cut.info["two_pass_scratch_bytes"] >= 16384 and cut.info["cc_flops"] == tp.info["cc_flops"]
+    tiny = Plan(prob, host_only=True, large_tiles=True, two_pass_scratch_bytes=8)
+    dmax = max(s.dim for s in prob.sec_l + prob.sec_r)
+    assert 8 < tiny.info["two_pass_scratch_bytes"] <= 8 * (dmax * (dmax + 3) + 2 * (dmax + 3))
+    # hybrid: only tasks whose four extents reach min_dim leave the fused kernel
+    hyb = Plan(prob, host_only=True, large_tiles=True, two_pass_min_dim=10)
+    assert 0 < hyb.info["two_pass_tasks"] < hyb.info["ntasks"]
+    # executed flops: the cheaper product order and narrow edge tiles; never below CC
+    assert tp.info["executed_flops"] >= tp.info["cc_flops"]
+    with pytest.raises(Su2Error):
+        Plan(prob, host_only=True, large_tiles=True, two_pass_min_dim=-1)
+    with pytest.raises(Su2Error):
+        Plan(prob, host_only=True, large_tiles=True, two_pass_scratch_bytes=-5)
