@@ -7,7 +7,7 @@
 //   pass 2:  partial[chunk] = sum_{pos in chunk} T_pos Dop_pos^T   (K loop over (pos, n))     (order 1: sum_pos Aop_pos T_pos)
 //   reduce:  F_s += partial slabs in index order (deterministic, no atomics; row a5)
 // Why: on sm_100a what decides DMMA throughput is the register tile of a warp and the number of independent CTAs per SM
-// (profiles/r02_cfg5_shapes.md, r02_two_pass_kernel.md): four warps of 32 x 64, two CTAs per SM reach 90-95 % of the pipe, the
+// (profiles/r02_cfg5_shapes.md, r02_two_pass_route.md): four warps of 32 x 64, two CTAs per SM reach 90-95 % of the pipe, the
 // fused kernel (heff_tma.cu: both products' accumulators in registers, T chunk in shared memory, one CTA per SM) 79 %.  T costs
 // 16 bytes of HBM traffic per entry against 2 (k + p) flops.
 //
@@ -333,13 +333,20 @@ tp_gemm_kernel(const TpSlice* __restrict__ slices, int nslices, int pass, int ni
   }
 }
 
-// F_s += partial slabs in index order: fixed order, one thread per element (row a5).
+// F_s += partial slabs in index order: fixed order, one thread per element (row a5).  HBM-bound: the slabs of four
+// consecutive chunks are fetched before they are added (the additions stay in index order).
 __global__ void __launch_bounds__(256)
 tp_reduce_kernel(const TpReduce* __restrict__ red, const double* __restrict__ partial, double* __restrict__ out) {
   const TpReduce r = red[blockIdx.y];
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < r.size; i += (int64_t)gridDim.x * blockDim.x) {
     double s = out[r.f_off + i];
-    for (int g = 0; g < r.nslab; ++g) s += partial[r.part_off + (int64_t)g * r.slab + i];
+    const double* __restrict__ q = partial + r.part_off + i;
+    int g = 0;
+    for (; g + 4 <= r.nslab; g += 4) {
+      const double a = q[(int64_t)g * r.slab], b = q[(int64_t)(g + 1) * r.slab], c = q[(int64_t)(g + 2) * r.slab], d = q[(int64_t)(g + 3) * r.slab];
+      s += a; s += b; s += c; s += d;
+    }
+    for (; g < r.nslab; ++g) s += q[(int64_t)g * r.slab];
     out[r.f_off + i] = s;
   }
 }
@@ -398,7 +405,7 @@ su2_status launch_heff_two_pass(const su2_plan* plan, double* out, double* tp_pa
                                                                                      (const CUtensorMap*)plan->d_maps, plan->d_tp_scratch, tp_partial);
     tp_gemm_kernel<<<g.items2, TP_THREADS, TP_SMEM, stream>>>(plan->d_tp_slices + g.slice0, ns, 1, g.items2, 1, plan->d_tasks,
                                                              (const CUtensorMap*)plan->d_maps, plan->d_tp_scratch, tp_partial);
-    dim3 grid(64, (unsigned)(g.red1 - g.red0));
+    dim3 grid(296, (unsigned)(g.red1 - g.red0));   // few records per group (often one output sector): many CTAs per record
     tp_reduce_kernel<<<grid, 256, 0, stream>>>(plan->d_tp_reduce + g.red0, tp_partial, out);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { set_cuda_error("two-pass launch", (int)e); return SU2_ERR_CUDA; }

@@ -610,11 +610,14 @@ def test_gemm_pair_batched(m, k, n, p, batch):
 
 
 @pytest.mark.parametrize("m,k,n,p,batch", [(64, 20, 128, 128, 2), (256, 256, 256, 256, 3), (300, 260, 258, 384, 2), (70, 33, 45, 129, 5),
-                                           (131, 577, 99, 250, 2), (1, 1, 1, 1, 3), (65, 21, 129, 2, 4), (512, 512, 512, 512, 2)])
+                                           (131, 577, 99, 250, 2), (1, 1, 1, 1, 3), (65, 21, 129, 2, 4), (512, 512, 512, 512, 2),
+                                           (48, 200, 48, 52, 700), (200, 48, 300, 49, 40), (128, 128, 128, 128, 300)])
 def test_gemm_pair_two_pass_route(m, k, n, p, batch):
-    """Route 4 (gemm_two_pass.cu): T = A X through a scratch, C += alpha T B^T, both on dgemm_tma_kernel (K-major and N-major
-    right operands, ragged tiles, K tails, odd leading dimensions re-pitched, beta epilogue), against numpy; the automatic
-    route (which picks it for items >= 256 that its 64 x 128 tiles fit) gives the same bits as the explicit one."""
+    """Route 4 (gemm_two_pass.cu): the batch items as the positions of one task on tp_gemm_kernel (heff_two_pass.cu) -- T through
+    a scratch in the cheaper product order (A X first or X B^T first: both occur below), own X and own output per item,
+    accumulators initialised from C, ragged edge tiles, K tails, odd leading dimensions re-pitched, several items per CTA (the
+    batches of hundreds) -- against numpy; the automatic route (which picks it from 48 in every extent up) gives the same bits
+    as the explicit one."""
     torch = _torch()
     from paper_2309_16724_b200 import gemm_pair_batched
     rng = np.random.default_rng(m * 1000 + p + 1)
@@ -625,7 +628,7 @@ def test_gemm_pair_two_pass_route(m, k, n, p, batch):
     gemm_pair_batched(m, k, n, p, batch, 0.5, dA.data_ptr(), dX.data_ptr(), dB.data_ptr(), dC.data_ptr(), st, 4)
     ref = C0 + 0.5 * np.matmul(np.matmul(A, X), np.swapaxes(B, 1, 2))
     assert _rel(dC.cpu().numpy(), ref) <= 1e-12
-    if min(m, k, n, p) >= 256 and m % 64 == 0 and n % 128 == 0 and p % 128 == 0:      # shapes the automatic route sends here
+    if min(m, k, n, p) >= 48:      # shapes the automatic route sends here
         auto = torch.from_numpy(C0).cuda()
         gemm_pair_batched(m, k, n, p, batch, 0.5, dA.data_ptr(), dX.data_ptr(), dB.data_ptr(), auto.data_ptr(), st)
         assert torch.equal(auto, dC)
