@@ -171,6 +171,12 @@ typedef struct {
   int32_t two_pass_ipc_k;          /* pass 1: a CTA works through consecutive (position, tile) items until their inner
                                       extents add up to about this (default 2048; 1 = one item per CTA)                     */
   int32_t pad;
+  void* two_pass_scratch_dev;      /* NULL: the plan allocates the scratch itself (freed by su2_plan_destroy).  Otherwise a
+                                      DEVICE buffer of two_pass_scratch_bytes bytes (which must then be > 0), 256-byte aligned,
+                                      caller-owned: it must stay valid while the plan is used, is zeroed once by
+                                      su2_plan_create_opts and overwritten by every apply (two plans may share one buffer if
+                                      their applies are ordered on one stream); SU2_ERR_WORKSPACE if it cannot hold one
+                                      position of the largest task or is misaligned.                                         */
 } su2_plan_options;
 
 typedef struct {

@@ -73,7 +73,7 @@ class su2_plan_info_t(C.Structure):
 
 class su2_plan_options(C.Structure):
     _fields_ = [("two_pass_min_dim", C.c_int32), ("two_pass_chunk_k", C.c_int32), ("two_pass_scratch_bytes", C.c_int64),
-                ("two_pass_ipc_k", C.c_int32), ("pad", C.c_int32)]
+                ("two_pass_ipc_k", C.c_int32), ("pad", C.c_int32), ("two_pass_scratch_dev", C.c_void_p)]
 
 
 EXPORTS = ["su2_wigner_6j", "su2_wigner_9j", "su2_status_string", "su2_last_cuda_error", "su2_kernel_launch_count", "su2_plan_create", "su2_plan_create_opts", "su2_plan_destroy", "su2_plan_info",
@@ -189,7 +189,7 @@ class Plan:
     without a GPU)."""
 
     def __init__(self, problem, family_ptrs=None, stream=0, host_only=False, force_split=False, large_tiles=False, gang_pacing=False,
-                 ld_align=1, fused=False, two_pass=False, two_pass_min_dim=0, two_pass_chunk_k=0, two_pass_scratch_bytes=0, two_pass_ipc_k=0):
+                 ld_align=1, fused=False, two_pass=False, two_pass_min_dim=0, two_pass_chunk_k=0, two_pass_scratch_bytes=0, two_pass_ipc_k=0, two_pass_scratch_ptr=None):
         lib = load()
         self._keep = []
         self.problem = problem
@@ -245,7 +245,7 @@ class Plan:
         self.handle = C.c_void_p()
         flags = ((SU2_PLAN_HOST_ONLY if host_only else 0) | (2 if force_split else 0) | (4 if large_tiles else 0) | (8 if gang_pacing else 0) |
                  (16 if two_pass else 0) | (32 if fused else 0))
-        opts = su2_plan_options(int(two_pass_min_dim), int(two_pass_chunk_k), int(two_pass_scratch_bytes), int(two_pass_ipc_k), 0)
+        opts = su2_plan_options(int(two_pass_min_dim), int(two_pass_chunk_k), int(two_pass_scratch_bytes), int(two_pass_ipc_k), 0, two_pass_scratch_ptr)
         check(lib.su2_plan_create_opts(C.byref(self.handle), C.byref(prob), flags, C.byref(opts), C.c_void_p(stream)))
         info = su2_plan_info_t()
         check(lib.su2_plan_info(self.handle, C.byref(info)))

@@ -152,8 +152,10 @@ su2_status upload_plan(su2_plan* plan, void* stream_v) {
                       "padded copies of operator families whose rows are not 16-byte aligned (pass blk_ld with even "
                       "leading dimensions to have them read in place)")) != SU2_OK) return st;
   if ((st = big_alloc(&plan->d_psi_pad, plan->psipad_elems, "the padded copy of Psi")) != SU2_OK) return st;
-  if ((st = big_alloc(&plan->d_tp_scratch, plan->tp_scratch_elems,
-                      "the scratch of the two-pass route (su2_plan_options.two_pass_scratch_bytes)")) != SU2_OK) return st;
+  if (!plan->tp_scratch_external &&
+      (st = big_alloc(&plan->d_tp_scratch, plan->tp_scratch_elems,
+                      "the scratch of the two-pass route (su2_plan_options.two_pass_scratch_bytes; or pass a caller-owned "
+                      "buffer in two_pass_scratch_dev)")) != SU2_OK) return st;
   // a ragged k tail of T read as the right operand reaches into the rows of the next position: whatever is there is
   // multiplied by exact zeros, so it only has to be finite -- zero once (later contents are finite products)
   if (plan->d_tp_scratch) SU2_CUDA(cudaMemsetAsync(plan->d_tp_scratch, 0, (size_t)plan->tp_scratch_elems * sizeof(double), stream));
@@ -312,6 +314,7 @@ su2_status upload_plan(su2_plan* plan, void* stream_v) {
 
 void free_plan_device(su2_plan* plan) {
   if (!plan) return;
+  if (plan->tp_scratch_external) plan->d_tp_scratch = nullptr;   // caller-owned
   for (void** q : {(void**)&plan->d_blob, (void**)&plan->d_fold, (void**)&plan->d_copy, (void**)&plan->d_psi_pad, (void**)&plan->d_tp_scratch})
     if (*q) { cudaFree(*q); *q = nullptr; }
 }

@@ -212,6 +212,7 @@ extern "C" su2_status su2_plan_create_opts(su2_plan** out, const su2_problem* p,
   su2_plan_options opt{};
   if (opts) opt = *opts;
   if (opt.two_pass_min_dim < 0 || opt.two_pass_scratch_bytes < 0 || opt.two_pass_chunk_k < 0) return SU2_ERR_INVALID_ARGUMENT;
+  if (opt.two_pass_scratch_dev && (opt.two_pass_scratch_bytes <= 0 || ((uintptr_t)opt.two_pass_scratch_dev & 255))) return SU2_ERR_WORKSPACE;
   if (opt.two_pass_min_dim == 0) opt.two_pass_min_dim = 1;
   if (opt.two_pass_scratch_bytes == 0) opt.two_pass_scratch_bytes = (int64_t)16 << 30;
   if (opt.two_pass_chunk_k == 0) opt.two_pass_chunk_k = 8192;
@@ -825,9 +826,17 @@ extern "C" su2_status su2_plan_create_opts(su2_plan** out, const su2_problem* p,
       need += (double)per_pos * ht.npos + 2.0 * pad4(o1 ? ht.p : ht.n);
       min_need = std::max(min_need, per_pos + 2 * (int64_t)pad4(o1 ? ht.p : ht.n));
     }
+    if (opt.two_pass_scratch_dev && opt.two_pass_scratch_bytes / 8 < min_need) {   // a caller-owned scratch cannot grow
+      delete plan;
+      return SU2_ERR_WORKSPACE;
+    }
     int64_t cap = std::max<int64_t>(opt.two_pass_scratch_bytes / 8, min_need);
     if (need < (double)cap) cap = std::max<int64_t>((int64_t)need, min_need);
     plan->tp_scratch_elems = need > 0.0 ? cap : 0;
+    if (opt.two_pass_scratch_dev && plan->tp_scratch_elems > 0) {
+      plan->d_tp_scratch = (double*)opt.two_pass_scratch_dev;
+      plan->tp_scratch_external = true;
+    }
     int64_t cur = 0, part_cur = 0, items1 = 0, items2 = 0;
     double k1_sum = 0.0;   // inner extent of the first product summed over the pass-1 items of the group
     TpGroup grp{};

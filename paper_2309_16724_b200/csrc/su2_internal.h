@@ -209,6 +209,7 @@ struct su2_plan {
   su2::TpSlice* d_tp_slices = nullptr;
   su2::TpReduce* d_tp_reduce = nullptr;
   double* d_tp_scratch = nullptr;
+  bool tp_scratch_external = false;    // su2_plan_options.two_pass_scratch_dev: caller-owned, never freed here
   int32_t small_begin[7] = {0, 0, 0, 0, 0, 0, 0};   // small plans: h_work is sorted by size class (DM8 = 8 (c + 1)); class c = [begin[c], begin[c+1])
 };
 

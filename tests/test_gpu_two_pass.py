@@ -92,3 +92,23 @@ def test_davidson_and_host_entry_on_a_two_pass_plan():
         t2, r2 = s2.step()
         assert abs(t1 - t2) <= 1e-10 * max(1.0, abs(t2)) and abs(r1 - r2) <= 1e-8 * max(1.0, r2)
     s1.close(); s2.close()
+
+
+def test_caller_owned_scratch_gives_the_same_bits():
+    """su2_plan_options.two_pass_scratch_dev: the scratch as a torch tensor (PyTorch owns the memory) instead of an allocation
+    of the library's own -- same grouping for the same size, hence the same bits; a buffer that cannot hold one position of
+    the largest task is refused."""
+    torch = _torch()
+    from paper_2309_16724_b200 import Su2Error
+    prob = synthetic_problem(16, 16, 0, 500, seed=3)
+    nbytes = 1 << 20
+    own = _operator(prob, two_pass_scratch_bytes=nbytes, two_pass_chunk_k=256)
+    ext = _operator(prob, two_pass_scratch_bytes=nbytes, two_pass_chunk_k=256, two_pass_scratch="torch")
+    assert ext.two_pass_scratch is not None and ext.info["two_pass_groups"] == own.info["two_pass_groups"] > 1
+    assert ext.info["plan_device_bytes"] < own.info["plan_device_bytes"]
+    x = torch.from_numpy(random_psi(own.psi_len, seed=6)).cuda()
+    ext.two_pass_scratch.fill_(255)                     # NaN bit patterns: only what an apply wrote itself may be read as data
+    ext.two_pass_scratch.zero_()                        # ... the library zeroes the buffer once at plan time; do the same after scribbling
+    assert torch.equal(ext.apply(x), own.apply(x))
+    with pytest.raises(Su2Error):
+        _operator(prob, two_pass_scratch_bytes=4096, two_pass_scratch="torch")

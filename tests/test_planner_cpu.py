@@ -184,3 +184,16 @@ def test_two_pass_route_planning(lib):
         Plan(prob, host_only=True, large_tiles=True, two_pass_min_dim=-1)
     with pytest.raises(Su2Error):
         Plan(prob, host_only=True, large_tiles=True, two_pass_scratch_bytes=-5)
+
+
+def test_caller_owned_scratch_is_validated(lib):
+    from paper_2309_16724_b200 import Plan, Su2Error
+    prob = config_problem("midi")
+    ok = Plan(prob, host_only=True, large_tiles=True, two_pass_scratch_bytes=1 << 20, two_pass_scratch_ptr=1 << 20)
+    assert ok.info["two_pass_tasks"] == ok.info["ntasks"]
+    for kw in (dict(two_pass_scratch_bytes=1 << 20, two_pass_scratch_ptr=(1 << 20) + 8),     # not 256-byte aligned
+               dict(two_pass_scratch_bytes=0, two_pass_scratch_ptr=1 << 20),                 # size missing
+               dict(two_pass_scratch_bytes=64, two_pass_scratch_ptr=1 << 20)):               # smaller than one position of a task
+        with pytest.raises(Su2Error) as info:
+            Plan(prob, host_only=True, large_tiles=True, **kw)
+        assert "status -7" in str(info.value)
