@@ -212,21 +212,45 @@ __host__ __device__ __forceinline__ int tp_nj_for(int rem) {
   return rem >= TP_TN ? 8 : (rem + 15) / 16;
 }
 
-// What item `item` of a launch is: which slice (binary search over the slices' first items), which tile, which positions.
+// The producer's memory of the slice it is in: the items of a CTA are consecutive, so slice and task records are fetched once
+// per slice, not once per item.
+struct TpCache {
+  int lo = -1, end = 0;     // slice index; first item beyond the slice
+  TpSlice sl;
+  int m, k, n, p, transA, transD, stepA, stepD;
+  double coef;
+  const double* alpha;
+};
+
+// What item `item` of a launch is: which slice (binary search over the slices' first items for the first item of a CTA, then
+// the next slices in order), which tile, which positions.  Called by the producer thread only; the consumers get the result
+// through shared memory (tp_gemm_kernel).
 __device__ __forceinline__ TpItem tp_decode(const TpSlice* __restrict__ slices, int nslices, int pass, const DevTask* __restrict__ tasks,
                                             const CUtensorMap* __restrict__ maps, double* __restrict__ scratch,
-                                            double* __restrict__ partial, int item) {
-  // ---- which slice, which item of it (binary search over the slices' first items)
-  int lo = 0, hi = nslices - 1;
-  while (lo < hi) {
-    const int mid = (lo + hi + 1) >> 1;
-    if ((pass ? slices[mid].item2 : slices[mid].item1) <= item) lo = mid; else hi = mid - 1;
+                                            double* __restrict__ partial, int item, TpCache& c) {
+  if (c.lo < 0 || item >= c.end) {
+    if (c.lo < 0) {
+      int hi = nslices - 1;
+      c.lo = 0;
+      while (c.lo < hi) {
+        const int mid = (c.lo + hi + 1) >> 1;
+        if ((pass ? slices[mid].item2 : slices[mid].item1) <= item) c.lo = mid; else hi = mid - 1;
+      }
+    } else {
+      while (c.lo + 1 < nslices && (pass ? slices[c.lo + 1].item2 : slices[c.lo + 1].item1) <= item) ++c.lo;
+    }
+    c.end = c.lo + 1 < nslices ? (pass ? slices[c.lo + 1].item2 : slices[c.lo + 1].item1) : 0x7fffffff;
+    c.sl = slices[c.lo];
+    const DevTask* __restrict__ tk = tasks + c.sl.task;
+    c.m = tk->m; c.k = tk->k; c.n = tk->n; c.p = tk->p;
+    c.transA = (tk->flags & TASK_TRANS_A) != 0; c.transD = (tk->flags & TASK_TRANS_D) != 0;
+    c.stepA = tk->strideA != 0; c.stepD = tk->strideD != 0;
+    c.coef = tk->coef; c.alpha = tk->alpha;
   }
-  const TpSlice sl = slices[lo];
-  const DevTask* __restrict__ tk = tasks + sl.task;
-  const int m = tk->m, k = tk->k, n = tk->n, p = tk->p;
-  const bool transA = tk->flags & TASK_TRANS_A, transD = tk->flags & TASK_TRANS_D;
-  const int stepA = tk->strideA != 0, stepD = tk->strideD != 0;
+  const TpSlice& sl = c.sl;
+  const int m = c.m, k = c.k, n = c.n, p = c.p;
+  const bool transA = c.transA, transD = c.transD;
+  const int stepA = c.stepA, stepD = c.stepD;
   const int local = item - (pass ? sl.item2 : sl.item1);
   TpItem it;
   int pl0;   // first position (relative to the slice) of the item
@@ -250,8 +274,8 @@ __device__ __forceinline__ TpItem tp_decode(const TpSlice* __restrict__ slices, 
     pl0 = outer;
     it.npl = 1;
     it.acc_init = 0;
-    const double al = tk->alpha ? tk->alpha[sl.pos0 + pl0] : 1.0;
-    it.scale = tk->coef * al;
+    const double al = c.alpha ? c.alpha[sl.pos0 + pl0] : 1.0;
+    it.scale = c.coef * al;
     it.dst = scratch + ((int64_t)sl.t_row0 + (int64_t)pl0 * rowsT) * sl.ldt;
     it.ldd = sl.ldt;
     if (sl.order == 0) {   // T = Aop E
@@ -282,14 +306,17 @@ __device__ __forceinline__ TpItem tp_decode(const TpSlice* __restrict__ slices, 
 
 // pass = 0: T_pos of every position of the group's slices; pass = 1: the partial slabs.  Items are numbered over the group;
 // CTA b works through items [b ipc, (b + 1) ipc) one after the other WITHOUT draining its pipeline in between: the producer
-// thread and the consumer warps decode the items independently and count the same stages, so the producer is already staging
-// the next item while the consumers store the current one (pass 1 of small blocks: a CTA's start-up is spread over ipc items).
+// thread decodes the items (tables in global memory) and hands each descriptor to the consumer warps through shared memory
+// together with the item's first stage; both sides count the same stages, so the producer is already staging the next item
+// while the consumers store the current one (pass 1 of small blocks: a CTA's start-up is spread over ipc items, and the
+// consumers never wait for a table look-up).
 __global__ void __launch_bounds__(TP_THREADS, 2)
 tp_gemm_kernel(const TpSlice* __restrict__ slices, int nslices, int pass, int nitems, int ipc, const DevTask* __restrict__ tasks,
                const CUtensorMap* __restrict__ maps, double* __restrict__ scratch, double* __restrict__ partial) {
   extern __shared__ __align__(1024) double smem[];
   __shared__ __align__(8) uint64_t full[TP_NS];
   __shared__ __align__(8) uint64_t empty[TP_NS];
+  __shared__ __align__(16) TpItem ring[4];        // item descriptors, producer -> consumers (TP_NS + 1 slots)
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   if (tid == 0) {
     for (int i = 0; i < TP_NS; ++i) {
@@ -302,10 +329,11 @@ tp_gemm_kernel(const TpSlice* __restrict__ slices, int nslices, int pass, int ni
   const int item0 = blockIdx.x * ipc, item1 = min(nitems, item0 + ipc);
   int step = 0;
   if (warp == TP_CONSUMERS) {
-    // ---- producer: one thread, two boxes per stage
+    // ---- producer: one thread; per item: decode, publish the descriptor, then two boxes per stage
     if (lane != 0) return;
+    TpCache cache;
     for (int item = item0; item < item1; ++item) {
-      const TpItem it = tp_decode(slices, nslices, pass, tasks, maps, scratch, partial, item);
+      const TpItem it = tp_decode(slices, nslices, pass, tasks, maps, scratch, partial, item, cache);
       const unsigned bytes = (unsigned)(((it.lt ? TP_LBOX_M : TP_LBOX_K) + (it.rn ? TP_RBOX_N : TP_RBOX_K)) * sizeof(double));
       const int nsteps = (it.K + TP_KS - 1) / TP_KS;
       for (int pl = 0; pl < it.npl; ++pl) {
@@ -314,6 +342,10 @@ tp_gemm_kernel(const TpSlice* __restrict__ slices, int nslices, int pass, int ni
         for (int s = 0; s < nsteps; ++s, ++step) {
           const int b = step % TP_NS, round = step / TP_NS;
           if (round > 0) tp_mbar_wait(&empty[b], (round - 1) & 1);
+          // The descriptor goes out with the item's first stage: written after the wait above (the consumers have released a
+          // stage of item - TP_NS or later, so they are done reading slot (item - TP_NS - 1) & 3 and older) and before the
+          // arrive below, whose release / the consumers' acquire on `full` make it visible to them.
+          if (pl == 0 && s == 0) ring[(item - item0) & 3] = it;
           tp_mbar_expect(&full[b], bytes);
           const unsigned st = tp_smem_u32(smem + (size_t)b * TP_STAGE);
           if (it.lt) tp_tma_box(st, it.mapL, lrow, s * TP_KS, litem, &full[b]);
@@ -325,8 +357,10 @@ tp_gemm_kernel(const TpSlice* __restrict__ slices, int nslices, int pass, int ni
     }
     return;
   }
+  // ---- consumers: the descriptor of an item is valid once the item's first stage has landed
   for (int item = item0; item < item1; ++item) {
-    const TpItem it = tp_decode(slices, nslices, pass, tasks, maps, scratch, partial, item);
+    tp_mbar_wait(&full[step % TP_NS], (step / TP_NS) & 1);
+    const TpItem it = ring[(item - item0) & 3];
     if (it.lt) tp_consume_ni<true, true>(it, smem, full, empty, warp, lane, step);     // Aop read transposed: R is E or T (columns contiguous)
     else if (it.rn) tp_consume_ni<false, true>(it, smem, full, empty, warp, lane, step);
     else tp_consume_ni<false, false>(it, smem, full, empty, warp, lane, step);
