@@ -53,14 +53,18 @@ class HeffOperator:
                 self.family_tensors[(side, i)] = t
                 ptrs[(side, i)] = t.data_ptr()
         self.stream = torch.cuda.current_stream(self.device)
-        # two_pass_scratch="torch": the scratch of the two-pass route is a torch tensor of two_pass_scratch_bytes bytes
-        # (PyTorch owns the memory, su2_plan_options.two_pass_scratch_dev) instead of an allocation of the library's own
+        # The scratch of the two-pass route is a torch tensor (PyTorch owns every large allocation; the plan gets its address
+        # through su2_plan_options.two_pass_scratch_dev).  Its size is what the plan itself would take: asked of a host-only
+        # plan with the same flags and options first.  two_pass_scratch="library": the plan allocates it itself.
         self.two_pass_scratch = None
-        if two_pass_opts.pop("two_pass_scratch", None) == "torch":
-            nbytes = int(two_pass_opts.get("two_pass_scratch_bytes", 0))
-            assert nbytes > 0, "two_pass_scratch='torch' needs two_pass_scratch_bytes"
-            self.two_pass_scratch = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
-            two_pass_opts["two_pass_scratch_ptr"] = self.two_pass_scratch.data_ptr()
+        if two_pass_opts.pop("two_pass_scratch", "torch") == "torch" and not fused and not gang_pacing:
+            probe = Plan(problem, family_ptrs=None, host_only=True, force_split=force_split, large_tiles=large_tiles, ld_align=ld_align,
+                         two_pass=two_pass, **two_pass_opts)
+            nbytes = int(probe.info["two_pass_scratch_bytes"])
+            del probe
+            if nbytes > 0:
+                self.two_pass_scratch = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+                two_pass_opts = dict(two_pass_opts, two_pass_scratch_bytes=nbytes, two_pass_scratch_ptr=self.two_pass_scratch.data_ptr())
         self.plan = Plan(problem, family_ptrs=ptrs, stream=self.stream.cuda_stream, force_split=force_split,
                          large_tiles=large_tiles, ld_align=ld_align, gang_pacing=gang_pacing, fused=fused, two_pass=two_pass, **two_pass_opts)
         self.psi_len = self.plan.psi_len

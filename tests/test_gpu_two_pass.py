@@ -102,13 +102,17 @@ def test_caller_owned_scratch_gives_the_same_bits():
     from paper_2309_16724_b200 import Su2Error
     prob = synthetic_problem(16, 16, 0, 500, seed=3)
     nbytes = 1 << 20
-    own = _operator(prob, two_pass_scratch_bytes=nbytes, two_pass_chunk_k=256)
-    ext = _operator(prob, two_pass_scratch_bytes=nbytes, two_pass_chunk_k=256, two_pass_scratch="torch")
-    assert ext.two_pass_scratch is not None and ext.info["two_pass_groups"] == own.info["two_pass_groups"] > 1
+    own = _operator(prob, two_pass_scratch_bytes=nbytes, two_pass_chunk_k=256, two_pass_scratch="library")
+    ext = _operator(prob, two_pass_scratch_bytes=nbytes, two_pass_chunk_k=256)          # the runtime's default: a torch tensor
+    assert own.two_pass_scratch is None and ext.two_pass_scratch is not None and ext.two_pass_scratch.numel() == ext.info["two_pass_scratch_bytes"]
+    assert ext.info["two_pass_groups"] == own.info["two_pass_groups"] > 1
     assert ext.info["plan_device_bytes"] < own.info["plan_device_bytes"]
     x = torch.from_numpy(random_psi(own.psi_len, seed=6)).cuda()
     ext.two_pass_scratch.fill_(255)                     # NaN bit patterns: only what an apply wrote itself may be read as data
     ext.two_pass_scratch.zero_()                        # ... the library zeroes the buffer once at plan time; do the same after scribbling
     assert torch.equal(ext.apply(x), own.apply(x))
+    from paper_2309_16724_b200 import Plan
+    small = torch.empty(4096, dtype=torch.uint8, device="cuda")
     with pytest.raises(Su2Error):
-        _operator(prob, two_pass_scratch_bytes=4096, two_pass_scratch="torch")
+        Plan(prob, family_ptrs={k: t.data_ptr() for k, t in own.family_tensors.items()}, ld_align=own.ld_align,
+             two_pass_scratch_bytes=4096, two_pass_scratch_ptr=small.data_ptr())
