@@ -29,9 +29,11 @@
  * DEVICE pointers that must stay valid and unchanged while the plan is used.  The library
  * allocates on the device only what belongs to the plan (freed by su2_plan_destroy): its task tables and tensor
  * maps, the position-folded operators of one-sided rows (sum_pos alpha_pos A_pos, formed once per plan), a padded
- * copy of Psi refreshed by every apply (the large-tile kernel loads its tiles with bulk-tensor copies, which need
- * 16-byte aligned rows) and, only for operator families whose stored layout is not 16-byte aligned, a padded copy
- * of the family (su2_plan_info_t.padded_copy_bytes; see su2_opfamily.blk_ld).
+ * copy of Psi refreshed by every apply (the large-tile kernels load their tiles with bulk-tensor copies, which need
+ * 16-byte aligned rows), only for operator families whose stored layout is not 16-byte aligned, a padded copy
+ * of the family (su2_plan_info_t.padded_copy_bytes; see su2_opfamily.blk_ld) and, for plans on the two-pass route
+ * (SU2_PLAN_TWO_PASS, the default of large-block bonds), the scratch the intermediates T_pos go through -- unless the
+ * caller hands in that buffer (su2_plan_options.two_pass_scratch_dev).
  * Errors: every entry point returns 0 on success and a negative su2_status otherwise; no
  * exceptions, no aborts, no partial state.  Results are bit-reproducible for a fixed plan.
  */
