@@ -143,10 +143,13 @@ gemm_pair_kernel(int m, int k, int n, int p, int64_t batch, double alpha, const 
 // rows of `cols` doubles (pitch cols) -> rows of pitch ld (> cols); the pad columns are never read (the tensor maps keep the
 // true extent, out-of-bounds columns are zero-filled by the copy engine)
 __global__ void __launch_bounds__(256) repitch_kernel(const double* __restrict__ src, double* __restrict__ dst, int64_t rows, int cols, int ld) {
-  const int64_t total = rows * cols;
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
-    const int64_t r = i / cols;
-    dst[r * ld + (i - r * cols)] = src[i];
+  // one warp per row (no division per element), lanes along the row
+  const int lane = threadIdx.x & 31;
+  const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarp = ((int64_t)gridDim.x * blockDim.x) >> 5;
+  for (int64_t r = warp0; r < rows; r += nwarp) {
+    const double* __restrict__ s = src + r * cols;
+    double* __restrict__ d = dst + r * ld;
+    for (int c = lane; c < cols; c += 32) d[c] = s[c];
   }
 }
 
@@ -206,12 +209,12 @@ su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double al
     const size_t b_padB = padB ? (((size_t)batch * p * ldB * 8 + 255) & ~(size_t)255) : 0;
     char* pads = nullptr;
     if (b_padA + b_padX + b_padB) {
-      cudaError_t e = cudaMallocAsync((void**)&pads, b_padA + b_padX + b_padB, stream);
-      if (e != cudaSuccess) { set_cuda_error("cudaMallocAsync(gemm_pair re-pitch)", (int)e); return SU2_ERR_CUDA; }
+      su2_status sp = gemm_scratch_alloc((void**)&pads, b_padA + b_padX + b_padB, stream_v);   // the pool of gemm_two_pass.cu
+      if (sp != SU2_OK) return sp;
     }
     const double *mA = A, *mX = X, *mB = B;
     auto repitch = [&](const double* src, char* dst, int64_t rows, int cols, int ld) {
-      repitch_kernel<<<(unsigned)std::min<int64_t>((rows * cols + 255) / 256, 148 * 32), 256, 0, stream>>>(src, (double*)dst, rows, cols, ld);
+      repitch_kernel<<<(unsigned)std::min<int64_t>((rows + 7) / 8, 148 * 32), 256, 0, stream>>>(src, (double*)dst, rows, cols, ld);
       count_launch();
       return (const double*)dst;
     };
@@ -252,7 +255,7 @@ su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double al
       char* pads = buf + b_maps + b_task + b_unit + b_work + 256;
       const double *mA = A, *mX = X, *mB = B;
       auto repitch = [&](const double* src, char* dst, int64_t rows, int cols, int ld) {
-        repitch_kernel<<<(unsigned)std::min<int64_t>((rows * cols + 255) / 256, 148 * 32), 256, 0, stream>>>(src, (double*)dst, rows, cols, ld);
+        repitch_kernel<<<(unsigned)std::min<int64_t>((rows + 7) / 8, 148 * 32), 256, 0, stream>>>(src, (double*)dst, rows, cols, ld);
         count_launch();
         return (const double*)dst;
       };

@@ -54,6 +54,16 @@ su2_status scratch_pool(cudaMemPool_t* out) {
 }
 }  // namespace
 
+// stream-ordered allocation from that pool (freed with cudaFreeAsync)
+su2_status gemm_scratch_alloc(void** out, size_t bytes, void* stream_v) {
+  cudaMemPool_t pool;
+  su2_status st = scratch_pool(&pool);
+  if (st != SU2_OK) return st;
+  cudaError_t e = cudaMallocFromPoolAsync(out, bytes, pool, (cudaStream_t)stream_v);
+  if (e != cudaSuccess) { set_cuda_error("cudaMallocFromPoolAsync(gemm_pair scratch)", (int)e); return SU2_ERR_CUDA; }
+  return SU2_OK;
+}
+
 // C_b += alpha (A_b X_b) B_b^T in two passes; operands with even leading dimensions and 16-byte aligned bases (the caller
 // re-pitches the others); T and the three small tables live in stream-ordered allocations.
 su2_status launch_gemm_two_pass(int m, int k, int n, int p, int64_t batch, double alpha, const double* A, int ldA, const double* X, int ldX,

@@ -243,6 +243,7 @@ su2_status launch_gemm_pair(int m, int k, int n, int p, int64_t batch, double al
 // gemm_pair_small.cu: returns SU2_OK after launching, 1 if the item shape does not fit the small-block kernel
 su2_status launch_gemm_two_pass(int m, int k, int n, int p, int64_t batch, double alpha, const double* A, int ldA, const double* X, int ldX,
                                 const double* B, int ldB, double* C, void* stream);   // gemm_two_pass.cu
+su2_status gemm_scratch_alloc(void** out, size_t bytes, void* stream);   // gemm_two_pass.cu: from the library's own memory pool
 su2_status launch_gemm_pair_small(int m, int k, int n, int p, int64_t batch, double alpha, const double* A, const double* X,
                                   const double* B, double* C, void* stream, int wpi_force, int nbuf_force);
 void set_cuda_error(const char* what, int code);
