@@ -167,7 +167,7 @@ enum {
 /* Tuning of SU2_PLAN_TWO_PASS (su2_plan_create_opts; 0 = default for every field). */
 typedef struct {
   int32_t two_pass_min_dim;        /* a task takes the two-pass route if its four extents all reach this (default 1: all do) */
-  int32_t two_pass_chunk_k;        /* target length of the inner (position, index) loop of one pass-2 CTA (default 8192)      */
+  int32_t two_pass_chunk_k;        /* target length of the inner (position, index) loop of one pass-2 CTA (default 4096)      */
   int64_t two_pass_scratch_bytes;  /* upper bound of the plan-owned scratch for T (default 16 GiB; never less than one
                                       position of the largest task; su2_plan_info_t.two_pass_scratch_bytes = what was taken) */
   int32_t two_pass_ipc_k;          /* pass 1: a CTA works through consecutive (position, tile) items until their inner

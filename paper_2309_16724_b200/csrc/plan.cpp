@@ -215,7 +215,7 @@ extern "C" su2_status su2_plan_create_opts(su2_plan** out, const su2_problem* p,
   if (opt.two_pass_scratch_dev && (opt.two_pass_scratch_bytes <= 0 || ((uintptr_t)opt.two_pass_scratch_dev & 255))) return SU2_ERR_WORKSPACE;
   if (opt.two_pass_min_dim == 0) opt.two_pass_min_dim = 1;
   if (opt.two_pass_scratch_bytes == 0) opt.two_pass_scratch_bytes = (int64_t)16 << 30;
-  if (opt.two_pass_chunk_k == 0) opt.two_pass_chunk_k = 8192;
+  if (opt.two_pass_chunk_k == 0) opt.two_pass_chunk_k = 4096;
   if (opt.two_pass_ipc_k < 0) return SU2_ERR_INVALID_ARGUMENT;
   if (opt.two_pass_ipc_k == 0) opt.two_pass_ipc_k = 2048;
   const auto t_start = std::chrono::steady_clock::now();
