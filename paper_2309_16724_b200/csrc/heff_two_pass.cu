@@ -93,21 +93,33 @@ __device__ __forceinline__ void tp_consume(const TpItem& it, const double* __res
 #pragma unroll
     for (int j = 0; j < NJ; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
   if (it.acc_init) {   // dst += ...: start from the old values (fetched while the pipeline fills) instead of adding them at the end
-    const int cb = it.col0 + wc * 8 * NJ + 2 * t;
+    const int cb = it.col0 + wc * 8 * NJ + 2 * t, rb = it.row0 + wr * 8 * NI + g;
+    if (!(it.ldd & 1) && !((uintptr_t)it.dst & 15) && rb + 8 * (NI - 1) < it.M && cb + 8 * (NJ - 1) + 1 < it.N) {
+      const double* __restrict__ o = it.dst + (int64_t)rb * it.ldd + cb;   // the whole share inside the output: plain 16-byte loads
+      const int64_t rstep = (int64_t)8 * it.ldd;
 #pragma unroll
-    for (int i = 0; i < NI; ++i) {
-      const int r = it.row0 + wr * 8 * NI + i * 8 + g;
-      if (r >= it.M) continue;
+      for (int i = 0; i < NI; ++i, o += rstep)
 #pragma unroll
-      for (int j = 0; j < NJ; ++j) {
-        const int c = cb + j * 8;
-        const double* o = it.dst + (int64_t)r * it.ldd + c;
-        if (!(it.ldd & 1) && !((uintptr_t)it.dst & 15) && c + 1 < it.N) {
-          const double2 v = *(const double2*)o;
+        for (int j = 0; j < NJ; ++j) {
+          const double2 v = *(const double2*)(o + 8 * j);
           acc[i][j][0] = v.x; acc[i][j][1] = v.y;
-        } else {
-          if (c < it.N) acc[i][j][0] = o[0];
-          if (c + 1 < it.N) acc[i][j][1] = o[1];
+        }
+    } else {
+#pragma unroll
+      for (int i = 0; i < NI; ++i) {
+        const int r = rb + i * 8;
+        if (r >= it.M) continue;
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) {
+          const int c = cb + j * 8;
+          const double* o = it.dst + (int64_t)r * it.ldd + c;
+          if (!(it.ldd & 1) && !((uintptr_t)it.dst & 15) && c + 1 < it.N) {
+            const double2 v = *(const double2*)o;
+            acc[i][j][0] = v.x; acc[i][j][1] = v.y;
+          } else {
+            if (c < it.N) acc[i][j][0] = o[0];
+            if (c + 1 < it.N) acc[i][j][1] = o[1];
+          }
         }
       }
     }
@@ -162,12 +174,23 @@ __device__ __forceinline__ void tp_consume(const TpItem& it, const double* __res
       __syncwarp();
       if (lane == 0) tp_mbar_arrive(&empty[b]);
     }
-  // epilogue: dst = scale * acc (accumulator layout: row g, columns 2t, 2t + 1 of every m8n8 tile), guarded
+  // epilogue: dst = scale * acc (accumulator layout: row g, columns 2t, 2t + 1 of every m8n8 tile)
   const bool vec = !(it.ldd & 1) && !((uintptr_t)it.dst & 15);
   const int cbase = it.col0 + wc * 8 * NJ + 2 * t;
+  const int rbase = it.row0 + wr * 8 * NI + g;
+  if (vec && rbase + 8 * (NI - 1) < it.M && cbase + 8 * (NJ - 1) + 1 < it.N) {
+    // this thread's whole share lies inside the output (every tile but the ragged last ones): plain 16-byte stores
+    double* __restrict__ o = it.dst + (int64_t)rbase * it.ldd + cbase;
+    const int64_t rstep = (int64_t)8 * it.ldd;
+#pragma unroll
+    for (int i = 0; i < NI; ++i, o += rstep)
+#pragma unroll
+      for (int j = 0; j < NJ; ++j) *(double2*)(o + 8 * j) = make_double2(it.scale * acc[i][j][0], it.scale * acc[i][j][1]);
+    return;
+  }
 #pragma unroll
   for (int i = 0; i < NI; ++i) {
-    const int r = it.row0 + wr * 8 * NI + i * 8 + g;
+    const int r = rbase + i * 8;
     if (r >= it.M) continue;
 #pragma unroll
     for (int j = 0; j < NJ; ++j) {
