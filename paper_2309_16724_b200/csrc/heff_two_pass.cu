@@ -1,8 +1,8 @@
-// Two-pass route of H_eff * Psi (row a4 of SURVEY.md section 8; plan flag SU2_PLAN_TWO_PASS): the task
+// Two-pass route of H_eff * Psi (row a4 of SURVEY.md section 8; plan flag SU2_PLAN_TWO_PASS, the default of large-block bonds): the task
 //     F_s (m x p) += coef sum_pos alpha_pos Aop_pos (m x k) E_s' (k x n) Dop_pos^T (n x p)          (Eq. (3))
 // executed the way the paper does it (a strided-batched GEMM per product, the sum over positions as the
 // inner dimension of the second one -- the "stripe" trick), but with both products on this library's own
-// TMA-fed DMMA.8x8x4 GEMM and the intermediate T in a plan-owned scratch:
+// TMA-fed DMMA.8x8x4 GEMM and the intermediate T in a scratch that belongs to the plan (allocated by it or handed in by the caller):
 //   pass 1:  T_pos = coef alpha_pos Aop_pos E           for every position of a slice        (order 1: T_pos = coef alpha_pos E Dop_pos^T)
 //   pass 2:  partial[chunk] = sum_{pos in chunk} T_pos Dop_pos^T   (K loop over (pos, n))     (order 1: sum_pos Aop_pos T_pos)
 //   reduce:  F_s += partial slabs in index order (deterministic, no atomics; row a5)
@@ -14,7 +14,9 @@
 // One kernel serves both passes (tp_gemm_kernel): D (M x N) = scale * sum_pos L_pos (M x K) R_pos (K x N), CTA tile 64 x 128,
 // k stages of 20 staged by one elected thread with bulk-tensor copies (true extents in the tensor maps: ragged edges and the
 // k tail arrive as zeros), 4 consumer warps (2 x 2).  Ragged last row / column tiles run a narrower instantiation
-// (warp tile 8 NI x 8 NJ) instead of multiplying zeros.
+// (warp tile 8 NI x 8 NJ) instead of multiplying zeros.  A CTA works through several consecutive items with its pipeline kept
+// full; only the producer thread reads the tables and hands the item descriptors to the consumers through shared memory.
+// su2_gemm_pair_batched (gemm_two_pass.cu) runs on the same kernel with the batch items in the place of the positions.
 #include <cuda.h>
 #include <cuda_runtime.h>
 
